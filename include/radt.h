@@ -1,0 +1,187 @@
+/*
+ * radt.h -- C ABI of the B200-native differentiable line radiative transfer render.
+ *
+ * The library renders velocity cubes of one molecular line in LTE by backward ray tracing through
+ * gridded density / temperature / velocity fields, and returns the gradient of a scalar loss with
+ * respect to the stored grid values.  It implements the render of
+ *   "Revealing Fine Structure in Protoplanetary Disks with Physics Constrained Neural Fields"
+ *   (RadJAX), section "Line Radiative Transfer with RadJAX", Eq. 11-17,
+ * discretised as stated in DESIGN.md (algorithm O1-O11).
+ *
+ * Conventions
+ *   - plain C, no torch / C++ types; every pointer is documented as HOST or DEVICE memory;
+ *   - the library never allocates device memory and never synchronises in the *_device* entry
+ *     points: the caller passes a workspace (size from radt_workspace_bytes) and a CUDA stream;
+ *     all work is enqueued on that stream (stream-ordered, CUDA-graph capturable);
+ *   - the *_host entry points take HOST buffers, allocate stream-ordered device memory internally,
+ *     copy in, run the same kernels, copy out and synchronise the stream before returning;
+ *   - units: lengths au, velocities cm/s, number densities cm^-3, temperatures K, angles rad,
+ *     frequencies Hz, masses g;
+ *   - arrays are C-contiguous, last index fastest: axisymmetric grids [b][ir][izeta], 3-D grids
+ *     [b][ix][iy][iz], cubes [b][iy][ix][channel];
+ *   - return value 0 on success, a negative RADT_E_* code otherwise; radt_last_error() returns a
+ *     thread-local message.  Numerical conditions are not errors: T is clamped to >= 1 K (zero
+ *     gradient through the clamp), NaN inputs propagate.
+ *   - there is no CPU fallback and no other back-end: without a CUDA device every compute entry
+ *     point fails with RADT_E_CUDA.
+ */
+#ifndef RADT_H
+#define RADT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RADT_VERSION 100          /* 0.1.0 */
+#define RADT_MAX_LEVELS 64        /* partition-function table length limit */
+#define RADT_MAX_CHANNELS 256     /* channels per render call */
+
+enum {
+    RADT_OK = 0,
+    RADT_E_INVALID = -1,          /* null pointer, non-positive size, bad struct_size, limits exceeded */
+    RADT_E_UNSUPPORTED = -2,      /* grid kind / flag combination not implemented */
+    RADT_E_WORKSPACE = -3,        /* workspace too small */
+    RADT_E_CUDA = -4              /* CUDA runtime error (message in radt_last_error) */
+};
+
+enum { RADT_GRID_AXISYM = 0, RADT_GRID_CART3D = 1 };
+enum { RADT_DENS_LINEAR = 0, RADT_DENS_LN = 1 };
+enum { RADT_VEL_VPHI = 0, RADT_VEL_KEPLER_FRAC = 1 };
+enum { RADT_UNIT_S0 = 0, RADT_UNIT_CGS = 1, RADT_UNIT_JY_PIXEL = 2 };
+enum { RADT_PASS_FWD = 0, RADT_PASS_BWD = 1 };
+
+/* Image plane and viewing geometry of ONE batch item (Table 2 "Ray-tracing
+ * Geometry": inclination, position angle, azimuth, distance, v_LSR).  Rays are orthographic, one per
+ * pixel centre, X_ix = x0 + (ix + 1/2 - nx/2) fov_x / nx (O1-O3).  All batch items of a
+ * call must share nx, ny and nstep. */
+typedef struct radt_geom {
+    uint32_t struct_size;         /* = sizeof(radt_geom) */
+    int32_t nx, ny;               /* image size in pixels */
+    int32_t nstep;                /* steps per ray (midpoint rule over the clipped interval) */
+    double fov_x, fov_y;          /* au, full extent of the image */
+    double x0, y0;                /* au, sky offset of the image centre from the star */
+    double incl, pa, az;          /* rad */
+    double dist_pc;               /* pc; only used by RADT_UNIT_JY_PIXEL */
+    double vsys;                  /* cm/s, systemic velocity (v_LSR) */
+    double gm_star;               /* cm^3 s^-2, G M_star; only used by RADT_VEL_KEPLER_FRAC */
+} radt_geom;
+
+/* One line in LTE and the channel grid (Eq. 13-17).  Level tables are HOST
+ * pointers; the library copies them into kernel arguments at call time. */
+typedef struct radt_line {
+    uint32_t struct_size;         /* = sizeof(radt_line) */
+    int32_t nlev;                 /* 1 .. RADT_MAX_LEVELS */
+    int32_t nchan;                /* 1 .. RADT_MAX_CHANNELS */
+    int32_t unit;                 /* RADT_UNIT_* of the output cube */
+    double nu0;                   /* Hz, rest frequency */
+    double a_ul;                  /* s^-1, Einstein A */
+    double g_u;                   /* degeneracy of the upper level */
+    double e_u_K;                 /* E_u / k [K] */
+    const double *e_lev_K;        /* HOST [nlev], level energies / k for Q(T) */
+    const double *g_lev;          /* HOST [nlev], level degeneracies */
+    double m_line;                /* g, mass of the emitting molecule (m_CO in Eq. 16) */
+    double m_gas;                 /* g, mean molecular mass (m_mol in Eq. 17) */
+    double vturb_abs;             /* cm/s, absolute micro-turbulence added in quadrature */
+    double vturb_mach;            /* dimensionless turbulent velocity of Eq. 16 */
+    const double *vchan;          /* HOST [nchan], channel-centre velocities, cm/s, radio convention */
+} radt_line;
+
+/* Field grids of the whole batch (regular or log-spaced grids).
+ *   AXISYM : n = {nr, nzeta, 1}; nodes r_i = lo[0] (hi[0]/lo[0])^(i/(nr-1)), zeta_j = lo[1] +
+ *            (hi[1]-lo[1]) j/(nzeta-1), zeta = |z|/r if mirror_z else z/r (mirror_z needs lo[1] >= 0);
+ *   CART3D : n = {nx, ny, nz}; nodes lo[a] + (hi[a]-lo[a]) i/(n[a]-1) in the disk frame.
+ * Interpolation is bi/tri-linear in index space; outside the node range is vacuum.
+ * dens/temp/vel are DEVICE pointers to float32 arrays [batch][cells]; item b starts at
+ * ptr + b * batch_stride (elements).  Caller owns all memory. */
+typedef struct radt_grid {
+    uint32_t struct_size;         /* = sizeof(radt_grid) */
+    int32_t kind;                 /* RADT_GRID_* */
+    int32_t n[3];
+    int32_t mirror_z;             /* AXISYM only */
+    int32_t dens_mode;            /* RADT_DENS_LINEAR: n [cm^-3]; RADT_DENS_LN: ln n */
+    int32_t vel_mode;             /* RADT_VEL_VPHI: v_phi [cm/s]; RADT_VEL_KEPLER_FRAC: delta, v_phi = v_K (1 + delta) */
+    double lo[3], hi[3];
+    int64_t batch_stride;         /* elements between batch items (>= cells), ignored for batch 1 */
+    const float *dens;            /* DEVICE (HOST for the *_host entry points) */
+    const float *temp;
+    const float *vel;
+} radt_grid;
+
+int radt_version(void);
+const char *radt_last_error(void);
+
+/* Run-time options (process-wide; for measurements).  Keys: */
+enum {
+    RADT_OPT_WINDOW = 1,          /* 1 (default): skip channel groups outside the +-6.4 alpha line window; 0: dense */
+    RADT_OPT_SKIP_EMPTY = 2       /* 1 (default): skip steps with zero opacity in the forward march; 0: dense */
+};
+int radt_set_option(int key, int value);
+int radt_get_option(int key);
+
+/* Bytes of DEVICE workspace needed by radt_render (pass = RADT_PASS_FWD) or radt_render_bwd
+ * (RADT_PASS_BWD) for `batch` items.  HOST pointers in, size out. */
+int radt_workspace_bytes(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                         int32_t pass, size_t *bytes_out);
+
+/* K1: ray geometry (O1-O3).  Writes for every ray of every batch item
+ * rays_out[(b*ny + iy)*nx + ix] = {s0, ds} (two doubles, au; ds = 0 marks a ray that misses the
+ * volume).  geom: HOST [batch]; rays_out: DEVICE [batch*ny*nx*2] doubles. */
+int radt_ray_geometry(const radt_geom *geom, const radt_grid *grid, int32_t batch, double *rays_out,
+                      void *cuda_stream);
+
+/* Forward render (O1-O10; Eq. 11-17).  Overwrites
+ * cube [batch][ny][nx][nchan] (DEVICE float32, rays that miss write zeros).  geom: HOST [batch];
+ * line, grid: HOST structs; ws: DEVICE workspace of ws_bytes.  Asynchronous on cuda_stream. */
+int radt_render(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                float *cube, void *ws, size_t ws_bytes, void *cuda_stream);
+
+/* Adjoint (O11; Fig. 2 E).  Given the forward output `cube` and
+ * dl_dcube = dLoss/dcube (both DEVICE float32 [batch][ny][nx][nchan]) OVERWRITES g_dens, g_temp,
+ * g_vel (DEVICE float32, grid-shaped incl. batch with the grid's batch_stride; any may be NULL) with
+ * dLoss/d(stored grid value): d/d(ln n) for RADT_DENS_LN, d/d(delta) for RADT_VEL_KEPLER_FRAC.
+ * Memory-free: no per-step activations are stored; the rays are re-marched.  Float atomics make
+ * the last bits order-dependent. */
+int radt_render_bwd(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                    const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel,
+                    void *ws, size_t ws_bytes, void *cuda_stream);
+
+/* L2 data term used by the configs (chi^2 of PAPER.md:79, 252):
+ * L = 1/(2 n) sum ((cube - target)/sigma)^2, dl_dcube = (cube - target)/(sigma^2 n).
+ * cube, target, dl_dcube: DEVICE float32 [n]; loss_out: DEVICE double[1] (overwritten). */
+int radt_l2_loss_grad(const float *cube, const float *target, double sigma, int64_t n, float *dl_dcube,
+                      double *loss_out, void *cuda_stream);
+
+/* Same operations with HOST buffers (grid->dens/temp/vel, cube, dl_dcube, g_* are HOST pointers).
+ * Device memory is allocated stream-ordered on stream 0 of the current device; the call returns
+ * after the results are in host memory. */
+int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                     float *cube);
+/* Forward + L2 loss against `target` (HOST) + adjoint in one call; cube may be NULL. */
+int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                       const float *target, double sigma, float *cube, double *loss_out,
+                       float *g_dens, float *g_temp, float *g_vel);
+int radt_render_bwd_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                         const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel);
+
+/* M1 micro-benchmarks of the issue peaks the roofline is quoted against.
+ * Runs a full-occupancy dependent-chain loop of `kind` on the current device and returns the
+ * achieved rate in lane-operations per second (HOST double).  kind: 0 MUFU.EX2, 1 FFMA, 2 DFMA,
+ * 3 FFMA2 (packed f32x2, counted as 2 lane-ops). */
+int radt_pipe_peak(int32_t kind, double *ops_per_s_out, double *sm_clock_mhz_out);
+
+/* Work counters of the last render / adjoint that used workspace `ws` (DEVICE): copies 4 uint64 to
+ * out4 (HOST): {forward active ray-steps, forward executed 32-channel groups, adjoint active ray-steps,
+ * adjoint executed groups}.  Synchronises cuda_stream. */
+int radt_read_counters(const void *ws, uint64_t *out4, void *cuda_stream);
+
+/* Counters of the last radt_render / radt_render_bwd call on this thread (HOST): number of kernel
+ * launches enqueued. */
+int radt_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RADT_H */

@@ -1,0 +1,232 @@
+"""Thin ctypes binding of libradt.so (include/radt.h): argument marshalling only.
+
+Every step of the render runs in the CUDA kernels of csrc/; this module converts `synth.Scene`
+containers and torch tensors (device memory + streams) into the C structs and pointers of the ABI.
+There is no CPU path: if the shared library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libradt.so")
+
+PASS_FWD, PASS_BWD = 0, 1
+OPT_WINDOW, OPT_SKIP_EMPTY = 1, 2
+
+EXPORTS = ["radt_version", "radt_last_error", "radt_set_option", "radt_get_option", "radt_workspace_bytes",
+           "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_l2_loss_grad", "radt_render_host",
+           "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
+           "radt_last_launch_count"]
+
+
+class RadtError(RuntimeError):
+    pass
+
+
+class radt_geom(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("nx", C.c_int32), ("ny", C.c_int32), ("nstep", C.c_int32),
+                ("fov_x", C.c_double), ("fov_y", C.c_double), ("x0", C.c_double), ("y0", C.c_double),
+                ("incl", C.c_double), ("pa", C.c_double), ("az", C.c_double), ("dist_pc", C.c_double),
+                ("vsys", C.c_double), ("gm_star", C.c_double)]
+
+
+class radt_line(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("nlev", C.c_int32), ("nchan", C.c_int32), ("unit", C.c_int32),
+                ("nu0", C.c_double), ("a_ul", C.c_double), ("g_u", C.c_double), ("e_u_K", C.c_double),
+                ("e_lev_K", C.POINTER(C.c_double)), ("g_lev", C.POINTER(C.c_double)),
+                ("m_line", C.c_double), ("m_gas", C.c_double), ("vturb_abs", C.c_double), ("vturb_mach", C.c_double),
+                ("vchan", C.POINTER(C.c_double))]
+
+
+class radt_grid(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("kind", C.c_int32), ("n", C.c_int32 * 3), ("mirror_z", C.c_int32),
+                ("dens_mode", C.c_int32), ("vel_mode", C.c_int32), ("lo", C.c_double * 3), ("hi", C.c_double * 3),
+                ("batch_stride", C.c_int64), ("dens", C.c_void_p), ("temp", C.c_void_p), ("vel", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libradt.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RadtError(f"{LIB_PATH} not found: build it with `python -m paper_2509_03623_b200.build` "
+                            "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        gp, lp, rp = C.POINTER(radt_geom), C.POINTER(radt_line), C.POINTER(radt_grid)
+        L.radt_version.restype = C.c_int
+        L.radt_last_error.restype = C.c_char_p
+        L.radt_set_option.argtypes = [C.c_int, C.c_int]
+        L.radt_get_option.argtypes = [C.c_int]
+        L.radt_workspace_bytes.argtypes = [gp, lp, rp, i32, i32, C.POINTER(C.c_size_t)]
+        L.radt_ray_geometry.argtypes = [gp, rp, i32, vp, vp]
+        L.radt_render.argtypes = [gp, lp, rp, i32, vp, vp, C.c_size_t, vp]
+        L.radt_render_bwd.argtypes = [gp, lp, rp, i32, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        L.radt_l2_loss_grad.argtypes = [vp, vp, dbl, i64, vp, vp, vp]
+        L.radt_render_host.argtypes = [gp, lp, rp, i32, vp]
+        L.radt_fit_step_host.argtypes = [gp, lp, rp, i32, vp, dbl, vp, C.POINTER(dbl), vp, vp, vp]
+        L.radt_render_bwd_host.argtypes = [gp, lp, rp, i32, vp, vp, vp, vp, vp]
+        L.radt_pipe_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
+        L.radt_read_counters.argtypes = [vp, C.POINTER(C.c_uint64), vp]
+        L.radt_last_launch_count.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise RadtError(f"radt error {rc}: {lib().radt_last_error().decode()}")
+
+
+def _as_list(scenes):
+    return list(scenes) if isinstance(scenes, (list, tuple)) else [scenes]
+
+
+class Descriptors:
+    """C descriptors of a batch of scenes that share line, grid geometry and image size."""
+
+    def __init__(self, scenes):
+        scenes = _as_list(scenes)
+        s0 = scenes[0]
+        self.batch = len(scenes)
+        self.geom = (radt_geom * self.batch)()
+        for b, sc in enumerate(scenes):
+            g = sc.geom
+            self.geom[b] = radt_geom(C.sizeof(radt_geom), g.nx, g.ny, g.nstep, g.fov_x, g.fov_y, g.x0, g.y0, g.incl,
+                                     g.pa, g.az, g.dist_pc, g.vsys, g.gm_star)
+        ln = s0.line
+        self._e = np.ascontiguousarray(ln.e_lev_K, np.float64)
+        self._g = np.ascontiguousarray(ln.g_lev, np.float64)
+        self._v = np.ascontiguousarray(ln.vchan, np.float64)
+        dp = C.POINTER(C.c_double)
+        self.line = radt_line(C.sizeof(radt_line), len(self._e), len(self._v), ln.unit, ln.nu0, ln.a_ul, ln.g_u,
+                              ln.e_u_K, self._e.ctypes.data_as(dp), self._g.ctypes.data_as(dp), ln.m_line, ln.m_gas,
+                              ln.vturb_abs, ln.vturb_mach, self._v.ctypes.data_as(dp))
+        gr = s0.grid
+        n3 = tuple(gr.n) + (1,) * (3 - len(gr.n))
+        lo3 = tuple(gr.lo) + (0.0,) * (3 - len(gr.lo))
+        hi3 = tuple(gr.hi) + (0.0,) * (3 - len(gr.hi))
+        self.cells = int(np.prod(gr.n))
+        self.grid_shape = tuple(gr.n)
+        self.grid = radt_grid(C.sizeof(radt_grid), gr.kind, (C.c_int32 * 3)(*n3), int(gr.mirror_z), gr.dens_mode,
+                              gr.vel_mode, (C.c_double * 3)(*lo3), (C.c_double * 3)(*hi3), self.cells, None, None, None)
+        self.nx, self.ny, self.nchan, self.nstep = s0.geom.nx, s0.geom.ny, len(self._v), s0.geom.nstep
+        self.cube_shape = (self.batch, self.ny, self.nx, self.nchan)
+
+    def with_fields(self, dens_ptr, temp_ptr, vel_ptr):
+        self.grid.dens, self.grid.temp, self.grid.vel = dens_ptr, temp_ptr, vel_ptr
+        return self
+
+
+def stack_fields(scenes):
+    """Host float32 arrays [batch, *grid] of the three fields."""
+    scenes = _as_list(scenes)
+    return tuple(np.ascontiguousarray(np.stack([np.asarray(getattr(sc.grid, f), np.float32) for sc in scenes]))
+                 for f in ("dens", "temp", "vel"))
+
+
+def _stream_ptr(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+# ------------------------------------------------------------------------------------------------
+# same names as the C ABI
+# ------------------------------------------------------------------------------------------------
+def radt_version() -> int:
+    return lib().radt_version()
+
+
+def radt_set_option(key: int, value: int):
+    _check(lib().radt_set_option(key, value))
+
+
+def radt_get_option(key: int) -> int:
+    return lib().radt_get_option(key)
+
+
+def radt_workspace_bytes(desc: Descriptors, pass_: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().radt_workspace_bytes(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, pass_, C.byref(out)))
+    return out.value
+
+
+def radt_ray_geometry(desc: Descriptors, rays_out, stream=None):
+    """rays_out: CUDA float64 tensor [batch, ny, nx, 2]."""
+    _check(lib().radt_ray_geometry(desc.geom, C.byref(desc.grid), desc.batch, C.c_void_p(rays_out.data_ptr()),
+                                   _stream_ptr(stream)))
+
+
+def radt_render(desc: Descriptors, dens, temp, vel, cube, ws, stream=None):
+    """dens/temp/vel: CUDA float32 tensors [batch, *grid]; cube: CUDA float32 [batch, ny, nx, nchan]; ws: CUDA uint8."""
+    desc.with_fields(dens.data_ptr(), temp.data_ptr(), vel.data_ptr())
+    _check(lib().radt_render(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, C.c_void_p(cube.data_ptr()),
+                             C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(stream)))
+
+
+def radt_render_bwd(desc: Descriptors, dens, temp, vel, cube, dl_dcube, g_dens, g_temp, g_vel, ws, stream=None):
+    desc.with_fields(dens.data_ptr(), temp.data_ptr(), vel.data_ptr())
+
+    def p(t):
+        return C.c_void_p(t.data_ptr()) if t is not None else None
+    _check(lib().radt_render_bwd(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, p(cube), p(dl_dcube),
+                                 p(g_dens), p(g_temp), p(g_vel), C.c_void_p(ws.data_ptr()), ws.numel(),
+                                 _stream_ptr(stream)))
+
+
+def radt_l2_loss_grad(cube, target, sigma: float, dl_dcube, loss_out, stream=None):
+    """loss_out: CUDA float64 tensor [1]."""
+    _check(lib().radt_l2_loss_grad(C.c_void_p(cube.data_ptr()), C.c_void_p(target.data_ptr()), float(sigma),
+                                   cube.numel(), C.c_void_p(dl_dcube.data_ptr()), C.c_void_p(loss_out.data_ptr()),
+                                   _stream_ptr(stream)))
+
+
+def radt_read_counters(ws, stream=None):
+    out = (C.c_uint64 * 4)()
+    _check(lib().radt_read_counters(C.c_void_p(ws.data_ptr()), out, _stream_ptr(stream)))
+    return [int(x) for x in out]
+
+
+def radt_last_launch_count() -> int:
+    return lib().radt_last_launch_count()
+
+
+def _hptr(a):
+    return C.c_void_p(a.ctypes.data) if a is not None else None
+
+
+def radt_render_host(desc: Descriptors, dens, temp, vel, cube):
+    """HOST numpy float32 arrays in, HOST cube out (copies inside the call)."""
+    desc.with_fields(dens.ctypes.data, temp.ctypes.data, vel.ctypes.data)
+    _check(lib().radt_render_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _hptr(cube)))
+
+
+def radt_fit_step_host(desc: Descriptors, dens, temp, vel, target, sigma, cube, g_dens, g_temp, g_vel) -> float:
+    desc.with_fields(dens.ctypes.data, temp.ctypes.data, vel.ctypes.data)
+    loss = C.c_double(0.0)
+    _check(lib().radt_fit_step_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _hptr(target),
+                                    float(sigma), _hptr(cube), C.byref(loss), _hptr(g_dens), _hptr(g_temp), _hptr(g_vel)))
+    return loss.value
+
+
+def radt_render_bwd_host(desc: Descriptors, dens, temp, vel, cube, dl_dcube, g_dens, g_temp, g_vel):
+    desc.with_fields(dens.ctypes.data, temp.ctypes.data, vel.ctypes.data)
+    _check(lib().radt_render_bwd_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _hptr(cube),
+                                      _hptr(dl_dcube), _hptr(g_dens), _hptr(g_temp), _hptr(g_vel)))
+
+
+def radt_pipe_peak(kind: int):
+    """Returns (lane-ops per second, SM clock in MHz) of pipe `kind` (0 MUFU.EX2, 1 FFMA, 2 DFMA, 3 FFMA2)."""
+    ops, clk = C.c_double(0.0), C.c_double(0.0)
+    _check(lib().radt_pipe_peak(kind, C.byref(ops), C.byref(clk)))
+    return ops.value, clk.value

@@ -1,0 +1,474 @@
+// radt_api.cu -- the C ABI of include/radt.h: validation, host-side constants, workspace layout, launches.
+// No CPU fallback: every compute entry point enqueues CUDA kernels or fails with RADT_E_CUDA.
+#include "../../include/radt.h"
+#include "radt_dev.cuh"
+#include "radt_kernels.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+namespace {
+
+thread_local char g_err[512] = "";
+thread_local int g_launches = 0;
+int g_opt_window = 1;
+int g_opt_skip_empty = 1;
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                     \
+    do {                                                                                   \
+        cudaError_t e_ = (expr);                                                           \
+        if (e_ != cudaSuccess) return fail(RADT_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+    } while (0)
+
+// CODATA 2018, CGS
+const double kH = 6.62607015e-27, kK = 1.380649e-16, kC = 2.99792458e10;
+const double kAU = 1.495978707e13, kPC = 3.0856775814913673e18, kPI = 3.14159265358979323846;
+const double kLOG2E = 1.4426950408889634;
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int validate(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int batch)
+{
+    if (!geom || !grid) return fail(RADT_E_INVALID, "null descriptor");
+    if (batch < 1) return fail(RADT_E_INVALID, "batch must be >= 1");
+    if (grid->struct_size != sizeof(radt_grid)) return fail(RADT_E_INVALID, "radt_grid.struct_size mismatch");
+    for (int b = 0; b < batch; ++b) {
+        const radt_geom &g = geom[b];
+        if (g.struct_size != sizeof(radt_geom)) return fail(RADT_E_INVALID, "radt_geom.struct_size mismatch");
+        if (g.nx < 1 || g.ny < 1 || g.nstep < 1) return fail(RADT_E_INVALID, "nx, ny, nstep must be positive");
+        if (!(g.fov_x > 0) || !(g.fov_y > 0)) return fail(RADT_E_INVALID, "fov must be positive");
+        if (g.nx != geom[0].nx || g.ny != geom[0].ny || g.nstep != geom[0].nstep)
+            return fail(RADT_E_INVALID, "all batch items must share nx, ny, nstep");
+        if ((long long)g.nx * g.ny * (long long)batch > (1ll << 40)) return fail(RADT_E_INVALID, "too many rays");
+    }
+    if (line) {
+        if (line->struct_size != sizeof(radt_line)) return fail(RADT_E_INVALID, "radt_line.struct_size mismatch");
+        if (line->nlev < 1 || line->nlev > RADT_MAX_LEVELS) return fail(RADT_E_INVALID, "nlev out of range");
+        if (line->nchan < 1 || line->nchan > RADT_MAX_CHANNELS) return fail(RADT_E_INVALID, "nchan out of range (max %d)", RADT_MAX_CHANNELS);
+        if (!line->e_lev_K || !line->g_lev || !line->vchan) return fail(RADT_E_INVALID, "null line table");
+        if (!(line->nu0 > 0) || !(line->a_ul > 0) || !(line->m_line > 0) || !(line->m_gas > 0))
+            return fail(RADT_E_INVALID, "line constants must be positive");
+        if (line->unit < 0 || line->unit > 2) return fail(RADT_E_INVALID, "unknown intensity unit");
+    }
+    if (grid->kind == RADT_GRID_AXISYM) {
+        if (grid->n[0] < 2 || grid->n[1] < 2) return fail(RADT_E_INVALID, "axisymmetric grid needs >= 2 nodes per axis");
+        if (!(grid->lo[0] > 0) || !(grid->hi[0] > grid->lo[0])) return fail(RADT_E_INVALID, "need 0 < r_min < r_max");
+        if (!(grid->hi[1] > grid->lo[1])) return fail(RADT_E_INVALID, "need zeta_lo < zeta_hi");
+        if (grid->mirror_z && grid->lo[1] < 0) return fail(RADT_E_INVALID, "mirror_z needs zeta_lo >= 0");
+    } else if (grid->kind == RADT_GRID_CART3D) {
+        for (int a = 0; a < 3; ++a) {
+            if (grid->n[a] < 2) return fail(RADT_E_INVALID, "3-D grid needs >= 2 nodes per axis");
+            if (!(grid->hi[a] > grid->lo[a])) return fail(RADT_E_INVALID, "need lo < hi");
+        }
+        if (grid->mirror_z) return fail(RADT_E_UNSUPPORTED, "mirror_z applies to axisymmetric grids only");
+    } else {
+        return fail(RADT_E_UNSUPPORTED, "unknown grid kind %d", grid->kind);
+    }
+    if (grid->dens_mode < 0 || grid->dens_mode > 1 || grid->vel_mode < 0 || grid->vel_mode > 1)
+        return fail(RADT_E_UNSUPPORTED, "unknown dens_mode / vel_mode");
+    return RADT_OK;
+}
+
+long long grid_cells(const radt_grid *grid)
+{
+    return grid->kind == RADT_GRID_AXISYM ? (long long)grid->n[0] * grid->n[1]
+                                          : (long long)grid->n[0] * grid->n[1] * grid->n[2];
+}
+
+void make_dev_grid(const radt_grid *grid, DevGrid &d)
+{
+    memset(&d, 0, sizeof(d));
+    d.kind = grid->kind; d.mirror = grid->mirror_z; d.dens_mode = grid->dens_mode; d.vel_mode = grid->vel_mode;
+    d.n0 = grid->n[0]; d.n1 = grid->n[1]; d.n2 = grid->kind == RADT_GRID_AXISYM ? 1 : grid->n[2];
+    d.cells = grid_cells(grid);
+    if (grid->kind == RADT_GRID_AXISYM) {
+        double rmin = grid->lo[0], rmax = grid->hi[0];
+        d.rmin2 = rmin * rmin; d.rmax2 = rmax * rmax; d.inv_rmin = 1.0 / rmin;
+        d.zlo = grid->lo[1]; d.zhi = grid->hi[1];
+        d.lg2_ratio = std::log2(rmax / rmin);
+        d.uscale = (float)((double)(grid->n[0] - 1) / d.lg2_ratio);
+        d.wscale_d = (double)(grid->n[1] - 1) / (grid->hi[1] - grid->lo[1]);
+        double cell_lg2 = d.lg2_ratio / (double)(grid->n[0] - 1);
+        d.inv_cell_lg2 = (float)(1.0 / cell_lg2);
+        d.inv_cell_ln = (float)(1.0 / (cell_lg2 * std::log(2.0)));
+        d.fine_r = (std::exp2(cell_lg2) - 1.0) < 0.15;
+        double zm = std::fmax(std::fabs(grid->lo[1]), std::fabs(grid->hi[1]));
+        d.rb2 = rmax * rmax * (1.0 + zm * zm);
+    } else {
+        for (int a = 0; a < 3; ++a) {
+            d.lo[a] = grid->lo[a]; d.hi[a] = grid->hi[a];
+            d.inv_d[a] = (double)(grid->n[a] - 1) / (grid->hi[a] - grid->lo[a]);
+        }
+    }
+}
+
+double source_unit(const radt_geom &g, const radt_line *line)
+{
+    double S0 = 2.0 * kH * line->nu0 * line->nu0 * line->nu0 / (kC * kC);
+    if (line->unit == RADT_UNIT_CGS) return S0;
+    if (line->unit == RADT_UNIT_JY_PIXEL) {
+        double d_au = g.dist_pc * kPC / kAU;
+        return S0 * (g.fov_x / g.nx) * (g.fov_y / g.ny) / (d_au * d_au) * 1.0e23;
+    }
+    return 1.0;
+}
+
+void make_dev_geom(const radt_geom &g, const radt_line *line, DevGeom &d)
+{
+    double th = g.pa + 0.5 * kPI;
+    d.cth = std::cos(th); d.sth = std::sin(th);
+    d.ci = std::cos(g.incl); d.si = std::sin(g.incl);
+    d.ca = std::cos(g.az); d.sa = std::sin(g.az);
+    d.wx = d.si * d.sa; d.wy = d.si * d.ca; d.wz = -d.ci;
+    d.x0 = g.x0; d.y0 = g.y0; d.pix_x = g.fov_x / g.nx; d.pix_y = g.fov_y / g.ny;
+    d.gm_au_d = std::fmax(g.gm_star, 0.0) / kAU;
+    d.sunit = line ? (float)source_unit(g, line) : 1.0f;
+}
+
+void make_dev_line(const radt_line *line, DevLine &d)
+{
+    double T0 = kH * line->nu0 / kK;
+    d.T0 = (float)T0; d.T0l2 = (float)(T0 * kLOG2E);
+    d.Eu = (float)line->e_u_K; d.Eul2 = (float)(line->e_u_K * kLOG2E);
+    d.gu = (float)line->g_u;
+    d.a1 = (float)(2.0 * kK / line->m_line + line->vturb_mach * line->vturb_mach * 2.0 * kK / line->m_gas);
+    d.a0 = (float)(line->vturb_abs * line->vturb_abs);
+    double Ck = kC * kC / (8.0 * kPI * line->nu0 * line->nu0) * line->a_ul * kC / (line->nu0 * std::sqrt(kPI)) * kAU;
+    d.Ck2 = (float)(Ck * kLOG2E);
+    d.nchan = line->nchan;
+    d.ngroups = (line->nchan + 31) / 32;
+}
+
+struct WsLayout {
+    size_t rays, qtab, vcs, rnode, cells, grad, counters, total;
+};
+
+WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass)
+{
+    WsLayout w;
+    size_t off = 0;
+    size_t nrays = (size_t)geom[0].nx * geom[0].ny * (size_t)batch;
+    w.counters = off; off = align256(off + 8 * sizeof(unsigned long long));
+    w.rays = off; off = align256(off + nrays * sizeof(double2));
+    w.qtab = off; off = align256(off + (RADT_NQ + 2) * sizeof(float2));
+    w.vcs = off; off = align256(off + (size_t)batch * RADT_MAXCHAN * sizeof(float2));
+    w.rnode = off; off = align256(off + (size_t)(grid->kind == RADT_GRID_AXISYM ? grid->n[0] : 1) * sizeof(double2));
+    size_t cells = (size_t)grid_cells(grid) * (size_t)batch;
+    w.cells = off; off = align256(off + cells * sizeof(float4));
+    w.grad = off;
+    if (pass == RADT_PASS_BWD) off = align256(off + cells * 4 * sizeof(double));
+    w.total = off;
+    return w;
+}
+
+DevWs make_dev_ws(void *ws, const WsLayout &w)
+{
+    char *base = (char *)ws;
+    DevWs d;
+    d.counters = (unsigned long long *)(base + w.counters);
+    d.rays = (double2 *)(base + w.rays);
+    d.qtab = (float2 *)(base + w.qtab);
+    d.vcs = (float2 *)(base + w.vcs);
+    d.rnode = (double2 *)(base + w.rnode);
+    d.cells = (float4 *)(base + w.cells);
+    d.grad = (double *)(base + w.grad);
+    return d;
+}
+
+// Enqueue setup + march for all batch chunks.  pass 0: forward into `cube`; pass 1: adjoint.
+int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int batch, int pass, float *cube,
+             const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel, void *ws, size_t ws_bytes,
+             cudaStream_t st)
+{
+    int rc = validate(geom, line, grid, batch);
+    if (rc) return rc;
+    if (!line) return fail(RADT_E_INVALID, "null line descriptor");
+    if (!ws) return fail(RADT_E_INVALID, "null workspace");
+    if (!grid->dens || !grid->temp || !grid->vel) return fail(RADT_E_INVALID, "null field pointer");
+    if (!cube) return fail(RADT_E_INVALID, "null cube pointer");
+    if (pass == RADT_PASS_BWD && !dl_dcube) return fail(RADT_E_INVALID, "null dl_dcube pointer");
+    WsLayout w = ws_layout(geom, grid, batch, pass);
+    if (ws_bytes < w.total) return fail(RADT_E_WORKSPACE, "workspace too small: need %zu bytes, got %zu", w.total, ws_bytes);
+    if (((uintptr_t)ws & 15) != 0) return fail(RADT_E_INVALID, "workspace must be 16-byte aligned");
+    long long stride = batch > 1 ? grid->batch_stride : grid_cells(grid);
+    if (batch > 1 && stride < grid_cells(grid)) return fail(RADT_E_INVALID, "batch_stride smaller than the grid");
+
+    g_launches = 0;
+    static thread_local MarchParams MP;
+    static thread_local SetupParams SP;
+    static thread_local LevelTable LT;
+    static thread_local ChanTable CT;
+    memset(&LT, 0, sizeof(LT));
+    memset(&CT, 0, sizeof(CT));
+    for (int l = 0; l < line->nlev; ++l) { LT.e[l] = line->e_lev_K[l]; LT.g[l] = line->g_lev[l]; }
+    for (int c = 0; c < line->nchan; ++c) CT.v[c] = line->vchan[c];
+
+    DevGrid dg;
+    make_dev_grid(grid, dg);
+    DevWs dws = make_dev_ws(ws, w);
+    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, 8 * sizeof(unsigned long long), st));
+    for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
+        int nb = batch - b0 < RADT_MAXB ? batch - b0 : RADT_MAXB;
+        memset(&SP, 0, sizeof(SP));
+        for (int b = 0; b < nb; ++b) {
+            make_dev_geom(geom[b0 + b], line, SP.geom[b]);
+            SP.vsys[b] = geom[b0 + b].vsys;
+        }
+        SP.grid = dg; SP.ws = dws;
+        SP.nx = geom[0].nx; SP.ny = geom[0].ny; SP.nstep = geom[0].nstep; SP.nbatch = nb; SP.b0 = b0;
+        SP.nlev = line->nlev; SP.nchan = line->nchan;
+        SP.do_rays = 1; SP.do_tables = 1; SP.do_pack = 1; SP.do_zero_grad = (pass == RADT_PASS_BWD);
+        SP.batch_stride = stride;
+        SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;
+        CUDA_TRY(radt_launch_setup(SP, LT, CT, st));
+        ++g_launches;
+
+        memset(&MP, 0, sizeof(MP));
+        memcpy(MP.geom, SP.geom, sizeof(MP.geom));
+        MP.grid = dg; MP.ws = dws;
+        make_dev_line(line, MP.line);
+        MP.nx = SP.nx; MP.ny = SP.ny; MP.nstep = SP.nstep;
+        MP.tiles_x = (MP.nx + RADT_TILE_X - 1) / RADT_TILE_X;
+        MP.tiles_y = (MP.ny + RADT_TILE_Y - 1) / RADT_TILE_Y;
+        MP.b0 = b0;
+        MP.opt_window = g_opt_window; MP.opt_skip_empty = g_opt_skip_empty;
+        MP.chan_lo = 0;
+        for (int b = 0; b < nb && !MP.chan_lo; ++b)
+            for (int c = 0; c < line->nchan; ++c) {
+                double vv = line->vchan[c] - geom[b0 + b].vsys;
+                if ((double)(float)vv != vv) { MP.chan_lo = 1; break; }
+            }
+        MP.cube = cube; MP.dl_dcube = dl_dcube;
+        if (pass == RADT_PASS_FWD) CUDA_TRY(radt_launch_march_fwd(MP, nb, st));
+        else CUDA_TRY(radt_launch_march_bwd(MP, nb, st));
+        ++g_launches;
+    }
+    if (pass == RADT_PASS_BWD && (g_dens || g_temp || g_vel)) {
+        CUDA_TRY(radt_launch_unpack(dws.grad, dg.cells, batch, stride, g_dens, g_temp, g_vel, st));
+        ++g_launches;
+    }
+    return RADT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int radt_version(void) { return RADT_VERSION; }
+const char *radt_last_error(void) { return g_err; }
+int radt_last_launch_count(void) { return g_launches; }
+
+int radt_set_option(int key, int value)
+{
+    if (key == RADT_OPT_WINDOW) { g_opt_window = value != 0; return RADT_OK; }
+    if (key == RADT_OPT_SKIP_EMPTY) { g_opt_skip_empty = value != 0; return RADT_OK; }
+    return fail(RADT_E_INVALID, "unknown option %d", key);
+}
+
+int radt_get_option(int key)
+{
+    if (key == RADT_OPT_WINDOW) return g_opt_window;
+    if (key == RADT_OPT_SKIP_EMPTY) return g_opt_skip_empty;
+    return fail(RADT_E_INVALID, "unknown option %d", key);
+}
+
+int radt_workspace_bytes(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                         int32_t pass, size_t *bytes_out)
+{
+    if (!bytes_out) return fail(RADT_E_INVALID, "null bytes_out");
+    int rc = validate(geom, line, grid, batch);
+    if (rc) return rc;
+    if (pass != RADT_PASS_FWD && pass != RADT_PASS_BWD) return fail(RADT_E_INVALID, "unknown pass");
+    *bytes_out = ws_layout(geom, grid, batch, pass).total;
+    return RADT_OK;
+}
+
+int radt_ray_geometry(const radt_geom *geom, const radt_grid *grid, int32_t batch, double *rays_out, void *cuda_stream)
+{
+    int rc = validate(geom, nullptr, grid, batch);
+    if (rc) return rc;
+    if (!rays_out) return fail(RADT_E_INVALID, "null rays_out");
+    static thread_local SetupParams SP;
+    static thread_local LevelTable LT;
+    static thread_local ChanTable CT;
+    DevGrid dg;
+    make_dev_grid(grid, dg);
+    g_launches = 0;
+    for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
+        int nb = batch - b0 < RADT_MAXB ? batch - b0 : RADT_MAXB;
+        memset(&SP, 0, sizeof(SP));
+        for (int b = 0; b < nb; ++b) make_dev_geom(geom[b0 + b], nullptr, SP.geom[b]);
+        SP.grid = dg;
+        SP.ws.rays = (double2 *)rays_out;
+        SP.nx = geom[0].nx; SP.ny = geom[0].ny; SP.nstep = geom[0].nstep; SP.nbatch = nb; SP.b0 = b0;
+        SP.do_rays = 1;
+        CUDA_TRY(radt_launch_setup(SP, LT, CT, (cudaStream_t)cuda_stream));
+        ++g_launches;
+    }
+    return RADT_OK;
+}
+
+int radt_render(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, float *cube,
+                void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    return run_pass(geom, line, grid, batch, RADT_PASS_FWD, cube, nullptr, nullptr, nullptr, nullptr, ws, ws_bytes,
+                    (cudaStream_t)cuda_stream);
+}
+
+int radt_render_bwd(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                    const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel, void *ws,
+                    size_t ws_bytes, void *cuda_stream)
+{
+    return run_pass(geom, line, grid, batch, RADT_PASS_BWD, const_cast<float *>(cube), dl_dcube, g_dens, g_temp, g_vel,
+                    ws, ws_bytes, (cudaStream_t)cuda_stream);
+}
+
+int radt_l2_loss_grad(const float *cube, const float *target, double sigma, int64_t n, float *dl_dcube,
+                      double *loss_out, void *cuda_stream)
+{
+    if (!cube || !target || !dl_dcube || !loss_out) return fail(RADT_E_INVALID, "null pointer");
+    if (n < 1 || !(sigma > 0)) return fail(RADT_E_INVALID, "need n >= 1 and sigma > 0");
+    CUDA_TRY(radt_launch_l2(cube, target, sigma, n, dl_dcube, loss_out, (cudaStream_t)cuda_stream));
+    g_launches = 1;
+    return RADT_OK;
+}
+
+int radt_read_counters(const void *ws, uint64_t *out4, void *cuda_stream)
+{
+    if (!ws || !out4) return fail(RADT_E_INVALID, "null pointer");
+    CUDA_TRY(cudaMemcpyAsync(out4, ws, 4 * sizeof(uint64_t), cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    return RADT_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// HOST-buffer entry points: stream-ordered allocation, H2D, same kernels, D2H, synchronise.
+// ------------------------------------------------------------------------------------------
+namespace {
+struct DevBufs {
+    cudaStream_t st = 0;
+    void *ptrs[16];
+    int n = 0;
+    void *alloc(size_t bytes)
+    {
+        void *p = nullptr;
+        if (cudaMallocAsync(&p, bytes ? bytes : 16, st) != cudaSuccess) return nullptr;
+        ptrs[n++] = p;
+        return p;
+    }
+    ~DevBufs()
+    {
+        for (int i = 0; i < n; ++i) cudaFreeAsync(ptrs[i], st);
+    }
+};
+}  // namespace
+
+static int host_common(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, int mode,
+                       const float *target, double sigma, float *cube, const float *cube_in, const float *dl_in,
+                       double *loss_out, float *g_dens, float *g_temp, float *g_vel)
+{
+    // mode 0: forward only; 1: forward + L2 + adjoint; 2: adjoint from given cube and dl_dcube
+    int rc = validate(geom, line, grid, batch);
+    if (rc) return rc;
+    if (!line) return fail(RADT_E_INVALID, "null line descriptor");
+    if (!grid->dens || !grid->temp || !grid->vel) return fail(RADT_E_INVALID, "null field pointer");
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count < 1) return fail(RADT_E_CUDA, "no CUDA device");
+    DevBufs B;
+    long long cells = grid_cells(grid);
+    long long stride = batch > 1 ? grid->batch_stride : cells;
+    size_t fbytes = (size_t)((batch - 1) * stride + cells) * sizeof(float);
+    size_t nvox = (size_t)batch * geom[0].nx * geom[0].ny * line->nchan;
+    float *d_dens = (float *)B.alloc(fbytes), *d_temp = (float *)B.alloc(fbytes), *d_vel = (float *)B.alloc(fbytes);
+    float *d_cube = (float *)B.alloc(nvox * sizeof(float));
+    if (!d_dens || !d_temp || !d_vel || !d_cube) return fail(RADT_E_CUDA, "device allocation failed");
+    CUDA_TRY(cudaMemcpyAsync(d_dens, grid->dens, fbytes, cudaMemcpyHostToDevice, B.st));
+    CUDA_TRY(cudaMemcpyAsync(d_temp, grid->temp, fbytes, cudaMemcpyHostToDevice, B.st));
+    CUDA_TRY(cudaMemcpyAsync(d_vel, grid->vel, fbytes, cudaMemcpyHostToDevice, B.st));
+    radt_grid dgrid = *grid;
+    dgrid.dens = d_dens; dgrid.temp = d_temp; dgrid.vel = d_vel;
+    size_t wsb = ws_layout(geom, grid, batch, mode == 0 ? RADT_PASS_FWD : RADT_PASS_BWD).total;
+    void *ws = B.alloc(wsb);
+    if (!ws) return fail(RADT_E_CUDA, "device allocation failed");
+    int launches = 0;
+    if (mode == 0 || mode == 1) {
+        rc = radt_render(geom, line, &dgrid, batch, d_cube, ws, wsb, B.st);
+        if (rc) return rc;
+        launches += g_launches;
+        if (cube) CUDA_TRY(cudaMemcpyAsync(cube, d_cube, nvox * sizeof(float), cudaMemcpyDeviceToHost, B.st));
+    }
+    if (mode == 1 || mode == 2) {
+        float *d_dl = (float *)B.alloc(nvox * sizeof(float));
+        float *d_g[3] = { nullptr, nullptr, nullptr };
+        float *h_g[3] = { g_dens, g_temp, g_vel };
+        for (int i = 0; i < 3; ++i)
+            if (h_g[i] && !(d_g[i] = (float *)B.alloc(fbytes))) return fail(RADT_E_CUDA, "device allocation failed");
+        if (!d_dl) return fail(RADT_E_CUDA, "device allocation failed");
+        if (mode == 1) {
+            if (!target) return fail(RADT_E_INVALID, "null target");
+            float *d_t = (float *)B.alloc(nvox * sizeof(float));
+            double *d_loss = (double *)B.alloc(sizeof(double));
+            if (!d_t || !d_loss) return fail(RADT_E_CUDA, "device allocation failed");
+            CUDA_TRY(cudaMemcpyAsync(d_t, target, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
+            rc = radt_l2_loss_grad(d_cube, d_t, sigma, (int64_t)nvox, d_dl, d_loss, B.st);
+            if (rc) return rc;
+            ++launches;
+            if (loss_out) CUDA_TRY(cudaMemcpyAsync(loss_out, d_loss, sizeof(double), cudaMemcpyDeviceToHost, B.st));
+        } else {
+            if (!cube_in || !dl_in) return fail(RADT_E_INVALID, "null cube / dl_dcube");
+            CUDA_TRY(cudaMemcpyAsync(d_cube, cube_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
+            CUDA_TRY(cudaMemcpyAsync(d_dl, dl_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
+        }
+        rc = radt_render_bwd(geom, line, &dgrid, batch, d_cube, d_dl, d_g[0], d_g[1], d_g[2], ws, wsb, B.st);
+        if (rc) return rc;
+        launches += g_launches;
+        for (int i = 0; i < 3; ++i)
+            if (h_g[i]) CUDA_TRY(cudaMemcpyAsync(h_g[i], d_g[i], fbytes, cudaMemcpyDeviceToHost, B.st));
+    }
+    CUDA_TRY(cudaStreamSynchronize(B.st));
+    g_launches = launches;
+    return RADT_OK;
+}
+
+int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, float *cube)
+{
+    if (!cube) return fail(RADT_E_INVALID, "null cube pointer");
+    return host_common(geom, line, grid, batch, 0, nullptr, 0.0, cube, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+}
+
+int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                       const float *target, double sigma, float *cube, double *loss_out, float *g_dens, float *g_temp,
+                       float *g_vel)
+{
+    if (!(sigma > 0)) return fail(RADT_E_INVALID, "sigma must be positive");
+    return host_common(geom, line, grid, batch, 1, target, sigma, cube, nullptr, nullptr, loss_out, g_dens, g_temp, g_vel);
+}
+
+int radt_render_bwd_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                         const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel)
+{
+    return host_common(geom, line, grid, batch, 2, nullptr, 0.0, nullptr, cube, dl_dcube, nullptr, g_dens, g_temp, g_vel);
+}
+
+int radt_pipe_peak(int32_t kind, double *ops_per_s_out, double *sm_clock_mhz_out)
+{
+    if (!ops_per_s_out) return fail(RADT_E_INVALID, "null output");
+    if (kind < 0 || kind > 3) return fail(RADT_E_INVALID, "unknown pipe kind");
+    double clk = 0.0;
+    CUDA_TRY(radt_run_pipe_peak(kind, ops_per_s_out, &clk));
+    if (sm_clock_mhz_out) *sm_clock_mhz_out = clk;
+    return RADT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,123 @@
+// radt_dev.cuh -- device-side parameter blocks and math helpers of the B200 line-RT render.
+// Product code: shares nothing with oracle/.  Algorithm statement: DESIGN.md O1-O11
+// (Eq. 11-17).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define RADT_WARPS_PER_CTA 8          // one warp per ray; CTA = 4 x 2 pixel tile
+#define RADT_TILE_X 4
+#define RADT_TILE_Y 2
+#define RADT_MAXB 16                  // batch items per launch (geometry travels in kernel params)
+#define RADT_NQ 4096                  // partition-function table intervals over log2 T in [0, 14]
+#define RADT_NQ_OCTAVES 14.0f
+#define RADT_MAXLEV 64
+#define RADT_MAXCHAN 256
+
+#define RADT_LOG2E 1.4426950408889634f
+#define RADT_LN2 0.6931471805599453f
+#define RADT_SQRT_LOG2E 1.2011224087864498f
+
+// Per batch item viewing geometry, precomputed on the host in fp64 (O1-O2).
+struct DevGeom {
+    double cth, sth, ci, si, ca, sa;   // cos/sin of PA + pi/2, inclination, azimuth
+    double wx, wy, wz;                 // ray direction (increasing s) in the disk frame
+    double x0, y0, pix_x, pix_y;       // image centre offset and pixel pitch, au
+    double gm_au_d;                    // G M / au  [(cm/s)^2 au]  (KEPLER_FRAC)
+    float sunit;                       // S0 / intensity unit
+};
+
+struct DevGrid {
+    int kind, mirror, dens_mode, vel_mode;
+    int n0, n1, n2;
+    long long cells;                   // cells per batch item
+    // axisymmetric
+    double rmin2, rmax2, inv_rmin, zlo, zhi;
+    double wscale_d;                   // (nzeta-1)/(zeta_hi-zeta_lo)
+    double lg2_ratio;                  // log2(r_max/r_min)
+    float uscale;                      // (nr-1)/log2(r_max/r_min)
+    float inv_cell_ln, inv_cell_lg2;   // 1/ln(rho), 1/log2(rho), rho = node ratio r_{i+1}/r_i
+    int fine_r;                        // rho - 1 < 0.15: log1p series for the in-cell fraction
+    // cartesian
+    double lo[3], hi[3], inv_d[3];
+    double rb2;                        // bounding sphere radius^2 (axisym clip)
+};
+
+struct DevLine {
+    float T0;          // h nu0 / k
+    float T0l2;        // T0 * log2(e)
+    float Eu;          // E_u / k
+    float Eul2;        // Eu * log2(e)
+    float gu;
+    float a1, a0;      // alpha^2 = a1 T + a0   [(cm/s)^2]
+    float Ck2;         // line-centre dtau * log2e = Ck2 * n * W * (e^x - 1) * ds[au] / alpha
+    int nchan;
+    int ngroups;       // ceil(nchan / 32)
+};
+
+// Workspace layout (all offsets in bytes from the workspace base, 256-byte aligned)
+struct DevWs {
+    double2 *rays;         // [batch*ny*nx] {s0, ds}
+    float2 *qtab;          // [RADT_NQ + 2] {Q, dQ/dlnT}
+    float2 *vcs;           // [batch][RADT_MAXCHAN] channel velocity minus v_sys, cm/s, as (hi, lo) float pair
+    double2 *rnode;        // [nr] {r_i, 1/r_i} node radii of the log-spaced axis (axisym), fp64
+    float4 *cells;         // [batch][cells] packed {dens, temp, vel, 0}
+    double *grad;          // [batch][cells][4] packed fp64 gradient accumulators {dens, temp, vel, -} (bwd only)
+    unsigned long long *counters;   // [8] 0-3 work counters; [4] bits of the grid's maximum temperature
+};
+
+struct MarchParams {
+    DevGeom geom[RADT_MAXB];
+    DevGrid grid;
+    DevLine line;
+    DevWs ws;
+    int nx, ny, nstep;
+    int tiles_x, tiles_y;
+    int b0;                // first batch item of this launch
+    int opt_window, opt_skip_empty;
+    int chan_lo;           // some channel velocity is not exactly representable in fp32: use the lo parts
+    float *cube;           // fwd: output; bwd: saved forward output (const)
+    const float *dl_dcube; // bwd
+};
+
+struct SetupParams {
+    DevGeom geom[RADT_MAXB];
+    DevGrid grid;
+    DevWs ws;
+    int nx, ny, nstep, nbatch, b0;
+    int nlev, nchan;
+    int do_rays, do_tables, do_pack, do_zero_grad;
+    long long batch_stride;
+    const float *dens, *temp, *vel;
+    double vsys[RADT_MAXB];
+};
+
+struct LevelTable {
+    double e[RADT_MAXLEV];
+    double g[RADT_MAXLEV];
+};
+
+struct ChanTable {
+    double v[RADT_MAXCHAN];
+};
+
+// ---- single-instruction SFU helpers (MUFU.*) ----
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// Disk-frame position of the s = 0 point of pixel (ix, iy)  (O1-O2).
+__device__ __forceinline__ void pixel_origin(const DevGeom &G, int nx, int ny, int ix, int iy,
+                                             double &ox, double &oy, double &oz, double &X, double &Y)
+{
+    X = G.x0 + ((double)ix + 0.5 - 0.5 * (double)nx) * G.pix_x;
+    Y = G.y0 + ((double)iy + 0.5 - 0.5 * (double)ny) * G.pix_y;
+    double xp = X * G.cth + Y * G.sth;
+    double yp = -X * G.sth + Y * G.cth;
+    double ypp = yp * G.ci;
+    oz = yp * G.si;
+    ox = xp * G.ca + ypp * G.sa;
+    oy = -xp * G.sa + ypp * G.ca;
+}

@@ -1,0 +1,12 @@
+// radt_kernels.h -- host-callable launchers of the CUDA kernels (internal to the library).
+#pragma once
+#include "radt_dev.cuh"
+
+cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const ChanTable &V, cudaStream_t st);
+cudaError_t radt_launch_unpack(const double *grad, long long cells, int nbatch, long long batch_stride, float *g_dens,
+                               float *g_temp, float *g_vel, cudaStream_t st);
+cudaError_t radt_launch_l2(const float *cube, const float *target, double sigma, long long n, float *dl, double *loss,
+                           cudaStream_t st);
+cudaError_t radt_launch_march_fwd(const MarchParams &P, int nbatch, cudaStream_t st);
+cudaError_t radt_launch_march_bwd(const MarchParams &P, int nbatch, cudaStream_t st);
+cudaError_t radt_run_pipe_peak(int kind, double *ops_per_s, double *clock_mhz);

@@ -1,0 +1,189 @@
+// radt_setup.cu -- K1 ray geometry, per-call tables, field packing, gradient unpacking, L2 loss.
+// One fused "setup" launch precedes every march so that small problems stay launch-lean.
+#include "radt_dev.cuh"
+#include "radt_kernels.h"
+
+// ---------------------------------------------------------------------------------------------
+// K1 ray geometry (O1-O3): per pixel the clipped interval {s0, ds}; ds = 0 marks a miss.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double2 clip_ray(const DevGeom &G, const DevGrid &g, int nx, int ny, int nstep, int ix, int iy)
+{
+    double ox, oy, oz, X, Y;
+    pixel_origin(G, nx, ny, ix, iy, ox, oy, oz, X, Y);
+    if (g.kind == 0) {
+        // s = 0 is the closest approach to the star, |p(s)|^2 = b^2 + s^2
+        double b2 = X * X + Y * Y;
+        if (!(b2 < g.rb2)) return make_double2(0.0, 0.0);
+        double sh = sqrt(g.rb2 - b2);
+        return make_double2(-sh, 2.0 * sh / (double)nstep);
+    }
+    const double o[3] = { ox, oy, oz }, d[3] = { G.wx, G.wy, G.wz };
+    double tmin = -INFINITY, tmax = INFINITY;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (d[a] != 0.0) {
+            double t1 = (g.lo[a] - o[a]) / d[a], t2 = (g.hi[a] - o[a]) / d[a];
+            tmin = fmax(tmin, fmin(t1, t2));
+            tmax = fmin(tmax, fmax(t1, t2));
+        } else if (o[a] < g.lo[a] || o[a] > g.hi[a]) {
+            return make_double2(0.0, 0.0);
+        }
+    }
+    if (!(tmax > tmin)) return make_double2(0.0, 0.0);
+    return make_double2(tmin, (tmax - tmin) / (double)nstep);
+}
+
+// Block roles: [0, nb_rays) rays; [nb_rays, nb_rays + nb_tab) tables; the rest pack fields.
+__global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupParams P, const __grid_constant__ LevelTable L,
+                                               const __grid_constant__ ChanTable V, int nb_rays, int nb_tab)
+{
+    int blk = blockIdx.x;
+    if (blk < nb_rays) {
+        long long per_item = (long long)P.nx * P.ny;
+        long long q = (long long)blk * blockDim.x + threadIdx.x;
+        if (q >= per_item * P.nbatch) return;
+        int b = (int)(q / per_item);
+        long long rem = q - (long long)b * per_item;
+        int iy = (int)(rem / P.nx), ix = (int)(rem - (long long)iy * P.nx);
+        P.ws.rays[(long long)(P.b0 + b) * per_item + rem] = clip_ray(P.geom[b], P.grid, P.nx, P.ny, P.nstep, ix, iy);
+        return;
+    }
+    blk -= nb_rays;
+    if (blk < nb_tab) {
+        int t = blk * blockDim.x + threadIdx.x;
+        if (t <= RADT_NQ + 1) {
+            // partition function Q(T) = sum g_J exp(-E_J/T) and dQ/dlnT on a log2-T lattice
+            double T = exp2((double)t * (double)RADT_NQ_OCTAVES / (double)RADT_NQ);
+            double q = 0.0, dq = 0.0;
+            for (int l = 0; l < P.nlev; ++l) {
+                double y = L.e[l] / T;
+                double w = L.g[l] * exp(-y);
+                q += w;
+                dq += w * y;
+            }
+            P.ws.qtab[t] = make_float2((float)q, (float)dq);
+        }
+        if (t < P.nbatch * RADT_MAXCHAN) {
+            int b = t / RADT_MAXCHAN, c = t % RADT_MAXCHAN;
+            double vv = (c < P.nchan) ? V.v[c] - P.vsys[b] : 0.0;
+            float hi = (float)vv;
+            P.ws.vcs[(size_t)(P.b0 + b) * RADT_MAXCHAN + c] = make_float2(hi, (float)(vv - (double)hi));
+        }
+        if (P.grid.kind == 0 && t < P.grid.n0 && P.b0 == 0) {
+            // node radii of the log-spaced axis, r_i = r_min (r_max/r_min)^(i/(nr-1))
+            double ri = exp2((double)t * P.grid.lg2_ratio / (double)(P.grid.n0 - 1)) / P.grid.inv_rmin;
+            if (t == 0) ri = 1.0 / P.grid.inv_rmin;
+            P.ws.rnode[t] = make_double2(ri, 1.0 / ri);
+        }
+        return;
+    }
+    blk -= nb_tab;
+    // pack SoA planes into float4 cells {dens, temp, vel, 0}; optionally zero the gradient cells
+    long long total = P.grid.cells * P.nbatch;
+    long long stride = (long long)(gridDim.x - nb_rays - nb_tab) * blockDim.x;
+    float tmax = 0.f;
+    for (long long q = (long long)blk * blockDim.x + threadIdx.x; q < total; q += stride) {
+        int b = (int)(q / P.grid.cells);
+        long long c = q - (long long)b * P.grid.cells;
+        long long src = (long long)(P.b0 + b) * P.batch_stride + c;
+        long long dst = (long long)(P.b0 + b) * P.grid.cells + c;
+        if (P.do_pack) {
+            float tt = __ldg(P.temp + src);
+            tmax = fmaxf(tmax, tt);
+            P.ws.cells[dst] = make_float4(__ldg(P.dens + src), tt, __ldg(P.vel + src), 0.0f);
+        }
+        if (P.do_zero_grad) {
+            double4 *gz = reinterpret_cast<double4 *>(P.ws.grad) + dst;
+            *gz = make_double4(0.0, 0.0, 0.0, 0.0);
+        }
+    }
+    // grid-wide maximum temperature (bounds the source function in the adjoint); counters[4] holds its bits
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, m));
+    if ((threadIdx.x & 31) == 0 && tmax > 0.f) atomicMax(reinterpret_cast<int *>(P.ws.counters + 4), __float_as_int(tmax));
+}
+
+__global__ void __launch_bounds__(256) k_unpack_grad(const double *__restrict__ grad, long long cells, int nbatch,
+                                                     long long batch_stride, float *g_dens, float *g_temp, float *g_vel)
+{
+    long long total = cells * nbatch;
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += stride) {
+        int b = (int)(q / cells);
+        long long c = q - (long long)b * cells;
+        double4 v = *(reinterpret_cast<const double4 *>(grad) + q);
+        long long dst = (long long)b * batch_stride + c;
+        if (g_dens) g_dens[dst] = (float)v.x;
+        if (g_temp) g_temp[dst] = (float)v.y;
+        if (g_vel) g_vel[dst] = (float)v.z;
+    }
+}
+
+// L = 1/(2n) sum ((I - D)/sigma)^2 ; dL/dI = (I - D)/(sigma^2 n)   (chi^2 data term)
+__global__ void __launch_bounds__(256) k_l2_loss_grad(const float *__restrict__ cube, const float *__restrict__ target,
+                                                      float inv_s2n, double half_inv_s2n, long long n, float *dl,
+                                                      double *loss)
+{
+    long long stride = (long long)gridDim.x * blockDim.x;
+    double acc = 0.0;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) {
+        float r = cube[q] - target[q];
+        dl[q] = r * inv_s2n;
+        acc += (double)r * (double)r;
+    }
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, m);
+    __shared__ double part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += part[w];
+        atomicAdd(loss, s * half_inv_s2n);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-side launchers
+// ---------------------------------------------------------------------------------------------
+cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const ChanTable &V, cudaStream_t st)
+{
+    long long nrays = (long long)P.nx * P.ny * P.nbatch;
+    int nb_rays = P.do_rays ? (int)((nrays + 255) / 256) : 0;
+    int need_tab = RADT_NQ + 2;
+    if (P.nbatch * RADT_MAXCHAN > need_tab) need_tab = P.nbatch * RADT_MAXCHAN;
+    if (P.grid.kind == 0 && P.grid.n0 > need_tab) need_tab = P.grid.n0;
+    int nb_tab = P.do_tables ? (need_tab + 255) / 256 : 0;
+    long long total = P.grid.cells * P.nbatch;
+    int nb_pack = 0;
+    if (P.do_pack || P.do_zero_grad) {
+        long long nb = (total + 255) / 256;
+        nb_pack = (int)(nb < 148 * 16 ? nb : 148 * 16);
+    }
+    int nb = nb_rays + nb_tab + nb_pack;
+    if (nb == 0) return cudaSuccess;
+    k_setup<<<nb, 256, 0, st>>>(P, L, V, nb_rays, nb_tab);
+    return cudaGetLastError();
+}
+
+cudaError_t radt_launch_unpack(const double *grad, long long cells, int nbatch, long long batch_stride, float *g_dens,
+                               float *g_temp, float *g_vel, cudaStream_t st)
+{
+    long long total = cells * nbatch;
+    long long nb = (total + 255) / 256;
+    if (nb > 148 * 16) nb = 148 * 16;
+    k_unpack_grad<<<(int)nb, 256, 0, st>>>(grad, cells, nbatch, batch_stride, g_dens, g_temp, g_vel);
+    return cudaGetLastError();
+}
+
+cudaError_t radt_launch_l2(const float *cube, const float *target, double sigma, long long n, float *dl, double *loss,
+                           cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(loss, 0, sizeof(double), st);
+    if (e != cudaSuccess) return e;
+    double inv = 1.0 / (sigma * sigma * (double)n);
+    long long nb = (n + 255) / 256;
+    if (nb > 148 * 8) nb = 148 * 8;
+    k_l2_loss_grad<<<(int)nb, 256, 0, st>>>(cube, target, (float)inv, 0.5 * inv, n, dl, loss);
+    return cudaGetLastError();
+}

@@ -1,0 +1,75 @@
+"""Device-buffer plumbing around the C ABI: owns the torch tensors a render needs and forwards pointers."""
+from __future__ import annotations
+
+import numpy as np
+
+from . import binding as B
+
+
+class Renderer:
+    """Holds fields, workspace, cube and gradient buffers on one CUDA device for a batch of scenes."""
+
+    def __init__(self, scenes, device="cuda:0", need_bwd=True):
+        import torch
+        if not torch.cuda.is_available():
+            raise B.RadtError("no CUDA device: the render has no CPU fallback")
+        B.lib()
+        self.torch = torch
+        self.device = torch.device(device)
+        self.desc = B.Descriptors(scenes)
+        d = self.desc
+        host = B.stack_fields(scenes)
+        self.dens, self.temp, self.vel = (torch.from_numpy(h).to(self.device) for h in host)
+        self.cube = torch.empty(d.cube_shape, dtype=torch.float32, device=self.device)
+        nbytes = B.radt_workspace_bytes(d, B.PASS_BWD if need_bwd else B.PASS_FWD)
+        self.ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.need_bwd = need_bwd
+        if need_bwd:
+            self.dl_dcube = torch.empty_like(self.cube)
+            self.g_dens = torch.empty_like(self.dens)
+            self.g_temp = torch.empty_like(self.temp)
+            self.g_vel = torch.empty_like(self.vel)
+            self.loss = torch.zeros(1, dtype=torch.float64, device=self.device)
+        self.target = None
+        self.sigma = None
+
+    # ---- hot path: every call below is one C-ABI entry point ----
+    def render(self, stream=None):
+        B.radt_render(self.desc, self.dens, self.temp, self.vel, self.cube, self.ws, stream)
+        return self.cube
+
+    def render_bwd(self, dl_dcube=None, stream=None):
+        g = self.dl_dcube if dl_dcube is None else dl_dcube
+        B.radt_render_bwd(self.desc, self.dens, self.temp, self.vel, self.cube, g, self.g_dens, self.g_temp, self.g_vel,
+                          self.ws, stream)
+        return self.g_dens, self.g_temp, self.g_vel
+
+    def set_target(self, target, sigma):
+        t = self.torch.as_tensor(np.ascontiguousarray(target, np.float32)) if not self.torch.is_tensor(target) else target
+        self.target = t.to(self.device, dtype=self.torch.float32).reshape(self.cube.shape).contiguous()
+        self.sigma = float(sigma)
+
+    def l2_loss_grad(self, stream=None):
+        B.radt_l2_loss_grad(self.cube, self.target, self.sigma, self.dl_dcube, self.loss, stream)
+        return self.loss
+
+    def fit_step(self, stream=None):
+        """forward -> L2 data term -> adjoint (one pass of the whole hot path)."""
+        self.render(stream)
+        self.l2_loss_grad(stream)
+        self.render_bwd(stream=stream)
+
+    def set_fields(self, dens=None, temp=None, vel=None):
+        for name, val in (("dens", dens), ("temp", temp), ("vel", vel)):
+            if val is not None:
+                getattr(self, name).copy_(self.torch.as_tensor(np.ascontiguousarray(val, np.float32)).reshape(
+                    getattr(self, name).shape))
+
+    def counters(self):
+        return B.radt_read_counters(self.ws)
+
+    def ray_table(self):
+        d = self.desc
+        rays = self.torch.empty((d.batch, d.ny, d.nx, 2), dtype=self.torch.float64, device=self.device)
+        B.radt_ray_geometry(d, rays)
+        return rays

@@ -89,13 +89,13 @@ def _axisym_grid(nr, nz, rng, mstar=2.0, h0=8.0, hscale=_hscale_none, noise=0.1)
 def _grf(shape, spacing_au, corr_au, rms, rng):
     """Gaussian random field: white noise filtered by exp(-k^2 l^2 / 2), normalised to `rms`."""
     white = rng.standard_normal(shape)
-    fk = np.fft.rfftn(white)
+    fk = np.fft.rfftn(white, axes=(0, 1, 2))
     ks = [2.0 * np.pi * np.fft.fftfreq(shape[0], d=spacing_au[0]),
           2.0 * np.pi * np.fft.fftfreq(shape[1], d=spacing_au[1]),
           2.0 * np.pi * np.fft.rfftfreq(shape[2], d=spacing_au[2])]
     k2 = ks[0][:, None, None] ** 2 + ks[1][None, :, None] ** 2 + ks[2][None, None, :] ** 2
     fk *= np.exp(-0.5 * k2 * corr_au * corr_au)
-    out = np.fft.irfftn(fk, s=shape)
+    out = np.fft.irfftn(fk, s=shape, axes=(0, 1, 2))
     out *= rms / out.std()
     return out
 

@@ -1,0 +1,101 @@
+"""The C-ABI library loads, exports every symbol include/radt.h declares, and validates arguments on the
+host (no GPU needed: no compute call is made here)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2509_03623_b200 import binding as B
+from paper_2509_03623_b200 import build as radt_build
+from synth import make_config, tiny_axisym_scene, tiny_cart_scene
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    radt_build.build()
+    return B.lib()
+
+
+def test_exports_match_header(lib):
+    hdr = open(os.path.join(ROOT, "include", "radt.h")).read()
+    declared = sorted(set(re.findall(r"\b(radt_[a-z0-9_]+)\s*\(", hdr)))
+    assert len(declared) >= 14
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in include/radt.h but not exported"
+    assert sorted(B.EXPORTS) == declared, "binding.EXPORTS must mirror include/radt.h"
+    assert lib.radt_version() == 100
+
+
+def test_struct_layouts_and_workspace_size(lib):
+    """radt_workspace_bytes is host-only and checks struct_size: a ctypes/C layout mismatch fails here."""
+    for sc in (tiny_axisym_scene(), tiny_cart_scene(), make_config(1)):
+        d = B.Descriptors(sc)
+        fwd = B.radt_workspace_bytes(d, B.PASS_FWD)
+        bwd = B.radt_workspace_bytes(d, B.PASS_BWD)
+        assert 0 < fwd < bwd
+        assert bwd - fwd >= d.cells * 32          # fp64 gradient cells
+    d = B.Descriptors(make_config(2))
+    assert B.radt_workspace_bytes(d, B.PASS_FWD) >= 256 * 256 * 16 + 256 * 128 * 16
+
+
+@pytest.mark.parametrize("mutate,code", [
+    (lambda d: setattr(d.geom[0], "struct_size", 3), -1),
+    (lambda d: setattr(d.geom[0], "nstep", 0), -1),
+    (lambda d: setattr(d.geom[0], "fov_x", -1.0), -1),
+    (lambda d: setattr(d.line, "nchan", 257), -1),
+    (lambda d: setattr(d.line, "nlev", 65), -1),
+    (lambda d: setattr(d.line, "nu0", 0.0), -1),
+    (lambda d: setattr(d.grid, "kind", 7), -2),
+    (lambda d: setattr(d.grid, "dens_mode", 5), -2),
+    (lambda d: d.grid.lo.__setitem__(0, -1.0), -1),
+    (lambda d: d.grid.n.__setitem__(1, 1), -1),
+])
+def test_invalid_arguments_are_rejected(lib, mutate, code):
+    d = B.Descriptors(tiny_axisym_scene())
+    mutate(d)
+    out = C.c_size_t(0)
+    rc = lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), d.batch, 0, C.byref(out))
+    assert rc == code
+    assert len(lib.radt_last_error()) > 0
+
+
+def test_null_and_unsupported(lib):
+    d = B.Descriptors(tiny_cart_scene())
+    d.grid.mirror_z = 1
+    out = C.c_size_t(0)
+    assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 1, 0, C.byref(out)) == -2
+    d = B.Descriptors(tiny_axisym_scene())
+    assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 1, 0, None) == -1
+    assert lib.radt_workspace_bytes(None, C.byref(d.line), C.byref(d.grid), 1, 0, C.byref(out)) == -1
+    assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 0, 0, C.byref(out)) == -1
+    assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 1, 9, C.byref(out)) == -1
+    assert lib.radt_set_option(99, 1) == -1
+    assert lib.radt_set_option(B.OPT_WINDOW, 1) == 0 and lib.radt_get_option(B.OPT_WINDOW) == 1
+
+
+def test_batch_items_must_share_image_shape(lib):
+    a, b = tiny_axisym_scene(npix=6), tiny_axisym_scene(npix=7)
+    d = B.Descriptors([a, b])
+    out = C.c_size_t(0)
+    assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 2, 0, C.byref(out)) == -1
+
+
+def test_no_cpu_fallback_without_a_device(lib):
+    """On a box without a GPU the compute entry points fail loudly (RADT_E_CUDA); nothing is computed on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    sc = tiny_axisym_scene()
+    d = B.Descriptors(sc)
+    h = B.stack_fields(sc)
+    cube = np.full(d.cube_shape, 7.0, np.float32)
+    with pytest.raises(B.RadtError, match="-4"):
+        B.radt_render_host(d, *h, cube)
+    assert np.all(cube == 7.0)
+    from paper_2509_03623_b200 import Renderer
+    with pytest.raises(B.RadtError):
+        Renderer(sc)

@@ -1,0 +1,369 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on the same
+seeded inputs.  Tolerances: tests/tolerances.py (cube 1e-4, gradients 1e-3; BASELINE.json north_star)."""
+import math
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+from oracle import pyoracle as po
+from synth import (UNIT_CGS, UNIT_JY_PIXEL, co_line, l2_target, make_config, slab_scene, tiny_axisym_scene,
+                   tiny_cart_scene)
+from tests.tolerances import check_cube, check_grad
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def rt():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2509_03623_b200 as pkg
+    pkg.binding.lib()     # fails loudly if the CUDA library was not built
+    return pkg
+
+
+def _as_list(s):
+    return s if isinstance(s, list) else [s]
+
+
+def _oracle_cube(scenes):
+    return np.stack([po.render(s) for s in _as_list(scenes)])
+
+
+def _gpu_forward(rt, scenes, need_bwd=False):
+    R = rt.Renderer(_as_list(scenes), need_bwd=need_bwd)
+    R.render()
+    torch.cuda.synchronize()
+    return R
+
+
+def _parity_fwd_bwd(rt, scenes, name, seed=0, grad=True):
+    scenes = _as_list(scenes)
+    ref = _oracle_cube(scenes)
+    R = _gpu_forward(rt, scenes, need_bwd=grad)
+    check_cube(f"{name} cube", R.cube.cpu().numpy(), ref)
+    if not grad:
+        return R
+    # L2 data term against a seed-generated target; the SAME dL/dcube goes to the oracle and the GPU adjoint,
+    # and the GPU adjoint re-marches with its own forward cube (the API contract of radt_render_bwd)
+    G = np.empty_like(ref)
+    for b in range(len(scenes)):
+        if ref[b].max() > 0:
+            tgt, sigma = l2_target(ref[b], 1000 + seed + b)
+            G[b] = (ref[b] - tgt) / (sigma ** 2 * ref[b].size)
+        else:       # dark cube: any dL/dcube will do
+            G[b] = 1e-6 * np.random.default_rng(seed + b).standard_normal(ref[b].shape)
+    G32 = G.astype(np.float32)
+    R.dl_dcube.copy_(torch.from_numpy(G32))
+    gd, gt, gv = (g.cpu().numpy() for g in R.render_bwd())
+    for b, sc in enumerate(scenes):
+        rd, rtm, rv = po.render_bwd(sc, G32[b].astype(np.float64))
+        check_grad(f"{name}[{b}] g_dens", gd[b], rd)
+        check_grad(f"{name}[{b}] g_temp", gt[b], rtm)
+        check_grad(f"{name}[{b}] g_vel", gv[b], rv)
+    return R
+
+
+# ------------------------------------------------------------------ K1 ray geometry
+@pytest.mark.parametrize("make", [lambda: tiny_axisym_scene(seed=1, npix=9, npix_y=5), lambda: tiny_cart_scene(seed=2, npix=7),
+                                  lambda: make_config(1), lambda: replace(make_config(1), geom=replace(make_config(1).geom, fov_x=1500.0, fov_y=1500.0))])
+def test_ray_geometry_matches_oracle(rt, make):
+    sc = make()
+    R = rt.Renderer([sc], need_bwd=False)
+    rays = R.ray_table().cpu().numpy()[0].reshape(-1, 2)
+    geo = po.ray_geometry(sc)
+    np.testing.assert_array_equal(rays[:, 1] != 0.0, geo["valid"] == 1)
+    np.testing.assert_allclose(rays[:, 0], geo["s0"], rtol=1e-13, atol=1e-10)
+    np.testing.assert_allclose(rays[:, 1], geo["ds"], rtol=1e-13, atol=1e-12)
+
+
+# ------------------------------------------------------------------ small scenes, every mode
+@pytest.mark.parametrize("kw", [
+    dict(seed=31),
+    dict(seed=32, dens_ln=True, kepler_frac=True, vsys=0.3e5, vturb_mach=0.3, mirror=False, az_deg=20.0),
+    dict(seed=33, incl_deg=0.0, pa_deg=0.0),
+    dict(seed=34, incl_deg=90.0, pa_deg=312.0, npix=5, npix_y=3),
+    dict(seed=35, nr=40, nz=33, npix=16, nchan=33, nstep=70),          # ragged channel group and step block
+    dict(seed=36, nr=5, nz=4, npix=3, nchan=1, nstep=1),
+])
+def test_tiny_axisym(rt, kw):
+    _parity_fwd_bwd(rt, tiny_axisym_scene(**kw), f"tiny_axisym{kw}")
+
+
+@pytest.mark.parametrize("kw", [dict(seed=41), dict(seed=42, dens_ln=False, kepler_frac=False),
+                                dict(seed=43, incl_deg=80.0, pa_deg=-40.0, ng=(20, 17, 13), npix=12, nchan=40, nstep=45)])
+def test_tiny_cart(rt, kw):
+    _parity_fwd_bwd(rt, tiny_cart_scene(**kw), f"tiny_cart{kw}")
+
+
+@pytest.mark.parametrize("n,T,v", [(1.0, 30.0, 0.0), (1e-4, 30.0, 0.0), (400.0, 150.0, 0.1e5), (1e6, 40.0, 0.0)])
+def test_slab_closed_form(rt, n, T, v, slab_golden):
+    sc = slab_scene(n_co=n, temp=T, vchan_cms=[v, 0.05e5], nstep=9, npix=3)
+    _parity_fwd_bwd(rt, sc, f"slab n={n} T={T}")
+
+
+def test_slab_worked_value_directly(rt, slab_golden):
+    """The GPU cube reproduces the paper-side worked number without going through the oracle."""
+    R = _gpu_forward(rt, slab_scene(vchan_cms=[0.0, 0.1e5, 0.3e5], npix=2))
+    got = R.cube.cpu().numpy()[0, 0, 0]
+    S0 = slab_golden["S0_cgs"]
+    assert got[0] == pytest.approx(slab_golden["I_v0_over_S0"], rel=1e-5)
+    assert got[1] * S0 == pytest.approx(slab_golden["I_v0p1kms_cgs"], rel=1e-5)
+    assert got[2] * S0 == pytest.approx(slab_golden["I_v0p3kms_cgs"], rel=1e-5)
+
+
+@pytest.mark.parametrize("unit", [UNIT_CGS, UNIT_JY_PIXEL])
+def test_units(rt, unit):
+    sc = tiny_axisym_scene(seed=37)
+    sc = replace(sc, line=replace(sc.line, unit=unit))
+    _parity_fwd_bwd(rt, sc, f"unit{unit}")
+
+
+def test_inexact_channel_velocities_and_vsys(rt):
+    """Channel velocities that are not exactly representable in fp32 take the (hi, lo) channel path."""
+    sc = tiny_axisym_scene(seed=38, nchan=9, vsys=5.76e5 + 1.0 / 3.0)
+    v = sc.line.vchan + 5.76e5 + math.pi * 1e-3
+    sc = replace(sc, line=replace(sc.line, vchan=v))
+    _parity_fwd_bwd(rt, sc, "inexact channels")
+
+
+# ------------------------------------------------------------------ the five configs
+def test_cfg1_full(rt):
+    _parity_fwd_bwd(rt, make_config(1), "cfg1")
+
+
+def test_cfg2_reduced(rt):
+    _parity_fwd_bwd(rt, make_config(2, npix=96), "cfg2 96px")
+
+
+def test_cfg2_full(rt):
+    _parity_fwd_bwd(rt, make_config(2), "cfg2 full")
+
+
+def test_cfg3_reduced(rt):
+    _parity_fwd_bwd(rt, make_config(3, npix=64), "cfg3 64px")
+
+
+def test_cfg4_reduced(rt):
+    _parity_fwd_bwd(rt, make_config(4, npix=48, ngrid3d=64), "cfg4 64^3 48px")
+
+
+def test_cfg5_reduced_batch(rt):
+    _parity_fwd_bwd(rt, make_config(5, npix=40, batch=3), "cfg5 b3 40px")
+
+
+def test_batch_larger_than_one_launch_chunk(rt):
+    scs = [tiny_axisym_scene(seed=50 + b, incl_deg=20.0 + 2 * b, npix=4) for b in range(19)]
+    # batch items must share the line and the grid geometry; only fields and viewing geometry differ
+    _parity_fwd_bwd(rt, scs, "batch19")
+
+
+# ------------------------------------------------------------------ full sizes, sampled rays
+def _sampled_full(rt, scenes, name, nsample=96, seed=5):
+    """Render the FULL config on the GPU in the launch configuration bench.py times; the oracle computes a
+    seeded sample of rays one by one.  The adjoint gets dL/dcube non-zero only on those rays."""
+    scenes = _as_list(scenes)
+    R = _gpu_forward(rt, scenes, need_bwd=True)
+    cube = R.cube.cpu().numpy()
+    rng = np.random.default_rng(seed)
+    d = R.desc
+    G = np.zeros(cube.shape, np.float32)
+    picks = []
+    for b, sc in enumerate(scenes):
+        # half of the sample where the cube is bright, half anywhere
+        flat = cube[b].reshape(-1, d.nchan)
+        bright = np.nonzero(flat.max(1) > 0.05 * flat.max())[0]
+        idx = np.unique(np.concatenate([rng.choice(bright, nsample // 2, replace=False),
+                                        rng.integers(0, flat.shape[0], nsample // 2)]))
+        ref = po.render(sc, rays=idx)
+        check_cube(f"{name}[{b}] sampled cube", flat[idx], ref)
+        g = (rng.standard_normal(ref.shape) * ref.max() * 1e-6).astype(np.float32)
+        G[b].reshape(-1, d.nchan)[idx] = g
+        picks.append((idx, g))
+    R.dl_dcube.copy_(torch.from_numpy(G))
+    gd, gt, gv = (g.cpu().numpy() for g in R.render_bwd())
+    for b, sc in enumerate(scenes):
+        idx, g = picks[b]
+        rd, rtm, rv = po.render_bwd(sc, g.astype(np.float64), rays=idx)
+        check_grad(f"{name}[{b}] g_dens", gd[b], rd)
+        check_grad(f"{name}[{b}] g_temp", gt[b], rtm)
+        check_grad(f"{name}[{b}] g_vel", gv[b], rv)
+    return R, cube
+
+
+def test_cfg3_full_sampled(rt):
+    R, cube = _sampled_full(rt, make_config(3), "cfg3 full")
+    assert cube.shape == (1, 512, 512, 128)
+    assert np.all(cube >= 0.0) and np.all(np.isfinite(cube))
+
+
+def test_cfg4_full_sampled(rt):
+    R, cube = _sampled_full(rt, make_config(4), "cfg4 full", nsample=64)
+    assert cube.shape == (1, 512, 512, 64)
+
+
+def test_cfg5_full_sampled(rt):
+    scs = make_config(5)
+    R = _gpu_forward(rt, scs, need_bwd=True)
+    cube = R.cube.cpu().numpy()
+    assert cube.shape == (16, 512, 512, 128)
+    rng = np.random.default_rng(9)
+    G = torch.zeros_like(R.dl_dcube)
+    refs = {}
+    for b in (0, 7, 15):
+        flat = cube[b].reshape(-1, 128)
+        bright = np.nonzero(flat.max(1) > 0.05 * flat.max())[0]
+        idx = np.unique(rng.choice(bright, 24, replace=False))
+        ref = po.render(scs[b], rays=idx)
+        check_cube(f"cfg5[{b}] sampled cube", flat[idx], ref)
+        g = (rng.standard_normal(ref.shape) * 1e-6).astype(np.float32)
+        G[b].view(-1, 128)[torch.from_numpy(idx).cuda()] = torch.from_numpy(g).cuda()
+        refs[b] = (idx, g)
+    R.dl_dcube.copy_(G)
+    gd, gt, gv = (g.cpu().numpy() for g in R.render_bwd())
+    for b in range(16):
+        if b in refs:
+            idx, g = refs[b]
+            rd, rtm, rv = po.render_bwd(scs[b], g.astype(np.float64), rays=idx)
+            check_grad(f"cfg5[{b}] g_dens", gd[b], rd)
+            check_grad(f"cfg5[{b}] g_temp", gt[b], rtm)
+            check_grad(f"cfg5[{b}] g_vel", gv[b], rv)
+        else:
+            assert not gd[b].any() and not gt[b].any() and not gv[b].any()    # batch items do not leak into each other
+
+
+# ------------------------------------------------------------------ properties that hold at any size
+def test_cfg2_full_symmetry_and_bounds(rt):
+    """Minor-axis mirror with velocity flip (SURVEY.md:290) on the full config-2 cube, and 0 <= I <= S(T_max)."""
+    sc = make_config(2)
+    R = _gpu_forward(rt, sc)
+    cube = R.cube.cpu().numpy()[0]
+    np.testing.assert_allclose(cube, cube[::-1, :, ::-1], rtol=2e-5, atol=2e-6 * cube.max())
+    tmax = float(sc.grid.temp.max())
+    smax = 1.0 / math.expm1(6.62607015e-27 * sc.line.nu0 / 1.380649e-16 / tmax)
+    assert cube.min() >= 0.0 and cube.max() <= smax * (1 + 1e-5)
+
+
+def test_forward_is_deterministic_and_adjoint_linear(rt):
+    sc = make_config(1)
+    R = _gpu_forward(rt, sc, need_bwd=True)
+    c1 = R.cube.clone()
+    R.render()
+    assert torch.equal(c1, R.cube)
+    g = torch.randn_like(R.cube) * 1e-5
+    R.dl_dcube.copy_(g)
+    a = [x.clone() for x in R.render_bwd()]
+    R.dl_dcube.copy_(-2.0 * g)
+    b = [x.clone() for x in R.render_bwd()]
+    for x, y in zip(a, b):
+        torch.testing.assert_close(y, -2.0 * x, rtol=1e-4, atol=1e-6 * float(x.abs().max()))
+
+
+def test_dense_and_skipping_kernels_agree(rt):
+    """Channel windowing and empty-step skipping change the cube by less than 1e-6 of its maximum."""
+    B = rt.binding
+    sc = make_config(2, npix=64)
+    R = rt.Renderer([sc])
+    try:
+        B.radt_set_option(B.OPT_WINDOW, 0); B.radt_set_option(B.OPT_SKIP_EMPTY, 0)
+        dense = R.render().clone()
+        cd = R.counters()
+    finally:
+        B.radt_set_option(B.OPT_WINDOW, 1); B.radt_set_option(B.OPT_SKIP_EMPTY, 1)
+    fast = R.render()
+    cf = R.counters()
+    assert float((dense - fast).abs().max()) <= 1e-6 * float(dense.max())
+    assert cf[0] < cd[0] and cf[1] < cd[1]
+    check_cube("dense cube", dense.cpu().numpy(), _oracle_cube(sc))
+
+
+# ------------------------------------------------------------------ edge cases
+def test_all_rays_miss(rt):
+    sc = tiny_axisym_scene(seed=60, npix=5)
+    sc = replace(sc, geom=replace(sc.geom, x0=5000.0))
+    R = _gpu_forward(rt, sc, need_bwd=True)
+    assert not R.cube.any()
+    R.dl_dcube.fill_(1.0)
+    for g in R.render_bwd():
+        assert not g.any()
+
+
+def test_zero_density_and_clamped_temperature(rt):
+    sc = slab_scene(n_co=0.0, temp=30.0, vchan_cms=[0.0, 0.02e5], nstep=5, npix=3)
+    R = _parity_fwd_bwd(rt, sc, "zero density")
+    assert not R.cube.any()
+    assert R.g_dens.abs().max() > 0          # dL/dn is finite and non-zero at n = 0
+    sc = slab_scene(n_co=0.5, temp=0.3, vchan_cms=[0.0], nstep=4, npix=2)
+    R = _parity_fwd_bwd(rt, sc, "T clamp")
+    assert not R.g_temp.any()
+
+
+def test_max_channels_and_odd_image(rt):
+    sc = tiny_axisym_scene(seed=61, nchan=256, npix=5, npix_y=3, nstep=40)
+    _parity_fwd_bwd(rt, sc, "256 channels")
+    sc = tiny_axisym_scene(seed=62, nchan=130, npix=7, nstep=33)
+    _parity_fwd_bwd(rt, sc, "130 channels")
+
+
+# ------------------------------------------------------------------ HOST-buffer entry points and the loss kernel
+def test_host_entry_points(rt):
+    B = rt.binding
+    sc = make_config(1)
+    d = B.Descriptors(sc)
+    h = B.stack_fields(sc)
+    cube = np.zeros(d.cube_shape, np.float32)
+    B.radt_render_host(d, *h, cube)
+    ref = _oracle_cube(sc)
+    check_cube("host cube", cube, ref)
+    tgt, sigma = l2_target(ref[0], 3)
+    tgt32 = np.ascontiguousarray(tgt[None], np.float32)
+    gd, gt, gv = (np.zeros_like(h[0]) for _ in range(3))
+    cube2 = np.zeros_like(cube)
+    loss = B.radt_fit_step_host(d, *h, tgt32, sigma, cube2, gd, gt, gv)
+    np.testing.assert_array_equal(cube, cube2)
+    res = cube.astype(np.float64) - tgt32
+    assert loss == pytest.approx(0.5 * np.mean((res / sigma) ** 2), rel=1e-6)
+    G = (res / (sigma ** 2 * res.size)).astype(np.float32)
+    rd, rtm, rv = po.render_bwd(sc, G[0].astype(np.float64))
+    check_grad("host g_dens", gd[0], rd); check_grad("host g_temp", gt[0], rtm); check_grad("host g_vel", gv[0], rv)
+    gd2, gt2, gv2 = (np.zeros_like(h[0]) for _ in range(3))
+    B.radt_render_bwd_host(d, *h, cube, G, gd2, gt2, gv2)
+    check_grad("host2 g_dens", gd2[0], rd); check_grad("host2 g_temp", gt2[0], rtm); check_grad("host2 g_vel", gv2[0], rv)
+
+
+def test_l2_loss_kernel(rt):
+    R = rt.Renderer([make_config(1)])
+    R.render()
+    cube = R.cube.cpu().numpy().astype(np.float64)
+    tgt, sigma = l2_target(cube[0], 4)
+    R.set_target(tgt[None], sigma)
+    loss = float(R.l2_loss_grad().cpu())
+    t32 = R.target.cpu().numpy().astype(np.float64)
+    assert loss == pytest.approx(0.5 * np.mean(((cube - t32) / sigma) ** 2), rel=1e-9)
+    np.testing.assert_allclose(R.dl_dcube.cpu().numpy(), (cube - t32) / (sigma ** 2 * cube.size), rtol=2e-6, atol=1e-12)
+
+
+def test_workspace_too_small_and_launch_count(rt):
+    B = rt.binding
+    sc = tiny_axisym_scene(seed=63)
+    R = rt.Renderer([sc])
+    small = torch.empty(64, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.RadtError, match="-3"):
+        B.radt_render(R.desc, R.dens, R.temp, R.vel, R.cube, small)
+    R.render()
+    assert B.radt_last_launch_count() == 2          # setup + march
+    R.dl_dcube.fill_(1e-6)
+    R.render_bwd()
+    assert B.radt_last_launch_count() == 3          # setup + adjoint march + unpack
+
+
+def test_pipe_peaks_are_sane(rt):
+    ops, clk = rt.binding.radt_pipe_peak(0)
+    assert 1000 < clk < 2200
+    per_sm_clk = ops / 148 / (clk * 1e6)
+    assert 14.0 < per_sm_clk < 16.5            # MUFU.EX2: 16 lanes / clk / SM
+    ops, clk = rt.binding.radt_pipe_peak(1)
+    assert 100.0 < ops / 148 / (clk * 1e6) < 130.0     # FFMA: 128 lanes / clk / SM
