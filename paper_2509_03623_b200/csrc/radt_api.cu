@@ -160,7 +160,7 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     size_t off = 0;
     size_t nrays = (size_t)geom[0].nx * geom[0].ny * (size_t)batch;
     w.counters = off; off = align256(off + 8 * sizeof(unsigned long long));
-    w.rays = off; off = align256(off + nrays * sizeof(double2));
+    w.rays = off; off = align256(off + nrays * sizeof(RayRec));
     w.qtab = off; off = align256(off + (RADT_NQ + 2) * sizeof(float2));
     w.vcs = off; off = align256(off + (size_t)batch * RADT_MAXCHAN * sizeof(float2));
     w.rnode = off; off = align256(off + (size_t)(grid->kind == RADT_GRID_AXISYM ? grid->n[0] : 1) * sizeof(double2));
@@ -177,7 +177,7 @@ DevWs make_dev_ws(void *ws, const WsLayout &w)
     char *base = (char *)ws;
     DevWs d;
     d.counters = (unsigned long long *)(base + w.counters);
-    d.rays = (double2 *)(base + w.rays);
+    d.rays = (RayRec *)(base + w.rays);
     d.qtab = (float2 *)(base + w.qtab);
     d.vcs = (float2 *)(base + w.vcs);
     d.rnode = (double2 *)(base + w.rnode);
@@ -310,7 +310,7 @@ int radt_ray_geometry(const radt_geom *geom, const radt_grid *grid, int32_t batc
         memset(&SP, 0, sizeof(SP));
         for (int b = 0; b < nb; ++b) make_dev_geom(geom[b0 + b], nullptr, SP.geom[b]);
         SP.grid = dg;
-        SP.ws.rays = (double2 *)rays_out;
+        SP.rays_user = (double2 *)rays_out;
         SP.nx = geom[0].nx; SP.ny = geom[0].ny; SP.nstep = geom[0].nstep; SP.nbatch = nb; SP.b0 = b0;
         SP.do_rays = 1;
         CUDA_TRY(radt_launch_setup(SP, LT, CT, (cudaStream_t)cuda_stream));

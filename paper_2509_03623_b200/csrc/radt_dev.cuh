@@ -56,9 +56,16 @@ struct DevLine {
     int ngroups;       // ceil(nchan / 32)
 };
 
+// K1 output per ray: clipped interval and the conservative range of steps that can lie inside the grid
+struct __align__(16) RayRec {
+    double s0, ds;         // au; ds = 0 marks a ray that misses the volume
+    int k_lo, k_hi;        // in-grid samples have k_lo <= k < k_hi
+    int pad0, pad1;
+};
+
 // Workspace layout (all offsets in bytes from the workspace base, 256-byte aligned)
 struct DevWs {
-    double2 *rays;         // [batch*ny*nx] {s0, ds}
+    RayRec *rays;          // [batch*ny*nx]
     float2 *qtab;          // [RADT_NQ + 2] {Q, dQ/dlnT}
     float2 *vcs;           // [batch][RADT_MAXCHAN] channel velocity minus v_sys, cm/s, as (hi, lo) float pair
     double2 *rnode;        // [nr] {r_i, 1/r_i} node radii of the log-spaced axis (axisym), fp64
@@ -90,6 +97,7 @@ struct SetupParams {
     int do_rays, do_tables, do_pack, do_zero_grad;
     long long batch_stride;
     const float *dens, *temp, *vel;
+    double2 *rays_user;    // radt_ray_geometry output {s0, ds} (may be null)
     double vsys[RADT_MAXB];
 };
 

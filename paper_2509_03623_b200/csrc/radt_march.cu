@@ -12,6 +12,7 @@
 #define FULL 0xffffffffu
 #define UWIN 7.75f          // |u'| cut (u' = u sqrt(log2 e)): exp(-u^2) < 2^-60 beyond it
 #define K2_EMPTY 1e-20f     // line-centre dtau*log2e below this adds < 1e-20 S per step: treated as vacuum
+#define N_EMPTY 1e-17f      // density below which a sample is empty (K2 < 1e-19 for any realistic line)
 
 struct StepState {
     bool inside;
@@ -25,7 +26,7 @@ struct StepState {
 
 __device__ __forceinline__ float lerp1(float a, float b, float f) { return fmaf(f, b - a, a); }
 
-template <int KIND>
+template <int KIND, bool FWD>
 __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, const float4 *__restrict__ cells,
                                         double ox, double oy, double oz, double s0, double ds, int k, StepState &st)
 {
@@ -125,9 +126,12 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
         vel = (float)vel_d;
         st.f0 = fx; st.f1 = fy; st.f2 = fz; st.cell = cell;
     }
-    st.inside = true;
     // ---- O7: channel-independent LTE quantities (Eq. 13-17) ----
     float n = (g.dens_mode == 1) ? ex2_approx(dens * RADT_LOG2E) : dens;
+    // empty samples: no opacity, hence no contribution to the cube; their only gradient is dL/dn, which exists
+    // when the grid stores n itself (LINEAR) and vanishes with n when it stores ln n
+    if ((FWD || g.dens_mode == 1) && P.opt_skip_empty && !(n > N_EMPTY)) return;
+    st.inside = true;
     bool tcl = !(temp >= 1.0f);
     float T = tcl ? 1.0f : temp;
     float invT = rcp_approx(T);
@@ -178,18 +182,64 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     st.qy = lerp1(q0.y, q1.y, fq) * iQ;      // dlnQ/dlnT
 }
 
-// 1 - 2^(-d) with full relative accuracy for small d (series on the FMA pipe), d >= 0
-__device__ __forceinline__ float one_minus_exp2neg(float d, float e)
+
+// ---------------------------------------------------------------------------------------------
+// packed f32x2 arithmetic (sm_100: FADD2 / FMUL2 / FFMA2 issue one slot for two lanes' worth of work)
+// ---------------------------------------------------------------------------------------------
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f2 pk1(float v) { return pk(v, v); }
+__device__ __forceinline__ void upk(f2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { f2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
+#define C_LN2 0.6931471805599453f
+#define C_LN2SQ_2 0.2402265069591007f
+#define C_LN2CU_6 0.05550410866482158f
+#define D_SERIES 0.015625f   // below this 1 - 2^-d comes from the series (else cancellation breaks 1e-4 in thin wings)
+
+// One (step, channel pair) sample of O8-O9 in log2 units.  q = {v_hi, A, -v_lo A, K'}; outputs u, g, d, e, 1-e.
+struct Pair {
+    f2 u, g, d, e, om;
+};
+template <bool CL>
+__device__ __forceinline__ f2 pair_u(f2 vcs, f2 vcl, const float4 &q)
 {
-    const float c1 = RADT_LN2, c2 = 0.5f * RADT_LN2 * RADT_LN2, c3 = RADT_LN2 * RADT_LN2 * RADT_LN2 / 6.0f;
-    float small = d * fmaf(d, fmaf(d, c3, -c2), c1);
-    return (d < 0.015625f) ? small : 1.0f - e;
+    f2 u = fma2(sub2(vcs, pk1(q.x)), pk1(q.y), pk1(q.z));      // exact difference of the hi parts
+    if (CL) u = fma2(vcl, pk1(q.y), u);
+    return u;
+}
+__device__ __forceinline__ void pair_eval(f2 u, float K2, Pair &s)
+{
+    s.u = u;
+    float t0, t1;
+    upk(mul2(u, u), t0, t1);
+    s.g = pk(ex2_approx(-t0), ex2_approx(-t1));
+    s.d = mul2(s.g, pk1(K2));
+    float d0, d1;
+    upk(s.d, d0, d1);
+    s.e = pk(ex2_approx(-d0), ex2_approx(-d1));
+    f2 sm = mul2(s.d, fma2(s.d, fma2(s.d, pk1(C_LN2CU_6), pk1(-C_LN2SQ_2)), pk1(C_LN2)));
+    f2 bg = fma2(s.e, pk1(-1.0f), pk1(1.0f));
+    float s0, s1, b0, b1;
+    upk(sm, s0, s1);
+    upk(bg, b0, b1);
+    s.om = pk(d0 < D_SERIES ? s0 : b0, d1 < D_SERIES ? s1 : b1);
+}
+__device__ __forceinline__ bool pair_in_window(f2 u)
+{
+    float u0, u1;
+    upk(u, u0, u1);
+    return fabsf(u0) < UWIN || fabsf(u1) < UWIN;
 }
 
 struct RayCtx {
     int ix, iy, b;
     size_t ray;
     double s0, ds, ox, oy, oz;
+    int k_lo, k_hi;
 };
 
 __device__ __forceinline__ bool ray_setup(const MarchParams &P, RayCtx &rc, int warp)
@@ -200,17 +250,17 @@ __device__ __forceinline__ bool ray_setup(const MarchParams &P, RayCtx &rc, int 
     rc.iy = ty * RADT_TILE_Y + (warp / RADT_TILE_X);
     if (rc.ix >= P.nx || rc.iy >= P.ny) return false;
     rc.ray = ((size_t)(P.b0 + rc.b) * P.ny + rc.iy) * P.nx + rc.ix;
-    double2 sd = P.ws.rays[rc.ray];
-    rc.s0 = sd.x; rc.ds = sd.y;
+    RayRec rr = P.ws.rays[rc.ray];
+    rc.s0 = rr.s0; rc.ds = rr.ds; rc.k_lo = rr.k_lo; rc.k_hi = rr.k_hi;
     double X, Y;
     pixel_origin(P.geom[rc.b], P.nx, P.ny, rc.ix, rc.iy, rc.ox, rc.oy, rc.oz, X, Y);
     return true;
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2 / K3 forward march
+// K2 / K3 forward march.  NP = channel-group pairs per lane: lane owns channels lane + 32 g, g < 2 NP.
 // ---------------------------------------------------------------------------------------------
-template <int KIND, int NG, bool CL>
+template <int KIND, int NP, bool CL>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __grid_constant__ MarchParams P)
 {
     __shared__ float4 sh_p[RADT_WARPS_PER_CTA][32];
@@ -221,69 +271,73 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
     const DevGeom &G = P.geom[rc.b];
     const int nchan = P.line.nchan;
     float *out = P.cube + rc.ray * (size_t)nchan;
-    float I[NG], T[NG], vcs[NG], vcl[NG];
+    f2 I[NP], T[NP], vcs[NP], vcl[NP];
     const float2 *vtab = P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN;
 #pragma unroll
-    for (int g = 0; g < NG; ++g) {
-        int c = lane + 32 * g;
-        I[g] = 0.f; T[g] = 1.f;
-        float2 vv = (c < nchan) ? __ldg(vtab + c) : make_float2(0.f, 0.f);
-        vcs[g] = vv.x; vcl[g] = vv.y;
+    for (int p = 0; p < NP; ++p) {
+        int c0 = lane + 64 * p, c1 = c0 + 32;
+        float2 v0 = (c0 < nchan) ? __ldg(vtab + c0) : make_float2(0.f, 0.f);
+        float2 v1 = (c1 < nchan) ? __ldg(vtab + c1) : make_float2(0.f, 0.f);
+        I[p] = pk(0.f, 0.f); T[p] = pk(1.f, 1.f);
+        vcs[p] = pk(v0.x, v1.x); vcl[p] = pk(v0.y, v1.y);
     }
-    unsigned long long n_steps = 0, n_groups = 0;
+    unsigned n_steps = 0, n_pairs = 0;
     if (rc.ds != 0.0) {
         const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
-        for (int kb = 0; kb < P.nstep; kb += 32) {
+        // only the 32-step blocks that can hold in-grid samples (K1's conservative step range)
+        for (int kb = rc.k_lo & ~31; kb < rc.k_hi; kb += 32) {
             StepState st;
-            phase_a<KIND>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, kb + lane, st);
+            phase_a<KIND, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, kb + lane, st);
             bool active = st.inside && (st.K2 > K2_EMPTY || !P.opt_skip_empty);
             unsigned mask = __ballot_sync(FULL, active);
             if (mask == 0u) continue;
-            sh_p[warp][lane] = make_float4(st.vh, st.A, st.mvlA, st.K2);
-            sh_s[warp][lane] = st.S;
+            // compact the active steps (in march order) so that phase B is a plain counted loop
+            if (active) {
+                int pos = __popc(mask & ((1u << lane) - 1u));
+                sh_p[warp][pos] = make_float4(st.vh, st.A, st.mvlA, st.K2);
+                sh_s[warp][pos] = st.S;
+            }
             __syncwarp();
-            n_steps += __popc(mask);
-            while (mask) {
-                int j = __ffs(mask) - 1;
-                mask &= mask - 1;
+            const int cnt = __popc(mask);
+            n_steps += cnt;
+            for (int j = 0; j < cnt; ++j) {
                 float4 q = sh_p[warp][j];
-                float S = sh_s[warp][j];
+                f2 S2 = pk1(sh_s[warp][j]);
 #pragma unroll
-                for (int g = 0; g < NG; ++g) {
-                    float u = fmaf(vcs[g] - q.x, q.y, q.z);      // exact difference of the hi parts
-                    if (CL) u = fmaf(vcl[g], q.y, u);
-                    if (P.opt_window && !__any_sync(FULL, fabsf(u) < UWIN)) continue;
-                    ++n_groups;
-                    float gph = ex2_approx(-u * u);
-                    float d = q.w * gph;
-                    float e = ex2_approx(-d);
-                    float om = one_minus_exp2neg(d, e);
-                    // contribution and partial sum are formed without FMA contraction so that the adjoint
-                    // re-march reproduces the forward's partial sums bit for bit
-                    I[g] = __fadd_rn(I[g], __fmul_rn(S, __fmul_rn(om, T[g])));
-                    T[g] *= e;
+                for (int p = 0; p < NP; ++p) {
+                    f2 u = pair_u<CL>(vcs[p], vcl[p], q);
+                    if (P.opt_window && !__any_sync(FULL, pair_in_window(u))) continue;
+                    ++n_pairs;
+                    Pair s;
+                    pair_eval(u, q.w, s);
+                    // contribution c = S ((1-e) T) and partial sum I += c as ONE explicit FMA: the adjoint
+                    // re-march repeats exactly this sequence and so reproduces the partial sums bit for bit
+                    I[p] = fma2(S2, mul2(s.om, T[p]), I[p]);
+                    T[p] = mul2(T[p], s.e);
                 }
             }
             __syncwarp();
         }
     }
 #pragma unroll
-    for (int g = 0; g < NG; ++g) {
-        int c = lane + 32 * g;
-        if (c < nchan) out[c] = I[g];
+    for (int p = 0; p < NP; ++p) {
+        int c0 = lane + 64 * p, c1 = c0 + 32;
+        float i0, i1;
+        upk(I[p], i0, i1);
+        if (c0 < nchan) out[c0] = i0;
+        if (c1 < nchan) out[c1] = i1;
     }
     if (lane == 0 && n_steps) {
-        atomicAdd(P.ws.counters + 0, n_steps);
-        atomicAdd(P.ws.counters + 1, n_groups);
+        atomicAdd(P.ws.counters + 0, (unsigned long long)n_steps);
+        atomicAdd(P.ws.counters + 1, (unsigned long long)n_pairs * 2ull);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// K4 / K5 adjoint march: front-to-back re-march with the saved cube (DESIGN.md "Adjoint")
-//   dL/d dtau_k,c = G_c (T_{k+1,c} S_k - (I_c - I_{<=k,c}))      dL/dS_k = sum_c G_c (1-e_k,c) T_k,c
+// K4 / K5 adjoint march: front-to-back re-march with the saved cube (DESIGN.md section 5)
+//   dL/d dtau_k,c = G_c (T_{k+1,c} S_k - R_k,c),  R_k = I - I_{<=k}        dL/dS_k = sum_c G_c (1-e_k,c) T_k,c
 // ---------------------------------------------------------------------------------------------
-// Gradient cells are accumulated in fp64: a cell sums ~1e3 signed contributions from many rays and the
-// velocity gradient cancels to ~1e-2 of its gross sum, which fp32 atomics cannot resolve to 1e-3.
+// Gradient cells are accumulated in fp64 (packed {dens, temp, vel, -}); unpacked to fp32 by k_unpack_grad.
 __device__ __forceinline__ void red_add_cell(double *cell, float w, float a, float b, float c)
 {
     double wd = (double)w;
@@ -292,7 +346,7 @@ __device__ __forceinline__ void red_add_cell(double *cell, float w, float a, flo
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(cell + 2), "d"(wd * (double)c) : "memory");
 }
 
-template <int KIND, int NG, bool CL>
+template <int KIND, int NP, bool CL>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __grid_constant__ MarchParams P)
 {
     __shared__ float4 sh_p[RADT_WARPS_PER_CTA][32];
@@ -307,19 +361,21 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __g
     const int nchan = L.nchan;
     const float *Isave = P.cube + rc.ray * (size_t)nchan;
     const float *Gin = P.dl_dcube + rc.ray * (size_t)nchan;
-    float R[NG], Pp[NG], T[NG], vcs[NG], vcl[NG], Gc[NG];   // R holds the saved intensity I
+    f2 Isv[NP], Pp[NP], T[NP], vcs[NP], vcl[NP], Gc[NP];
     const float2 *vtab = P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN;
     bool anyg = false;
 #pragma unroll
-    for (int g = 0; g < NG; ++g) {
-        int c = lane + 32 * g;
-        bool ok = c < nchan;
-        T[g] = 1.f; Pp[g] = 0.f;
-        float2 vv = ok ? __ldg(vtab + c) : make_float2(0.f, 0.f);
-        vcs[g] = vv.x; vcl[g] = vv.y;
-        R[g] = ok ? __ldg(Isave + c) : 0.f;
-        Gc[g] = ok ? __ldg(Gin + c) : 0.f;
-        anyg |= (Gc[g] != 0.f);
+    for (int p = 0; p < NP; ++p) {
+        int c0 = lane + 64 * p, c1 = c0 + 32;
+        bool ok0 = c0 < nchan, ok1 = c1 < nchan;
+        float2 v0 = ok0 ? __ldg(vtab + c0) : make_float2(0.f, 0.f);
+        float2 v1 = ok1 ? __ldg(vtab + c1) : make_float2(0.f, 0.f);
+        float g0 = ok0 ? __ldg(Gin + c0) : 0.f, g1 = ok1 ? __ldg(Gin + c1) : 0.f;
+        T[p] = pk(1.f, 1.f); Pp[p] = pk(0.f, 0.f);
+        vcs[p] = pk(v0.x, v1.x); vcl[p] = pk(v0.y, v1.y);
+        Isv[p] = pk(ok0 ? __ldg(Isave + c0) : 0.f, ok1 ? __ldg(Isave + c1) : 0.f);
+        Gc[p] = pk(g0, g1);
+        anyg |= (g0 != 0.f) || (g1 != 0.f);
     }
     if (!__any_sync(FULL, anyg)) return;     // dL/dcube vanishes on this ray: no gradient
     const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
@@ -328,52 +384,57 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __g
     // upper bound of the source function anywhere on the grid (S grows with T)
     const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + 4)), 1.0f);
     const float smax = G.sunit * 1.0001f / (ex2_approx(L.T0l2 / tmax) - 1.0f);
-    unsigned long long n_steps = 0, n_groups = 0;
-    for (int kb = 0; kb < P.nstep; kb += 32) {
+    unsigned n_steps = 0, n_pairs = 0;
+    for (int kb = rc.k_lo & ~31; kb < rc.k_hi; kb += 32) {
         StepState st;
-        phase_a<KIND>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, kb + lane, st);
-        // zero-density steps still carry dL/dn when the grid stores n itself (LINEAR); with ln n they carry nothing
+        phase_a<KIND, false>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, kb + lane, st);
+        // zero-density steps still carry dL/dn when the grid stores n itself (LINEAR)
         bool active = st.inside && (st.K2 > K2_EMPTY || P.grid.dens_mode == 0 || !P.opt_skip_empty);
         unsigned mask = __ballot_sync(FULL, active);
         if (mask == 0u) continue;
-        sh_p[warp][lane] = make_float4(st.vh, st.A, st.mvlA, st.K2);
-        sh_s[warp][lane] = st.S;
+        const int pos = __popc(mask & ((1u << lane) - 1u));
+        if (active) {
+            sh_p[warp][pos] = make_float4(st.vh, st.A, st.mvlA, st.K2);
+            sh_s[warp][pos] = st.S;
+        }
         __syncwarp();
-        n_steps += __popc(mask);
-        while (mask) {
-            int j = __ffs(mask) - 1;
-            mask &= mask - 1;
+        const int cnt = __popc(mask);
+        n_steps += cnt;
+        for (int j = 0; j < cnt; ++j) {
             float4 q = sh_p[warp][j];
             float S = sh_s[warp][j];
-            float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+            f2 S2 = pk1(S);
+            f2 p0 = pk(0.f, 0.f), p1 = p0, p2 = p0, p3 = p0;
 #pragma unroll
-            for (int g = 0; g < NG; ++g) {
-                float u = fmaf(vcs[g] - q.x, q.y, q.z);
-                if (CL) u = fmaf(vcl[g], q.y, u);
-                if (P.opt_window && !__any_sync(FULL, fabsf(u) < UWIN)) continue;
-                ++n_groups;
-                float gph = ex2_approx(-u * u);
-                float d = q.w * gph;
-                float e = ex2_approx(-d);
-                float om = one_minus_exp2neg(d, e);
-                float Tg = T[g];
-                float Tn = Tg * e;
-                // P = forward partial sum I_{<=k}, reproduced bit for bit; remainder R = I - P = T_{k+1} B_{k+1}.
-                // The truth lies in [0, T_{k+1} S_max]: clamping there makes the rounding error of the
-                // subtraction decay with the transmittance.
-                Pp[g] = __fadd_rn(Pp[g], __fmul_rn(S, __fmul_rn(om, Tg)));
-                float Rn = fminf(fmaxf(R[g] - Pp[g], 0.f), Tn * smax);
-                float a = Gc[g] * fmaf(Tn, S, -Rn);
-                float du = d * u;
-                p0 = fmaf(a, gph, p0);
-                p1 = fmaf(a, du, p1);
-                p2 = fmaf(a * du, u, p2);
-                p3 = fmaf(Gc[g] * om, Tg, p3);
-                T[g] = Tn;
+            for (int p = 0; p < NP; ++p) {
+                f2 u = pair_u<CL>(vcs[p], vcl[p], q);
+                if (P.opt_window && !__any_sync(FULL, pair_in_window(u))) continue;
+                ++n_pairs;
+                Pair s;
+                pair_eval(u, q.w, s);
+                f2 omT = mul2(s.om, T[p]);
+                Pp[p] = fma2(S2, omT, Pp[p]);                 // = the forward's partial sum I_{<=k}, bit for bit
+                f2 Tn = mul2(T[p], s.e);
+                // -R = P - I_saved, R = T_{k+1} B_{k+1}: the truth lies in [0, T_{k+1} S_max]; clamping there makes
+                // the rounding error of the subtraction decay with the transmittance
+                float r0, r1, b0, b1;
+                upk(sub2(Pp[p], Isv[p]), r0, r1);
+                upk(mul2(Tn, pk1(-smax)), b0, b1);
+                f2 nR = pk(fminf(fmaxf(r0, b0), 0.f), fminf(fmaxf(r1, b1), 0.f));
+                f2 a = mul2(Gc[p], fma2(Tn, S2, nR));
+                f2 du = mul2(s.d, s.u);
+                p0 = fma2(a, s.g, p0);
+                p1 = fma2(a, du, p1);
+                p2 = fma2(mul2(a, du), s.u, p2);
+                p3 = fma2(Gc[p], omT, p3);
+                T[p] = Tn;
             }
+            float a0, a1, b0, b1, c0, c1, d0, d1;
+            upk(p0, a0, a1); upk(p1, b0, b1); upk(p2, c0, c1); upk(p3, d0, d1);
+            float q0 = a0 + a1, q1 = b0 + b1, q2 = c0 + c1, q3 = d0 + d1;
             // transposed butterfly: 4 sums over 32 lanes in 6 shuffles
-            float s0 = h16 ? p0 : p2, s1 = h16 ? p1 : p3;
-            float k0 = h16 ? p2 : p0, k1 = h16 ? p3 : p1;
+            float s0 = h16 ? q0 : q2, s1 = h16 ? q1 : q3;
+            float k0 = h16 ? q2 : q0, k1 = h16 ? q3 : q1;
             k0 += __shfl_xor_sync(FULL, s0, 16);
             k1 += __shfl_xor_sync(FULL, s1, 16);
             float sv = h8 ? k0 : k1;
@@ -387,7 +448,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __g
         __syncwarp();
         // ---- phase C: chain rule to (n, T, v_phi) at this lane's step, scatter to the grid (O11) ----
         if (active) {
-            float4 sm = sh_sum[warp][lane];
+            float4 sm = sh_sum[warp][pos];
             const float iL2 = RADT_LN2;                       // 1 / log2(e)
             float A0 = sm.x;
             float A1 = sm.y * (iL2 / RADT_SQRT_LOG2E);
@@ -430,44 +491,42 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __g
         __syncwarp();
     }
     if (lane == 0 && n_steps) {
-        atomicAdd(P.ws.counters + 2, n_steps);
-        atomicAdd(P.ws.counters + 3, n_groups);
+        atomicAdd(P.ws.counters + 2, (unsigned long long)n_steps);
+        atomicAdd(P.ws.counters + 3, (unsigned long long)n_pairs * 2ull);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
-template <int KIND, int NG>
+template <int KIND, int NP>
 static cudaError_t launch_fwd_t(const MarchParams &P, int nbatch, cudaStream_t st)
 {
     dim3 grid(P.tiles_x * P.tiles_y, nbatch);
-    if (P.chan_lo) k_march_fwd<KIND, NG, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
-    else k_march_fwd<KIND, NG, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    if (P.chan_lo) k_march_fwd<KIND, NP, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else k_march_fwd<KIND, NP, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
     return cudaGetLastError();
 }
 
-template <int KIND, int NG>
+template <int KIND, int NP>
 static cudaError_t launch_bwd_t(const MarchParams &P, int nbatch, cudaStream_t st)
 {
     dim3 grid(P.tiles_x * P.tiles_y, nbatch);
-    if (P.chan_lo) k_march_bwd<KIND, NG, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
-    else k_march_bwd<KIND, NG, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    if (P.chan_lo) k_march_bwd<KIND, NP, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else k_march_bwd<KIND, NP, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
     return cudaGetLastError();
 }
 
 #define RADT_DISPATCH(fn)                                                        \
-    int ng = P.line.ngroups;                                                     \
+    int np = (P.line.ngroups + 1) / 2;                                           \
     if (P.grid.kind == 0) {                                                      \
-        if (ng <= 1) return fn<0, 1>(P, nbatch, st);                             \
-        if (ng <= 2) return fn<0, 2>(P, nbatch, st);                             \
-        if (ng <= 4) return fn<0, 4>(P, nbatch, st);                             \
-        return fn<0, 8>(P, nbatch, st);                                          \
+        if (np <= 1) return fn<0, 1>(P, nbatch, st);                             \
+        if (np <= 2) return fn<0, 2>(P, nbatch, st);                             \
+        return fn<0, 4>(P, nbatch, st);                                          \
     }                                                                            \
-    if (ng <= 1) return fn<1, 1>(P, nbatch, st);                                 \
-    if (ng <= 2) return fn<1, 2>(P, nbatch, st);                                 \
-    if (ng <= 4) return fn<1, 4>(P, nbatch, st);                                 \
-    return fn<1, 8>(P, nbatch, st);
+    if (np <= 1) return fn<1, 1>(P, nbatch, st);                                 \
+    if (np <= 2) return fn<1, 2>(P, nbatch, st);                                 \
+    return fn<1, 4>(P, nbatch, st);
 
 cudaError_t radt_launch_march_fwd(const MarchParams &P, int nbatch, cudaStream_t st) { RADT_DISPATCH(launch_fwd_t) }
 cudaError_t radt_launch_march_bwd(const MarchParams &P, int nbatch, cudaStream_t st) { RADT_DISPATCH(launch_bwd_t) }

@@ -6,16 +6,48 @@
 // ---------------------------------------------------------------------------------------------
 // K1 ray geometry (O1-O3): per pixel the clipped interval {s0, ds}; ds = 0 marks a miss.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double2 clip_ray(const DevGeom &G, const DevGrid &g, int nx, int ny, int nstep, int ix, int iy)
+__device__ __forceinline__ RayRec clip_ray(const DevGeom &G, const DevGrid &g, int nx, int ny, int nstep, int ix, int iy)
 {
     double ox, oy, oz, X, Y;
     pixel_origin(G, nx, ny, ix, iy, ox, oy, oz, X, Y);
+    RayRec rr;
+    rr.s0 = 0.0; rr.ds = 0.0; rr.k_lo = 0; rr.k_hi = 0; rr.pad0 = 0; rr.pad1 = 0;
     if (g.kind == 0) {
         // s = 0 is the closest approach to the star, |p(s)|^2 = b^2 + s^2
         double b2 = X * X + Y * Y;
-        if (!(b2 < g.rb2)) return make_double2(0.0, 0.0);
+        if (!(b2 < g.rb2)) return rr;
         double sh = sqrt(g.rb2 - b2);
-        return make_double2(-sh, 2.0 * sh / (double)nstep);
+        rr.s0 = -sh;
+        rr.ds = 2.0 * sh / (double)nstep;
+        // Conservative s-interval that contains every in-grid sample: inside the cylinder r <= r_max and, for a
+        // wedge symmetric about the midplane seen from outside its opening angle, between the two cones
+        // |z| <= zeta_hi r.  Each is a quadratic inequality in s.  One step of slack on both sides.
+        double sa = rr.s0, sb = -rr.s0;
+        double a = G.wx * G.wx + G.wy * G.wy, bq = ox * G.wx + oy * G.wy, c = ox * ox + oy * oy;
+        bool empty = false;
+        if (a > 1e-14) {
+            double disc = bq * bq - a * (c - g.rmax2);
+            if (disc < 0.0) empty = true;
+            else { double sq = sqrt(disc); sa = fmax(sa, (-bq - sq) / a); sb = fmin(sb, (-bq + sq) / a); }
+        } else if (c > g.rmax2) {
+            empty = true;
+        }
+        bool wedge = (g.mirror && g.zlo == 0.0) || (!g.mirror && g.zlo == -g.zhi);
+        if (wedge && !empty) {
+            double z2 = g.zhi * g.zhi;
+            double A = G.wz * G.wz - z2 * a, B = oz * G.wz - z2 * bq, C = oz * oz - z2 * c;   // A s^2 + 2 B s + C <= 0
+            if (A > 1e-12) {
+                double disc = B * B - A * C;
+                if (disc < 0.0) empty = true;
+                else { double sq = sqrt(disc); sa = fmax(sa, (-B - sq) / A); sb = fmin(sb, (-B + sq) / A); }
+            }
+        }
+        if (!empty && sb >= sa) {
+            double klo = floor((sa - rr.s0) / rr.ds - 0.5) - 1.0, khi = ceil((sb - rr.s0) / rr.ds - 0.5) + 2.0;
+            rr.k_lo = (int)fmin(fmax(klo, 0.0), (double)nstep);
+            rr.k_hi = (int)fmin(fmax(khi, 0.0), (double)nstep);
+        }
+        return rr;
     }
     const double o[3] = { ox, oy, oz }, d[3] = { G.wx, G.wy, G.wz };
     double tmin = -INFINITY, tmax = INFINITY;
@@ -26,11 +58,14 @@ __device__ __forceinline__ double2 clip_ray(const DevGeom &G, const DevGrid &g, 
             tmin = fmax(tmin, fmin(t1, t2));
             tmax = fmin(tmax, fmax(t1, t2));
         } else if (o[a] < g.lo[a] || o[a] > g.hi[a]) {
-            return make_double2(0.0, 0.0);
+            return rr;
         }
     }
-    if (!(tmax > tmin)) return make_double2(0.0, 0.0);
-    return make_double2(tmin, (tmax - tmin) / (double)nstep);
+    if (!(tmax > tmin)) return rr;
+    rr.s0 = tmin;
+    rr.ds = (tmax - tmin) / (double)nstep;
+    rr.k_lo = 0; rr.k_hi = nstep;
+    return rr;
 }
 
 // Block roles: [0, nb_rays) rays; [nb_rays, nb_rays + nb_tab) tables; the rest pack fields.
@@ -45,7 +80,10 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
         int b = (int)(q / per_item);
         long long rem = q - (long long)b * per_item;
         int iy = (int)(rem / P.nx), ix = (int)(rem - (long long)iy * P.nx);
-        P.ws.rays[(long long)(P.b0 + b) * per_item + rem] = clip_ray(P.geom[b], P.grid, P.nx, P.ny, P.nstep, ix, iy);
+        RayRec rr = clip_ray(P.geom[b], P.grid, P.nx, P.ny, P.nstep, ix, iy);
+        long long dst = (long long)(P.b0 + b) * per_item + rem;
+        if (P.ws.rays) P.ws.rays[dst] = rr;
+        if (P.rays_user) P.rays_user[dst] = make_double2(rr.s0, rr.ds);
         return;
     }
     blk -= nb_rays;
