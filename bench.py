@@ -253,8 +253,8 @@ def run_ours(args):
     t_l2 = time_kernel_group(lambda: R.l2_loss_grad(stream), stream, torch, flush, reps)
     t_bwd = time_kernel_group(lambda: R.render_bwd(stream=stream), stream, torch, flush, reps)
     cnt_b = R.counters()
-    fwd_exec = cnt[1] * 32
-    bwd_exec = cnt_b[3] * 32
+    fwd_exec = cnt[1] * 32 // 2        # executed samples, 2 MUFU.EX2 lane-ops each
+    bwd_exec = cnt_b[3] * 32 // 2      # 2-EX2 equivalents (zero-opacity adjoint samples need one EX2: counted as 1/2)
 
     # ---- roofline: SFU (MUFU.EX2) issue peak measured now, at the clock the GPU runs at
     mufu_peak, mufu_clk = B.radt_pipe_peak(0)

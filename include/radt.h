@@ -173,8 +173,9 @@ int radt_render_bwd_host(const radt_geom *geom, const radt_line *line, const rad
 int radt_pipe_peak(int32_t kind, double *ops_per_s_out, double *sm_clock_mhz_out);
 
 /* Work counters of the last render / adjoint that used workspace `ws` (DEVICE): copies 4 uint64 to
- * out4 (HOST): {forward active ray-steps, forward executed 32-channel groups, adjoint active ray-steps,
- * adjoint executed groups}.  Synchronises cuda_stream. */
+ * out4 (HOST): {forward active ray-steps, forward per-sample MUFU.EX2 warp instructions (x32 = transcendental
+ * lane-operations spent on (channel, step) samples), adjoint active ray-steps, adjoint per-sample MUFU.EX2 warp
+ * instructions}.  Synchronises cuda_stream. */
 int radt_read_counters(const void *ws, uint64_t *out4, void *cuda_stream);
 
 /* Counters of the last radt_render / radt_render_bwd call on this thread (HOST): number of kernel

@@ -167,7 +167,7 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     size_t cells = (size_t)grid_cells(grid) * (size_t)batch;
     w.cells = off; off = align256(off + cells * sizeof(float4));
     w.grad = off;
-    if (pass == RADT_PASS_BWD) off = align256(off + cells * 4 * sizeof(double));
+    if (pass == RADT_PASS_BWD) off = align256(off + cells * sizeof(float4));
     w.total = off;
     return w;
 }
@@ -182,7 +182,7 @@ DevWs make_dev_ws(void *ws, const WsLayout &w)
     d.vcs = (float2 *)(base + w.vcs);
     d.rnode = (double2 *)(base + w.rnode);
     d.cells = (float4 *)(base + w.cells);
-    d.grad = (double *)(base + w.grad);
+    d.grad = (float4 *)(base + w.grad);
     return d;
 }
 

@@ -70,7 +70,7 @@ struct DevWs {
     float2 *vcs;           // [batch][RADT_MAXCHAN] channel velocity minus v_sys, cm/s, as (hi, lo) float pair
     double2 *rnode;        // [nr] {r_i, 1/r_i} node radii of the log-spaced axis (axisym), fp64
     float4 *cells;         // [batch][cells] packed {dens, temp, vel, 0}
-    double *grad;          // [batch][cells][4] packed fp64 gradient accumulators {dens, temp, vel, -} (bwd only)
+    float4 *grad;          // [batch][cells] packed gradient accumulators {dens, temp, vel, -} (bwd only)
     unsigned long long *counters;   // [8] 0-3 work counters; [4] bits of the grid's maximum temperature
 };
 

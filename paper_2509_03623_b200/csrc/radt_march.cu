@@ -257,6 +257,34 @@ __device__ __forceinline__ bool ray_setup(const MarchParams &P, RayCtx &rc, int 
     return true;
 }
 
+// Channel velocities of this lane (pairs of channels lane + 64 p, lane + 64 p + 32) and the span of all
+// channels of the item: a step whose line window misses the whole span contributes nothing.
+template <int NP>
+__device__ __forceinline__ void load_channels(const float2 *__restrict__ vtab, int nchan, int lane, f2 (&vcs)[NP],
+                                              f2 (&vcl)[NP], float &vmin, float &vmax)
+{
+    vmin = 3.0e38f; vmax = -3.0e38f;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        int c0 = lane + 64 * p, c1 = c0 + 32;
+        float2 v0 = (c0 < nchan) ? __ldg(vtab + c0) : make_float2(0.f, 0.f);
+        float2 v1 = (c1 < nchan) ? __ldg(vtab + c1) : make_float2(0.f, 0.f);
+        vcs[p] = pk(v0.x, v1.x); vcl[p] = pk(v0.y, v1.y);
+        if (c0 < nchan) { vmin = fminf(vmin, v0.x); vmax = fmaxf(vmax, v0.x); }
+        if (c1 < nchan) { vmin = fminf(vmin, v1.x); vmax = fmaxf(vmax, v1.x); }
+    }
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) {
+        vmin = fminf(vmin, __shfl_xor_sync(FULL, vmin, m));
+        vmax = fmaxf(vmax, __shfl_xor_sync(FULL, vmax, m));
+    }
+}
+
+__device__ __forceinline__ bool line_hits_span(const StepState &st, float vmin, float vmax)
+{
+    return (vmin - st.vh) * st.A < UWIN && (vmax - st.vh) * st.A > -UWIN;
+}
+
 // ---------------------------------------------------------------------------------------------
 // K2 / K3 forward march.  NP = channel-group pairs per lane: lane owns channels lane + 32 g, g < 2 NP.
 // ---------------------------------------------------------------------------------------------
@@ -272,23 +300,19 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
     const int nchan = P.line.nchan;
     float *out = P.cube + rc.ray * (size_t)nchan;
     f2 I[NP], T[NP], vcs[NP], vcl[NP];
-    const float2 *vtab = P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN;
+    float vmin, vmax;
+    load_channels<NP>(P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN, nchan, lane, vcs, vcl, vmin, vmax);
 #pragma unroll
-    for (int p = 0; p < NP; ++p) {
-        int c0 = lane + 64 * p, c1 = c0 + 32;
-        float2 v0 = (c0 < nchan) ? __ldg(vtab + c0) : make_float2(0.f, 0.f);
-        float2 v1 = (c1 < nchan) ? __ldg(vtab + c1) : make_float2(0.f, 0.f);
-        I[p] = pk(0.f, 0.f); T[p] = pk(1.f, 1.f);
-        vcs[p] = pk(v0.x, v1.x); vcl[p] = pk(v0.y, v1.y);
-    }
-    unsigned n_steps = 0, n_pairs = 0;
+    for (int p = 0; p < NP; ++p) { I[p] = pk(0.f, 0.f); T[p] = pk(1.f, 1.f); }
+    unsigned n_steps = 0, n_mufu = 0;
     if (rc.ds != 0.0) {
         const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
         // only the 32-step blocks that can hold in-grid samples (K1's conservative step range)
         for (int kb = rc.k_lo & ~31; kb < rc.k_hi; kb += 32) {
             StepState st;
             phase_a<KIND, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, kb + lane, st);
-            bool active = st.inside && (st.K2 > K2_EMPTY || !P.opt_skip_empty);
+            bool active = st.inside && (st.K2 > K2_EMPTY || !P.opt_skip_empty) &&
+                          (!P.opt_window || line_hits_span(st, vmin, vmax));
             unsigned mask = __ballot_sync(FULL, active);
             if (mask == 0u) continue;
             // compact the active steps (in march order) so that phase B is a plain counted loop
@@ -300,14 +324,15 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
             __syncwarp();
             const int cnt = __popc(mask);
             n_steps += cnt;
+#pragma unroll 2
             for (int j = 0; j < cnt; ++j) {
                 float4 q = sh_p[warp][j];
                 f2 S2 = pk1(sh_s[warp][j]);
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
                     f2 u = pair_u<CL>(vcs[p], vcl[p], q);
-                    if (P.opt_window && !__any_sync(FULL, pair_in_window(u))) continue;
-                    ++n_pairs;
+                    if (NP > 1 && P.opt_window && !__any_sync(FULL, pair_in_window(u))) continue;
+                    n_mufu += 4;
                     Pair s;
                     pair_eval(u, q.w, s);
                     // contribution c = S ((1-e) T) and partial sum I += c as ONE explicit FMA: the adjoint
@@ -329,21 +354,126 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
     }
     if (lane == 0 && n_steps) {
         atomicAdd(P.ws.counters + 0, (unsigned long long)n_steps);
-        atomicAdd(P.ws.counters + 1, (unsigned long long)n_pairs * 2ull);
+        atomicAdd(P.ws.counters + 1, (unsigned long long)n_mufu);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // K4 / K5 adjoint march: front-to-back re-march with the saved cube
 //   dL/d dtau_k,c = G_c (T_{k+1,c} S_k - R_k,c),  R_k = I - I_{<=k}        dL/dS_k = sum_c G_c (1-e_k,c) T_k,c
+// Steps come in two kinds: E (emitting, K > 0) update the transmittance and the partial sums and feed all four
+// channel sums; Z (zero opacity, LINEAR density grids) leave the ray state untouched and feed dL/dn only.
+// Channel sums are written per lane to shared memory and reduced for RADT_NS steps at a time.
 // ---------------------------------------------------------------------------------------------
-// Gradient cells are accumulated in fp64 (packed {dens, temp, vel, -}); unpacked to fp32 by k_unpack_grad.
-__device__ __forceinline__ void red_add_cell(double *cell, float w, float a, float b, float c)
+#define RADT_NS 8
+
+// Gradient cells are accumulated as packed float4 {dens, temp, vel, -} (one vector reduction per corner),
+// unpacked to the caller's planes by k_unpack_grad.
+__device__ __forceinline__ void red_add_cell(float4 *cell, float w, float a, float b, float c)
 {
-    double wd = (double)w;
-    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(cell), "d"(wd * (double)a) : "memory");
-    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(cell + 1), "d"(wd * (double)b) : "memory");
-    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(cell + 2), "d"(wd * (double)c) : "memory");
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(cell), "f"(w * a), "f"(w * b), "f"(w * c), "f"(0.f)
+                 : "memory");
+}
+__device__ __forceinline__ void red_add_dens(float4 *cell, float v)
+{
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(cell), "f"(v) : "memory");
+}
+
+__device__ __forceinline__ f2 clamp_nR(f2 PmI, f2 Tn, f2 nsmax2)
+{
+    // -R = P - I_saved, R = T_{k+1} B_{k+1}: the truth lies in [0, T_{k+1} S_max]; clamping there makes the
+    // rounding error of the subtraction decay with the transmittance
+    float r0, r1, b0, b1;
+    upk(PmI, r0, r1);
+    upk(mul2(Tn, nsmax2), b0, b1);
+    return pk(fminf(fmaxf(r0, b0), 0.f), fminf(fmaxf(r1, b1), 0.f));
+}
+
+template <int NP, bool CL>
+__device__ __forceinline__ float4 bwd_estep(const float4 q, const float S, const float nsmax, const bool window,
+                                            f2 (&T)[NP], f2 (&Pp)[NP], const f2 (&Isv)[NP], const f2 (&Gc)[NP],
+                                            const f2 (&vcs)[NP], const f2 (&vcl)[NP], unsigned &n_mufu)
+{
+    const f2 S2 = pk1(S), nsm2 = pk1(nsmax);
+    f2 a0 = pk(0.f, 0.f), a1 = a0, a2 = a0, a3 = a0;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        f2 u = pair_u<CL>(vcs[p], vcl[p], q);
+        if (NP > 1 && window && !__any_sync(FULL, pair_in_window(u))) continue;
+        n_mufu += 4;
+        Pair s;
+        pair_eval(u, q.w, s);
+        f2 omT = mul2(s.om, T[p]);
+        Pp[p] = fma2(S2, omT, Pp[p]);                 // = the forward's partial sum I_{<=k}, bit for bit
+        f2 Tn = mul2(T[p], s.e);
+        f2 nR = clamp_nR(sub2(Pp[p], Isv[p]), Tn, nsm2);
+        f2 a = mul2(Gc[p], fma2(Tn, S2, nR));         // dL/d dtau
+        f2 w = mul2(a, s.g), wu = mul2(w, s.u);
+        if (NP == 1) {
+            a0 = w; a1 = wu; a2 = mul2(wu, s.u); a3 = mul2(Gc[p], omT);
+        } else {
+            a0 = add2(a0, w); a1 = add2(a1, wu); a2 = fma2(wu, s.u, a2); a3 = fma2(Gc[p], omT, a3);
+        }
+        T[p] = Tn;
+    }
+    float x0, x1, y0, y1, z0, z1, w0, w1;
+    upk(a0, x0, x1); upk(a1, y0, y1); upk(a2, z0, z1); upk(a3, w0, w1);
+    return make_float4(x0 + x1, y0 + y1, z0 + z1, w0 + w1);
+}
+
+template <int NP, bool CL>
+__device__ __forceinline__ float bwd_zstep(const float4 q, const float S, const bool window, const f2 (&GT)[NP],
+                                           const f2 (&GnR)[NP], const f2 (&vcs)[NP], const f2 (&vcl)[NP],
+                                           unsigned &n_mufu)
+{
+    const f2 S2 = pk1(S);
+    f2 acc = pk(0.f, 0.f);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        f2 u = pair_u<CL>(vcs[p], vcl[p], q);
+        if (NP > 1 && window && !__any_sync(FULL, pair_in_window(u))) continue;
+        n_mufu += 2;
+        float t0, t1;
+        upk(mul2(u, u), t0, t1);
+        f2 g = pk(ex2_approx(-t0), ex2_approx(-t1));
+        f2 w = mul2(fma2(GT[p], S2, GnR[p]), g);
+        acc = (NP == 1) ? w : add2(acc, w);
+    }
+    float x0, x1;
+    upk(acc, x0, x1);
+    return x0 + x1;
+}
+
+// Sum the RADT_NS x 32 per-lane partials of a batch over the lanes; lanes 0..nb-1 store the sums of steps 0..nb-1.
+// Lane (s = lane & 7, h = lane >> 3) adds the 8 source lanes 8h..8h+7 of step s (skewed: conflict-free
+// 16-byte reads), then the four quarters are combined with two shuffle rounds.
+template <bool ZONLY>
+__device__ __forceinline__ void reduce_batch(const float4 (*red)[32], int nb, float4 *out, int lane)
+{
+    const int s = lane & 7, h8 = lane & 24;
+    float4 acc;
+    if (ZONLY) {
+        acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) acc.x += red[s][h8 + ((i + s) & 7)].x;
+        acc.x += __shfl_xor_sync(FULL, acc.x, 8);
+        acc.x += __shfl_xor_sync(FULL, acc.x, 16);
+    } else {
+        acc = red[s][h8 + s];
+#pragma unroll
+        for (int i = 1; i < 8; ++i) {
+            float4 v = red[s][h8 + ((i + s) & 7)];
+            acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+        }
+#pragma unroll
+        for (int m = 8; m <= 16; m <<= 1) {
+            acc.x += __shfl_xor_sync(FULL, acc.x, m);
+            acc.y += __shfl_xor_sync(FULL, acc.y, m);
+            acc.z += __shfl_xor_sync(FULL, acc.z, m);
+            acc.w += __shfl_xor_sync(FULL, acc.w, m);
+        }
+    }
+    if (lane < nb) out[lane] = acc;
 }
 
 template <int KIND, int NP, bool CL>
@@ -352,6 +482,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __g
     __shared__ float4 sh_p[RADT_WARPS_PER_CTA][32];
     __shared__ float sh_s[RADT_WARPS_PER_CTA][32];
     __shared__ float4 sh_sum[RADT_WARPS_PER_CTA][32];
+    __shared__ float4 sh_red[RADT_WARPS_PER_CTA][RADT_NS][32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     RayCtx rc;
     if (!ray_setup(P, rc, warp)) return;
@@ -362,129 +493,134 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __g
     const float *Isave = P.cube + rc.ray * (size_t)nchan;
     const float *Gin = P.dl_dcube + rc.ray * (size_t)nchan;
     f2 Isv[NP], Pp[NP], T[NP], vcs[NP], vcl[NP], Gc[NP];
-    const float2 *vtab = P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN;
+    float vmin, vmax;
+    load_channels<NP>(P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN, nchan, lane, vcs, vcl, vmin, vmax);
     bool anyg = false;
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
         int c0 = lane + 64 * p, c1 = c0 + 32;
         bool ok0 = c0 < nchan, ok1 = c1 < nchan;
-        float2 v0 = ok0 ? __ldg(vtab + c0) : make_float2(0.f, 0.f);
-        float2 v1 = ok1 ? __ldg(vtab + c1) : make_float2(0.f, 0.f);
         float g0 = ok0 ? __ldg(Gin + c0) : 0.f, g1 = ok1 ? __ldg(Gin + c1) : 0.f;
         T[p] = pk(1.f, 1.f); Pp[p] = pk(0.f, 0.f);
-        vcs[p] = pk(v0.x, v1.x); vcl[p] = pk(v0.y, v1.y);
         Isv[p] = pk(ok0 ? __ldg(Isave + c0) : 0.f, ok1 ? __ldg(Isave + c1) : 0.f);
         Gc[p] = pk(g0, g1);
         anyg |= (g0 != 0.f) || (g1 != 0.f);
     }
     if (!__any_sync(FULL, anyg)) return;     // dL/dcube vanishes on this ray: no gradient
     const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
-    double *grad = P.ws.grad + 4 * (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
-    const bool h16 = lane & 16, h8 = lane & 8;
+    float4 *grad = P.ws.grad + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     // upper bound of the source function anywhere on the grid (S grows with T)
     const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + 4)), 1.0f);
-    const float smax = G.sunit * 1.0001f / (ex2_approx(L.T0l2 / tmax) - 1.0f);
-    unsigned n_steps = 0, n_pairs = 0;
+    const float nsmax = -G.sunit * 1.0001f / (ex2_approx(L.T0l2 / tmax) - 1.0f);
+    const float kthr = P.opt_skip_empty ? K2_EMPTY : 0.f;    // the forward's own test for an emitting step
+    const bool window = P.opt_window;
+    unsigned n_steps = 0, n_mufu = 0;
     for (int kb = rc.k_lo & ~31; kb < rc.k_hi; kb += 32) {
         StepState st;
         phase_a<KIND, false>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, kb + lane, st);
-        // zero-density steps still carry dL/dn when the grid stores n itself (LINEAR)
-        bool active = st.inside && (st.K2 > K2_EMPTY || P.grid.dens_mode == 0 || !P.opt_skip_empty);
-        unsigned mask = __ballot_sync(FULL, active);
+        const bool isE = st.inside && st.K2 > kthr;
+        // zero-opacity steps still carry dL/dn when the grid stores n itself (LINEAR)
+        const bool active = st.inside && (isE || P.grid.dens_mode == 0) && (!window || line_hits_span(st, vmin, vmax));
+        const unsigned mask = __ballot_sync(FULL, active);
         if (mask == 0u) continue;
         const int pos = __popc(mask & ((1u << lane) - 1u));
         if (active) {
-            sh_p[warp][pos] = make_float4(st.vh, st.A, st.mvlA, st.K2);
+            sh_p[warp][pos] = make_float4(st.vh, st.A, st.mvlA, isE ? st.K2 : 0.f);
             sh_s[warp][pos] = st.S;
         }
         __syncwarp();
         const int cnt = __popc(mask);
         n_steps += cnt;
-        for (int j = 0; j < cnt; ++j) {
-            float4 q = sh_p[warp][j];
-            float S = sh_s[warp][j];
-            f2 S2 = pk1(S);
-            f2 p0 = pk(0.f, 0.f), p1 = p0, p2 = p0, p3 = p0;
+        const unsigned emask = __ballot_sync(FULL, lane < cnt && sh_p[warp][lane].w > 0.f);   // compacted E flags
+        for (int base = 0; base < cnt; base += RADT_NS) {
+            const int nb = min(RADT_NS, cnt - base);
+            if ((emask >> base) & ((1u << RADT_NS) - 1u)) {
+#pragma unroll 2
+                for (int jj = 0; jj < nb; ++jj) {
+                    float4 q = sh_p[warp][base + jj];
+                    float S = sh_s[warp][base + jj];
+                    sh_red[warp][jj][lane] = bwd_estep<NP, CL>(q, S, nsmax, window, T, Pp, Isv, Gc, vcs, vcl, n_mufu);
+                }
+                __syncwarp();
+                reduce_batch<false>(sh_red[warp], nb, &sh_sum[warp][base], lane);
+            } else {
+                // a run of zero-opacity steps: T, P and hence G T and G R stay fixed
+                f2 GT[NP], GnR[NP];
+                const f2 nsm2 = pk1(nsmax);
 #pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                f2 u = pair_u<CL>(vcs[p], vcl[p], q);
-                if (P.opt_window && !__any_sync(FULL, pair_in_window(u))) continue;
-                ++n_pairs;
-                Pair s;
-                pair_eval(u, q.w, s);
-                f2 omT = mul2(s.om, T[p]);
-                Pp[p] = fma2(S2, omT, Pp[p]);                 // = the forward's partial sum I_{<=k}, bit for bit
-                f2 Tn = mul2(T[p], s.e);
-                // -R = P - I_saved, R = T_{k+1} B_{k+1}: the truth lies in [0, T_{k+1} S_max]; clamping there makes
-                // the rounding error of the subtraction decay with the transmittance
-                float r0, r1, b0, b1;
-                upk(sub2(Pp[p], Isv[p]), r0, r1);
-                upk(mul2(Tn, pk1(-smax)), b0, b1);
-                f2 nR = pk(fminf(fmaxf(r0, b0), 0.f), fminf(fmaxf(r1, b1), 0.f));
-                f2 a = mul2(Gc[p], fma2(Tn, S2, nR));
-                f2 du = mul2(s.d, s.u);
-                p0 = fma2(a, s.g, p0);
-                p1 = fma2(a, du, p1);
-                p2 = fma2(mul2(a, du), s.u, p2);
-                p3 = fma2(Gc[p], omT, p3);
-                T[p] = Tn;
+                for (int p = 0; p < NP; ++p) {
+                    GT[p] = mul2(Gc[p], T[p]);
+                    GnR[p] = mul2(Gc[p], clamp_nR(sub2(Pp[p], Isv[p]), T[p], nsm2));
+                }
+#pragma unroll 4
+                for (int jj = 0; jj < nb; ++jj) {
+                    float4 q = sh_p[warp][base + jj];
+                    float S = sh_s[warp][base + jj];
+                    sh_red[warp][jj][lane].x = bwd_zstep<NP, CL>(q, S, window, GT, GnR, vcs, vcl, n_mufu);
+                }
+                __syncwarp();
+                reduce_batch<true>(sh_red[warp], nb, &sh_sum[warp][base], lane);
             }
-            float a0, a1, b0, b1, c0, c1, d0, d1;
-            upk(p0, a0, a1); upk(p1, b0, b1); upk(p2, c0, c1); upk(p3, d0, d1);
-            float q0 = a0 + a1, q1 = b0 + b1, q2 = c0 + c1, q3 = d0 + d1;
-            // transposed butterfly: 4 sums over 32 lanes in 6 shuffles
-            float s0 = h16 ? q0 : q2, s1 = h16 ? q1 : q3;
-            float k0 = h16 ? q2 : q0, k1 = h16 ? q3 : q1;
-            k0 += __shfl_xor_sync(FULL, s0, 16);
-            k1 += __shfl_xor_sync(FULL, s1, 16);
-            float sv = h8 ? k0 : k1;
-            float kk = h8 ? k1 : k0;
-            kk += __shfl_xor_sync(FULL, sv, 8);
-            kk += __shfl_xor_sync(FULL, kk, 4);
-            kk += __shfl_xor_sync(FULL, kk, 2);
-            kk += __shfl_xor_sync(FULL, kk, 1);
-            if ((lane & 7) == 0) reinterpret_cast<float *>(&sh_sum[warp][j])[lane >> 3] = kk;
+            __syncwarp();
         }
-        __syncwarp();
         // ---- phase C: chain rule to (n, T, v_phi) at this lane's step, scatter to the grid (O11) ----
         if (active) {
             float4 sm = sh_sum[warp][pos];
             const float iL2 = RADT_LN2;                       // 1 / log2(e)
-            float A0 = sm.x;
-            float A1 = sm.y * (iL2 / RADT_SQRT_LOG2E);
-            float A2 = sm.z * (iL2 * iL2);
-            float Bs = sm.w;
-            float K = st.K2 * iL2;
             float ia = st.invalpha;
-            float dL_dvlos = 2.0f * ia * A1;
-            float dL_dalpha = ia * (2.0f * A2 - A0 * K);
+            float A0 = sm.x;
             float dL_dn = A0 * (L.Ck2 * iL2) * st.W * st.em1 * st.dsf * ia;
-            float iT2 = st.invT * st.invT;
-            float iem1 = rcp_approx(st.em1);
-            float exs = (st.em1 + 1.0f);                       // e^x, consistent with the series branch
-            float dlnF_dT = L.Eu * iT2 - L.T0 * iT2 * exs * iem1 - st.qy * st.invT;
-            float dS_dT = st.S * exs * iem1 * L.T0 * iT2;
-            float dalpha_dT = 0.5f * L.a1 * ia;
-            float dL_dT = A0 * K * dlnF_dT + dL_dalpha * dalpha_dT + Bs * dS_dT;
-            if (st.tclamp) dL_dT = 0.f;
-            float dL_dv = dL_dvlos * st.proj * st.vk;
             float dL_dd = (P.grid.dens_mode == 1) ? dL_dn * st.n : dL_dn;
-            double *gp = grad + 4 * st.cell;
-            if (KIND == 0) {
-                float fu = st.f0, fw = st.f1;
-                float w00 = (1.f - fu) * (1.f - fw), w01 = (1.f - fu) * fw, w10 = fu * (1.f - fw), w11 = fu * fw;
-                long long n1 = P.grid.n1;
-                red_add_cell(gp, w00, dL_dd, dL_dT, dL_dv);
-                red_add_cell(gp + 4, w01, dL_dd, dL_dT, dL_dv);
-                red_add_cell(gp + 4 * n1, w10, dL_dd, dL_dT, dL_dv);
-                red_add_cell(gp + 4 * n1 + 4, w11, dL_dd, dL_dT, dL_dv);
-            } else {
-                long long sy = P.grid.n2, sx = (long long)P.grid.n1 * P.grid.n2;
+            float4 *gp = grad + st.cell;
+            if (isE) {
+                // the lane sums are moments of w = a g: sum a dtau u^m = K sum w u^m
+                float A1 = st.K2 * sm.y * (iL2 / RADT_SQRT_LOG2E);
+                float A2 = st.K2 * sm.z * (iL2 * iL2);
+                float Bs = sm.w;
+                float K = st.K2 * iL2;
+                float dL_dvlos = 2.0f * ia * A1;
+                float dL_dalpha = ia * (2.0f * A2 - A0 * K);
+                float iT2 = st.invT * st.invT;
+                float iem1 = rcp_approx(st.em1);
+                float exs = (st.em1 + 1.0f);                       // e^x, consistent with the series branch
+                float dlnF_dT = L.Eu * iT2 - L.T0 * iT2 * exs * iem1 - st.qy * st.invT;
+                float dS_dT = st.S * exs * iem1 * L.T0 * iT2;
+                float dalpha_dT = 0.5f * L.a1 * ia;
+                float dL_dT = A0 * K * dlnF_dT + dL_dalpha * dalpha_dT + Bs * dS_dT;
+                if (st.tclamp) dL_dT = 0.f;
+                float dL_dv = dL_dvlos * st.proj * st.vk;
+                if (KIND == 0) {
+                    float fu = st.f0, fw = st.f1;
+                    long long n1 = P.grid.n1;
+                    red_add_cell(gp, (1.f - fu) * (1.f - fw), dL_dd, dL_dT, dL_dv);
+                    red_add_cell(gp + 1, (1.f - fu) * fw, dL_dd, dL_dT, dL_dv);
+                    red_add_cell(gp + n1, fu * (1.f - fw), dL_dd, dL_dT, dL_dv);
+                    red_add_cell(gp + n1 + 1, fu * fw, dL_dd, dL_dT, dL_dv);
+                } else {
+                    long long sy = P.grid.n2, sx = (long long)P.grid.n1 * P.grid.n2;
 #pragma unroll
-                for (int cidx = 0; cidx < 8; ++cidx) {
-                    int dx = (cidx >> 2) & 1, dy = (cidx >> 1) & 1, dz = cidx & 1;
-                    float w = (dx ? st.f0 : 1.f - st.f0) * (dy ? st.f1 : 1.f - st.f1) * (dz ? st.f2 : 1.f - st.f2);
-                    red_add_cell(gp + 4 * (dx * sx + dy * sy + dz), w, dL_dd, dL_dT, dL_dv);
+                    for (int cidx = 0; cidx < 8; ++cidx) {
+                        int dx = (cidx >> 2) & 1, dy = (cidx >> 1) & 1, dz = cidx & 1;
+                        float w = (dx ? st.f0 : 1.f - st.f0) * (dy ? st.f1 : 1.f - st.f1) * (dz ? st.f2 : 1.f - st.f2);
+                        red_add_cell(gp + (dx * sx + dy * sy + dz), w, dL_dd, dL_dT, dL_dv);
+                    }
+                }
+            } else {
+                if (KIND == 0) {
+                    float fu = st.f0, fw = st.f1;
+                    long long n1 = P.grid.n1;
+                    red_add_dens(gp, (1.f - fu) * (1.f - fw) * dL_dd);
+                    red_add_dens(gp + 1, (1.f - fu) * fw * dL_dd);
+                    red_add_dens(gp + n1, fu * (1.f - fw) * dL_dd);
+                    red_add_dens(gp + n1 + 1, fu * fw * dL_dd);
+                } else {
+                    long long sy = P.grid.n2, sx = (long long)P.grid.n1 * P.grid.n2;
+#pragma unroll
+                    for (int cidx = 0; cidx < 8; ++cidx) {
+                        int dx = (cidx >> 2) & 1, dy = (cidx >> 1) & 1, dz = cidx & 1;
+                        float w = (dx ? st.f0 : 1.f - st.f0) * (dy ? st.f1 : 1.f - st.f1) * (dz ? st.f2 : 1.f - st.f2);
+                        red_add_dens(gp + (dx * sx + dy * sy + dz), w * dL_dd);
+                    }
                 }
             }
         }
@@ -492,7 +628,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_bwd(const __g
     }
     if (lane == 0 && n_steps) {
         atomicAdd(P.ws.counters + 2, (unsigned long long)n_steps);
-        atomicAdd(P.ws.counters + 3, (unsigned long long)n_pairs * 2ull);
+        atomicAdd(P.ws.counters + 3, (unsigned long long)n_mufu);
     }
 }
 

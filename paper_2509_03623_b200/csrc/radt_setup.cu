@@ -131,8 +131,7 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
             P.ws.cells[dst] = make_float4(__ldg(P.dens + src), tt, __ldg(P.vel + src), 0.0f);
         }
         if (P.do_zero_grad) {
-            double4 *gz = reinterpret_cast<double4 *>(P.ws.grad) + dst;
-            *gz = make_double4(0.0, 0.0, 0.0, 0.0);
+            P.ws.grad[dst] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
     }
     // grid-wide maximum temperature (bounds the source function in the adjoint); counters[4] holds its bits
@@ -141,7 +140,7 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
     if ((threadIdx.x & 31) == 0 && tmax > 0.f) atomicMax(reinterpret_cast<int *>(P.ws.counters + 4), __float_as_int(tmax));
 }
 
-__global__ void __launch_bounds__(256) k_unpack_grad(const double *__restrict__ grad, long long cells, int nbatch,
+__global__ void __launch_bounds__(256) k_unpack_grad(const float4 *__restrict__ grad, long long cells, int nbatch,
                                                      long long batch_stride, float *g_dens, float *g_temp, float *g_vel)
 {
     long long total = cells * nbatch;
@@ -149,11 +148,11 @@ __global__ void __launch_bounds__(256) k_unpack_grad(const double *__restrict__ 
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += stride) {
         int b = (int)(q / cells);
         long long c = q - (long long)b * cells;
-        double4 v = *(reinterpret_cast<const double4 *>(grad) + q);
+        float4 v = grad[q];
         long long dst = (long long)b * batch_stride + c;
-        if (g_dens) g_dens[dst] = (float)v.x;
-        if (g_temp) g_temp[dst] = (float)v.y;
-        if (g_vel) g_vel[dst] = (float)v.z;
+        if (g_dens) g_dens[dst] = v.x;
+        if (g_temp) g_temp[dst] = v.y;
+        if (g_vel) g_vel[dst] = v.z;
     }
 }
 
@@ -204,7 +203,7 @@ cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const C
     return cudaGetLastError();
 }
 
-cudaError_t radt_launch_unpack(const double *grad, long long cells, int nbatch, long long batch_stride, float *g_dens,
+cudaError_t radt_launch_unpack(const float4 *grad, long long cells, int nbatch, long long batch_stride, float *g_dens,
                                float *g_temp, float *g_vel, cudaStream_t st)
 {
     long long total = cells * nbatch;
