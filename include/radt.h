@@ -116,7 +116,11 @@ const char *radt_last_error(void);
 /* Run-time options (process-wide; for measurements).  Keys: */
 enum {
     RADT_OPT_WINDOW = 1,          /* 1 (default): skip channel groups outside the +-6.4 alpha line window; 0: dense */
-    RADT_OPT_SKIP_EMPTY = 2       /* 1 (default): skip steps with zero opacity in the forward march; 0: dense */
+    RADT_OPT_SKIP_EMPTY = 2,      /* 1 (default): skip steps with zero opacity in the forward march; 0: dense */
+    RADT_OPT_WIN_PATH = 3         /* 1 (default): channel tables that are uniform lattices v_0 + c dv use the window
+                                     kernels (one channel per lane inside the line window); 0: always the
+                                     channel-table kernels.  radt_render and radt_render_bwd of one cube must run
+                                     under the same setting. */
 };
 int radt_set_option(int key, int value);
 int radt_get_option(int key);

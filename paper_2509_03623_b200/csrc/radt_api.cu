@@ -15,6 +15,7 @@ thread_local char g_err[512] = "";
 thread_local int g_launches = 0;
 int g_opt_window = 1;
 int g_opt_skip_empty = 1;
+int g_opt_win_path = 1;
 
 int fail(int code, const char *fmt, ...)
 {
@@ -102,7 +103,9 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
         double cell_lg2 = d.lg2_ratio / (double)(grid->n[0] - 1);
         d.inv_cell_lg2 = (float)(1.0 / cell_lg2);
         d.inv_cell_ln = (float)(1.0 / (cell_lg2 * std::log(2.0)));
-        d.fine_r = (std::exp2(cell_lg2) - 1.0) < 0.15;
+        d.fine_r = (std::exp2(2.0 * cell_lg2) - 1.0) < 0.35;
+        d.zlo_f = (float)d.zlo; d.wscale_f = (float)d.wscale_d;
+        d.inv_rmin2_f = (float)(1.0 / (rmin * rmin)); d.half_uscale = (float)(0.5 * (double)(grid->n[0] - 1) / d.lg2_ratio);
         double zm = std::fmax(std::fabs(grid->lo[1]), std::fabs(grid->hi[1]));
         d.rb2 = rmax * rmax * (1.0 + zm * zm);
     } else {
@@ -111,6 +114,26 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
             d.inv_d[a] = (double)(grid->n[a] - 1) / (grid->hi[a] - grid->lo[a]);
         }
     }
+}
+
+// The prefilter of the window kernels locates steps in fp32 (positions good to ~1e-7 of the grid's extent) and
+// tolerates one cell of error: require the smallest cell to be 100 times coarser than that.
+bool prefilter_safe(const radt_grid *grid)
+{
+    if (grid->kind == RADT_GRID_AXISYM) {
+        double rmin = grid->lo[0], rmax = grid->hi[0];
+        double zm = std::fmax(std::fabs(grid->lo[1]), std::fabs(grid->hi[1]));
+        double ext = rmax * std::sqrt(1.0 + zm * zm);
+        double dr = rmin * (std::pow(rmax / rmin, 1.0 / (grid->n[0] - 1)) - 1.0);
+        double dz = rmin * (grid->hi[1] - grid->lo[1]) / (grid->n[1] - 1);
+        return std::fmin(dr, dz) > 1.2e-5 * ext;
+    }
+    double ext = 0.0, dmin = 1e300;
+    for (int a = 0; a < 3; ++a) {
+        ext = std::fmax(ext, std::fmax(std::fabs(grid->lo[a]), std::fabs(grid->hi[a])));
+        dmin = std::fmin(dmin, (grid->hi[a] - grid->lo[a]) / (grid->n[a] - 1));
+    }
+    return dmin > 1.2e-5 * ext;
 }
 
 double source_unit(const radt_geom &g, const radt_line *line)
@@ -148,10 +171,21 @@ void make_dev_line(const radt_line *line, DevLine &d)
     d.Ck2 = (float)(Ck * kLOG2E);
     d.nchan = line->nchan;
     d.ngroups = (line->nchan + 31) / 32;
+    // uniform channel lattice v_c = v_0 + c dv (any sign of dv)?  One channel counts as a lattice of 1 km/s.
+    const int n = line->nchan;
+    double dv = n > 1 ? (line->vchan[n - 1] - line->vchan[0]) / (double)(n - 1) : 1.0e5;
+    bool uni = dv != 0.0 && std::isfinite(dv);
+    for (int c = 0; c < n && uni; ++c)
+        if (!(std::fabs(line->vchan[c] - (line->vchan[0] + c * dv)) <= 1e-9 * std::fabs(dv))) uni = false;
+    d.uniform = uni ? 1 : 0;
+    d.inv_dv = uni ? 1.0 / dv : 0.0;
+    d.dvf = uni ? (float)(dv * std::sqrt(kLOG2E)) : 0.f;
+    d.c_hw = uni ? (float)(1.0 / (std::sqrt(kLOG2E) * std::fabs(dv))) : 0.f;
 }
 
 struct WsLayout {
-    size_t rays, qtab, vcs, rnode, cells, grad, counters, total;
+    size_t rays, qtab, vcs, rnode, cells, occ, grad, counters, total;
+    int occ_wpr, occ_words;
 };
 
 WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass)
@@ -166,6 +200,9 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     w.rnode = off; off = align256(off + (size_t)(grid->kind == RADT_GRID_AXISYM ? grid->n[0] : 1) * sizeof(double2));
     size_t cells = (size_t)grid_cells(grid) * (size_t)batch;
     w.cells = off; off = align256(off + cells * sizeof(float4));
+    w.occ_wpr = grid->kind == RADT_GRID_AXISYM ? (grid->n[1] + 31) / 32 : 1;
+    w.occ_words = grid->kind == RADT_GRID_AXISYM ? grid->n[0] * w.occ_wpr : 1;
+    w.occ = off; off = align256(off + (size_t)w.occ_words * (size_t)batch * sizeof(unsigned));
     w.grad = off;
     if (pass == RADT_PASS_BWD) off = align256(off + cells * sizeof(float4));
     w.total = off;
@@ -182,6 +219,7 @@ DevWs make_dev_ws(void *ws, const WsLayout &w)
     d.vcs = (float2 *)(base + w.vcs);
     d.rnode = (double2 *)(base + w.rnode);
     d.cells = (float4 *)(base + w.cells);
+    d.occ = (unsigned *)(base + w.occ);
     d.grad = (float4 *)(base + w.grad);
     return d;
 }
@@ -217,12 +255,17 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
     DevGrid dg;
     make_dev_grid(grid, dg);
     DevWs dws = make_dev_ws(ws, w);
+    DevLine dl_probe;
+    make_dev_line(line, dl_probe);
+    // window kernels: uniform channel lattice, and cells no finer than the fp32 positions of the prefilter resolve
+    const bool use_win = g_opt_win_path && dl_probe.uniform && prefilter_safe(grid);
     CUDA_TRY(cudaMemsetAsync(dws.counters, 0, 8 * sizeof(unsigned long long), st));
     for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
         int nb = batch - b0 < RADT_MAXB ? batch - b0 : RADT_MAXB;
         memset(&SP, 0, sizeof(SP));
         for (int b = 0; b < nb; ++b) {
             make_dev_geom(geom[b0 + b], line, SP.geom[b]);
+            SP.geom[b].v0 = line->vchan[0] - geom[b0 + b].vsys;
             SP.vsys[b] = geom[b0 + b].vsys;
         }
         SP.grid = dg; SP.ws = dws;
@@ -230,6 +273,13 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         SP.nlev = line->nlev; SP.nchan = line->nchan;
         SP.do_rays = 1; SP.do_tables = 1; SP.do_pack = 1; SP.do_zero_grad = (pass == RADT_PASS_BWD);
         SP.batch_stride = stride;
+        // occupancy bitmap for the window kernels' prefilter (axisymmetric grids): with LINEAR densities the
+        // adjoint needs every in-grid step (dL/dn of empty cells), so only the forward and LN grids use it
+        const bool win = use_win;
+        const bool occ = win && grid->kind == RADT_GRID_AXISYM && g_opt_skip_empty &&
+                         (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN);
+        SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr;
+        SP.occ_thr = grid->dens_mode == RADT_DENS_LN ? -39.1439f : 1e-17f;     // N_EMPTY of the march kernels
         SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;
         CUDA_TRY(radt_launch_setup(SP, LT, CT, st));
         ++g_launches;
@@ -250,7 +300,10 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
                 if ((double)(float)vv != vv) { MP.chan_lo = 1; break; }
             }
         MP.cube = cube; MP.dl_dcube = dl_dcube;
-        if (pass == RADT_PASS_FWD) CUDA_TRY(radt_launch_march_fwd(MP, nb, st));
+        MP.use_win = win; MP.use_occ = occ; MP.occ_words = w.occ_words; MP.occ_wpr = w.occ_wpr;
+        if (pass == RADT_PASS_FWD && win) CUDA_TRY(radt_launch_march_fwd_win(MP, nb, st));
+        else if (pass == RADT_PASS_FWD) CUDA_TRY(radt_launch_march_fwd(MP, nb, st));
+        else if (win) CUDA_TRY(radt_launch_march_bwd_win(MP, nb, st));
         else CUDA_TRY(radt_launch_march_bwd(MP, nb, st));
         ++g_launches;
     }
@@ -273,6 +326,7 @@ int radt_set_option(int key, int value)
 {
     if (key == RADT_OPT_WINDOW) { g_opt_window = value != 0; return RADT_OK; }
     if (key == RADT_OPT_SKIP_EMPTY) { g_opt_skip_empty = value != 0; return RADT_OK; }
+    if (key == RADT_OPT_WIN_PATH) { g_opt_win_path = value != 0; return RADT_OK; }
     return fail(RADT_E_INVALID, "unknown option %d", key);
 }
 
@@ -280,6 +334,7 @@ int radt_get_option(int key)
 {
     if (key == RADT_OPT_WINDOW) return g_opt_window;
     if (key == RADT_OPT_SKIP_EMPTY) return g_opt_skip_empty;
+    if (key == RADT_OPT_WIN_PATH) return g_opt_win_path;
     return fail(RADT_E_INVALID, "unknown option %d", key);
 }
 

@@ -25,6 +25,7 @@ struct DevGeom {
     double wx, wy, wz;                 // ray direction (increasing s) in the disk frame
     double x0, y0, pix_x, pix_y;       // image centre offset and pixel pitch, au
     double gm_au_d;                    // G M / au  [(cm/s)^2 au]  (KEPLER_FRAC)
+    double v0;                         // velocity of channel 0 minus v_sys, cm/s (uniform channel lattice)
     float sunit;                       // S0 / intensity unit
 };
 
@@ -38,7 +39,9 @@ struct DevGrid {
     double lg2_ratio;                  // log2(r_max/r_min)
     float uscale;                      // (nr-1)/log2(r_max/r_min)
     float inv_cell_ln, inv_cell_lg2;   // 1/ln(rho), 1/log2(rho), rho = node ratio r_{i+1}/r_i
-    int fine_r;                        // rho - 1 < 0.15: log1p series for the in-cell fraction
+    int fine_r;                        // rho^2 - 1 < 0.35: log1p series for the in-cell fraction
+    float zlo_f, wscale_f;             // fp32 copies for the index coordinates
+    float inv_rmin2_f, half_uscale;    // u = lg2(r^2 / r_min^2) (nr-1) / (2 log2(r_max/r_min))
     // cartesian
     double lo[3], hi[3], inv_d[3];
     double rb2;                        // bounding sphere radius^2 (axisym clip)
@@ -54,6 +57,11 @@ struct DevLine {
     float Ck2;         // line-centre dtau * log2e = Ck2 * n * W * (e^x - 1) * ds[au] / alpha
     int nchan;
     int ngroups;       // ceil(nchan / 32)
+    // uniform channel lattice v_c = v0 + c dv (window path)
+    int uniform;       // the channel table is such a lattice
+    double inv_dv;     // 1 / dv
+    float dvf;         // dv sqrt(log2 e)           (u' step between channels = dvf / alpha)
+    float c_hw;        // 1 / (sqrt(log2 e) |dv|)   (half-width of the line window in channels = u'_cut c_hw alpha)
 };
 
 // K1 output per ray: clipped interval and the conservative range of steps that can lie inside the grid
@@ -68,9 +76,10 @@ struct DevWs {
     RayRec *rays;          // [batch*ny*nx]
     float2 *qtab;          // [RADT_NQ + 2] {Q, dQ/dlnT}
     float2 *vcs;           // [batch][RADT_MAXCHAN] channel velocity minus v_sys, cm/s, as (hi, lo) float pair
-    double2 *rnode;        // [nr] {r_i, 1/r_i} node radii of the log-spaced axis (axisym), fp64
+    double2 *rnode;        // [nr] {r_i, 1/r_i^2} node radii of the log-spaced axis (axisym), fp64
     float4 *cells;         // [batch][cells] packed {dens, temp, vel, 0}
     float4 *grad;          // [batch][cells] packed gradient accumulators {dens, temp, vel, -} (bwd only)
+    unsigned *occ;         // [batch][occ_words] bit (i, j): some cell within one cell of (i, j) can emit (axisym)
     unsigned long long *counters;   // [8] 0-3 work counters; [4] bits of the grid's maximum temperature
 };
 
@@ -84,6 +93,9 @@ struct MarchParams {
     int b0;                // first batch item of this launch
     int opt_window, opt_skip_empty;
     int chan_lo;           // some channel velocity is not exactly representable in fp32: use the lo parts
+    int use_win;           // uniform-channel window kernels (radt_march_win.cu)
+    int use_occ;           // candidate steps are prefiltered with the occupancy bitmap
+    int occ_words, occ_wpr; // words per batch item, words per radial row
     float *cube;           // fwd: output; bwd: saved forward output (const)
     const float *dl_dcube; // bwd
 };
@@ -94,7 +106,9 @@ struct SetupParams {
     DevWs ws;
     int nx, ny, nstep, nbatch, b0;
     int nlev, nchan;
-    int do_rays, do_tables, do_pack, do_zero_grad;
+    int do_rays, do_tables, do_pack, do_zero_grad, do_occ;
+    int occ_words, occ_wpr;
+    float occ_thr;         // stored density value above which a node can emit
     long long batch_stride;
     const float *dens, *temp, *vel;
     double2 *rays_user;    // radt_ray_geometry output {s0, ds} (may be null)
@@ -114,6 +128,7 @@ struct ChanTable {
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // Disk-frame position of the s = 0 point of pixel (ix, iy)  (O1-O2).

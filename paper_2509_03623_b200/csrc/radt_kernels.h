@@ -9,4 +9,6 @@ cudaError_t radt_launch_l2(const float *cube, const float *target, double sigma,
                            cudaStream_t st);
 cudaError_t radt_launch_march_fwd(const MarchParams &P, int nbatch, cudaStream_t st);
 cudaError_t radt_launch_march_bwd(const MarchParams &P, int nbatch, cudaStream_t st);
+cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st);
+cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStream_t st);
 cudaError_t radt_run_pipe_peak(int kind, double *ops_per_s, double *clock_mhz);

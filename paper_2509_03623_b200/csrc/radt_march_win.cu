@@ -1,0 +1,534 @@
+// radt_march_win.cu -- forward march (K2/K3) and adjoint march (K4/K5) on a UNIFORM channel lattice, sm_100a.
+//
+// The line profile of one ray step touches only the channels within +-6.4 alpha of its v_los (Eq. 15,
+// PAPER.md:280): ~21 of 64 channels in config 2.  This path therefore gives every lane ONE channel of the
+// step's 32-channel group [c_lo, c_lo + 32) instead of a fixed set of channels:
+//   prefilter (lanes over steps, fp32): drop steps that cannot lie in a cell that emits (occupancy bitmap,
+//       dilated by one cell), compact the candidates of several 32-step blocks;
+//   phase A (lanes over candidate steps): exact fp64 in/out decision, sampling, LTE thermodynamics, the step's
+//       channel window and group -> compacted step entries in shared memory, two steps per slot pair;
+//   phase B (lanes over channels): per PAIR of steps one packed f32x2 evaluation (4 MUFU.EX2) and the
+//       sequential accumulate of O9; the lane's (I, T) live in two scalar registers while the group is
+//       unchanged and are swapped with the per-group state when the group moves.
+// Steps wider than 32 channels (or RADT_OPT_WINDOW = 0) run one pass per fixed 32-channel block.
+// Algorithm: DESIGN.md O4-O11; PAPER.md:262-294 (Eq. 11-17).
+#include "radt_march.cuh"
+
+#define WIN_PAIRS 16         // slot pairs per batch of 32 steps
+#define NO_GROUP 0x7fffffff
+
+struct __align__(16) WinShared {          // per warp
+    float4 a[WIN_PAIRS];                  // {u0_a, u0_b, dvA_a, dvA_b}
+    float4 b[WIN_PAIRS];                  // {K2_a, K2_b, S_a, S_b}
+    float4 c[WIN_PAIRS];                  // {off_a, off_b, bits of c_lo, -}   off = c_lo - c_ref
+    int cand[64];                         // candidate step indices waiting for phase A
+    int2 win[32];                         // channel windows of the compacted steps
+};
+
+// fp32 copy of the ray and of the grid mapping for the prefilter
+struct PreCtx {
+    float ox, oy, oz, wx, wy, wz, s0, ds;
+    float us_half, lrm;                   // u = lg2(r^2) us_half - lrm
+    float zlo, wscale;
+    float lo[3], inv_d[3];
+};
+
+template <int KIND>
+__device__ __forceinline__ void pre_setup(const MarchParams &P, const DevGeom &G, const RayCtx &rc, PreCtx &pc)
+{
+    pc.ox = (float)rc.ox; pc.oy = (float)rc.oy; pc.oz = (float)rc.oz;
+    pc.wx = (float)G.wx; pc.wy = (float)G.wy; pc.wz = (float)G.wz;
+    pc.s0 = (float)rc.s0; pc.ds = (float)rc.ds;
+    if (KIND == 0) {
+        pc.us_half = 0.5f * P.grid.uscale;
+        pc.lrm = -lg2_approx((float)P.grid.inv_rmin) * P.grid.uscale;
+        pc.zlo = (float)P.grid.zlo; pc.wscale = (float)P.grid.wscale_d;
+    } else {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { pc.lo[a] = (float)P.grid.lo[a]; pc.inv_d[a] = (float)P.grid.inv_d[a]; }
+    }
+}
+
+// Can step k lie in a cell that matters?  A superset test in fp32: positions are good to ~1e-4 au, the test
+// accepts one cell of margin around the grid and the bitmap is dilated by one cell (radt_setup.cu).
+template <int KIND>
+__device__ __forceinline__ bool prefilter(const MarchParams &P, const PreCtx &pc, const unsigned *__restrict__ occ, int k)
+{
+    float s = fmaf((float)k + 0.5f, pc.ds, pc.s0);
+    float x = fmaf(s, pc.wx, pc.ox), y = fmaf(s, pc.wy, pc.oy), z = fmaf(s, pc.wz, pc.oz);
+    if (KIND == 0) {
+        float r2 = fmaf(x, x, y * y);
+        float ri = rsqrt_approx(fmaxf(r2, 1e-30f));
+        float zeta = (P.grid.mirror ? fabsf(z) : z) * ri;
+        float uf = fmaf(lg2_approx(fmaxf(r2, 1e-30f)), pc.us_half, -pc.lrm);
+        float wf = (zeta - pc.zlo) * pc.wscale;
+        bool in = uf > -1.0f && uf < (float)P.grid.n0 && wf > -1.0f && wf < (float)P.grid.n1;
+        if (!in) return false;
+        if (!P.use_occ) return true;
+        int i = min(max(rn_int(uf - 0.5f), 0), P.grid.n0 - 2);
+        int j = min(max(rn_int(wf - 0.5f), 0), P.grid.n1 - 2);
+        unsigned w = __ldg(occ + i * P.occ_wpr + (j >> 5));
+        return (w >> (j & 31)) & 1u;
+    } else {
+        float tx = (x - pc.lo[0]) * pc.inv_d[0], ty = (y - pc.lo[1]) * pc.inv_d[1], tz = (z - pc.lo[2]) * pc.inv_d[2];
+        return tx > -1.0f && tx < (float)P.grid.n0 && ty > -1.0f && ty < (float)P.grid.n1 && tz > -1.0f &&
+               tz < (float)P.grid.n2;
+    }
+}
+
+// Group of a step whose conservative window is [wlo, whi] (width <= 32): c_lo = wlo rounded down to a multiple
+// of q, with q the largest power of two that still keeps whi < c_lo + 32.  Consecutive steps of one crossing of
+// the emitting layer then share c_lo, and the lanes keep their channel.
+__device__ __forceinline__ int group_of(int wlo, int ww)
+{
+    int q = ww <= 17 ? 16 : ww <= 25 ? 8 : ww <= 29 ? 4 : ww <= 31 ? 2 : 1;
+    return wlo & -q;
+}
+
+// Compact the active steps of this batch (march order) into slot pairs {2i, 2i+1}.  The two steps of a pair share
+// one group, chosen for the union of their windows; an odd count is completed with a no-op entry (K2 = 0).
+// Returns the number of pairs; `wide` tells that some pair's union is wider than 32 channels (the caller then
+// runs one pass per fixed 32-channel block, `blk` >= 0).
+__device__ __forceinline__ int write_entries(WinShared &S, int lane, bool act, int blk, const StepState &st, float K2,
+                                         bool &wide, int &pos_out)
+{
+    const unsigned mask = __ballot_sync(FULL, act);
+    wide = false;
+    if (mask == 0u) return 0;
+    const int cnt = __popc(mask);
+    const int pos = __popc(mask & ((1u << lane) - 1u));
+    pos_out = pos;
+    int clo = blk;
+    if (blk < 0) {
+        if (act) S.win[pos] = make_int2(st.wlo, st.whi);
+        __syncwarp();
+        int ulo = st.wlo, uhi = st.whi;
+        if (act && (pos ^ 1) < cnt) {
+            const int2 pw = S.win[pos ^ 1];
+            ulo = min(ulo, pw.x); uhi = max(uhi, pw.y);
+        }
+        const int uw = uhi - ulo + 1;
+        wide = __any_sync(FULL, act && uw > 32);
+        if (wide) return 0;
+        clo = group_of(ulo, uw);
+    }
+    float *fa = reinterpret_cast<float *>(S.a), *fb = reinterpret_cast<float *>(S.b), *fc = reinterpret_cast<float *>(S.c);
+    if (act) {
+        const int q = (pos >> 1) * 4 + (pos & 1);
+        fa[q] = st.u0; fa[q + 2] = st.dvA;
+        fb[q] = K2; fb[q + 2] = st.S;
+        fc[q] = (float)(clo - st.cref);
+        if (!(pos & 1)) {
+            fc[q + 2] = __int_as_float(clo);
+            if (pos == cnt - 1) { fa[q + 1] = 0.f; fa[q + 3] = 0.f; fb[q + 1] = 0.f; fb[q + 3] = 0.f; fc[q + 1] = 0.f; }
+        }
+    }
+    __syncwarp();
+    return (cnt + 1) >> 1;
+}
+
+// Per-lane channel state of the window march: (I, T) of all the lane's channels c = lane + 32 g, and the pair
+// (Is, Ts) of the one channel the lane serves in the current group [cur, cur + 32).
+template <int NG>
+struct LaneState {
+    float I[NG], T[NG];
+    float Is, Ts, mf;
+    int cur, myg;
+    __device__ __forceinline__ void init()
+    {
+#pragma unroll
+        for (int g = 0; g < NG; ++g) { I[g] = 0.f; T[g] = 1.f; }
+        Is = 0.f; Ts = 1.f; mf = 0.f; cur = NO_GROUP; myg = -1;
+    }
+    __device__ __forceinline__ void put_back()
+    {
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+            if (myg == g) { I[g] = Is; T[g] = Ts; }
+    }
+    // the group moved: put the lane's channel state back, take the new channel's
+    __device__ __forceinline__ void regroup(int clo, int lane, int nchan)
+    {
+        put_back();
+        const int m = (lane - clo) & 31, c = clo + m;
+        myg = (unsigned)c < (unsigned)nchan ? (c >> 5) : -1;
+        mf = (float)m;
+        Is = 0.f; Ts = 1.f;
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+            if (myg == g) { Is = I[g]; Ts = T[g]; }
+        cur = clo;
+    }
+};
+
+// u' of the lane's channel for the two steps of a pair
+__device__ __forceinline__ f2 pair_u_win(const float4 &qa, const float4 &qc, float mf)
+{
+    return fma2(add2(pk1(mf), pk(qc.x, qc.y)), pk(qa.z, qa.w), pk(qa.x, qa.y));
+}
+
+// O9 for the two steps of a pair, in march order.  c = S ((1-e) T) and I += c with fixed roundings: the adjoint
+// re-march repeats exactly this sequence and so reproduces the partial sums bit for bit.
+__device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, const float4 &qc, f2 K2, float mf, float &Is,
+                                         float &Ts)
+{
+    Pair s;
+    pair_eval(pair_u_win(qa, qc, mf), K2, s);
+    float om0, om1, e0, e1;
+    upk(s.om, om0, om1);
+    upk(s.e, e0, e1);
+    Is = __fmaf_rn(qb.z, __fmul_rn(om0, Ts), Is);
+    Ts = __fmul_rn(Ts, e0);
+    Is = __fmaf_rn(qb.w, __fmul_rn(om1, Ts), Is);
+    Ts = __fmul_rn(Ts, e1);
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2 / K3 forward march, NG = ceil(nchan / 32) rounded up to {1, 2, 4, 8}
+// ---------------------------------------------------------------------------------------------
+template <int KIND, int NG>
+__global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_fwd_w(const __grid_constant__ MarchParams P)
+{
+    __shared__ WinShared sh[RADT_WARPS_PER_CTA];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    RayCtx rc;
+    if (!ray_setup(P, rc, warp)) return;
+    WinShared &S = sh[warp];
+    const DevGeom &G = P.geom[rc.b];
+    const int nchan = P.line.nchan;
+    float *out = P.cube + rc.ray * (size_t)nchan;
+    LaneState<NG> L;
+    L.init();
+    unsigned n_steps = 0, n_mufu = 0;
+    if (rc.ds != 0.0) {
+        const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
+        const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
+        PreCtx pc;
+        pre_setup<KIND>(P, G, rc, pc);
+        const unsigned lt = (1u << lane) - 1u;
+        int ncand = 0, kb = rc.k_lo & ~31;
+        while (true) {
+            while (ncand < 32 && kb < rc.k_hi) {
+                const int k = kb + lane;
+                const bool cnd = k >= rc.k_lo && k < rc.k_hi && prefilter<KIND>(P, pc, occ, k);
+                const unsigned m = __ballot_sync(FULL, cnd);
+                if (cnd) S.cand[ncand + __popc(m & lt)] = k;
+                ncand += __popc(m);
+                kb += 32;
+            }
+            if (ncand == 0) break;
+            __syncwarp();
+            const int n = min(ncand, 32);
+            const int k = lane < n ? S.cand[lane] : P.nstep;
+            const int kx = lane + 32 < ncand ? S.cand[lane + 32] : 0;
+            __syncwarp();
+            if (lane + 32 < ncand) S.cand[lane] = kx;
+            ncand -= n;
+
+            StepState st;
+            phase_a<KIND, true, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, k, st);
+            const bool act = st.inside && (st.K2 > K2_EMPTY || !P.opt_skip_empty) && st.whi >= 0 && st.wlo < nchan;
+            n_steps += __popc(__ballot_sync(FULL, act));
+            bool wide;
+            int pos;
+            int npairs = write_entries(S, lane, act, -1, st, st.K2, wide, pos);
+            const int npass = wide ? NG : 1;
+            for (int p = 0; p < npass; ++p) {
+                if (wide) {
+                    bool w2;
+                    npairs = write_entries(S, lane, act && st.wlo <= 32 * p + 31 && st.whi >= 32 * p, 32 * p, st, st.K2, w2, pos);
+                }
+                if (npairs == 0) continue;
+#pragma unroll 2
+                for (int i = 0; i < npairs; ++i) {
+                    const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
+                    const int clo = __float_as_int(qc.z);
+                    if (clo != L.cur) L.regroup(clo, lane, nchan);
+                    fwd_pair(qa, qb, qc, pk(qb.x, qb.y), L.mf, L.Is, L.Ts);
+                }
+                n_mufu += 4 * npairs;
+                __syncwarp();
+            }
+        }
+        L.put_back();
+    }
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+        const int c = lane + 32 * g;
+        if (c < nchan) out[c] = L.I[g];
+    }
+    if (lane == 0 && n_steps) {
+        atomicAdd(P.ws.counters + 0, (unsigned long long)n_steps);
+        atomicAdd(P.ws.counters + 1, (unsigned long long)n_mufu);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K4 / K5 adjoint march: front-to-back re-march with the saved cube
+//   dL/d dtau_k,c = G_c (T_{k+1,c} S_k - R_k,c),  R_k = I - I_{<=k}        dL/dS_k = sum_c G_c (1-e_k,c) T_k,c
+// Entries with K2 = 0 are zero-opacity steps (LINEAR density grids): they leave the ray state untouched and
+// feed dL/dn only.  Per pair of steps every lane writes its partial sums {w, w u', w u'^2, G (1-e) T} of both
+// steps (four float2) to shared memory; after BWD_SUB pairs the lanes sum them over the channels.
+// ---------------------------------------------------------------------------------------------
+#define BWD_SUB 4            // pairs per reduction batch
+
+template <int NG>
+struct BwdLane {
+    float T[NG], Pp[NG], Isv[NG], Gc[NG];
+    float Ts, Ps, Is, Gs, mf;                     // transmittance, partial sum, saved I, dL/dI of the served channel
+    int cur, myg;
+    __device__ __forceinline__ void put_back()
+    {
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+            if (myg == g) { T[g] = Ts; Pp[g] = Ps; }
+    }
+    __device__ __forceinline__ void regroup(int clo, int lane, int nchan)
+    {
+        put_back();
+        const int m = (lane - clo) & 31, c = clo + m;
+        myg = (unsigned)c < (unsigned)nchan ? (c >> 5) : -1;
+        mf = (float)m;
+        Ts = 1.f; Ps = 0.f; Is = 0.f; Gs = 0.f;    // lanes without a channel contribute nothing (G = 0)
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+            if (myg == g) { Ts = T[g]; Ps = Pp[g]; Is = Isv[g]; Gs = Gc[g]; }
+        cur = clo;
+    }
+};
+
+typedef float2 RedBuf[BWD_SUB][4][32];           // [pair][quantity][lane] {step a, step b}
+
+__device__ __forceinline__ float2 f2_as_float2(f2 v) { float a, b; upk(v, a, b); return make_float2(a, b); }
+
+// A pair with at least one emitting step.  Repeats the forward's O9 sequence bit for bit (fwd_pair).
+template <int NG>
+__device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane<NG> &L,
+                                           float nsmax, float2 (*red)[32], int lane)
+{
+    Pair s;
+    pair_eval(pair_u_win(qa, qc, L.mf), pk(qb.x, qb.y), s);
+    float om0, om1, e0, e1;
+    upk(s.om, om0, om1);
+    upk(s.e, e0, e1);
+    const float c0 = __fmul_rn(om0, L.Ts);
+    const float P0 = __fmaf_rn(qb.z, c0, L.Ps);
+    const float T1 = __fmul_rn(L.Ts, e0);
+    const float c1 = __fmul_rn(om1, T1);
+    const float P1 = __fmaf_rn(qb.w, c1, P0);
+    const float T2 = __fmul_rn(T1, e1);
+    const f2 Tn = pk(T1, T2), G2 = pk1(L.Gs);
+    const f2 nR = clamp_nR(sub2(pk(P0, P1), pk1(L.Is)), Tn, pk1(nsmax));
+    const f2 a = mul2(G2, fma2(Tn, pk(qb.z, qb.w), nR));          // dL/d dtau
+    const f2 w = mul2(a, s.g), wu = mul2(w, s.u);
+    red[0][lane] = f2_as_float2(w);
+    red[1][lane] = f2_as_float2(wu);
+    red[2][lane] = f2_as_float2(mul2(wu, s.u));
+    red[3][lane] = f2_as_float2(mul2(G2, pk(c0, c1)));
+    L.Ts = T2; L.Ps = P1;
+}
+
+// A pair of zero-opacity steps: T, P and hence G T and G R stay fixed; only sum w is needed.
+template <int NG>
+__device__ __forceinline__ void bwd_pair_z(const float4 &qa, const float4 &qb, const float4 &qc, const BwdLane<NG> &L,
+                                           float nsmax, float2 (*red)[32], int lane, bool zero_rest)
+{
+    const f2 u = pair_u_win(qa, qc, L.mf);
+    float t0, t1;
+    upk(mul2(u, u), t0, t1);
+    const f2 g = pk(ex2_approx(-t0), ex2_approx(-t1));
+    const float GT = L.Gs * L.Ts;
+    const float GnR = L.Gs * fminf(fmaxf(L.Ps - L.Is, L.Ts * nsmax), 0.f);
+    red[0][lane] = f2_as_float2(mul2(fma2(pk1(GT), pk(qb.z, qb.w), pk1(GnR)), g));
+    if (zero_rest) {
+        red[1][lane] = make_float2(0.f, 0.f); red[2][lane] = make_float2(0.f, 0.f); red[3][lane] = make_float2(0.f, 0.f);
+    }
+}
+
+// Sum the partials of nb <= BWD_SUB pairs over the 32 lanes; lane p < nb ends with the sums of pair p and stores
+// them as two float4 (steps 2p, 2p+1) into out.  Lane (p = lane & 3, h = lane >> 2) adds the source lanes
+// 4h..4h+3 of pair p (skewed: conflict-free 8-byte reads), then the eight groups are combined by three shuffle
+// rounds.
+template <bool ZONLY>
+__device__ __forceinline__ void reduce_pairs(const RedBuf &red, int nb, float4 *out, int lane)
+{
+    const int p = lane & 3, h4 = lane & 28;
+    float2 acc[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        if (ZONLY && q > 0) { acc[q] = make_float2(0.f, 0.f); continue; }
+        acc[q] = red[p][q][h4 + p];
+#pragma unroll
+        for (int i = 1; i < 4; ++i) {
+            const float2 v = red[p][q][h4 + ((i + p) & 3)];
+            acc[q].x += v.x; acc[q].y += v.y;
+        }
+#pragma unroll
+        for (int m = 4; m <= 16; m <<= 1) {
+            acc[q].x += __shfl_xor_sync(FULL, acc[q].x, m);
+            acc[q].y += __shfl_xor_sync(FULL, acc[q].y, m);
+        }
+    }
+    if (lane < nb) {
+        out[2 * lane] = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);
+        out[2 * lane + 1] = make_float4(acc[0].y, acc[1].y, acc[2].y, acc[3].y);
+    }
+}
+
+struct __align__(16) BwdShared {          // per warp
+    WinShared w;
+    RedBuf red;
+    float4 sum[32];                       // channel sums of the compacted steps
+};
+
+template <int KIND, int NG>
+__global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(const __grid_constant__ MarchParams P)
+{
+    __shared__ BwdShared sh[RADT_WARPS_PER_CTA];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    RayCtx rc;
+    if (!ray_setup(P, rc, warp)) return;
+    if (rc.ds == 0.0) return;
+    WinShared &S = sh[warp].w;
+    const DevGeom &G = P.geom[rc.b];
+    const DevLine &Ln = P.line;
+    const int nchan = Ln.nchan;
+    const float *Isave = P.cube + rc.ray * (size_t)nchan;
+    const float *Gin = P.dl_dcube + rc.ray * (size_t)nchan;
+    BwdLane<NG> L;
+    bool anyg = false;
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+        const int c = lane + 32 * g;
+        const bool ok = c < nchan;
+        L.T[g] = 1.f; L.Pp[g] = 0.f;
+        L.Isv[g] = ok ? __ldg(Isave + c) : 0.f;
+        L.Gc[g] = ok ? __ldg(Gin + c) : 0.f;
+        anyg |= L.Gc[g] != 0.f;
+    }
+    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.mf = 0.f; L.cur = NO_GROUP; L.myg = -1;
+    if (!__any_sync(FULL, anyg)) return;     // dL/dcube vanishes on this ray: no gradient
+    const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
+    const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
+    float4 *grad = P.ws.grad + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
+    // upper bound of the source function anywhere on the grid (S grows with T)
+    const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + 4)), 1.0f);
+    const float nsmax = -G.sunit * 1.0001f / (ex2_approx(Ln.T0l2 / tmax) - 1.0f);
+    const float kthr = P.opt_skip_empty ? K2_EMPTY : 0.f;    // the forward's own test for an emitting step
+    PreCtx pc;
+    pre_setup<KIND>(P, G, rc, pc);
+    const unsigned lt = (1u << lane) - 1u;
+    unsigned n_steps = 0, n_mufu = 0;
+    int ncand = 0, kb = rc.k_lo & ~31;
+    while (true) {
+        while (ncand < 32 && kb < rc.k_hi) {
+            const int k = kb + lane;
+            const bool cnd = k >= rc.k_lo && k < rc.k_hi && prefilter<KIND>(P, pc, occ, k);
+            const unsigned m = __ballot_sync(FULL, cnd);
+            if (cnd) S.cand[ncand + __popc(m & lt)] = k;
+            ncand += __popc(m);
+            kb += 32;
+        }
+        if (ncand == 0) break;
+        __syncwarp();
+        const int n = min(ncand, 32);
+        const int k = lane < n ? S.cand[lane] : P.nstep;
+        const int kx = lane + 32 < ncand ? S.cand[lane + 32] : 0;
+        __syncwarp();
+        if (lane + 32 < ncand) S.cand[lane] = kx;
+        ncand -= n;
+
+        StepState st;
+        phase_a<KIND, false, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, k, st);
+        const bool isE = st.inside && st.K2 > kthr;
+        // zero-opacity steps still carry dL/dn when the grid stores n itself (LINEAR)
+        const bool act = st.inside && (isE || P.grid.dens_mode == 0) && st.whi >= 0 && st.wlo < nchan;
+        const float K2e = isE ? st.K2 : 0.f;
+        n_steps += __popc(__ballot_sync(FULL, act));
+        bool wide;
+        int pos;
+        int npairs = write_entries(S, lane, act, -1, st, K2e, wide, pos);
+        const int npass = wide ? NG : 1;
+        float4 sm = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int p = 0; p < npass; ++p) {
+            bool a = act;
+            if (wide) {
+                bool w2;
+                a = act && st.wlo <= 32 * p + 31 && st.whi >= 32 * p;
+                npairs = write_entries(S, lane, a, 32 * p, st, K2e, w2, pos);
+            }
+            if (npairs == 0) continue;
+            // pairs that hold an emitting step
+            const unsigned emask = __ballot_sync(FULL, lane < npairs && (S.b[lane].x > 0.f || S.b[lane].y > 0.f));
+            for (int base = 0; base < npairs; base += BWD_SUB) {
+                const int nb = min(BWD_SUB, npairs - base);
+                const bool anyE = (emask >> base) & ((1u << BWD_SUB) - 1u);
+                for (int jj = 0; jj < nb; ++jj) {
+                    const int i = base + jj;
+                    const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
+                    const int clo = __float_as_int(qc.z);
+                    if (clo != L.cur) L.regroup(clo, lane, nchan);
+                    if ((emask >> i) & 1u) {
+                        bwd_pair_e<NG>(qa, qb, qc, L, nsmax, sh[warp].red[jj], lane);
+                        n_mufu += 4;
+                    } else {
+                        bwd_pair_z<NG>(qa, qb, qc, L, nsmax, sh[warp].red[jj], lane, anyE);
+                        n_mufu += 2;
+                    }
+                }
+                __syncwarp();
+                if (anyE) reduce_pairs<false>(sh[warp].red, nb, &sh[warp].sum[2 * base], lane);
+                else reduce_pairs<true>(sh[warp].red, nb, &sh[warp].sum[2 * base], lane);
+                __syncwarp();
+            }
+            if (a) {
+                const float4 v = sh[warp].sum[pos];
+                sm.x += v.x; sm.y += v.y; sm.z += v.z; sm.w += v.w;
+            }
+            __syncwarp();
+        }
+        // ---- phase C: chain rule to (n, T, v_phi) at this lane's step, scatter to the grid (O11) ----
+        if (act) phase_c<KIND>(P, st, sm, isE, grad);
+    }
+    if (lane == 0 && n_steps) {
+        atomicAdd(P.ws.counters + 2, (unsigned long long)n_steps);
+        atomicAdd(P.ws.counters + 3, (unsigned long long)n_mufu);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------------------------
+template <int KIND>
+static cudaError_t launch_fwd_w(const MarchParams &P, int nbatch, cudaStream_t st)
+{
+    dim3 grid(P.tiles_x * P.tiles_y, nbatch);
+    const int ng = P.line.ngroups, nt = RADT_WARPS_PER_CTA * 32;
+    if (ng <= 1) k_march_fwd_w<KIND, 1><<<grid, nt, 0, st>>>(P);
+    else if (ng <= 2) k_march_fwd_w<KIND, 2><<<grid, nt, 0, st>>>(P);
+    else if (ng <= 4) k_march_fwd_w<KIND, 4><<<grid, nt, 0, st>>>(P);
+    else k_march_fwd_w<KIND, 8><<<grid, nt, 0, st>>>(P);
+    return cudaGetLastError();
+}
+
+cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
+{
+    return P.grid.kind == 0 ? launch_fwd_w<0>(P, nbatch, st) : launch_fwd_w<1>(P, nbatch, st);
+}
+
+template <int KIND>
+static cudaError_t launch_bwd_w(const MarchParams &P, int nbatch, cudaStream_t st)
+{
+    dim3 grid(P.tiles_x * P.tiles_y, nbatch);
+    const int ng = P.line.ngroups, nt = RADT_WARPS_PER_CTA * 32;
+    if (ng <= 1) k_march_bwd_w<KIND, 1><<<grid, nt, 0, st>>>(P);
+    else if (ng <= 2) k_march_bwd_w<KIND, 2><<<grid, nt, 0, st>>>(P);
+    else if (ng <= 4) k_march_bwd_w<KIND, 4><<<grid, nt, 0, st>>>(P);
+    else k_march_bwd_w<KIND, 8><<<grid, nt, 0, st>>>(P);
+    return cudaGetLastError();
+}
+
+cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
+{
+    return P.grid.kind == 0 ? launch_bwd_w<0>(P, nbatch, st) : launch_bwd_w<1>(P, nbatch, st);
+}

@@ -68,9 +68,10 @@ __device__ __forceinline__ RayRec clip_ray(const DevGeom &G, const DevGrid &g, i
     return rr;
 }
 
-// Block roles: [0, nb_rays) rays; [nb_rays, nb_rays + nb_tab) tables; the rest pack fields.
+// Block roles: [0, nb_rays) rays; then nb_tab blocks of tables; then nb_occ blocks of occupancy words; the rest
+// pack fields.
 __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupParams P, const __grid_constant__ LevelTable L,
-                                               const __grid_constant__ ChanTable V, int nb_rays, int nb_tab)
+                                               const __grid_constant__ ChanTable V, int nb_rays, int nb_tab, int nb_occ)
 {
     int blk = blockIdx.x;
     if (blk < nb_rays) {
@@ -111,14 +112,39 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
             // node radii of the log-spaced axis, r_i = r_min (r_max/r_min)^(i/(nr-1))
             double ri = exp2((double)t * P.grid.lg2_ratio / (double)(P.grid.n0 - 1)) / P.grid.inv_rmin;
             if (t == 0) ri = 1.0 / P.grid.inv_rmin;
-            P.ws.rnode[t] = make_double2(ri, 1.0 / ri);
+            P.ws.rnode[t] = make_double2(ri, 1.0 / (ri * ri));
         }
         return;
     }
     blk -= nb_tab;
+    if (blk < nb_occ) {
+        // Occupancy bitmap of the (r, zeta) grid for the march prefilter: bit j of word (i, j / 32) is set when
+        // some node of the 4 x 4 block around cell (i, j) -- the corners of the cell and of its eight
+        // neighbours -- stores a density that can emit (or is NaN).  occ_thr = -inf gives all ones.
+        long long t = (long long)blk * blockDim.x + threadIdx.x;
+        if (t >= (long long)P.occ_words * P.nbatch) return;
+        int b = (int)(t / P.occ_words);
+        int w = (int)(t - (long long)b * P.occ_words);
+        int i = w / P.occ_wpr, jw = w - i * P.occ_wpr;
+        const float *dn = P.dens + (long long)(P.b0 + b) * P.batch_stride;
+        unsigned long long m = 0ull;
+        for (int di = -1; di <= 2; ++di) {
+            int ii = i + di;
+            if (ii < 0 || ii >= P.grid.n0) continue;
+            for (int tt = 0; tt < 35; ++tt) {
+                int jj = jw * 32 - 1 + tt;
+                if (jj < 0 || jj >= P.grid.n1) continue;
+                if (!(__ldg(dn + (long long)ii * P.grid.n1 + jj) <= P.occ_thr)) m |= 1ull << tt;
+            }
+        }
+        m |= (m >> 1) | (m >> 2) | (m >> 3);
+        P.ws.occ[(size_t)(P.b0 + b) * P.occ_words + w] = (unsigned)m;
+        return;
+    }
+    blk -= nb_occ;
     // pack SoA planes into float4 cells {dens, temp, vel, 0}; optionally zero the gradient cells
     long long total = P.grid.cells * P.nbatch;
-    long long stride = (long long)(gridDim.x - nb_rays - nb_tab) * blockDim.x;
+    long long stride = (long long)(gridDim.x - nb_rays - nb_tab - nb_occ) * blockDim.x;
     float tmax = 0.f;
     for (long long q = (long long)blk * blockDim.x + threadIdx.x; q < total; q += stride) {
         int b = (int)(q / P.grid.cells);
@@ -197,9 +223,10 @@ cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const C
         long long nb = (total + 255) / 256;
         nb_pack = (int)(nb < 148 * 16 ? nb : 148 * 16);
     }
-    int nb = nb_rays + nb_tab + nb_pack;
+    int nb_occ = P.do_occ ? (int)(((long long)P.occ_words * P.nbatch + 255) / 256) : 0;
+    int nb = nb_rays + nb_tab + nb_occ + nb_pack;
     if (nb == 0) return cudaSuccess;
-    k_setup<<<nb, 256, 0, st>>>(P, L, V, nb_rays, nb_tab);
+    k_setup<<<nb, 256, 0, st>>>(P, L, V, nb_rays, nb_tab, nb_occ);
     return cudaGetLastError();
 }
 

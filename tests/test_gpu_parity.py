@@ -16,13 +16,18 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 
-@pytest.fixture(scope="module")
-def rt():
+@pytest.fixture(scope="module", params=["win", "tab"])
+def rt(request):
+    """Every test runs on both kernel families: `win` (uniform channel lattice: one channel per lane inside the
+    line window; the default) and `tab` (channel-table kernels, which also serve non-uniform channel tables)."""
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_2509_03623_b200 as pkg
-    pkg.binding.lib()     # fails loudly if the CUDA library was not built
-    return pkg
+    B = pkg.binding
+    B.lib()     # fails loudly if the CUDA library was not built
+    B.radt_set_option(B.OPT_WIN_PATH, 1 if request.param == "win" else 0)
+    yield pkg
+    B.radt_set_option(B.OPT_WIN_PATH, 1)
 
 
 def _as_list(s):
