@@ -178,6 +178,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()
+    B.radt_set_option(B.OPT_WIN_PATH, args.win_path)
 
     scenes = _scenes(args.config)
     R = Renderer(scenes, device=f"cuda:{local}")
@@ -307,7 +308,8 @@ def run_ours(args):
         "config": {"workload": _workload_name(args.config), "rays": int(sum(s.nrays for s in scenes)),
                    "channels": d.nchan, "steps_per_ray": d.nstep, "grid": list(d.grid_shape),
                    "nominal_samples_per_step": int(nominal), "parallelism": f"independent disks x{world}",
-                   "l2": "flushed between timed steps (256 MiB fill outside the events)"},
+                   "l2": "flushed between timed steps (256 MiB fill outside the events)",
+                   "kernels": "window (uniform channel lattice)" if args.win_path else "channel table"},
         "fwd_value": nominal / (t_fwd * 1e-3), "fwd_ms": t_fwd, "l2_ms": t_l2, "bwd_ms": t_bwd,
         "executed_samples": {"fwd": int(fwd_exec), "bwd": int(bwd_exec), "fwd_active_ray_steps": int(cnt[0]),
                              "bwd_active_ray_steps": int(cnt_b[2]), "nominal": int(nominal)},
@@ -333,6 +335,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="SURVEY.md config 1..5 (BASELINE.json configs[k-1])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--win-path", type=int, default=1, choices=[0, 1],
+                    help="RADT_OPT_WIN_PATH: 1 = window kernels on uniform channel lattices (default), 0 = channel-table kernels")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -233,6 +233,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_fwd_w(cons
             int pos;
             int npairs = write_entries(S, lane, act, -1, st, st.K2, wide, pos);
             const int npass = wide ? NG : 1;
+#pragma unroll 1
             for (int p = 0; p < npass; ++p) {
                 if (wide) {
                     bool w2;
@@ -450,6 +451,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(cons
         int npairs = write_entries(S, lane, act, -1, st, K2e, wide, pos);
         const int npass = wide ? NG : 1;
         float4 sm = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 1
         for (int p = 0; p < npass; ++p) {
             bool a = act;
             if (wide) {
@@ -460,9 +462,11 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(cons
             if (npairs == 0) continue;
             // pairs that hold an emitting step
             const unsigned emask = __ballot_sync(FULL, lane < npairs && (S.b[lane].x > 0.f || S.b[lane].y > 0.f));
+#pragma unroll 1
             for (int base = 0; base < npairs; base += BWD_SUB) {
                 const int nb = min(BWD_SUB, npairs - base);
                 const bool anyE = (emask >> base) & ((1u << BWD_SUB) - 1u);
+#pragma unroll 1
                 for (int jj = 0; jj < nb; ++jj) {
                     const int i = base + jj;
                     const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
