@@ -20,7 +20,7 @@
 struct __align__(16) WinShared {          // per warp
     float4 a[WIN_PAIRS];                  // {u0_a, u0_b, dvA_a, dvA_b}
     float4 b[WIN_PAIRS];                  // {K2_a, K2_b, S_a, S_b}
-    float4 c[WIN_PAIRS];                  // {off_a, off_b, bits of c_lo, -}   off = c_lo - c_ref
+    float4 c[WIN_PAIRS];                  // {c_ref_a, c_ref_b, bits of u_lo, bits of u_hi}: union window of the pair
     int cand[64];                         // candidate step indices waiting for phase A
     int2 win[32];                         // channel windows of the compacted steps
 };
@@ -76,19 +76,11 @@ __device__ __forceinline__ bool prefilter(const MarchParams &P, const PreCtx &pc
     }
 }
 
-// Group of a step whose conservative window is [wlo, whi] (width <= 32): c_lo = wlo rounded down to a multiple
-// of q, with q the largest power of two that still keeps whi < c_lo + 32.  Consecutive steps of one crossing of
-// the emitting layer then share c_lo, and the lanes keep their channel.
-__device__ __forceinline__ int group_of(int wlo, int ww)
-{
-    int q = ww <= 17 ? 16 : ww <= 25 ? 8 : ww <= 29 ? 4 : ww <= 31 ? 2 : 1;
-    return wlo & -q;
-}
-
-// Compact the active steps of this batch (march order) into slot pairs {2i, 2i+1}.  The two steps of a pair share
-// one group, chosen for the union of their windows; an odd count is completed with a no-op entry (K2 = 0).
-// Returns the number of pairs; `wide` tells that some pair's union is wider than 32 channels (the caller then
-// runs one pass per fixed 32-channel block, `blk` >= 0).
+// Compact the active steps of this batch (march order) into slot pairs {2i, 2i+1}.  A pair is evaluated in ONE
+// 32-channel group that must contain the union [ulo, uhi] of its two line windows; the group itself is chosen in
+// phase B (hysteresis: the lanes keep their channels while the union still fits).  An odd count is completed with a
+// no-op entry (K2 = 0).  Returns the number of pairs; `wide` tells that some pair's union is wider than 32
+// channels (the caller then runs one pass per fixed 32-channel block, `blk` >= 0).
 __device__ __forceinline__ int write_entries(WinShared &S, int lane, bool act, int blk, const StepState &st, float K2,
                                          bool &wide, int &pos_out)
 {
@@ -98,28 +90,27 @@ __device__ __forceinline__ int write_entries(WinShared &S, int lane, bool act, i
     const int cnt = __popc(mask);
     const int pos = __popc(mask & ((1u << lane) - 1u));
     pos_out = pos;
-    int clo = blk;
+    int ulo = blk, uhi = blk + 31;
     if (blk < 0) {
         if (act) S.win[pos] = make_int2(st.wlo, st.whi);
         __syncwarp();
-        int ulo = st.wlo, uhi = st.whi;
+        ulo = st.wlo; uhi = st.whi;
         if (act && (pos ^ 1) < cnt) {
             const int2 pw = S.win[pos ^ 1];
             ulo = min(ulo, pw.x); uhi = max(uhi, pw.y);
         }
-        const int uw = uhi - ulo + 1;
-        wide = __any_sync(FULL, act && uw > 32);
+        wide = __any_sync(FULL, act && uhi - ulo > 31);
         if (wide) return 0;
-        clo = group_of(ulo, uw);
     }
     float *fa = reinterpret_cast<float *>(S.a), *fb = reinterpret_cast<float *>(S.b), *fc = reinterpret_cast<float *>(S.c);
     if (act) {
         const int q = (pos >> 1) * 4 + (pos & 1);
         fa[q] = st.u0; fa[q + 2] = st.dvA;
         fb[q] = K2; fb[q + 2] = st.S;
-        fc[q] = (float)(clo - st.cref);
+        fc[q] = (float)st.cref;
         if (!(pos & 1)) {
-            fc[q + 2] = __int_as_float(clo);
+            fc[q + 2] = __int_as_float(ulo);
+            fc[q + 3] = __int_as_float(uhi);
             if (pos == cnt - 1) { fa[q + 1] = 0.f; fa[q + 3] = 0.f; fb[q + 1] = 0.f; fb[q + 3] = 0.f; fc[q + 1] = 0.f; }
         }
     }
@@ -127,53 +118,53 @@ __device__ __forceinline__ int write_entries(WinShared &S, int lane, bool act, i
     return (cnt + 1) >> 1;
 }
 
-// Per-lane channel state of the window march: (I, T) of all the lane's channels c = lane + 32 g, and the pair
-// (Is, Ts) of the one channel the lane serves in the current group [cur, cur + 32).
-template <int NG>
+// The pair's union window [ulo, uhi] no longer fits the current group [cur, cur + 32)?
+__device__ __forceinline__ bool group_misses(int cur, int ulo, int uhi) { return ulo < cur || uhi > cur + 31; }
+// New group for that union: centred, so that the line can drift either way before the lanes change channel again.
+__device__ __forceinline__ int group_for(int ulo, int uhi) { return ulo - ((31 - (uhi - ulo)) >> 1); }
+
+// Per-lane channel state of the forward window march.  The (I, T) of all channels of the ray live in shared
+// memory (channel c is only ever touched by lane c & 31); the lane keeps the pair of the ONE channel it serves in
+// the current group [cur, cur + 32) in registers.
 struct LaneState {
-    float I[NG], T[NG];
-    float Is, Ts, mf;
-    int cur, myg;
-    __device__ __forceinline__ void init()
+    float Is, Ts, cf;
+    int cur, myc;
+    float *sI, *sT;
+    __device__ __forceinline__ void init(float *sI_, float *sT_, int lane, int ng)
     {
-#pragma unroll
-        for (int g = 0; g < NG; ++g) { I[g] = 0.f; T[g] = 1.f; }
-        Is = 0.f; Ts = 1.f; mf = 0.f; cur = NO_GROUP; myg = -1;
+        sI = sI_; sT = sT_;
+        for (int g = 0; g < ng; ++g) { sI[lane + 32 * g] = 0.f; sT[lane + 32 * g] = 1.f; }
+        Is = 0.f; Ts = 1.f; cf = 0.f; cur = NO_GROUP; myc = -1;
     }
     __device__ __forceinline__ void put_back()
     {
-#pragma unroll
-        for (int g = 0; g < NG; ++g)
-            if (myg == g) { I[g] = Is; T[g] = Ts; }
+        if (myc >= 0) { sI[myc] = Is; sT[myc] = Ts; }
     }
     // the group moved: put the lane's channel state back, take the new channel's
     __device__ __forceinline__ void regroup(int clo, int lane, int nchan)
     {
         put_back();
-        const int m = (lane - clo) & 31, c = clo + m;
-        myg = (unsigned)c < (unsigned)nchan ? (c >> 5) : -1;
-        mf = (float)m;
+        const int c = clo + ((lane - clo) & 31);
+        myc = (unsigned)c < (unsigned)nchan ? c : -1;
+        cf = (float)c;
         Is = 0.f; Ts = 1.f;
-#pragma unroll
-        for (int g = 0; g < NG; ++g)
-            if (myg == g) { Is = I[g]; Ts = T[g]; }
+        if (myc >= 0) { Is = sI[c]; Ts = sT[c]; }
         cur = clo;
     }
 };
 
-// u' of the lane's channel for the two steps of a pair
-__device__ __forceinline__ f2 pair_u_win(const float4 &qa, const float4 &qc, float mf)
+// u' of the lane's channel (cf, as a float) for the two steps of a pair: u'(c) = u0 + (c - c_ref) dvA
+__device__ __forceinline__ f2 pair_u_win(const float4 &qa, const float4 &qc, float cf)
 {
-    return fma2(add2(pk1(mf), pk(qc.x, qc.y)), pk(qa.z, qa.w), pk(qa.x, qa.y));
+    return fma2(sub2(pk1(cf), pk(qc.x, qc.y)), pk(qa.z, qa.w), pk(qa.x, qa.y));
 }
 
 // O9 for the two steps of a pair, in march order.  c = S ((1-e) T) and I += c with fixed roundings: the adjoint
 // re-march repeats exactly this sequence and so reproduces the partial sums bit for bit.
-__device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, const float4 &qc, f2 K2, float mf, float &Is,
-                                         float &Ts)
+__device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, const float4 &qc, float cf, float &Is, float &Ts)
 {
     Pair s;
-    pair_eval(pair_u_win(qa, qc, mf), K2, s);
+    pair_eval(pair_u_win(qa, qc, cf), pk(qb.x, qb.y), s);
     float om0, om1, e0, e1;
     upk(s.om, om0, om1);
     upk(s.e, e0, e1);
@@ -183,47 +174,68 @@ __device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, con
     Ts = __fmul_rn(Ts, e1);
 }
 
+// Candidate steps of the ray, compacted over 32-step blocks: fills S.cand until it holds >= 32 or the ray ends.
+template <int KIND>
+__device__ __forceinline__ void gather_candidates(const MarchParams &P, const PreCtx &pc, const unsigned *occ, WinShared &S,
+                                                  const RayCtx &rc, int lane, int &ncand, int &kb)
+{
+    const unsigned lt = (1u << lane) - 1u;
+    while (ncand < 32 && kb < rc.k_hi) {
+        const int k = kb + lane;
+        const bool cnd = k >= rc.k_lo && k < rc.k_hi && prefilter<KIND>(P, pc, occ, k);
+        const unsigned m = __ballot_sync(FULL, cnd);
+        if (cnd) S.cand[ncand + __popc(m & lt)] = k;
+        ncand += __popc(m);
+        kb += 32;
+    }
+}
+
+// Take up to 32 candidates (march order) out of S.cand; lanes beyond the count get k = nstep (outside).
+__device__ __forceinline__ int take_candidates(WinShared &S, int lane, int &ncand, int nstep)
+{
+    __syncwarp();
+    const int n = min(ncand, 32);
+    const int k = lane < n ? S.cand[lane] : nstep;
+    const int kx = lane + 32 < ncand ? S.cand[lane + 32] : 0;
+    __syncwarp();
+    if (lane + 32 < ncand) S.cand[lane] = kx;
+    ncand -= n;
+    return k;
+}
+
+extern __shared__ __align__(16) unsigned char win_smem[];
+
 // ---------------------------------------------------------------------------------------------
-// K2 / K3 forward march, NG = ceil(nchan / 32) rounded up to {1, 2, 4, 8}
+// K2 / K3 forward march.  Dynamic shared memory per warp: WinShared + (I, T) of 32 ngroups channels.
 // ---------------------------------------------------------------------------------------------
-template <int KIND, int NG>
+static size_t fwd_warp_bytes(int ng) { return sizeof(WinShared) + (size_t)ng * 256; }
+
+template <int KIND>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_fwd_w(const __grid_constant__ MarchParams P)
 {
-    __shared__ WinShared sh[RADT_WARPS_PER_CTA];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     RayCtx rc;
     if (!ray_setup(P, rc, warp)) return;
-    WinShared &S = sh[warp];
+    const int ng = P.line.ngroups;
+    unsigned char *base = win_smem + (size_t)warp * (sizeof(WinShared) + (size_t)ng * 256);
+    WinShared &S = *reinterpret_cast<WinShared *>(base);
+    float *sI = reinterpret_cast<float *>(base + sizeof(WinShared)), *sT = sI + 32 * ng;
     const DevGeom &G = P.geom[rc.b];
     const int nchan = P.line.nchan;
     float *out = P.cube + rc.ray * (size_t)nchan;
-    LaneState<NG> L;
-    L.init();
+    LaneState L;
+    L.init(sI, sT, lane, ng);
     unsigned n_steps = 0, n_mufu = 0;
     if (rc.ds != 0.0) {
         const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
         const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
         PreCtx pc;
         pre_setup<KIND>(P, G, rc, pc);
-        const unsigned lt = (1u << lane) - 1u;
         int ncand = 0, kb = rc.k_lo & ~31;
         while (true) {
-            while (ncand < 32 && kb < rc.k_hi) {
-                const int k = kb + lane;
-                const bool cnd = k >= rc.k_lo && k < rc.k_hi && prefilter<KIND>(P, pc, occ, k);
-                const unsigned m = __ballot_sync(FULL, cnd);
-                if (cnd) S.cand[ncand + __popc(m & lt)] = k;
-                ncand += __popc(m);
-                kb += 32;
-            }
+            gather_candidates<KIND>(P, pc, occ, S, rc, lane, ncand, kb);
             if (ncand == 0) break;
-            __syncwarp();
-            const int n = min(ncand, 32);
-            const int k = lane < n ? S.cand[lane] : P.nstep;
-            const int kx = lane + 32 < ncand ? S.cand[lane + 32] : 0;
-            __syncwarp();
-            if (lane + 32 < ncand) S.cand[lane] = kx;
-            ncand -= n;
+            const int k = take_candidates(S, lane, ncand, P.nstep);
 
             StepState st;
             phase_a<KIND, true, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, k, st);
@@ -232,7 +244,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_fwd_w(cons
             bool wide;
             int pos;
             int npairs = write_entries(S, lane, act, -1, st, st.K2, wide, pos);
-            const int npass = wide ? NG : 1;
+            const int npass = wide ? ng : 1;
 #pragma unroll 1
             for (int p = 0; p < npass; ++p) {
                 if (wide) {
@@ -243,9 +255,9 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_fwd_w(cons
 #pragma unroll 2
                 for (int i = 0; i < npairs; ++i) {
                     const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
-                    const int clo = __float_as_int(qc.z);
-                    if (clo != L.cur) L.regroup(clo, lane, nchan);
-                    fwd_pair(qa, qb, qc, pk(qb.x, qb.y), L.mf, L.Is, L.Ts);
+                    const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
+                    if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
+                    fwd_pair(qa, qb, qc, L.cf, L.Is, L.Ts);
                 }
                 n_mufu += 4 * npairs;
                 __syncwarp();
@@ -253,10 +265,9 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_fwd_w(cons
         }
         L.put_back();
     }
-#pragma unroll
-    for (int g = 0; g < NG; ++g) {
+    for (int g = 0; g < ng; ++g) {
         const int c = lane + 32 * g;
-        if (c < nchan) out[c] = L.I[g];
+        if (c < nchan) out[c] = sI[c];
     }
     if (lane == 0 && n_steps) {
         atomicAdd(P.ws.counters + 0, (unsigned long long)n_steps);
@@ -273,27 +284,25 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_fwd_w(cons
 // ---------------------------------------------------------------------------------------------
 #define BWD_SUB 4            // pairs per reduction batch
 
-template <int NG>
+// Per-lane channel state of the adjoint window march: transmittance and partial sum of all channels live in shared
+// memory; the saved intensity and dL/dI of the served channel are re-read (L1) when the group moves.
 struct BwdLane {
-    float T[NG], Pp[NG], Isv[NG], Gc[NG];
-    float Ts, Ps, Is, Gs, mf;                     // transmittance, partial sum, saved I, dL/dI of the served channel
-    int cur, myg;
+    float Ts, Ps, Is, Gs, cf;                     // transmittance, partial sum, saved I, dL/dI of the served channel
+    int cur, myc;
+    float *sT, *sP;
+    const float *Isave, *Gin;
     __device__ __forceinline__ void put_back()
     {
-#pragma unroll
-        for (int g = 0; g < NG; ++g)
-            if (myg == g) { T[g] = Ts; Pp[g] = Ps; }
+        if (myc >= 0) { sT[myc] = Ts; sP[myc] = Ps; }
     }
     __device__ __forceinline__ void regroup(int clo, int lane, int nchan)
     {
         put_back();
-        const int m = (lane - clo) & 31, c = clo + m;
-        myg = (unsigned)c < (unsigned)nchan ? (c >> 5) : -1;
-        mf = (float)m;
+        const int c = clo + ((lane - clo) & 31);
+        myc = (unsigned)c < (unsigned)nchan ? c : -1;
+        cf = (float)c;
         Ts = 1.f; Ps = 0.f; Is = 0.f; Gs = 0.f;    // lanes without a channel contribute nothing (G = 0)
-#pragma unroll
-        for (int g = 0; g < NG; ++g)
-            if (myg == g) { Ts = T[g]; Ps = Pp[g]; Is = Isv[g]; Gs = Gc[g]; }
+        if (myc >= 0) { Ts = sT[c]; Ps = sP[c]; Is = __ldg(Isave + c); Gs = __ldg(Gin + c); }
         cur = clo;
     }
 };
@@ -303,12 +312,11 @@ typedef float2 RedBuf[BWD_SUB][4][32];           // [pair][quantity][lane] {step
 __device__ __forceinline__ float2 f2_as_float2(f2 v) { float a, b; upk(v, a, b); return make_float2(a, b); }
 
 // A pair with at least one emitting step.  Repeats the forward's O9 sequence bit for bit (fwd_pair).
-template <int NG>
-__device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane<NG> &L,
+__device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane &L,
                                            float nsmax, float2 (*red)[32], int lane)
 {
     Pair s;
-    pair_eval(pair_u_win(qa, qc, L.mf), pk(qb.x, qb.y), s);
+    pair_eval(pair_u_win(qa, qc, L.cf), pk(qb.x, qb.y), s);
     float om0, om1, e0, e1;
     upk(s.om, om0, om1);
     upk(s.e, e0, e1);
@@ -330,11 +338,10 @@ __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, c
 }
 
 // A pair of zero-opacity steps: T, P and hence G T and G R stay fixed; only sum w is needed.
-template <int NG>
-__device__ __forceinline__ void bwd_pair_z(const float4 &qa, const float4 &qb, const float4 &qc, const BwdLane<NG> &L,
+__device__ __forceinline__ void bwd_pair_z(const float4 &qa, const float4 &qb, const float4 &qc, const BwdLane &L,
                                            float nsmax, float2 (*red)[32], int lane, bool zero_rest)
 {
-    const f2 u = pair_u_win(qa, qc, L.mf);
+    const f2 u = pair_u_win(qa, qc, L.cf);
     float t0, t1;
     upk(mul2(u, u), t0, t1);
     const f2 g = pk(ex2_approx(-t0), ex2_approx(-t1));
@@ -376,38 +383,38 @@ __device__ __forceinline__ void reduce_pairs(const RedBuf &red, int nb, float4 *
     }
 }
 
-struct __align__(16) BwdShared {          // per warp
+struct __align__(16) BwdShared {          // per warp, followed by (T, P) of 32 ngroups channels
     WinShared w;
     RedBuf red;
     float4 sum[32];                       // channel sums of the compacted steps
 };
+static size_t bwd_warp_bytes(int ng) { return sizeof(BwdShared) + (size_t)ng * 256; }
 
-template <int KIND, int NG>
+template <int KIND>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(const __grid_constant__ MarchParams P)
 {
-    __shared__ BwdShared sh[RADT_WARPS_PER_CTA];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     RayCtx rc;
     if (!ray_setup(P, rc, warp)) return;
     if (rc.ds == 0.0) return;
-    WinShared &S = sh[warp].w;
+    const int ng = P.line.ngroups;
+    unsigned char *base = win_smem + (size_t)warp * (sizeof(BwdShared) + (size_t)ng * 256);
+    BwdShared &B = *reinterpret_cast<BwdShared *>(base);
+    WinShared &S = B.w;
     const DevGeom &G = P.geom[rc.b];
     const DevLine &Ln = P.line;
     const int nchan = Ln.nchan;
-    const float *Isave = P.cube + rc.ray * (size_t)nchan;
-    const float *Gin = P.dl_dcube + rc.ray * (size_t)nchan;
-    BwdLane<NG> L;
+    BwdLane L;
+    L.sT = reinterpret_cast<float *>(base + sizeof(BwdShared)); L.sP = L.sT + 32 * ng;
+    L.Isave = P.cube + rc.ray * (size_t)nchan;
+    L.Gin = P.dl_dcube + rc.ray * (size_t)nchan;
     bool anyg = false;
-#pragma unroll
-    for (int g = 0; g < NG; ++g) {
+    for (int g = 0; g < ng; ++g) {
         const int c = lane + 32 * g;
-        const bool ok = c < nchan;
-        L.T[g] = 1.f; L.Pp[g] = 0.f;
-        L.Isv[g] = ok ? __ldg(Isave + c) : 0.f;
-        L.Gc[g] = ok ? __ldg(Gin + c) : 0.f;
-        anyg |= L.Gc[g] != 0.f;
+        L.sT[c] = 1.f; L.sP[c] = 0.f;
+        anyg |= c < nchan && __ldg(L.Gin + c) != 0.f;
     }
-    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.mf = 0.f; L.cur = NO_GROUP; L.myg = -1;
+    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.cf = 0.f; L.cur = NO_GROUP; L.myc = -1;
     if (!__any_sync(FULL, anyg)) return;     // dL/dcube vanishes on this ray: no gradient
     const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
@@ -418,26 +425,12 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(cons
     const float kthr = P.opt_skip_empty ? K2_EMPTY : 0.f;    // the forward's own test for an emitting step
     PreCtx pc;
     pre_setup<KIND>(P, G, rc, pc);
-    const unsigned lt = (1u << lane) - 1u;
     unsigned n_steps = 0, n_mufu = 0;
     int ncand = 0, kb = rc.k_lo & ~31;
     while (true) {
-        while (ncand < 32 && kb < rc.k_hi) {
-            const int k = kb + lane;
-            const bool cnd = k >= rc.k_lo && k < rc.k_hi && prefilter<KIND>(P, pc, occ, k);
-            const unsigned m = __ballot_sync(FULL, cnd);
-            if (cnd) S.cand[ncand + __popc(m & lt)] = k;
-            ncand += __popc(m);
-            kb += 32;
-        }
+        gather_candidates<KIND>(P, pc, occ, S, rc, lane, ncand, kb);
         if (ncand == 0) break;
-        __syncwarp();
-        const int n = min(ncand, 32);
-        const int k = lane < n ? S.cand[lane] : P.nstep;
-        const int kx = lane + 32 < ncand ? S.cand[lane + 32] : 0;
-        __syncwarp();
-        if (lane + 32 < ncand) S.cand[lane] = kx;
-        ncand -= n;
+        const int k = take_candidates(S, lane, ncand, P.nstep);
 
         StepState st;
         phase_a<KIND, false, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, k, st);
@@ -449,7 +442,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(cons
         bool wide;
         int pos;
         int npairs = write_entries(S, lane, act, -1, st, K2e, wide, pos);
-        const int npass = wide ? NG : 1;
+        const int npass = wide ? ng : 1;
         float4 sm = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
         for (int p = 0; p < npass; ++p) {
@@ -463,30 +456,30 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(cons
             // pairs that hold an emitting step
             const unsigned emask = __ballot_sync(FULL, lane < npairs && (S.b[lane].x > 0.f || S.b[lane].y > 0.f));
 #pragma unroll 1
-            for (int base = 0; base < npairs; base += BWD_SUB) {
-                const int nb = min(BWD_SUB, npairs - base);
-                const bool anyE = (emask >> base) & ((1u << BWD_SUB) - 1u);
+            for (int base_i = 0; base_i < npairs; base_i += BWD_SUB) {
+                const int nb = min(BWD_SUB, npairs - base_i);
+                const bool anyE = (emask >> base_i) & ((1u << BWD_SUB) - 1u);
 #pragma unroll 1
                 for (int jj = 0; jj < nb; ++jj) {
-                    const int i = base + jj;
+                    const int i = base_i + jj;
                     const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
-                    const int clo = __float_as_int(qc.z);
-                    if (clo != L.cur) L.regroup(clo, lane, nchan);
+                    const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
+                    if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
                     if ((emask >> i) & 1u) {
-                        bwd_pair_e<NG>(qa, qb, qc, L, nsmax, sh[warp].red[jj], lane);
+                        bwd_pair_e(qa, qb, qc, L, nsmax, B.red[jj], lane);
                         n_mufu += 4;
                     } else {
-                        bwd_pair_z<NG>(qa, qb, qc, L, nsmax, sh[warp].red[jj], lane, anyE);
+                        bwd_pair_z(qa, qb, qc, L, nsmax, B.red[jj], lane, anyE);
                         n_mufu += 2;
                     }
                 }
                 __syncwarp();
-                if (anyE) reduce_pairs<false>(sh[warp].red, nb, &sh[warp].sum[2 * base], lane);
-                else reduce_pairs<true>(sh[warp].red, nb, &sh[warp].sum[2 * base], lane);
+                if (anyE) reduce_pairs<false>(B.red, nb, &B.sum[2 * base_i], lane);
+                else reduce_pairs<true>(B.red, nb, &B.sum[2 * base_i], lane);
                 __syncwarp();
             }
             if (a) {
-                const float4 v = sh[warp].sum[pos];
+                const float4 v = B.sum[pos];
                 sm.x += v.x; sm.y += v.y; sm.z += v.z; sm.w += v.w;
             }
             __syncwarp();
@@ -503,36 +496,25 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd_w(cons
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
-template <int KIND>
-static cudaError_t launch_fwd_w(const MarchParams &P, int nbatch, cudaStream_t st)
+template <typename K>
+static cudaError_t launch_w(K kern, const MarchParams &P, int nbatch, size_t warp_bytes, cudaStream_t st)
 {
+    const size_t smem = warp_bytes * RADT_WARPS_PER_CTA;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     dim3 grid(P.tiles_x * P.tiles_y, nbatch);
-    const int ng = P.line.ngroups, nt = RADT_WARPS_PER_CTA * 32;
-    if (ng <= 1) k_march_fwd_w<KIND, 1><<<grid, nt, 0, st>>>(P);
-    else if (ng <= 2) k_march_fwd_w<KIND, 2><<<grid, nt, 0, st>>>(P);
-    else if (ng <= 4) k_march_fwd_w<KIND, 4><<<grid, nt, 0, st>>>(P);
-    else k_march_fwd_w<KIND, 8><<<grid, nt, 0, st>>>(P);
+    kern<<<grid, RADT_WARPS_PER_CTA * 32, smem, st>>>(P);
     return cudaGetLastError();
 }
 
 cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    return P.grid.kind == 0 ? launch_fwd_w<0>(P, nbatch, st) : launch_fwd_w<1>(P, nbatch, st);
-}
-
-template <int KIND>
-static cudaError_t launch_bwd_w(const MarchParams &P, int nbatch, cudaStream_t st)
-{
-    dim3 grid(P.tiles_x * P.tiles_y, nbatch);
-    const int ng = P.line.ngroups, nt = RADT_WARPS_PER_CTA * 32;
-    if (ng <= 1) k_march_bwd_w<KIND, 1><<<grid, nt, 0, st>>>(P);
-    else if (ng <= 2) k_march_bwd_w<KIND, 2><<<grid, nt, 0, st>>>(P);
-    else if (ng <= 4) k_march_bwd_w<KIND, 4><<<grid, nt, 0, st>>>(P);
-    else k_march_bwd_w<KIND, 8><<<grid, nt, 0, st>>>(P);
-    return cudaGetLastError();
+    const size_t wb = fwd_warp_bytes(P.line.ngroups);
+    return P.grid.kind == 0 ? launch_w(k_march_fwd_w<0>, P, nbatch, wb, st) : launch_w(k_march_fwd_w<1>, P, nbatch, wb, st);
 }
 
 cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    return P.grid.kind == 0 ? launch_bwd_w<0>(P, nbatch, st) : launch_bwd_w<1>(P, nbatch, st);
+    const size_t wb = bwd_warp_bytes(P.line.ngroups);
+    return P.grid.kind == 0 ? launch_w(k_march_bwd_w<0>, P, nbatch, wb, st) : launch_w(k_march_bwd_w<1>, P, nbatch, wb, st);
 }
