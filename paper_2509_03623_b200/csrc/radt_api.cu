@@ -185,7 +185,7 @@ void make_dev_line(const radt_line *line, DevLine &d)
 
 struct WsLayout {
     size_t rays, qtab, vcs, rnode, cells, occ, grad, counters, total;
-    int occ_wpr, occ_words;
+    int occ_wpr, occ_words, occ_nbj;
 };
 
 WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass)
@@ -200,8 +200,17 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     w.rnode = off; off = align256(off + (size_t)(grid->kind == RADT_GRID_AXISYM ? grid->n[0] : 1) * sizeof(double2));
     size_t cells = (size_t)grid_cells(grid) * (size_t)batch;
     w.cells = off; off = align256(off + cells * sizeof(float4));
-    w.occ_wpr = grid->kind == RADT_GRID_AXISYM ? (grid->n[1] + 31) / 32 : 1;
-    w.occ_words = grid->kind == RADT_GRID_AXISYM ? grid->n[0] * w.occ_wpr : 1;
+    if (grid->kind == RADT_GRID_AXISYM) {
+        w.occ_wpr = (grid->n[1] + 31) / 32;
+        w.occ_words = grid->n[0] * w.occ_wpr;
+        w.occ_nbj = 1;
+    } else {
+        // 3-D: one bit per block of 4 x 4 x 4 cells
+        int nbi = (grid->n[0] - 1 + 3) / 4, nbj = (grid->n[1] - 1 + 3) / 4, nbl = (grid->n[2] - 1 + 3) / 4;
+        w.occ_wpr = (nbl + 31) / 32;
+        w.occ_nbj = nbj;
+        w.occ_words = nbi * nbj * w.occ_wpr;
+    }
     w.occ = off; off = align256(off + (size_t)w.occ_words * (size_t)batch * sizeof(unsigned));
     w.grad = off;
     if (pass == RADT_PASS_BWD) off = align256(off + cells * sizeof(float4));
@@ -276,9 +285,8 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         // occupancy bitmap for the window kernels' prefilter (axisymmetric grids): with LINEAR densities the
         // adjoint needs every in-grid step (dL/dn of empty cells), so only the forward and LN grids use it
         const bool win = use_win;
-        const bool occ = win && grid->kind == RADT_GRID_AXISYM && g_opt_skip_empty &&
-                         (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN);
-        SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr;
+        const bool occ = win && g_opt_skip_empty && (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN);
+        SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr; SP.occ_nbj = w.occ_nbj;
         SP.occ_thr = grid->dens_mode == RADT_DENS_LN ? -39.1439f : 1e-17f;     // N_EMPTY of the march kernels
         SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;
         CUDA_TRY(radt_launch_setup(SP, LT, CT, st));
@@ -300,7 +308,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
                 if ((double)(float)vv != vv) { MP.chan_lo = 1; break; }
             }
         MP.cube = cube; MP.dl_dcube = dl_dcube;
-        MP.use_win = win; MP.use_occ = occ; MP.occ_words = w.occ_words; MP.occ_wpr = w.occ_wpr;
+        MP.use_win = win; MP.use_occ = occ; MP.occ_words = w.occ_words; MP.occ_wpr = w.occ_wpr; MP.occ_nbj = w.occ_nbj;
         if (pass == RADT_PASS_FWD && win) CUDA_TRY(radt_launch_march_fwd_win(MP, nb, st));
         else if (pass == RADT_PASS_FWD) CUDA_TRY(radt_launch_march_fwd(MP, nb, st));
         else if (win) CUDA_TRY(radt_launch_march_bwd_win(MP, nb, st));

@@ -79,7 +79,8 @@ struct DevWs {
     double2 *rnode;        // [nr] {r_i, 1/r_i^2} node radii of the log-spaced axis (axisym), fp64
     float4 *cells;         // [batch][cells] packed {dens, temp, vel, 0}
     float4 *grad;          // [batch][cells] packed gradient accumulators {dens, temp, vel, -} (bwd only)
-    unsigned *occ;         // [batch][occ_words] bit (i, j): some cell within one cell of (i, j) can emit (axisym)
+    unsigned *occ;         // [batch][occ_words] axisym: bit (i, j): some cell within one cell of (i, j) can emit;
+                           // 3-D: one bit per block of 4 x 4 x 4 cells, same dilation (radt_setup.cu)
     unsigned long long *counters;   // [8] 0-3 work counters; [4] bits of the grid's maximum temperature
 };
 
@@ -95,7 +96,8 @@ struct MarchParams {
     int chan_lo;           // some channel velocity is not exactly representable in fp32: use the lo parts
     int use_win;           // uniform-channel window kernels (radt_march_win.cu)
     int use_occ;           // candidate steps are prefiltered with the occupancy bitmap
-    int occ_words, occ_wpr; // words per batch item, words per radial row
+    int occ_words, occ_wpr; // words per batch item; words per radial row (axisym) / per line of blocks along z (3-D)
+    int occ_nbj;            // 3-D: blocks along y
     float *cube;           // fwd: output; bwd: saved forward output (const)
     const float *dl_dcube; // bwd
 };
@@ -107,7 +109,7 @@ struct SetupParams {
     int nx, ny, nstep, nbatch, b0;
     int nlev, nchan;
     int do_rays, do_tables, do_pack, do_zero_grad, do_occ;
-    int occ_words, occ_wpr;
+    int occ_words, occ_wpr, occ_nbj;
     float occ_thr;         // stored density value above which a node can emit
     long long batch_stride;
     const float *dens, *temp, *vel;

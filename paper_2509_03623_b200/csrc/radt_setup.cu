@@ -117,6 +117,33 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
         return;
     }
     blk -= nb_tab;
+    if (blk < nb_occ && P.grid.kind == 1) {
+        // 3-D occupancy: one bit per block of 4 x 4 x 4 cells, set when some node of the block's cells or of the
+        // cells next to them (nodes 4I-1 .. 4I+5 per axis) stores a density that can emit (or is NaN).  One thread
+        // per bit; the 32 bits of a word are the lanes of one warp.
+        long long t = (long long)blk * blockDim.x + threadIdx.x;
+        long long w = t >> 5;
+        if (w >= (long long)P.occ_words * P.nbatch) return;
+        int b = (int)(w / P.occ_words);
+        int wi = (int)(w - (long long)b * P.occ_words);
+        int Lw = wi % P.occ_wpr, IJ = wi / P.occ_wpr;
+        int J = IJ % P.occ_nbj, I = IJ / P.occ_nbj, Lb = Lw * 32 + (threadIdx.x & 31);
+        const float *dn = P.dens + (long long)(P.b0 + b) * P.batch_stride;
+        bool found = false;
+        if (4 * Lb < P.grid.n2 - 1) {
+            int i0 = max(4 * I - 1, 0), i1 = min(4 * I + 5, P.grid.n0 - 1);
+            int j0 = max(4 * J - 1, 0), j1 = min(4 * J + 5, P.grid.n1 - 1);
+            int l0 = max(4 * Lb - 1, 0), l1 = min(4 * Lb + 5, P.grid.n2 - 1);
+            for (int i = i0; i <= i1 && !found; ++i)
+                for (int j = j0; j <= j1 && !found; ++j) {
+                    const float *row = dn + ((long long)i * P.grid.n1 + j) * P.grid.n2;
+                    for (int l = l0; l <= l1; ++l) found |= !(__ldg(row + l) <= P.occ_thr);
+                }
+        }
+        unsigned word = __ballot_sync(0xffffffffu, found);
+        if ((threadIdx.x & 31) == 0) P.ws.occ[(size_t)(P.b0 + b) * P.occ_words + wi] = word;
+        return;
+    }
     if (blk < nb_occ) {
         // Occupancy bitmap of the (r, zeta) grid for the march prefilter: bit j of word (i, j / 32) is set when
         // some node of the 4 x 4 block around cell (i, j) -- the corners of the cell and of its eight
@@ -223,7 +250,8 @@ cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const C
         long long nb = (total + 255) / 256;
         nb_pack = (int)(nb < 148 * 16 ? nb : 148 * 16);
     }
-    int nb_occ = P.do_occ ? (int)(((long long)P.occ_words * P.nbatch + 255) / 256) : 0;
+    long long occ_threads = (long long)P.occ_words * P.nbatch * (P.grid.kind == 1 ? 32 : 1);
+    int nb_occ = P.do_occ ? (int)((occ_threads + 255) / 256) : 0;
     int nb = nb_rays + nb_tab + nb_occ + nb_pack;
     if (nb == 0) return cudaSuccess;
     k_setup<<<nb, 256, 0, st>>>(P, L, V, nb_rays, nb_tab, nb_occ);
