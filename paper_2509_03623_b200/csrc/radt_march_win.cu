@@ -288,8 +288,8 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
 // K4 / K5 adjoint march: front-to-back re-march with the saved cube
 //   dL/d dtau_k,c = G_c (T_{k+1,c} S_k - R_k,c),  R_k = I - I_{<=k}        dL/dS_k = sum_c G_c (1-e_k,c) T_k,c
 // Entries with K2 = 0 are zero-opacity steps (LINEAR density grids): they leave the ray state untouched and
-// feed dL/dn only.  Per pair of steps every lane writes its partial sums {w, w u', w u'^2, G (1-e) T} of both
-// steps (four float2) to shared memory; after BWD_SUB pairs the lanes sum them over the channels.
+// feed dL/dn only.  Per step every lane writes its partial sums {w, w u', w u'^2, G (1-e) T} (one float4; one float
+// in batches of zero-opacity steps) to shared memory; after BWD_SUB pairs the lanes sum them over the channels.
 // ---------------------------------------------------------------------------------------------
 #define BWD_SUB 4            // pairs per reduction batch
 
@@ -316,13 +316,11 @@ struct BwdLane {
     }
 };
 
-typedef float2 RedBuf[BWD_SUB][4][32];           // [pair][quantity][lane] {step a, step b}
-
-__device__ __forceinline__ float2 f2_as_float2(f2 v) { float a, b; upk(v, a, b); return make_float2(a, b); }
+typedef float4 RedBuf[2 * BWD_SUB][32];          // [step of the reduction batch][lane] {w, w u', w u'^2, G (1-e) T}
 
 // A pair with at least one emitting step.  Repeats the forward's O9 sequence bit for bit (fwd_pair).
 __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane &L,
-                                           float nsmax, float2 (*red)[32], int lane)
+                                           float nsmax, float4 (*red)[32], int lane)
 {
     Pair s;
     pair_eval(pair_u_win(qa, qc, L.cf), pk(qb.x, qb.y), s);
@@ -338,58 +336,60 @@ __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, c
     const f2 Tn = pk(T1, T2), G2 = pk1(L.Gs);
     const f2 nR = clamp_nR(sub2(pk(P0, P1), pk1(L.Is)), Tn, pk1(nsmax));
     const f2 a = mul2(G2, fma2(Tn, pk(qb.z, qb.w), nR));          // dL/d dtau
-    const f2 w = mul2(a, s.g), wu = mul2(w, s.u);
-    red[0][lane] = f2_as_float2(w);
-    red[1][lane] = f2_as_float2(wu);
-    red[2][lane] = f2_as_float2(mul2(wu, s.u));
-    red[3][lane] = f2_as_float2(mul2(G2, pk(c0, c1)));
+    const f2 w = mul2(a, s.g), wu = mul2(w, s.u), wuu = mul2(wu, s.u), gc = mul2(G2, pk(c0, c1));
+    float w0, w1, x0, x1, y0, y1, z0, z1;
+    upk(w, w0, w1); upk(wu, x0, x1); upk(wuu, y0, y1); upk(gc, z0, z1);
+    red[0][lane] = make_float4(w0, x0, y0, z0);
+    red[1][lane] = make_float4(w1, x1, y1, z1);
     L.Ts = T2; L.Ps = P1;
 }
 
-// A pair of zero-opacity steps: T, P and hence G T and G R stay fixed; only sum w is needed.
-__device__ __forceinline__ void bwd_pair_z(const float4 &qa, const float4 &qb, const float4 &qc, const BwdLane &L,
-                                           float nsmax, float2 (*red)[32], int lane, bool zero_rest)
+// Zero-opacity steps leave T and P untouched, so G T and G R are fixed while the lane keeps its channel; only
+// sum w = sum (G T S_k - G R) g is needed.  {GT, GnR} of the served channel:
+__device__ __forceinline__ float2 z_frozen(const BwdLane &L, float nsmax)
 {
-    const f2 u = pair_u_win(qa, qc, L.cf);
+    return make_float2(L.Gs * L.Ts, L.Gs * fminf(fmaxf(L.Ps - L.Is, L.Ts * nsmax), 0.f));
+}
+__device__ __forceinline__ f2 z_pair_w(const float4 &qa, float Sa, float Sb, const float4 &qc, float cf, float2 fr)
+{
+    const f2 u = pair_u_win(qa, qc, cf);
     float t0, t1;
     upk(mul2(u, u), t0, t1);
     const f2 g = pk(ex2_approx(-t0), ex2_approx(-t1));
-    const float GT = L.Gs * L.Ts;
-    const float GnR = L.Gs * fminf(fmaxf(L.Ps - L.Is, L.Ts * nsmax), 0.f);
-    red[0][lane] = f2_as_float2(mul2(fma2(pk1(GT), pk(qb.z, qb.w), pk1(GnR)), g));
-    if (zero_rest) {
-        red[1][lane] = make_float2(0.f, 0.f); red[2][lane] = make_float2(0.f, 0.f); red[3][lane] = make_float2(0.f, 0.f);
-    }
+    return mul2(fma2(pk1(fr.x), pk(Sa, Sb), pk1(fr.y)), g);
 }
 
-// Sum the partials of nb <= BWD_SUB pairs over the 32 lanes; lane p < nb ends with the sums of pair p and stores
-// them as two float4 (steps 2p, 2p+1) into out.  Lane (p = lane & 3, h = lane >> 2) adds the source lanes
-// 4h..4h+3 of pair p (skewed: conflict-free 8-byte reads), then the eight groups are combined by three shuffle
-// rounds.
-template <bool ZONLY>
-__device__ __forceinline__ void reduce_pairs(const RedBuf &red, int nb, float4 *out, int lane)
+// Sum the partials of nb <= BWD_SUB pairs (2 nb steps) over the 32 lanes.  Lane (s = lane & 7, h = lane >> 3) adds
+// the source lanes 8h .. 8h+7 of step s (skewed: conflict-free 16-byte reads), two shuffle rounds combine the four
+// quarters, and lane s < 2 nb stores the four sums of step s.
+__device__ __forceinline__ void reduce_steps_e(const RedBuf &red, int nb, float4 *out, int lane)
 {
-    const int p = lane & 3, h4 = lane & 28;
-    float2 acc[4];
+    const int s = lane & 7, h8 = lane & 24;
+    float4 acc = red[s][h8 + s];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        if (ZONLY && q > 0) { acc[q] = make_float2(0.f, 0.f); continue; }
-        acc[q] = red[p][q][h4 + p];
-#pragma unroll
-        for (int i = 1; i < 4; ++i) {
-            const float2 v = red[p][q][h4 + ((i + p) & 3)];
-            acc[q].x += v.x; acc[q].y += v.y;
-        }
-#pragma unroll
-        for (int m = 4; m <= 16; m <<= 1) {
-            acc[q].x += __shfl_xor_sync(FULL, acc[q].x, m);
-            acc[q].y += __shfl_xor_sync(FULL, acc[q].y, m);
-        }
+    for (int i = 1; i < 8; ++i) {
+        const float4 v = red[s][h8 + ((i + s) & 7)];
+        acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
     }
-    if (lane < nb) {
-        out[2 * lane] = make_float4(acc[0].x, acc[1].x, acc[2].x, acc[3].x);
-        out[2 * lane + 1] = make_float4(acc[0].y, acc[1].y, acc[2].y, acc[3].y);
+#pragma unroll
+    for (int m = 8; m <= 16; m <<= 1) {
+        acc.x += __shfl_xor_sync(FULL, acc.x, m);
+        acc.y += __shfl_xor_sync(FULL, acc.y, m);
+        acc.z += __shfl_xor_sync(FULL, acc.z, m);
+        acc.w += __shfl_xor_sync(FULL, acc.w, m);
     }
+    if (lane < 2 * nb) out[lane] = acc;
+}
+// Same for a batch of zero-opacity pairs: one float per (step, lane) in the first kilobyte of the buffer.
+__device__ __forceinline__ void reduce_steps_z(const float (*redz)[32], int nb, float4 *out, int lane)
+{
+    const int s = lane & 7, h8 = lane & 24;
+    float acc = redz[s][h8 + s];
+#pragma unroll
+    for (int i = 1; i < 8; ++i) acc += redz[s][h8 + ((i + s) & 7)];
+    acc += __shfl_xor_sync(FULL, acc, 8);
+    acc += __shfl_xor_sync(FULL, acc, 16);
+    if (lane < 2 * nb) out[lane] = make_float4(acc, 0.f, 0.f, 0.f);
 }
 
 struct __align__(16) BwdShared {          // per warp, followed by (T, P) of 32 ngroups channels
@@ -468,6 +468,31 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
             for (int base_i = 0; base_i < npairs; base_i += BWD_SUB) {
                 const int nb = min(BWD_SUB, npairs - base_i);
                 const bool anyE = (emask >> base_i) & ((1u << BWD_SUB) - 1u);
+                if (!anyE) {
+                    // a batch of zero-opacity pairs: the ray state is frozen
+                    float (*redz)[32] = reinterpret_cast<float (*)[32]>(&B.red[0][0]);
+                    float2 fr = z_frozen(L, nsmax);
+#pragma unroll 1
+                    for (int jj = 0; jj < nb; ++jj) {
+                        const int i = base_i + jj;
+                        const float4 qa = S.a[i], qc = S.c[i];
+                        const float2 Sab = *reinterpret_cast<const float2 *>(&S.b[i].z);
+                        const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
+                        if (group_misses(L.cur, ulo, uhi)) {
+                            L.regroup(group_for(ulo, uhi), lane, nchan);
+                            fr = z_frozen(L, nsmax);
+                        }
+                        float w0, w1;
+                        upk(z_pair_w(qa, Sab.x, Sab.y, qc, L.cf, fr), w0, w1);
+                        redz[2 * jj][lane] = w0;
+                        redz[2 * jj + 1][lane] = w1;
+                    }
+                    n_mufu += 2 * nb;
+                    __syncwarp();
+                    reduce_steps_z(redz, nb, &B.sum[2 * base_i], lane);
+                    __syncwarp();
+                    continue;
+                }
 #pragma unroll 1
                 for (int jj = 0; jj < nb; ++jj) {
                     const int i = base_i + jj;
@@ -475,16 +500,18 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
                     const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
                     if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
                     if ((emask >> i) & 1u) {
-                        bwd_pair_e(qa, qb, qc, L, nsmax, B.red[jj], lane);
+                        bwd_pair_e(qa, qb, qc, L, nsmax, &B.red[2 * jj], lane);
                         n_mufu += 4;
                     } else {
-                        bwd_pair_z(qa, qb, qc, L, nsmax, B.red[jj], lane, anyE);
+                        float w0, w1;
+                        upk(z_pair_w(qa, qb.z, qb.w, qc, L.cf, z_frozen(L, nsmax)), w0, w1);
+                        B.red[2 * jj][lane] = make_float4(w0, 0.f, 0.f, 0.f);
+                        B.red[2 * jj + 1][lane] = make_float4(w1, 0.f, 0.f, 0.f);
                         n_mufu += 2;
                     }
                 }
                 __syncwarp();
-                if (anyE) reduce_pairs<false>(B.red, nb, &B.sum[2 * base_i], lane);
-                else reduce_pairs<true>(B.red, nb, &B.sum[2 * base_i], lane);
+                reduce_steps_e(B.red, nb, &B.sum[2 * base_i], lane);
                 __syncwarp();
             }
             if (a) {
