@@ -316,11 +316,16 @@ struct BwdLane {
     }
 };
 
-typedef float4 RedBuf[2 * BWD_SUB][32];          // [step of the reduction batch][lane] {w, w u', w u'^2, G (1-e) T}
+// Partial sums of a reduction batch, rows padded by one element so that both the per-lane writes and the per-step
+// reads are free of bank conflicts with plain immediate offsets:
+//   emitting batches   float4 [2 BWD_SUB steps][33]   {w, w u', w u'^2, G (1-e) T} per (step, lane)
+//   zero-opacity runs  float  [32 steps][33]          w per (step, lane)
+#define RED_ROW 33
+typedef float4 RedBuf[2 * BWD_SUB][RED_ROW];
 
 // A pair with at least one emitting step.  Repeats the forward's O9 sequence bit for bit (fwd_pair).
 __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane &L,
-                                           float nsmax, float4 (*red)[32], int lane)
+                                           float nsmax, float4 (*red)[RED_ROW], int lane)
 {
     Pair s;
     pair_eval(pair_u_win(qa, qc, L.cf), pk(qb.x, qb.y), s);
@@ -360,15 +365,15 @@ __device__ __forceinline__ f2 z_pair_w(const float4 &qa, float Sa, float Sb, con
 }
 
 // Sum the partials of nb <= BWD_SUB pairs (2 nb steps) over the 32 lanes.  Lane (s = lane & 7, h = lane >> 3) adds
-// the source lanes 8h .. 8h+7 of step s (skewed: conflict-free 16-byte reads), two shuffle rounds combine the four
-// quarters, and lane s < 2 nb stores the four sums of step s.
+// the source lanes 8h .. 8h+7 of step s, two shuffle rounds combine the four quarters, and lane s < 2 nb stores the
+// four sums of step s.
 __device__ __forceinline__ void reduce_steps_e(const RedBuf &red, int nb, float4 *out, int lane)
 {
-    const int s = lane & 7, h8 = lane & 24;
-    float4 acc = red[s][h8 + s];
+    const float4 *row = &red[lane & 7][lane & 24];
+    float4 acc = row[0];
 #pragma unroll
     for (int i = 1; i < 8; ++i) {
-        const float4 v = red[s][h8 + ((i + s) & 7)];
+        const float4 v = row[i];
         acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
     }
 #pragma unroll
@@ -380,21 +385,21 @@ __device__ __forceinline__ void reduce_steps_e(const RedBuf &red, int nb, float4
     }
     if (lane < 2 * nb) out[lane] = acc;
 }
-// Same for a batch of zero-opacity pairs: one float per (step, lane) in the first kilobyte of the buffer.
-__device__ __forceinline__ void reduce_steps_z(const float (*redz)[32], int nb, float4 *out, int lane)
+// A run of nz <= 16 zero-opacity pairs: lane s < 2 nz sums the 32 partials of step s.
+__device__ __forceinline__ void reduce_steps_z(const float (*redz)[RED_ROW], int nz, float4 *out, int lane)
 {
-    const int s = lane & 7, h8 = lane & 24;
-    float acc = redz[s][h8 + s];
+    if (lane < 2 * nz) {
+        const float *row = redz[lane];
+        float a0 = row[0], a1 = row[1], a2 = row[2], a3 = row[3];
 #pragma unroll
-    for (int i = 1; i < 8; ++i) acc += redz[s][h8 + ((i + s) & 7)];
-    acc += __shfl_xor_sync(FULL, acc, 8);
-    acc += __shfl_xor_sync(FULL, acc, 16);
-    if (lane < 2 * nb) out[lane] = make_float4(acc, 0.f, 0.f, 0.f);
+        for (int i = 4; i < 32; i += 4) { a0 += row[i]; a1 += row[i + 1]; a2 += row[i + 2]; a3 += row[i + 3]; }
+        out[lane] = make_float4((a0 + a1) + (a2 + a3), 0.f, 0.f, 0.f);
+    }
 }
 
 struct __align__(16) BwdShared {          // per warp, followed by (T, P) of 32 ngroups channels
     WinShared w;
-    RedBuf red;
+    RedBuf red;                           // 8 x 33 float4 = 32 x 33 float
     float4 sum[32];                       // channel sums of the compacted steps
 };
 static size_t bwd_warp_bytes(int ng) { return sizeof(BwdShared) + (size_t)ng * 256; }
@@ -464,16 +469,17 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
             if (npairs == 0) continue;
             // pairs that hold an emitting step
             const unsigned emask = __ballot_sync(FULL, lane < npairs && (S.b[lane].x > 0.f || S.b[lane].y > 0.f));
+            int base_i = 0;
 #pragma unroll 1
-            for (int base_i = 0; base_i < npairs; base_i += BWD_SUB) {
-                const int nb = min(BWD_SUB, npairs - base_i);
-                const bool anyE = (emask >> base_i) & ((1u << BWD_SUB) - 1u);
-                if (!anyE) {
-                    // a batch of zero-opacity pairs: the ray state is frozen
-                    float (*redz)[32] = reinterpret_cast<float (*)[32]>(&B.red[0][0]);
+            while (base_i < npairs) {
+                const unsigned erest = emask >> base_i;
+                if (!(erest & 1u)) {
+                    // a run of zero-opacity pairs (up to the whole batch): the ray state is frozen
+                    const int nz = min(erest ? __ffs(erest) - 1 : 32, npairs - base_i);
+                    float (*redz)[RED_ROW] = reinterpret_cast<float (*)[RED_ROW]>(&B.red[0][0]);
                     float2 fr = z_frozen(L, nsmax);
 #pragma unroll 1
-                    for (int jj = 0; jj < nb; ++jj) {
+                    for (int jj = 0; jj < nz; ++jj) {
                         const int i = base_i + jj;
                         const float4 qa = S.a[i], qc = S.c[i];
                         const float2 Sab = *reinterpret_cast<const float2 *>(&S.b[i].z);
@@ -487,32 +493,28 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
                         redz[2 * jj][lane] = w0;
                         redz[2 * jj + 1][lane] = w1;
                     }
-                    n_mufu += 2 * nb;
+                    n_mufu += 2 * nz;
                     __syncwarp();
-                    reduce_steps_z(redz, nb, &B.sum[2 * base_i], lane);
+                    reduce_steps_z(redz, nz, &B.sum[2 * base_i], lane);
                     __syncwarp();
+                    base_i += nz;
                     continue;
                 }
+                // up to BWD_SUB consecutive pairs that hold an emitting step
+                const int nb = min(min(BWD_SUB, __ffs(~erest) - 1), npairs - base_i);
 #pragma unroll 1
                 for (int jj = 0; jj < nb; ++jj) {
                     const int i = base_i + jj;
                     const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
                     const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
                     if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
-                    if ((emask >> i) & 1u) {
-                        bwd_pair_e(qa, qb, qc, L, nsmax, &B.red[2 * jj], lane);
-                        n_mufu += 4;
-                    } else {
-                        float w0, w1;
-                        upk(z_pair_w(qa, qb.z, qb.w, qc, L.cf, z_frozen(L, nsmax)), w0, w1);
-                        B.red[2 * jj][lane] = make_float4(w0, 0.f, 0.f, 0.f);
-                        B.red[2 * jj + 1][lane] = make_float4(w1, 0.f, 0.f, 0.f);
-                        n_mufu += 2;
-                    }
+                    bwd_pair_e(qa, qb, qc, L, nsmax, &B.red[2 * jj], lane);
                 }
+                n_mufu += 4 * nb;
                 __syncwarp();
                 reduce_steps_e(B.red, nb, &B.sum[2 * base_i], lane);
                 __syncwarp();
+                base_i += nb;
             }
             if (a) {
                 const float4 v = B.sum[pos];
