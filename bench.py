@@ -107,12 +107,20 @@ def oracle_sample_step(scene, stride, G=None):
     return dt, len(idx) * len(scene.line.vchan) * scene.geom.nstep
 
 
-def cpu_baseline(scene, stride=4):
+def cpu_baseline(scene, budget_s=12.0):
+    """The oracle as it stands on this box's host cores: whole fwd + adjoint passes over every 2nd ray of the scene,
+    repeated until about `budget_s` seconds of wall time (>= 2 passes)."""
     from oracle import pyoracle as po
-    oracle_sample_step(scene, stride * 16)          # load the library, touch the pages
-    dt, n = oracle_sample_step(scene, stride)
-    return {"value": n / dt, "unit": UNIT, "cores": po.num_threads(), "kind": "oracle",
-            "sample": f"{scene.name}: every {stride}th ray ({n:.3g} samples), fp64 forward + adjoint, {dt:.2f} s"}
+    oracle_sample_step(scene, 64)          # load the library, touch the pages
+    stride, tot_t, tot_n, passes = 2, 0.0, 0, 0
+    while passes < 2 or tot_t < budget_s:
+        dt, n = oracle_sample_step(scene, stride)
+        tot_t += dt
+        tot_n += n
+        passes += 1
+    return {"value": tot_n / tot_t, "unit": UNIT, "cores": po.num_threads(), "kind": "oracle",
+            "sample": f"{scene.name}: {passes} passes over every {stride}nd ray ({tot_n:.3g} samples), fp64 forward + adjoint, "
+                      f"{tot_t:.1f} s wall"}
 
 
 def run_reference(args):

@@ -90,17 +90,27 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
     blk -= nb_rays;
     if (blk < nb_tab) {
         int t = blk * blockDim.x + threadIdx.x;
-        if (t <= RADT_NQ + 1) {
-            // partition function Q(T) = sum g_J exp(-E_J/T) and dQ/dlnT on a log2-T lattice
-            double T = exp2((double)t * (double)RADT_NQ_OCTAVES / (double)RADT_NQ);
-            double q = 0.0, dq = 0.0;
-            for (int l = 0; l < P.nlev; ++l) {
-                double y = L.e[l] / T;
-                double w = L.g[l] * exp(-y);
-                q += w;
-                dq += w * y;
+        {
+            // partition function Q(T) = sum g_J exp(-E_J/T) and dQ/dlnT on a log2-T lattice: one warp
+            // per entry, lanes over levels (a per-thread loop over the levels was a 41-deep chain of fp64 exp and
+            // the longest pole of the launch)
+            int e = t >> 5, ln = t & 31;
+            if (e <= RADT_NQ + 1) {
+                double T = exp2((double)e * (double)RADT_NQ_OCTAVES / (double)RADT_NQ);
+                double q = 0.0, dq = 0.0;
+                for (int l = ln; l < P.nlev; l += 32) {
+                    double y = L.e[l] / T;
+                    double w = L.g[l] * exp(-y);
+                    q += w;
+                    dq += w * y;
+                }
+#pragma unroll
+                for (int m = 16; m > 0; m >>= 1) {
+                    q += __shfl_xor_sync(0xffffffffu, q, m);
+                    dq += __shfl_xor_sync(0xffffffffu, dq, m);
+                }
+                if (ln == 0) P.ws.qtab[e] = make_float2((float)q, (float)dq);
             }
-            P.ws.qtab[t] = make_float2((float)q, (float)dq);
         }
         if (t < P.nbatch * RADT_MAXCHAN) {
             int b = t / RADT_MAXCHAN, c = t % RADT_MAXCHAN;
@@ -148,23 +158,27 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
         // Occupancy bitmap of the (r, zeta) grid for the march prefilter: bit j of word (i, j / 32) is set when
         // some node of the 4 x 4 block around cell (i, j) -- the corners of the cell and of its eight
         // neighbours -- stores a density that can emit (or is NaN).  occ_thr = -inf gives all ones.
+        // One warp per word, lanes over the 35 nodes jw*32 - 1 .. jw*32 + 33 of each of the four radial rows.
         long long t = (long long)blk * blockDim.x + threadIdx.x;
-        if (t >= (long long)P.occ_words * P.nbatch) return;
-        int b = (int)(t / P.occ_words);
-        int w = (int)(t - (long long)b * P.occ_words);
+        long long wq = t >> 5;
+        if (wq >= (long long)P.occ_words * P.nbatch) return;
+        const int ln = threadIdx.x & 31;
+        int b = (int)(wq / P.occ_words);
+        int w = (int)(wq - (long long)b * P.occ_words);
         int i = w / P.occ_wpr, jw = w - i * P.occ_wpr;
         const float *dn = P.dens + (long long)(P.b0 + b) * P.batch_stride;
-        unsigned long long m = 0ull;
+        bool f0 = false, f1 = false;                      // node tt = ln, node tt = ln + 32 (ln < 3)
         for (int di = -1; di <= 2; ++di) {
             int ii = i + di;
             if (ii < 0 || ii >= P.grid.n0) continue;
-            for (int tt = 0; tt < 35; ++tt) {
-                int jj = jw * 32 - 1 + tt;
-                if (jj < 0 || jj >= P.grid.n1) continue;
-                if (!(__ldg(dn + (long long)ii * P.grid.n1 + jj) <= P.occ_thr)) m |= 1ull << tt;
-            }
+            int j0 = jw * 32 - 1 + ln, j1 = j0 + 32;
+            if (j0 >= 0 && j0 < P.grid.n1) f0 |= !(__ldg(dn + (long long)ii * P.grid.n1 + j0) <= P.occ_thr);
+            if (ln < 3 && j1 < P.grid.n1) f1 |= !(__ldg(dn + (long long)ii * P.grid.n1 + j1) <= P.occ_thr);
         }
+        unsigned long long m = (unsigned long long)__ballot_sync(0xffffffffu, f0) |
+                               ((unsigned long long)__ballot_sync(0xffffffffu, f1) << 32);
         m |= (m >> 1) | (m >> 2) | (m >> 3);
+        if (ln != 0) return;
         P.ws.occ[(size_t)(P.b0 + b) * P.occ_words + w] = (unsigned)m;
         return;
     }
@@ -240,7 +254,7 @@ cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const C
 {
     long long nrays = (long long)P.nx * P.ny * P.nbatch;
     int nb_rays = P.do_rays ? (int)((nrays + 255) / 256) : 0;
-    int need_tab = RADT_NQ + 2;
+    int need_tab = (RADT_NQ + 2) * 32;
     if (P.nbatch * RADT_MAXCHAN > need_tab) need_tab = P.nbatch * RADT_MAXCHAN;
     if (P.grid.kind == 0 && P.grid.n0 > need_tab) need_tab = P.grid.n0;
     int nb_tab = P.do_tables ? (need_tab + 255) / 256 : 0;
@@ -250,7 +264,7 @@ cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const C
         long long nb = (total + 255) / 256;
         nb_pack = (int)(nb < 148 * 16 ? nb : 148 * 16);
     }
-    long long occ_threads = (long long)P.occ_words * P.nbatch * (P.grid.kind == 1 ? 32 : 1);
+    long long occ_threads = (long long)P.occ_words * P.nbatch * 32;
     int nb_occ = P.do_occ ? (int)((occ_threads + 255) / 256) : 0;
     int nb = nb_rays + nb_tab + nb_occ + nb_pack;
     if (nb == 0) return cudaSuccess;
