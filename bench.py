@@ -1,8 +1,8 @@
 #!/usr/bin/env python
 """Benchmark of the line-RT render hot path (BASELINE.json metric: ray.channel.step samples/s, fwd+bwd).
 
-A *step* is one pass of the whole hot path over one synthetic disk: ray geometry + forward march -> L2 data
-term -> memory-free adjoint (SURVEY.md section 8(a) rows a-j).  The workload at N = 1 is BASELINE.json
+A *step* is one pass of the whole hot path over one synthetic disk: ray geometry + forward march with the L2 data
+term fused into its epilogue (radt_render_loss) -> memory-free adjoint (SURVEY.md section 8(a) rows a-j).  The workload at N = 1 is BASELINE.json
 `configs[1]` (256x128 (r,z) grid, 256x256 px, 64 channels, 256 steps per ray).  With N > 1 every rank renders
 its own disk (independent problems, no data-path collective): weak scaling.
 
@@ -214,8 +214,7 @@ def run_ours(args):
         R.fit_step(stream)
 
     launches_per_step = 0
-    R.render(stream); launches_per_step += B.radt_last_launch_count()
-    R.l2_loss_grad(stream); launches_per_step += B.radt_last_launch_count()
+    R.render_loss(stream); launches_per_step += B.radt_last_launch_count()
     R.render_bwd(stream=stream); launches_per_step += B.radt_last_launch_count()
 
     for _ in range(max(args.warmup, 3)):
@@ -259,6 +258,7 @@ def run_ours(args):
     reps = max(5, min(args.steps, 30))
     t_fwd = time_kernel_group(lambda: R.render(stream), stream, torch, flush, reps)
     cnt = R.counters()
+    t_fl = time_kernel_group(lambda: R.render_loss(stream), stream, torch, flush, reps)
     t_l2 = time_kernel_group(lambda: R.l2_loss_grad(stream), stream, torch, flush, reps)
     t_bwd = time_kernel_group(lambda: R.render_bwd(stream=stream), stream, torch, flush, reps)
     cnt_b = R.counters()
@@ -318,7 +318,7 @@ def run_ours(args):
                    "nominal_samples_per_step": int(nominal), "parallelism": f"independent disks x{world}",
                    "l2": "flushed between timed steps (256 MiB fill outside the events)",
                    "kernels": "window (uniform channel lattice)" if args.win_path else "channel table"},
-        "fwd_value": nominal / (t_fwd * 1e-3), "fwd_ms": t_fwd, "l2_ms": t_l2, "bwd_ms": t_bwd,
+        "fwd_value": nominal / (t_fwd * 1e-3), "fwd_ms": t_fwd, "fwd_loss_fused_ms": t_fl, "l2_ms": t_l2, "bwd_ms": t_bwd,
         "executed_samples": {"fwd": int(fwd_exec), "bwd": int(bwd_exec), "fwd_active_ray_steps": int(cnt[0]),
                              "bwd_active_ray_steps": int(cnt_b[2]), "nominal": int(nominal)},
         "roofline": dominant, "roofline_other": other,

@@ -158,12 +158,21 @@ int radt_render_bwd(const radt_geom *geom, const radt_line *line, const radt_gri
 int radt_l2_loss_grad(const float *cube, const float *target, double sigma, int64_t n, float *dl_dcube,
                       double *loss_out, void *cuda_stream);
 
+/* Forward render with the chi^2 data term fused into its epilogue (the step after the render in
+ * the paper's fit, Fig. 2 D): writes cube as radt_render does and, without a second pass
+ * over it, dl_dcube = (cube - target) / (sigma^2 n) and *loss_out = sum (cube - target)^2 / (2 sigma^2 n), n = number
+ * of voxels of the whole batch.  Same results as radt_render followed by radt_l2_loss_grad (the loss up to the
+ * order of its fp64 sum).  target, cube, dl_dcube: DEVICE float32 [batch][ny][nx][nchan]; loss_out: DEVICE double[1]. */
+int radt_render_loss(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                     const float *target, double sigma, float *cube, float *dl_dcube, double *loss_out, void *ws,
+                     size_t ws_bytes, void *cuda_stream);
+
 /* Same operations with HOST buffers (grid->dens/temp/vel, cube, dl_dcube, g_* are HOST pointers).
  * Device memory is allocated stream-ordered on stream 0 of the current device; the call returns
  * after the results are in host memory. */
 int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                      float *cube);
-/* Forward + L2 loss against `target` (HOST) + adjoint in one call; cube may be NULL. */
+/* Forward with the fused L2 loss against `target` (HOST) + adjoint in one call; cube may be NULL. */
 int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                        const float *target, double sigma, float *cube, double *loss_out,
                        float *g_dens, float *g_temp, float *g_vel);

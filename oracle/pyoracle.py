@@ -176,3 +176,15 @@ def num_threads() -> int:
 
 def set_num_threads(n: int):
     os.environ["OMP_NUM_THREADS"] = str(n)
+
+
+def chi2_loss_grad(cube, target, sigma: float):
+    """Pixel-wise chi^2 data term of the fit ("chi^2 ... averaged over pixels"; the L2 loss of
+    BASELINE.json configs 2-5), plain numpy in fp64:
+        L = 1/(2 n) sum_i ((I_i - D_i)/sigma)^2,    dL/dI_i = (I_i - D_i) / (sigma^2 n),    n = number of voxels.
+    Returns (L, dL/dI).  Pinned in tests/test_oracle_closed_forms.py (constant residual, finite differences)."""
+    I = np.asarray(cube, dtype=np.float64)
+    D = np.asarray(target, dtype=np.float64)
+    n = I.size
+    r = I - D
+    return float(np.sum((r / sigma) ** 2) / (2.0 * n)), r / (sigma * sigma * n)

@@ -20,7 +20,7 @@ OPT_WINDOW, OPT_SKIP_EMPTY, OPT_WIN_PATH = 1, 2, 3
 
 EXPORTS = ["radt_version", "radt_last_error", "radt_set_option", "radt_get_option", "radt_workspace_bytes",
            "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_l2_loss_grad", "radt_render_host",
-           "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
+           "radt_render_loss", "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
            "radt_last_launch_count"]
 
 
@@ -71,6 +71,7 @@ def lib():
         L.radt_render.argtypes = [gp, lp, rp, i32, vp, vp, C.c_size_t, vp]
         L.radt_render_bwd.argtypes = [gp, lp, rp, i32, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_l2_loss_grad.argtypes = [vp, vp, dbl, i64, vp, vp, vp]
+        L.radt_render_loss.argtypes = [gp, lp, rp, i32, vp, dbl, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_render_host.argtypes = [gp, lp, rp, i32, vp]
         L.radt_fit_step_host.argtypes = [gp, lp, rp, i32, vp, dbl, vp, C.POINTER(dbl), vp, vp, vp]
         L.radt_render_bwd_host.argtypes = [gp, lp, rp, i32, vp, vp, vp, vp, vp]
@@ -189,6 +190,15 @@ def radt_l2_loss_grad(cube, target, sigma: float, dl_dcube, loss_out, stream=Non
     _check(lib().radt_l2_loss_grad(C.c_void_p(cube.data_ptr()), C.c_void_p(target.data_ptr()), float(sigma),
                                    cube.numel(), C.c_void_p(dl_dcube.data_ptr()), C.c_void_p(loss_out.data_ptr()),
                                    _stream_ptr(stream)))
+
+
+def radt_render_loss(desc: Descriptors, dens, temp, vel, target, sigma: float, cube, dl_dcube, loss_out, ws, stream=None):
+    """Forward render with the fused chi^2 data term: cube, dl_dcube, loss_out (CUDA float64 [1]) in one pass."""
+    desc.with_fields(dens.data_ptr(), temp.data_ptr(), vel.data_ptr())
+    _check(lib().radt_render_loss(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch,
+                                  C.c_void_p(target.data_ptr()), C.c_double(float(sigma)), C.c_void_p(cube.data_ptr()),
+                                  C.c_void_p(dl_dcube.data_ptr()), C.c_void_p(loss_out.data_ptr()),
+                                  C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream_ptr(stream)))
 
 
 def radt_read_counters(ws, stream=None):

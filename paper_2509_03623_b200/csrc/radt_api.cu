@@ -193,7 +193,7 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     WsLayout w;
     size_t off = 0;
     size_t nrays = (size_t)geom[0].nx * geom[0].ny * (size_t)batch;
-    w.counters = off; off = align256(off + 8 * sizeof(unsigned long long));
+    w.counters = off; off = align256(off + (8 + RADT_LOSS_SLOTS) * sizeof(unsigned long long));
     w.rays = off; off = align256(off + nrays * sizeof(RayRec));
     w.qtab = off; off = align256(off + (RADT_NQ + 2) * sizeof(float2));
     w.vcs = off; off = align256(off + (size_t)batch * RADT_MAXCHAN * sizeof(float2));
@@ -233,10 +233,18 @@ DevWs make_dev_ws(void *ws, const WsLayout &w)
     return d;
 }
 
+// fused chi^2 data term of a forward pass (radt_render_loss); target == nullptr: plain render
+struct LossArgs {
+    const float *target = nullptr;
+    float *dl_out = nullptr;
+    double *loss = nullptr;
+    double sigma = 0.0;
+};
+
 // Enqueue setup + march for all batch chunks.  pass 0: forward into `cube`; pass 1: adjoint.
 int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int batch, int pass, float *cube,
              const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel, void *ws, size_t ws_bytes,
-             cudaStream_t st)
+             cudaStream_t st, const LossArgs &loss = LossArgs())
 {
     int rc = validate(geom, line, grid, batch);
     if (rc) return rc;
@@ -268,7 +276,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
     make_dev_line(line, dl_probe);
     // window kernels: uniform channel lattice, and cells no finer than the fp32 positions of the prefilter resolve
     const bool use_win = g_opt_win_path && dl_probe.uniform && prefilter_safe(grid);
-    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, 8 * sizeof(unsigned long long), st));
+    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, (8 + RADT_LOSS_SLOTS) * sizeof(unsigned long long), st));
     for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
         int nb = batch - b0 < RADT_MAXB ? batch - b0 : RADT_MAXB;
         memset(&SP, 0, sizeof(SP));
@@ -308,11 +316,23 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
                 if ((double)(float)vv != vv) { MP.chan_lo = 1; break; }
             }
         MP.cube = cube; MP.dl_dcube = dl_dcube;
+        if (pass == RADT_PASS_FWD && loss.target) {
+            const double nvox = (double)batch * geom[0].nx * geom[0].ny * line->nchan;
+            const double inv = 1.0 / (loss.sigma * loss.sigma * nvox);
+            MP.target = loss.target; MP.dl_out = loss.dl_out;
+            MP.inv_s2n = (float)inv;
+        }
         MP.use_win = win; MP.use_occ = occ; MP.occ_words = w.occ_words; MP.occ_wpr = w.occ_wpr; MP.occ_nbj = w.occ_nbj;
         if (pass == RADT_PASS_FWD && win) CUDA_TRY(radt_launch_march_fwd_win(MP, nb, st));
         else if (pass == RADT_PASS_FWD) CUDA_TRY(radt_launch_march_fwd(MP, nb, st));
         else if (win) CUDA_TRY(radt_launch_march_bwd_win(MP, nb, st));
         else CUDA_TRY(radt_launch_march_bwd(MP, nb, st));
+        ++g_launches;
+    }
+    if (pass == RADT_PASS_FWD && loss.target) {
+        const double nvox = (double)batch * geom[0].nx * geom[0].ny * line->nchan;
+        CUDA_TRY(radt_launch_loss_finish(reinterpret_cast<double *>(dws.counters + 8),
+                                         0.5 / (loss.sigma * loss.sigma * nvox), loss.loss, st));
         ++g_launches;
     }
     if (pass == RADT_PASS_BWD && (g_dens || g_temp || g_vel)) {
@@ -387,6 +407,18 @@ int radt_render(const radt_geom *geom, const radt_line *line, const radt_grid *g
 {
     return run_pass(geom, line, grid, batch, RADT_PASS_FWD, cube, nullptr, nullptr, nullptr, nullptr, ws, ws_bytes,
                     (cudaStream_t)cuda_stream);
+}
+
+int radt_render_loss(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                     const float *target, double sigma, float *cube, float *dl_dcube, double *loss_out, void *ws,
+                     size_t ws_bytes, void *cuda_stream)
+{
+    if (!target || !dl_dcube || !loss_out) return fail(RADT_E_INVALID, "null target / dl_dcube / loss_out pointer");
+    if (!(sigma > 0)) return fail(RADT_E_INVALID, "sigma must be positive");
+    LossArgs la;
+    la.target = target; la.dl_out = dl_dcube; la.loss = loss_out; la.sigma = sigma;
+    return run_pass(geom, line, grid, batch, RADT_PASS_FWD, cube, nullptr, nullptr, nullptr, nullptr, ws, ws_bytes,
+                    (cudaStream_t)cuda_stream, la);
 }
 
 int radt_render_bwd(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
@@ -465,30 +497,32 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     void *ws = B.alloc(wsb);
     if (!ws) return fail(RADT_E_CUDA, "device allocation failed");
     int launches = 0;
-    if (mode == 0 || mode == 1) {
+    float *d_dl = nullptr;
+    if (mode != 0 && !(d_dl = (float *)B.alloc(nvox * sizeof(float)))) return fail(RADT_E_CUDA, "device allocation failed");
+    if (mode == 0) {
         rc = radt_render(geom, line, &dgrid, batch, d_cube, ws, wsb, B.st);
         if (rc) return rc;
         launches += g_launches;
-        if (cube) CUDA_TRY(cudaMemcpyAsync(cube, d_cube, nvox * sizeof(float), cudaMemcpyDeviceToHost, B.st));
+    } else if (mode == 1) {
+        // forward with the fused chi^2 data term
+        if (!target) return fail(RADT_E_INVALID, "null target");
+        float *d_t = (float *)B.alloc(nvox * sizeof(float));
+        double *d_loss = (double *)B.alloc(sizeof(double));
+        if (!d_t || !d_loss) return fail(RADT_E_CUDA, "device allocation failed");
+        CUDA_TRY(cudaMemcpyAsync(d_t, target, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
+        rc = radt_render_loss(geom, line, &dgrid, batch, d_t, sigma, d_cube, d_dl, d_loss, ws, wsb, B.st);
+        if (rc) return rc;
+        launches += g_launches;
+        if (loss_out) CUDA_TRY(cudaMemcpyAsync(loss_out, d_loss, sizeof(double), cudaMemcpyDeviceToHost, B.st));
     }
+    if ((mode == 0 || mode == 1) && cube)
+        CUDA_TRY(cudaMemcpyAsync(cube, d_cube, nvox * sizeof(float), cudaMemcpyDeviceToHost, B.st));
     if (mode == 1 || mode == 2) {
-        float *d_dl = (float *)B.alloc(nvox * sizeof(float));
         float *d_g[3] = { nullptr, nullptr, nullptr };
         float *h_g[3] = { g_dens, g_temp, g_vel };
         for (int i = 0; i < 3; ++i)
             if (h_g[i] && !(d_g[i] = (float *)B.alloc(fbytes))) return fail(RADT_E_CUDA, "device allocation failed");
-        if (!d_dl) return fail(RADT_E_CUDA, "device allocation failed");
-        if (mode == 1) {
-            if (!target) return fail(RADT_E_INVALID, "null target");
-            float *d_t = (float *)B.alloc(nvox * sizeof(float));
-            double *d_loss = (double *)B.alloc(sizeof(double));
-            if (!d_t || !d_loss) return fail(RADT_E_CUDA, "device allocation failed");
-            CUDA_TRY(cudaMemcpyAsync(d_t, target, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
-            rc = radt_l2_loss_grad(d_cube, d_t, sigma, (int64_t)nvox, d_dl, d_loss, B.st);
-            if (rc) return rc;
-            ++launches;
-            if (loss_out) CUDA_TRY(cudaMemcpyAsync(loss_out, d_loss, sizeof(double), cudaMemcpyDeviceToHost, B.st));
-        } else {
+        if (mode == 2) {
             if (!cube_in || !dl_in) return fail(RADT_E_INVALID, "null cube / dl_dcube");
             CUDA_TRY(cudaMemcpyAsync(d_cube, cube_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
             CUDA_TRY(cudaMemcpyAsync(d_dl, dl_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));

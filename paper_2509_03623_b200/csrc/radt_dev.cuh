@@ -14,6 +14,7 @@
 #define RADT_NQ_OCTAVES 14.0f
 #define RADT_MAXLEV 64
 #define RADT_MAXCHAN 256
+#define RADT_LOSS_SLOTS 1024           // partial sums of the fused chi^2 loss
 
 #define RADT_LOG2E 1.4426950408889634f
 #define RADT_LN2 0.6931471805599453f
@@ -81,7 +82,8 @@ struct DevWs {
     float4 *grad;          // [batch][cells] packed gradient accumulators {dens, temp, vel, -} (bwd only)
     unsigned *occ;         // [batch][occ_words] axisym: bit (i, j): some cell within one cell of (i, j) can emit;
                            // 3-D: one bit per block of 4 x 4 x 4 cells, same dilation (radt_setup.cu)
-    unsigned long long *counters;   // [8] 0-3 work counters; [4] bits of the grid's maximum temperature
+    unsigned long long *counters;   // [8 + RADT_LOSS_SLOTS] 0-3 work counters; [4] bits of the grid's maximum
+                                    // temperature; [8..] partial sums of the fused loss (double)
 };
 
 struct MarchParams {
@@ -100,6 +102,10 @@ struct MarchParams {
     int occ_nbj;            // 3-D: blocks along y
     float *cube;           // fwd: output; bwd: saved forward output (const)
     const float *dl_dcube; // bwd
+    // fused chi^2 data term of the forward (radt_render_loss): all null / 0 for a plain render
+    const float *target;   // [batch][ny][nx][nchan]
+    float *dl_out;         // dL/dcube = (cube - target) / (sigma^2 n)
+    float inv_s2n;
 };
 
 struct SetupParams {

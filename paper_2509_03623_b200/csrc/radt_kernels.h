@@ -7,6 +7,7 @@ cudaError_t radt_launch_unpack(const float4 *grad, long long cells, int nbatch, 
                                float *g_temp, float *g_vel, cudaStream_t st);
 cudaError_t radt_launch_l2(const float *cube, const float *target, double sigma, long long n, float *dl, double *loss,
                            cudaStream_t st);
+cudaError_t radt_launch_loss_finish(double *part, double scale, double *loss, cudaStream_t st);
 cudaError_t radt_launch_march_fwd(const MarchParams &P, int nbatch, cudaStream_t st);
 cudaError_t radt_launch_march_bwd(const MarchParams &P, int nbatch, cudaStream_t st);
 cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st);

@@ -51,6 +51,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
     const DevGeom &G = P.geom[rc.b];
     const int nchan = P.line.nchan;
     float *out = P.cube + rc.ray * (size_t)nchan;
+    if (P.target) loss_prefetch(P, rc.ray * (size_t)nchan, nchan, lane);
     f2 I[NP], T[NP], vcs[NP], vcl[NP];
     float vmin, vmax;
     load_channels<NP>(P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN, nchan, lane, vcs, vcl, vmin, vmax);
@@ -96,6 +97,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
             __syncwarp();
         }
     }
+    double r2 = 0.0;
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
         int c0 = lane + 64 * p, c1 = c0 + 32;
@@ -103,7 +105,12 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
         upk(I[p], i0, i1);
         if (c0 < nchan) out[c0] = i0;
         if (c1 < nchan) out[c1] = i1;
+        if (P.target) {
+            if (c0 < nchan) r2 += loss_voxel(P, rc.ray * (size_t)nchan + c0, i0);
+            if (c1 < nchan) r2 += loss_voxel(P, rc.ray * (size_t)nchan + c1, i1);
+        }
     }
+    if (P.target) loss_report(P, r2, lane);
     if (lane == 0 && n_steps) {
         atomicAdd(P.ws.counters + 0, (unsigned long long)n_steps);
         atomicAdd(P.ws.counters + 1, (unsigned long long)n_mufu);

@@ -271,6 +271,31 @@ __device__ __forceinline__ bool ray_setup(const MarchParams &P, RayCtx &rc, int 
     return true;
 }
 
+// Fused chi^2 data term: a warp adds the squared residuals of its ray to one
+// of RADT_LOSS_SLOTS double slots with a fire-and-forget reduction; k_loss_finish (radt_setup.cu) sums the slots
+// after the last march launch of the call.  The ray's target row is prefetched to L2 before the march.
+__device__ __forceinline__ void loss_prefetch(const MarchParams &P, size_t row, int nchan, int lane)
+{
+    if (lane * 32 < nchan) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.target + row + lane * 32));
+}
+__device__ __forceinline__ void loss_report(const MarchParams &P, double acc, int lane)
+{
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) acc += __shfl_xor_sync(FULL, acc, m);
+    if (lane == 0 && acc != 0.0) {
+        double *part = reinterpret_cast<double *>(P.ws.counters + 8);
+        const unsigned w = (blockIdx.y * gridDim.x + blockIdx.x) * RADT_WARPS_PER_CTA + (threadIdx.x >> 5);
+        asm volatile("red.global.add.f64 [%0], %1;" ::"l"(part + (w & (RADT_LOSS_SLOTS - 1))), "d"(acc) : "memory");
+    }
+}
+// residual of one voxel: writes dL/dcube, returns r^2
+__device__ __forceinline__ double loss_voxel(const MarchParams &P, size_t idx, float I)
+{
+    const float r = I - __ldg(P.target + idx);
+    P.dl_out[idx] = r * P.inv_s2n;
+    return (double)r * (double)r;
+}
+
 // Gradient cells are accumulated as packed float4 {dens, temp, vel, -} (one vector reduction per corner),
 // unpacked to the caller's planes by k_unpack_grad.
 __device__ __forceinline__ void red_add_cell(float4 *cell, float w, float a, float b, float c)

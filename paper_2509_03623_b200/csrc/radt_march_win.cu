@@ -234,6 +234,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
     float *out = P.cube + rc.ray * (size_t)nchan;
     LaneState L;
     L.init(sI, sT, lane, ng);
+    if (P.target) loss_prefetch(P, rc.ray * (size_t)nchan, nchan, lane);
     unsigned n_steps = 0, n_mufu = 0;
     if (rc.ds != 0.0) {
         const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
@@ -274,10 +275,16 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
         }
         L.put_back();
     }
+    double r2 = 0.0;
     for (int g = 0; g < ng; ++g) {
         const int c = lane + 32 * g;
-        if (c < nchan) out[c] = sI[c];
+        if (c < nchan) {
+            const float Ic = sI[c];
+            out[c] = Ic;
+            if (P.target) r2 += loss_voxel(P, rc.ray * (size_t)nchan + c, Ic);
+        }
     }
+    if (P.target) loss_report(P, r2, lane);
     if (lane == 0 && n_steps) {
         atomicAdd(P.ws.counters + 0, (unsigned long long)n_steps);
         atomicAdd(P.ws.counters + 1, (unsigned long long)n_mufu);

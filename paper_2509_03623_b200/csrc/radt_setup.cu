@@ -247,6 +247,25 @@ __global__ void __launch_bounds__(256) k_l2_loss_grad(const float *__restrict__ 
     }
 }
 
+// Sum of the partial-loss slots of the fused forward (radt_march.cuh loss_report): loss = scale * sum; the slots are
+// cleared for the next call.
+__global__ void __launch_bounds__(RADT_LOSS_SLOTS) k_loss_finish(double *part, double scale, double *loss)
+{
+    double v = part[threadIdx.x];
+    part[threadIdx.x] = 0.0;
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
+    __shared__ double wsum[RADT_LOSS_SLOTS / 32];
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double s = wsum[threadIdx.x];
+#pragma unroll
+        for (int m = 16; m > 0; m >>= 1) s += __shfl_xor_sync(0xffffffffu, s, m);
+        if (threadIdx.x == 0) *loss = s * scale;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // host-side launchers
 // ---------------------------------------------------------------------------------------------
@@ -291,5 +310,11 @@ cudaError_t radt_launch_l2(const float *cube, const float *target, double sigma,
     long long nb = (n + 255) / 256;
     if (nb > 148 * 8) nb = 148 * 8;
     k_l2_loss_grad<<<(int)nb, 256, 0, st>>>(cube, target, (float)inv, 0.5 * inv, n, dl, loss);
+    return cudaGetLastError();
+}
+
+cudaError_t radt_launch_loss_finish(double *part, double scale, double *loss, cudaStream_t st)
+{
+    k_loss_finish<<<1, RADT_LOSS_SLOTS, 0, st>>>(part, scale, loss);
     return cudaGetLastError();
 }

@@ -53,10 +53,19 @@ class Renderer:
         B.radt_l2_loss_grad(self.cube, self.target, self.sigma, self.dl_dcube, self.loss, stream)
         return self.loss
 
-    def fit_step(self, stream=None):
+    def render_loss(self, stream=None):
+        """forward with the chi^2 data term fused into its epilogue: cube, dl_dcube and loss in one pass."""
+        B.radt_render_loss(self.desc, self.dens, self.temp, self.vel, self.target, self.sigma, self.cube, self.dl_dcube,
+                           self.loss, self.ws, stream)
+        return self.loss
+
+    def fit_step(self, stream=None, fused=True):
         """forward -> L2 data term -> adjoint (one pass of the whole hot path)."""
-        self.render(stream)
-        self.l2_loss_grad(stream)
+        if fused:
+            self.render_loss(stream)
+        else:
+            self.render(stream)
+            self.l2_loss_grad(stream)
         self.render_bwd(stream=stream)
 
     def set_fields(self, dens=None, temp=None, vel=None):

@@ -342,3 +342,30 @@ def test_ray_subset_matches_full():
     full = po.render(sc).reshape(-1, len(sc.line.vchan))
     idx = np.array([0, 5, 13, 24, 48])
     np.testing.assert_array_equal(po.render(sc, rays=idx), full[idx])
+
+
+# ---------------------------------------------------------------------------------------------
+# chi^2 data term: pins of oracle.pyoracle.chi2_loss_grad
+# ---------------------------------------------------------------------------------------------
+def test_chi2_constant_residual_and_zero():
+    rng = np.random.default_rng(5)
+    D = rng.normal(size=(3, 4, 5))
+    L, g = po.chi2_loss_grad(D + 0.3, D, 0.3)          # every residual is one sigma: chi^2/n = 1, L = 1/2
+    assert L == pytest.approx(0.5, rel=1e-12)
+    np.testing.assert_allclose(g, 1.0 / (0.3 * D.size), rtol=1e-12)
+    L0, g0 = po.chi2_loss_grad(D, D, 2.0)
+    assert L0 == 0.0 and not g0.any()
+
+
+def test_chi2_gradient_matches_finite_differences_and_scaling():
+    rng = np.random.default_rng(6)
+    I, D = rng.normal(size=(2, 3, 4)), rng.normal(size=(2, 3, 4))
+    L, g = po.chi2_loss_grad(I, D, 0.7)
+    for idx in [(0, 0, 0), (1, 2, 3), (0, 1, 2)]:
+        e = np.zeros_like(I)
+        e[idx] = 1e-6
+        fd = (po.chi2_loss_grad(I + e, D, 0.7)[0] - po.chi2_loss_grad(I - e, D, 0.7)[0]) / 2e-6
+        assert g[idx] == pytest.approx(fd, rel=1e-7)
+    # quadratic in the residual, inverse quadratic in sigma
+    assert po.chi2_loss_grad(D + 2 * (I - D), D, 0.7)[0] == pytest.approx(4 * L, rel=1e-12)
+    assert po.chi2_loss_grad(I, D, 1.4)[0] == pytest.approx(L / 4, rel=1e-12)
