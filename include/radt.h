@@ -172,7 +172,8 @@ int radt_render_loss(const radt_geom *geom, const radt_line *line, const radt_gr
  * after the results are in host memory. */
 int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                      float *cube);
-/* Forward with the fused L2 loss against `target` (HOST) + adjoint in one call; cube may be NULL. */
+/* Forward + L2 loss against `target` (HOST; uploaded on a second stream under the forward march) + adjoint in one
+ * call; cube may be NULL. */
 int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                        const float *target, double sigma, float *cube, double *loss_out,
                        float *g_dens, float *g_temp, float *g_vel);

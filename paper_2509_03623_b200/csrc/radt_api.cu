@@ -504,13 +504,28 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
         if (rc) return rc;
         launches += g_launches;
     } else if (mode == 1) {
-        // forward with the fused chi^2 data term
+        // The target cube is the bulk of the input bytes: its upload runs on a second stream under the forward
+        // march, and the chi^2 term follows as its own pass (the fused radt_render_loss would have to wait for it).
         if (!target) return fail(RADT_E_INVALID, "null target");
+        static thread_local cudaStream_t s2 = nullptr;
+        static thread_local cudaEvent_t ev_alloc = nullptr, ev_copied = nullptr;
+        if (!s2) {
+            CUDA_TRY(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+            CUDA_TRY(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&ev_copied, cudaEventDisableTiming));
+        }
         float *d_t = (float *)B.alloc(nvox * sizeof(float));
         double *d_loss = (double *)B.alloc(sizeof(double));
         if (!d_t || !d_loss) return fail(RADT_E_CUDA, "device allocation failed");
-        CUDA_TRY(cudaMemcpyAsync(d_t, target, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
-        rc = radt_render_loss(geom, line, &dgrid, batch, d_t, sigma, d_cube, d_dl, d_loss, ws, wsb, B.st);
+        CUDA_TRY(cudaEventRecord(ev_alloc, B.st));
+        CUDA_TRY(cudaStreamWaitEvent(s2, ev_alloc, 0));
+        CUDA_TRY(cudaMemcpyAsync(d_t, target, nvox * sizeof(float), cudaMemcpyHostToDevice, s2));
+        CUDA_TRY(cudaEventRecord(ev_copied, s2));
+        rc = radt_render(geom, line, &dgrid, batch, d_cube, ws, wsb, B.st);
+        if (rc) return rc;
+        launches += g_launches;
+        CUDA_TRY(cudaStreamWaitEvent(B.st, ev_copied, 0));
+        rc = radt_l2_loss_grad(d_cube, d_t, sigma, (int64_t)nvox, d_dl, d_loss, B.st);
         if (rc) return rc;
         launches += g_launches;
         if (loss_out) CUDA_TRY(cudaMemcpyAsync(loss_out, d_loss, sizeof(double), cudaMemcpyDeviceToHost, B.st));
