@@ -276,18 +276,24 @@ def run_ours(args):
         except Exception:      # noqa: BLE001
             traffic = None
 
-    def roof(kernel, t_ms, exec_samples, key):
-        achieved = 2.0 * exec_samples / (t_ms * 1e-3)       # 2 transcendental lane-ops per executed sample
-        return {"kernel": kernel, "bound": "alu", "achieved": achieved / 1e12, "peak": mufu_peak / 1e12,
-                "unit": "T MUFU lane-op/s", "frac": achieved / mufu_peak,
-                "frac_nominal": 2.0 * nominal / (t_ms * 1e-3) / mufu_peak,
-                "executed_samples": exec_samples, "ms": t_ms,
-                "peak_source": f"radt_pipe_peak(MUFU.EX2) measured in this run at {mufu_clk:.0f} MHz "
-                               "(MEASURED_PEAKS.json holds no SFU figure)",
+    def roof(kernel, t_ms, exec_samples, key, ops, peak, unit, why):
+        """ALGORITHMIC lane-operations of the executed samples (per-sample figure x samples one
+        launch executes) over the launch time, against the issue peak of the pipe that binds, measured in this run."""
+        achieved = ops * exec_samples / (t_ms * 1e-3)
+        return {"kernel": kernel, "bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": unit,
+                "frac": achieved / peak, "frac_nominal": ops * nominal / (t_ms * 1e-3) / peak,
+                "frac_mufu": 2.0 * exec_samples / (t_ms * 1e-3) / mufu_peak,
+                "ops_per_sample": ops, "executed_samples": exec_samples, "ms": t_ms,
+                "peak_source": f"{why}, measured by radt_pipe_peak in this run at {mufu_clk:.0f} MHz "
+                               "(MEASURED_PEAKS.json holds no SFU/FP32 issue figure)",
                 "traffic": (traffic or {}).get(key)}
 
-    r_f = roof("k_march_fwd (includes the fused setup launch)", t_fwd, fwd_exec, "k_march_fwd")
-    r_b = roof("k_march_bwd (includes setup and gradient unpack)", t_bwd, bwd_exec, "k_march_bwd")
+    # forward: 2 MUFU.EX2 + ~8 FP32 per sample -> the SFU pipe (16 lanes/clk/SM) binds before FP32 (128 lanes/clk/SM);
+    # adjoint: 2 MUFU.EX2 + ~20 FP32 per sample (SURVEY.md section 8(d)) -> 20/128 > 2/16: FP32 issue binds
+    r_f = roof("k_march_fwd (includes the fused setup launch)", t_fwd, fwd_exec, "k_march_fwd", 2.0, mufu_peak,
+               "T MUFU lane-op/s", "SFU issue peak (MUFU.EX2)")
+    r_b = roof("k_march_bwd (includes setup and gradient unpack)", t_bwd, bwd_exec, "k_march_bwd", 20.0, ffma_peak,
+               "T FP32 lane-op/s", "FP32 issue peak (FFMA)")
     dominant, other = (r_b, r_f) if t_bwd >= t_fwd else (r_f, r_b)
 
     # ---- e2e: the same step through the HOST-buffer C-ABI entry point, pinned host memory

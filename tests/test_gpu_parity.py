@@ -135,6 +135,19 @@ def test_inexact_channel_velocities_and_vsys(rt):
     _parity_fwd_bwd(rt, sc, "inexact channels")
 
 
+def test_channel_minibatch_random_subset(rt):
+    """Channel mini-batching of the fit (a random batch of 50 of the 115 slices per step; SURVEY.md
+    NEXT-2): the channel list is an input, so a seeded random subset of config 2's channels (not a lattice any more:
+    the channel-table kernels serve it) is rendered and differentiated like any cube, and equals those channels of
+    the full render."""
+    full = make_config(2, npix=40)
+    pick = np.sort(np.random.default_rng(221).choice(full.line.vchan.size, 28, replace=False))
+    sub = replace(full, line=replace(full.line, vchan=full.line.vchan[pick]))
+    R = _parity_fwd_bwd(rt, sub, "cfg2 channel subset")
+    Rf = _gpu_forward(rt, [full], need_bwd=False)
+    check_cube("subset vs full render", R.cube.cpu().numpy()[0], Rf.cube.cpu().numpy()[0][..., pick].astype(np.float64))
+
+
 # ------------------------------------------------------------------ the five configs
 def test_cfg1_full(rt):
     _parity_fwd_bwd(rt, make_config(1), "cfg1")
