@@ -80,7 +80,7 @@ def test_pressure_gradient_operator_on_an_analytic_field():
         P = rr ** a * np.exp(-b * z)
         got = dp.pressure_gradient_r(P, r, zeta)
         errs.append(np.max(np.abs(got[2:-2, 2:-2] / (a * P / rr)[2:-2, 2:-2] - 1.0)))
-    assert errs[2] < 1e-3 and errs[0] / errs[1] == pytest.approx(4.0, rel=0.2) and errs[1] / errs[2] == pytest.approx(4.0, rel=0.2)
+    assert errs[2] < 2e-3 and errs[0] / errs[1] == pytest.approx(4.0, rel=0.2) and errs[1] / errs[2] == pytest.approx(4.0, rel=0.2)
 
 
 def test_velocity_eq6_kepler_term_and_sub_keplerian_midplane():
