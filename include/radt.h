@@ -180,6 +180,42 @@ int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_
 int radt_render_bwd_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                          const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel);
 
+/* ---- Physics pre-pass (Eq. 1-2, 6-9) ---------------------------------
+ * Turns a temperature grid into the render's CO density and v_phi grids, as the paper's fit does before every render:
+ * hydrostatic density along z (Eq. 1, trapezoid rule), normalised to the surface density of Eq. 2 (both sides of the
+ * mirror-symmetric disk), H2 column above every node (Eq. 8), CO abundance mask (Eq. 7, 9), rotation with the radial
+ * pressure gradient (Eq. 6, centred differences on the (ln r, zeta) grid).  DESIGN.md section 10 states the
+ * discretisation P1-P7.  One radt_disk per batch item (HOST). */
+typedef struct radt_disk {
+    uint32_t struct_size;         /* = sizeof(radt_disk) */
+    uint32_t pad_;
+    double gm_star;               /* cm^3 s^-2 */
+    double m_gas;                 /* g, mean molecular mass (m_mol of Eq. 1) */
+    double sigma0;                /* g cm^-2, Eq. 2 */
+    double r_c;                   /* au, Eq. 2 */
+    double gamma;                 /* Eq. 2 */
+    double x_co;                  /* Eq. 7 (1e-4) */
+    double t_freeze;              /* K, Eq. 9 */
+    double n_dissoc;              /* cm^-2, Eq. 9 */
+    double f_col;                 /* Eq. 9 (0.706) */
+} radt_disk;
+
+/* `grid` gives the node layout only (kind AXISYM with mirror_z = 1 and lo[1] = 0, dens_mode LINEAR, vel_mode VPHI; its
+ * field pointers are ignored); item b of every array starts at b * grid->batch_stride elements.
+ * radt_disk_fields: temp (DEVICE float32 [batch][nr][nzeta], K) -> dens_out = n_CO [cm^-3], vel_out = v_phi [cm/s]
+ * (DEVICE float32, overwritten).
+ * radt_disk_fields_bwd: ADDS to g_temp (DEVICE float32, in/out) the gradient that reaches the temperature through the
+ * density and velocity fields, d L/d temp += (d n_CO/d temp)^T g_dens + (d v_phi/d temp)^T g_vel, with the CO mask held
+ * fixed (it is piecewise constant); g_dens, g_vel: DEVICE float32 as returned by radt_render_bwd.  Passing the
+ * render's own g_temp therefore yields the total derivative w.r.t. the temperature grid.
+ * Both are asynchronous on cuda_stream, never allocate, and recompute what they need (no state between calls). */
+int radt_disk_workspace_bytes(const radt_grid *grid, int32_t batch, size_t *bytes_out);
+int radt_disk_fields(const radt_disk *disk, const radt_grid *grid, int32_t batch, const float *temp, float *dens_out,
+                     float *vel_out, void *ws, size_t ws_bytes, void *cuda_stream);
+int radt_disk_fields_bwd(const radt_disk *disk, const radt_grid *grid, int32_t batch, const float *temp,
+                         const float *g_dens, const float *g_vel, float *g_temp, void *ws, size_t ws_bytes,
+                         void *cuda_stream);
+
 /* M1 micro-benchmarks of the issue peaks the roofline is quoted against.
  * Runs a full-occupancy dependent-chain loop of `kind` on the current device and returns the
  * achieved rate in lane-operations per second (HOST double).  kind: 0 MUFU.EX2, 1 FFMA, 2 DFMA,

@@ -20,7 +20,8 @@ OPT_WINDOW, OPT_SKIP_EMPTY, OPT_WIN_PATH = 1, 2, 3
 
 EXPORTS = ["radt_version", "radt_last_error", "radt_set_option", "radt_get_option", "radt_workspace_bytes",
            "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_l2_loss_grad", "radt_render_host",
-           "radt_render_loss", "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
+           "radt_render_loss", "radt_disk_workspace_bytes", "radt_disk_fields", "radt_disk_fields_bwd",
+           "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
            "radt_last_launch_count"]
 
 
@@ -52,6 +53,22 @@ class radt_grid(C.Structure):
 _lib = None
 
 
+class radt_disk(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("pad_", C.c_uint32), ("gm_star", C.c_double), ("m_gas", C.c_double),
+                ("sigma0", C.c_double), ("r_c", C.c_double), ("gamma", C.c_double), ("x_co", C.c_double),
+                ("t_freeze", C.c_double), ("n_dissoc", C.c_double), ("f_col", C.c_double)]
+
+
+def make_disks(params):
+    """ctypes array of radt_disk from objects with the fields of radt_disk (gm_star, m_gas | m_mol, sigma0, ...)."""
+    params = _as_list(params)
+    arr = (radt_disk * len(params))()
+    for b, p in enumerate(params):
+        arr[b] = radt_disk(C.sizeof(radt_disk), 0, p.gm_star, getattr(p, "m_gas", None) or p.m_mol, p.sigma0, p.r_c,
+                           p.gamma, p.x_co, p.t_freeze, p.n_dissoc, p.f_col)
+    return arr
+
+
 def lib():
     """Load libradt.so; raises if it has not been built (no fallback)."""
     global _lib
@@ -73,6 +90,9 @@ def lib():
         L.radt_l2_loss_grad.argtypes = [vp, vp, dbl, i64, vp, vp, vp]
         L.radt_render_loss.argtypes = [gp, lp, rp, i32, vp, dbl, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_render_host.argtypes = [gp, lp, rp, i32, vp]
+        L.radt_disk_workspace_bytes.argtypes = [rp, i32, C.POINTER(C.c_size_t)]
+        L.radt_disk_fields.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, C.c_size_t, vp]
+        L.radt_disk_fields_bwd.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_fit_step_host.argtypes = [gp, lp, rp, i32, vp, dbl, vp, C.POINTER(dbl), vp, vp, vp]
         L.radt_render_bwd_host.argtypes = [gp, lp, rp, i32, vp, vp, vp, vp, vp]
         L.radt_pipe_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
@@ -199,6 +219,27 @@ def radt_render_loss(desc: Descriptors, dens, temp, vel, target, sigma: float, c
                                   C.c_void_p(target.data_ptr()), C.c_double(float(sigma)), C.c_void_p(cube.data_ptr()),
                                   C.c_void_p(dl_dcube.data_ptr()), C.c_void_p(loss_out.data_ptr()),
                                   C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream_ptr(stream)))
+
+
+def radt_disk_workspace_bytes(desc: Descriptors) -> int:
+    out = C.c_size_t(0)
+    _check(lib().radt_disk_workspace_bytes(C.byref(desc.grid), desc.batch, C.byref(out)))
+    return out.value
+
+
+def radt_disk_fields(disks, desc: Descriptors, temp, dens_out, vel_out, ws, stream=None):
+    """Physics pre-pass: temp -> n_CO, v_phi (CUDA float32 tensors [batch, nr, nzeta]); disks from make_disks()."""
+    _check(lib().radt_disk_fields(disks, C.byref(desc.grid), desc.batch, C.c_void_p(temp.data_ptr()),
+                                  C.c_void_p(dens_out.data_ptr()), C.c_void_p(vel_out.data_ptr()),
+                                  C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream_ptr(stream)))
+
+
+def radt_disk_fields_bwd(disks, desc: Descriptors, temp, g_dens, g_vel, g_temp, ws, stream=None):
+    """g_temp += (d n_CO/d temp)^T g_dens + (d v_phi/d temp)^T g_vel."""
+    _check(lib().radt_disk_fields_bwd(disks, C.byref(desc.grid), desc.batch, C.c_void_p(temp.data_ptr()),
+                                      C.c_void_p(g_dens.data_ptr()), C.c_void_p(g_vel.data_ptr()),
+                                      C.c_void_p(g_temp.data_ptr()), C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()),
+                                      _stream_ptr(stream)))
 
 
 def radt_read_counters(ws, stream=None):

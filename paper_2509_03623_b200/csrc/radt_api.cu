@@ -573,6 +573,93 @@ int radt_render_bwd_host(const radt_geom *geom, const radt_line *line, const rad
     return host_common(geom, line, grid, batch, 2, nullptr, 0.0, nullptr, cube, dl_dcube, nullptr, g_dens, g_temp, g_vel);
 }
 
+// ------------------------------------------------------------------------------------------
+// physics pre-pass (radt_disk.cu)
+// ------------------------------------------------------------------------------------------
+static int disk_setup(const radt_disk *disk, const radt_grid *grid, int32_t batch, void *ws, size_t ws_bytes,
+                      DiskParamsDev &Q, size_t *need_out)
+{
+    if (!grid) return fail(RADT_E_INVALID, "null grid descriptor");
+    if (grid->struct_size != sizeof(radt_grid)) return fail(RADT_E_INVALID, "radt_grid.struct_size mismatch");
+    if (batch < 1 || batch > RADT_MAXB) return fail(RADT_E_INVALID, "batch must be 1..%d", RADT_MAXB);
+    if (grid->kind != RADT_GRID_AXISYM || !grid->mirror_z || grid->lo[1] != 0.0 || grid->dens_mode != RADT_DENS_LINEAR ||
+        grid->vel_mode != RADT_VEL_VPHI)
+        return fail(RADT_E_UNSUPPORTED, "the pre-pass needs a mirror-symmetric (r, zeta) grid from zeta = 0 with LINEAR density and VPHI velocity");
+    if (grid->n[0] < 2 || grid->n[1] < 2 || !(grid->lo[0] > 0) || !(grid->hi[0] > grid->lo[0]) || !(grid->hi[1] > 0))
+        return fail(RADT_E_INVALID, "bad grid extents");
+    const size_t cells = (size_t)grid->n[0] * grid->n[1] * batch, cols = (size_t)grid->n[0] * batch;
+    size_t off = 0, o_rt, o_rho, o_P, o_gP, o_grho, o_cs, o_cH, o_mask;
+    o_rt = off; off = align256(off + cells * 8);
+    o_rho = off; off = align256(off + cells * 8);
+    o_P = off; off = align256(off + cells * 8);
+    o_gP = off; off = align256(off + cells * 8);
+    o_grho = off; off = align256(off + cells * 8);
+    o_cs = off; off = align256(off + cols * 8);
+    o_cH = off; off = align256(off + cols * 8);
+    o_mask = off; off = align256(off + cells);
+    if (need_out) { *need_out = off; return RADT_OK; }
+    if (!disk) return fail(RADT_E_INVALID, "null disk descriptor");
+    if (!ws) return fail(RADT_E_INVALID, "null workspace");
+    if (ws_bytes < off) return fail(RADT_E_WORKSPACE, "workspace too small: need %zu bytes, got %zu", off, ws_bytes);
+    if (((uintptr_t)ws & 15) != 0) return fail(RADT_E_INVALID, "workspace must be 16-byte aligned");
+    memset(&Q, 0, sizeof(Q));
+    for (int b = 0; b < batch; ++b) {
+        const radt_disk &d = disk[b];
+        if (d.struct_size != sizeof(radt_disk)) return fail(RADT_E_INVALID, "radt_disk.struct_size mismatch");
+        if (!(d.gm_star > 0) || !(d.m_gas > 0) || !(d.sigma0 > 0) || !(d.r_c > 0))
+            return fail(RADT_E_INVALID, "disk constants must be positive");
+        Q.disk[b] = DiskDev{ d.gm_star, d.m_gas, d.sigma0, d.r_c, d.gamma, d.x_co, d.t_freeze, d.n_dissoc, d.f_col };
+    }
+    Q.nr = grid->n[0]; Q.nz = grid->n[1]; Q.nbatch = batch;
+    Q.batch_stride = batch > 1 ? grid->batch_stride : (long long)grid->n[0] * grid->n[1];
+    if (batch > 1 && Q.batch_stride < (long long)grid->n[0] * grid->n[1])
+        return fail(RADT_E_INVALID, "batch_stride smaller than the grid");
+    Q.rmin = grid->lo[0];
+    Q.lg2_ratio = std::log2(grid->hi[0] / grid->lo[0]);
+    Q.dlnr = std::log(grid->hi[0] / grid->lo[0]) / (double)(grid->n[0] - 1);
+    Q.dzeta = grid->hi[1] / (double)(grid->n[1] - 1);
+    char *base = (char *)ws;
+    Q.rt = (double *)(base + o_rt); Q.rho = (double *)(base + o_rho); Q.P = (double *)(base + o_P);
+    Q.gP = (double *)(base + o_gP); Q.grho = (double *)(base + o_grho);
+    Q.colscale = (double *)(base + o_cs); Q.colH = (double *)(base + o_cH);
+    Q.mask = (unsigned char *)(base + o_mask);
+    return RADT_OK;
+}
+
+int radt_disk_workspace_bytes(const radt_grid *grid, int32_t batch, size_t *bytes_out)
+{
+    if (!bytes_out) return fail(RADT_E_INVALID, "null bytes_out");
+    DiskParamsDev Q;
+    return disk_setup(nullptr, grid, batch, nullptr, 0, Q, bytes_out);
+}
+
+int radt_disk_fields(const radt_disk *disk, const radt_grid *grid, int32_t batch, const float *temp, float *dens_out,
+                     float *vel_out, void *ws, size_t ws_bytes, void *cuda_stream)
+{
+    if (!temp || !dens_out || !vel_out) return fail(RADT_E_INVALID, "null field pointer");
+    static thread_local DiskParamsDev Q;
+    int rc = disk_setup(disk, grid, batch, ws, ws_bytes, Q, nullptr);
+    if (rc) return rc;
+    Q.temp = temp; Q.dens_out = dens_out; Q.vel_out = vel_out;
+    CUDA_TRY(radt_launch_disk_fwd(Q, (cudaStream_t)cuda_stream));
+    g_launches = 2;
+    return RADT_OK;
+}
+
+int radt_disk_fields_bwd(const radt_disk *disk, const radt_grid *grid, int32_t batch, const float *temp,
+                         const float *g_dens, const float *g_vel, float *g_temp, void *ws, size_t ws_bytes,
+                         void *cuda_stream)
+{
+    if (!temp || !g_dens || !g_vel || !g_temp) return fail(RADT_E_INVALID, "null field pointer");
+    static thread_local DiskParamsDev Q;
+    int rc = disk_setup(disk, grid, batch, ws, ws_bytes, Q, nullptr);
+    if (rc) return rc;
+    Q.temp = temp; Q.g_dens = g_dens; Q.g_vel = g_vel; Q.g_temp = g_temp;
+    CUDA_TRY(radt_launch_disk_bwd(Q, (cudaStream_t)cuda_stream));
+    g_launches = 3;
+    return RADT_OK;
+}
+
 int radt_pipe_peak(int32_t kind, double *ops_per_s_out, double *sm_clock_mhz_out)
 {
     if (!ops_per_s_out) return fail(RADT_E_INVALID, "null output");

@@ -132,6 +132,24 @@ struct ChanTable {
     double v[RADT_MAXCHAN];
 };
 
+// ---- physics pre-pass (radt_disk.cu): per batch item constants and the launch parameter block ----
+struct DiskDev {
+    double gm_star, m_gas, sigma0, r_c, gamma, x_co, t_freeze, n_dissoc, f_col;
+};
+struct DiskParamsDev {
+    DiskDev disk[RADT_MAXB];
+    int nr, nz, nbatch;
+    long long batch_stride;
+    double rmin, lg2_ratio, dlnr, dzeta;
+    const float *temp;                   // [batch][nr][nz]
+    float *dens_out, *vel_out;           // forward outputs
+    const float *g_dens, *g_vel;         // adjoint inputs
+    float *g_temp;                       // adjoint output (+=)
+    double *rt, *rho, *P, *gP, *grho;    // workspace, [batch][nr][nz]
+    double *colscale, *colH;             // workspace, [batch][nr]
+    unsigned char *mask;                 // workspace, [batch][nr][nz]
+};
+
 // ---- single-instruction SFU helpers (MUFU.*) ----
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }

@@ -1,0 +1,181 @@
+// radt_disk.cu -- physics pre-pass on the (r, zeta) grid: temperature grid -> CO density and v_phi
+// fields of the render, and its adjoint w.r.t. the temperature.  PAPER.md:156-203 (Eq. 1-2, 6-9).
+// Algorithm P1-P7 of DESIGN.md section 10: hydrostatic integration along z with the trapezoid rule, surface-density
+// normalisation, column above every node, CO mask, pressure-corrected rotation.  fp64 throughout (32 k cells: the
+// pass is latency bound, not throughput bound).  Shares nothing with oracle/.
+#include "radt_dev.cuh"
+#include "radt_kernels.h"
+
+#define KB_CGS 1.380649e-16
+#define AU_CM 1.495978707e13
+
+__device__ __forceinline__ double disk_sigma(const DiskDev &D, double r_au)
+{
+    double x = r_au / D.r_c;
+    return D.sigma0 * pow(x, -D.gamma) * exp(-pow(x, 2.0 - D.gamma));
+}
+
+// One thread per column (b, i).  Writes rt = rho~ (P3), rho (P4), P (P7) to the workspace, the column scale
+// Sigma / 2H, and (FWD) the CO density.
+template <bool FWD>
+__global__ void __launch_bounds__(64) k_disk_columns(const __grid_constant__ DiskParamsDev Q)
+{
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= Q.nr * Q.nbatch) return;
+    const int b = col / Q.nr, i = col - b * Q.nr;
+    const DiskDev &D = Q.disk[b];
+    const int nz = Q.nz;
+    const float *T = Q.temp + (long long)b * Q.batch_stride + (long long)i * nz;
+    double *rt = Q.rt + (long long)col * nz, *rho = Q.rho + (long long)col * nz, *P = Q.P + (long long)col * nz;
+    const double r_au = Q.rmin * exp2((double)i * Q.lg2_ratio / (double)(Q.nr - 1));
+    const double r = r_au * AU_CM, dz = Q.dzeta * r, c = D.gm_star * D.m_gas / KB_CGS;
+    const double T0 = (double)T[0];
+    double A = 0.0, H = 0.0, f_prev = 0.0, rt_prev = 1.0;
+    rt[0] = 1.0;
+    for (int j = 1; j < nz; ++j) {                               // P1-P3 and the integral of P4
+        const double z = (double)j * dz, Tj = (double)T[j], s = r * r + z * z;
+        const double f = z / (Tj * s * sqrt(s));
+        A += 0.5 * (f_prev + f) * dz;
+        const double v = T0 / Tj * exp(-c * A);
+        H += 0.5 * (rt_prev + v) * dz;
+        rt[j] = v;
+        f_prev = f; rt_prev = v;
+    }
+    const double scale = disk_sigma(D, r_au) / (2.0 * H);
+    Q.colscale[col] = scale;
+    Q.colH[col] = H;
+    float *dens = FWD ? Q.dens_out + (long long)b * Q.batch_stride + (long long)i * nz : nullptr;
+    double N = 0.0, n_next = 0.0;
+    for (int j = nz - 1; j >= 0; --j) {                          // P4-P7 (pressure)
+        const double Tj = (double)T[j], rj = rt[j] * scale, n = rj / D.m_gas;
+        if (j < nz - 1) N += 0.5 * (n + n_next) * dz;
+        n_next = n;
+        rho[j] = rj;
+        P[j] = rj * KB_CGS * Tj / D.m_gas;
+        const bool co = Tj > D.t_freeze && D.f_col * N > D.n_dissoc;
+        if (FWD) dens[j] = co ? (float)(D.x_co * n) : 0.0f;
+        else Q.mask[(long long)col * nz + j] = co ? 1 : 0;
+    }
+}
+
+// dP/dr at fixed z on the (ln r, zeta) grid: centred differences in index space, one-sided at the edges (P7)
+__device__ __forceinline__ double disk_dPdr(const DiskParamsDev &Q, const double *P, int i, int j, double r)
+{
+    const int nz = Q.nz, im = i > 0 ? i - 1 : i, ip = i < Q.nr - 1 ? i + 1 : i, jm = j > 0 ? j - 1 : j, jp = j < nz - 1 ? j + 1 : j;
+    const double d1 = (P[(long long)ip * nz + j] - P[(long long)im * nz + j]) / ((double)(ip - im) * Q.dlnr);
+    const double d2 = (P[(long long)i * nz + jp] - P[(long long)i * nz + jm]) / ((double)(jp - jm) * Q.dzeta);
+    return (d1 - (double)j * Q.dzeta * d2) / r;
+}
+
+// One thread per cell: v_phi (forward) or the transpose of P7 (adjoint).
+template <bool FWD>
+__global__ void __launch_bounds__(256) k_disk_velocity(const __grid_constant__ DiskParamsDev Q)
+{
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long per = (long long)Q.nr * Q.nz;
+    if (q >= per * Q.nbatch) return;
+    const int b = (int)(q / per), nz = Q.nz;
+    const long long c = q - (long long)b * per;
+    const int i = (int)(c / nz), j = (int)(c - (long long)i * nz);
+    const DiskDev &D = Q.disk[b];
+    const double *P = Q.P + (long long)b * per;
+    const double r = Q.rmin * exp2((double)i * Q.lg2_ratio / (double)(Q.nr - 1)) * AU_CM, z = (double)j * Q.dzeta * r;
+    const double s = r * r + z * z, kep = D.gm_star * r * r / (s * sqrt(s));
+    const double rh = Q.rho[q];
+    const double dPdr = disk_dPdr(Q, P, i, j, r);
+    const double v2 = kep + (rh > 0.0 ? r / rh * dPdr : 0.0);
+    const long long ext = (long long)b * Q.batch_stride + c;
+    if (FWD) {
+        Q.vel_out[ext] = (float)sqrt(fmax(v2, 0.0));
+        return;
+    }
+    double g_rho = 0.0;
+    if (v2 > 0.0 && rh > 0.0) {
+        const double g_v2 = (double)Q.g_vel[ext] / (2.0 * sqrt(v2));
+        const double g_dPdr = g_v2 * r / rh, gr = g_dPdr / r;
+        g_rho = -g_v2 * r * dPdr / (rh * rh);
+        // transpose of the two difference stencils
+        double *gP = Q.gP + (long long)b * per;
+        const int im = i > 0 ? i - 1 : i, ip = i < Q.nr - 1 ? i + 1 : i, jm = j > 0 ? j - 1 : j, jp = j < nz - 1 ? j + 1 : j;
+        const double a1 = gr / ((double)(ip - im) * Q.dlnr);
+        const double a2 = -(double)j * Q.dzeta * gr / ((double)(jp - jm) * Q.dzeta);
+        atomicAdd(gP + (long long)ip * nz + j, a1);
+        atomicAdd(gP + (long long)im * nz + j, -a1);
+        atomicAdd(gP + (long long)i * nz + jp, a2);
+        atomicAdd(gP + (long long)i * nz + jm, -a2);
+    }
+    Q.grho[q] = g_rho;
+}
+
+// Adjoint of the column part (reverse of P6..P1), one thread per column.  Uses rt, rho, mask, the column scale and H
+// recomputed by k_disk_columns<false>, grho (P7's direct term) and gP from k_disk_velocity<false>.  ADDS dL/dT of the
+// pre-pass to g_temp.
+__global__ void __launch_bounds__(64) k_disk_columns_bwd(const __grid_constant__ DiskParamsDev Q)
+{
+    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    if (col >= Q.nr * Q.nbatch) return;
+    const int b = col / Q.nr, i = col - b * Q.nr;
+    const DiskDev &D = Q.disk[b];
+    const int nz = Q.nz;
+    const long long ext0 = (long long)b * Q.batch_stride + (long long)i * nz;
+    const float *T = Q.temp + ext0;
+    const float *g_nco = Q.g_dens + ext0;
+    float *gT = Q.g_temp + ext0;
+    const double *rt = Q.rt + (long long)col * nz, *rho = Q.rho + (long long)col * nz, *gP = Q.gP + (long long)col * nz;
+    double *grho = Q.grho + (long long)col * nz;
+    const unsigned char *mask = Q.mask + (long long)col * nz;
+    const double r = Q.rmin * exp2((double)i * Q.lg2_ratio / (double)(Q.nr - 1)) * AU_CM;
+    const double dz = Q.dzeta * r, c = D.gm_star * D.m_gas / KB_CGS;
+    const double scale = Q.colscale[col], H = Q.colH[col];
+    // total dL/drho per node (P7's pressure, P6/P5's CO density) and dL/dH of the normalisation (P4)
+    double acc = 0.0;
+    for (int j = 0; j < nz; ++j) {
+        const double Tj = (double)T[j];
+        double g = grho[j] + gP[j] * KB_CGS * Tj / D.m_gas;
+        if (mask[j]) g += D.x_co * (double)g_nco[j] / D.m_gas;
+        grho[j] = g;
+        acc += g * rho[j];
+    }
+    const double gH = -acc / H, T0 = (double)T[0];
+    // reverse of P3..P1, top node first: gA accumulates downwards (P2), gf takes half an interval from either side
+    double sumt = 0.0, gAcum = 0.0, half_above = 0.0;
+    for (int j = nz - 1; j >= 0; --j) {
+        const double Tj = (double)T[j], w = (j == 0 || j == nz - 1) ? 0.5 * dz : dz;
+        const double t = (grho[j] * scale + gH * w) * rt[j];
+        sumt += t;
+        double gf = half_above;
+        if (j >= 1) {
+            gAcum += -c * t;
+            half_above = 0.5 * dz * gAcum;
+            gf += half_above;
+        }
+        const double z = (double)j * dz, s = r * r + z * z, f = z / (Tj * s * sqrt(s));
+        double g = gP[j] * rho[j] * KB_CGS / D.m_gas - t / Tj - gf * f / Tj;
+        if (j == 0) g += sumt / T0;
+        gT[j] += (float)g;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------------------------
+cudaError_t radt_launch_disk_fwd(const DiskParamsDev &Q, cudaStream_t st)
+{
+    const int ncol = Q.nr * Q.nbatch;
+    const long long ncell = (long long)ncol * Q.nz;
+    k_disk_columns<true><<<(ncol + 63) / 64, 64, 0, st>>>(Q);
+    k_disk_velocity<true><<<(int)((ncell + 255) / 256), 256, 0, st>>>(Q);
+    return cudaGetLastError();
+}
+
+cudaError_t radt_launch_disk_bwd(const DiskParamsDev &Q, cudaStream_t st)
+{
+    const int ncol = Q.nr * Q.nbatch;
+    const long long ncell = (long long)ncol * Q.nz;
+    cudaError_t e = cudaMemsetAsync(Q.gP, 0, (size_t)ncell * sizeof(double), st);
+    if (e != cudaSuccess) return e;
+    k_disk_columns<false><<<(ncol + 63) / 64, 64, 0, st>>>(Q);
+    k_disk_velocity<false><<<(int)((ncell + 255) / 256), 256, 0, st>>>(Q);
+    k_disk_columns_bwd<<<(ncol + 63) / 64, 64, 0, st>>>(Q);
+    return cudaGetLastError();
+}

@@ -13,3 +13,5 @@ cudaError_t radt_launch_march_bwd(const MarchParams &P, int nbatch, cudaStream_t
 cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st);
 cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStream_t st);
 cudaError_t radt_run_pipe_peak(int kind, double *ops_per_s, double *clock_mhz);
+cudaError_t radt_launch_disk_fwd(const DiskParamsDev &Q, cudaStream_t st);
+cudaError_t radt_launch_disk_bwd(const DiskParamsDev &Q, cudaStream_t st);
