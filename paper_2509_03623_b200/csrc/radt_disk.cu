@@ -15,45 +15,103 @@ __device__ __forceinline__ double disk_sigma(const DiskDev &D, double r_au)
     return D.sigma0 * pow(x, -D.gamma) * exp(-pow(x, 2.0 - D.gamma));
 }
 
-// One thread per column (b, i).  Writes rt = rho~ (P3), rho (P4), P (P7) to the workspace, the column scale
-// Sigma / 2H, and (FWD) the CO density.
-template <bool FWD>
-__global__ void __launch_bounds__(64) k_disk_columns(const __grid_constant__ DiskParamsDev Q)
+// Warp-wide scans over the lanes' chunk totals (fp64)
+__device__ __forceinline__ double warp_excl_scan_up(double v, int lane)        // sum of the lanes below
 {
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    double inc = v;
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) {
+        const double t = __shfl_up_sync(0xffffffffu, inc, m);
+        if (lane >= m) inc += t;
+    }
+    return inc - v;
+}
+__device__ __forceinline__ double warp_excl_scan_down(double v, int lane)      // sum of the lanes above
+{
+    double inc = v;
+#pragma unroll
+    for (int m = 1; m < 32; m <<= 1) {
+        const double t = __shfl_down_sync(0xffffffffu, inc, m);
+        if (lane + m < 32) inc += t;
+    }
+    return inc - v;
+}
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
+    return v;
+}
+
+// One WARP per column (b, i); lane l owns the nodes [l C, (l+1) C), C = ceil(nz / 32): the expensive terms (sqrt, exp)
+// of different nodes are independent, only the running sums of P2, P4 and P5 are scans (a thread per column was a chain
+// of nz fp64 exp: 0.12 ms for 128 nodes).  Writes rt = rho~ (P3), rho (P4), P (P7) to the workspace, the column
+// scale Sigma / 2H and H, and the CO density (FWD) or the mask (adjoint).
+template <bool FWD>
+__global__ void __launch_bounds__(128) k_disk_columns(const __grid_constant__ DiskParamsDev Q)
+{
+    const int col = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (col >= Q.nr * Q.nbatch) return;
     const int b = col / Q.nr, i = col - b * Q.nr;
     const DiskDev &D = Q.disk[b];
-    const int nz = Q.nz;
+    const int nz = Q.nz, C = (nz + 31) >> 5, j0 = min(lane * C, nz), j1 = min(j0 + C, nz);
     const float *T = Q.temp + (long long)b * Q.batch_stride + (long long)i * nz;
     double *rt = Q.rt + (long long)col * nz, *rho = Q.rho + (long long)col * nz, *P = Q.P + (long long)col * nz;
     const double r_au = Q.rmin * exp2((double)i * Q.lg2_ratio / (double)(Q.nr - 1));
     const double r = r_au * AU_CM, dz = Q.dzeta * r, c = D.gm_star * D.m_gas / KB_CGS;
     const double T0 = (double)T[0];
-    double A = 0.0, H = 0.0, f_prev = 0.0, rt_prev = 1.0;
-    rt[0] = 1.0;
-    for (int j = 1; j < nz; ++j) {                               // P1-P3 and the integral of P4
-        const double z = (double)j * dz, Tj = (double)T[j], s = r * r + z * z;
-        const double f = z / (Tj * s * sqrt(s));
-        A += 0.5 * (f_prev + f) * dz;
-        const double v = T0 / Tj * exp(-c * A);
-        H += 0.5 * (rt_prev + v) * dz;
-        rt[j] = v;
-        f_prev = f; rt_prev = v;
+    auto fgrav = [&](int j) {                                     // P1
+        const double z = (double)j * dz, s = r * r + z * z;
+        return z / ((double)T[j] * s * sqrt(s));
+    };
+    // P2: A_j, chunk-local running sum first (kept in rho[] as scratch), then the offset of the lanes below
+    double f_prev = j0 > 0 && j0 < nz ? fgrav(j0 - 1) : 0.0, a = 0.0;
+    for (int j = j0; j < j1; ++j) {
+        const double f = fgrav(j);
+        if (j > 0) a += 0.5 * (f_prev + f) * dz;
+        rho[j] = a;
+        f_prev = f;
     }
+    const double a_off = warp_excl_scan_up(a, lane);
+    // P3 and the integral of P4
+    double first = 0.0, last = 0.0;
+    for (int j = j0; j < j1; ++j) {
+        const double v = T0 / (double)T[j] * exp(-c * (a_off + rho[j]));
+        rt[j] = v;
+        if (j == j0) first = v;
+        last = v;
+    }
+    // the value just below / above the chunk (empty chunks sit at the top and pass nothing on)
+    double below = __shfl_up_sync(0xffffffffu, last, 1), above = __shfl_down_sync(0xffffffffu, first, 1);
+    double h = 0.0, prev = below;
+    for (int j = j0; j < j1; ++j) {
+        const double v = rt[j];
+        if (j > 0) h += 0.5 * (prev + v) * dz;
+        prev = v;
+    }
+    const double H = warp_sum(h);
     const double scale = disk_sigma(D, r_au) / (2.0 * H);
-    Q.colscale[col] = scale;
-    Q.colH[col] = H;
+    if (lane == 0) { Q.colscale[col] = scale; Q.colH[col] = H; }
+    // P5: column above every node: chunk-local from the chunk's top node down, plus everything in the lanes above
+    double nloc = 0.0, next = above;
+    for (int j = j1 - 1; j >= j0; --j) {
+        const double v = rt[j];
+        if (j < nz - 1) nloc += 0.5 * (v + next) * dz;
+        next = v;
+    }
+    const double n_off = warp_excl_scan_down(nloc, lane);
     float *dens = FWD ? Q.dens_out + (long long)b * Q.batch_stride + (long long)i * nz : nullptr;
-    double N = 0.0, n_next = 0.0;
-    for (int j = nz - 1; j >= 0; --j) {                          // P4-P7 (pressure)
-        const double Tj = (double)T[j], rj = rt[j] * scale, n = rj / D.m_gas;
-        if (j < nz - 1) N += 0.5 * (n + n_next) * dz;
-        n_next = n;
+    const double nscale = scale / D.m_gas;
+    double N = n_off;
+    next = above;
+    for (int j = j1 - 1; j >= j0; --j) {                         // P4-P7 (pressure)
+        const double v = rt[j], Tj = (double)T[j], rj = v * scale;
+        if (j < nz - 1) N += 0.5 * (v + next) * dz;
+        next = v;
         rho[j] = rj;
         P[j] = rj * KB_CGS * Tj / D.m_gas;
-        const bool co = Tj > D.t_freeze && D.f_col * N > D.n_dissoc;
-        if (FWD) dens[j] = co ? (float)(D.x_co * n) : 0.0f;
+        const bool co = Tj > D.t_freeze && D.f_col * (N * nscale) > D.n_dissoc;
+        if (FWD) dens[j] = co ? (float)(D.x_co * rj / D.m_gas) : 0.0f;
         else Q.mask[(long long)col * nz + j] = co ? 1 : 0;
     }
 }
@@ -107,16 +165,16 @@ __global__ void __launch_bounds__(256) k_disk_velocity(const __grid_constant__ D
     Q.grho[q] = g_rho;
 }
 
-// Adjoint of the column part (reverse of P6..P1), one thread per column.  Uses rt, rho, mask, the column scale and H
-// recomputed by k_disk_columns<false>, grho (P7's direct term) and gP from k_disk_velocity<false>.  ADDS dL/dT of the
-// pre-pass to g_temp.
-__global__ void __launch_bounds__(64) k_disk_columns_bwd(const __grid_constant__ DiskParamsDev Q)
+// Adjoint of the column part (reverse of P6..P1), one warp per column, lanes over chunks of nodes as above.  Uses
+// rt, rho, mask, the column scale and H recomputed by k_disk_columns<false>, grho (P7's direct term) and gP from
+// k_disk_velocity<false>.  ADDS dL/dT of the pre-pass to g_temp.
+__global__ void __launch_bounds__(128) k_disk_columns_bwd(const __grid_constant__ DiskParamsDev Q)
 {
-    const int col = blockIdx.x * blockDim.x + threadIdx.x;
+    const int col = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (col >= Q.nr * Q.nbatch) return;
     const int b = col / Q.nr, i = col - b * Q.nr;
     const DiskDev &D = Q.disk[b];
-    const int nz = Q.nz;
+    const int nz = Q.nz, C = (nz + 31) >> 5, j0 = min(lane * C, nz), j1 = min(j0 + C, nz);
     const long long ext0 = (long long)b * Q.batch_stride + (long long)i * nz;
     const float *T = Q.temp + ext0;
     const float *g_nco = Q.g_dens + ext0;
@@ -129,20 +187,28 @@ __global__ void __launch_bounds__(64) k_disk_columns_bwd(const __grid_constant__
     const double scale = Q.colscale[col], H = Q.colH[col];
     // total dL/drho per node (P7's pressure, P6/P5's CO density) and dL/dH of the normalisation (P4)
     double acc = 0.0;
-    for (int j = 0; j < nz; ++j) {
-        const double Tj = (double)T[j];
-        double g = grho[j] + gP[j] * KB_CGS * Tj / D.m_gas;
+    for (int j = j0; j < j1; ++j) {
+        double g = grho[j] + gP[j] * KB_CGS * (double)T[j] / D.m_gas;
         if (mask[j]) g += D.x_co * (double)g_nco[j] / D.m_gas;
         grho[j] = g;
         acc += g * rho[j];
     }
-    const double gH = -acc / H, T0 = (double)T[0];
-    // reverse of P3..P1, top node first: gA accumulates downwards (P2), gf takes half an interval from either side
-    double sumt = 0.0, gAcum = 0.0, half_above = 0.0;
-    for (int j = nz - 1; j >= 0; --j) {
-        const double Tj = (double)T[j], w = (j == 0 || j == nz - 1) ? 0.5 * dz : dz;
+    const double gH = -warp_sum(acc) / H, T0 = (double)T[0];
+    // t_j = dL/drt_j rt_j; gA accumulates from the top node down (P2): chunk-local sum plus the lanes above
+    double tsum = 0.0, asum = 0.0;
+    for (int j = j0; j < j1; ++j) {
+        const double w = (j == 0 || j == nz - 1) ? 0.5 * dz : dz;
         const double t = (grho[j] * scale + gH * w) * rt[j];
-        sumt += t;
+        grho[j] = t;                                              // keep t_j
+        tsum += t;
+        if (j >= 1) asum += -c * t;
+    }
+    const double sumt = warp_sum(tsum);
+    const double a_above = warp_excl_scan_down(asum, lane);
+    // gAcum of the first node of the chunk above (= a_above when that node exists and is >= 1)
+    double gAcum = a_above, half_above = (j1 < nz) ? 0.5 * dz * a_above : 0.0;
+    for (int j = j1 - 1; j >= j0; --j) {
+        const double Tj = (double)T[j], t = grho[j];
         double gf = half_above;
         if (j >= 1) {
             gAcum += -c * t;
@@ -163,7 +229,7 @@ cudaError_t radt_launch_disk_fwd(const DiskParamsDev &Q, cudaStream_t st)
 {
     const int ncol = Q.nr * Q.nbatch;
     const long long ncell = (long long)ncol * Q.nz;
-    k_disk_columns<true><<<(ncol + 63) / 64, 64, 0, st>>>(Q);
+    k_disk_columns<true><<<(ncol + 3) / 4, 128, 0, st>>>(Q);
     k_disk_velocity<true><<<(int)((ncell + 255) / 256), 256, 0, st>>>(Q);
     return cudaGetLastError();
 }
@@ -174,8 +240,8 @@ cudaError_t radt_launch_disk_bwd(const DiskParamsDev &Q, cudaStream_t st)
     const long long ncell = (long long)ncol * Q.nz;
     cudaError_t e = cudaMemsetAsync(Q.gP, 0, (size_t)ncell * sizeof(double), st);
     if (e != cudaSuccess) return e;
-    k_disk_columns<false><<<(ncol + 63) / 64, 64, 0, st>>>(Q);
+    k_disk_columns<false><<<(ncol + 3) / 4, 128, 0, st>>>(Q);
     k_disk_velocity<false><<<(int)((ncell + 255) / 256), 256, 0, st>>>(Q);
-    k_disk_columns_bwd<<<(ncol + 63) / 64, 64, 0, st>>>(Q);
+    k_disk_columns_bwd<<<(ncol + 3) / 4, 128, 0, st>>>(Q);
     return cudaGetLastError();
 }
