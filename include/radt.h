@@ -216,6 +216,29 @@ int radt_disk_fields_bwd(const radt_disk *disk, const radt_grid *grid, int32_t b
                          const float *g_dens, const float *g_vel, float *g_temp, void *ws, size_t ws_bytes,
                          void *cuda_stream);
 
+/* ---- Symmetric MLP temperature field (Eq. 10) ----------------------------------------
+ * T(r, |z|) = MLP_w(gamma(r, |z|)) on the nodes of an AXISYM grid (mirror symmetric, so a function of |z|):
+ * p = (i/(nr-1), j/(nzeta-1)); gamma(p) = (p_0, p_1, {sin(2^k pi p_0), cos(2^k pi p_0), sin(2^k pi p_1), cos(2^k pi p_1)},
+ * k = 0..L-1); `nhidden` fully connected layers of `width` units with ReLU; T = t_lo + (t_hi - t_lo) sigmoid(w . h + b).
+ * Parameters: one flat DEVICE float32 vector [W_1 (width x D) | b_1 | W_2 (width x width) | b_2 | ... | w_out (width) |
+ * b_out], row-major, D = 2 + 4 L; its length comes from radt_mlp_num_params.  This build supports width = 64,
+ * nhidden = 4 (the paper's network) and L <= 8. */
+typedef struct radt_mlp {
+    uint32_t struct_size;         /* = sizeof(radt_mlp) */
+    int32_t L;                    /* degree of the positional encoding (paper: 4) */
+    int32_t width, nhidden;       /* 64, 4 */
+    double t_lo, t_hi;            /* K (paper: 5, 400) */
+} radt_mlp;
+
+int radt_mlp_num_params(const radt_mlp *mlp, int64_t *count_out);
+/* temp_out: DEVICE float32 [nr][nzeta] (overwritten).  grid: node counts only (kind AXISYM). */
+int radt_mlp_temperature(const radt_mlp *mlp, const radt_grid *grid, const float *params, float *temp_out,
+                         void *cuda_stream);
+/* g_params (DEVICE float32 [num_params], OVERWRITTEN) = (dT/dparams)^T g_temp; g_temp: DEVICE float32 [nr][nzeta].
+ * Recomputes the activations (nothing is kept from the forward); float atomics make the last bits order dependent. */
+int radt_mlp_temperature_bwd(const radt_mlp *mlp, const radt_grid *grid, const float *params, const float *g_temp,
+                             float *g_params, void *cuda_stream);
+
 /* M1 micro-benchmarks of the issue peaks the roofline is quoted against.
  * Runs a full-occupancy dependent-chain loop of `kind` on the current device and returns the
  * achieved rate in lane-operations per second (HOST double).  kind: 0 MUFU.EX2, 1 FFMA, 2 DFMA,

@@ -77,6 +77,20 @@ def forward(params, nr: int, nz: int, L: int = 4, t_lo: float = 5.0, t_hi: float
     return (T, acts, s) if keep else T
 
 
+def near_kink(params, nr: int, nz: int, L: int = 4, tol: float = 1e-4):
+    """Nodes [nr][nz] where some hidden pre-activation lies within `tol` of the ReLU kink: there the derivative is a
+    subgradient (any value between the two one-sided ones is valid) and lower-precision arithmetic may take the other
+    branch, so parity tests give such nodes no incoming gradient."""
+    layers = split(params, L)
+    a = encode(nr, nz, L)
+    bad = np.zeros(a.shape[0], dtype=bool)
+    for W, b in layers[:-1]:
+        x = a @ W.T + b
+        bad |= np.any(np.abs(x) < tol * np.maximum(1.0, np.abs(a).max()), axis=1)
+        a = np.maximum(x, 0.0)
+    return bad.reshape(nr, nz)
+
+
 def adjoint(params, g_temp, nr: int, nz: int, L: int = 4, t_lo: float = 5.0, t_hi: float = 400.0):
     """dL/d(parameters) (flat, same layout) from dL/dT [nr][nz]: reverse of M4..M3."""
     layers = split(params, L)

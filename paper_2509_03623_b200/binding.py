@@ -21,6 +21,7 @@ OPT_WINDOW, OPT_SKIP_EMPTY, OPT_WIN_PATH = 1, 2, 3
 EXPORTS = ["radt_version", "radt_last_error", "radt_set_option", "radt_get_option", "radt_workspace_bytes",
            "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_l2_loss_grad", "radt_render_host",
            "radt_render_loss", "radt_disk_workspace_bytes", "radt_disk_fields", "radt_disk_fields_bwd",
+           "radt_mlp_num_params", "radt_mlp_temperature", "radt_mlp_temperature_bwd",
            "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
            "radt_last_launch_count"]
 
@@ -59,6 +60,15 @@ class radt_disk(C.Structure):
                 ("t_freeze", C.c_double), ("n_dissoc", C.c_double), ("f_col", C.c_double)]
 
 
+class radt_mlp(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("L", C.c_int32), ("width", C.c_int32), ("nhidden", C.c_int32),
+                ("t_lo", C.c_double), ("t_hi", C.c_double)]
+
+
+def make_mlp(L=4, t_lo=5.0, t_hi=400.0, width=64, nhidden=4):
+    return radt_mlp(C.sizeof(radt_mlp), L, width, nhidden, t_lo, t_hi)
+
+
 def make_disks(params):
     """ctypes array of radt_disk from objects with the fields of radt_disk (gm_star, m_gas | m_mol, sigma0, ...)."""
     params = _as_list(params)
@@ -90,6 +100,9 @@ def lib():
         L.radt_l2_loss_grad.argtypes = [vp, vp, dbl, i64, vp, vp, vp]
         L.radt_render_loss.argtypes = [gp, lp, rp, i32, vp, dbl, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_render_host.argtypes = [gp, lp, rp, i32, vp]
+        L.radt_mlp_num_params.argtypes = [C.POINTER(radt_mlp), C.POINTER(C.c_int64)]
+        L.radt_mlp_temperature.argtypes = [C.POINTER(radt_mlp), rp, vp, vp, vp]
+        L.radt_mlp_temperature_bwd.argtypes = [C.POINTER(radt_mlp), rp, vp, vp, vp, vp]
         L.radt_disk_workspace_bytes.argtypes = [rp, i32, C.POINTER(C.c_size_t)]
         L.radt_disk_fields.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_disk_fields_bwd.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, vp, C.c_size_t, vp]
@@ -240,6 +253,24 @@ def radt_disk_fields_bwd(disks, desc: Descriptors, temp, g_dens, g_vel, g_temp, 
                                       C.c_void_p(g_dens.data_ptr()), C.c_void_p(g_vel.data_ptr()),
                                       C.c_void_p(g_temp.data_ptr()), C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()),
                                       _stream_ptr(stream)))
+
+
+def radt_mlp_num_params(mlp) -> int:
+    out = C.c_int64(0)
+    _check(lib().radt_mlp_num_params(C.byref(mlp), C.byref(out)))
+    return out.value
+
+
+def radt_mlp_temperature(mlp, desc: Descriptors, params, temp_out, stream=None):
+    """MLP temperature field on the grid nodes: params CUDA float32 [num_params] -> temp_out CUDA float32 [nr, nzeta]."""
+    _check(lib().radt_mlp_temperature(C.byref(mlp), C.byref(desc.grid), C.c_void_p(params.data_ptr()),
+                                      C.c_void_p(temp_out.data_ptr()), _stream_ptr(stream)))
+
+
+def radt_mlp_temperature_bwd(mlp, desc: Descriptors, params, g_temp, g_params, stream=None):
+    _check(lib().radt_mlp_temperature_bwd(C.byref(mlp), C.byref(desc.grid), C.c_void_p(params.data_ptr()),
+                                          C.c_void_p(g_temp.data_ptr()), C.c_void_p(g_params.data_ptr()),
+                                          _stream_ptr(stream)))
 
 
 def radt_read_counters(ws, stream=None):

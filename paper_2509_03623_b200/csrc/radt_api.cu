@@ -660,6 +660,74 @@ int radt_disk_fields_bwd(const radt_disk *disk, const radt_grid *grid, int32_t b
     return RADT_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// MLP temperature field (radt_mlp.cu)
+// ------------------------------------------------------------------------------------------
+static int mlp_check(const radt_mlp *mlp, const radt_grid *grid, long long *count)
+{
+    if (!mlp) return fail(RADT_E_INVALID, "null mlp descriptor");
+    if (mlp->struct_size != sizeof(radt_mlp)) return fail(RADT_E_INVALID, "radt_mlp.struct_size mismatch");
+    if (mlp->width != 64 || mlp->nhidden != 4) return fail(RADT_E_UNSUPPORTED, "this build supports width 64 and 4 hidden layers");
+    if (mlp->L < 0 || mlp->L > 8) return fail(RADT_E_UNSUPPORTED, "encoding degree L must be 0..8");
+    if (!(mlp->t_hi > mlp->t_lo)) return fail(RADT_E_INVALID, "need t_lo < t_hi");
+    if (grid) {
+        if (grid->struct_size != sizeof(radt_grid)) return fail(RADT_E_INVALID, "radt_grid.struct_size mismatch");
+        if (grid->kind != RADT_GRID_AXISYM) return fail(RADT_E_UNSUPPORTED, "the MLP field lives on an axisymmetric grid");
+        if (grid->n[0] < 2 || grid->n[1] < 2) return fail(RADT_E_INVALID, "grid needs >= 2 nodes per axis");
+    }
+    const long long D = 2 + 4 * mlp->L;
+    if (count) *count = 64 * D + 64 + 3 * (64 * 64 + 64) + 64 + 1;
+    return RADT_OK;
+}
+
+int radt_mlp_num_params(const radt_mlp *mlp, int64_t *count_out)
+{
+    if (!count_out) return fail(RADT_E_INVALID, "null count_out");
+    long long c = 0;
+    int rc = mlp_check(mlp, nullptr, &c);
+    if (rc) return rc;
+    *count_out = c;
+    return RADT_OK;
+}
+
+static void mlp_fill(const radt_mlp *mlp, const radt_grid *grid, MlpParamsDev &Q)
+{
+    memset(&Q, 0, sizeof(Q));
+    Q.nr = grid->n[0]; Q.nz = grid->n[1]; Q.L = mlp->L;
+    Q.t_lo = (float)mlp->t_lo; Q.t_hi = (float)mlp->t_hi;
+}
+
+int radt_mlp_temperature(const radt_mlp *mlp, const radt_grid *grid, const float *params, float *temp_out,
+                         void *cuda_stream)
+{
+    if (!grid) return fail(RADT_E_INVALID, "null grid descriptor");
+    int rc = mlp_check(mlp, grid, nullptr);
+    if (rc) return rc;
+    if (!params || !temp_out) return fail(RADT_E_INVALID, "null pointer");
+    MlpParamsDev Q;
+    mlp_fill(mlp, grid, Q);
+    Q.params = params; Q.temp_out = temp_out;
+    CUDA_TRY(radt_launch_mlp_fwd(Q, (cudaStream_t)cuda_stream));
+    g_launches = 1;
+    return RADT_OK;
+}
+
+int radt_mlp_temperature_bwd(const radt_mlp *mlp, const radt_grid *grid, const float *params, const float *g_temp,
+                             float *g_params, void *cuda_stream)
+{
+    if (!grid) return fail(RADT_E_INVALID, "null grid descriptor");
+    long long count = 0;
+    int rc = mlp_check(mlp, grid, &count);
+    if (rc) return rc;
+    if (!params || !g_temp || !g_params) return fail(RADT_E_INVALID, "null pointer");
+    MlpParamsDev Q;
+    mlp_fill(mlp, grid, Q);
+    Q.params = params; Q.g_temp = g_temp; Q.g_params = g_params;
+    CUDA_TRY(radt_launch_mlp_bwd(Q, (int)count, (cudaStream_t)cuda_stream));
+    g_launches = 1;
+    return RADT_OK;
+}
+
 int radt_pipe_peak(int32_t kind, double *ops_per_s_out, double *sm_clock_mhz_out)
 {
     if (!ops_per_s_out) return fail(RADT_E_INVALID, "null output");

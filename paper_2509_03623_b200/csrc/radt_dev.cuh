@@ -150,6 +150,16 @@ struct DiskParamsDev {
     unsigned char *mask;                 // workspace, [batch][nr][nz]
 };
 
+// ---- MLP temperature field (radt_mlp.cu) ----
+struct MlpParamsDev {
+    int nr, nz, L;
+    float t_lo, t_hi;
+    const float *params;                 // flat parameter vector (layout: include/radt.h radt_mlp)
+    float *temp_out;                     // forward: [nr][nz]
+    const float *g_temp;                 // adjoint input
+    float *g_params;                     // adjoint output
+};
+
 // ---- single-instruction SFU helpers (MUFU.*) ----
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }

@@ -1,0 +1,99 @@
+"""GPU parity of the MLP temperature field (radt_mlp_temperature / _bwd) against oracle/mlp_field.py."""
+import numpy as np
+import pytest
+
+from oracle import mlp_field as mf
+from synth import make_config
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+def _desc(cfg):
+    from paper_2509_03623_b200 import binding as B
+    B.lib()
+    return B, B.Descriptors([make_config(cfg, npix=8)])
+
+
+@pytest.mark.parametrize("cfg,L,seed", [(1, 4, 1), (2, 4, 2), (1, 2, 3), (1, 8, 4), (1, 0, 5)])
+def test_mlp_temperature_matches_oracle(cfg, L, seed):
+    B, desc = _desc(cfg)
+    nr, nz = desc.grid_shape
+    mlp = B.make_mlp(L=L)
+    assert B.radt_mlp_num_params(mlp) == mf.n_params(L)
+    p = 3.0 * mf.init_params(L, seed)                       # scaled up so that the output leaves the sigmoid's middle
+    T = torch.empty((nr, nz), dtype=torch.float32, device="cuda")
+    B.radt_mlp_temperature(mlp, desc, torch.from_numpy(p).cuda(), T)
+    want = mf.forward(p, nr, nz, L)
+    # fp32 accumulation over 64-term dot products, four layers deep: 1e-5 of the 395 K range
+    assert np.max(np.abs(T.cpu().numpy() - want)) <= 1e-5 * 395.0
+    assert want.max() - want.min() > 0.1
+
+
+@pytest.mark.parametrize("cfg,L,seed", [(1, 4, 11), (2, 4, 12), (1, 1, 13)])
+def test_mlp_adjoint_matches_oracle(cfg, L, seed):
+    B, desc = _desc(cfg)
+    nr, nz = desc.grid_shape
+    mlp = B.make_mlp(L=L)
+    p = 3.0 * mf.init_params(L, seed)
+    gT = np.random.default_rng(seed).standard_normal((nr, nz)).astype(np.float32)
+    kink = mf.near_kink(p, nr, nz, L)          # ReLU subgradients: both branches are correct there
+    assert kink.mean() < 0.2
+    gT[kink] = 0.0
+    gp = torch.full((mf.n_params(L),), 7.0, dtype=torch.float32, device="cuda")      # must be overwritten
+    B.radt_mlp_temperature_bwd(mlp, desc, torch.from_numpy(p).cuda(), torch.from_numpy(gT).cuda(), gp)
+    want = mf.adjoint(p, gT, nr, nz, L)
+    got = gp.cpu().numpy().astype(np.float64)
+    # BASELINE.json gradient tolerance (1e-3 of the maximum); measured far below
+    assert np.max(np.abs(got - want)) <= 1e-3 * np.abs(want).max()
+    assert np.linalg.norm(got - want) <= 1e-4 * np.linalg.norm(want)
+
+
+def test_neural_field_fit_reduces_the_loss():
+    """The paper's chain end to end on the GPU (Fig. 2): parameters -> MLP T grid -> physics pre-pass -> render ->
+    chi^2 -> adjoints back to the parameters; a few plain gradient steps towards a target cube rendered from a known
+    temperature grid lower the loss, and the chain's gradient matches a finite difference of the GPU loss."""
+    from types import SimpleNamespace
+    from paper_2509_03623_b200 import Renderer, binding as B
+    sc = make_config(1, npix=32)
+    R = Renderer([sc])
+    desc = R.desc
+    nr, nz = desc.grid_shape
+    disks = B.make_disks([SimpleNamespace(gm_star=2.0 * 1.32712440018e26, m_gas=2.37 * 1.66053906660e-24, sigma0=30.0,
+                                          r_c=150.0, gamma=1.0, x_co=1e-4, t_freeze=19.0, n_dissoc=1e21, f_col=0.706)])
+    pws = torch.empty(B.radt_disk_workspace_bytes(desc), dtype=torch.uint8, device="cuda")
+    mlp = B.make_mlp(L=4)
+
+    def chain(params, need_grad):
+        B.radt_mlp_temperature(mlp, desc, params, R.temp[0])
+        B.radt_disk_fields(disks, desc, R.temp, R.dens, R.vel, pws)
+        if not need_grad:
+            R.render_loss()
+            return float(R.loss.cpu()), None
+        R.fit_step()
+        gT = R.g_temp.clone()
+        B.radt_disk_fields_bwd(disks, desc, R.temp, R.g_dens, R.g_vel, gT, pws)
+        gp = torch.empty_like(params)
+        B.radt_mlp_temperature_bwd(mlp, desc, params, gT[0], gp)
+        return float(R.loss.cpu()), gp
+
+    # target: the cube of the config's own (noisy, parametric) temperature grid pushed through the same pre-pass
+    B.radt_disk_fields(disks, desc, R.temp, R.dens, R.vel, pws)
+    R.render()
+    target = R.cube.clone()
+    R.set_target(target, 0.015 * float(target.max()))
+    params = torch.from_numpy(mf.init_params(4, 21)).cuda()
+    loss0, g = chain(params, True)
+    # directional finite difference of the GPU chain along the gradient
+    d = g / g.norm()
+    eps = 2e-3
+    lp, _ = chain(params + eps * d, False)
+    lm, _ = chain(params - eps * d, False)
+    assert float((g * d).sum()) == pytest.approx((lp - lm) / (2 * eps), rel=5e-2)
+    # normalised gradient descent with a decaying step
+    loss = loss0
+    for it in range(40):
+        loss, g = chain(params, True)
+        params = params - 0.05 * (0.95 ** it) * g / g.norm()
+    loss_end, _ = chain(params, False)
+    assert loss_end < 0.7 * loss0
