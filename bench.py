@@ -277,7 +277,14 @@ def run_ours(args):
         t_pf = time_kernel_group(lambda: B.radt_disk_fields(disks, R.desc, R.temp, pd, pv, pws, stream), stream, torch, flush, reps)
         t_pb = time_kernel_group(lambda: B.radt_disk_fields_bwd(disks, R.desc, R.temp, R.g_dens, R.g_vel, pg, pws, stream),
                                  stream, torch, flush, reps)
-        prepass = {"fwd_ms": t_pf, "bwd_ms": t_pb, "what": "radt_disk_fields(_bwd): T grid -> n_CO, v_phi; outside the timed step"}
+        mlp = B.make_mlp(L=4)
+        mp = torch.zeros(B.radt_mlp_num_params(mlp), dtype=torch.float32, device=R.device).uniform_(-0.1, 0.1)
+        mg, mt = torch.empty_like(mp), torch.empty_like(R.temp[0])
+        t_mf = time_kernel_group(lambda: B.radt_mlp_temperature(mlp, R.desc, mp, mt, stream), stream, torch, flush, reps)
+        t_mb = time_kernel_group(lambda: B.radt_mlp_temperature_bwd(mlp, R.desc, mp, pg[0], mg, stream), stream, torch, flush, reps)
+        prepass = {"fwd_ms": t_pf, "bwd_ms": t_pb, "mlp_fwd_ms": t_mf, "mlp_bwd_ms": t_mb,
+                   "what": "radt_disk_fields(_bwd): T grid -> n_CO, v_phi; radt_mlp_temperature(_bwd): parameters -> T grid "
+                           "(one grid); both outside the timed step, each figure includes the host-side enqueue"}
 
     # ---- roofline: SFU (MUFU.EX2) issue peak measured now, at the clock the GPU runs at
     mufu_peak, mufu_clk = B.radt_pipe_peak(0)

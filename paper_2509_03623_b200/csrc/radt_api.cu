@@ -693,6 +693,7 @@ int radt_mlp_num_params(const radt_mlp *mlp, int64_t *count_out)
 static void mlp_fill(const radt_mlp *mlp, const radt_grid *grid, MlpParamsDev &Q)
 {
     memset(&Q, 0, sizeof(Q));
+    Q.nparams = 64 * (2 + 4 * mlp->L) + 64 + 3 * (64 * 64 + 64) + 64 + 1;
     Q.nr = grid->n[0]; Q.nz = grid->n[1]; Q.L = mlp->L;
     Q.t_lo = (float)mlp->t_lo; Q.t_hi = (float)mlp->t_hi;
 }
@@ -704,6 +705,7 @@ int radt_mlp_temperature(const radt_mlp *mlp, const radt_grid *grid, const float
     int rc = mlp_check(mlp, grid, nullptr);
     if (rc) return rc;
     if (!params || !temp_out) return fail(RADT_E_INVALID, "null pointer");
+    if (((uintptr_t)params & 15) != 0) return fail(RADT_E_INVALID, "params must be 16-byte aligned");
     MlpParamsDev Q;
     mlp_fill(mlp, grid, Q);
     Q.params = params; Q.temp_out = temp_out;

@@ -152,7 +152,7 @@ struct DiskParamsDev {
 
 // ---- MLP temperature field (radt_mlp.cu) ----
 struct MlpParamsDev {
-    int nr, nz, L;
+    int nr, nz, L, nparams;
     float t_lo, t_hi;
     const float *params;                 // flat parameter vector (layout: include/radt.h radt_mlp)
     float *temp_out;                     // forward: [nr][nz]

@@ -10,6 +10,8 @@
 #define MLP_H 4                        // hidden layers
 #define MLP_TF 128                     // nodes per block, forward
 #define MLP_TB 64                      // nodes per block, adjoint
+#define MLP_S 4                        // threads per node: each computes MLP_W / MLP_S units of a layer
+#define MLP_PW (MLP_W / MLP_S)
 #define MLP_SA (MLP_TB + 1)            // activation row stride (adjoint): scalar reads by unit are conflict free
 #define MLP_SD (MLP_TB + 4)            // delta row stride: 16-byte aligned rows for broadcast float4 reads
 
@@ -48,35 +50,35 @@ __device__ __forceinline__ void mlp_encode(const MlpParamsDev &Q, int i, int j, 
 
 // M3, first layer: fan-in D (rows are not 16-byte aligned: scalar uniform loads)
 __device__ __forceinline__ void mlp_layer_first(const float *__restrict__ W, const float *__restrict__ b, int D,
-                                                const float *in, float *out, int stride, int node)
+                                                const float *in, float *out, int stride, int node, int part)
 {
     float h[34];
 #pragma unroll
     for (int i = 0; i < 34; ++i) h[i] = i < D ? in[i * stride + node] : 0.f;
-#pragma unroll 2
-    for (int o = 0; o < MLP_W; ++o) {
-        float acc = __ldg(b + o);
+#pragma unroll 4
+    for (int o = part * MLP_PW; o < (part + 1) * MLP_PW; ++o) {
+        float acc = b[o];
 #pragma unroll
         for (int i = 0; i < 34; ++i)
-            if (i < D) acc = fmaf(__ldg(W + o * D + i), h[i], acc);
+            if (i < D) acc = fmaf(W[o * D + i], h[i], acc);
         out[o * stride + node] = fmaxf(acc, 0.f);
     }
 }
 
 // M3, hidden layer 64 -> 64: the node's inputs in registers, one output unit at a time, weight rows as float4
 __device__ __forceinline__ void mlp_layer(const float *__restrict__ W, const float *__restrict__ b, const float *in,
-                                          float *out, int stride, int node)
+                                          float *out, int stride, int node, int part)
 {
     float h[MLP_W];
 #pragma unroll
     for (int i = 0; i < MLP_W; ++i) h[i] = in[i * stride + node];
-#pragma unroll 2
-    for (int o = 0; o < MLP_W; ++o) {
+#pragma unroll 4
+    for (int o = part * MLP_PW; o < (part + 1) * MLP_PW; ++o) {
         const float4 *row = reinterpret_cast<const float4 *>(W + o * MLP_W);
-        float a0 = __ldg(b + o), a1 = 0.f;
+        float a0 = b[o], a1 = 0.f;
 #pragma unroll
         for (int q = 0; q < MLP_W / 4; ++q) {
-            const float4 w = __ldg(row + q);
+            const float4 w = row[q];
             a0 = fmaf(w.x, h[4 * q], a0); a1 = fmaf(w.y, h[4 * q + 1], a1);
             a0 = fmaf(w.z, h[4 * q + 2], a0); a1 = fmaf(w.w, h[4 * q + 3], a1);
         }
@@ -89,38 +91,56 @@ __device__ __forceinline__ float mlp_head(const float *__restrict__ w5, float b5
 {
     float o = b5;
 #pragma unroll 8
-    for (int i = 0; i < MLP_W; ++i) o = fmaf(__ldg(w5 + i), in[i * stride + node], o);
+    for (int i = 0; i < MLP_W; ++i) o = fmaf(w5[i], in[i * stride + node], o);
     return 1.0f / (1.0f + __expf(-o));
 }
 
 extern __shared__ __align__(16) float mlp_smem[];
 
-__global__ void __launch_bounds__(MLP_TF) k_mlp_fwd(const __grid_constant__ MlpParamsDev Q)
+// cooperative copy of `count` floats into shared memory (src and dst 16-byte aligned)
+__device__ __forceinline__ void mlp_stage(float *dst, const float *__restrict__ src, int count, int nthreads)
 {
-    const int node = threadIdx.x, q = blockIdx.x * MLP_TF + node, n = Q.nr * Q.nz;
+    const float4 *s4 = reinterpret_cast<const float4 *>(src);
+    float4 *d4 = reinterpret_cast<float4 *>(dst);
+    for (int q = threadIdx.x; q < count / 4; q += nthreads) d4[q] = __ldg(s4 + q);
+    for (int q = (count & ~3) + threadIdx.x; q < count; q += nthreads) dst[q] = __ldg(src + q);
+}
+
+__global__ void __launch_bounds__(MLP_TF * MLP_S) k_mlp_fwd(const __grid_constant__ MlpParamsDev Q)
+{
+    const int node = threadIdx.x & (MLP_TF - 1), part = threadIdx.x / MLP_TF;     // part is warp uniform
+    const int q = blockIdx.x * MLP_TF + node, n = Q.nr * Q.nz;
     const int qq = min(q, n - 1), i = qq / Q.nz, j = qq - i * Q.nz;
     const MlpOff F = mlp_offsets(Q.L);
     float *A = mlp_smem, *B = mlp_smem + MLP_W * MLP_TF;           // ping-pong [unit][node]
-    mlp_encode(Q, i, j, A, MLP_TF, node);
-    mlp_layer_first(Q.params + F.W[0], Q.params + F.b[0], F.D, A, B, MLP_TF, node);
-    mlp_layer(Q.params + F.W[1], Q.params + F.b[1], B, A, MLP_TF, node);
-    mlp_layer(Q.params + F.W[2], Q.params + F.b[2], A, B, MLP_TF, node);
-    mlp_layer(Q.params + F.W[3], Q.params + F.b[3], B, A, MLP_TF, node);
-    const float s = mlp_head(Q.params + F.W[4], __ldg(Q.params + F.b[4]), A, MLP_TF, node);
+    float *sP = B + MLP_W * MLP_TF;                                // all parameters (a uniform global load per weight
+    mlp_stage(sP, Q.params, F.b[MLP_H] + 1, MLP_TF * MLP_S);       // left the kernel waiting on L1/L2: 17 stall cycles per issue)
+    if (part == 0) mlp_encode(Q, i, j, A, MLP_TF, node);
+    __syncthreads();
+    mlp_layer_first(sP + F.W[0], sP + F.b[0], F.D, A, B, MLP_TF, node, part);
+    __syncthreads();
+    mlp_layer(sP + F.W[1], sP + F.b[1], B, A, MLP_TF, node, part);
+    __syncthreads();
+    mlp_layer(sP + F.W[2], sP + F.b[2], A, B, MLP_TF, node, part);
+    __syncthreads();
+    mlp_layer(sP + F.W[3], sP + F.b[3], B, A, MLP_TF, node, part);
+    __syncthreads();
+    if (part != 0) return;
+    const float s = mlp_head(sP + F.W[4], sP[F.b[4]], A, MLP_TF, node);
     if (q < n) Q.temp_out[q] = fmaf(Q.t_hi - Q.t_lo, s, Q.t_lo);
 }
 
 // dW[o][i] = sum_n delta[o][n] a[i][n] for this block's nodes; thread t owns input unit i = t (its activations over
 // the nodes sit in registers), output units one at a time with broadcast float4 reads of the delta rows.
 __device__ __forceinline__ void mlp_grad_weights(const float *act, const float *delta, int fan_in, float *gW, float *gb,
-                                                 int nout, int t)
+                                                 int nout, int t, int part)
 {
     if (t < fan_in) {
         float a[MLP_TB];
 #pragma unroll
         for (int n = 0; n < MLP_TB; ++n) a[n] = act[t * MLP_SA + n];
 #pragma unroll 2
-        for (int o = 0; o < nout; ++o) {
+        for (int o = part * MLP_PW; o < (part + 1) * MLP_PW; ++o) {
             const float4 *row = reinterpret_cast<const float4 *>(delta + o * MLP_SD);
             float s0 = 0.f, s1 = 0.f;
 #pragma unroll
@@ -132,7 +152,7 @@ __device__ __forceinline__ void mlp_grad_weights(const float *act, const float *
             atomicAdd(gW + o * fan_in + t, s0 + s1);
         }
     }
-    if (t < nout) {
+    if (part == 0 && t < nout) {
         const float4 *row = reinterpret_cast<const float4 *>(delta + t * MLP_SD);
         float s = 0.f;
 #pragma unroll
@@ -144,85 +164,110 @@ __device__ __forceinline__ void mlp_grad_weights(const float *act, const float *
     }
 }
 
-// delta_in[i][node] = relu'(a_in[i][node]) sum_o W[o][i] delta_out[o][node]
-__device__ __forceinline__ void mlp_back_layer(const float *__restrict__ W, const float *dout, const float *ain, float *din,
-                                               int node)
+// delta_in[i][node] = relu'(a_in[i][node]) sum_o W[o][i] delta_out[o][node] for the input units i of this thread's
+// part; in place (din = dout): every part reads the whole column first, the block synchronises, then writes.
+__device__ __forceinline__ void mlp_back_layer(const float *__restrict__ W, float *dl, const float *ain, int node, int part)
 {
-    float acc[MLP_W];
+    float acc[MLP_PW];
 #pragma unroll
-    for (int i = 0; i < MLP_W; ++i) acc[i] = 0.f;
-#pragma unroll 2
+    for (int i = 0; i < MLP_PW; ++i) acc[i] = 0.f;
+#pragma unroll 4
     for (int o = 0; o < MLP_W; ++o) {
-        const float d = dout[o * MLP_SD + node];
-        const float4 *row = reinterpret_cast<const float4 *>(W + o * MLP_W);
+        const float d = dl[o * MLP_SD + node];
+        const float4 *row = reinterpret_cast<const float4 *>(W + o * MLP_W + part * MLP_PW);
 #pragma unroll
-        for (int q = 0; q < MLP_W / 4; ++q) {
-            const float4 w = __ldg(row + q);
+        for (int q = 0; q < MLP_PW / 4; ++q) {
+            const float4 w = row[q];
             acc[4 * q] = fmaf(w.x, d, acc[4 * q]); acc[4 * q + 1] = fmaf(w.y, d, acc[4 * q + 1]);
             acc[4 * q + 2] = fmaf(w.z, d, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(w.w, d, acc[4 * q + 3]);
         }
     }
+    __syncthreads();
 #pragma unroll
-    for (int i = 0; i < MLP_W; ++i) din[i * MLP_SD + node] = ain[i * MLP_SA + node] > 0.f ? acc[i] : 0.f;
+    for (int i = 0; i < MLP_PW; ++i) {
+        const int u = part * MLP_PW + i;
+        dl[u * MLP_SD + node] = ain[u * MLP_SA + node] > 0.f ? acc[i] : 0.f;
+    }
 }
 
 // Adjoint: recomputes the activations of its 64 nodes (nothing is stored between the passes), then walks the layers
-// backwards; parameter gradients leave the block as float atomics.
-__global__ void __launch_bounds__(MLP_TB) k_mlp_bwd(const __grid_constant__ MlpParamsDev Q)
+// backwards; parameter gradients leave the block as float atomics.  Shared memory: all activations, ONE delta buffer
+// (a node's column is private to its thread, so the back-propagation runs in place) and the weights of the layer
+// at hand.
+#define MLP_WBUF (MLP_W * MLP_W + MLP_W)
+__global__ void __launch_bounds__(MLP_TB * MLP_S, 2) k_mlp_bwd(const __grid_constant__ MlpParamsDev Q)
 {
-    const int node = threadIdx.x, q = blockIdx.x * MLP_TB + node, n = Q.nr * Q.nz;
+    const int node = threadIdx.x & (MLP_TB - 1), part = threadIdx.x / MLP_TB;   // part is warp uniform
+    const int q = blockIdx.x * MLP_TB + node, n = Q.nr * Q.nz;
     const int qq = min(q, n - 1), i = qq / Q.nz, j = qq - i * Q.nz;
     const MlpOff F = mlp_offsets(Q.L);
-    float *a0 = mlp_smem;                                  // [34][SA]
-    float *a[MLP_H + 1];
-    a[0] = a0;
-    for (int l = 1; l <= MLP_H; ++l) a[l] = a0 + 34 * MLP_SA + (l - 1) * MLP_W * MLP_SA;
-    float *dA = a0 + 34 * MLP_SA + MLP_H * MLP_W * MLP_SA;
-    dA += (4 - ((dA - mlp_smem) & 3)) & 3;                 // 16-byte aligned rows
-    float *dB = dA + MLP_W * MLP_SD, *go = dB + MLP_W * MLP_SD;
-    mlp_encode(Q, i, j, a[0], MLP_SA, node);
-    mlp_layer_first(Q.params + F.W[0], Q.params + F.b[0], F.D, a[0], a[1], MLP_SA, node);
-    for (int l = 1; l < MLP_H; ++l) mlp_layer(Q.params + F.W[l], Q.params + F.b[l], a[l], a[l + 1], MLP_SA, node);
-    const float s = mlp_head(Q.params + F.W[MLP_H], __ldg(Q.params + F.b[MLP_H]), a[MLP_H], MLP_SA, node);
+    float *sW = mlp_smem;                                  // [MLP_WBUF] W_l | b_l of the layer at hand
+    float *a0 = sW + MLP_WBUF;                             // [34][SA]
+    float *a1 = a0 + 34 * MLP_SA;                          // a_l = a1 + (l - 1) 64 SA, l = 1..4
+    float *dl = a1 + MLP_H * MLP_W * MLP_SA;
+    dl += (4 - ((dl - mlp_smem) & 3)) & 3;                 // 16-byte aligned rows
+    float *go = dl + MLP_W * MLP_SD;
+    auto act = [&](int l) { return l == 0 ? a0 : a1 + (l - 1) * MLP_W * MLP_SA; };
+    // layer l: W at F.W[l] (64 x fan) followed by b at F.b[l] = F.W[l] + 64 fan: one contiguous block
+    auto stage = [&](int l) {
+        __syncthreads();
+        const int fan = l == 0 ? F.D : MLP_W, cnt = l < MLP_H ? MLP_W * fan + MLP_W : MLP_W + 1;
+        const int lead = F.W[l] & 3;                       // keep the 16-byte phase of the source
+        for (int t = threadIdx.x; t < cnt; t += MLP_TB * MLP_S) sW[lead + t] = __ldg(Q.params + F.W[l] + t);
+        __syncthreads();
+        return sW + lead;
+    };
+    if (part == 0) mlp_encode(Q, i, j, a0, MLP_SA, node);
+    {
+        const float *w = stage(0);
+        mlp_layer_first(w, w + MLP_W * F.D, F.D, a0, a1, MLP_SA, node, part);
+    }
+    for (int l = 1; l < MLP_H; ++l) {
+        const float *w = stage(l);                         // (its barriers also order the layers)
+        mlp_layer(w, w + MLP_W * MLP_W, act(l), act(l + 1), MLP_SA, node, part);
+    }
+    const float *w5 = stage(MLP_H);
+    const float *a4 = act(MLP_H);
+    const float s = mlp_head(w5, w5[MLP_W], a4, MLP_SA, node);
     // M4 and the output unit
     const float g_o = q < n ? __ldg(Q.g_temp + q) * (Q.t_hi - Q.t_lo) * s * (1.0f - s) : 0.f;
-    go[node] = g_o;
-    for (int o = 0; o < MLP_W; ++o)
-        dA[o * MLP_SD + node] = a[MLP_H][o * MLP_SA + node] > 0.f ? g_o * __ldg(Q.params + F.W[MLP_H] + o) : 0.f;
+    if (part == 0) go[node] = g_o;
+    for (int o = part * MLP_PW; o < (part + 1) * MLP_PW; ++o)
+        dl[o * MLP_SD + node] = a4[o * MLP_SA + node] > 0.f ? g_o * w5[o] : 0.f;
     __syncthreads();
-    {
+    if (part == 0) {
         float s5 = 0.f, sb = 0.f;
         for (int m = 0; m < MLP_TB; ++m) {
             const float g = go[m];
-            s5 = fmaf(g, a[MLP_H][node * MLP_SA + m], s5);
+            s5 = fmaf(g, a4[node * MLP_SA + m], s5);
             sb += g;
         }
         atomicAdd(Q.g_params + F.W[MLP_H] + node, s5);     // node doubles as the unit index here (MLP_TB == MLP_W)
         if (node == 0) atomicAdd(Q.g_params + F.b[MLP_H], sb);
     }
-    float *dcur = dA, *dnext = dB;
     for (int l = MLP_H - 1; l >= 0; --l) {
-        mlp_grad_weights(a[l], dcur, l == 0 ? F.D : MLP_W, Q.g_params + F.W[l], Q.g_params + F.b[l], MLP_W, node);
+        mlp_grad_weights(act(l), dl, l == 0 ? F.D : MLP_W, Q.g_params + F.W[l], Q.g_params + F.b[l], MLP_W, node, part);
         if (l > 0) {
-            mlp_back_layer(Q.params + F.W[l], dcur, a[l], dnext, node);
-            float *t = dcur; dcur = dnext; dnext = t;
+            const float *w = stage(l);                     // (its barriers also fence the reads of dl above)
+            mlp_back_layer(w, dl, act(l), node, part);
+            __syncthreads();
         }
-        __syncthreads();
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
-static size_t mlp_bwd_smem() { return (size_t)(34 * MLP_SA + MLP_H * MLP_W * MLP_SA + 4 + 2 * MLP_W * MLP_SD + MLP_TB) * sizeof(float); }
+static size_t mlp_bwd_smem() { return (size_t)(MLP_WBUF + 4 + 34 * MLP_SA + MLP_H * MLP_W * MLP_SA + 4 + MLP_W * MLP_SD + MLP_TB) * sizeof(float); }
 
 cudaError_t radt_launch_mlp_fwd(const MlpParamsDev &Q, cudaStream_t st)
 {
-    const size_t smem = (size_t)2 * MLP_W * MLP_TF * sizeof(float);
+    // two activation buffers + the whole parameter vector (padded to the allocation granularity of the caller)
+    const size_t smem = (size_t)(2 * MLP_W * MLP_TF + ((Q.nparams + 3) & ~3)) * sizeof(float);
     cudaError_t e = cudaFuncSetAttribute(k_mlp_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int n = Q.nr * Q.nz;
-    k_mlp_fwd<<<(n + MLP_TF - 1) / MLP_TF, MLP_TF, smem, st>>>(Q);
+    k_mlp_fwd<<<(n + MLP_TF - 1) / MLP_TF, MLP_TF * MLP_S, smem, st>>>(Q);
     return cudaGetLastError();
 }
 
@@ -234,6 +279,6 @@ cudaError_t radt_launch_mlp_bwd(const MlpParamsDev &Q, int nparams, cudaStream_t
     e = cudaFuncSetAttribute(k_mlp_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int n = Q.nr * Q.nz;
-    k_mlp_bwd<<<(n + MLP_TB - 1) / MLP_TB, MLP_TB, smem, st>>>(Q);
+    k_mlp_bwd<<<(n + MLP_TB - 1) / MLP_TB, MLP_TB * MLP_S, smem, st>>>(Q);
     return cudaGetLastError();
 }
