@@ -117,6 +117,15 @@ static int orc_clip(const orc_geom *g, const orc_grid *gr, const orc_orient *o, 
         *s0 = -sh; *s1 = sh;
         return 1;
     }
+    if (gr->kind == ORC_SPH3D) {
+        /* spherical (r, theta, phi) grid: bounding sphere of radius r_max */
+        double Rb = gr->hi[0];
+        double b = hypot(X, Y);
+        if (!(b < Rb)) return 0;
+        double sh = sqrt(Rb * Rb - b * b);
+        *s0 = -sh; *s1 = sh;
+        return 1;
+    }
     double tmin = -INFINITY, tmax = INFINITY;
     for (int a = 0; a < 3; ++a) {
         double d = o->dir[a];
@@ -165,6 +174,41 @@ static void orc_locate(const orc_grid *gr, double x, double y, double z, orc_sam
             int di = c >> 1, dj = c & 1;
             sp->idx[c] = (int64_t)(i + di) * nz + (j + dj);
             sp->w[c] = (di ? fu : 1.0 - fu) * (dj ? fw : 1.0 - fw);
+        }
+        return;
+    }
+    if (gr->kind == ORC_SPH3D) {
+        /* nodes: r_i = r_min (r_max/r_min)^(i/(nr-1)); theta_j = lo[1] + (hi[1]-lo[1]) j/(nt-1), the polar angle from
+         * the +z axis of the disk frame; phi_k = 2 pi k/np, periodic (the cell after node np-1 ends at node 0).
+         * Tri-linear in index space (ln r, theta, phi); outside the (r, theta) range is vacuum. */
+        int nr = gr->n[0], nt = gr->n[1], np_ = gr->n[2];
+        double rmin = gr->lo[0], rmax = gr->hi[0], tlo = gr->lo[1], thi = gr->hi[1];
+        const double two_pi = 6.283185307179586476925286766559;
+        if (!(sp->rho > 0.0)) return;
+        double theta = acos(z / sp->rho);
+        if (!(sp->rho >= rmin && sp->rho <= rmax && theta >= tlo && theta <= thi)) return;
+        double phi = atan2(y, x);
+        if (phi < 0.0) phi += two_pi;
+        double u = log(sp->rho / rmin) / log(rmax / rmin) * (double)(nr - 1);
+        double w = (theta - tlo) / (thi - tlo) * (double)(nt - 1);
+        double q = phi / two_pi * (double)np_;
+        if (u < 0.0) u = 0.0;
+        if (u > (double)(nr - 1)) u = (double)(nr - 1);
+        if (w < 0.0) w = 0.0;
+        if (w > (double)(nt - 1)) w = (double)(nt - 1);
+        if (q < 0.0) q = 0.0;
+        if (q > (double)np_) q = (double)np_;
+        int i = (int)floor(u); if (i > nr - 2) i = nr - 2;
+        int j = (int)floor(w); if (j > nt - 2) j = nt - 2;
+        int k = (int)floor(q); if (k > np_ - 1) k = np_ - 1;
+        double fu = u - (double)i, fw = w - (double)j, fq = q - (double)k;
+        int k1 = (k + 1) % np_;
+        sp->inside = 1;
+        sp->ncorner = 8;
+        for (int c = 0; c < 8; ++c) {
+            int di = (c >> 2) & 1, dj = (c >> 1) & 1, dk = c & 1;
+            sp->idx[c] = ((int64_t)(i + di) * nt + (j + dj)) * np_ + (dk ? k1 : k);
+            sp->w[c] = (di ? fu : 1.0 - fu) * (dj ? fw : 1.0 - fw) * (dk ? fq : 1.0 - fq);
         }
         return;
     }

@@ -29,7 +29,7 @@
 extern "C" {
 #endif
 
-enum { ORC_AXISYM = 0, ORC_CART3D = 1 };
+enum { ORC_AXISYM = 0, ORC_CART3D = 1, ORC_SPH3D = 2 };
 enum { ORC_DENS_LINEAR = 0, ORC_DENS_LN = 1 };
 enum { ORC_VEL_VPHI = 0, ORC_VEL_KEPLER_FRAC = 1 };
 enum { ORC_UNIT_S0 = 0, ORC_UNIT_CGS = 1, ORC_UNIT_JY_PIXEL = 2 };

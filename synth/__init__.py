@@ -5,13 +5,14 @@ line table used by the configs, the analytic disk family of BASELINE.json `confi
 analytic scenes (slabs) for the closed-form pins.  It holds none of the render's arithmetic
 (no ray geometry, no profile, no transfer) and imports neither `oracle/` nor the CUDA package.
 """
-from .scene import Geom, Line, Grid, Scene, AXISYM, CART3D, DENS_LINEAR, DENS_LN, VEL_VPHI, VEL_KEPLER_FRAC
+from .scene import Geom, Line, Grid, Scene, AXISYM, CART3D, SPH3D, DENS_LINEAR, DENS_LN, VEL_VPHI, VEL_KEPLER_FRAC
 from .scene import UNIT_S0, UNIT_CGS, UNIT_JY_PIXEL
 from .lines import co_line
 from .disks import make_config, config_names, slab_scene, tiny_axisym_scene, tiny_cart_scene, l2_target
+from .disks import tiny_sph_scene, sph_benchmark_scene
 
 __all__ = [
-    "Geom", "Line", "Grid", "Scene", "AXISYM", "CART3D", "DENS_LINEAR", "DENS_LN", "VEL_VPHI",
+    "Geom", "Line", "Grid", "Scene", "AXISYM", "CART3D", "SPH3D", "DENS_LINEAR", "DENS_LN", "VEL_VPHI",
     "VEL_KEPLER_FRAC", "UNIT_S0", "UNIT_CGS", "UNIT_JY_PIXEL", "co_line", "make_config",
-    "config_names", "slab_scene", "tiny_axisym_scene", "tiny_cart_scene", "l2_target",
+    "config_names", "slab_scene", "tiny_axisym_scene", "tiny_cart_scene", "l2_target", "tiny_sph_scene", "sph_benchmark_scene",
 ]

@@ -17,6 +17,7 @@ import numpy as np
 from scipy.special import erfc
 
 from .lines import co_line, channels_centered
+from .scene import SPH3D
 from .scene import (AXISYM, CART3D, DENS_LINEAR, DENS_LN, VEL_KEPLER_FRAC, VEL_VPHI, Geom, Grid, Scene,
                     UNIT_S0)
 
@@ -269,3 +270,60 @@ def tiny_cart_scene(seed=2, ng=(7, 6, 5), npix=5, nchan=5, nstep=10, incl_deg=35
                 pa=math.radians(pa_deg), az=math.radians(az_deg), nstep=nstep, vsys=vsys, gm_star=gm)
     line = co_line(np.linspace(-5.0, 5.0, nchan) * KMS, vturb_abs=0.4 * KMS)
     return Scene(geom, line, grid, "tiny_cart")
+
+
+def _sph_nodes(n, rmin, rmax, th_half):
+    r = rmin * (rmax / rmin) ** (np.arange(n[0]) / (n[0] - 1.0))
+    th = (0.5 * math.pi - th_half) + 2.0 * th_half * np.arange(n[1]) / (n[1] - 1.0)
+    ph = 2.0 * math.pi * np.arange(n[2]) / n[2]
+    return r, th, ph
+
+
+def tiny_sph_scene(seed=3, ng=(7, 6, 8), npix=6, nchan=5, nstep=14, incl_deg=50.0, pa_deg=40.0, az_deg=20.0,
+                   dens_ln=False, kepler_frac=False, vsys=-0.1e5) -> Scene:
+    """Small random spherical (r, theta, phi) scene; theta spans +-0.7 rad about the equator."""
+    rng = np.random.default_rng(np.random.PCG64(3000 + seed))
+    lo, hi = (30.0, 0.5 * math.pi - 0.7, 0.0), (220.0, 0.5 * math.pi + 0.7, 2.0 * math.pi)
+    r, th, ph = _sph_nodes(ng, lo[0], hi[0], 0.7)
+    rr, tt, pp = np.meshgrid(r, th, ph, indexing="ij")
+    rc, zz = rr * np.sin(tt), rr * np.cos(tt)
+    n = 40.0 * (rc / 100.0) ** -1.0 * np.exp(-0.5 * (zz / 35.0) ** 2) * np.exp(0.3 * rng.standard_normal(rr.shape))
+    t = (25.0 + 0.3 * np.abs(zz)) * np.exp(0.1 * rng.standard_normal(rr.shape))
+    gm = 2.0 * GM_SUN
+    if kepler_frac:
+        v = 0.1 * rng.standard_normal(rr.shape)
+    else:
+        v = np.sqrt(gm / (rc * AU_CM)) * (1.0 + 0.05 * rng.standard_normal(rr.shape))
+    dens = np.log(n) if dens_ln else n
+    grid = Grid(kind=SPH3D, n=tuple(ng), lo=lo, hi=hi,
+                dens=np.ascontiguousarray(dens, np.float32), temp=np.ascontiguousarray(t, np.float32),
+                vel=np.ascontiguousarray(v, np.float32), mirror_z=False,
+                dens_mode=DENS_LN if dens_ln else DENS_LINEAR,
+                vel_mode=VEL_KEPLER_FRAC if kepler_frac else VEL_VPHI)
+    geom = Geom(nx=npix, ny=npix, fov_x=460.0, fov_y=460.0, incl=math.radians(incl_deg),
+                pa=math.radians(pa_deg), az=math.radians(az_deg), nstep=nstep, vsys=vsys, gm_star=gm)
+    line = co_line(np.linspace(-5.0, 5.0, nchan) * KMS, vturb_abs=0.4 * KMS)
+    return Scene(geom, line, grid, "tiny_sph")
+
+
+def sph_benchmark_scene(ng=(512, 96, 256), npix=256, nchan=64, nstep=256, seed=36236) -> Scene:
+    """Stand-in for the workload of the paper's only timing benchmark (hydro-simulation fields on a
+    512 x 96 x 256 spherical grid rendered at 256 x 256 px; the simulation of ref. [3] is not available): the config-2
+    disk family evaluated on a spherical grid (r in [10, 600] au, theta within +-0.46 rad of the equator, all phi) with a
+    two-armed logarithmic spiral (15 % in density, 5 % in temperature, 2 % in rotation speed) and 5 % log-normal
+    noise, so that the fields depend on all three coordinates as hydro fields do."""
+    rng = np.random.default_rng(np.random.PCG64(seed))
+    th_half = 0.46
+    lo, hi = (10.0, 0.5 * math.pi - th_half, 0.0), (600.0, 0.5 * math.pi + th_half, 2.0 * math.pi)
+    r, th, ph = _sph_nodes(ng, lo[0], hi[0], th_half)
+    rc, zz = np.outer(r, np.sin(th)), np.outer(r, np.cos(th))                      # [nr][nt]
+    n_co, temp, vphi = disk_family(rc, np.abs(zz))
+    arm = np.cos(2.0 * ph[None, None, :] - 6.0 * np.log(r / 100.0)[:, None, None])   # [nr][1][np]
+    dens = n_co[:, :, None] * (1.0 + 0.15 * arm) * np.exp(0.05 * rng.standard_normal(tuple(ng)))
+    tt = temp[:, :, None] * (1.0 + 0.05 * arm) * np.exp(0.05 * rng.standard_normal(tuple(ng)))
+    vv = vphi[:, :, None] * (1.0 + 0.02 * arm)
+    grid = Grid(kind=SPH3D, n=tuple(ng), lo=lo, hi=hi, dens=np.ascontiguousarray(dens, np.float32),
+                temp=np.ascontiguousarray(tt, np.float32), vel=np.ascontiguousarray(vv, np.float32), mirror_z=False)
+    geom = Geom(nx=npix, ny=npix, fov_x=1200.0, fov_y=1200.0, incl=math.radians(45.0), pa=0.0, dist_pc=100.0, nstep=nstep)
+    line = co_line(channels_centered(nchan, 0.1 * KMS), vturb_abs=0.05 * KMS)
+    return Scene(geom, line, grid, f"sph{ng[0]}x{ng[1]}x{ng[2]}_img{npix}_c{nchan}_n{nstep}")

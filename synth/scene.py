@@ -14,6 +14,7 @@ import numpy as np
 # grid kinds
 AXISYM = 0   # (r, zeta=z/r) grid, r log-spaced, zeta uniform
 CART3D = 1   # uniform Cartesian box in the disk frame
+SPH3D = 2    # spherical (r, theta, phi): r log-spaced, theta (polar angle from +z) uniform, phi periodic over 2 pi
 # density storage
 DENS_LINEAR = 0  # grid stores n [cm^-3], interpolated linearly
 DENS_LN = 1      # grid stores ln n, interpolated then exponentiated
@@ -63,7 +64,7 @@ class Line:
 
 @dataclass
 class Grid:
-    """Field grids. AXISYM: arrays [nr][nzeta]; CART3D: arrays [nx][ny][nz] (last index fastest)."""
+    """Field grids. AXISYM: arrays [nr][nzeta]; CART3D: arrays [nx][ny][nz]; SPH3D: arrays [nr][ntheta][nphi] (last index fastest)."""
     kind: int
     n: tuple                   # (nr, nzeta) or (nx, ny, nz)
     lo: tuple                  # AXISYM: (r_min, zeta_lo); CART3D: box lower corner, au

@@ -52,6 +52,12 @@ def render(scene):
         nr, nz = gr.n
         lnr_nodes = np.log(gr.lo[0]) + (np.log(gr.hi[0]) - np.log(gr.lo[0])) * np.arange(nr) / (nr - 1)
         zeta_nodes = gr.lo[1] + (gr.hi[1] - gr.lo[1]) * np.arange(nz) / (nz - 1)
+    elif gr.kind == 2:
+        lnr_nodes = np.log(gr.lo[0]) + (np.log(gr.hi[0]) - np.log(gr.lo[0])) * np.arange(gr.n[0]) / (gr.n[0] - 1)
+        th_nodes = gr.lo[1] + (gr.hi[1] - gr.lo[1]) * np.arange(gr.n[1]) / (gr.n[1] - 1)
+        ph_nodes = 2 * np.pi * np.arange(gr.n[2] + 1) / gr.n[2]          # one extra node: 2 pi is node 0 again
+        wrap = lambda f: np.concatenate([f, f[:, :, :1]], axis=2)        # noqa: E731
+        dens, temp, vel = wrap(dens), wrap(temp), wrap(vel)
     else:
         axes = [np.linspace(gr.lo[a], gr.hi[a], gr.n[a]) for a in range(3)]
     cube = np.zeros((g.ny, g.nx, C))
@@ -60,8 +66,8 @@ def render(scene):
             X = g.x0 + (ix + 0.5 - g.nx / 2) * g.fov_x / g.nx
             Y = g.y0 + (iy + 0.5 - g.ny / 2) * g.fov_y / g.ny
             org = M @ np.array([X, Y, 0.0])
-            if gr.kind == 0:
-                zm = max(abs(gr.lo[1]), abs(gr.hi[1]))
+            if gr.kind in (0, 2):
+                zm = max(abs(gr.lo[1]), abs(gr.hi[1])) if gr.kind == 0 else 0.0
                 Rb = gr.hi[0] * np.sqrt(1 + zm ** 2)
                 b2 = X * X + Y * Y
                 if b2 >= Rb * Rb:
@@ -99,7 +105,13 @@ def render(scene):
                     def samp(f):
                         return (wa0 * (wb0 * f[i, j] + wb1 * f[i, j + 1]) + wa1 * (wb0 * f[i + 1, j] + wb1 * f[i + 1, j + 1]))
                 else:
-                    ws = [_interp_weights(axes[a], p[a]) for a in range(3)]
+                    if gr.kind == 2:
+                        rho_ = np.linalg.norm(p)
+                        phi_ = np.arctan2(p[1], p[0]) % (2 * np.pi)
+                        ws = [_interp_weights(lnr_nodes, np.log(rho_)), _interp_weights(th_nodes, np.arccos(p[2] / rho_)),
+                              _interp_weights(ph_nodes, phi_)]
+                    else:
+                        ws = [_interp_weights(axes[a], p[a]) for a in range(3)]
                     if any(w is None for w in ws):
                         continue
                     (i, wx0, wx1), (j, wy0, wy1), (l, wz0, wz1) = ws

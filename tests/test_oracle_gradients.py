@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from oracle import pyoracle as po
-from synth import slab_scene, tiny_axisym_scene, tiny_cart_scene
+from synth import slab_scene, tiny_axisym_scene, tiny_cart_scene, tiny_sph_scene
 
 FIELDS = ("dens", "temp", "vel")
 
@@ -44,6 +44,8 @@ SCENES = {
                                                   mirror=False, az_deg=20.0),
     "cart_ln_kepler": lambda: tiny_cart_scene(seed=33),
     "cart_lin_vphi": lambda: tiny_cart_scene(seed=34, dens_ln=False, kepler_frac=False),
+    "sph_lin_vphi": lambda: tiny_sph_scene(seed=35),
+    "sph_ln_kepler": lambda: tiny_sph_scene(seed=36, dens_ln=True, kepler_frac=True),
 }
 
 
