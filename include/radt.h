@@ -47,7 +47,7 @@ enum {
     RADT_E_CUDA = -4              /* CUDA runtime error (message in radt_last_error) */
 };
 
-enum { RADT_GRID_AXISYM = 0, RADT_GRID_CART3D = 1 };
+enum { RADT_GRID_AXISYM = 0, RADT_GRID_CART3D = 1, RADT_GRID_SPH3D = 2 };
 enum { RADT_DENS_LINEAR = 0, RADT_DENS_LN = 1 };
 enum { RADT_VEL_VPHI = 0, RADT_VEL_KEPLER_FRAC = 1 };
 enum { RADT_UNIT_S0 = 0, RADT_UNIT_CGS = 1, RADT_UNIT_JY_PIXEL = 2 };
@@ -93,6 +93,9 @@ typedef struct radt_line {
  *   AXISYM : n = {nr, nzeta, 1}; nodes r_i = lo[0] (hi[0]/lo[0])^(i/(nr-1)), zeta_j = lo[1] +
  *            (hi[1]-lo[1]) j/(nzeta-1), zeta = |z|/r if mirror_z else z/r (mirror_z needs lo[1] >= 0);
  *   CART3D : n = {nx, ny, nz}; nodes lo[a] + (hi[a]-lo[a]) i/(n[a]-1) in the disk frame.
+ *   SPH3D  : n = {nr, ntheta, nphi}; r_i as AXISYM (spherical radius); theta_j = lo[1] + (hi[1]-lo[1]) j/(ntheta-1), the
+ *            polar angle from the +z axis of the disk frame, 0 <= lo[1] < hi[1] <= pi; phi_k = 2 pi k/nphi, periodic
+ *            (lo[2], hi[2] are ignored); arrays [b][ir][itheta][iphi].
  * Interpolation is bi/tri-linear in index space; outside the node range is vacuum.
  * dens/temp/vel are DEVICE pointers to float32 arrays [batch][cells]; item b starts at
  * ptr + b * batch_stride (elements).  Caller owns all memory. */

@@ -73,6 +73,13 @@ int validate(const radt_geom *geom, const radt_line *line, const radt_grid *grid
             if (!(grid->hi[a] > grid->lo[a])) return fail(RADT_E_INVALID, "need lo < hi");
         }
         if (grid->mirror_z) return fail(RADT_E_UNSUPPORTED, "mirror_z applies to axisymmetric grids only");
+    } else if (grid->kind == RADT_GRID_SPH3D) {
+        for (int a = 0; a < 3; ++a)
+            if (grid->n[a] < 2) return fail(RADT_E_INVALID, "spherical grid needs >= 2 nodes per axis");
+        if (!(grid->lo[0] > 0) || !(grid->hi[0] > grid->lo[0])) return fail(RADT_E_INVALID, "need 0 < r_min < r_max");
+        if (!(grid->lo[1] >= 0) || !(grid->hi[1] > grid->lo[1]) || !(grid->hi[1] <= kPI))
+            return fail(RADT_E_INVALID, "need 0 <= theta_lo < theta_hi <= pi");
+        if (grid->mirror_z) return fail(RADT_E_UNSUPPORTED, "mirror_z applies to axisymmetric grids only");
     } else {
         return fail(RADT_E_UNSUPPORTED, "unknown grid kind %d", grid->kind);
     }
@@ -93,7 +100,7 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
     d.kind = grid->kind; d.mirror = grid->mirror_z; d.dens_mode = grid->dens_mode; d.vel_mode = grid->vel_mode;
     d.n0 = grid->n[0]; d.n1 = grid->n[1]; d.n2 = grid->kind == RADT_GRID_AXISYM ? 1 : grid->n[2];
     d.cells = grid_cells(grid);
-    if (grid->kind == RADT_GRID_AXISYM) {
+    if (grid->kind == RADT_GRID_AXISYM || grid->kind == RADT_GRID_SPH3D) {
         double rmin = grid->lo[0], rmax = grid->hi[0];
         d.rmin2 = rmin * rmin; d.rmax2 = rmax * rmax; d.inv_rmin = 1.0 / rmin;
         d.zlo = grid->lo[1]; d.zhi = grid->hi[1];
@@ -108,6 +115,14 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
         d.inv_rmin2_f = (float)(1.0 / (rmin * rmin)); d.half_uscale = (float)(0.5 * (double)(grid->n[0] - 1) / d.lg2_ratio);
         double zm = std::fmax(std::fabs(grid->lo[1]), std::fabs(grid->hi[1]));
         d.rb2 = rmax * rmax * (1.0 + zm * zm);
+        if (grid->kind == RADT_GRID_SPH3D) {
+            d.n2 = grid->n[2];
+            d.rb2 = rmax * rmax;
+            d.cos_tlo = std::cos(grid->lo[1]); d.cos_thi = std::cos(grid->hi[1]);
+            d.th_c0 = (float)(0.5 * kPI - grid->lo[1]);
+            d.th_scale = (float)((double)(grid->n[1] - 1) / (grid->hi[1] - grid->lo[1]));
+            d.ph_scale = (float)((double)grid->n[2] / (2.0 * kPI));
+        }
     } else {
         for (int a = 0; a < 3; ++a) {
             d.lo[a] = grid->lo[a]; d.hi[a] = grid->hi[a];
@@ -120,6 +135,7 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
 // tolerates one cell of error: require the smallest cell to be 100 times coarser than that.
 bool prefilter_safe(const radt_grid *grid)
 {
+    if (grid->kind == RADT_GRID_SPH3D) return true;      // its prefilter tests the (r, theta) range with wide margins only
     if (grid->kind == RADT_GRID_AXISYM) {
         double rmin = grid->lo[0], rmax = grid->hi[0];
         double zm = std::fmax(std::fabs(grid->lo[1]), std::fabs(grid->hi[1]));
@@ -197,13 +213,15 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     w.rays = off; off = align256(off + nrays * sizeof(RayRec));
     w.qtab = off; off = align256(off + (RADT_NQ + 2) * sizeof(float2));
     w.vcs = off; off = align256(off + (size_t)batch * RADT_MAXCHAN * sizeof(float2));
-    w.rnode = off; off = align256(off + (size_t)(grid->kind == RADT_GRID_AXISYM ? grid->n[0] : 1) * sizeof(double2));
+    w.rnode = off; off = align256(off + (size_t)(grid->kind != RADT_GRID_CART3D ? grid->n[0] : 1) * sizeof(double2));
     size_t cells = (size_t)grid_cells(grid) * (size_t)batch;
     w.cells = off; off = align256(off + cells * sizeof(float4));
     if (grid->kind == RADT_GRID_AXISYM) {
         w.occ_wpr = (grid->n[1] + 31) / 32;
         w.occ_words = grid->n[0] * w.occ_wpr;
         w.occ_nbj = 1;
+    } else if (grid->kind == RADT_GRID_SPH3D) {
+        w.occ_wpr = 1; w.occ_words = 1; w.occ_nbj = 1;          // no occupancy bitmap for spherical grids yet
     } else {
         // 3-D: one bit per block of 4 x 4 x 4 cells
         int nbi = (grid->n[0] - 1 + 3) / 4, nbj = (grid->n[1] - 1 + 3) / 4, nbl = (grid->n[2] - 1 + 3) / 4;
@@ -293,7 +311,8 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         // occupancy bitmap for the window kernels' prefilter (axisymmetric grids): with LINEAR densities the
         // adjoint needs every in-grid step (dL/dn of empty cells), so only the forward and LN grids use it
         const bool win = use_win;
-        const bool occ = win && g_opt_skip_empty && (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN);
+        const bool occ = win && g_opt_skip_empty && grid->kind != RADT_GRID_SPH3D &&
+                         (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN);
         SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr; SP.occ_nbj = w.occ_nbj;
         SP.occ_thr = grid->dens_mode == RADT_DENS_LN ? -39.1439f : 1e-17f;     // N_EMPTY of the march kernels
         SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;

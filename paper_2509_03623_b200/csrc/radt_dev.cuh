@@ -45,7 +45,10 @@ struct DevGrid {
     float inv_rmin2_f, half_uscale;    // u = lg2(r^2 / r_min^2) (nr-1) / (2 log2(r_max/r_min))
     // cartesian
     double lo[3], hi[3], inv_d[3];
-    double rb2;                        // bounding sphere radius^2 (axisym clip)
+    double rb2;                        // bounding sphere radius^2 (axisym and spherical clip)
+    // spherical (kind 2): n0 = nr (log-spaced, shares rmin2/rmax2/uscale/... with the axisymmetric axis), n1 = ntheta, n2 = nphi
+    double cos_tlo, cos_thi;           // cos of the theta range (decreasing in theta)
+    float th_c0, th_scale, ph_scale;   // theta index = (th_c0 - asin(z/rho)) th_scale, th_c0 = pi/2 - theta_lo; phi index = phi ph_scale
 };
 
 struct DevLine {

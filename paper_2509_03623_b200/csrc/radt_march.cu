@@ -338,6 +338,11 @@ static cudaError_t launch_bwd_t(const MarchParams &P, int nbatch, cudaStream_t s
         if (np <= 2) return fn<0, 2>(P, nbatch, st);                             \
         return fn<0, 4>(P, nbatch, st);                                          \
     }                                                                            \
+    if (P.grid.kind == 2) {                                                      \
+        if (np <= 1) return fn<2, 1>(P, nbatch, st);                             \
+        if (np <= 2) return fn<2, 2>(P, nbatch, st);                             \
+        return fn<2, 4>(P, nbatch, st);                                          \
+    }                                                                            \
     if (np <= 1) return fn<1, 1>(P, nbatch, st);                                 \
     if (np <= 2) return fn<1, 2>(P, nbatch, st);                                 \
     return fn<1, 4>(P, nbatch, st);

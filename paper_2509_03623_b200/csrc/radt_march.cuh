@@ -18,6 +18,7 @@ struct StepState {
     float n, T, invT, ex, em1, W, invalpha, proj, vk, dsf, qy;
     float f0, f1, f2;
     long long cell;
+    int dk;                             // spherical grids: offset of the next phi node (1, or 1 - nphi across the seam)
     bool tclamp;
     // uniform channel lattice (window path): u'(c) = u0 + (c - cref) dvA; channels wlo..whi can lie inside the line
     float u0, dvA;
@@ -85,6 +86,58 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
             vel_d = fma(fud, a1 - a0, a0);
         }
         st.f0 = fu; st.f1 = fw; st.f2 = 0.f; st.cell = cell;
+    } else if (KIND == 2) {
+        // spherical (r, theta, phi) grid.  In/out decision in fp64 on rho^2 and cos(theta);
+        // radial index as on the axisymmetric grid (cell from an fp32 estimate, in-cell fraction from rho^2/r_i^2);
+        // theta through asin(z/rho), which is well conditioned around the equator where disk grids live; phi
+        // through atan2 in fp32 (1e-7 rad is 4e-6 of a cell at 256 nodes).
+        double rho2 = r2 + z * z;
+        double irho = (double)rsqrt_approx((float)rho2);
+        irho = irho * fma(-0.5 * rho2, irho * irho, 1.5);
+        double cz = z * irho;
+        bool in = (k < P.nstep) && (r2 > 0.0) && (rho2 >= g.rmin2) && (rho2 <= g.rmax2) && (cz <= g.cos_tlo) && (cz >= g.cos_thi);
+        if (!in) return;
+        float wf = fminf(fmaxf((g.th_c0 - asinf((float)cz)) * g.th_scale, 0.f), (float)(g.n1 - 1));
+        int j = min(max(rn_int(wf - 0.5f), 0), g.n1 - 2);
+        float fw = wf - (float)j;
+        float uf = lg2_approx((float)rho2 * g.inv_rmin2_f) * g.half_uscale;
+        int i = min(max(rn_int(uf - 0.5f), 0), g.n0 - 2);
+        double t = rho2 * __ldg(P.ws.rnode + i).y;
+        float fu;
+        if (g.fine_r) {
+            float xm = (float)(t - 1.0);
+            float sq = xm * rcp_approx(2.0f + xm);
+            float s2 = sq * sq;
+            fu = sq * fmaf(s2, fmaf(s2, fmaf(s2, fmaf(s2, 1.0f / 9.0f, 1.0f / 7.0f), 0.2f), 1.0f / 3.0f), 1.0f) * g.inv_cell_ln;
+        } else {
+            fu = lg2_approx((float)t) * (0.5f * g.inv_cell_lg2);
+        }
+        float qf = atan2f((float)y, (float)x) * g.ph_scale;
+        if (qf < 0.f) qf += (float)g.n2;
+        qf = fminf(fmaxf(qf, 0.f), (float)g.n2);
+        int l = min(max(rn_int(qf - 0.5f), 0), g.n2 - 1);
+        float fq = fminf(fmaxf(qf - (float)l, 0.f), 1.f);
+        int dk = (l == g.n2 - 1) ? 1 - g.n2 : 1;
+        long long cell = ((long long)i * g.n1 + j) * g.n2 + l;
+        long long sy = g.n2, sx = (long long)g.n1 * g.n2;
+        float4 c000 = __ldg(cells + cell), c001 = __ldg(cells + cell + dk);
+        float4 c010 = __ldg(cells + cell + sy), c011 = __ldg(cells + cell + sy + dk);
+        float4 c100 = __ldg(cells + cell + sx), c101 = __ldg(cells + cell + sx + dk);
+        float4 c110 = __ldg(cells + cell + sx + sy), c111 = __ldg(cells + cell + sx + sy + dk);
+        dens = lerp1(lerp1(lerp1(c000.x, c001.x, fq), lerp1(c010.x, c011.x, fq), fw),
+                     lerp1(lerp1(c100.x, c101.x, fq), lerp1(c110.x, c111.x, fq), fw), fu);
+        temp = lerp1(lerp1(lerp1(c000.y, c001.y, fq), lerp1(c010.y, c011.y, fq), fw),
+                     lerp1(lerp1(c100.y, c101.y, fq), lerp1(c110.y, c111.y, fq), fw), fu);
+        {
+            double fzd = (double)fq, fyd = (double)fw, fxd = (double)fu;
+            double a00 = fma(fzd, (double)c001.z - (double)c000.z, (double)c000.z);
+            double a01 = fma(fzd, (double)c011.z - (double)c010.z, (double)c010.z);
+            double a10 = fma(fzd, (double)c101.z - (double)c100.z, (double)c100.z);
+            double a11 = fma(fzd, (double)c111.z - (double)c110.z, (double)c110.z);
+            double b0 = fma(fyd, a01 - a00, a00), b1 = fma(fyd, a11 - a10, a10);
+            vel_d = fma(fxd, b1 - b0, b0);
+        }
+        st.f0 = fu; st.f1 = fw; st.f2 = fq; st.cell = cell; st.dk = dk;
     } else {
         bool in = (k < P.nstep) && (r2 > 0.0) && (x >= g.lo[0]) && (x <= g.hi[0]) && (y >= g.lo[1]) && (y <= g.hi[1]) &&
                   (z >= g.lo[2]) && (z <= g.hi[2]);
@@ -114,7 +167,7 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
             double b0 = fma(fyd, a01 - a00, a00), b1 = fma(fyd, a11 - a10, a10);
             vel_d = fma(fxd, b1 - b0, b0);
         }
-        st.f0 = fx; st.f1 = fy; st.f2 = fz; st.cell = cell;
+        st.f0 = fx; st.f1 = fy; st.f2 = fz; st.cell = cell; st.dk = 1;
     }
     // ---- O7: channel-independent LTE quantities (Eq. 13-17) ----
     float n = (g.dens_mode == 1) ? ex2_approx(dens * RADT_LOG2E) : dens;
@@ -365,7 +418,7 @@ __device__ __forceinline__ void phase_c(const MarchParams &P, const StepState &s
             for (int cidx = 0; cidx < 8; ++cidx) {
                 int dx = (cidx >> 2) & 1, dy = (cidx >> 1) & 1, dz = cidx & 1;
                 float w = (dx ? st.f0 : 1.f - st.f0) * (dy ? st.f1 : 1.f - st.f1) * (dz ? st.f2 : 1.f - st.f2);
-                red_add_cell(gp + (dx * sx + dy * sy + dz), w, dL_dd, dL_dT, dL_dv);
+                red_add_cell(gp + (dx * sx + dy * sy + dz * st.dk), w, dL_dd, dL_dT, dL_dv);
             }
         }
     } else {
@@ -382,7 +435,7 @@ __device__ __forceinline__ void phase_c(const MarchParams &P, const StepState &s
             for (int cidx = 0; cidx < 8; ++cidx) {
                 int dx = (cidx >> 2) & 1, dy = (cidx >> 1) & 1, dz = cidx & 1;
                 float w = (dx ? st.f0 : 1.f - st.f0) * (dy ? st.f1 : 1.f - st.f1) * (dz ? st.f2 : 1.f - st.f2);
-                red_add_dens(gp + (dx * sx + dy * sy + dz), w * dL_dd);
+                red_add_dens(gp + (dx * sx + dy * sy + dz * st.dk), w * dL_dd);
             }
         }
     }

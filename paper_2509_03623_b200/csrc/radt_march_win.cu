@@ -32,6 +32,7 @@ struct PreCtx {
     float ox, oy, oz, wx, wy, wz, s0, ds;
     float us_half, lrm;                   // u = lg2(r^2) us_half - lrm
     float zlo, wscale;
+    float r2lo, r2hi, czlo, czhi;         // spherical: accepted ranges of rho^2 and z/rho, with margins
     float lo[3], inv_d[3];
 };
 
@@ -45,6 +46,11 @@ __device__ __forceinline__ void pre_setup(const MarchParams &P, const DevGeom &G
         pc.us_half = 0.5f * P.grid.uscale;
         pc.lrm = -lg2_approx((float)P.grid.inv_rmin) * P.grid.uscale;
         pc.zlo = (float)P.grid.zlo; pc.wscale = (float)P.grid.wscale_d;
+    } else if (KIND == 2) {
+        // margins: one percent in radius, two theta cells in z/rho (|d cos| <= |d theta|)
+        const float dth = 2.0f / P.grid.th_scale;
+        pc.r2lo = (float)P.grid.rmin2 * 0.98f; pc.r2hi = (float)P.grid.rmax2 * 1.02f;
+        pc.czlo = (float)P.grid.cos_thi - dth; pc.czhi = (float)P.grid.cos_tlo + dth;
     } else {
 #pragma unroll
         for (int a = 0; a < 3; ++a) { pc.lo[a] = (float)P.grid.lo[a]; pc.inv_d[a] = (float)P.grid.inv_d[a]; }
@@ -71,6 +77,10 @@ __device__ __forceinline__ bool prefilter(const MarchParams &P, const PreCtx &pc
         int j = min(max(rn_int(wf - 0.5f), 0), P.grid.n1 - 2);
         unsigned w = __ldg(occ + i * P.occ_wpr + (j >> 5));
         return (w >> (j & 31)) & 1u;
+    } else if (KIND == 2) {
+        float rho2 = fmaf(x, x, fmaf(y, y, z * z));
+        float cz = z * rsqrt_approx(fmaxf(rho2, 1e-30f));
+        return rho2 > pc.r2lo && rho2 < pc.r2hi && cz > pc.czlo && cz < pc.czhi;
     } else {
         float tx = (x - pc.lo[0]) * pc.inv_d[0], ty = (y - pc.lo[1]) * pc.inv_d[1], tz = (z - pc.lo[2]) * pc.inv_d[2];
         bool in = tx > -1.0f && tx < (float)P.grid.n0 && ty > -1.0f && ty < (float)P.grid.n1 && tz > -1.0f &&
@@ -555,11 +565,13 @@ static cudaError_t launch_w(K kern, const MarchParams &P, int nbatch, size_t war
 cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
     const size_t wb = fwd_warp_bytes(P.line.ngroups);
-    return P.grid.kind == 0 ? launch_w(k_march_fwd_w<0>, P, nbatch, wb, st) : launch_w(k_march_fwd_w<1>, P, nbatch, wb, st);
+    return P.grid.kind == 0 ? launch_w(k_march_fwd_w<0>, P, nbatch, wb, st)
+         : P.grid.kind == 1 ? launch_w(k_march_fwd_w<1>, P, nbatch, wb, st) : launch_w(k_march_fwd_w<2>, P, nbatch, wb, st);
 }
 
 cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
     const size_t wb = bwd_warp_bytes(P.line.ngroups);
-    return P.grid.kind == 0 ? launch_w(k_march_bwd_w<0>, P, nbatch, wb, st) : launch_w(k_march_bwd_w<1>, P, nbatch, wb, st);
+    return P.grid.kind == 0 ? launch_w(k_march_bwd_w<0>, P, nbatch, wb, st)
+         : P.grid.kind == 1 ? launch_w(k_march_bwd_w<1>, P, nbatch, wb, st) : launch_w(k_march_bwd_w<2>, P, nbatch, wb, st);
 }

@@ -49,6 +49,16 @@ __device__ __forceinline__ RayRec clip_ray(const DevGeom &G, const DevGrid &g, i
         }
         return rr;
     }
+    if (g.kind == 2) {
+        // spherical grid: bounding sphere of radius r_max; every step may lie inside
+        double b2 = X * X + Y * Y;
+        if (!(b2 < g.rb2)) return rr;
+        double sh = sqrt(g.rb2 - b2);
+        rr.s0 = -sh;
+        rr.ds = 2.0 * sh / (double)nstep;
+        rr.k_lo = 0; rr.k_hi = nstep;
+        return rr;
+    }
     const double o[3] = { ox, oy, oz }, d[3] = { G.wx, G.wy, G.wz };
     double tmin = -INFINITY, tmax = INFINITY;
 #pragma unroll
@@ -118,7 +128,7 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
             float hi = (float)vv;
             P.ws.vcs[(size_t)(P.b0 + b) * RADT_MAXCHAN + c] = make_float2(hi, (float)(vv - (double)hi));
         }
-        if (P.grid.kind == 0 && t < P.grid.n0 && P.b0 == 0) {
+        if (P.grid.kind != 1 && t < P.grid.n0 && P.b0 == 0) {
             // node radii of the log-spaced axis, r_i = r_min (r_max/r_min)^(i/(nr-1))
             double ri = exp2((double)t * P.grid.lg2_ratio / (double)(P.grid.n0 - 1)) / P.grid.inv_rmin;
             if (t == 0) ri = 1.0 / P.grid.inv_rmin;
@@ -275,7 +285,7 @@ cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const C
     int nb_rays = P.do_rays ? (int)((nrays + 255) / 256) : 0;
     int need_tab = (RADT_NQ + 2) * 32;
     if (P.nbatch * RADT_MAXCHAN > need_tab) need_tab = P.nbatch * RADT_MAXCHAN;
-    if (P.grid.kind == 0 && P.grid.n0 > need_tab) need_tab = P.grid.n0;
+    if (P.grid.kind != 1 && P.grid.n0 > need_tab) need_tab = P.grid.n0;
     int nb_tab = P.do_tables ? (need_tab + 255) / 256 : 0;
     long long total = P.grid.cells * P.nbatch;
     int nb_pack = 0;

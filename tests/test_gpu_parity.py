@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 from oracle import pyoracle as po
-from synth import (UNIT_CGS, UNIT_JY_PIXEL, co_line, l2_target, make_config, slab_scene, tiny_axisym_scene,
+from synth import (UNIT_CGS, UNIT_JY_PIXEL, co_line, l2_target, make_config, slab_scene, sph_benchmark_scene, tiny_axisym_scene,
+                   tiny_sph_scene,
                    tiny_cart_scene)
 from tests.tolerances import check_cube, check_grad
 
@@ -102,6 +103,19 @@ def test_tiny_axisym(rt, kw):
                                 dict(seed=43, incl_deg=80.0, pa_deg=-40.0, ng=(20, 17, 13), npix=12, nchan=40, nstep=45)])
 def test_tiny_cart(rt, kw):
     _parity_fwd_bwd(rt, tiny_cart_scene(**kw), f"tiny_cart{kw}")
+
+
+@pytest.mark.parametrize("kw", [dict(seed=71), dict(seed=72, dens_ln=True, kepler_frac=True),
+                                dict(seed=73, incl_deg=0.0, pa_deg=0.0, az_deg=0.0, npix=9),
+                                dict(seed=74, ng=(9, 12, 5), incl_deg=88.0, npix=11, nstep=40, nchan=37),
+                                dict(seed=75, ng=(6, 5, 64), npix=8, nstep=33)])
+def test_tiny_spherical(rt, kw):
+    """Spherical (r, theta, phi) grids: the phi seam, few and many phi nodes, pole-on and edge-on."""
+    _parity_fwd_bwd(rt, tiny_sph_scene(**kw), f"tiny_sph {kw}")
+
+
+def test_spherical_benchmark_shape_reduced(rt):
+    _parity_fwd_bwd(rt, sph_benchmark_scene(ng=(64, 24, 48), npix=40, nchan=32, nstep=96), "sph benchmark reduced")
 
 
 @pytest.mark.parametrize("n,T,v", [(1.0, 30.0, 0.0), (1e-4, 30.0, 0.0), (400.0, 150.0, 0.1e5), (1e6, 40.0, 0.0)])
@@ -221,6 +235,11 @@ def test_cfg3_full_sampled(rt):
 def test_cfg4_full_sampled(rt):
     R, cube = _sampled_full(rt, make_config(4), "cfg4 full", nsample=64)
     assert cube.shape == (1, 512, 512, 64)
+
+
+def test_spherical_benchmark_full_sampled(rt):
+    """The stand-in for the paper's timing benchmark (512 x 96 x 256 spherical grid, 256 x 256 px) at full size."""
+    _sampled_full(rt, sph_benchmark_scene(), "sph benchmark", nsample=64)
 
 
 def test_cfg5_full_sampled(rt):
