@@ -33,15 +33,19 @@ METRIC = "ray*channel*step samples/s (fwd+bwd step)"
 UNIT = "samples/s"
 
 
+def _scenes(cfg):
+    """Configs 1-5: BASELINE.json configs[0..4]; 6: stand-in for the paper's own timing benchmark."""
+    from synth import make_config, sph_benchmark_scene
+    s = sph_benchmark_scene() if cfg == 6 else make_config(cfg)
+    return s if isinstance(s, list) else [s]
+
+
 def _workload_name(cfg):
     from synth import config_names
-    return config_names()[cfg]
+    return "cfg6_" + _SPH_NAME if cfg == 6 else config_names()[cfg]
 
 
-def _scenes(cfg):
-    from synth import make_config
-    s = make_config(cfg)
-    return s if isinstance(s, list) else [s]
+_SPH_NAME = "sph512x96x256_img256_c64_n256"
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -368,7 +372,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=2, help="SURVEY.md config 1..5 (BASELINE.json configs[k-1])")
+    ap.add_argument("--config", type=int, default=2, help="SURVEY.md config 1..5 (BASELINE.json configs[k-1]); 6 = spherical 512x96x256 grid at 256x256 px, the shape "
+                         "of the paper's own timing benchmark")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--win-path", type=int, default=1, choices=[0, 1],
