@@ -309,9 +309,24 @@ struct RayCtx {
     int k_lo, k_hi;
 };
 
+// k-th index of 0..n-1 in centre-out order: c, c-1, c+1, c-2, ... with c = n/2 (a bijection for any n)
+__device__ __forceinline__ int centre_out(int k, int n)
+{
+    const int c = n >> 1, h = (k + 1) >> 1;
+    int t = (k & 1) ? c - h : c + h;
+    // one side runs out first when n is even (c + h reaches n): the remaining indices continue on the other side
+    if (t >= n) t = n - 1 - k;
+    if (t < 0) t = k;
+    return t;
+}
+
 __device__ __forceinline__ bool ray_setup(const MarchParams &P, RayCtx &rc, int warp)
 {
-    int tx = blockIdx.x % P.tiles_x, ty = blockIdx.x / P.tiles_x;
+    // Tiles are issued from the image centre outwards (rows, and tiles within a row, alternate around the centre):
+    // rays through the disk centre carry the most steps, the empty corners fill the tail of the launch
+    // (measured on config 2: under 1 % either way; kept because the heavy tiles no longer depend on the PA).
+    int kx = blockIdx.x % P.tiles_x, ky = blockIdx.x / P.tiles_x;
+    int tx = centre_out(kx, P.tiles_x), ty = centre_out(ky, P.tiles_y);
     rc.b = blockIdx.y;
     rc.ix = tx * RADT_TILE_X + (warp & (RADT_TILE_X - 1));
     rc.iy = ty * RADT_TILE_Y + (warp / RADT_TILE_X);
