@@ -499,6 +499,20 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     if (!grid->dens || !grid->temp || !grid->vel) return fail(RADT_E_INVALID, "null field pointer");
     int count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || count < 1) return fail(RADT_E_CUDA, "no CUDA device");
+    {
+        // keep freed blocks in the stream-ordered pool across calls: by default the pool hands its memory back to the
+        // driver at every synchronisation and each call would pay for fresh cudaMalloc's
+        static thread_local int pool_dev = -1;
+        int dev = 0;
+        CUDA_TRY(cudaGetDevice(&dev));
+        if (pool_dev != dev) {
+            cudaMemPool_t pool;
+            CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, dev));
+            unsigned long long keep = ~0ull;
+            CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+            pool_dev = dev;
+        }
+    }
     DevBufs B;
     long long cells = grid_cells(grid);
     long long stride = batch > 1 ? grid->batch_stride : cells;
