@@ -433,3 +433,36 @@ def test_pipe_peaks_are_sane(rt):
     assert 14.0 < per_sm_clk < 16.5            # MUFU.EX2: 16 lanes / clk / SM
     ops, clk = rt.binding.radt_pipe_peak(1)
     assert 100.0 < ops / 148 / (clk * 1e6) < 130.0     # FFMA: 128 lanes / clk / SM
+
+
+def test_fit_step_is_cuda_graph_capturable(rt):
+    """include/radt.h: the device entry points never allocate or synchronise and enqueue everything on the caller's
+    stream, so a whole fit step can be captured into a CUDA graph and replayed with new field values."""
+    sc = make_config(1, npix=32)
+    R = rt.Renderer([sc])
+    R.render()
+    tgt, sigma = l2_target(R.cube.cpu().numpy()[0], 3)
+    R.set_target(tgt[None], sigma)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        R.fit_step(side)                                  # warm-up on the capture stream
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        R.fit_step(torch.cuda.current_stream())
+    # new inputs, eager reference first
+    R.temp.mul_(1.05)
+    R.fit_step()
+    torch.cuda.synchronize()
+    want = [t.clone() for t in (R.cube, R.dl_dcube, R.loss, R.g_dens, R.g_temp, R.g_vel)]
+    for t in (R.cube, R.dl_dcube, R.g_dens, R.g_temp, R.g_vel):
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(R.cube.cpu().numpy(), want[0].cpu().numpy())
+    np.testing.assert_array_equal(R.dl_dcube.cpu().numpy(), want[1].cpu().numpy())
+    assert float(R.loss.cpu()) == pytest.approx(float(want[2].cpu()), rel=1e-12)
+    for got, ref, nm in zip((R.g_dens, R.g_temp, R.g_vel), want[3:], ("dens", "temp", "vel")):
+        check_grad(f"graph replay g_{nm}", got.cpu().numpy()[0], ref.cpu().numpy()[0].astype(np.float64))
