@@ -33,19 +33,19 @@ METRIC = "ray*channel*step samples/s (fwd+bwd step)"
 UNIT = "samples/s"
 
 
+_SPH = {"npix": 256, "nchan": 64}       # config 6 image size and channel count (--sph-npix / --sph-nchan sweep them)
+
+
 def _scenes(cfg):
     """Configs 1-5: BASELINE.json configs[0..4]; 6: stand-in for the paper's own timing benchmark."""
     from synth import make_config, sph_benchmark_scene
-    s = sph_benchmark_scene() if cfg == 6 else make_config(cfg)
+    s = sph_benchmark_scene(npix=_SPH["npix"], nchan=_SPH["nchan"]) if cfg == 6 else make_config(cfg)
     return s if isinstance(s, list) else [s]
 
 
 def _workload_name(cfg):
     from synth import config_names
-    return "cfg6_" + _SPH_NAME if cfg == 6 else config_names()[cfg]
-
-
-_SPH_NAME = "sph512x96x256_img256_c64_n256"
+    return f"cfg6_sph512x96x256_img{_SPH['npix']}_c{_SPH['nchan']}_n256" if cfg == 6 else config_names()[cfg]
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -378,7 +378,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--win-path", type=int, default=1, choices=[0, 1],
                     help="RADT_OPT_WIN_PATH: 1 = window kernels on uniform channel lattices (default), 0 = channel-table kernels")
+    ap.add_argument("--sph-npix", type=int, default=256, help="config 6: image size (the paper sweeps it at 20 channels)")
+    ap.add_argument("--sph-nchan", type=int, default=64, help="config 6: channels of 0.1 km/s (the paper sweeps them at 256 px)")
     args = ap.parse_args()
+    _SPH.update(npix=args.sph_npix, nchan=args.sph_nchan)
     if args.impl == "reference":
         run_reference(args)
     else:
