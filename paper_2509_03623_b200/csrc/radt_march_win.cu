@@ -8,8 +8,9 @@
 //   phase A (lanes over candidate steps): exact fp64 in/out decision, sampling, LTE thermodynamics, the step's
 //       channel window and group -> compacted step entries in shared memory, two steps per slot pair;
 //   phase B (lanes over channels): per PAIR of steps one packed f32x2 evaluation (4 MUFU.EX2) and the
-//       sequential accumulate of O9; the lane's (I, T) live in two scalar registers while the group is
-//       unchanged and are swapped with the per-group state when the group moves.
+//       sequential accumulate of O9; the (I, T) of all channels of the ray sit in shared memory, the lane
+//       keeps those of the one channel it serves in registers and swaps them when the group moves, which
+//       happens only when the next pair's union window no longer fits the current group (hysteresis).
 // Steps wider than 32 channels (or RADT_OPT_WINDOW = 0) run one pass per fixed 32-channel block.
 // Algorithm: DESIGN.md O4-O11; PAPER.md:262-294 (Eq. 11-17).
 #include "radt_march.cuh"
