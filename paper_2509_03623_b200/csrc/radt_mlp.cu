@@ -15,6 +15,12 @@
 #define MLP_SA (MLP_TB + 1)            // activation row stride (adjoint): scalar reads by unit are conflict free
 #define MLP_SD (MLP_TB + 4)            // delta row stride: 16-byte aligned rows for broadcast float4 reads
 
+// packed f32x2 FMA (sm_100): every dot product below runs as two interleaved partial sums, one FFMA2 per two terms
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 mlp_pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ float mlp_sum2(f2 v) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return lo + hi; }
+__device__ __forceinline__ f2 mlp_fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+
 struct MlpOff {
     int W[MLP_H + 1], b[MLP_H + 1], D;
 };
@@ -69,20 +75,20 @@ __device__ __forceinline__ void mlp_layer_first(const float *__restrict__ W, con
 __device__ __forceinline__ void mlp_layer(const float *__restrict__ W, const float *__restrict__ b, const float *in,
                                           float *out, int stride, int node, int part)
 {
-    float h[MLP_W];
+    f2 h[MLP_W / 2];
 #pragma unroll
-    for (int i = 0; i < MLP_W; ++i) h[i] = in[i * stride + node];
+    for (int i = 0; i < MLP_W / 2; ++i) h[i] = mlp_pk(in[2 * i * stride + node], in[(2 * i + 1) * stride + node]);
 #pragma unroll 4
     for (int o = part * MLP_PW; o < (part + 1) * MLP_PW; ++o) {
-        const float4 *row = reinterpret_cast<const float4 *>(W + o * MLP_W);
-        float a0 = b[o], a1 = 0.f;
+        const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(W + o * MLP_W);
+        f2 a0 = mlp_pk(b[o], 0.f), a1 = mlp_pk(0.f, 0.f);
 #pragma unroll
         for (int q = 0; q < MLP_W / 4; ++q) {
-            const float4 w = row[q];
-            a0 = fmaf(w.x, h[4 * q], a0); a1 = fmaf(w.y, h[4 * q + 1], a1);
-            a0 = fmaf(w.z, h[4 * q + 2], a0); a1 = fmaf(w.w, h[4 * q + 3], a1);
+            const ulonglong2 w = row[q];
+            a0 = mlp_fma2(w.x, h[2 * q], a0);
+            a1 = mlp_fma2(w.y, h[2 * q + 1], a1);
         }
-        out[o * stride + node] = fmaxf(a0 + a1, 0.f);
+        out[o * stride + node] = fmaxf(mlp_sum2(a0) + mlp_sum2(a1), 0.f);
     }
 }
 
@@ -136,20 +142,20 @@ __device__ __forceinline__ void mlp_grad_weights(const float *act, const float *
                                                  int nout, int t, int part)
 {
     if (t < fan_in) {
-        float a[MLP_TB];
+        f2 a[MLP_TB / 2];
 #pragma unroll
-        for (int n = 0; n < MLP_TB; ++n) a[n] = act[t * MLP_SA + n];
+        for (int n = 0; n < MLP_TB / 2; ++n) a[n] = mlp_pk(act[t * MLP_SA + 2 * n], act[t * MLP_SA + 2 * n + 1]);
 #pragma unroll 2
         for (int o = part * MLP_PW; o < (part + 1) * MLP_PW; ++o) {
-            const float4 *row = reinterpret_cast<const float4 *>(delta + o * MLP_SD);
-            float s0 = 0.f, s1 = 0.f;
+            const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(delta + o * MLP_SD);
+            f2 s0 = mlp_pk(0.f, 0.f), s1 = s0;
 #pragma unroll
             for (int q = 0; q < MLP_TB / 4; ++q) {
-                const float4 d = row[q];
-                s0 = fmaf(d.x, a[4 * q], s0); s1 = fmaf(d.y, a[4 * q + 1], s1);
-                s0 = fmaf(d.z, a[4 * q + 2], s0); s1 = fmaf(d.w, a[4 * q + 3], s1);
+                const ulonglong2 d = row[q];
+                s0 = mlp_fma2(d.x, a[2 * q], s0);
+                s1 = mlp_fma2(d.y, a[2 * q + 1], s1);
             }
-            atomicAdd(gW + o * fan_in + t, s0 + s1);
+            atomicAdd(gW + o * fan_in + t, mlp_sum2(s0) + mlp_sum2(s1));
         }
     }
     if (part == 0 && t < nout) {
@@ -168,20 +174,24 @@ __device__ __forceinline__ void mlp_grad_weights(const float *act, const float *
 // part; in place (din = dout): every part reads the whole column first, the block synchronises, then writes.
 __device__ __forceinline__ void mlp_back_layer(const float *__restrict__ W, float *dl, const float *ain, int node, int part)
 {
-    float acc[MLP_PW];
+    f2 acc2[MLP_PW / 2];
 #pragma unroll
-    for (int i = 0; i < MLP_PW; ++i) acc[i] = 0.f;
+    for (int i = 0; i < MLP_PW / 2; ++i) acc2[i] = mlp_pk(0.f, 0.f);
 #pragma unroll 4
     for (int o = 0; o < MLP_W; ++o) {
         const float d = dl[o * MLP_SD + node];
-        const float4 *row = reinterpret_cast<const float4 *>(W + o * MLP_W + part * MLP_PW);
+        const f2 dd = mlp_pk(d, d);
+        const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(W + o * MLP_W + part * MLP_PW);
 #pragma unroll
         for (int q = 0; q < MLP_PW / 4; ++q) {
-            const float4 w = row[q];
-            acc[4 * q] = fmaf(w.x, d, acc[4 * q]); acc[4 * q + 1] = fmaf(w.y, d, acc[4 * q + 1]);
-            acc[4 * q + 2] = fmaf(w.z, d, acc[4 * q + 2]); acc[4 * q + 3] = fmaf(w.w, d, acc[4 * q + 3]);
+            const ulonglong2 w = row[q];
+            acc2[2 * q] = mlp_fma2(w.x, dd, acc2[2 * q]);
+            acc2[2 * q + 1] = mlp_fma2(w.y, dd, acc2[2 * q + 1]);
         }
     }
+    float acc[MLP_PW];
+#pragma unroll
+    for (int i = 0; i < MLP_PW / 2; ++i) asm("mov.b64 {%0, %1}, %2;" : "=f"(acc[2 * i]), "=f"(acc[2 * i + 1]) : "l"(acc2[i]));
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < MLP_PW; ++i) {
