@@ -122,9 +122,15 @@ def cpu_baseline(scene, budget_s=12.0):
         tot_t += dt
         tot_n += n
         passes += 1
-    return {"value": tot_n / tot_t, "unit": UNIT, "cores": po.num_threads(), "kind": "oracle",
+    cores = po.num_threads()
+    # the same oracle on ONE thread (every 16th ray): the per-core figure SURVEY.md section 8(d) asks for
+    po.set_num_threads(1)
+    dt1, n1 = oracle_sample_step(scene, 16)
+    po.set_num_threads(cores)
+    return {"value": tot_n / tot_t, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{scene.name}: {passes} passes over every {stride}nd ray ({tot_n:.3g} samples), fp64 forward + adjoint, "
-                      f"{tot_t:.1f} s wall"}
+                      f"{tot_t:.1f} s wall",
+            "value_1thread": n1 / dt1}
 
 
 def run_reference(args):

@@ -57,6 +57,8 @@ def lib():
         _lib.orc_source_unit.argtypes = [C.POINTER(_Line), C.POINTER(_Geom)]
         _lib.orc_source_unit.restype = C.c_double
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_set_num_threads.argtypes = [C.c_int]
+        _lib.orc_set_num_threads.restype = None
     return _lib
 
 
@@ -175,7 +177,8 @@ def num_threads() -> int:
 
 
 def set_num_threads(n: int):
-    os.environ["OMP_NUM_THREADS"] = str(n)
+    """Threads for the following oracle calls (timing only)."""
+    lib().orc_set_num_threads(int(n))
 
 
 def chi2_loss_grad(cube, target, sigma: float):

@@ -73,6 +73,16 @@ int orc_num_threads(void)
 #endif
 }
 
+/* Threads the ray loops may use from now on (timing only: the arithmetic of a ray does not depend on it). */
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 /* O2 orientation: sky (X right, Y up, zeta to the observer, s = -zeta) -> disk frame.
  * Geometry parameters: Table 2 (inclination, position angle, azimuth). */
 static void orc_make_orient(const orc_geom *g, orc_orient *o)

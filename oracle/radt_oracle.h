@@ -88,6 +88,7 @@ int orc_trace_ray(const orc_geom *geom, const orc_line *line, const orc_grid *gr
 double orc_partition(const orc_line *line, double T);
 double orc_source_unit(const orc_line *line, const orc_geom *geom);   /* S0 / intensity unit */
 int orc_num_threads(void);
+void orc_set_num_threads(int n);
 
 #ifdef __cplusplus
 }
