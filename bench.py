@@ -300,7 +300,7 @@ def run_ours(args):
     mufu_peak, mufu_clk = B.radt_pipe_peak(0)
     ffma_peak, _ = B.radt_pipe_peak(1)
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.txt")      # one JSON object: DRAM bytes per launch from the ncu capture
     if os.path.exists(tpath):
         try:
             traffic = json.load(open(tpath))
