@@ -171,8 +171,9 @@ int radt_render_loss(const radt_geom *geom, const radt_line *line, const radt_gr
                      size_t ws_bytes, void *cuda_stream);
 
 /* Same operations with HOST buffers (grid->dens/temp/vel, cube, dl_dcube, g_* are HOST pointers).
- * Device memory is allocated stream-ordered on stream 0 of the current device; the call returns
- * after the results are in host memory. */
+ * Device memory comes from an arena the library keeps per calling thread and device (grown on demand, never
+ * returned); the work runs on stream 0 of the current device and the call returns after the results are in host
+ * memory. */
 int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                      float *cube);
 /* Forward + L2 loss against `target` (HOST; uploaded on a second stream under the forward march) + adjoint in one

@@ -470,20 +470,43 @@ int radt_read_counters(const void *ws, uint64_t *out4, void *cuda_stream)
 // HOST-buffer entry points: stream-ordered allocation, H2D, same kernels, D2H, synchronise.
 // ------------------------------------------------------------------------------------------
 namespace {
+// Device memory of the HOST-buffer entry points: one arena per thread and device, grown when a call needs more and kept
+// between calls (a fit loop calls with the same sizes; per-call cudaMallocAsync / cudaFreeAsync of nine buffers made the
+// call time vary by 0.7 ms from process to process).  Every call ends with a stream synchronisation, so the arena
+// is idle when the next call starts.
+struct DevArena {
+    char *base = nullptr;
+    size_t cap = 0;
+    int dev = -1;
+};
+thread_local DevArena g_arena;
+
 struct DevBufs {
     cudaStream_t st = 0;
-    void *ptrs[16];
-    int n = 0;
+    size_t used = 0;
+    bool reserve(size_t bytes)
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return false;
+        if (g_arena.dev == dev && g_arena.cap >= bytes) return true;
+        if (g_arena.base) {
+            cudaSetDevice(g_arena.dev);
+            cudaFree(g_arena.base);
+            cudaSetDevice(dev);
+        }
+        g_arena = DevArena();
+        void *p = nullptr;
+        if (cudaMalloc(&p, bytes) != cudaSuccess) return false;
+        g_arena.base = (char *)p; g_arena.cap = bytes; g_arena.dev = dev;
+        return true;
+    }
     void *alloc(size_t bytes)
     {
-        void *p = nullptr;
-        if (cudaMallocAsync(&p, bytes ? bytes : 16, st) != cudaSuccess) return nullptr;
-        ptrs[n++] = p;
+        const size_t a = align256(bytes ? bytes : 16);
+        if (used + a > g_arena.cap) return nullptr;
+        void *p = g_arena.base + used;
+        used += a;
         return p;
-    }
-    ~DevBufs()
-    {
-        for (int i = 0; i < n; ++i) cudaFreeAsync(ptrs[i], st);
     }
 };
 }  // namespace
@@ -499,25 +522,15 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     if (!grid->dens || !grid->temp || !grid->vel) return fail(RADT_E_INVALID, "null field pointer");
     int count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || count < 1) return fail(RADT_E_CUDA, "no CUDA device");
-    {
-        // keep freed blocks in the stream-ordered pool across calls: by default the pool hands its memory back to the
-        // driver at every synchronisation and each call would pay for fresh cudaMalloc's
-        static thread_local int pool_dev = -1;
-        int dev = 0;
-        CUDA_TRY(cudaGetDevice(&dev));
-        if (pool_dev != dev) {
-            cudaMemPool_t pool;
-            CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, dev));
-            unsigned long long keep = ~0ull;
-            CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-            pool_dev = dev;
-        }
-    }
     DevBufs B;
     long long cells = grid_cells(grid);
     long long stride = batch > 1 ? grid->batch_stride : cells;
     size_t fbytes = (size_t)((batch - 1) * stride + cells) * sizeof(float);
     size_t nvox = (size_t)batch * geom[0].nx * geom[0].ny * line->nchan;
+    CUDA_TRY(cudaStreamSynchronize(B.st));       // an earlier call that failed half-way may still own the arena
+    const size_t wsb_need = ws_layout(geom, grid, batch, mode == 0 ? RADT_PASS_FWD : RADT_PASS_BWD).total;
+    if (!B.reserve(6 * align256(fbytes) + 3 * align256(nvox * sizeof(float)) + align256(wsb_need) + 4096))
+        return fail(RADT_E_CUDA, "device allocation failed");
     float *d_dens = (float *)B.alloc(fbytes), *d_temp = (float *)B.alloc(fbytes), *d_vel = (float *)B.alloc(fbytes);
     float *d_cube = (float *)B.alloc(nvox * sizeof(float));
     if (!d_dens || !d_temp || !d_vel || !d_cube) return fail(RADT_E_CUDA, "device allocation failed");
