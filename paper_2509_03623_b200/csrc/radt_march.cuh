@@ -38,8 +38,12 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     const DevLine &L = P.line;
     st.inside = false;
     st.K2 = 0.f; st.A = 0.f; st.vh = 0.f; st.mvlA = 0.f; st.S = 0.f;
-    double s = s0 + ((double)k + 0.5) * ds;
-    double x = fma(s, G.wx, ox), y = fma(s, G.wy, oy), z = fma(s, G.wz, oz);
+    // Sample position with every product and sum rounded separately (no FMA contraction): the in/out decisions and
+    // the r = 0 rule are exact comparisons, and they agree with a plain fp64 evaluation of O4 only if the
+    // position carries the same roundings (a ray through the star whose midpoint falls on it gave s = 1e-14 with
+    // an FMA and s = 0, a skipped step, without: randomised parity scenes 5, 20, 21).
+    const double s = __dadd_rn(s0, __dmul_rn((double)k + 0.5, ds));
+    const double x = __dadd_rn(ox, __dmul_rn(s, G.wx)), y = __dadd_rn(oy, __dmul_rn(s, G.wy)), z = __dadd_rn(oz, __dmul_rn(s, G.wz));
     double r2 = x * x + y * y;
     float r2f = (float)r2;
     // fp64 1/r by one Newton step on the SFU seed

@@ -466,3 +466,44 @@ def test_fit_step_is_cuda_graph_capturable(rt):
     assert float(R.loss.cpu()) == pytest.approx(float(want[2].cpu()), rel=1e-12)
     for got, ref, nm in zip((R.g_dens, R.g_temp, R.g_vel), want[3:], ("dens", "temp", "vel")):
         check_grad(f"graph replay g_{nm}", got.cpu().numpy()[0], ref.cpu().numpy()[0].astype(np.float64))
+
+
+# ------------------------------------------------------------------ randomised scenes
+def _random_scene(seed):
+    """A seeded random small scene: grid kind, sizes, viewing angles, channel count / spacing / offset, density and
+    velocity modes, zeroed density patches (zero-opacity runs) and image shapes that leave warps without rays."""
+    rng = np.random.default_rng(9000 + seed)
+    kind = int(rng.integers(0, 3))
+    nchan = int(rng.choice([1, 2, 7, 31, 32, 33, 64, 100, 150, 256]))
+    common = dict(seed=int(rng.integers(1, 10 ** 6)), nchan=nchan, nstep=int(rng.integers(5, 70)),
+                  incl_deg=float(rng.uniform(0, 90)), pa_deg=float(rng.uniform(-180, 180)), az_deg=float(rng.uniform(0, 360)),
+                  dens_ln=bool(rng.integers(0, 2)), kepler_frac=bool(rng.integers(0, 2)), vsys=float(rng.uniform(-1e5, 1e5)))
+    if kind == 0:
+        sc = tiny_axisym_scene(nr=int(rng.integers(3, 20)), nz=int(rng.integers(3, 16)), npix=int(rng.integers(3, 11)),
+                               npix_y=int(rng.integers(1, 9)), mirror=bool(rng.integers(0, 2)),
+                               vturb_mach=float(rng.choice([0.0, 0.3])), **common)
+    elif kind == 1:
+        sc = tiny_cart_scene(ng=tuple(int(v) for v in rng.integers(3, 12, 3)), npix=int(rng.integers(3, 10)), **common)
+    else:
+        sc = tiny_sph_scene(ng=(int(rng.integers(3, 12)), int(rng.integers(3, 10)), int(rng.integers(3, 40))),
+                            npix=int(rng.integers(3, 10)), **common)
+    # channel lattice: random spacing from a fifth of the thermal width to several widths, random offset
+    if nchan > 1:
+        dv = float(rng.choice([0.02, 0.1, 0.4, 1.5])) * 1e5
+        v = (np.arange(nchan) - rng.uniform(0, nchan)) * dv * float(rng.choice([1.0, -1.0]))
+        sc = replace(sc, line=replace(sc.line, vchan=v))
+    # zero the density in a random patch (LINEAR grids only: zero-opacity steps in the adjoint)
+    if not common["dens_ln"] and rng.integers(0, 2):
+        d = np.array(sc.grid.dens)
+        sl = tuple(slice(int(a), int(a) + max(1, n // 2)) for a, n in ((rng.integers(0, n), n) for n in d.shape))
+        d[sl] = 0.0
+        sc = sc.with_fields(dens=d)
+    return sc
+
+
+import os  # noqa: E402
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_SCENES", "24"))))
+def test_random_scenes(rt, seed):
+    _parity_fwd_bwd(rt, _random_scene(seed), f"random scene {seed}", seed=seed)
