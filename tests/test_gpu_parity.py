@@ -492,6 +492,9 @@ def _random_scene(seed):
         dv = float(rng.choice([0.02, 0.1, 0.4, 1.5])) * 1e5
         v = (np.arange(nchan) - rng.uniform(0, nchan)) * dv * float(rng.choice([1.0, -1.0]))
         sc = replace(sc, line=replace(sc.line, vchan=v))
+    else:
+        # one channel: keep it on the line (a channel 12 line widths away renders 1e-68, beyond fp32 on either side)
+        sc = replace(sc, line=replace(sc.line, vchan=np.array([common["vsys"] + 0.2e5])))
     # zero the density in a random patch (LINEAR grids only: zero-opacity steps in the adjoint)
     if not common["dens_ln"] and rng.integers(0, 2):
         d = np.array(sc.grid.dens)
@@ -507,3 +510,26 @@ import os  # noqa: E402
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_SCENES", "24"))))
 def test_random_scenes(rt, seed):
     _parity_fwd_bwd(rt, _random_scene(seed), f"random scene {seed}", seed=seed)
+
+
+def test_optically_thick_central_ray_gradient_bound(rt):
+    """Known limit of the front-to-back adjoint: R_k = I_saved - P_k carries the rounding of the
+    forward's own fp32 sum (~1e-7 I).  On a ray that is optically thick in EVERY channel from its first steps
+    (random scene 228: edge-on ray through the star, 33 channels inside the line core, tau ~ 0.25 per step) all gradient
+    terms sit where T S - R cancels to ~1e-2 of its parts, and the density gradient is good to 7e-4 of its maximum
+    instead of the usual 1e-6: inside BASELINE.json's 1e-3 in the max and L2 norms, outside the element-wise
+    criterion with the 1e-5 floor.  The test pins that behaviour."""
+    sc = _random_scene(228)
+    scenes = [sc]
+    ref = _oracle_cube(scenes)
+    R = _gpu_forward(rt, scenes, need_bwd=True)
+    check_cube("thick central ray cube", R.cube.cpu().numpy(), ref)
+    tgt, sigma = l2_target(ref[0], 1000 + 228)
+    G32 = ((ref[0] - tgt) / (sigma ** 2 * ref[0].size)).astype(np.float32)[None]
+    R.dl_dcube.copy_(torch.from_numpy(G32))
+    got = [g.cpu().numpy()[0].astype(np.float64) for g in R.render_bwd()]
+    want = po.render_bwd(sc, G32[0].astype(np.float64))
+    for nm, a, b in zip(("dens", "temp"), got, want):          # (v_los vanishes on this ray: dL/dv = 1e-25)
+        m = np.abs(b).max()
+        assert np.abs(a - b).max() <= 1e-3 * m and np.linalg.norm(a - b) <= 1e-3 * np.linalg.norm(b), nm
+    check_grad("thick central ray g_temp", got[1], want[1])
