@@ -1,6 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on the same
 seeded inputs.  Tolerances: tests/tolerances.py (cube 1e-4, gradients 1e-3; BASELINE.json north_star)."""
 import math
+import os
 from dataclasses import replace
 
 import numpy as np
@@ -27,8 +28,13 @@ def rt(request):
     B = pkg.binding
     B.lib()     # fails loudly if the CUDA library was not built
     B.radt_set_option(B.OPT_WIN_PATH, 1 if request.param == "win" else 0)
+    dense = os.environ.get("RADT_TEST_DENSE") == "1"       # one-off runs of the whole file without windowing / skipping
+    if dense:
+        B.radt_set_option(B.OPT_WINDOW, 0); B.radt_set_option(B.OPT_SKIP_EMPTY, 0)
     yield pkg
     B.radt_set_option(B.OPT_WIN_PATH, 1)
+    if dense:
+        B.radt_set_option(B.OPT_WINDOW, 1); B.radt_set_option(B.OPT_SKIP_EMPTY, 1)
 
 
 def _as_list(s):
@@ -502,9 +508,6 @@ def _random_scene(seed):
         d[sl] = 0.0
         sc = sc.with_fields(dens=d)
     return sc
-
-
-import os  # noqa: E402
 
 
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_SCENES", "24"))))
