@@ -92,6 +92,46 @@ __device__ __forceinline__ void mlp_layer(const float *__restrict__ W, const flo
     }
 }
 
+// M3, hidden layer 64 -> 64 for TWO nodes per thread and 8 of the 64 output units (part = 0..7): every broadcast weight
+// load feeds both nodes (the one-node version is bound by shared-memory wavefronts: 16 LDS.128 per 32 FFMA2), inputs
+// in two chunks of 32 so that the 16 accumulator pairs and the inputs of both nodes fit the register file.
+#define MLP_P8 8
+__device__ __forceinline__ void mlp_layer2(const float *__restrict__ W, const float *__restrict__ b, const float *in,
+                                           float *out, int stride, int n0, int n1, int part)
+{
+    const int o0 = part * MLP_P8;
+    f2 acc0[MLP_P8], acc1[MLP_P8];
+#pragma unroll
+    for (int o = 0; o < MLP_P8; ++o) { acc0[o] = mlp_pk(b[o0 + o], 0.f); acc1[o] = acc0[o]; }
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        f2 h0[16], h1[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const float *p = in + (32 * c + 2 * i) * stride;
+            h0[i] = mlp_pk(p[n0], p[stride + n0]);
+            h1[i] = mlp_pk(p[n1], p[stride + n1]);
+        }
+#pragma unroll
+        for (int o = 0; o < MLP_P8; ++o) {
+            const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(W + (o0 + o) * MLP_W + 32 * c);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const ulonglong2 w = row[q];
+                acc0[o] = mlp_fma2(w.x, h0[2 * q], acc0[o]);
+                acc1[o] = mlp_fma2(w.x, h1[2 * q], acc1[o]);
+                acc0[o] = mlp_fma2(w.y, h0[2 * q + 1], acc0[o]);
+                acc1[o] = mlp_fma2(w.y, h1[2 * q + 1], acc1[o]);
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 0; o < MLP_P8; ++o) {
+        out[(o0 + o) * stride + n0] = fmaxf(mlp_sum2(acc0[o]), 0.f);
+        out[(o0 + o) * stride + n1] = fmaxf(mlp_sum2(acc1[o]), 0.f);
+    }
+}
+
 // output unit and M4; returns the sigmoid
 __device__ __forceinline__ float mlp_head(const float *__restrict__ w5, float b5, const float *in, int stride, int node)
 {
@@ -112,26 +152,31 @@ __device__ __forceinline__ void mlp_stage(float *dst, const float *__restrict__ 
     for (int q = (count & ~3) + threadIdx.x; q < count; q += nthreads) dst[q] = __ldg(src + q);
 }
 
-__global__ void __launch_bounds__(MLP_TF * MLP_S) k_mlp_fwd(const __grid_constant__ MlpParamsDev Q)
+__global__ void __launch_bounds__(MLP_TF / 2 * MLP_P8) k_mlp_fwd(const __grid_constant__ MlpParamsDev Q)
 {
-    const int node = threadIdx.x & (MLP_TF - 1), part = threadIdx.x / MLP_TF;     // part is warp uniform
-    const int q = blockIdx.x * MLP_TF + node, n = Q.nr * Q.nz;
-    const int qq = min(q, n - 1), i = qq / Q.nz, j = qq - i * Q.nz;
+    // 64 node pairs x 8 parts: thread (pair, part) serves nodes pair and pair + 64 and output units 8 part .. 8 part + 7
+    const int pair = threadIdx.x & (MLP_TF / 2 - 1), part = threadIdx.x / (MLP_TF / 2);     // part is warp uniform
+    const int n0 = pair, n1 = pair + MLP_TF / 2, n = Q.nr * Q.nz;
     const MlpOff F = mlp_offsets(Q.L);
     float *A = mlp_smem, *B = mlp_smem + MLP_W * MLP_TF;           // ping-pong [unit][node]
     float *sP = B + MLP_W * MLP_TF;                                // all parameters (a uniform global load per weight
-    mlp_stage(sP, Q.params, F.b[MLP_H] + 1, MLP_TF * MLP_S);       // left the kernel waiting on L1/L2: 17 stall cycles per issue)
-    if (part == 0) mlp_encode(Q, i, j, A, MLP_TF, node);
+    mlp_stage(sP, Q.params, F.b[MLP_H] + 1, MLP_TF / 2 * MLP_P8);  // left the kernel waiting on L1/L2: 17 stall cycles per issue)
+    if (part < 2) {
+        const int node = part == 0 ? n0 : n1, qq = min(blockIdx.x * MLP_TF + node, n - 1);
+        mlp_encode(Q, qq / Q.nz, qq % Q.nz, A, MLP_TF, node);
+    }
     __syncthreads();
-    mlp_layer_first(sP + F.W[0], sP + F.b[0], F.D, A, B, MLP_TF, node, part);
+    // first layer: 4 parts x 16 units for each of the two nodes (parts 0-3: n0, parts 4-7: n1)
+    mlp_layer_first(sP + F.W[0], sP + F.b[0], F.D, A, B, MLP_TF, part < 4 ? n0 : n1, part & 3);
     __syncthreads();
-    mlp_layer(sP + F.W[1], sP + F.b[1], B, A, MLP_TF, node, part);
+    mlp_layer2(sP + F.W[1], sP + F.b[1], B, A, MLP_TF, n0, n1, part);
     __syncthreads();
-    mlp_layer(sP + F.W[2], sP + F.b[2], A, B, MLP_TF, node, part);
+    mlp_layer2(sP + F.W[2], sP + F.b[2], A, B, MLP_TF, n0, n1, part);
     __syncthreads();
-    mlp_layer(sP + F.W[3], sP + F.b[3], B, A, MLP_TF, node, part);
+    mlp_layer2(sP + F.W[3], sP + F.b[3], B, A, MLP_TF, n0, n1, part);
     __syncthreads();
-    if (part != 0) return;
+    if (part >= 2) return;
+    const int node = part == 0 ? n0 : n1, q = blockIdx.x * MLP_TF + node;
     const float s = mlp_head(sP + F.W[4], sP[F.b[4]], A, MLP_TF, node);
     if (q < n) Q.temp_out[q] = fmaf(Q.t_hi - Q.t_lo, s, Q.t_lo);
 }
@@ -277,7 +322,7 @@ cudaError_t radt_launch_mlp_fwd(const MlpParamsDev &Q, cudaStream_t st)
     cudaError_t e = cudaFuncSetAttribute(k_mlp_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int n = Q.nr * Q.nz;
-    k_mlp_fwd<<<(n + MLP_TF - 1) / MLP_TF, MLP_TF * MLP_S, smem, st>>>(Q);
+    k_mlp_fwd<<<(n + MLP_TF - 1) / MLP_TF, MLP_TF / 2 * MLP_P8, smem, st>>>(Q);
     return cudaGetLastError();
 }
 
