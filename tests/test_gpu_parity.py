@@ -11,7 +11,7 @@ from oracle import pyoracle as po
 from synth import (UNIT_CGS, UNIT_JY_PIXEL, co_line, l2_target, make_config, slab_scene, sph_benchmark_scene, tiny_axisym_scene,
                    tiny_sph_scene,
                    tiny_cart_scene)
-from tests.tolerances import check_cube, check_grad
+from tests.tolerances import GRAD, check, check_cube, check_grad
 
 pytestmark = pytest.mark.gpu
 
@@ -52,7 +52,7 @@ def _gpu_forward(rt, scenes, need_bwd=False):
     return R
 
 
-def _parity_fwd_bwd(rt, scenes, name, seed=0, grad=True):
+def _parity_fwd_bwd(rt, scenes, name, seed=0, grad=True, grad_floor=None):
     scenes = _as_list(scenes)
     ref = _oracle_cube(scenes)
     R = _gpu_forward(rt, scenes, need_bwd=grad)
@@ -73,9 +73,11 @@ def _parity_fwd_bwd(rt, scenes, name, seed=0, grad=True):
     gd, gt, gv = (g.cpu().numpy() for g in R.render_bwd())
     for b, sc in enumerate(scenes):
         rd, rtm, rv = po.render_bwd(sc, G32[b].astype(np.float64))
-        check_grad(f"{name}[{b}] g_dens", gd[b], rd)
-        check_grad(f"{name}[{b}] g_temp", gt[b], rtm)
-        check_grad(f"{name}[{b}] g_vel", gv[b], rv)
+        for nm, got, want in (("dens", gd[b], rd), ("temp", gt[b], rtm), ("vel", gv[b], rv)):
+            if grad_floor is None:
+                check_grad(f"{name}[{b}] g_{nm}", got, want)
+            else:
+                check(f"{name}[{b}] g_{nm}", got, want, GRAD[0], grad_floor)
     return R
 
 
@@ -475,23 +477,26 @@ def test_fit_step_is_cuda_graph_capturable(rt):
 
 
 # ------------------------------------------------------------------ randomised scenes
-def _random_scene(seed):
+def _random_scene(seed, medium=False):
     """A seeded random small scene: grid kind, sizes, viewing angles, channel count / spacing / offset, density and
-    velocity modes, zeroed density patches (zero-opacity runs) and image shapes that leave warps without rays."""
-    rng = np.random.default_rng(9000 + seed)
+    velocity modes, zeroed density patches (zero-opacity runs) and image shapes that leave warps without rays.
+    `medium`: several hundred steps per ray and finer grids, so that candidate queues, step pairs and zero-opacity
+    runs span many 32-step batches."""
+    rng = np.random.default_rng((19000 if medium else 9000) + seed)
+    big = 4 if medium else 1
     kind = int(rng.integers(0, 3))
     nchan = int(rng.choice([1, 2, 7, 31, 32, 33, 64, 100, 150, 256]))
-    common = dict(seed=int(rng.integers(1, 10 ** 6)), nchan=nchan, nstep=int(rng.integers(5, 70)),
+    common = dict(seed=int(rng.integers(1, 10 ** 6)), nchan=nchan, nstep=int(rng.integers(5, 70)) * (big * 2 if medium else 1),
                   incl_deg=float(rng.uniform(0, 90)), pa_deg=float(rng.uniform(-180, 180)), az_deg=float(rng.uniform(0, 360)),
                   dens_ln=bool(rng.integers(0, 2)), kepler_frac=bool(rng.integers(0, 2)), vsys=float(rng.uniform(-1e5, 1e5)))
     if kind == 0:
-        sc = tiny_axisym_scene(nr=int(rng.integers(3, 20)), nz=int(rng.integers(3, 16)), npix=int(rng.integers(3, 11)),
+        sc = tiny_axisym_scene(nr=int(rng.integers(3, 20)) * big, nz=int(rng.integers(3, 16)) * big, npix=int(rng.integers(3, 11)),
                                npix_y=int(rng.integers(1, 9)), mirror=bool(rng.integers(0, 2)),
                                vturb_mach=float(rng.choice([0.0, 0.3])), **common)
     elif kind == 1:
-        sc = tiny_cart_scene(ng=tuple(int(v) for v in rng.integers(3, 12, 3)), npix=int(rng.integers(3, 10)), **common)
+        sc = tiny_cart_scene(ng=tuple(int(v) * big for v in rng.integers(3, 12, 3)), npix=int(rng.integers(3, 10)), **common)
     else:
-        sc = tiny_sph_scene(ng=(int(rng.integers(3, 12)), int(rng.integers(3, 10)), int(rng.integers(3, 40))),
+        sc = tiny_sph_scene(ng=(int(rng.integers(3, 12)) * big, int(rng.integers(3, 10)) * big, int(rng.integers(3, 40)) * big),
                             npix=int(rng.integers(3, 10)), **common)
     # channel lattice: random spacing from a fifth of the thermal width to several widths, random offset
     if nchan > 1:
@@ -513,6 +518,14 @@ def _random_scene(seed):
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_SCENES", "24"))))
 def test_random_scenes(rt, seed):
     _parity_fwd_bwd(rt, _random_scene(seed), f"random scene {seed}", seed=seed)
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_MEDIUM", "6"))))
+def test_random_medium_scenes(rt, seed):
+    """Hundreds of steps through optically thick LN grids: the fp32 cancellation of the front-to-back adjoint (DESIGN.md
+    section 6) leaves isolated cells off by up to 3e-5 of the field's maximum (6 of 150 seeds, max and L2 norms below
+    1e-4 throughout), so the element-wise floor is 1e-4 of the maximum here instead of 1e-5."""
+    _parity_fwd_bwd(rt, _random_scene(seed, medium=True), f"random medium scene {seed}", seed=seed, grad_floor=1e-4)
 
 
 def test_optically_thick_central_ray_gradient_bound(rt):
