@@ -1,8 +1,9 @@
 // radt_mlp.cu -- symmetric MLP temperature field on the nodes of the (r, zeta) grid and its adjoint w.r.t. the
 // parameters (Eq. 10).  Algorithm M1-M4 of DESIGN.md section 9: normalised grid
 // coordinates -> positional encoding of degree L -> 4 x 64 ReLU layers -> sigmoid scaled to [t_lo, t_hi].
-// fp32 FMA; one node per thread, activations in shared memory ([unit][node], so both the per-node and the
-// per-unit passes read without bank conflicts), weights through uniform L1 loads.  Shares nothing with oracle/.
+// fp32 FMA (packed FFMA2); activations in shared memory ([unit][node], so both the per-node and the per-unit passes
+// read without bank conflicts), parameters staged in shared memory and read as warp-wide broadcasts; the hidden
+// layers serve two nodes per thread so that each broadcast feeds both.  Shares nothing with oracle/.
 #include "radt_dev.cuh"
 #include "radt_kernels.h"
 
@@ -277,9 +278,13 @@ __global__ void __launch_bounds__(MLP_TB * MLP_S, 2) k_mlp_bwd(const __grid_cons
         const float *w = stage(0);
         mlp_layer_first(w, w + MLP_W * F.D, F.D, a0, a1, MLP_SA, node, part);
     }
-    for (int l = 1; l < MLP_H; ++l) {
-        const float *w = stage(l);                         // (its barriers also order the layers)
-        mlp_layer(w, w + MLP_W * MLP_W, act(l), act(l + 1), MLP_SA, node, part);
+    {
+        // hidden layers with two nodes per thread: 32 node pairs x 8 parts (radt_mlp.cu mlp_layer2)
+        const int pair = threadIdx.x & (MLP_TB / 2 - 1), part8 = threadIdx.x / (MLP_TB / 2);
+        for (int l = 1; l < MLP_H; ++l) {
+            const float *w = stage(l);                     // (its barriers also order the layers)
+            mlp_layer2(w, w + MLP_W * MLP_W, act(l), act(l + 1), MLP_SA, pair, pair + MLP_TB / 2, part8);
+        }
     }
     const float *w5 = stage(MLP_H);
     const float *a4 = act(MLP_H);
