@@ -120,6 +120,13 @@ const char *radt_last_error(void);
 enum {
     RADT_OPT_WINDOW = 1,          /* 1 (default): skip channel groups outside the +-6.4 alpha line window; 0: dense */
     RADT_OPT_SKIP_EMPTY = 2,      /* 1 (default): skip steps with zero opacity in the forward march; 0: dense */
+    RADT_OPT_COMPENSATED = 4,     /* 0 (default) / 1: the forward also keeps, per voxel, the low-order word of its fp32 sum in
+                                     the workspace (8 bytes per voxel more: query radt_workspace_bytes under the same
+                                     setting) and the adjoint, given THE SAME workspace, uses it to form the residual
+                                     intensity without cancellation noise: gradients on rays that are optically thick
+                                     in every channel improve from ~1e-3 to ~1e-6 of the maximum.
+                                     A different or overwritten workspace falls back to the plain difference, voxel by
+                                     voxel.  Window kernels only. */
     RADT_OPT_WIN_PATH = 3         /* 1 (default): channel tables that are uniform lattices v_0 + c dv use the window
                                      kernels (one channel per lane inside the line window); 0: always the
                                      channel-table kernels.  radt_render and radt_render_bwd of one cube must run

@@ -16,6 +16,7 @@ thread_local int g_launches = 0;
 int g_opt_window = 1;
 int g_opt_skip_empty = 1;
 int g_opt_win_path = 1;
+int g_opt_compensated = 0;
 
 int fail(int code, const char *fmt, ...)
 {
@@ -200,11 +201,11 @@ void make_dev_line(const radt_line *line, DevLine &d)
 }
 
 struct WsLayout {
-    size_t rays, qtab, vcs, rnode, cells, occ, grad, counters, total;
+    size_t rays, qtab, vcs, rnode, cells, occ, ilo, grad, counters, total;
     int occ_wpr, occ_words, occ_nbj;
 };
 
-WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass)
+WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass, int nchan = 0)
 {
     WsLayout w;
     size_t off = 0;
@@ -230,6 +231,9 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
         w.occ_words = nbi * nbj * w.occ_wpr;
     }
     w.occ = off; off = align256(off + (size_t)w.occ_words * (size_t)batch * sizeof(unsigned));
+    // {I, low-order word} per voxel, shared by the forward and the adjoint of a cube (RADT_OPT_COMPENSATED)
+    w.ilo = off;
+    if (g_opt_compensated && nchan > 0) off = align256(off + nrays * (size_t)nchan * sizeof(float2));
     w.grad = off;
     if (pass == RADT_PASS_BWD) off = align256(off + cells * sizeof(float4));
     w.total = off;
@@ -248,6 +252,7 @@ DevWs make_dev_ws(void *ws, const WsLayout &w)
     d.cells = (float4 *)(base + w.cells);
     d.occ = (unsigned *)(base + w.occ);
     d.grad = (float4 *)(base + w.grad);
+    d.ilo = w.grad > w.ilo ? (float2 *)(base + w.ilo) : nullptr;
     return d;
 }
 
@@ -271,7 +276,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
     if (!grid->dens || !grid->temp || !grid->vel) return fail(RADT_E_INVALID, "null field pointer");
     if (!cube) return fail(RADT_E_INVALID, "null cube pointer");
     if (pass == RADT_PASS_BWD && !dl_dcube) return fail(RADT_E_INVALID, "null dl_dcube pointer");
-    WsLayout w = ws_layout(geom, grid, batch, pass);
+    WsLayout w = ws_layout(geom, grid, batch, pass, line->nchan);
     if (ws_bytes < w.total) return fail(RADT_E_WORKSPACE, "workspace too small: need %zu bytes, got %zu", w.total, ws_bytes);
     if (((uintptr_t)ws & 15) != 0) return fail(RADT_E_INVALID, "workspace must be 16-byte aligned");
     long long stride = batch > 1 ? grid->batch_stride : grid_cells(grid);
@@ -322,6 +327,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         memset(&MP, 0, sizeof(MP));
         memcpy(MP.geom, SP.geom, sizeof(MP.geom));
         MP.grid = dg; MP.ws = dws;
+        if (!use_win) MP.ws.ilo = nullptr;            // only the window kernels carry the low-order words
         make_dev_line(line, MP.line);
         MP.nx = SP.nx; MP.ny = SP.ny; MP.nstep = SP.nstep;
         MP.tiles_x = (MP.nx + RADT_TILE_X - 1) / RADT_TILE_X;
@@ -374,6 +380,7 @@ int radt_set_option(int key, int value)
     if (key == RADT_OPT_WINDOW) { g_opt_window = value != 0; return RADT_OK; }
     if (key == RADT_OPT_SKIP_EMPTY) { g_opt_skip_empty = value != 0; return RADT_OK; }
     if (key == RADT_OPT_WIN_PATH) { g_opt_win_path = value != 0; return RADT_OK; }
+    if (key == RADT_OPT_COMPENSATED) { g_opt_compensated = value != 0; return RADT_OK; }
     return fail(RADT_E_INVALID, "unknown option %d", key);
 }
 
@@ -382,6 +389,7 @@ int radt_get_option(int key)
     if (key == RADT_OPT_WINDOW) return g_opt_window;
     if (key == RADT_OPT_SKIP_EMPTY) return g_opt_skip_empty;
     if (key == RADT_OPT_WIN_PATH) return g_opt_win_path;
+    if (key == RADT_OPT_COMPENSATED) return g_opt_compensated;
     return fail(RADT_E_INVALID, "unknown option %d", key);
 }
 
@@ -392,7 +400,7 @@ int radt_workspace_bytes(const radt_geom *geom, const radt_line *line, const rad
     int rc = validate(geom, line, grid, batch);
     if (rc) return rc;
     if (pass != RADT_PASS_FWD && pass != RADT_PASS_BWD) return fail(RADT_E_INVALID, "unknown pass");
-    *bytes_out = ws_layout(geom, grid, batch, pass).total;
+    *bytes_out = ws_layout(geom, grid, batch, pass, line ? line->nchan : 0).total;
     return RADT_OK;
 }
 
@@ -528,7 +536,7 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     size_t fbytes = (size_t)((batch - 1) * stride + cells) * sizeof(float);
     size_t nvox = (size_t)batch * geom[0].nx * geom[0].ny * line->nchan;
     CUDA_TRY(cudaStreamSynchronize(B.st));       // an earlier call that failed half-way may still own the arena
-    const size_t wsb_need = ws_layout(geom, grid, batch, mode == 0 ? RADT_PASS_FWD : RADT_PASS_BWD).total;
+    const size_t wsb_need = ws_layout(geom, grid, batch, mode == 0 ? RADT_PASS_FWD : RADT_PASS_BWD, line->nchan).total;
     if (!B.reserve(6 * align256(fbytes) + 3 * align256(nvox * sizeof(float)) + align256(wsb_need) + 4096))
         return fail(RADT_E_CUDA, "device allocation failed");
     float *d_dens = (float *)B.alloc(fbytes), *d_temp = (float *)B.alloc(fbytes), *d_vel = (float *)B.alloc(fbytes);
@@ -539,7 +547,7 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     CUDA_TRY(cudaMemcpyAsync(d_vel, grid->vel, fbytes, cudaMemcpyHostToDevice, B.st));
     radt_grid dgrid = *grid;
     dgrid.dens = d_dens; dgrid.temp = d_temp; dgrid.vel = d_vel;
-    size_t wsb = ws_layout(geom, grid, batch, mode == 0 ? RADT_PASS_FWD : RADT_PASS_BWD).total;
+    size_t wsb = wsb_need;
     void *ws = B.alloc(wsb);
     if (!ws) return fail(RADT_E_CUDA, "device allocation failed");
     int launches = 0;

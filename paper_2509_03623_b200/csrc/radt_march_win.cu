@@ -146,19 +146,28 @@ __device__ __forceinline__ int group_for(int ulo, int uhi) { return ulo - ((31 -
 // Per-lane channel state of the forward window march.  The (I, T) of all channels of the ray live in shared
 // memory (channel c is only ever touched by lane c & 31); the lane keeps the pair of the ONE channel it serves in
 // the current group [cur, cur + 32) in registers.
+// COMP (RADT_OPT_COMPENSATED): the rounding errors of the sum I += c are collected in a low-order word Ls, which the
+// adjoint uses to form R_k = I - I_{<=k} without the cancellation noise of the fp32 sum.
+template <bool COMP>
 struct LaneState {
-    float Is, Ts, cf;
+    float Is, Ts, cf, Ls;
     int cur, myc;
-    float *sI, *sT;
+    float *sI, *sT, *sL;
     __device__ __forceinline__ void init(float *sI_, float *sT_, int lane, int ng)
     {
-        sI = sI_; sT = sT_;
-        for (int g = 0; g < ng; ++g) { sI[lane + 32 * g] = 0.f; sT[lane + 32 * g] = 1.f; }
-        Is = 0.f; Ts = 1.f; cf = 0.f; cur = NO_GROUP; myc = -1;
+        sI = sI_; sT = sT_; sL = sT_ + 32 * ng;
+        for (int g = 0; g < ng; ++g) {
+            sI[lane + 32 * g] = 0.f; sT[lane + 32 * g] = 1.f;
+            if (COMP) sL[lane + 32 * g] = 0.f;
+        }
+        Is = 0.f; Ts = 1.f; cf = 0.f; Ls = 0.f; cur = NO_GROUP; myc = -1;
     }
     __device__ __forceinline__ void put_back()
     {
-        if (myc >= 0) { sI[myc] = Is; sT[myc] = Ts; }
+        if (myc >= 0) {
+            sI[myc] = Is; sT[myc] = Ts;
+            if (COMP) sL[myc] = Ls;
+        }
     }
     // the group moved: put the lane's channel state back, take the new channel's
     __device__ __forceinline__ void regroup(int clo, int lane, int nchan)
@@ -167,8 +176,11 @@ struct LaneState {
         const int c = clo + ((lane - clo) & 31);
         myc = (unsigned)c < (unsigned)nchan ? c : -1;
         cf = (float)c;
-        Is = 0.f; Ts = 1.f;
-        if (myc >= 0) { Is = sI[c]; Ts = sT[c]; }
+        Is = 0.f; Ts = 1.f; Ls = 0.f;
+        if (myc >= 0) {
+            Is = sI[c]; Ts = sT[c];
+            if (COMP) Ls = sL[c];
+        }
         cur = clo;
     }
 };
@@ -181,16 +193,25 @@ __device__ __forceinline__ f2 pair_u_win(const float4 &qa, const float4 &qc, flo
 
 // O9 for the two steps of a pair, in march order.  c = S ((1-e) T) and I += c with fixed roundings: the adjoint
 // re-march repeats exactly this sequence and so reproduces the partial sums bit for bit.
-__device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, const float4 &qc, float cf, float &Is, float &Ts)
+template <bool COMP>
+__device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, const float4 &qc, float cf, float &Is, float &Ts,
+                                         float &Ls)
 {
     Pair s;
     pair_eval(pair_u_win(qa, qc, cf), pk(qb.x, qb.y), s);
     float om0, om1, e0, e1;
     upk(s.om, om0, om1);
     upk(s.e, e0, e1);
-    Is = __fmaf_rn(qb.z, __fmul_rn(om0, Ts), Is);
+    const float m0 = __fmul_rn(om0, Ts);
+    const float I1 = __fmaf_rn(qb.z, m0, Is);
+    // rounding error of I1 = fl(S m + Is): Is - I1 is exact whenever the contribution is small against the sum, which
+    // is when it matters
+    if (COMP) Ls += __fmaf_rn(qb.z, m0, __fsub_rn(Is, I1));
     Ts = __fmul_rn(Ts, e0);
-    Is = __fmaf_rn(qb.w, __fmul_rn(om1, Ts), Is);
+    const float m1 = __fmul_rn(om1, Ts);
+    const float I2 = __fmaf_rn(qb.w, m1, I1);
+    if (COMP) Ls += __fmaf_rn(qb.w, m1, __fsub_rn(I1, I2));
+    Is = I2;
     Ts = __fmul_rn(Ts, e1);
 }
 
@@ -228,22 +249,22 @@ extern __shared__ __align__(16) unsigned char win_smem[];
 // ---------------------------------------------------------------------------------------------
 // K2 / K3 forward march.  Dynamic shared memory per warp: WinShared + (I, T) of 32 ngroups channels.
 // ---------------------------------------------------------------------------------------------
-static size_t fwd_warp_bytes(int ng) { return sizeof(WinShared) + (size_t)ng * 256; }
+static size_t fwd_warp_bytes(int ng, bool comp) { return sizeof(WinShared) + (size_t)ng * (comp ? 384 : 256); }
 
-template <int KIND>
+template <int KIND, bool COMP>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_march_fwd_w(const __grid_constant__ MarchParams P)
 {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     RayCtx rc;
     if (!ray_setup(P, rc, warp)) return;
     const int ng = P.line.ngroups;
-    unsigned char *base = win_smem + (size_t)warp * (sizeof(WinShared) + (size_t)ng * 256);
+    unsigned char *base = win_smem + (size_t)warp * (sizeof(WinShared) + (size_t)ng * (COMP ? 384 : 256));
     WinShared &S = *reinterpret_cast<WinShared *>(base);
     float *sI = reinterpret_cast<float *>(base + sizeof(WinShared)), *sT = sI + 32 * ng;
     const DevGeom &G = P.geom[rc.b];
     const int nchan = P.line.nchan;
     float *out = P.cube + rc.ray * (size_t)nchan;
-    LaneState L;
+    LaneState<COMP> L;
     L.init(sI, sT, lane, ng);
     if (P.target) loss_prefetch(P, rc.ray * (size_t)nchan, nchan, lane);
     unsigned n_steps = 0, n_mufu = 0;
@@ -278,7 +299,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
                     const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
                     const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
                     if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
-                    fwd_pair(qa, qb, qc, L.cf, L.Is, L.Ts);
+                    fwd_pair<COMP>(qa, qb, qc, L.cf, L.Is, L.Ts, L.Ls);
                 }
                 n_mufu += 4 * npairs;
                 __syncwarp();
@@ -292,6 +313,9 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
         if (c < nchan) {
             const float Ic = sI[c];
             out[c] = Ic;
+            // the cube value travels with its low-order word: the adjoint takes the word only where the value still
+            // equals the cube it is given
+            if (COMP) P.ws.ilo[rc.ray * (size_t)nchan + c] = make_float2(Ic, L.sL[c]);
             if (P.target) r2 += loss_voxel(P, rc.ray * (size_t)nchan + c, Ic);
         }
     }
@@ -313,14 +337,21 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
 
 // Per-lane channel state of the adjoint window march: transmittance and partial sum of all channels live in shared
 // memory; the saved intensity and dL/dI of the served channel are re-read (L1) when the group moves.
+template <bool COMP>
 struct BwdLane {
     float Ts, Ps, Is, Gs, cf;                     // transmittance, partial sum, saved I, dL/dI of the served channel
+    float Qs, Ils, vs;                            // COMP: low-order words of the partial sum and of the saved I; vs = 1
+                                                  // where the saved word is valid, else 0 (plain difference)
     int cur, myc;
-    float *sT, *sP;
+    float *sT, *sP, *sQ;
     const float *Isave, *Gin;
+    const float2 *Ilo;
     __device__ __forceinline__ void put_back()
     {
-        if (myc >= 0) { sT[myc] = Ts; sP[myc] = Ps; }
+        if (myc >= 0) {
+            sT[myc] = Ts; sP[myc] = Ps;
+            if (COMP) sQ[myc] = Qs;
+        }
     }
     __device__ __forceinline__ void regroup(int clo, int lane, int nchan)
     {
@@ -329,9 +360,23 @@ struct BwdLane {
         myc = (unsigned)c < (unsigned)nchan ? c : -1;
         cf = (float)c;
         Ts = 1.f; Ps = 0.f; Is = 0.f; Gs = 0.f;    // lanes without a channel contribute nothing (G = 0)
-        if (myc >= 0) { Ts = sT[c]; Ps = sP[c]; Is = __ldg(Isave + c); Gs = __ldg(Gin + c); }
+        Qs = 0.f; Ils = 0.f; vs = 0.f;
+        if (myc >= 0) {
+            Ts = sT[c]; Ps = sP[c]; Is = __ldg(Isave + c); Gs = __ldg(Gin + c);
+            if (COMP) {
+                // the forward left {I, low-order word} in the workspace: the word is only taken where the value is
+                // bit for bit the cube's (another workspace, or one written since, falls back to the plain difference)
+                Qs = sQ[c];
+                const float2 w = __ldg(Ilo + c);
+                const bool ok = __float_as_int(w.x) == __float_as_int(Is);
+                Ils = ok ? w.y : 0.f;
+                vs = ok ? 1.f : 0.f;
+            }
+        }
         cur = clo;
     }
+    // -R = (P - I) + (P_lo - I_lo) of the served channel
+    __device__ __forceinline__ float neg_r() const { return COMP ? fmaf(vs, Qs - Ils, Ps - Is) : Ps - Is; }
 };
 
 // Partial sums of a reduction batch, rows padded by one element so that both the per-lane writes and the per-step
@@ -342,7 +387,8 @@ struct BwdLane {
 typedef float4 RedBuf[2 * BWD_SUB][RED_ROW];
 
 // A pair with at least one emitting step.  Repeats the forward's O9 sequence bit for bit (fwd_pair).
-__device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane &L,
+template <bool COMP>
+__device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane<COMP> &L,
                                            float nsmax, float4 (*red)[RED_ROW], int lane)
 {
     Pair s;
@@ -357,7 +403,15 @@ __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, c
     const float P1 = __fmaf_rn(qb.w, c1, P0);
     const float T2 = __fmul_rn(T1, e1);
     const f2 Tn = pk(T1, T2), G2 = pk1(L.Gs);
-    const f2 nR = clamp_nR(sub2(pk(P0, P1), pk1(L.Is)), Tn, pk1(nsmax));
+    f2 PmI = sub2(pk(P0, P1), pk1(L.Is));
+    if (COMP) {
+        // the same error words the forward collected (fwd_pair), so that P + Q tracks the exact partial sum
+        const float Q0 = L.Qs + __fmaf_rn(qb.z, c0, __fsub_rn(L.Ps, P0));
+        const float Q1 = Q0 + __fmaf_rn(qb.w, c1, __fsub_rn(P0, P1));
+        PmI = fma2(pk1(L.vs), sub2(pk(Q0, Q1), pk1(L.Ils)), PmI);
+        L.Qs = Q1;
+    }
+    const f2 nR = clamp_nR(PmI, Tn, pk1(nsmax));
     const f2 a = mul2(G2, fma2(Tn, pk(qb.z, qb.w), nR));          // dL/d dtau
     const f2 w = mul2(a, s.g), wu = mul2(w, s.u), wuu = mul2(wu, s.u), gc = mul2(G2, pk(c0, c1));
     float w0, w1, x0, x1, y0, y1, z0, z1;
@@ -369,9 +423,10 @@ __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, c
 
 // Zero-opacity steps leave T and P untouched, so G T and G R are fixed while the lane keeps its channel; only
 // sum w = sum (G T S_k - G R) g is needed.  {GT, GnR} of the served channel:
-__device__ __forceinline__ float2 z_frozen(const BwdLane &L, float nsmax)
+template <bool COMP>
+__device__ __forceinline__ float2 z_frozen(const BwdLane<COMP> &L, float nsmax)
 {
-    return make_float2(L.Gs * L.Ts, L.Gs * fminf(fmaxf(L.Ps - L.Is, L.Ts * nsmax), 0.f));
+    return make_float2(L.Gs * L.Ts, L.Gs * fminf(fmaxf(L.neg_r(), L.Ts * nsmax), 0.f));
 }
 __device__ __forceinline__ f2 z_pair_w(const float4 &qa, float Sa, float Sb, const float4 &qc, float cf, float2 fr)
 {
@@ -420,9 +475,9 @@ struct __align__(16) BwdShared {          // per warp, followed by (T, P) of 32 
     RedBuf red;                           // 8 x 33 float4 = 32 x 33 float
     float4 sum[32];                       // channel sums of the compacted steps
 };
-static size_t bwd_warp_bytes(int ng) { return sizeof(BwdShared) + (size_t)ng * 256; }
+static size_t bwd_warp_bytes(int ng, bool comp) { return sizeof(BwdShared) + (size_t)ng * (comp ? 384 : 256); }
 
-template <int KIND>
+template <int KIND, bool COMP>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_march_bwd_w(const __grid_constant__ MarchParams P)
 {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -430,23 +485,25 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
     if (!ray_setup(P, rc, warp)) return;
     if (rc.ds == 0.0) return;
     const int ng = P.line.ngroups;
-    unsigned char *base = win_smem + (size_t)warp * (sizeof(BwdShared) + (size_t)ng * 256);
+    unsigned char *base = win_smem + (size_t)warp * (sizeof(BwdShared) + (size_t)ng * (COMP ? 384 : 256));
     BwdShared &B = *reinterpret_cast<BwdShared *>(base);
     WinShared &S = B.w;
     const DevGeom &G = P.geom[rc.b];
     const DevLine &Ln = P.line;
     const int nchan = Ln.nchan;
-    BwdLane L;
-    L.sT = reinterpret_cast<float *>(base + sizeof(BwdShared)); L.sP = L.sT + 32 * ng;
+    BwdLane<COMP> L;
+    L.sT = reinterpret_cast<float *>(base + sizeof(BwdShared)); L.sP = L.sT + 32 * ng; L.sQ = L.sP + 32 * ng;
+    L.Ilo = P.ws.ilo + rc.ray * (size_t)nchan;
     L.Isave = P.cube + rc.ray * (size_t)nchan;
     L.Gin = P.dl_dcube + rc.ray * (size_t)nchan;
     bool anyg = false;
     for (int g = 0; g < ng; ++g) {
         const int c = lane + 32 * g;
         L.sT[c] = 1.f; L.sP[c] = 0.f;
+        if (COMP) L.sQ[c] = 0.f;
         anyg |= c < nchan && __ldg(L.Gin + c) != 0.f;
     }
-    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.cf = 0.f; L.cur = NO_GROUP; L.myc = -1;
+    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.cf = 0.f; L.Qs = 0.f; L.Ils = 0.f; L.vs = 0.f; L.cur = NO_GROUP; L.myc = -1;
     if (!__any_sync(FULL, anyg)) return;     // dL/dcube vanishes on this ray: no gradient
     const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
@@ -526,7 +583,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
                     const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
                     const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
                     if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
-                    bwd_pair_e(qa, qb, qc, L, nsmax, &B.red[2 * jj], lane);
+                    bwd_pair_e<COMP>(qa, qb, qc, L, nsmax, &B.red[2 * jj], lane);
                 }
                 n_mufu += 4 * nb;
                 __syncwarp();
@@ -565,14 +622,26 @@ static cudaError_t launch_w(K kern, const MarchParams &P, int nbatch, size_t war
 
 cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    const size_t wb = fwd_warp_bytes(P.line.ngroups);
-    return P.grid.kind == 0 ? launch_w(k_march_fwd_w<0>, P, nbatch, wb, st)
-         : P.grid.kind == 1 ? launch_w(k_march_fwd_w<1>, P, nbatch, wb, st) : launch_w(k_march_fwd_w<2>, P, nbatch, wb, st);
+    const bool comp = P.ws.ilo != nullptr;
+    const size_t wb = fwd_warp_bytes(P.line.ngroups, comp);
+    if (comp)
+        return P.grid.kind == 0 ? launch_w(k_march_fwd_w<0, true>, P, nbatch, wb, st)
+             : P.grid.kind == 1 ? launch_w(k_march_fwd_w<1, true>, P, nbatch, wb, st)
+                                : launch_w(k_march_fwd_w<2, true>, P, nbatch, wb, st);
+    return P.grid.kind == 0 ? launch_w(k_march_fwd_w<0, false>, P, nbatch, wb, st)
+         : P.grid.kind == 1 ? launch_w(k_march_fwd_w<1, false>, P, nbatch, wb, st)
+                            : launch_w(k_march_fwd_w<2, false>, P, nbatch, wb, st);
 }
 
 cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    const size_t wb = bwd_warp_bytes(P.line.ngroups);
-    return P.grid.kind == 0 ? launch_w(k_march_bwd_w<0>, P, nbatch, wb, st)
-         : P.grid.kind == 1 ? launch_w(k_march_bwd_w<1>, P, nbatch, wb, st) : launch_w(k_march_bwd_w<2>, P, nbatch, wb, st);
+    const bool comp = P.ws.ilo != nullptr;
+    const size_t wb = bwd_warp_bytes(P.line.ngroups, comp);
+    if (comp)
+        return P.grid.kind == 0 ? launch_w(k_march_bwd_w<0, true>, P, nbatch, wb, st)
+             : P.grid.kind == 1 ? launch_w(k_march_bwd_w<1, true>, P, nbatch, wb, st)
+                                : launch_w(k_march_bwd_w<2, true>, P, nbatch, wb, st);
+    return P.grid.kind == 0 ? launch_w(k_march_bwd_w<0, false>, P, nbatch, wb, st)
+         : P.grid.kind == 1 ? launch_w(k_march_bwd_w<1, false>, P, nbatch, wb, st)
+                            : launch_w(k_march_bwd_w<2, false>, P, nbatch, wb, st);
 }

@@ -31,7 +31,12 @@ def rt(request):
     dense = os.environ.get("RADT_TEST_DENSE") == "1"       # one-off runs of the whole file without windowing / skipping
     if dense:
         B.radt_set_option(B.OPT_WINDOW, 0); B.radt_set_option(B.OPT_SKIP_EMPTY, 0)
+    comp = os.environ.get("RADT_TEST_COMP") == "1"         # one-off runs of the whole file with RADT_OPT_COMPENSATED
+    if comp:
+        B.radt_set_option(B.OPT_COMPENSATED, 1)
     yield pkg
+    if comp:
+        B.radt_set_option(B.OPT_COMPENSATED, 0)
     B.radt_set_option(B.OPT_WIN_PATH, 1)
     if dense:
         B.radt_set_option(B.OPT_WINDOW, 1); B.radt_set_option(B.OPT_SKIP_EMPTY, 1)
@@ -549,3 +554,41 @@ def test_optically_thick_central_ray_gradient_bound(rt):
         m = np.abs(b).max()
         assert np.abs(a - b).max() <= 1e-3 * m and np.linalg.norm(a - b) <= 1e-3 * np.linalg.norm(b), nm
     check_grad("thick central ray g_temp", got[1], want[1])
+
+
+def _with_compensation(rt):
+    B = rt.binding
+    return B, B.radt_get_option(B.OPT_WIN_PATH) == 1
+
+
+@pytest.mark.parametrize("case", ["thick228", "medium81", "medium97", "medium143", "cfg1"])
+def test_compensated_adjoint(rt, case):
+    """RADT_OPT_COMPENSATED: the forward keeps the low-order word of its fp32 sum in the workspace and the adjoint forms
+    R_k = I - I_{<=k} from both words.  Same cube bit for bit; the scenes that exceed the element-wise gradient floor
+    without it (optically thick rays) now pass the strict criteria.  Window kernels only."""
+    B, win = _with_compensation(rt)
+    if not win:
+        pytest.skip("the channel-table kernels do not carry the low-order words")
+    sc = {"thick228": lambda: _random_scene(228), "medium81": lambda: _random_scene(81, medium=True),
+          "medium97": lambda: _random_scene(97, medium=True), "medium143": lambda: _random_scene(143, medium=True),
+          "cfg1": lambda: make_config(1)}[case]()
+    plain = _gpu_forward(rt, [sc]).cube.cpu().numpy()
+    B.radt_set_option(B.OPT_COMPENSATED, 1)
+    try:
+        R = _parity_fwd_bwd(rt, sc, f"compensated {case}")           # strict floors
+        np.testing.assert_array_equal(R.cube.cpu().numpy(), plain)
+        # a workspace that does not hold this cube's words falls back to the plain difference, voxel by voxel
+        R.ws.zero_()
+        g0 = [g.clone() for g in (R.g_dens, R.g_temp, R.g_vel)]
+        R.render_bwd()
+        B.radt_set_option(B.OPT_COMPENSATED, 0)
+        R2 = rt.Renderer([sc])
+        R2.render()
+        R2.dl_dcube.copy_(R.dl_dcube)
+        R2.render_bwd()
+        for a, b in zip((R.g_dens, R.g_temp, R.g_vel), (R2.g_dens, R2.g_temp, R2.g_vel)):
+            m = float(b.abs().max())
+            assert float((a - b).abs().max()) <= 2e-5 * m + 1e-30        # same arithmetic up to the order of the atomics
+        del g0
+    finally:
+        B.radt_set_option(B.OPT_COMPENSATED, 0)
