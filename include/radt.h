@@ -127,6 +127,12 @@ enum {
                                      in every channel improve from ~1e-3 to ~1e-6 of the maximum.
                                      A different or overwritten workspace falls back to the plain difference, voxel by
                                      voxel.  Window kernels only. */
+    RADT_OPT_ZERO_DENS_GRAD = 5,  /* 1 (default): exact gradient; 0: the adjoint skips steps without opacity on LINEAR density
+                                     grids.  Those steps carry only dL/dn of cells whose density is exactly zero (masked
+                                     CO, Eq. 9), which a fit through radt_disk_fields_bwd discards anyway (the
+                                     mask is held fixed), so g_temp, g_vel and g_dens at cells with non-zero density are
+                                     unchanged; g_dens at zero-density cells then only holds what emitting steps
+                                     contribute.  They are 48-65 % of the adjoint's steps on the disk configs. */
     RADT_OPT_WIN_PATH = 3         /* 1 (default): channel tables that are uniform lattices v_0 + c dv use the window
                                      kernels (one channel per lane inside the line window); 0: always the
                                      channel-table kernels.  radt_render and radt_render_bwd of one cube must run

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libradt.so")
 
 PASS_FWD, PASS_BWD = 0, 1
-OPT_WINDOW, OPT_SKIP_EMPTY, OPT_WIN_PATH, OPT_COMPENSATED = 1, 2, 3, 4
+OPT_WINDOW, OPT_SKIP_EMPTY, OPT_WIN_PATH, OPT_COMPENSATED, OPT_ZERO_DENS_GRAD = 1, 2, 3, 4, 5
 
 EXPORTS = ["radt_version", "radt_last_error", "radt_set_option", "radt_get_option", "radt_workspace_bytes",
            "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_l2_loss_grad", "radt_render_host",

@@ -17,6 +17,7 @@ int g_opt_window = 1;
 int g_opt_skip_empty = 1;
 int g_opt_win_path = 1;
 int g_opt_compensated = 0;
+int g_opt_zero_dens_grad = 1;
 
 int fail(int code, const char *fmt, ...)
 {
@@ -317,7 +318,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         // adjoint needs every in-grid step (dL/dn of empty cells), so only the forward and LN grids use it
         const bool win = use_win;
         const bool occ = win && g_opt_skip_empty && grid->kind != RADT_GRID_SPH3D &&
-                         (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN);
+                         (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN || !g_opt_zero_dens_grad);
         SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr; SP.occ_nbj = w.occ_nbj;
         SP.occ_thr = grid->dens_mode == RADT_DENS_LN ? -39.1439f : 1e-17f;     // N_EMPTY of the march kernels
         SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;
@@ -334,6 +335,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         MP.tiles_y = (MP.ny + RADT_TILE_Y - 1) / RADT_TILE_Y;
         MP.b0 = b0;
         MP.opt_window = g_opt_window; MP.opt_skip_empty = g_opt_skip_empty;
+        MP.opt_zero_grad = g_opt_zero_dens_grad || !g_opt_skip_empty;
         MP.chan_lo = 0;
         for (int b = 0; b < nb && !MP.chan_lo; ++b)
             for (int c = 0; c < line->nchan; ++c) {
@@ -381,6 +383,7 @@ int radt_set_option(int key, int value)
     if (key == RADT_OPT_SKIP_EMPTY) { g_opt_skip_empty = value != 0; return RADT_OK; }
     if (key == RADT_OPT_WIN_PATH) { g_opt_win_path = value != 0; return RADT_OK; }
     if (key == RADT_OPT_COMPENSATED) { g_opt_compensated = value != 0; return RADT_OK; }
+    if (key == RADT_OPT_ZERO_DENS_GRAD) { g_opt_zero_dens_grad = value != 0; return RADT_OK; }
     return fail(RADT_E_INVALID, "unknown option %d", key);
 }
 
@@ -390,6 +393,7 @@ int radt_get_option(int key)
     if (key == RADT_OPT_SKIP_EMPTY) return g_opt_skip_empty;
     if (key == RADT_OPT_WIN_PATH) return g_opt_win_path;
     if (key == RADT_OPT_COMPENSATED) return g_opt_compensated;
+    if (key == RADT_OPT_ZERO_DENS_GRAD) return g_opt_zero_dens_grad;
     return fail(RADT_E_INVALID, "unknown option %d", key);
 }
 

@@ -99,6 +99,7 @@ struct MarchParams {
     int tiles_x, tiles_y;
     int b0;                // first batch item of this launch
     int opt_window, opt_skip_empty;
+    int opt_zero_grad;     // adjoint: zero-opacity steps of LINEAR density grids are marched for their dL/dn (default)
     int chan_lo;           // some channel velocity is not exactly representable in fp32: use the lo parts
     int use_win;           // uniform-channel window kernels (radt_march_win.cu)
     int use_occ;           // candidate steps are prefiltered with the occupancy bitmap

@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd(const 
         phase_a<KIND, false, false>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, kb + lane, st);
         const bool isE = st.inside && st.K2 > kthr;
         // zero-opacity steps still carry dL/dn when the grid stores n itself (LINEAR)
-        const bool active = st.inside && (isE || P.grid.dens_mode == 0) && (!window || line_hits_span(st, vmin, vmax));
+        const bool active = st.inside && (isE || (P.grid.dens_mode == 0 && P.opt_zero_grad)) && (!window || line_hits_span(st, vmin, vmax));
         const unsigned mask = __ballot_sync(FULL, active);
         if (mask == 0u) continue;
         const int pos = __popc(mask & ((1u << lane) - 1u));

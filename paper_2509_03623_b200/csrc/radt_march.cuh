@@ -177,7 +177,7 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     float n = (g.dens_mode == 1) ? ex2_approx(dens * RADT_LOG2E) : dens;
     // empty samples: no opacity, hence no contribution to the cube; their only gradient is dL/dn, which exists
     // when the grid stores n itself (LINEAR) and vanishes with n when it stores ln n
-    if ((FWD || g.dens_mode == 1) && P.opt_skip_empty && !(n > N_EMPTY)) return;
+    if ((FWD || g.dens_mode == 1 || !P.opt_zero_grad) && P.opt_skip_empty && !(n > N_EMPTY)) return;
     st.inside = true;
     bool tcl = !(temp >= 1.0f);
     float T = tcl ? 1.0f : temp;

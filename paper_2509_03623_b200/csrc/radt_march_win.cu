@@ -525,7 +525,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
         phase_a<KIND, false, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, k, st);
         const bool isE = st.inside && st.K2 > kthr;
         // zero-opacity steps still carry dL/dn when the grid stores n itself (LINEAR)
-        const bool act = st.inside && (isE || P.grid.dens_mode == 0) && st.whi >= 0 && st.wlo < nchan;
+        const bool act = st.inside && (isE || (P.grid.dens_mode == 0 && P.opt_zero_grad)) && st.whi >= 0 && st.wlo < nchan;
         const float K2e = isE ? st.K2 : 0.f;
         n_steps += __popc(__ballot_sync(FULL, act));
         bool wide;

@@ -47,6 +47,9 @@ def main():
     pws = torch.empty(B.radt_disk_workspace_bytes(desc), dtype=torch.uint8, device=R.device)
     mlp = B.make_mlp(L=4)
     nparams = B.radt_mlp_num_params(mlp)
+    # the pre-pass holds the CO mask fixed and discards dL/dn of masked cells: the render adjoint need not march the
+    # steps that only feed those cells
+    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 0)
 
     # observed cube: the config's temperature grid through the pre-pass and the render, plus noise
     t_true = R.temp.clone()

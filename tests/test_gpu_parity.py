@@ -592,3 +592,36 @@ def test_compensated_adjoint(rt, case):
         del g0
     finally:
         B.radt_set_option(B.OPT_COMPENSATED, 0)
+
+
+@pytest.mark.parametrize("make", [lambda: make_config(2, npix=48), lambda: tiny_axisym_scene(seed=91, nstep=40)])
+def test_skip_zero_opacity_steps_in_the_adjoint(rt, make):
+    """RADT_OPT_ZERO_DENS_GRAD = 0: steps without opacity are not marched in the adjoint.  They only carry dL/dn of
+    cells whose density is exactly zero, so g_temp, g_vel and g_dens at non-zero cells equal the exact gradient."""
+    B = rt.binding
+    sc = make()
+    d = np.array(sc.grid.dens)
+    if not (d == 0).any():                       # the tiny scene has no masked cells of its own
+        d[: d.shape[0] // 2, d.shape[1] // 2:] = 0.0
+        sc = sc.with_fields(dens=d)
+    ref = _oracle_cube([sc])
+    tgt, sigma = l2_target(ref[0], 77)
+    G32 = ((ref[0] - tgt) / (sigma ** 2 * ref[0].size)).astype(np.float32)
+    want = po.render_bwd(sc, G32.astype(np.float64))
+    R = _gpu_forward(rt, [sc], need_bwd=True)
+    R.dl_dcube.copy_(torch.from_numpy(G32[None]))
+    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 0)
+    try:
+        gd, gt, gv = (g.cpu().numpy()[0].astype(np.float64) for g in R.render_bwd())
+        steps_skip = R.counters()[2]
+    finally:
+        B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 1)
+    R.render_bwd()
+    steps_all = R.counters()[2]
+    assert steps_skip < steps_all
+    check_grad("skip-Z g_temp", gt, want[1])
+    check_grad("skip-Z g_vel", gv, want[2])
+    nz = d != 0
+    m = np.abs(want[0]).max()
+    assert np.all(np.abs(gd[nz] - want[0][nz]) <= 1e-3 * np.abs(want[0][nz]) + 1e-5 * m)
+    assert np.all(np.isfinite(gd[~nz]))          # zero-density cells keep what the emitting steps around them contribute
