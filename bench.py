@@ -272,6 +272,10 @@ def run_ours(args):
     t_l2 = time_kernel_group(lambda: R.l2_loss_grad(stream), stream, torch, flush, reps)
     t_bwd = time_kernel_group(lambda: R.render_bwd(stream=stream), stream, torch, flush, reps)
     cnt_b = R.counters()
+    # the exact shortcut of the paper's fit chain: no march of the steps without opacity
+    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 0)
+    t_bwd_fit = time_kernel_group(lambda: R.render_bwd(stream=stream), stream, torch, flush, reps)
+    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 1)
     fwd_exec = cnt[1] * 32 // 2        # executed samples, 2 MUFU.EX2 lane-ops each
     bwd_exec = cnt_b[3] * 32 // 2      # 2-EX2 equivalents (zero-opacity adjoint samples need one EX2: counted as 1/2)
 
@@ -356,6 +360,7 @@ def run_ours(args):
                    "l2": "flushed between timed steps (256 MiB fill outside the events)",
                    "kernels": "window (uniform channel lattice)" if args.win_path else "channel table"},
         "fwd_value": nominal / (t_fwd * 1e-3), "fwd_ms": t_fwd, "fwd_loss_fused_ms": t_fl, "l2_ms": t_l2, "bwd_ms": t_bwd,
+        "bwd_ms_zero_dens_grad_off": t_bwd_fit,
         "executed_samples": {"fwd": int(fwd_exec), "bwd": int(bwd_exec), "fwd_active_ray_steps": int(cnt[0]),
                              "bwd_active_ray_steps": int(cnt_b[2]), "nominal": int(nominal)},
         "prepass": prepass,
