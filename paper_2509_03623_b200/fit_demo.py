@@ -35,6 +35,8 @@ def main():
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--lr", type=float, default=5e-4)
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--full-dens-grad", action="store_true", help="keep RADT_OPT_ZERO_DENS_GRAD on (march the steps without opacity)")
+    ap.add_argument("--no-graph", action="store_true", help="enqueue every step from Python instead of replaying one CUDA graph")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("fit_demo needs a CUDA device: there is no CPU fallback")
@@ -49,7 +51,7 @@ def main():
     nparams = B.radt_mlp_num_params(mlp)
     # the pre-pass holds the CO mask fixed and discards dL/dn of masked cells: the render adjoint need not march the
     # steps that only feed those cells
-    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 0)
+    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 1 if args.full_dens_grad else 0)
 
     # observed cube: the config's temperature grid through the pre-pass and the render, plus noise
     t_true = R.temp.clone()
@@ -73,23 +75,56 @@ def main():
     params = params.to(R.device)
     assert params.numel() == nparams
     params.grad = torch.zeros_like(params)
-    opt = torch.optim.Adam([params], lr=args.lr)
-    sched = torch.optim.lr_scheduler.PolynomialLR(opt, total_iters=args.steps, power=2.0)
+    use_graph = not args.no_graph
+    # the learning rate lives on the device so that the captured optimiser step follows the schedule
+    lr_t = torch.tensor(args.lr, device=R.device)
+    opt = torch.optim.Adam([params], lr=lr_t if use_graph else args.lr, capturable=use_graph)
 
-    def step():
-        B.radt_mlp_temperature(mlp, desc, params, R.temp[0])
-        B.radt_disk_fields(disks, desc, R.temp, R.dens, R.vel, pws)
-        R.fit_step()                                          # render + chi^2 + render adjoint
-        B.radt_disk_fields_bwd(disks, desc, R.temp, R.g_dens, R.g_vel, R.g_temp, pws)
-        B.radt_mlp_temperature_bwd(mlp, desc, params, R.g_temp[0], params.grad)
+    def lr_at(it):                      # polynomial decay to zero, power 2 ("polynomially decays")
+        return args.lr * (1.0 - min(it, args.steps) / args.steps) ** 2
+
+    def chain(stream=None):
+        B.radt_mlp_temperature(mlp, desc, params, R.temp[0], stream)
+        B.radt_disk_fields(disks, desc, R.temp, R.dens, R.vel, pws, stream)
+        R.fit_step(stream)                                    # render + chi^2 + render adjoint
+        B.radt_disk_fields_bwd(disks, desc, R.temp, R.g_dens, R.g_vel, R.g_temp, pws, stream)
+        B.radt_mlp_temperature_bwd(mlp, desc, params, R.g_temp[0], params.grad, stream)
         opt.step()
-        sched.step()
+
+    graph = None
+    if use_graph:
+        # every entry point is stream ordered and allocation free, so one fit step is one CUDA graph
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            snap = params.clone()
+            for _ in range(3):
+                chain(side)                                   # warm-up (also creates the optimiser state)
+            params.copy_(snap)
+            for st in opt.state.values():
+                for v in st.values():
+                    if torch.is_tensor(v):
+                        v.zero_()
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            chain(torch.cuda.current_stream())
+
+    def step(it):
+        if use_graph:
+            lr_t.fill_(lr_at(it))
+            graph.replay()
+        else:
+            for gp in opt.param_groups:
+                gp["lr"] = lr_at(it)
+            chain()
 
     losses = []
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for it in range(args.steps):
-        step()
+        step(it)
         if it % max(1, args.steps // 10) == 0 or it == args.steps - 1:
             losses.append((it, float(R.loss.cpu())))
     torch.cuda.synchronize()
@@ -99,6 +134,7 @@ def main():
     print(json.dumps({"workload": sc.name, "steps": args.steps, "ms_per_fit_step": 1e3 * dt / args.steps,
                       "fit_steps_per_s": args.steps / dt, "loss": losses,
                       "median_rel_T_error_in_CO_layer": rel, "n_params": nparams,
+                      "cuda_graph": use_graph,
                       "chain": "MLP -> pre-pass -> render -> chi^2 -> adjoints -> ADAM (torch elementwise update)"}))
 
 
