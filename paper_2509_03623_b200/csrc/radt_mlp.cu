@@ -246,6 +246,76 @@ __device__ __forceinline__ void mlp_back_layer(const float *__restrict__ W, floa
     }
 }
 
+// Two-node / two-unit versions of the adjoint's inner routines (same arithmetic; every broadcast row load feeds two
+// accumulator sets, which halves the shared-memory wavefronts per FMA as in mlp_layer2).
+// dW[o][i] for units i = u0, u1 and the 8 output units of `part`, nodes in two chunks of 32.
+__device__ __forceinline__ void mlp_grad_weights2(const float *act, const float *delta, float *gW, int u0, int u1, int part)
+{
+    const int o0 = part * MLP_P8;
+    f2 s0[MLP_P8], s1[MLP_P8];
+#pragma unroll
+    for (int o = 0; o < MLP_P8; ++o) { s0[o] = mlp_pk(0.f, 0.f); s1[o] = s0[o]; }
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        f2 a0[16], a1[16];
+#pragma unroll
+        for (int n = 0; n < 16; ++n) {
+            a0[n] = mlp_pk(act[u0 * MLP_SA + 32 * c + 2 * n], act[u0 * MLP_SA + 32 * c + 2 * n + 1]);
+            a1[n] = mlp_pk(act[u1 * MLP_SA + 32 * c + 2 * n], act[u1 * MLP_SA + 32 * c + 2 * n + 1]);
+        }
+#pragma unroll
+        for (int o = 0; o < MLP_P8; ++o) {
+            const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(delta + (o0 + o) * MLP_SD + 32 * c);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const ulonglong2 d = row[q];
+                s0[o] = mlp_fma2(d.x, a0[2 * q], s0[o]);
+                s1[o] = mlp_fma2(d.x, a1[2 * q], s1[o]);
+                s0[o] = mlp_fma2(d.y, a0[2 * q + 1], s0[o]);
+                s1[o] = mlp_fma2(d.y, a1[2 * q + 1], s1[o]);
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 0; o < MLP_P8; ++o) {
+        atomicAdd(gW + (o0 + o) * MLP_W + u0, mlp_sum2(s0[o]));
+        atomicAdd(gW + (o0 + o) * MLP_W + u1, mlp_sum2(s1[o]));
+    }
+}
+
+// delta_in for nodes n0, n1 and the 8 input units of `part`; in place like mlp_back_layer
+__device__ __forceinline__ void mlp_back_layer2(const float *__restrict__ W, float *dl, const float *ain, int n0, int n1, int part)
+{
+    const int i0 = part * MLP_P8;
+    f2 acc0[MLP_P8 / 2], acc1[MLP_P8 / 2];
+#pragma unroll
+    for (int i = 0; i < MLP_P8 / 2; ++i) { acc0[i] = mlp_pk(0.f, 0.f); acc1[i] = acc0[i]; }
+#pragma unroll 8
+    for (int o = 0; o < MLP_W; ++o) {
+        const float d0 = dl[o * MLP_SD + n0], d1 = dl[o * MLP_SD + n1];
+        const f2 dd0 = mlp_pk(d0, d0), dd1 = mlp_pk(d1, d1);
+        const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(W + o * MLP_W + i0);
+#pragma unroll
+        for (int q = 0; q < MLP_P8 / 4; ++q) {
+            const ulonglong2 w = row[q];
+            acc0[2 * q] = mlp_fma2(w.x, dd0, acc0[2 * q]); acc1[2 * q] = mlp_fma2(w.x, dd1, acc1[2 * q]);
+            acc0[2 * q + 1] = mlp_fma2(w.y, dd0, acc0[2 * q + 1]); acc1[2 * q + 1] = mlp_fma2(w.y, dd1, acc1[2 * q + 1]);
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < MLP_P8 / 2; ++i) {
+        float a, b;
+        const int u = i0 + 2 * i;
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(acc0[i]));
+        dl[u * MLP_SD + n0] = ain[u * MLP_SA + n0] > 0.f ? a : 0.f;
+        dl[(u + 1) * MLP_SD + n0] = ain[(u + 1) * MLP_SA + n0] > 0.f ? b : 0.f;
+        asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(acc1[i]));
+        dl[u * MLP_SD + n1] = ain[u * MLP_SA + n1] > 0.f ? a : 0.f;
+        dl[(u + 1) * MLP_SD + n1] = ain[(u + 1) * MLP_SA + n1] > 0.f ? b : 0.f;
+    }
+}
+
 // Adjoint: recomputes the activations of its 64 nodes (nothing is stored between the passes), then walks the layers
 // backwards; parameter gradients leave the block as float atomics.  Shared memory: all activations, ONE delta buffer
 // (a node's column is private to its thread, so the back-propagation runs in place) and the weights of the layer
@@ -306,10 +376,23 @@ __global__ void __launch_bounds__(MLP_TB * MLP_S, 2) k_mlp_bwd(const __grid_cons
         if (node == 0) atomicAdd(Q.g_params + F.b[MLP_H], sb);
     }
     for (int l = MLP_H - 1; l >= 0; --l) {
-        mlp_grad_weights(act(l), dl, l == 0 ? F.D : MLP_W, Q.g_params + F.W[l], Q.g_params + F.b[l], MLP_W, node, part);
-        if (l > 0) {
+        const int pair = threadIdx.x & (MLP_TB / 2 - 1), part8 = threadIdx.x / (MLP_TB / 2);
+        if (l == 0) {
+            mlp_grad_weights(act(0), dl, F.D, Q.g_params + F.W[0], Q.g_params + F.b[0], MLP_W, node, part);
+        } else {
+            mlp_grad_weights2(act(l), dl, Q.g_params + F.W[l], pair, pair + MLP_TB / 2, part8);
+            if (threadIdx.x < MLP_W) {                     // bias gradients: one unit per thread
+                const float4 *row = reinterpret_cast<const float4 *>(dl + threadIdx.x * MLP_SD);
+                float sb = 0.f;
+#pragma unroll
+                for (int q = 0; q < MLP_TB / 4; ++q) {
+                    const float4 d = row[q];
+                    sb += (d.x + d.y) + (d.z + d.w);
+                }
+                atomicAdd(Q.g_params + F.b[l] + threadIdx.x, sb);
+            }
             const float *w = stage(l);                     // (its barriers also fence the reads of dl above)
-            mlp_back_layer(w, dl, act(l), node, part);
+            mlp_back_layer2(w, dl, act(l), pair, pair + MLP_TB / 2, part8);
             __syncthreads();
         }
     }
