@@ -533,6 +533,15 @@ def test_random_medium_scenes(rt, seed):
     _parity_fwd_bwd(rt, _random_scene(seed, medium=True), f"random medium scene {seed}", seed=seed, grad_floor=1e-4)
 
 
+@pytest.mark.parametrize("kind", ["cart", "sph"])
+def test_batches_of_3d_scenes(rt, kind):
+    """Batch items share the line, the grid layout and the image size; fields and viewing geometry differ."""
+    make = tiny_cart_scene if kind == "cart" else tiny_sph_scene
+    scs = [make(seed=120 + b, incl_deg=15.0 + 20 * b, pa_deg=-50.0 + 40 * b, az_deg=30.0 * b, npix=6, vsys=1e4 * b)
+           for b in range(3)]
+    _parity_fwd_bwd(rt, scs, f"batch of 3 {kind}")
+
+
 def test_optically_thick_central_ray_gradient_bound(rt):
     """Known limit of the front-to-back adjoint: R_k = I_saved - P_k carries the rounding of the
     forward's own fp32 sum (~1e-7 I).  On a ray that is optically thick in EVERY channel from its first steps
