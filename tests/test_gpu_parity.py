@@ -533,6 +533,18 @@ def test_random_medium_scenes(rt, seed):
     _parity_fwd_bwd(rt, _random_scene(seed, medium=True), f"random medium scene {seed}", seed=seed, grad_floor=1e-4)
 
 
+@pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_OFFCENTRE", "8"))))
+def test_random_offcentre_scenes(rt, seed):
+    """Images that are not centred on the star and not square in extent, in CGS or Jy/pixel units."""
+    rng = np.random.default_rng(777 + seed)
+    sc = _random_scene(500 + seed)
+    g = sc.geom
+    sc = replace(sc, geom=replace(g, x0=float(rng.uniform(-60, 60)), y0=float(rng.uniform(-60, 60)),
+                                  fov_y=g.fov_y * float(rng.uniform(0.5, 1.0)), dist_pc=float(rng.uniform(60, 160))),
+                 line=replace(sc.line, unit=int(rng.choice([UNIT_CGS, UNIT_JY_PIXEL, 0]))))
+    _parity_fwd_bwd(rt, sc, f"off-centre scene {seed}", seed=seed)
+
+
 @pytest.mark.parametrize("kind", ["cart", "sph"])
 def test_batches_of_3d_scenes(rt, kind):
     """Batch items share the line, the grid layout and the image size; fields and viewing geometry differ."""
