@@ -442,13 +442,16 @@ __device__ __forceinline__ f2 z_pair_w(const float4 &qa, float Sa, float Sb, con
 // four sums of step s.
 __device__ __forceinline__ void reduce_steps_e(const RedBuf &red, int nb, float4 *out, int lane)
 {
-    const float4 *row = &red[lane & 7][lane & 24];
-    float4 acc = row[0];
+    // rows as pairs of packed f32x2: one FADD2 per two sums
+    const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(&red[lane & 7][lane & 24]);
+    ulonglong2 a = row[0];
 #pragma unroll
     for (int i = 1; i < 8; ++i) {
-        const float4 v = row[i];
-        acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+        const ulonglong2 v = row[i];
+        a.x = add2(a.x, v.x); a.y = add2(a.y, v.y);
     }
+    float4 acc;
+    upk(a.x, acc.x, acc.y); upk(a.y, acc.z, acc.w);
 #pragma unroll
     for (int m = 8; m <= 16; m <<= 1) {
         acc.x += __shfl_xor_sync(FULL, acc.x, m);
