@@ -1,18 +1,24 @@
 #!/usr/bin/env python
-"""Benchmark of the line-RT render hot path (BASELINE.json metric: ray.channel.step samples/s, fwd+bwd).
+"""Benchmark of the line-RT render hot path (BASELINE.json metric: ray.channel.step samples/s, fwd and fwd+bwd).
 
-A *step* is one pass of the whole hot path over one synthetic disk: ray geometry + forward march with the L2 data
-term fused into its epilogue (radt_render_loss) -> memory-free adjoint (SURVEY.md section 8(a) rows a-j).  The workload at N = 1 is BASELINE.json
-`configs[1]` (256x128 (r,z) grid, 256x256 px, 64 channels, 256 steps per ray).  With N > 1 every rank renders
-its own disk (independent problems, no data-path collective): weak scaling.
+A *step* is one pass of the whole hot path over one synthetic workload: ray geometry + forward march with the chi^2 data
+term fused into its epilogue (radt_render_loss, low-order words kept) -> memory-free adjoint reusing the forward's setup
+(SURVEY.md section 8(a) rows a-j).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k | --configs 1,2,...] [--impl ours|reference]
 
-One JSON line is printed by rank 0.  `value` = nominal samples (rays x channels x steps, summed over ranks and
-steps) / device time of the K steps (inputs resident in HBM; L2 flushed between steps outside the timed
-events).  `e2e` = the same step through the HOST-buffer C-ABI entry point (copies inside the timed region).
-`roofline` = the dominant kernel against the SFU issue peak measured in this run.
-`cpu_baseline` = the fp64 oracle, as it stands, on this box's host cores, on a bounded ray sample.
+ONE run measures every config (BASELINE.json configs[0..4] = 1..5, and 6 = the stand-in for the paper's own timing benchmark,
+a 512 x 96 x 256 spherical grid) and rank 0 prints ONE JSON line.  Its top-level `value`, `ms_per_step`, `config.workload`,
+`roofline`, `e2e`, `cpu_baseline` are those of the HEADLINE workload: config 5 (16 x 512^2 px x 128 channels x 512 steps,
+2.75e11 nominal samples), the largest single-GPU configuration; `per_config` carries the same measurements for every config.
+With N > 1 every rank renders its own disks (independent problems, no data-path collective): weak scaling.
+
+`value` = nominal samples (rays x channels x steps, summed over ranks and steps) / device time of the K steps (inputs resident
+in HBM; L2 flushed between steps outside the timed events).  `e2e` = the same step through the HOST-buffer C-ABI entry point
+radt_fit_step_host (pinned host buffers, copies inside the timed region); `e2e_render` = radt_render_host (cube D2H inside).
+`roofline` = the dominant kernel against the issue peak measured in this run: `frac` counts EXECUTED
+samples only; `speedup_from_skipping` = nominal / executed samples (an algorithmic saving, not pipe efficiency).
+`cpu_baseline` = the fp64 oracle, as it stands, on this box's host cores, on a bounded ray sample of the headline workload.
 """
 from __future__ import annotations
 
@@ -31,7 +37,8 @@ import numpy as np  # noqa: E402
 
 METRIC = "ray*channel*step samples/s (fwd+bwd step)"
 UNIT = "samples/s"
-
+HEADLINE = 5
+ALL_CONFIGS = (1, 2, 3, 4, 5, 6)
 
 _SPH = {"npix": 256, "nchan": 64}       # config 6 image size and channel count (--sph-npix / --sph-nchan sweep them)
 
@@ -46,6 +53,17 @@ def _scenes(cfg):
 def _workload_name(cfg):
     from synth import config_names
     return f"cfg6_sph512x96x256_img{_SPH['npix']}_c{_SPH['nchan']}_n256" if cfg == 6 else config_names()[cfg]
+
+
+def _config_dict(cfg, scenes, world):
+    """The workload description: the same dict in both arms (ours and --impl reference)."""
+    s0 = scenes[0]
+    return {"workload": _workload_name(cfg), "rays": int(sum(s.nrays for s in scenes)), "channels": int(len(s0.line.vchan)),
+            "steps_per_ray": int(s0.geom.nstep), "grid": [int(n) for n in s0.grid.n], "batch": len(scenes),
+            "nominal_samples_per_step": int(sum(s.nominal_samples for s in scenes)),
+            "parallelism": f"independent disks x{world}",
+            "l2": "GPU arm: flushed between timed steps (256 MiB fill outside the events); CPU oracle arm: n/a",
+            "headline_rule": "largest single-GPU configuration of BASELINE.json (configs[4]); every config is in per_config"}
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -98,67 +116,90 @@ class ClockSampler(threading.Thread):
 # ----------------------------------------------------------------------------------------------------
 # CPU baseline: the oracle as it stands, on a bounded sample of the same workload
 # ----------------------------------------------------------------------------------------------------
-def oracle_sample_step(scene, stride, G=None):
-    """One fwd+adjoint pass of the oracle over every `stride`-th ray of `scene`; returns (seconds, samples)."""
+def _subset(scene, stride_xy):
+    """Every `stride_xy`-th row and column of the image (SURVEY.md:328 allows this ray subset for the large configs)."""
+    ny, nx = scene.geom.ny, scene.geom.nx
+    iy, ix = np.arange(0, ny, stride_xy), np.arange(0, nx, stride_xy)
+    return (iy[:, None] * nx + ix[None, :]).reshape(-1).astype(np.int64)
+
+
+def oracle_pass(scene, idx):
+    """One fwd + adjoint pass of the oracle over rays `idx` of `scene`; returns (seconds, samples)."""
     from oracle import pyoracle as po
-    nrays = scene.nrays
-    idx = np.arange(0, nrays, stride, dtype=np.int64)
     t0 = time.perf_counter()
     cube = po.render(scene, rays=idx)
-    g = cube * 1e-6 if G is None else G
-    po.render_bwd(scene, g, rays=idx)
+    po.render_bwd(scene, cube * 1e-6, rays=idx)
     dt = time.perf_counter() - t0
     return dt, len(idx) * len(scene.line.vchan) * scene.geom.nstep
 
 
-def cpu_baseline(scene, budget_s=12.0):
-    """The oracle as it stands on this box's host cores: whole fwd + adjoint passes over every 2nd ray of the scene,
-    repeated until about `budget_s` seconds of wall time (>= 2 passes)."""
+def _sample_stride(scenes, budget_s, npasses):
+    """Row/column stride such that `npasses` oracle passes over the subset of ALL scenes take about budget_s."""
+    probe = _subset(scenes[0], 32)
+    oracle_pass(scenes[0], probe[:64])                      # load the library, touch the pages
+    dt, n = oracle_pass(scenes[0], probe)
+    rate = n / dt                                           # samples / s
+    total = sum(s.nominal_samples for s in scenes)
+    want = max(rate * budget_s / max(npasses, 1), 1.0)      # samples per pass
+    return int(min(max(np.ceil(np.sqrt(total / want)), 1), 64))
+
+
+def cpu_baseline(scenes, name, budget_s=12.0):
+    """The oracle as it stands on this box's host cores: whole fwd + adjoint passes over a fixed ray subset of every batch
+    item (every s-th row and column), repeated until about `budget_s` seconds of wall time (>= 2 passes)."""
     from oracle import pyoracle as po
-    oracle_sample_step(scene, 64)          # load the library, touch the pages
-    stride, tot_t, tot_n, passes = 2, 0.0, 0, 0
+    stride = _sample_stride(scenes, budget_s, 2)
+    tot_t, tot_n, passes = 0.0, 0, 0
     while passes < 2 or tot_t < budget_s:
-        dt, n = oracle_sample_step(scene, stride)
-        tot_t += dt
-        tot_n += n
+        for sc in scenes:
+            dt, n = oracle_pass(sc, _subset(sc, stride))
+            tot_t += dt
+            tot_n += n
         passes += 1
     cores = po.num_threads()
-    # the same oracle on ONE thread (every 16th ray): the per-core figure SURVEY.md section 8(d) asks for
+    # the same oracle on ONE thread: the per-core figure SURVEY.md section 8(d) asks for
     po.set_num_threads(1)
-    dt1, n1 = oracle_sample_step(scene, 16)
+    dt1, n1 = oracle_pass(scenes[0], _subset(scenes[0], max(4 * stride, 16)))
     po.set_num_threads(cores)
     return {"value": tot_n / tot_t, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{scene.name}: {passes} passes over every {stride}nd ray ({tot_n:.3g} samples), fp64 forward + adjoint, "
-                      f"{tot_t:.1f} s wall",
+            "sample": f"{name}: {passes} passes over every {stride}th row and column of all {len(scenes)} item(s) "
+                      f"({tot_n:.3g} samples), fp64 forward + adjoint, {tot_t:.1f} s wall",
             "value_1thread": n1 / dt1}
 
 
-def run_reference(args):
-    """--impl reference: the reference arm of this tier is the fp64 CPU oracle on the host cores."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+def run_reference(args, configs):
+    """--impl reference: the reference arm of this tier is the fp64 CPU oracle on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     from oracle import pyoracle as po
-    scene = _scenes(args.config)[0]
-    # size the per-step ray sample so that the whole run stays within ~2 minutes on this box
-    oracle_sample_step(scene, 256)
-    dt, _ = oracle_sample_step(scene, 64)
-    t_full = dt * 64.0
-    stride = int(min(max(np.ceil(t_full * (args.steps + args.warmup) / 120.0), 1), scene.nrays // 8))
+    cfg = configs[-1] if len(configs) == 1 else HEADLINE
+    scenes = _scenes(cfg)
+    # size the per-step ray sample so that the whole run stays within ~100 s on this box
+    stride = _sample_stride(scenes, 100.0, args.steps + args.warmup)
+    subsets = [_subset(sc, stride) for sc in scenes]
+
+    def step():
+        t, n = 0.0, 0
+        for sc, idx in zip(scenes, subsets):
+            dt, nn = oracle_pass(sc, idx)
+            t += dt
+            n += nn
+        return t, n
+
     for _ in range(args.warmup):
-        oracle_sample_step(scene, stride)
+        step()
     tot_t, tot_n = 0.0, 0
     for _ in range(args.steps):
-        dt, n = oracle_sample_step(scene, stride)
+        dt, n = step()
         tot_t += dt
         tot_n += n
     val = tot_n / tot_t
+    sample = f"every {stride}th row and column of all {len(scenes)} item(s) of {_workload_name(cfg)} per step, fwd + adjoint"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(args.config), "sample": f"every {stride}th ray per step"},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": po.num_threads(), "kind": "oracle",
-                             "sample": f"every {stride}th ray of {_workload_name(args.config)} per step, fwd + adjoint"},
+            "config": _config_dict(cfg, scenes, 1),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": po.num_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -181,41 +222,40 @@ def time_kernel_group(fn, stream, torch, flush, reps):
     return tot / reps
 
 
-def run_ours(args):
-    import torch
-    import torch.distributed as dist
-    from paper_2509_03623_b200 import Renderer, binding as B
-    from synth import l2_target
+def _load_traffic():
+    """DRAM bytes per launch from the committed ncu captures (profiles/traffic_r02.json, one entry per config and kernel);
+    configs without a capture report null."""
+    path = os.path.join(ROOT, "profiles", "traffic_r02.json")
+    try:
+        with open(path) as f:
+            return json.load(f)
+    except Exception:      # noqa: BLE001
+        return {}
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the render has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    B.lib()
-    B.radt_set_option(B.OPT_WIN_PATH, args.win_path)
 
-    scenes = _scenes(args.config)
-    R = Renderer(scenes, device=f"cuda:{local}")
+def measure_config(cfg, args, ctx, with_cpu):
+    """All measurements of one config on this rank; rank 0 gets the full dict."""
+    torch, dist, B, Renderer = ctx["torch"], ctx["dist"], ctx["B"], ctx["Renderer"]
+    world, rank, local = ctx["world"], ctx["rank"], ctx["local"]
+    scenes = _scenes(cfg)
+    R = Renderer(scenes, device=f"cuda:{local}", options=dict(win_path=args.win_path))
     stream = torch.cuda.current_stream()
     nominal = sum(s.nominal_samples for s in scenes)
+    d = R.desc
 
-    # target cube of the L2 data term: seed-generated from a first render (an input, built before timing)
+    # target cube of the L2 data term, D = I (1 + 0.05 xi) + sigma eta, sigma = 0.015 max I (DESIGN.md section 3), built from a
+    # first render before timing; drawn on the device (torch Philox, seeded) so that the 2 GB of config 5 take no host time
     R.render()
-    torch.cuda.synchronize()
-    cube0 = R.cube.cpu().numpy()
-    tgt = np.empty_like(cube0)
-    sig = 0.0
-    for b in range(cube0.shape[0]):
-        t, s = l2_target(cube0[b], 36230 + args.config + 97 * rank + b)
-        tgt[b] = t
-        sig = max(sig, s)
+    gen = torch.Generator(device=R.device).manual_seed(36230 + cfg + 97 * rank)
+    sig = 0.015 * float(R.cube.amax())
+    tgt = torch.empty_like(R.cube)
+    for b in range(R.cube.shape[0]):          # item by item: no second cube-sized temporary
+        tgt[b] = R.cube[b] * (1.0 + 0.05 * torch.randn(R.cube[b].shape, generator=gen, device=R.device))
+        tgt[b] += sig * torch.randn(R.cube[b].shape, generator=gen, device=R.device)
     R.set_target(tgt, sig)
+    del tgt
 
-    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=R.device)     # > 126 MB L2
+    flush_buf = ctx["flush_buf"]
 
     def flush():
         flush_buf.fill_(1)
@@ -225,9 +265,10 @@ def run_ours(args):
 
     launches_per_step = 0
     R.render_loss(stream); launches_per_step += B.radt_last_launch_count()
-    R.render_bwd(stream=stream); launches_per_step += B.radt_last_launch_count()
+    R.render_bwd(stream=stream, reuse_setup=True); launches_per_step += B.radt_last_launch_count()
 
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         flush()
         step()
     torch.cuda.synchronize()
@@ -258,86 +299,72 @@ def run_ours(args):
     loss = float(R.loss.cpu())
     ms_step = ms_total / args.steps
     value = world * nominal * args.steps / (ms_total * 1e-3)
-
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
 
     # ---- per-kernel device times (forward march, adjoint march) and work counters
-    reps = max(5, min(args.steps, 30))
+    reps = max(3, min(args.steps, 20 if nominal < 1e11 else 5))
     t_fwd = time_kernel_group(lambda: R.render(stream), stream, torch, flush, reps)
     cnt = R.counters()
     t_fl = time_kernel_group(lambda: R.render_loss(stream), stream, torch, flush, reps)
     t_l2 = time_kernel_group(lambda: R.l2_loss_grad(stream), stream, torch, flush, reps)
-    t_bwd = time_kernel_group(lambda: R.render_bwd(stream=stream), stream, torch, flush, reps)
+    R.render_loss(stream)
+    t_bwd = time_kernel_group(lambda: R.render_bwd(stream=stream, reuse_setup=True), stream, torch, flush, reps)
     cnt_b = R.counters()
+    t_bwd_own = time_kernel_group(lambda: R.render_bwd(stream=stream), stream, torch, flush, reps)
     # the exact shortcut of the paper's fit chain: no march of the steps without opacity
-    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 0)
-    t_bwd_fit = time_kernel_group(lambda: R.render_bwd(stream=stream), stream, torch, flush, reps)
-    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 1)
+    R.set_options(zero_dens_grad=0)
+    R.render_loss(stream)
+    t_bwd_fit = time_kernel_group(lambda: R.render_bwd(stream=stream, reuse_setup=True), stream, torch, flush, reps)
+    R.set_options(zero_dens_grad=1)
+    # without the low-order words (cube_lo = NULL): what the compensation costs
+    Rp = None
+    t_plain = None
+    if nominal < 1e11:
+        Rp = Renderer(scenes, device=f"cuda:{local}", options=dict(win_path=args.win_path), compensated=False)
+        Rp.set_target(R.target, sig)
+        Rp.fit_step(stream)
+        t_plain = time_kernel_group(lambda: Rp.fit_step(stream), stream, torch, flush, reps)
+        del Rp
     fwd_exec = cnt[1] * 32 // 2        # executed samples, 2 MUFU.EX2 lane-ops each
     bwd_exec = cnt_b[3] * 32 // 2      # 2-EX2 equivalents (zero-opacity adjoint samples need one EX2: counted as 1/2)
 
-    # ---- physics pre-pass: T grid -> n_CO, v_phi and its adjoint, timed beside the step
-    prepass = None
-    if scenes[0].grid.kind == 0 and scenes[0].grid.mirror_z and len(scenes) <= 16:
-        from types import SimpleNamespace
-        disks = B.make_disks([SimpleNamespace(gm_star=2.0 * 1.32712440018e26, m_gas=2.37 * 1.66053906660e-24, sigma0=30.0,
-                                              r_c=150.0, gamma=1.0, x_co=1e-4, t_freeze=19.0, n_dissoc=1e21, f_col=0.706)
-                              for _ in scenes])
-        pws = torch.empty(B.radt_disk_workspace_bytes(R.desc), dtype=torch.uint8, device=R.device)
-        pd, pv, pg = torch.empty_like(R.temp), torch.empty_like(R.temp), torch.zeros_like(R.temp)
-        t_pf = time_kernel_group(lambda: B.radt_disk_fields(disks, R.desc, R.temp, pd, pv, pws, stream), stream, torch, flush, reps)
-        t_pb = time_kernel_group(lambda: B.radt_disk_fields_bwd(disks, R.desc, R.temp, R.g_dens, R.g_vel, pg, pws, stream),
-                                 stream, torch, flush, reps)
-        mlp = B.make_mlp(L=4)
-        mp = torch.zeros(B.radt_mlp_num_params(mlp), dtype=torch.float32, device=R.device).uniform_(-0.1, 0.1)
-        mg, mt = torch.empty_like(mp), torch.empty_like(R.temp[0])
-        t_mf = time_kernel_group(lambda: B.radt_mlp_temperature(mlp, R.desc, mp, mt, stream), stream, torch, flush, reps)
-        t_mb = time_kernel_group(lambda: B.radt_mlp_temperature_bwd(mlp, R.desc, mp, pg[0], mg, stream), stream, torch, flush, reps)
-        prepass = {"fwd_ms": t_pf, "bwd_ms": t_pb, "mlp_fwd_ms": t_mf, "mlp_bwd_ms": t_mb,
-                   "what": "radt_disk_fields(_bwd): T grid -> n_CO, v_phi; radt_mlp_temperature(_bwd): parameters -> T grid "
-                           "(one grid); both outside the timed step, each figure includes the host-side enqueue"}
-
-    # ---- roofline: SFU (MUFU.EX2) issue peak measured now, at the clock the GPU runs at
-    mufu_peak, mufu_clk = B.radt_pipe_peak(0)
-    ffma_peak, _ = B.radt_pipe_peak(1)
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.txt")      # one JSON object: DRAM bytes per launch from the ncu capture
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath))
-        except Exception:      # noqa: BLE001
-            traffic = None
+    mufu_peak, ffma_peak, mufu_clk = ctx["mufu_peak"], ctx["ffma_peak"], ctx["mufu_clk"]
+    traffic = ctx["traffic"].get(f"cfg{cfg}", {})
 
     def roof(kernel, t_ms, exec_samples, key, ops, peak, unit, why):
-        """ALGORITHMIC lane-operations of the executed samples (per-sample figure x samples one
-        launch executes) over the launch time, against the issue peak of the pipe that binds, measured in this run."""
+        """ALGORITHMIC lane-operations of the EXECUTED samples (per-sample figure x samples one launch
+        executes) over the launch time, against the issue peak of the pipe that binds, measured in this run."""
         achieved = ops * exec_samples / (t_ms * 1e-3)
         return {"kernel": kernel, "bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": unit,
-                "frac": achieved / peak, "frac_nominal": ops * nominal / (t_ms * 1e-3) / peak,
+                "frac": achieved / peak,
                 "frac_mufu": 2.0 * exec_samples / (t_ms * 1e-3) / mufu_peak,
-                "ops_per_sample": ops, "executed_samples": exec_samples, "ms": t_ms,
+                "speedup_from_skipping": nominal / max(exec_samples, 1),
+                "ops_per_sample": ops, "executed_samples": int(exec_samples), "ms": t_ms,
                 "peak_source": f"{why}, measured by radt_pipe_peak in this run at {mufu_clk:.0f} MHz "
                                "(MEASURED_PEAKS.json holds no SFU/FP32 issue figure)",
-                "traffic": (traffic or {}).get(key)}
+                "traffic": traffic.get(key)}
 
     # forward: 2 MUFU.EX2 + ~8 FP32 per sample -> the SFU pipe (16 lanes/clk/SM) binds before FP32 (128 lanes/clk/SM);
     # adjoint: 2 MUFU.EX2 + ~20 FP32 per sample (SURVEY.md section 8(d)) -> 20/128 > 2/16: FP32 issue binds
     r_f = roof("k_march_fwd (includes the fused setup launch)", t_fwd, fwd_exec, "k_march_fwd", 2.0, mufu_peak,
                "T MUFU lane-op/s", "SFU issue peak (MUFU.EX2)")
-    r_b = roof("k_march_bwd (includes setup and gradient unpack)", t_bwd, bwd_exec, "k_march_bwd", 20.0, ffma_peak,
-               "T FP32 lane-op/s", "FP32 issue peak (FFMA)")
+    r_b = roof("k_march_bwd (adjoint march + gradient unpack, setup reused from the forward)", t_bwd, bwd_exec, "k_march_bwd", 20.0,
+               ffma_peak, "T FP32 lane-op/s", "FP32 issue peak (FFMA)")
     dominant, other = (r_b, r_f) if t_bwd >= t_fwd else (r_f, r_b)
 
-    # ---- e2e: the same step through the HOST-buffer C-ABI entry point, pinned host memory
-    d = R.desc
+    # ---- e2e: the same step through the HOST-buffer C-ABI entry points, pinned host memory
     hf = [torch.from_numpy(h).pin_memory() for h in B.stack_fields(scenes)]
-    ht = torch.from_numpy(np.ascontiguousarray(tgt, np.float32)).pin_memory()
+    ht = torch.empty(R.target.shape, dtype=torch.float32, pin_memory=True)
+    ht.copy_(R.target)
     hg = [torch.empty_like(h).pin_memory() for h in hf]
-    e2e_steps = max(3, min(args.steps, 50))
-    for _ in range(max(args.warmup, 10)):      # the stream-ordered pool and the copy engines need a few calls to settle
+    hc = torch.empty(R.cube.shape, dtype=torch.float32, pin_memory=True)
+    nvox = R.cube.numel()
+    del R
+    torch.cuda.empty_cache()
+    big = nominal > 1e10
+    e2e_steps = max(3, min(args.steps, 5 if big else 50))
+    for _ in range(2 if big else max(args.warmup, 10)):      # the arena and the copy engines need a few calls to settle
         B.radt_fit_step_host(d, *[h.numpy() for h in hf], ht.numpy(), sig, None, *[g.numpy() for g in hg])
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -347,30 +374,118 @@ def run_ours(args):
     e2e_t = (time.perf_counter() - t0) / e2e_steps
     h2d = sum(h.numel() * 4 for h in hf) + ht.numel() * 4
     d2h = sum(g.numel() * 4 for g in hg) + 8
+    for _ in range(2):
+        B.radt_render_host(d, *[h.numpy() for h in hf], hc.numpy())
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        B.radt_render_host(d, *[h.numpy() for h in hf], hc.numpy())
+    e2e_r = (time.perf_counter() - t0) / e2e_steps
+    del ht, hc
 
-    cpu = cpu_baseline(scenes[0]) if world == 1 and not args.no_cpu_baseline else None
+    cpu = cpu_baseline(scenes, _workload_name(cfg)) if with_cpu else None
 
-    line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic",
-        "config": {"workload": _workload_name(args.config), "rays": int(sum(s.nrays for s in scenes)),
-                   "channels": d.nchan, "steps_per_ray": d.nstep, "grid": list(d.grid_shape),
-                   "nominal_samples_per_step": int(nominal), "parallelism": f"independent disks x{world}",
-                   "l2": "flushed between timed steps (256 MiB fill outside the events)",
-                   "kernels": "window (uniform channel lattice)" if args.win_path else "channel table"},
-        "fwd_value": nominal / (t_fwd * 1e-3), "fwd_ms": t_fwd, "fwd_loss_fused_ms": t_fl, "l2_ms": t_l2, "bwd_ms": t_bwd,
-        "bwd_ms_zero_dens_grad_off": t_bwd_fit,
+    return {
+        "config": _config_dict(cfg, scenes, world), "value": value, "unit": UNIT, "steps": args.steps, "warmup": warm,
+        "ms_per_step": ms_step, "fwd_value": nominal / (t_fwd * 1e-3),
+        "fwd_ms": t_fwd, "fwd_loss_fused_ms": t_fl, "l2_ms": t_l2, "bwd_ms": t_bwd, "bwd_ms_own_setup": t_bwd_own,
+        "bwd_ms_zero_dens_grad_off": t_bwd_fit, "step_ms_without_cube_lo": t_plain,
         "executed_samples": {"fwd": int(fwd_exec), "bwd": int(bwd_exec), "fwd_active_ray_steps": int(cnt[0]),
-                             "bwd_active_ray_steps": int(cnt_b[2]), "nominal": int(nominal)},
-        "prepass": prepass,
+                             "bwd_active_ray_steps": int(cnt_b[2]), "nominal": int(nominal),
+                             "fwd_executed_over_nominal": fwd_exec / nominal},
         "roofline": dominant, "roofline_other": other,
-        "pipe_peaks": {"mufu_lane_ops_per_s": mufu_peak, "ffma_lane_ops_per_s": ffma_peak, "sm_mhz": mufu_clk},
-        "cpu_baseline": cpu,
         "e2e": {"value": nominal / e2e_t, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                "ms_per_step": 1e3 * e2e_t, "api": "radt_fit_step_host (pinned host buffers)"},
-        "gpu_launches": int(launches_per_step * args.steps),
-        "clocks": clocks, "loss": loss, "wall_s": t_wall,
+                "ms_per_step": 1e3 * e2e_t, "steps": e2e_steps, "api": "radt_fit_step_host (pinned host buffers)"},
+        "e2e_render": {"value": nominal / e2e_r, "unit": "samples/s (forward only)", "h2d_bytes_per_step": int(sum(h.numel() * 4 for h in hf)),
+                       "d2h_bytes_per_step": int(nvox * 4), "ms_per_step": 1e3 * e2e_r, "api": "radt_render_host (cube D2H inside)"},
+        "gpu_launches": int(launches_per_step * args.steps), "launches_per_step": int(launches_per_step),
+        "clocks": clocks, "loss": loss, "wall_s": t_wall, "cpu_baseline": cpu,
+    }
+
+
+def prepass_times(ctx, args):
+    """Physics pre-pass and MLP field on the config-2 grid, timed beside the step."""
+    from types import SimpleNamespace
+    torch, B, Renderer = ctx["torch"], ctx["B"], ctx["Renderer"]
+    scenes = _scenes(2)
+    R = Renderer(scenes, device=f"cuda:{ctx['local']}")
+    stream = torch.cuda.current_stream()
+    R.render(); R.dl_dcube.fill_(1e-9); R.render_bwd()
+
+    def flush():
+        ctx["flush_buf"].fill_(1)
+    reps = 10
+    disks = B.make_disks([SimpleNamespace(gm_star=2.0 * 1.32712440018e26, m_gas=2.37 * 1.66053906660e-24, sigma0=30.0,
+                                          r_c=150.0, gamma=1.0, x_co=1e-4, t_freeze=19.0, n_dissoc=1e21, f_col=0.706)
+                          for _ in scenes])
+    pws = torch.empty(B.radt_disk_workspace_bytes(R.desc), dtype=torch.uint8, device=R.device)
+    pd, pv, pg = torch.empty_like(R.temp), torch.empty_like(R.temp), torch.zeros_like(R.temp)
+    t_pf = time_kernel_group(lambda: B.radt_disk_fields(disks, R.desc, R.temp, pd, pv, pws, stream), stream, torch, flush, reps)
+    t_pb = time_kernel_group(lambda: B.radt_disk_fields_bwd(disks, R.desc, R.temp, R.g_dens, R.g_vel, pg, pws, stream),
+                             stream, torch, flush, reps)
+    mlp = B.make_mlp(L=4)
+    mp = torch.zeros(B.radt_mlp_num_params(mlp), dtype=torch.float32, device=R.device).uniform_(-0.1, 0.1)
+    mg, mt = torch.empty_like(mp), torch.empty_like(R.temp[0])
+    t_mf = time_kernel_group(lambda: B.radt_mlp_temperature(mlp, R.desc, mp, mt, stream), stream, torch, flush, reps)
+    t_mb = time_kernel_group(lambda: B.radt_mlp_temperature_bwd(mlp, R.desc, mp, pg[0], mg, stream), stream, torch, flush, reps)
+    return {"grid": "config 2 (256 x 128)", "fwd_ms": t_pf, "bwd_ms": t_pb, "mlp_fwd_ms": t_mf, "mlp_bwd_ms": t_mb,
+            "what": "radt_disk_fields(_bwd): T grid -> n_CO, v_phi; radt_mlp_temperature(_bwd): parameters -> T grid "
+                    "(one grid); both outside the timed step, each figure includes the host-side enqueue"}
+
+
+def run_ours(args, configs):
+    import torch
+    import torch.distributed as dist
+    from paper_2509_03623_b200 import Renderer, binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the render has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+    ctx = {"torch": torch, "dist": dist, "B": B, "Renderer": Renderer, "world": world, "rank": rank, "local": local,
+           "flush_buf": torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}"),     # > 126 MB L2
+           "traffic": _load_traffic()}
+    # roofline denominators: issue peaks measured now, at the clock the GPU runs at
+    ctx["mufu_peak"], ctx["mufu_clk"] = B.radt_pipe_peak(0)
+    ctx["ffma_peak"], _ = B.radt_pipe_peak(1)
+
+    head = configs[0] if len(configs) == 1 else (HEADLINE if HEADLINE in configs else configs[-1])
+    results = {}
+    t_start = time.perf_counter()
+    for cfg in configs:
+        t0 = time.perf_counter()
+        res = measure_config(cfg, args, ctx, with_cpu=(cfg == head and world == 1 and not args.no_cpu_baseline))
+        if res is not None:
+            res["bench_wall_s"] = time.perf_counter() - t0
+            results[cfg] = res
+        torch.cuda.empty_cache()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    prepass = prepass_times(ctx, args) if (world == 1 and not args.no_prepass) else None
+
+    H = results[head]
+    keep = ("config", "value", "ms_per_step", "steps", "fwd_value", "fwd_ms", "fwd_loss_fused_ms", "l2_ms", "bwd_ms",
+            "bwd_ms_own_setup", "bwd_ms_zero_dens_grad_off", "step_ms_without_cube_lo", "executed_samples", "roofline",
+            "roofline_other", "e2e", "e2e_render", "launches_per_step", "clocks", "bench_wall_s")
+    per_config = [{k: results[c][k] for k in keep} for c in configs]
+    line = {
+        "metric": METRIC, "value": H["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": H["warmup"],
+        "ms_per_step": H["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": H["config"],
+        "fwd_value": H["fwd_value"], "fwd_ms": H["fwd_ms"], "fwd_loss_fused_ms": H["fwd_loss_fused_ms"], "bwd_ms": H["bwd_ms"],
+        "executed_samples": H["executed_samples"],
+        "roofline": H["roofline"], "roofline_other": H["roofline_other"],
+        "pipe_peaks": {"mufu_lane_ops_per_s": ctx["mufu_peak"], "ffma_lane_ops_per_s": ctx["ffma_peak"], "sm_mhz": ctx["mufu_clk"]},
+        "cpu_baseline": H["cpu_baseline"], "e2e": H["e2e"], "e2e_render": H["e2e_render"],
+        "gpu_launches": H["gpu_launches"], "clocks": H["clocks"], "loss": H["loss"], "wall_s": H["wall_s"],
+        "kernels": "window (uniform channel lattice)" if args.win_path else "channel table",
+        "per_config": per_config, "prepass": prepass, "bench_total_wall_s": time.perf_counter() - t_start,
         "context": "paper: ~10,000x vs RADMC-3D, ~100 ms per cube, A6000 vs Xeon Gold 6348 (PAPER.md:302-304); another machine and workload",
     }
     print(json.dumps(line), flush=True)
@@ -381,22 +496,30 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=2, help="SURVEY.md config 1..5 (BASELINE.json configs[k-1]); 6 = spherical 512x96x256 grid at 256x256 px, the shape "
-                         "of the paper's own timing benchmark")
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=None, help="measure ONE config (1..5 = BASELINE.json configs[k-1]; 6 = spherical "
+                    "512x96x256 grid at 256x256 px, the shape of the paper's own timing benchmark); default: all, headline 5")
+    ap.add_argument("--configs", type=str, default=None, help="comma-separated subset, e.g. 2,3,5")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-prepass", action="store_true")
     ap.add_argument("--win-path", type=int, default=1, choices=[0, 1],
-                    help="RADT_OPT_WIN_PATH: 1 = window kernels on uniform channel lattices (default), 0 = channel-table kernels")
+                    help="radt_options.win_path: 1 = window kernels on uniform channel lattices (default), 0 = channel-table kernels")
     ap.add_argument("--sph-npix", type=int, default=256, help="config 6: image size (the paper sweeps it at 20 channels)")
     ap.add_argument("--sph-nchan", type=int, default=64, help="config 6: channels of 0.1 km/s (the paper sweeps them at 256 px)")
     args = ap.parse_args()
     _SPH.update(npix=args.sph_npix, nchan=args.sph_nchan)
-    if args.impl == "reference":
-        run_reference(args)
+    if args.config is not None:
+        configs = [args.config]
+    elif args.configs:
+        configs = [int(c) for c in args.configs.split(",")]
     else:
-        run_ours(args)
+        configs = list(ALL_CONFIGS)
+    if args.impl == "reference":
+        run_reference(args, configs)
+    else:
+        run_ours(args, configs)
 
 
 if __name__ == "__main__":

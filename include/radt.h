@@ -20,8 +20,10 @@
  *   - arrays are C-contiguous, last index fastest: axisymmetric grids [b][ir][izeta], 3-D grids
  *     [b][ix][iy][iz], cubes [b][iy][ix][channel];
  *   - return value 0 on success, a negative RADT_E_* code otherwise; radt_last_error() returns a
- *     thread-local message.  Numerical conditions are not errors: T is clamped to >= 1 K (zero
- *     gradient through the clamp), NaN inputs propagate.
+ *     thread-local message.  Numerical conditions are not errors: the temperature is clamped to
+ *     [1 K, 16384 K] (the range of the device partition-function table; zero gradient through either
+ *     clamp; a NaN temperature counts as below the clamp, i.e. 1 K); NaN densities and velocities
+ *     propagate into the cube.
  *   - there is no CPU fallback and no other back-end: without a CUDA device every compute entry
  *     point fails with RADT_E_CUDA.
  */
@@ -35,7 +37,7 @@
 extern "C" {
 #endif
 
-#define RADT_VERSION 100          /* 0.1.0 */
+#define RADT_VERSION 200          /* 0.2.0: per-call radt_options, cube_lo, packed-gradient access */
 #define RADT_MAX_LEVELS 64        /* partition-function table length limit */
 #define RADT_MAX_CHANNELS 256     /* channels per render call */
 
@@ -116,33 +118,36 @@ typedef struct radt_grid {
 int radt_version(void);
 const char *radt_last_error(void);
 
-/* Run-time options (process-wide; for measurements).  Keys: */
-enum {
-    RADT_OPT_WINDOW = 1,          /* 1 (default): skip channel groups outside the +-6.4 alpha line window; 0: dense */
-    RADT_OPT_SKIP_EMPTY = 2,      /* 1 (default): skip steps with zero opacity in the forward march; 0: dense */
-    RADT_OPT_COMPENSATED = 4,     /* 0 (default) / 1: the forward also keeps, per voxel, the low-order word of its fp32 sum in
-                                     the workspace (8 bytes per voxel more: query radt_workspace_bytes under the same
-                                     setting) and the adjoint, given THE SAME workspace, uses it to form the residual
-                                     intensity without cancellation noise: gradients on rays that are optically thick
-                                     in every channel improve from ~1e-3 to ~1e-6 of the maximum.
-                                     A different or overwritten workspace falls back to the plain difference, voxel by
-                                     voxel.  Window kernels only. */
-    RADT_OPT_ZERO_DENS_GRAD = 5,  /* 1 (default): exact gradient; 0: the adjoint skips steps without opacity on LINEAR density
-                                     grids.  Those steps carry only dL/dn of cells whose density is exactly zero (masked
-                                     CO, Eq. 9), which a fit through radt_disk_fields_bwd discards anyway (the
-                                     mask is held fixed), so g_temp, g_vel and g_dens at cells with non-zero density are
-                                     unchanged; g_dens at zero-density cells then only holds what emitting steps
-                                     contribute.  They are 48-65 % of the adjoint's steps on the disk configs. */
-    RADT_OPT_WIN_PATH = 3         /* 1 (default): channel tables that are uniform lattices v_0 + c dv use the window
-                                     kernels (one channel per lane inside the line window); 0: always the
-                                     channel-table kernels.  radt_render and radt_render_bwd of one cube must run
-                                     under the same setting. */
-};
-int radt_set_option(int key, int value);
-int radt_get_option(int key);
+/* Per-call options.  Every compute entry point takes a `const radt_options *` (HOST; NULL = the defaults that
+ * radt_options_default writes).  There is no process-wide state: two threads may render with different options.
+ * radt_render (or radt_render_loss) and the radt_render_bwd that differentiates its cube must be called with the same
+ * window / skip_empty / win_path and the same cube_lo choice, because the adjoint re-marches the ray with the very
+ * arithmetic of the forward; the library remembers, per cube pointer, the options of the last
+ * forward that wrote it and radt_render_bwd fails with RADT_E_INVALID when they differ. */
+typedef struct radt_options {
+    uint32_t struct_size;         /* = sizeof(radt_options) */
+    int32_t window;               /* 1 (default): channels outside the line window of a step (dtau < 2^-60 .. 2^-40 of its
+                                     line-centre value) are skipped; 0: every channel of every step (dense) */
+    int32_t skip_empty;           /* 1 (default): steps with zero opacity are skipped in the forward; 0: dense */
+    int32_t win_path;             /* 1 (default): channel tables that are uniform lattices v_0 + c dv use the window kernels
+                                     (one channel per lane inside the line window); 0: always the channel-table kernels */
+    int32_t zero_dens_grad;       /* 1 (default): exact gradient; 0: the adjoint skips steps without opacity on LINEAR
+                                     density grids.  Those steps carry only dL/dn of cells whose density is exactly zero
+                                     (masked CO, Eq. 9), which a fit through radt_disk_fields_bwd discards anyway
+                                     (the mask is held fixed), so g_temp, g_vel and g_dens at cells with non-zero density
+                                     are unchanged.  They are 48-65 % of the adjoint's steps on the disk configs. */
+    int32_t reuse_setup;          /* radt_render_bwd only.  0 (default): the call rebuilds ray table, Q(T) table, packed
+                                     fields and occupancy words in the workspace.  1: the caller states that `ws` was last
+                                     used by radt_render / radt_render_loss with the same geom, line, grid (same field
+                                     pointers AND unchanged field values) and options; the adjoint then reuses what that
+                                     call left there.  The library checks what it can (descriptors, pointers, options,
+                                     remembered per workspace pointer) and fails with RADT_E_INVALID otherwise. */
+} radt_options;
+void radt_options_default(radt_options *opt);
 
 /* Bytes of DEVICE workspace needed by radt_render (pass = RADT_PASS_FWD) or radt_render_bwd
- * (RADT_PASS_BWD) for `batch` items.  HOST pointers in, size out. */
+ * (RADT_PASS_BWD) for `batch` items.  The size does not depend on the options; a RADT_PASS_BWD workspace also
+ * serves the forward (same layout, the gradient cells come last).  HOST pointers in, size out. */
 int radt_workspace_bytes(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                          int32_t pass, size_t *bytes_out);
 
@@ -154,19 +159,35 @@ int radt_ray_geometry(const radt_geom *geom, const radt_grid *grid, int32_t batc
 
 /* Forward render (O1-O10; Eq. 11-17).  Overwrites
  * cube [batch][ny][nx][nchan] (DEVICE float32, rays that miss write zeros).  geom: HOST [batch];
- * line, grid: HOST structs; ws: DEVICE workspace of ws_bytes.  Asynchronous on cuda_stream. */
+ * line, grid, opt: HOST structs; ws: DEVICE workspace of ws_bytes.  Asynchronous on cuda_stream.
+ * cube_lo (DEVICE float32, same shape as cube, or NULL): the low-order word of the fp32 sum behind every voxel,
+ * cube + cube_lo being that sum to about twice the precision.  Pass it on to radt_render_bwd: the adjoint forms the
+ * residual intensity behind a step as (cube - P_k) + (cube_lo - P_lo,k), free of the cancellation noise that a ray
+ * which is optically thick in every channel would otherwise put on its gradients.  `cube` is
+ * the same bit for bit with and without it. */
 int radt_render(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                float *cube, void *ws, size_t ws_bytes, void *cuda_stream);
+                const radt_options *opt, float *cube, float *cube_lo, void *ws, size_t ws_bytes, void *cuda_stream);
 
-/* Adjoint (O11; Fig. 2 E).  Given the forward output `cube` and
- * dl_dcube = dLoss/dcube (both DEVICE float32 [batch][ny][nx][nchan]) OVERWRITES g_dens, g_temp,
- * g_vel (DEVICE float32, grid-shaped incl. batch with the grid's batch_stride; any may be NULL) with
+/* Adjoint (O11; Fig. 2 E).  Given the forward output `cube` (and `cube_lo` if the
+ * forward wrote one, else NULL) and dl_dcube = dLoss/dcube (all DEVICE float32 [batch][ny][nx][nchan]) OVERWRITES
+ * g_dens, g_temp, g_vel (DEVICE float32, grid-shaped incl. batch with the grid's batch_stride; any may be NULL) with
  * dLoss/d(stored grid value): d/d(ln n) for RADT_DENS_LN, d/d(delta) for RADT_VEL_KEPLER_FRAC.
  * Memory-free: no per-step activations are stored; the rays are re-marched.  Float atomics make
- * the last bits order-dependent. */
+ * the last bits order-dependent.  With all three outputs NULL the gradient stays in the workspace as packed cells
+ * (radt_grad_layout), e.g. for ONE all-reduce over ranks before radt_unpack_grad. */
 int radt_render_bwd(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                    const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel,
-                    void *ws, size_t ws_bytes, void *cuda_stream);
+                    const radt_options *opt, const float *cube, const float *cube_lo, const float *dl_dcube,
+                    float *g_dens, float *g_temp, float *g_vel, void *ws, size_t ws_bytes, void *cuda_stream);
+
+/* Where radt_render_bwd leaves the gradient inside a RADT_PASS_BWD workspace: [batch][cells] packed float4 cells
+ * {dL/d dens, dL/d temp, dL/d vel, 0}, *nfloat_out floats starting *offset_out bytes into `ws` (HOST outputs).
+ * Multi-GPU image sharding sums exactly this range over the ranks with one all-reduce on the
+ * adjoint's stream and then calls radt_unpack_grad. */
+int radt_grad_layout(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                     size_t *offset_out, size_t *nfloat_out);
+/* Packed cells of `ws` -> the caller's three planes (DEVICE float32, grid's batch_stride; any may be NULL). */
+int radt_unpack_grad(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                     const void *ws, size_t ws_bytes, float *g_dens, float *g_temp, float *g_vel, void *cuda_stream);
 
 /* L2 data term used by the configs (chi^2 of PAPER.md:79, 252):
  * L = 1/(2 n) sum ((cube - target)/sigma)^2, dl_dcube = (cube - target)/(sigma^2 n).
@@ -175,27 +196,29 @@ int radt_l2_loss_grad(const float *cube, const float *target, double sigma, int6
                       double *loss_out, void *cuda_stream);
 
 /* Forward render with the chi^2 data term fused into its epilogue (the step after the render in
- * the paper's fit, Fig. 2 D): writes cube as radt_render does and, without a second pass
- * over it, dl_dcube = (cube - target) / (sigma^2 n) and *loss_out = sum (cube - target)^2 / (2 sigma^2 n), n = number
- * of voxels of the whole batch.  Same results as radt_render followed by radt_l2_loss_grad (the loss up to the
- * order of its fp64 sum).  target, cube, dl_dcube: DEVICE float32 [batch][ny][nx][nchan]; loss_out: DEVICE double[1]. */
+ * the paper's fit, Fig. 2 D): writes cube (and cube_lo) as radt_render does and, without a
+ * second pass over it, dl_dcube = (cube - target) / (sigma^2 n) and *loss_out = sum (cube - target)^2 / (2 sigma^2 n),
+ * n = number of voxels of the whole batch.  Same results as radt_render followed by radt_l2_loss_grad (the loss up to
+ * the order of its fp64 sum).  target, cube, cube_lo, dl_dcube: DEVICE float32 [batch][ny][nx][nchan]; loss_out:
+ * DEVICE double[1]. */
 int radt_render_loss(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                     const float *target, double sigma, float *cube, float *dl_dcube, double *loss_out, void *ws,
-                     size_t ws_bytes, void *cuda_stream);
+                     const radt_options *opt, const float *target, double sigma, float *cube, float *cube_lo,
+                     float *dl_dcube, double *loss_out, void *ws, size_t ws_bytes, void *cuda_stream);
 
-/* Same operations with HOST buffers (grid->dens/temp/vel, cube, dl_dcube, g_* are HOST pointers).
+/* Same operations with HOST buffers (grid->dens/temp/vel, cube, cube_lo, dl_dcube, g_* are HOST pointers).
  * Device memory comes from an arena the library keeps per calling thread and device (grown on demand, never
  * returned); the work runs on stream 0 of the current device and the call returns after the results are in host
- * memory. */
+ * memory.  cube_lo may be NULL in both calls that take it. */
 int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                     float *cube);
-/* Forward + L2 loss against `target` (HOST; uploaded on a second stream under the forward march) + adjoint in one
- * call; cube may be NULL. */
+                     const radt_options *opt, float *cube, float *cube_lo);
+/* Forward + chi^2 term against `target` (HOST; uploaded on a second stream under the forward march) + adjoint in one
+ * call; the low-order words stay on the device; cube may be NULL. */
 int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                       const float *target, double sigma, float *cube, double *loss_out,
+                       const radt_options *opt, const float *target, double sigma, float *cube, double *loss_out,
                        float *g_dens, float *g_temp, float *g_vel);
 int radt_render_bwd_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                         const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel);
+                         const radt_options *opt, const float *cube, const float *cube_lo, const float *dl_dcube,
+                         float *g_dens, float *g_temp, float *g_vel);
 
 /* ---- Physics pre-pass (Eq. 1-2, 6-9) ---------------------------------
  * Turns a temperature grid into the render's CO density and v_phi grids, as the paper's fit does before every render:

@@ -16,10 +16,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libradt.so")
 
 PASS_FWD, PASS_BWD = 0, 1
-OPT_WINDOW, OPT_SKIP_EMPTY, OPT_WIN_PATH, OPT_COMPENSATED, OPT_ZERO_DENS_GRAD = 1, 2, 3, 4, 5
 
-EXPORTS = ["radt_version", "radt_last_error", "radt_set_option", "radt_get_option", "radt_workspace_bytes",
-           "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_l2_loss_grad", "radt_render_host",
+EXPORTS = ["radt_version", "radt_last_error", "radt_options_default", "radt_workspace_bytes",
+           "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_grad_layout", "radt_unpack_grad",
+           "radt_l2_loss_grad", "radt_render_host",
            "radt_render_loss", "radt_disk_workspace_bytes", "radt_disk_fields", "radt_disk_fields_bwd",
            "radt_mlp_num_params", "radt_mlp_temperature", "radt_mlp_temperature_bwd",
            "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
@@ -51,7 +51,27 @@ class radt_grid(C.Structure):
                 ("batch_stride", C.c_int64), ("dens", C.c_void_p), ("temp", C.c_void_p), ("vel", C.c_void_p)]
 
 
+class radt_options(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("window", C.c_int32), ("skip_empty", C.c_int32), ("win_path", C.c_int32),
+                ("zero_dens_grad", C.c_int32), ("reuse_setup", C.c_int32)]
+
+
 _lib = None
+
+
+def make_options(**kw):
+    """radt_options with the library's defaults (radt_options_default), fields overridden by keyword."""
+    o = radt_options()
+    lib().radt_options_default(C.byref(o))
+    for k, v in kw.items():
+        if k not in ("window", "skip_empty", "win_path", "zero_dens_grad", "reuse_setup"):
+            raise KeyError(f"unknown radt_options field {k!r}")
+        setattr(o, k, int(v))
+    return o
+
+
+def _optp(opt):
+    return C.byref(opt) if opt is not None else None
 
 
 class radt_disk(C.Structure):
@@ -91,23 +111,26 @@ def lib():
         gp, lp, rp = C.POINTER(radt_geom), C.POINTER(radt_line), C.POINTER(radt_grid)
         L.radt_version.restype = C.c_int
         L.radt_last_error.restype = C.c_char_p
-        L.radt_set_option.argtypes = [C.c_int, C.c_int]
-        L.radt_get_option.argtypes = [C.c_int]
+        op = C.POINTER(radt_options)
+        L.radt_options_default.argtypes = [op]
+        L.radt_options_default.restype = None
         L.radt_workspace_bytes.argtypes = [gp, lp, rp, i32, i32, C.POINTER(C.c_size_t)]
         L.radt_ray_geometry.argtypes = [gp, rp, i32, vp, vp]
-        L.radt_render.argtypes = [gp, lp, rp, i32, vp, vp, C.c_size_t, vp]
-        L.radt_render_bwd.argtypes = [gp, lp, rp, i32, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        L.radt_render.argtypes = [gp, lp, rp, i32, op, vp, vp, vp, C.c_size_t, vp]
+        L.radt_render_bwd.argtypes = [gp, lp, rp, i32, op, vp, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        L.radt_grad_layout.argtypes = [gp, lp, rp, i32, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
+        L.radt_unpack_grad.argtypes = [gp, lp, rp, i32, vp, C.c_size_t, vp, vp, vp, vp]
         L.radt_l2_loss_grad.argtypes = [vp, vp, dbl, i64, vp, vp, vp]
-        L.radt_render_loss.argtypes = [gp, lp, rp, i32, vp, dbl, vp, vp, vp, vp, C.c_size_t, vp]
-        L.radt_render_host.argtypes = [gp, lp, rp, i32, vp]
+        L.radt_render_loss.argtypes = [gp, lp, rp, i32, op, vp, dbl, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        L.radt_render_host.argtypes = [gp, lp, rp, i32, op, vp, vp]
         L.radt_mlp_num_params.argtypes = [C.POINTER(radt_mlp), C.POINTER(C.c_int64)]
         L.radt_mlp_temperature.argtypes = [C.POINTER(radt_mlp), rp, vp, vp, vp]
         L.radt_mlp_temperature_bwd.argtypes = [C.POINTER(radt_mlp), rp, vp, vp, vp, vp]
         L.radt_disk_workspace_bytes.argtypes = [rp, i32, C.POINTER(C.c_size_t)]
         L.radt_disk_fields.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_disk_fields_bwd.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, vp, C.c_size_t, vp]
-        L.radt_fit_step_host.argtypes = [gp, lp, rp, i32, vp, dbl, vp, C.POINTER(dbl), vp, vp, vp]
-        L.radt_render_bwd_host.argtypes = [gp, lp, rp, i32, vp, vp, vp, vp, vp]
+        L.radt_fit_step_host.argtypes = [gp, lp, rp, i32, op, vp, dbl, vp, C.POINTER(dbl), vp, vp, vp]
+        L.radt_render_bwd_host.argtypes = [gp, lp, rp, i32, op, vp, vp, vp, vp, vp, vp]
         L.radt_pipe_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
         L.radt_read_counters.argtypes = [vp, C.POINTER(C.c_uint64), vp]
         L.radt_last_launch_count.restype = C.c_int
@@ -167,11 +190,31 @@ def stack_fields(scenes):
                  for f in ("dens", "temp", "vel"))
 
 
-def _stream_ptr(stream):
+class _on:
+    """Make the tensor's device current for the duration of a C-ABI call: the library launches on the CURRENT device,
+    so a Renderer on cuda:1 must not run its kernels on cuda:0 against cuda:1 pointers."""
+
+    def __init__(self, t):
+        import torch
+        self._ctx = torch.cuda.device(t.device)
+
+    def __enter__(self):
+        return self._ctx.__enter__()
+
+    def __exit__(self, *a):
+        return self._ctx.__exit__(*a)
+
+
+def _stream_ptr(stream, like=None):
+    """Pointer of `stream`, or of the current stream of the device that holds tensor `like`."""
     import torch
     if stream is None:
-        stream = torch.cuda.current_stream()
+        stream = torch.cuda.current_stream(like.device if like is not None else None)
     return C.c_void_p(stream.cuda_stream)
+
+
+def _p(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
 
 
 # ------------------------------------------------------------------------------------------------
@@ -179,14 +222,6 @@ def _stream_ptr(stream):
 # ------------------------------------------------------------------------------------------------
 def radt_version() -> int:
     return lib().radt_version()
-
-
-def radt_set_option(key: int, value: int):
-    _check(lib().radt_set_option(key, value))
-
-
-def radt_get_option(key: int) -> int:
-    return lib().radt_get_option(key)
 
 
 def radt_workspace_bytes(desc: Descriptors, pass_: int) -> int:
@@ -197,41 +232,56 @@ def radt_workspace_bytes(desc: Descriptors, pass_: int) -> int:
 
 def radt_ray_geometry(desc: Descriptors, rays_out, stream=None):
     """rays_out: CUDA float64 tensor [batch, ny, nx, 2]."""
-    _check(lib().radt_ray_geometry(desc.geom, C.byref(desc.grid), desc.batch, C.c_void_p(rays_out.data_ptr()),
-                                   _stream_ptr(stream)))
+    with _on(rays_out):
+        _check(lib().radt_ray_geometry(desc.geom, C.byref(desc.grid), desc.batch, _p(rays_out), _stream_ptr(stream, rays_out)))
 
 
-def radt_render(desc: Descriptors, dens, temp, vel, cube, ws, stream=None):
-    """dens/temp/vel: CUDA float32 tensors [batch, *grid]; cube: CUDA float32 [batch, ny, nx, nchan]; ws: CUDA uint8."""
+def radt_render(desc: Descriptors, dens, temp, vel, cube, ws, stream=None, opt=None, cube_lo=None):
+    """dens/temp/vel: CUDA float32 tensors [batch, *grid]; cube (and cube_lo, optional): CUDA float32 [batch, ny, nx, nchan];
+    ws: CUDA uint8; opt: radt_options or None (defaults)."""
     desc.with_fields(dens.data_ptr(), temp.data_ptr(), vel.data_ptr())
-    _check(lib().radt_render(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, C.c_void_p(cube.data_ptr()),
-                             C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(stream)))
+    with _on(cube):
+        _check(lib().radt_render(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _optp(opt), _p(cube),
+                                 _p(cube_lo), _p(ws), ws.numel(), _stream_ptr(stream, cube)))
 
 
-def radt_render_bwd(desc: Descriptors, dens, temp, vel, cube, dl_dcube, g_dens, g_temp, g_vel, ws, stream=None):
+def radt_render_bwd(desc: Descriptors, dens, temp, vel, cube, dl_dcube, g_dens, g_temp, g_vel, ws, stream=None, opt=None,
+                    cube_lo=None):
     desc.with_fields(dens.data_ptr(), temp.data_ptr(), vel.data_ptr())
+    with _on(cube):
+        _check(lib().radt_render_bwd(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _optp(opt), _p(cube),
+                                     _p(cube_lo), _p(dl_dcube), _p(g_dens), _p(g_temp), _p(g_vel), _p(ws), ws.numel(),
+                                     _stream_ptr(stream, cube)))
 
-    def p(t):
-        return C.c_void_p(t.data_ptr()) if t is not None else None
-    _check(lib().radt_render_bwd(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, p(cube), p(dl_dcube),
-                                 p(g_dens), p(g_temp), p(g_vel), C.c_void_p(ws.data_ptr()), ws.numel(),
-                                 _stream_ptr(stream)))
+
+def radt_grad_layout(desc: Descriptors):
+    """(byte offset, number of floats) of the packed gradient cells inside a PASS_BWD workspace."""
+    off, n = C.c_size_t(0), C.c_size_t(0)
+    _check(lib().radt_grad_layout(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, C.byref(off), C.byref(n)))
+    return off.value, n.value
+
+
+def radt_unpack_grad(desc: Descriptors, ws, g_dens, g_temp, g_vel, stream=None):
+    with _on(ws):
+        _check(lib().radt_unpack_grad(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _p(ws), ws.numel(),
+                                      _p(g_dens), _p(g_temp), _p(g_vel), _stream_ptr(stream, ws)))
 
 
 def radt_l2_loss_grad(cube, target, sigma: float, dl_dcube, loss_out, stream=None):
     """loss_out: CUDA float64 tensor [1]."""
-    _check(lib().radt_l2_loss_grad(C.c_void_p(cube.data_ptr()), C.c_void_p(target.data_ptr()), float(sigma),
-                                   cube.numel(), C.c_void_p(dl_dcube.data_ptr()), C.c_void_p(loss_out.data_ptr()),
-                                   _stream_ptr(stream)))
+    with _on(cube):
+        _check(lib().radt_l2_loss_grad(_p(cube), _p(target), float(sigma), cube.numel(), _p(dl_dcube), _p(loss_out),
+                                       _stream_ptr(stream, cube)))
 
 
-def radt_render_loss(desc: Descriptors, dens, temp, vel, target, sigma: float, cube, dl_dcube, loss_out, ws, stream=None):
+def radt_render_loss(desc: Descriptors, dens, temp, vel, target, sigma: float, cube, dl_dcube, loss_out, ws, stream=None,
+                     opt=None, cube_lo=None):
     """Forward render with the fused chi^2 data term: cube, dl_dcube, loss_out (CUDA float64 [1]) in one pass."""
     desc.with_fields(dens.data_ptr(), temp.data_ptr(), vel.data_ptr())
-    _check(lib().radt_render_loss(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch,
-                                  C.c_void_p(target.data_ptr()), C.c_double(float(sigma)), C.c_void_p(cube.data_ptr()),
-                                  C.c_void_p(dl_dcube.data_ptr()), C.c_void_p(loss_out.data_ptr()),
-                                  C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream_ptr(stream)))
+    with _on(cube):
+        _check(lib().radt_render_loss(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _optp(opt), _p(target),
+                                      C.c_double(float(sigma)), _p(cube), _p(cube_lo), _p(dl_dcube), _p(loss_out), _p(ws),
+                                      C.c_size_t(ws.numel()), _stream_ptr(stream, cube)))
 
 
 def radt_disk_workspace_bytes(desc: Descriptors) -> int:
@@ -242,17 +292,16 @@ def radt_disk_workspace_bytes(desc: Descriptors) -> int:
 
 def radt_disk_fields(disks, desc: Descriptors, temp, dens_out, vel_out, ws, stream=None):
     """Physics pre-pass: temp -> n_CO, v_phi (CUDA float32 tensors [batch, nr, nzeta]); disks from make_disks()."""
-    _check(lib().radt_disk_fields(disks, C.byref(desc.grid), desc.batch, C.c_void_p(temp.data_ptr()),
-                                  C.c_void_p(dens_out.data_ptr()), C.c_void_p(vel_out.data_ptr()),
-                                  C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()), _stream_ptr(stream)))
+    with _on(temp):
+        _check(lib().radt_disk_fields(disks, C.byref(desc.grid), desc.batch, _p(temp), _p(dens_out), _p(vel_out), _p(ws),
+                                      C.c_size_t(ws.numel()), _stream_ptr(stream, temp)))
 
 
 def radt_disk_fields_bwd(disks, desc: Descriptors, temp, g_dens, g_vel, g_temp, ws, stream=None):
     """g_temp += (d n_CO/d temp)^T g_dens + (d v_phi/d temp)^T g_vel."""
-    _check(lib().radt_disk_fields_bwd(disks, C.byref(desc.grid), desc.batch, C.c_void_p(temp.data_ptr()),
-                                      C.c_void_p(g_dens.data_ptr()), C.c_void_p(g_vel.data_ptr()),
-                                      C.c_void_p(g_temp.data_ptr()), C.c_void_p(ws.data_ptr()), C.c_size_t(ws.numel()),
-                                      _stream_ptr(stream)))
+    with _on(temp):
+        _check(lib().radt_disk_fields_bwd(disks, C.byref(desc.grid), desc.batch, _p(temp), _p(g_dens), _p(g_vel), _p(g_temp),
+                                          _p(ws), C.c_size_t(ws.numel()), _stream_ptr(stream, temp)))
 
 
 def radt_mlp_num_params(mlp) -> int:
@@ -263,19 +312,21 @@ def radt_mlp_num_params(mlp) -> int:
 
 def radt_mlp_temperature(mlp, desc: Descriptors, params, temp_out, stream=None):
     """MLP temperature field on the grid nodes: params CUDA float32 [num_params] -> temp_out CUDA float32 [nr, nzeta]."""
-    _check(lib().radt_mlp_temperature(C.byref(mlp), C.byref(desc.grid), C.c_void_p(params.data_ptr()),
-                                      C.c_void_p(temp_out.data_ptr()), _stream_ptr(stream)))
+    with _on(params):
+        _check(lib().radt_mlp_temperature(C.byref(mlp), C.byref(desc.grid), _p(params), _p(temp_out),
+                                          _stream_ptr(stream, params)))
 
 
 def radt_mlp_temperature_bwd(mlp, desc: Descriptors, params, g_temp, g_params, stream=None):
-    _check(lib().radt_mlp_temperature_bwd(C.byref(mlp), C.byref(desc.grid), C.c_void_p(params.data_ptr()),
-                                          C.c_void_p(g_temp.data_ptr()), C.c_void_p(g_params.data_ptr()),
-                                          _stream_ptr(stream)))
+    with _on(params):
+        _check(lib().radt_mlp_temperature_bwd(C.byref(mlp), C.byref(desc.grid), _p(params), _p(g_temp), _p(g_params),
+                                              _stream_ptr(stream, params)))
 
 
 def radt_read_counters(ws, stream=None):
     out = (C.c_uint64 * 4)()
-    _check(lib().radt_read_counters(C.c_void_p(ws.data_ptr()), out, _stream_ptr(stream)))
+    with _on(ws):
+        _check(lib().radt_read_counters(_p(ws), out, _stream_ptr(stream, ws)))
     return [int(x) for x in out]
 
 
@@ -287,24 +338,25 @@ def _hptr(a):
     return C.c_void_p(a.ctypes.data) if a is not None else None
 
 
-def radt_render_host(desc: Descriptors, dens, temp, vel, cube):
-    """HOST numpy float32 arrays in, HOST cube out (copies inside the call)."""
+def radt_render_host(desc: Descriptors, dens, temp, vel, cube, opt=None, cube_lo=None):
+    """HOST numpy float32 arrays in, HOST cube (and optionally its low-order words) out (copies inside the call)."""
     desc.with_fields(dens.ctypes.data, temp.ctypes.data, vel.ctypes.data)
-    _check(lib().radt_render_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _hptr(cube)))
+    _check(lib().radt_render_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _optp(opt), _hptr(cube),
+                                  _hptr(cube_lo)))
 
 
-def radt_fit_step_host(desc: Descriptors, dens, temp, vel, target, sigma, cube, g_dens, g_temp, g_vel) -> float:
+def radt_fit_step_host(desc: Descriptors, dens, temp, vel, target, sigma, cube, g_dens, g_temp, g_vel, opt=None) -> float:
     desc.with_fields(dens.ctypes.data, temp.ctypes.data, vel.ctypes.data)
     loss = C.c_double(0.0)
-    _check(lib().radt_fit_step_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _hptr(target),
+    _check(lib().radt_fit_step_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _optp(opt), _hptr(target),
                                     float(sigma), _hptr(cube), C.byref(loss), _hptr(g_dens), _hptr(g_temp), _hptr(g_vel)))
     return loss.value
 
 
-def radt_render_bwd_host(desc: Descriptors, dens, temp, vel, cube, dl_dcube, g_dens, g_temp, g_vel):
+def radt_render_bwd_host(desc: Descriptors, dens, temp, vel, cube, dl_dcube, g_dens, g_temp, g_vel, opt=None, cube_lo=None):
     desc.with_fields(dens.ctypes.data, temp.ctypes.data, vel.ctypes.data)
-    _check(lib().radt_render_bwd_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _hptr(cube),
-                                      _hptr(dl_dcube), _hptr(g_dens), _hptr(g_temp), _hptr(g_vel)))
+    _check(lib().radt_render_bwd_host(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _optp(opt), _hptr(cube),
+                                      _hptr(cube_lo), _hptr(dl_dcube), _hptr(g_dens), _hptr(g_temp), _hptr(g_vel)))
 
 
 def radt_pipe_peak(kind: int):

@@ -8,16 +8,12 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 
 namespace {
 
 thread_local char g_err[512] = "";
 thread_local int g_launches = 0;
-int g_opt_window = 1;
-int g_opt_skip_empty = 1;
-int g_opt_win_path = 1;
-int g_opt_compensated = 0;
-int g_opt_zero_dens_grad = 1;
 
 int fail(int code, const char *fmt, ...)
 {
@@ -33,6 +29,60 @@ int fail(int code, const char *fmt, ...)
         cudaError_t e_ = (expr);                                                           \
         if (e_ != cudaSuccess) return fail(RADT_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
     } while (0)
+
+// Resolved per-call options (include/radt.h radt_options; NULL = defaults).  No process-wide option state.
+struct Opts {
+    int window = 1, skip_empty = 1, win_path = 1, zero_dens_grad = 1, reuse_setup = 0;
+};
+
+int resolve_options(const radt_options *o, Opts &out)
+{
+    out = Opts();
+    if (!o) return RADT_OK;
+    if (o->struct_size != sizeof(radt_options)) return fail(RADT_E_INVALID, "radt_options.struct_size mismatch");
+    out.window = o->window != 0; out.skip_empty = o->skip_empty != 0; out.win_path = o->win_path != 0;
+    out.zero_dens_grad = o->zero_dens_grad != 0; out.reuse_setup = o->reuse_setup != 0;
+    return RADT_OK;
+}
+
+// What the library remembers between a forward and its adjoint (HOST side, keyed by device pointer, a few entries,
+// oldest replaced): per cube the options that shaped its partial sums, per workspace what the last forward left there.
+struct Remembered {
+    const void *key = nullptr;
+    unsigned long long tag = 0;
+    unsigned long long age = 0;
+};
+struct Registry {
+    static const int N = 64;
+    Remembered e[N];
+    unsigned long long clock = 0;
+    std::mutex mu;
+    void put(const void *key, unsigned long long tag)
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        int slot = 0;
+        for (int i = 0; i < N; ++i) {
+            if (e[i].key == key) { slot = i; break; }
+            if (e[i].age < e[slot].age) slot = i;
+        }
+        e[slot].key = key; e[slot].tag = tag; e[slot].age = ++clock;
+    }
+    bool get(const void *key, unsigned long long &tag)
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        for (int i = 0; i < N; ++i)
+            if (e[i].key == key && e[i].age) { tag = e[i].tag; return true; }
+        return false;
+    }
+};
+Registry g_cubes, g_workspaces;
+
+unsigned long long fnv(unsigned long long h, const void *p, size_t n)
+{
+    const unsigned char *b = (const unsigned char *)p;
+    for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+    return h;
+}
 
 // CODATA 2018, CGS
 const double kH = 6.62607015e-27, kK = 1.380649e-16, kC = 2.99792458e10;
@@ -202,11 +252,11 @@ void make_dev_line(const radt_line *line, DevLine &d)
 }
 
 struct WsLayout {
-    size_t rays, qtab, vcs, rnode, cells, occ, ilo, grad, counters, total;
+    size_t rays, qtab, vcs, rnode, cells, occ, grad, counters, total;
     int occ_wpr, occ_words, occ_nbj;
 };
 
-WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass, int nchan = 0)
+WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass)
 {
     WsLayout w;
     size_t off = 0;
@@ -232,9 +282,6 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
         w.occ_words = nbi * nbj * w.occ_wpr;
     }
     w.occ = off; off = align256(off + (size_t)w.occ_words * (size_t)batch * sizeof(unsigned));
-    // {I, low-order word} per voxel, shared by the forward and the adjoint of a cube (RADT_OPT_COMPENSATED)
-    w.ilo = off;
-    if (g_opt_compensated && nchan > 0) off = align256(off + nrays * (size_t)nchan * sizeof(float2));
     w.grad = off;
     if (pass == RADT_PASS_BWD) off = align256(off + cells * sizeof(float4));
     w.total = off;
@@ -253,7 +300,6 @@ DevWs make_dev_ws(void *ws, const WsLayout &w)
     d.cells = (float4 *)(base + w.cells);
     d.occ = (unsigned *)(base + w.occ);
     d.grad = (float4 *)(base + w.grad);
-    d.ilo = w.grad > w.ilo ? (float2 *)(base + w.ilo) : nullptr;
     return d;
 }
 
@@ -265,19 +311,46 @@ struct LossArgs {
     double sigma = 0.0;
 };
 
+// What shapes the partial sums of a cube (a forward and its adjoint must agree on it) ...
+unsigned long long cube_tag(const Opts &o, bool use_win, bool comp, const radt_geom *geom, const radt_line *line, int batch)
+{
+    unsigned long long h = 1469598103934665603ull;
+    const int v[8] = { o.window, o.skip_empty, use_win ? 1 : 0, comp ? 1 : 0, line->nchan, geom[0].nx, geom[0].ny, batch };
+    return fnv(h, v, sizeof(v)) | 1ull;
+}
+// ... and what a forward leaves in its workspace for an adjoint with reuse_setup: every input of the setup kernel.
+unsigned long long setup_tag(const Opts &o, bool use_win, const radt_geom *geom, const radt_line *line, const radt_grid *grid,
+                             int batch)
+{
+    unsigned long long h = 1469598103934665603ull;
+    h = fnv(h, geom, sizeof(radt_geom) * (size_t)batch);
+    h = fnv(h, grid, sizeof(radt_grid));
+    radt_line l = *line;
+    l.e_lev_K = nullptr; l.g_lev = nullptr; l.vchan = nullptr;
+    h = fnv(h, &l, sizeof(l));
+    h = fnv(h, line->e_lev_K, sizeof(double) * (size_t)line->nlev);
+    h = fnv(h, line->g_lev, sizeof(double) * (size_t)line->nlev);
+    h = fnv(h, line->vchan, sizeof(double) * (size_t)line->nchan);
+    const int v[4] = { o.window, o.skip_empty, use_win ? 1 : 0, batch };
+    return fnv(h, v, sizeof(v)) | 1ull;
+}
+
 // Enqueue setup + march for all batch chunks.  pass 0: forward into `cube`; pass 1: adjoint.
-int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int batch, int pass, float *cube,
-             const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel, void *ws, size_t ws_bytes,
-             cudaStream_t st, const LossArgs &loss = LossArgs())
+int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int batch, const radt_options *opt_in,
+             int pass, float *cube, float *cube_lo, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel,
+             void *ws, size_t ws_bytes, cudaStream_t st, const LossArgs &loss = LossArgs())
 {
     int rc = validate(geom, line, grid, batch);
     if (rc) return rc;
+    Opts opt;
+    if ((rc = resolve_options(opt_in, opt)) != 0) return rc;
     if (!line) return fail(RADT_E_INVALID, "null line descriptor");
     if (!ws) return fail(RADT_E_INVALID, "null workspace");
     if (!grid->dens || !grid->temp || !grid->vel) return fail(RADT_E_INVALID, "null field pointer");
     if (!cube) return fail(RADT_E_INVALID, "null cube pointer");
     if (pass == RADT_PASS_BWD && !dl_dcube) return fail(RADT_E_INVALID, "null dl_dcube pointer");
-    WsLayout w = ws_layout(geom, grid, batch, pass, line->nchan);
+    if (pass == RADT_PASS_FWD && opt.reuse_setup) return fail(RADT_E_INVALID, "reuse_setup applies to radt_render_bwd only");
+    WsLayout w = ws_layout(geom, grid, batch, pass);
     if (ws_bytes < w.total) return fail(RADT_E_WORKSPACE, "workspace too small: need %zu bytes, got %zu", w.total, ws_bytes);
     if (((uintptr_t)ws & 15) != 0) return fail(RADT_E_INVALID, "workspace must be 16-byte aligned");
     long long stride = batch > 1 ? grid->batch_stride : grid_cells(grid);
@@ -299,8 +372,34 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
     DevLine dl_probe;
     make_dev_line(line, dl_probe);
     // window kernels: uniform channel lattice, and cells no finer than the fp32 positions of the prefilter resolve
-    const bool use_win = g_opt_win_path && dl_probe.uniform && prefilter_safe(grid);
-    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, (8 + RADT_LOSS_SLOTS) * sizeof(unsigned long long), st));
+    const bool use_win = opt.win_path && dl_probe.uniform && prefilter_safe(grid);
+    const bool comp = cube_lo != nullptr;
+
+    // a forward and its adjoint must agree on what shapes the partial sums of the cube
+    const unsigned long long ctag = cube_tag(opt, use_win, comp, geom, line, batch);
+    const unsigned long long stag = setup_tag(opt, use_win, geom, line, grid, batch);
+    bool reuse = false;
+    if (pass == RADT_PASS_FWD) {
+        g_cubes.put(cube, ctag);
+        g_workspaces.put(ws, stag);
+    } else {
+        unsigned long long seen = 0;
+        if (g_cubes.get(cube, seen) && seen != 0 && seen != ctag)      // (tag 0: a cube of unknown origin)
+            return fail(RADT_E_INVALID, "this cube was rendered with other options (window / skip_empty / win_path / cube_lo) "
+                                        "than radt_render_bwd was given: the adjoint re-marches with the forward's arithmetic");
+        if (opt.reuse_setup) {
+            if (!g_workspaces.get(ws, seen) || seen != stag)
+                return fail(RADT_E_INVALID, "reuse_setup: this workspace was not last set up by a forward with the same "
+                                            "geom, line, grid and options");
+            reuse = true;
+        } else {
+            g_workspaces.put(ws, 0);          // the adjoint's own setup replaces the forward's (no occupancy words for LINEAR grids)
+        }
+    }
+
+    // counters: 0-3 work counters, 4 the grid's maximum temperature (setup), 8.. loss slots (forward)
+    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, (reuse ? 4 : 8 + RADT_LOSS_SLOTS) * sizeof(unsigned long long), st));
+    if (reuse) CUDA_TRY(cudaMemsetAsync(dws.grad, 0, (size_t)grid_cells(grid) * (size_t)batch * sizeof(float4), st));
     for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
         int nb = batch - b0 < RADT_MAXB ? batch - b0 : RADT_MAXB;
         memset(&SP, 0, sizeof(SP));
@@ -314,35 +413,37 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         SP.nlev = line->nlev; SP.nchan = line->nchan;
         SP.do_rays = 1; SP.do_tables = 1; SP.do_pack = 1; SP.do_zero_grad = (pass == RADT_PASS_BWD);
         SP.batch_stride = stride;
-        // occupancy bitmap for the window kernels' prefilter (axisymmetric grids): with LINEAR densities the
-        // adjoint needs every in-grid step (dL/dn of empty cells), so only the forward and LN grids use it
+        // Occupancy words for the window kernels' prefilter.  The forward always builds them (an adjoint with
+        // reuse_setup may want them); with LINEAR densities the exact adjoint needs every in-grid step (dL/dn of
+        // empty cells) and marches without them.
         const bool win = use_win;
-        const bool occ = win && g_opt_skip_empty && grid->kind != RADT_GRID_SPH3D &&
-                         (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN || !g_opt_zero_dens_grad);
+        const bool occ_fwd = win && opt.skip_empty && grid->kind != RADT_GRID_SPH3D;   // (spherical: range test only)
+        const bool occ = occ_fwd && (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN || !opt.zero_dens_grad);
         SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr; SP.occ_nbj = w.occ_nbj;
         SP.occ_thr = grid->dens_mode == RADT_DENS_LN ? -39.1439f : 1e-17f;     // N_EMPTY of the march kernels
         SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;
-        CUDA_TRY(radt_launch_setup(SP, LT, CT, st));
-        ++g_launches;
+        if (!reuse) {
+            CUDA_TRY(radt_launch_setup(SP, LT, CT, st));
+            ++g_launches;
+        }
 
         memset(&MP, 0, sizeof(MP));
         memcpy(MP.geom, SP.geom, sizeof(MP.geom));
         MP.grid = dg; MP.ws = dws;
-        if (!use_win) MP.ws.ilo = nullptr;            // only the window kernels carry the low-order words
         make_dev_line(line, MP.line);
         MP.nx = SP.nx; MP.ny = SP.ny; MP.nstep = SP.nstep;
         MP.tiles_x = (MP.nx + RADT_TILE_X - 1) / RADT_TILE_X;
         MP.tiles_y = (MP.ny + RADT_TILE_Y - 1) / RADT_TILE_Y;
         MP.b0 = b0;
-        MP.opt_window = g_opt_window; MP.opt_skip_empty = g_opt_skip_empty;
-        MP.opt_zero_grad = g_opt_zero_dens_grad || !g_opt_skip_empty;
+        MP.opt_window = opt.window; MP.opt_skip_empty = opt.skip_empty;
+        MP.opt_zero_grad = opt.zero_dens_grad || !opt.skip_empty;
         MP.chan_lo = 0;
         for (int b = 0; b < nb && !MP.chan_lo; ++b)
             for (int c = 0; c < line->nchan; ++c) {
                 double vv = line->vchan[c] - geom[b0 + b].vsys;
                 if ((double)(float)vv != vv) { MP.chan_lo = 1; break; }
             }
-        MP.cube = cube; MP.dl_dcube = dl_dcube;
+        MP.cube = cube; MP.cube_lo = cube_lo; MP.dl_dcube = dl_dcube;
         if (pass == RADT_PASS_FWD && loss.target) {
             const double nvox = (double)batch * geom[0].nx * geom[0].ny * line->nchan;
             const double inv = 1.0 / (loss.sigma * loss.sigma * nvox);
@@ -377,24 +478,11 @@ int radt_version(void) { return RADT_VERSION; }
 const char *radt_last_error(void) { return g_err; }
 int radt_last_launch_count(void) { return g_launches; }
 
-int radt_set_option(int key, int value)
+void radt_options_default(radt_options *opt)
 {
-    if (key == RADT_OPT_WINDOW) { g_opt_window = value != 0; return RADT_OK; }
-    if (key == RADT_OPT_SKIP_EMPTY) { g_opt_skip_empty = value != 0; return RADT_OK; }
-    if (key == RADT_OPT_WIN_PATH) { g_opt_win_path = value != 0; return RADT_OK; }
-    if (key == RADT_OPT_COMPENSATED) { g_opt_compensated = value != 0; return RADT_OK; }
-    if (key == RADT_OPT_ZERO_DENS_GRAD) { g_opt_zero_dens_grad = value != 0; return RADT_OK; }
-    return fail(RADT_E_INVALID, "unknown option %d", key);
-}
-
-int radt_get_option(int key)
-{
-    if (key == RADT_OPT_WINDOW) return g_opt_window;
-    if (key == RADT_OPT_SKIP_EMPTY) return g_opt_skip_empty;
-    if (key == RADT_OPT_WIN_PATH) return g_opt_win_path;
-    if (key == RADT_OPT_COMPENSATED) return g_opt_compensated;
-    if (key == RADT_OPT_ZERO_DENS_GRAD) return g_opt_zero_dens_grad;
-    return fail(RADT_E_INVALID, "unknown option %d", key);
+    if (!opt) return;
+    opt->struct_size = sizeof(radt_options);
+    opt->window = 1; opt->skip_empty = 1; opt->win_path = 1; opt->zero_dens_grad = 1; opt->reuse_setup = 0;
 }
 
 int radt_workspace_bytes(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
@@ -404,7 +492,37 @@ int radt_workspace_bytes(const radt_geom *geom, const radt_line *line, const rad
     int rc = validate(geom, line, grid, batch);
     if (rc) return rc;
     if (pass != RADT_PASS_FWD && pass != RADT_PASS_BWD) return fail(RADT_E_INVALID, "unknown pass");
-    *bytes_out = ws_layout(geom, grid, batch, pass, line ? line->nchan : 0).total;
+    *bytes_out = ws_layout(geom, grid, batch, pass).total;
+    return RADT_OK;
+}
+
+int radt_grad_layout(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                     size_t *offset_out, size_t *nfloat_out)
+{
+    if (!offset_out || !nfloat_out) return fail(RADT_E_INVALID, "null output pointer");
+    int rc = validate(geom, line, grid, batch);
+    if (rc) return rc;
+    WsLayout w = ws_layout(geom, grid, batch, RADT_PASS_BWD);
+    *offset_out = w.grad;
+    *nfloat_out = (size_t)grid_cells(grid) * (size_t)batch * 4;
+    return RADT_OK;
+}
+
+int radt_unpack_grad(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, const void *ws,
+                     size_t ws_bytes, float *g_dens, float *g_temp, float *g_vel, void *cuda_stream)
+{
+    int rc = validate(geom, line, grid, batch);
+    if (rc) return rc;
+    if (!ws) return fail(RADT_E_INVALID, "null workspace");
+    WsLayout w = ws_layout(geom, grid, batch, RADT_PASS_BWD);
+    if (ws_bytes < w.total) return fail(RADT_E_WORKSPACE, "workspace too small: need %zu bytes, got %zu", w.total, ws_bytes);
+    long long stride = batch > 1 ? grid->batch_stride : grid_cells(grid);
+    g_launches = 0;
+    if (g_dens || g_temp || g_vel) {
+        CUDA_TRY(radt_launch_unpack((const float4 *)((const char *)ws + w.grad), grid_cells(grid), batch, stride, g_dens, g_temp,
+                                    g_vel, (cudaStream_t)cuda_stream));
+        g_launches = 1;
+    }
     return RADT_OK;
 }
 
@@ -433,31 +551,31 @@ int radt_ray_geometry(const radt_geom *geom, const radt_grid *grid, int32_t batc
     return RADT_OK;
 }
 
-int radt_render(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, float *cube,
-                void *ws, size_t ws_bytes, void *cuda_stream)
+int radt_render(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, const radt_options *opt,
+                float *cube, float *cube_lo, void *ws, size_t ws_bytes, void *cuda_stream)
 {
-    return run_pass(geom, line, grid, batch, RADT_PASS_FWD, cube, nullptr, nullptr, nullptr, nullptr, ws, ws_bytes,
-                    (cudaStream_t)cuda_stream);
+    return run_pass(geom, line, grid, batch, opt, RADT_PASS_FWD, cube, cube_lo, nullptr, nullptr, nullptr, nullptr, ws,
+                    ws_bytes, (cudaStream_t)cuda_stream);
 }
 
 int radt_render_loss(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                     const float *target, double sigma, float *cube, float *dl_dcube, double *loss_out, void *ws,
-                     size_t ws_bytes, void *cuda_stream)
+                     const radt_options *opt, const float *target, double sigma, float *cube, float *cube_lo,
+                     float *dl_dcube, double *loss_out, void *ws, size_t ws_bytes, void *cuda_stream)
 {
     if (!target || !dl_dcube || !loss_out) return fail(RADT_E_INVALID, "null target / dl_dcube / loss_out pointer");
     if (!(sigma > 0)) return fail(RADT_E_INVALID, "sigma must be positive");
     LossArgs la;
     la.target = target; la.dl_out = dl_dcube; la.loss = loss_out; la.sigma = sigma;
-    return run_pass(geom, line, grid, batch, RADT_PASS_FWD, cube, nullptr, nullptr, nullptr, nullptr, ws, ws_bytes,
-                    (cudaStream_t)cuda_stream, la);
+    return run_pass(geom, line, grid, batch, opt, RADT_PASS_FWD, cube, cube_lo, nullptr, nullptr, nullptr, nullptr, ws,
+                    ws_bytes, (cudaStream_t)cuda_stream, la);
 }
 
 int radt_render_bwd(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                    const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel, void *ws,
-                    size_t ws_bytes, void *cuda_stream)
+                    const radt_options *opt, const float *cube, const float *cube_lo, const float *dl_dcube, float *g_dens,
+                    float *g_temp, float *g_vel, void *ws, size_t ws_bytes, void *cuda_stream)
 {
-    return run_pass(geom, line, grid, batch, RADT_PASS_BWD, const_cast<float *>(cube), dl_dcube, g_dens, g_temp, g_vel,
-                    ws, ws_bytes, (cudaStream_t)cuda_stream);
+    return run_pass(geom, line, grid, batch, opt, RADT_PASS_BWD, const_cast<float *>(cube), const_cast<float *>(cube_lo),
+                    dl_dcube, g_dens, g_temp, g_vel, ws, ws_bytes, (cudaStream_t)cuda_stream);
 }
 
 int radt_l2_loss_grad(const float *cube, const float *target, double sigma, int64_t n, float *dl_dcube,
@@ -523,13 +641,17 @@ struct DevBufs {
 };
 }  // namespace
 
-static int host_common(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, int mode,
-                       const float *target, double sigma, float *cube, const float *cube_in, const float *dl_in,
-                       double *loss_out, float *g_dens, float *g_temp, float *g_vel)
+static int host_common(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                       const radt_options *opt, int mode, const float *target, double sigma, float *cube, float *cube_lo,
+                       const float *cube_in, const float *lo_in, const float *dl_in, double *loss_out, float *g_dens,
+                       float *g_temp, float *g_vel)
 {
-    // mode 0: forward only; 1: forward + L2 + adjoint; 2: adjoint from given cube and dl_dcube
+    // mode 0: forward only; 1: forward + chi^2 term + adjoint; 2: adjoint from given cube and dl_dcube
     int rc = validate(geom, line, grid, batch);
     if (rc) return rc;
+    Opts o;
+    if ((rc = resolve_options(opt, o)) != 0) return rc;
+    if (o.reuse_setup) return fail(RADT_E_INVALID, "reuse_setup is for the device entry points (the host calls manage their own workspace)");
     if (!line) return fail(RADT_E_INVALID, "null line descriptor");
     if (!grid->dens || !grid->temp || !grid->vel) return fail(RADT_E_INVALID, "null field pointer");
     int count = 0;
@@ -539,13 +661,21 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     long long stride = batch > 1 ? grid->batch_stride : cells;
     size_t fbytes = (size_t)((batch - 1) * stride + cells) * sizeof(float);
     size_t nvox = (size_t)batch * geom[0].nx * geom[0].ny * line->nchan;
-    CUDA_TRY(cudaStreamSynchronize(B.st));       // an earlier call that failed half-way may still own the arena
-    const size_t wsb_need = ws_layout(geom, grid, batch, mode == 0 ? RADT_PASS_FWD : RADT_PASS_BWD, line->nchan).total;
-    if (!B.reserve(6 * align256(fbytes) + 3 * align256(nvox * sizeof(float)) + align256(wsb_need) + 4096))
+    static thread_local cudaStream_t s2 = nullptr;
+    static thread_local cudaEvent_t ev_alloc = nullptr, ev_copied = nullptr;
+    // an earlier call that failed half-way may still own the arena (main stream, or the target upload on s2)
+    CUDA_TRY(cudaStreamSynchronize(B.st));
+    if (s2) CUDA_TRY(cudaStreamSynchronize(s2));
+    const size_t wsb_need = ws_layout(geom, grid, batch, mode == 0 ? RADT_PASS_FWD : RADT_PASS_BWD).total;
+    if (!B.reserve(6 * align256(fbytes) + 4 * align256(nvox * sizeof(float)) + align256(wsb_need) + 4096))
         return fail(RADT_E_CUDA, "device allocation failed");
     float *d_dens = (float *)B.alloc(fbytes), *d_temp = (float *)B.alloc(fbytes), *d_vel = (float *)B.alloc(fbytes);
     float *d_cube = (float *)B.alloc(nvox * sizeof(float));
-    if (!d_dens || !d_temp || !d_vel || !d_cube) return fail(RADT_E_CUDA, "device allocation failed");
+    // low-order words: kept on the device between the forward and the adjoint of a fit step; mode 0 / 2 only when the
+    // caller has a host buffer for them
+    const bool want_lo = mode == 1 || (mode == 0 && cube_lo) || (mode == 2 && lo_in);
+    float *d_lo = want_lo ? (float *)B.alloc(nvox * sizeof(float)) : nullptr;
+    if (!d_dens || !d_temp || !d_vel || !d_cube || (want_lo && !d_lo)) return fail(RADT_E_CUDA, "device allocation failed");
     CUDA_TRY(cudaMemcpyAsync(d_dens, grid->dens, fbytes, cudaMemcpyHostToDevice, B.st));
     CUDA_TRY(cudaMemcpyAsync(d_temp, grid->temp, fbytes, cudaMemcpyHostToDevice, B.st));
     CUDA_TRY(cudaMemcpyAsync(d_vel, grid->vel, fbytes, cudaMemcpyHostToDevice, B.st));
@@ -557,16 +687,19 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     int launches = 0;
     float *d_dl = nullptr;
     if (mode != 0 && !(d_dl = (float *)B.alloc(nvox * sizeof(float)))) return fail(RADT_E_CUDA, "device allocation failed");
+    radt_options ob;
+    radt_options_default(&ob);
+    if (opt) ob = *opt;
     if (mode == 0) {
-        rc = radt_render(geom, line, &dgrid, batch, d_cube, ws, wsb, B.st);
+        rc = radt_render(geom, line, &dgrid, batch, opt, d_cube, d_lo, ws, wsb, B.st);
         if (rc) return rc;
         launches += g_launches;
     } else if (mode == 1) {
-        // The target cube is the bulk of the input bytes: its upload runs on a second stream under the forward
-        // march, and the chi^2 term follows as its own pass (the fused radt_render_loss would have to wait for it).
+        // The target cube is the bulk of the input bytes (97 % on config 2) and PCIe is the long pole of this call: its
+        // upload runs on a second stream UNDER the setup and the forward march, and the chi^2 term follows as its own
+        // small pass (the fused radt_render_loss would have to wait for the whole upload before its first ray:
+        // measured 0.15 ms slower per step on config 2, 17 ms on config 5).
         if (!target) return fail(RADT_E_INVALID, "null target");
-        static thread_local cudaStream_t s2 = nullptr;
-        static thread_local cudaEvent_t ev_alloc = nullptr, ev_copied = nullptr;
         if (!s2) {
             CUDA_TRY(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
             CUDA_TRY(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
@@ -579,17 +712,18 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
         CUDA_TRY(cudaStreamWaitEvent(s2, ev_alloc, 0));
         CUDA_TRY(cudaMemcpyAsync(d_t, target, nvox * sizeof(float), cudaMemcpyHostToDevice, s2));
         CUDA_TRY(cudaEventRecord(ev_copied, s2));
-        rc = radt_render(geom, line, &dgrid, batch, d_cube, ws, wsb, B.st);
-        if (rc) return rc;
+        rc = radt_render(geom, line, &dgrid, batch, opt, d_cube, d_lo, ws, wsb, B.st);
+        if (rc) { cudaStreamSynchronize(s2); return rc; }
         launches += g_launches;
         CUDA_TRY(cudaStreamWaitEvent(B.st, ev_copied, 0));
         rc = radt_l2_loss_grad(d_cube, d_t, sigma, (int64_t)nvox, d_dl, d_loss, B.st);
-        if (rc) return rc;
+        if (rc) { cudaStreamSynchronize(s2); return rc; }
         launches += g_launches;
         if (loss_out) CUDA_TRY(cudaMemcpyAsync(loss_out, d_loss, sizeof(double), cudaMemcpyDeviceToHost, B.st));
     }
     if ((mode == 0 || mode == 1) && cube)
         CUDA_TRY(cudaMemcpyAsync(cube, d_cube, nvox * sizeof(float), cudaMemcpyDeviceToHost, B.st));
+    if (mode == 0 && cube_lo) CUDA_TRY(cudaMemcpyAsync(cube_lo, d_lo, nvox * sizeof(float), cudaMemcpyDeviceToHost, B.st));
     if (mode == 1 || mode == 2) {
         float *d_g[3] = { nullptr, nullptr, nullptr };
         float *h_g[3] = { g_dens, g_temp, g_vel };
@@ -598,9 +732,12 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
         if (mode == 2) {
             if (!cube_in || !dl_in) return fail(RADT_E_INVALID, "null cube / dl_dcube");
             CUDA_TRY(cudaMemcpyAsync(d_cube, cube_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
+            if (lo_in) CUDA_TRY(cudaMemcpyAsync(d_lo, lo_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
             CUDA_TRY(cudaMemcpyAsync(d_dl, dl_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
+            g_cubes.put(d_cube, 0);          // a cube from the host: nothing is known about the options that made it
         }
-        rc = radt_render_bwd(geom, line, &dgrid, batch, d_cube, d_dl, d_g[0], d_g[1], d_g[2], ws, wsb, B.st);
+        ob.reuse_setup = mode == 1;          // the forward of this very call set the workspace up
+        rc = radt_render_bwd(geom, line, &dgrid, batch, &ob, d_cube, d_lo, d_dl, d_g[0], d_g[1], d_g[2], ws, wsb, B.st);
         if (rc) return rc;
         launches += g_launches;
         for (int i = 0; i < 3; ++i)
@@ -611,24 +748,29 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     return RADT_OK;
 }
 
-int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch, float *cube)
+int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                     const radt_options *opt, float *cube, float *cube_lo)
 {
     if (!cube) return fail(RADT_E_INVALID, "null cube pointer");
-    return host_common(geom, line, grid, batch, 0, nullptr, 0.0, cube, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+    return host_common(geom, line, grid, batch, opt, 0, nullptr, 0.0, cube, cube_lo, nullptr, nullptr, nullptr, nullptr,
+                       nullptr, nullptr, nullptr);
 }
 
 int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                       const float *target, double sigma, float *cube, double *loss_out, float *g_dens, float *g_temp,
-                       float *g_vel)
+                       const radt_options *opt, const float *target, double sigma, float *cube, double *loss_out,
+                       float *g_dens, float *g_temp, float *g_vel)
 {
     if (!(sigma > 0)) return fail(RADT_E_INVALID, "sigma must be positive");
-    return host_common(geom, line, grid, batch, 1, target, sigma, cube, nullptr, nullptr, loss_out, g_dens, g_temp, g_vel);
+    return host_common(geom, line, grid, batch, opt, 1, target, sigma, cube, nullptr, nullptr, nullptr, nullptr, loss_out,
+                       g_dens, g_temp, g_vel);
 }
 
 int radt_render_bwd_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
-                         const float *cube, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel)
+                         const radt_options *opt, const float *cube, const float *cube_lo, const float *dl_dcube,
+                         float *g_dens, float *g_temp, float *g_vel)
 {
-    return host_common(geom, line, grid, batch, 2, nullptr, 0.0, nullptr, cube, dl_dcube, nullptr, g_dens, g_temp, g_vel);
+    return host_common(geom, line, grid, batch, opt, 2, nullptr, 0.0, nullptr, nullptr, cube, cube_lo, dl_dcube, nullptr,
+                       g_dens, g_temp, g_vel);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -83,7 +83,6 @@ struct DevWs {
     double2 *rnode;        // [nr] {r_i, 1/r_i^2} node radii of the log-spaced axis (axisym), fp64
     float4 *cells;         // [batch][cells] packed {dens, temp, vel, 0}
     float4 *grad;          // [batch][cells] packed gradient accumulators {dens, temp, vel, -} (bwd only)
-    float2 *ilo;           // [batch*ny*nx*nchan] {I, low-order word of its sum} (RADT_OPT_COMPENSATED; else null)
     unsigned *occ;         // [batch][occ_words] axisym: bit (i, j): some cell within one cell of (i, j) can emit;
                            // 3-D: one bit per block of 4 x 4 x 4 cells, same dilation (radt_setup.cu)
     unsigned long long *counters;   // [8 + RADT_LOSS_SLOTS] 0-3 work counters; [4] bits of the grid's maximum
@@ -106,6 +105,7 @@ struct MarchParams {
     int occ_words, occ_wpr; // words per batch item; words per radial row (axisym) / per line of blocks along z (3-D)
     int occ_nbj;            // 3-D: blocks along y
     float *cube;           // fwd: output; bwd: saved forward output (const)
+    float *cube_lo;        // low-order word of the fp32 sum behind every voxel (fwd: output, bwd: input); may be null
     const float *dl_dcube; // bwd
     // fused chi^2 data term of the forward (radt_render_loss): all null / 0 for a plain render
     const float *target;   // [batch][ny][nx][nchan]

@@ -40,7 +40,9 @@ __device__ __forceinline__ bool line_hits_span(const StepState &st, float vmin, 
 // ---------------------------------------------------------------------------------------------
 // K2 / K3 forward march.  NP = channel-group pairs per lane: lane owns channels lane + 32 g, g < 2 NP.
 // ---------------------------------------------------------------------------------------------
-template <int KIND, int NP, bool CL>
+// COMP (the caller passed cube_lo): the rounding errors of every I += c are collected in a low-order word per channel,
+// which the adjoint uses to form R_k = I - I_{<=k} without the cancellation noise of the fp32 sum.
+template <int KIND, int NP, bool CL, bool COMP>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __grid_constant__ MarchParams P)
 {
     __shared__ float4 sh_p[RADT_WARPS_PER_CTA][32];
@@ -52,11 +54,14 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
     const int nchan = P.line.nchan;
     float *out = P.cube + rc.ray * (size_t)nchan;
     if (P.target) loss_prefetch(P, rc.ray * (size_t)nchan, nchan, lane);
-    f2 I[NP], T[NP], vcs[NP], vcl[NP];
+    f2 I[NP], T[NP], vcs[NP], vcl[NP], Lw[COMP ? NP : 1];
     float vmin, vmax;
     load_channels<NP>(P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN, nchan, lane, vcs, vcl, vmin, vmax);
 #pragma unroll
-    for (int p = 0; p < NP; ++p) { I[p] = pk(0.f, 0.f); T[p] = pk(1.f, 1.f); }
+    for (int p = 0; p < NP; ++p) {
+        I[p] = pk(0.f, 0.f); T[p] = pk(1.f, 1.f);
+        if (COMP) Lw[p] = pk(0.f, 0.f);
+    }
     unsigned n_steps = 0, n_mufu = 0;
     if (rc.ds != 0.0) {
         const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
@@ -90,7 +95,12 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
                     pair_eval(u, q.w, s);
                     // contribution c = S ((1-e) T) and partial sum I += c as ONE explicit FMA: the adjoint
                     // re-march repeats exactly this sequence and so reproduces the partial sums bit for bit
-                    I[p] = fma2(S2, mul2(s.om, T[p]), I[p]);
+                    const f2 m = mul2(s.om, T[p]);
+                    const f2 In = fma2(S2, m, I[p]);
+                    // rounding error of In = fl(S m + I): I - In is exact whenever the contribution is small against the
+                    // sum, which is when it matters
+                    if (COMP) Lw[p] = add2(Lw[p], fma2(S2, m, sub2(I[p], In)));
+                    I[p] = In;
                     T[p] = mul2(T[p], s.e);
                 }
             }
@@ -105,6 +115,13 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
         upk(I[p], i0, i1);
         if (c0 < nchan) out[c0] = i0;
         if (c1 < nchan) out[c1] = i1;
+        if (COMP) {
+            float l0, l1;
+            upk(Lw[p], l0, l1);
+            float *lo = P.cube_lo + rc.ray * (size_t)nchan;
+            if (c0 < nchan) lo[c0] = l0;
+            if (c1 < nchan) lo[c1] = l1;
+        }
         if (P.target) {
             if (c0 < nchan) r2 += loss_voxel(P, rc.ray * (size_t)nchan + c0, i0);
             if (c1 < nchan) r2 += loss_voxel(P, rc.ray * (size_t)nchan + c1, i1);
@@ -126,10 +143,10 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32) k_march_fwd(const __g
 // ---------------------------------------------------------------------------------------------
 #define RADT_NS 8
 
-template <int NP, bool CL>
+template <int NP, bool CL, bool COMP, int NQ>
 __device__ __forceinline__ float4 bwd_estep(const float4 q, const float S, const float nsmax, const bool window,
-                                            f2 (&T)[NP], f2 (&Pp)[NP], const f2 (&Isv)[NP], const f2 (&Gc)[NP],
-                                            const f2 (&vcs)[NP], const f2 (&vcl)[NP], unsigned &n_mufu)
+                                            f2 (&T)[NP], f2 (&Pp)[NP], f2 (&Qp)[NQ], const f2 (&Isv)[NP], const f2 (&Ilo)[NQ],
+                                            const f2 (&Gc)[NP], const f2 (&vcs)[NP], const f2 (&vcl)[NP], unsigned &n_mufu)
 {
     const f2 S2 = pk1(S), nsm2 = pk1(nsmax);
     f2 a0 = pk(0.f, 0.f), a1 = a0, a2 = a0, a3 = a0;
@@ -141,9 +158,16 @@ __device__ __forceinline__ float4 bwd_estep(const float4 q, const float S, const
         Pair s;
         pair_eval(u, q.w, s);
         f2 omT = mul2(s.om, T[p]);
-        Pp[p] = fma2(S2, omT, Pp[p]);                 // = the forward's partial sum I_{<=k}, bit for bit
+        const f2 Pn = fma2(S2, omT, Pp[p]);           // = the forward's partial sum I_{<=k}, bit for bit
+        f2 PmI = sub2(Pn, Isv[p]);
+        if (COMP) {
+            // the same error words the forward collected, so that P + Q tracks the exact partial sum
+            Qp[p] = add2(Qp[p], fma2(S2, omT, sub2(Pp[p], Pn)));
+            PmI = add2(PmI, sub2(Qp[p], Ilo[p]));
+        }
+        Pp[p] = Pn;
         f2 Tn = mul2(T[p], s.e);
-        f2 nR = clamp_nR(sub2(Pp[p], Isv[p]), Tn, nsm2);
+        f2 nR = clamp_nR(PmI, Tn, nsm2);
         f2 a = mul2(Gc[p], fma2(Tn, S2, nR));         // dL/d dtau
         f2 w = mul2(a, s.g), wu = mul2(w, s.u);
         if (NP == 1) {
@@ -213,8 +237,8 @@ __device__ __forceinline__ void reduce_batch(const float4 (*red)[32], int nb, fl
     if (lane < nb) out[lane] = acc;
 }
 
-template <int KIND, int NP, bool CL>
-__global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd(const __grid_constant__ MarchParams P)
+template <int KIND, int NP, bool CL, bool COMP>
+__global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, (COMP && NP == 4) ? 2 : 3) k_march_bwd(const __grid_constant__ MarchParams P)
 {
     __shared__ float4 sh_p[RADT_WARPS_PER_CTA][32];
     __shared__ float sh_s[RADT_WARPS_PER_CTA][32];
@@ -229,7 +253,9 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd(const 
     const int nchan = L.nchan;
     const float *Isave = P.cube + rc.ray * (size_t)nchan;
     const float *Gin = P.dl_dcube + rc.ray * (size_t)nchan;
-    f2 Isv[NP], Pp[NP], T[NP], vcs[NP], vcl[NP], Gc[NP];
+    constexpr int NQ = COMP ? NP : 1;
+    f2 Isv[NP], Pp[NP], T[NP], vcs[NP], vcl[NP], Gc[NP], Qp[NQ], Ilo[NQ];
+    const float *Lsave = COMP ? P.cube_lo + rc.ray * (size_t)nchan : nullptr;
     float vmin, vmax;
     load_channels<NP>(P.ws.vcs + (size_t)(P.b0 + rc.b) * RADT_MAXCHAN, nchan, lane, vcs, vcl, vmin, vmax);
     bool anyg = false;
@@ -240,6 +266,10 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd(const 
         float g0 = ok0 ? __ldg(Gin + c0) : 0.f, g1 = ok1 ? __ldg(Gin + c1) : 0.f;
         T[p] = pk(1.f, 1.f); Pp[p] = pk(0.f, 0.f);
         Isv[p] = pk(ok0 ? __ldg(Isave + c0) : 0.f, ok1 ? __ldg(Isave + c1) : 0.f);
+        if (COMP) {
+            Qp[p] = pk(0.f, 0.f);
+            Ilo[p] = pk(ok0 ? __ldg(Lsave + c0) : 0.f, ok1 ? __ldg(Lsave + c1) : 0.f);
+        }
         Gc[p] = pk(g0, g1);
         anyg |= (g0 != 0.f) || (g1 != 0.f);
     }
@@ -276,7 +306,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd(const 
                 for (int jj = 0; jj < nb; ++jj) {
                     float4 q = sh_p[warp][base + jj];
                     float S = sh_s[warp][base + jj];
-                    sh_red[warp][jj][lane] = bwd_estep<NP, CL>(q, S, nsmax, window, T, Pp, Isv, Gc, vcs, vcl, n_mufu);
+                    sh_red[warp][jj][lane] = bwd_estep<NP, CL, COMP, NQ>(q, S, nsmax, window, T, Pp, Qp, Isv, Ilo, Gc, vcs, vcl, n_mufu);
                 }
                 __syncwarp();
                 reduce_batch<false>(sh_red[warp], nb, &sh_sum[warp][base], lane);
@@ -287,7 +317,9 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, 3) k_march_bwd(const 
 #pragma unroll
                 for (int p = 0; p < NP; ++p) {
                     GT[p] = mul2(Gc[p], T[p]);
-                    GnR[p] = mul2(Gc[p], clamp_nR(sub2(Pp[p], Isv[p]), T[p], nsm2));
+                    f2 PmI = sub2(Pp[p], Isv[p]);
+                    if (COMP) PmI = add2(PmI, sub2(Qp[p], Ilo[p]));
+                    GnR[p] = mul2(Gc[p], clamp_nR(PmI, T[p], nsm2));
                 }
 #pragma unroll 4
                 for (int jj = 0; jj < nb; ++jj) {
@@ -317,8 +349,11 @@ template <int KIND, int NP>
 static cudaError_t launch_fwd_t(const MarchParams &P, int nbatch, cudaStream_t st)
 {
     dim3 grid(P.tiles_x * P.tiles_y, nbatch);
-    if (P.chan_lo) k_march_fwd<KIND, NP, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
-    else k_march_fwd<KIND, NP, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    const bool comp = P.cube_lo != nullptr;
+    if (P.chan_lo && comp) k_march_fwd<KIND, NP, true, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else if (P.chan_lo) k_march_fwd<KIND, NP, true, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else if (comp) k_march_fwd<KIND, NP, false, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else k_march_fwd<KIND, NP, false, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
     return cudaGetLastError();
 }
 
@@ -326,8 +361,11 @@ template <int KIND, int NP>
 static cudaError_t launch_bwd_t(const MarchParams &P, int nbatch, cudaStream_t st)
 {
     dim3 grid(P.tiles_x * P.tiles_y, nbatch);
-    if (P.chan_lo) k_march_bwd<KIND, NP, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
-    else k_march_bwd<KIND, NP, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    const bool comp = P.cube_lo != nullptr;
+    if (P.chan_lo && comp) k_march_bwd<KIND, NP, true, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else if (P.chan_lo) k_march_bwd<KIND, NP, true, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else if (comp) k_march_bwd<KIND, NP, false, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
+    else k_march_bwd<KIND, NP, false, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
     return cudaGetLastError();
 }
 

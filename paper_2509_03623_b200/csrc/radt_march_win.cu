@@ -146,7 +146,7 @@ __device__ __forceinline__ int group_for(int ulo, int uhi) { return ulo - ((31 -
 // Per-lane channel state of the forward window march.  The (I, T) of all channels of the ray live in shared
 // memory (channel c is only ever touched by lane c & 31); the lane keeps the pair of the ONE channel it serves in
 // the current group [cur, cur + 32) in registers.
-// COMP (RADT_OPT_COMPENSATED): the rounding errors of the sum I += c are collected in a low-order word Ls, which the
+// COMP (the caller passed cube_lo): the rounding errors of the sum I += c are collected in a low-order word Ls, which the
 // adjoint uses to form R_k = I - I_{<=k} without the cancellation noise of the fp32 sum.
 template <bool COMP>
 struct LaneState {
@@ -313,9 +313,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
         if (c < nchan) {
             const float Ic = sI[c];
             out[c] = Ic;
-            // the cube value travels with its low-order word: the adjoint takes the word only where the value still
-            // equals the cube it is given
-            if (COMP) P.ws.ilo[rc.ray * (size_t)nchan + c] = make_float2(Ic, L.sL[c]);
+            if (COMP) P.cube_lo[rc.ray * (size_t)nchan + c] = L.sL[c];
             if (P.target) r2 += loss_voxel(P, rc.ray * (size_t)nchan + c, Ic);
         }
     }
@@ -340,12 +338,10 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
 template <bool COMP>
 struct BwdLane {
     float Ts, Ps, Is, Gs, cf;                     // transmittance, partial sum, saved I, dL/dI of the served channel
-    float Qs, Ils, vs;                            // COMP: low-order words of the partial sum and of the saved I; vs = 1
-                                                  // where the saved word is valid, else 0 (plain difference)
+    float Qs, Ils;                                // COMP: low-order words of the partial sum and of the saved I
     int cur, myc;
     float *sT, *sP, *sQ;
-    const float *Isave, *Gin;
-    const float2 *Ilo;
+    const float *Isave, *Gin, *Ilo;
     __device__ __forceinline__ void put_back()
     {
         if (myc >= 0) {
@@ -360,23 +356,15 @@ struct BwdLane {
         myc = (unsigned)c < (unsigned)nchan ? c : -1;
         cf = (float)c;
         Ts = 1.f; Ps = 0.f; Is = 0.f; Gs = 0.f;    // lanes without a channel contribute nothing (G = 0)
-        Qs = 0.f; Ils = 0.f; vs = 0.f;
+        Qs = 0.f; Ils = 0.f;
         if (myc >= 0) {
             Ts = sT[c]; Ps = sP[c]; Is = __ldg(Isave + c); Gs = __ldg(Gin + c);
-            if (COMP) {
-                // the forward left {I, low-order word} in the workspace: the word is only taken where the value is
-                // bit for bit the cube's (another workspace, or one written since, falls back to the plain difference)
-                Qs = sQ[c];
-                const float2 w = __ldg(Ilo + c);
-                const bool ok = __float_as_int(w.x) == __float_as_int(Is);
-                Ils = ok ? w.y : 0.f;
-                vs = ok ? 1.f : 0.f;
-            }
+            if (COMP) { Qs = sQ[c]; Ils = __ldg(Ilo + c); }
         }
         cur = clo;
     }
     // -R = (P - I) + (P_lo - I_lo) of the served channel
-    __device__ __forceinline__ float neg_r() const { return COMP ? fmaf(vs, Qs - Ils, Ps - Is) : Ps - Is; }
+    __device__ __forceinline__ float neg_r() const { return COMP ? (Ps - Is) + (Qs - Ils) : Ps - Is; }
 };
 
 // Partial sums of a reduction batch, rows padded by one element so that both the per-lane writes and the per-step
@@ -408,7 +396,7 @@ __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, c
         // the same error words the forward collected (fwd_pair), so that P + Q tracks the exact partial sum
         const float Q0 = L.Qs + __fmaf_rn(qb.z, c0, __fsub_rn(L.Ps, P0));
         const float Q1 = Q0 + __fmaf_rn(qb.w, c1, __fsub_rn(P0, P1));
-        PmI = fma2(pk1(L.vs), sub2(pk(Q0, Q1), pk1(L.Ils)), PmI);
+        PmI = add2(PmI, sub2(pk(Q0, Q1), pk1(L.Ils)));
         L.Qs = Q1;
     }
     const f2 nR = clamp_nR(PmI, Tn, pk1(nsmax));
@@ -496,7 +484,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
     const int nchan = Ln.nchan;
     BwdLane<COMP> L;
     L.sT = reinterpret_cast<float *>(base + sizeof(BwdShared)); L.sP = L.sT + 32 * ng; L.sQ = L.sP + 32 * ng;
-    L.Ilo = P.ws.ilo + rc.ray * (size_t)nchan;
+    L.Ilo = P.cube_lo + rc.ray * (size_t)nchan;
     L.Isave = P.cube + rc.ray * (size_t)nchan;
     L.Gin = P.dl_dcube + rc.ray * (size_t)nchan;
     bool anyg = false;
@@ -506,7 +494,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
         if (COMP) L.sQ[c] = 0.f;
         anyg |= c < nchan && __ldg(L.Gin + c) != 0.f;
     }
-    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.cf = 0.f; L.Qs = 0.f; L.Ils = 0.f; L.vs = 0.f; L.cur = NO_GROUP; L.myc = -1;
+    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.cf = 0.f; L.Qs = 0.f; L.Ils = 0.f; L.cur = NO_GROUP; L.myc = -1;
     if (!__any_sync(FULL, anyg)) return;     // dL/dcube vanishes on this ray: no gradient
     const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
@@ -625,7 +613,7 @@ static cudaError_t launch_w(K kern, const MarchParams &P, int nbatch, size_t war
 
 cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    const bool comp = P.ws.ilo != nullptr;
+    const bool comp = P.cube_lo != nullptr;
     const size_t wb = fwd_warp_bytes(P.line.ngroups, comp);
     if (comp)
         return P.grid.kind == 0 ? launch_w(k_march_fwd_w<0, true>, P, nbatch, wb, st)
@@ -638,7 +626,7 @@ cudaError_t radt_launch_march_fwd_win(const MarchParams &P, int nbatch, cudaStre
 
 cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    const bool comp = P.ws.ilo != nullptr;
+    const bool comp = P.cube_lo != nullptr;
     const size_t wb = bwd_warp_bytes(P.line.ngroups, comp);
     if (comp)
         return P.grid.kind == 0 ? launch_w(k_march_bwd_w<0, true>, P, nbatch, wb, st)

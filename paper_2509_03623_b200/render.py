@@ -7,9 +7,13 @@ from . import binding as B
 
 
 class Renderer:
-    """Holds fields, workspace, cube and gradient buffers on one CUDA device for a batch of scenes."""
+    """Holds fields, workspace, cube and gradient buffers on one CUDA device for a batch of scenes.
 
-    def __init__(self, scenes, device="cuda:0", need_bwd=True):
+    options: radt_options fields (window, skip_empty, win_path, zero_dens_grad) for every call of this object;
+    compensated: keep the low-order words of the cube (cube_lo) so that the adjoint is free of cancellation noise on
+    optically thick rays (the default; include/radt.h radt_render)."""
+
+    def __init__(self, scenes, device="cuda:0", need_bwd=True, options=None, compensated=True):
         import torch
         if not torch.cuda.is_available():
             raise B.RadtError("no CUDA device: the render has no CPU fallback")
@@ -17,10 +21,14 @@ class Renderer:
         self.torch = torch
         self.device = torch.device(device)
         self.desc = B.Descriptors(scenes)
+        self.options = dict(options or {})
+        self.opt = B.make_options(**self.options)
+        self.opt_reuse = B.make_options(**self.options, reuse_setup=1)
         d = self.desc
         host = B.stack_fields(scenes)
         self.dens, self.temp, self.vel = (torch.from_numpy(h).to(self.device) for h in host)
         self.cube = torch.empty(d.cube_shape, dtype=torch.float32, device=self.device)
+        self.cube_lo = torch.empty_like(self.cube) if (compensated and need_bwd) else None
         nbytes = B.radt_workspace_bytes(d, B.PASS_BWD if need_bwd else B.PASS_FWD)
         self.ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         self.need_bwd = need_bwd
@@ -33,15 +41,33 @@ class Renderer:
         self.target = None
         self.sigma = None
 
+    def set_options(self, **kw):
+        """Change this object's radt_options for the calls that follow (a forward and its adjoint must share them)."""
+        self.options.update(kw)
+        self.opt = B.make_options(**self.options)
+        self.opt_reuse = B.make_options(**self.options, reuse_setup=1)
+
     # ---- hot path: every call below is one C-ABI entry point ----
     def render(self, stream=None):
-        B.radt_render(self.desc, self.dens, self.temp, self.vel, self.cube, self.ws, stream)
+        B.radt_render(self.desc, self.dens, self.temp, self.vel, self.cube, self.ws, stream, self.opt, self.cube_lo)
         return self.cube
 
-    def render_bwd(self, dl_dcube=None, stream=None):
+    def render_bwd(self, dl_dcube=None, stream=None, reuse_setup=False, unpack=True):
+        """reuse_setup: the workspace still holds what this object's last render()/render_loss() of the same fields left
+        there.  unpack=False leaves the gradient as packed cells in the workspace (grad_packed())."""
         g = self.dl_dcube if dl_dcube is None else dl_dcube
-        B.radt_render_bwd(self.desc, self.dens, self.temp, self.vel, self.cube, g, self.g_dens, self.g_temp, self.g_vel,
-                          self.ws, stream)
+        outs = (self.g_dens, self.g_temp, self.g_vel) if unpack else (None, None, None)
+        B.radt_render_bwd(self.desc, self.dens, self.temp, self.vel, self.cube, g, *outs, self.ws, stream,
+                          self.opt_reuse if reuse_setup else self.opt, self.cube_lo)
+        return self.g_dens, self.g_temp, self.g_vel
+
+    def grad_packed(self):
+        """View of the packed float4 gradient cells inside the workspace (what ONE all-reduce over ranks sums)."""
+        off, n = B.radt_grad_layout(self.desc)
+        return self.ws[off:off + 4 * n].view(self.torch.float32)
+
+    def unpack_grad(self, stream=None):
+        B.radt_unpack_grad(self.desc, self.ws, self.g_dens, self.g_temp, self.g_vel, stream)
         return self.g_dens, self.g_temp, self.g_vel
 
     def set_target(self, target, sigma):
@@ -56,17 +82,17 @@ class Renderer:
     def render_loss(self, stream=None):
         """forward with the chi^2 data term fused into its epilogue: cube, dl_dcube and loss in one pass."""
         B.radt_render_loss(self.desc, self.dens, self.temp, self.vel, self.target, self.sigma, self.cube, self.dl_dcube,
-                           self.loss, self.ws, stream)
+                           self.loss, self.ws, stream, self.opt, self.cube_lo)
         return self.loss
 
     def fit_step(self, stream=None, fused=True):
-        """forward -> L2 data term -> adjoint (one pass of the whole hot path)."""
+        """forward -> L2 data term -> adjoint (one pass of the whole hot path); the adjoint reuses the forward's setup."""
         if fused:
             self.render_loss(stream)
         else:
             self.render(stream)
             self.l2_loss_grad(stream)
-        self.render_bwd(stream=stream)
+        self.render_bwd(stream=stream, reuse_setup=True)
 
     def set_fields(self, dens=None, temp=None, vel=None):
         for name, val in (("dens", dens), ("temp", temp), ("vel", vel)):

@@ -27,7 +27,7 @@ def test_exports_match_header(lib):
     for name in declared:
         assert hasattr(lib, name), f"{name} declared in include/radt.h but not exported"
     assert sorted(B.EXPORTS) == declared, "binding.EXPORTS must mirror include/radt.h"
-    assert lib.radt_version() == 100
+    assert lib.radt_version() == 200
 
 
 def test_struct_layouts_and_workspace_size(lib):
@@ -73,8 +73,56 @@ def test_null_and_unsupported(lib):
     assert lib.radt_workspace_bytes(None, C.byref(d.line), C.byref(d.grid), 1, 0, C.byref(out)) == -1
     assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 0, 0, C.byref(out)) == -1
     assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 1, 9, C.byref(out)) == -1
-    assert lib.radt_set_option(99, 1) == -1
-    assert lib.radt_set_option(B.OPT_WINDOW, 1) == 0 and lib.radt_get_option(B.OPT_WINDOW) == 1
+
+
+def test_options_struct_defaults_and_size_check(lib):
+    """radt_options: per-call POD with struct_size first; NULL means the defaults radt_options_default writes."""
+    o = B.make_options()
+    assert (o.struct_size, o.window, o.skip_empty, o.win_path, o.zero_dens_grad, o.reuse_setup) == (C.sizeof(B.radt_options), 1, 1, 1, 1, 0)
+    assert B.make_options(window=0, zero_dens_grad=0).window == 0
+    with pytest.raises(KeyError):
+        B.make_options(compensated=1)
+    assert not hasattr(lib, "radt_set_option") and not hasattr(lib, "radt_get_option")     # no process-wide option state
+    d = B.Descriptors(tiny_axisym_scene())
+    bad = B.make_options()
+    bad.struct_size = 8
+    fake = C.c_void_p(0x1000)          # never dereferenced: the options are checked before any device work
+    assert lib.radt_render(d.geom, C.byref(d.line), C.byref(d.grid), 1, C.byref(bad), fake, None, fake, 1 << 30, None) == -1
+    assert b"radt_options" in lib.radt_last_error()
+
+
+def test_forward_adjoint_option_mismatch_is_refused_on_the_host(lib):
+    """The library remembers per cube pointer the options of the forward that wrote it; an adjoint with other options
+    (or another cube_lo choice) fails with RADT_E_INVALID before any device work.  Runs where there is no GPU: the
+    pointers are fakes, and every call that gets past the host checks fails with RADT_E_CUDA."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present: tests/test_gpu_parity.py covers this with real buffers")
+    d = B.Descriptors(tiny_axisym_scene())
+    d.with_fields(0x10000, 0x20000, 0x30000)
+    cube, lo, dl, ws = (C.c_void_p(a) for a in (0x100000, 0x200000, 0x300000, 0x400000))
+    args = (d.geom, C.byref(d.line), C.byref(d.grid), 1)
+    o = B.make_options()
+    assert lib.radt_render(*args, C.byref(o), cube, lo, ws, 1 << 30, None) == -4          # registered, then no device
+    for bad in (B.make_options(window=0), B.make_options(skip_empty=0), B.make_options(win_path=0)):
+        assert lib.radt_render_bwd(*args, C.byref(bad), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -1
+    assert lib.radt_render_bwd(*args, C.byref(o), cube, None, dl, None, None, None, ws, 1 << 30, None) == -1      # cube_lo dropped
+    assert lib.radt_render_bwd(*args, C.byref(o), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -4        # consistent
+    r = B.make_options(reuse_setup=1)
+    assert lib.radt_render(*args, C.byref(r), cube, lo, ws, 1 << 30, None) == -1                                 # adjoint-only option
+    other = C.c_void_p(0x500000)
+    assert lib.radt_render_bwd(*args, C.byref(r), cube, lo, dl, None, None, None, other, 1 << 30, None) == -1    # unknown workspace
+    assert lib.radt_render(*args, C.byref(o), cube, lo, ws, 1 << 30, None) == -4
+    assert lib.radt_render_bwd(*args, C.byref(r), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -4       # same inputs: accepted
+    d.geom[0].incl = 0.3
+    assert lib.radt_render_bwd(*args, C.byref(r), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -1       # other geometry
+
+
+def test_grad_layout(lib):
+    d = B.Descriptors(make_config(1))
+    off, n = B.radt_grad_layout(d)
+    assert n == 4 * d.cells and off % 256 == 0
+    assert off + 4 * n <= B.radt_workspace_bytes(d, B.PASS_BWD)
 
 
 def test_batch_items_must_share_image_shape(lib):
@@ -95,6 +143,8 @@ def test_no_cpu_fallback_without_a_device(lib):
     cube = np.full(d.cube_shape, 7.0, np.float32)
     with pytest.raises(B.RadtError, match="-4"):
         B.radt_render_host(d, *h, cube)
+    with pytest.raises(B.RadtError, match="-4"):
+        B.radt_render_host(d, *h, cube, B.make_options(window=0), np.zeros_like(cube))
     assert np.all(cube == 7.0)
     from paper_2509_03623_b200 import Renderer
     with pytest.raises(B.RadtError):

@@ -11,11 +11,24 @@ from oracle import pyoracle as po
 from synth import (UNIT_CGS, UNIT_JY_PIXEL, co_line, l2_target, make_config, slab_scene, sph_benchmark_scene, tiny_axisym_scene,
                    tiny_sph_scene,
                    tiny_cart_scene)
-from tests.tolerances import GRAD, check, check_cube, check_grad
+from tests.tolerances import check_cube, check_grad
 
 pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
+
+
+class _Family:
+    """The package with one kernel family selected through per-call options (include/radt.h radt_options)."""
+
+    def __init__(self, pkg, **options):
+        self.pkg, self.binding, self.options = pkg, pkg.binding, options
+
+    def Renderer(self, scenes, options=None, **kw):
+        return self.pkg.Renderer(scenes, options={**self.options, **(options or {})}, **kw)
+
+    def opt(self, **kw):
+        return self.binding.make_options(**{**self.options, **kw})
 
 
 @pytest.fixture(scope="module", params=["win", "tab"])
@@ -25,21 +38,11 @@ def rt(request):
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_2509_03623_b200 as pkg
-    B = pkg.binding
-    B.lib()     # fails loudly if the CUDA library was not built
-    B.radt_set_option(B.OPT_WIN_PATH, 1 if request.param == "win" else 0)
-    dense = os.environ.get("RADT_TEST_DENSE") == "1"       # one-off runs of the whole file without windowing / skipping
-    if dense:
-        B.radt_set_option(B.OPT_WINDOW, 0); B.radt_set_option(B.OPT_SKIP_EMPTY, 0)
-    comp = os.environ.get("RADT_TEST_COMP") == "1"         # one-off runs of the whole file with RADT_OPT_COMPENSATED
-    if comp:
-        B.radt_set_option(B.OPT_COMPENSATED, 1)
-    yield pkg
-    if comp:
-        B.radt_set_option(B.OPT_COMPENSATED, 0)
-    B.radt_set_option(B.OPT_WIN_PATH, 1)
-    if dense:
-        B.radt_set_option(B.OPT_WINDOW, 1); B.radt_set_option(B.OPT_SKIP_EMPTY, 1)
+    pkg.binding.lib()     # fails loudly if the CUDA library was not built
+    options = dict(win_path=1 if request.param == "win" else 0)
+    if os.environ.get("RADT_TEST_DENSE") == "1":       # one-off runs of the whole file without windowing / skipping
+        options.update(window=0, skip_empty=0)
+    return _Family(pkg, **options)
 
 
 def _as_list(s):
@@ -50,17 +53,17 @@ def _oracle_cube(scenes):
     return np.stack([po.render(s) for s in _as_list(scenes)])
 
 
-def _gpu_forward(rt, scenes, need_bwd=False):
-    R = rt.Renderer(_as_list(scenes), need_bwd=need_bwd)
+def _gpu_forward(rt, scenes, need_bwd=False, **rkw):
+    R = rt.Renderer(_as_list(scenes), need_bwd=need_bwd, **rkw)
     R.render()
     torch.cuda.synchronize()
     return R
 
 
-def _parity_fwd_bwd(rt, scenes, name, seed=0, grad=True, grad_floor=None):
+def _parity_fwd_bwd(rt, scenes, name, seed=0, grad=True, **rkw):
     scenes = _as_list(scenes)
     ref = _oracle_cube(scenes)
-    R = _gpu_forward(rt, scenes, need_bwd=grad)
+    R = _gpu_forward(rt, scenes, need_bwd=grad, **rkw)
     check_cube(f"{name} cube", R.cube.cpu().numpy(), ref)
     if not grad:
         return R
@@ -79,10 +82,7 @@ def _parity_fwd_bwd(rt, scenes, name, seed=0, grad=True, grad_floor=None):
     for b, sc in enumerate(scenes):
         rd, rtm, rv = po.render_bwd(sc, G32[b].astype(np.float64))
         for nm, got, want in (("dens", gd[b], rd), ("temp", gt[b], rtm), ("vel", gv[b], rv)):
-            if grad_floor is None:
-                check_grad(f"{name}[{b}] g_{nm}", got, want)
-            else:
-                check(f"{name}[{b}] g_{nm}", got, want, GRAD[0], grad_floor)
+            check_grad(f"{name}[{b}] g_{nm}", got, want)
     return R
 
 
@@ -314,15 +314,12 @@ def test_forward_is_deterministic_and_adjoint_linear(rt):
 
 def test_dense_and_skipping_kernels_agree(rt):
     """Channel windowing and empty-step skipping change the cube by less than 1e-6 of its maximum."""
-    B = rt.binding
     sc = make_config(2, npix=64)
     R = rt.Renderer([sc])
-    try:
-        B.radt_set_option(B.OPT_WINDOW, 0); B.radt_set_option(B.OPT_SKIP_EMPTY, 0)
-        dense = R.render().clone()
-        cd = R.counters()
-    finally:
-        B.radt_set_option(B.OPT_WINDOW, 1); B.radt_set_option(B.OPT_SKIP_EMPTY, 1)
+    R.set_options(window=0, skip_empty=0)
+    dense = R.render().clone()
+    cd = R.counters()
+    R.set_options(window=1, skip_empty=1)
     fast = R.render()
     cf = R.counters()
     assert float((dense - fast).abs().max()) <= 1e-6 * float(dense.max())
@@ -365,14 +362,16 @@ def test_host_entry_points(rt):
     d = B.Descriptors(sc)
     h = B.stack_fields(sc)
     cube = np.zeros(d.cube_shape, np.float32)
-    B.radt_render_host(d, *h, cube)
+    cube_lo = np.ones(d.cube_shape, np.float32)
+    B.radt_render_host(d, *h, cube, rt.opt(), cube_lo)
     ref = _oracle_cube(sc)
     check_cube("host cube", cube, ref)
+    assert np.abs(cube_lo).max() <= 1e-5 * cube.max()            # low-order words: a few ulp of the sums
     tgt, sigma = l2_target(ref[0], 3)
     tgt32 = np.ascontiguousarray(tgt[None], np.float32)
     gd, gt, gv = (np.zeros_like(h[0]) for _ in range(3))
     cube2 = np.zeros_like(cube)
-    loss = B.radt_fit_step_host(d, *h, tgt32, sigma, cube2, gd, gt, gv)
+    loss = B.radt_fit_step_host(d, *h, tgt32, sigma, cube2, gd, gt, gv, rt.opt())
     np.testing.assert_array_equal(cube, cube2)
     res = cube.astype(np.float64) - tgt32
     assert loss == pytest.approx(0.5 * np.mean((res / sigma) ** 2), rel=1e-6)
@@ -380,8 +379,10 @@ def test_host_entry_points(rt):
     rd, rtm, rv = po.render_bwd(sc, G[0].astype(np.float64))
     check_grad("host g_dens", gd[0], rd); check_grad("host g_temp", gt[0], rtm); check_grad("host g_vel", gv[0], rv)
     gd2, gt2, gv2 = (np.zeros_like(h[0]) for _ in range(3))
-    B.radt_render_bwd_host(d, *h, cube, G, gd2, gt2, gv2)
+    B.radt_render_bwd_host(d, *h, cube, G, gd2, gt2, gv2, rt.opt(), cube_lo)
     check_grad("host2 g_dens", gd2[0], rd); check_grad("host2 g_temp", gt2[0], rtm); check_grad("host2 g_vel", gv2[0], rv)
+    B.radt_render_bwd_host(d, *h, cube, G, gd2, gt2, gv2, rt.opt())            # without the low-order words
+    check_grad("host3 g_dens", gd2[0], rd); check_grad("host3 g_temp", gt2[0], rtm); check_grad("host3 g_vel", gv2[0], rv)
 
 
 def test_l2_loss_kernel(rt):
@@ -431,12 +432,72 @@ def test_workspace_too_small_and_launch_count(rt):
     R = rt.Renderer([sc])
     small = torch.empty(64, dtype=torch.uint8, device="cuda")
     with pytest.raises(B.RadtError, match="-3"):
-        B.radt_render(R.desc, R.dens, R.temp, R.vel, R.cube, small)
+        B.radt_render(R.desc, R.dens, R.temp, R.vel, R.cube, small, opt=R.opt)
     R.render()
     assert B.radt_last_launch_count() == 2          # setup + march
     R.dl_dcube.fill_(1e-6)
     R.render_bwd()
     assert B.radt_last_launch_count() == 3          # setup + adjoint march + unpack
+    R.render()
+    R.render_bwd(reuse_setup=True)
+    assert B.radt_last_launch_count() == 2          # adjoint march + unpack: the forward's setup is reused
+    R.render_bwd(reuse_setup=True, unpack=False)
+    assert B.radt_last_launch_count() == 1
+
+
+def test_options_are_per_call_and_mismatches_are_refused(rt):
+    """include/radt.h radt_options: no process-wide state; the adjoint of a cube must get the options (and the cube_lo
+    choice) of the forward that wrote it; reuse_setup needs a workspace the same forward set up."""
+    B = rt.binding
+    sc = tiny_axisym_scene(seed=64)
+    R = rt.Renderer([sc])
+    R.dl_dcube.fill_(1e-6)
+    R.render()
+    g_ref = [g.clone() for g in R.render_bwd()]
+    for bad in (dict(window=0), dict(skip_empty=0), dict(win_path=1 - R.opt.win_path)):
+        with pytest.raises(B.RadtError, match="-1"):
+            B.radt_render_bwd(R.desc, R.dens, R.temp, R.vel, R.cube, R.dl_dcube, R.g_dens, R.g_temp, R.g_vel, R.ws,
+                              opt=rt.opt(**bad), cube_lo=R.cube_lo)
+    with pytest.raises(B.RadtError, match="-1"):      # the forward wrote low-order words, the adjoint is not given them
+        B.radt_render_bwd(R.desc, R.dens, R.temp, R.vel, R.cube, R.dl_dcube, R.g_dens, R.g_temp, R.g_vel, R.ws, opt=R.opt)
+    with pytest.raises(B.RadtError, match="-1"):      # reuse_setup is an adjoint option
+        B.radt_render(R.desc, R.dens, R.temp, R.vel, R.cube, R.ws, opt=rt.opt(reuse_setup=1), cube_lo=R.cube_lo)
+    # reuse_setup: refused after an adjoint that rebuilt the workspace for itself, after a forward of another scene ...
+    with pytest.raises(B.RadtError, match="-1"):
+        R.render_bwd(reuse_setup=True)
+    R.render()
+    R2 = rt.Renderer([tiny_axisym_scene(seed=64, incl_deg=33.0)])
+    with pytest.raises(B.RadtError, match="-1"):
+        B.radt_render_bwd(R2.desc, R.dens, R.temp, R.vel, R.cube, R.dl_dcube, R.g_dens, R.g_temp, R.g_vel, R.ws,
+                          opt=R.opt_reuse, cube_lo=R.cube_lo)
+    # ... and accepted right after the forward of the same inputs, with the same result
+    R.render()
+    for a, b in zip(R.render_bwd(reuse_setup=True), g_ref):
+        check_grad("reuse_setup", a.cpu().numpy(), b.cpu().numpy().astype(np.float64))
+    # the packed cells in the workspace are what unpack_grad writes out
+    R.render()
+    R.render_bwd(reuse_setup=True, unpack=False)
+    packed = R.grad_packed().clone().view(-1, 4)
+    for g in (R.g_dens, R.g_temp, R.g_vel):
+        g.zero_()
+    gd, gt, gv = R.unpack_grad()
+    assert torch.equal(packed[:, 0], gd.flatten()) and torch.equal(packed[:, 1], gt.flatten()) and torch.equal(packed[:, 2], gv.flatten())
+    # two renderers with different options side by side: neither changes the other (no global option state)
+    Ra, Rb = rt.Renderer([sc], options=dict(window=0, skip_empty=0)), rt.Renderer([sc])
+    ca, cb = Ra.render().clone(), Rb.render().clone()
+    assert torch.equal(Ra.render(), ca) and torch.equal(Rb.render(), cb) and torch.equal(cb, R.cube)
+
+
+def test_renderer_on_a_device_that_is_not_current(rt):
+    """The binding makes the tensors' device current for every call (a Renderer on cuda:1 while cuda:0 is current)."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    sc = tiny_axisym_scene(seed=65)
+    assert torch.cuda.current_device() == 0
+    R1 = rt.Renderer([sc], device="cuda:1")
+    R0 = rt.Renderer([sc], device="cuda:0")
+    assert torch.equal(R1.render().cpu(), R0.render().cpu())
+    assert torch.cuda.current_device() == 0
 
 
 def test_pipe_peaks_are_sane(rt):
@@ -527,10 +588,15 @@ def test_random_scenes(rt, seed):
 
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_MEDIUM", "6"))))
 def test_random_medium_scenes(rt, seed):
-    """Hundreds of steps through optically thick LN grids: the fp32 cancellation of the front-to-back adjoint (DESIGN.md
-    section 6) leaves isolated cells off by up to 3e-5 of the field's maximum (6 of 150 seeds, max and L2 norms below
-    1e-4 throughout), so the element-wise floor is 1e-4 of the maximum here instead of 1e-5."""
-    _parity_fwd_bwd(rt, _random_scene(seed, medium=True), f"random medium scene {seed}", seed=seed, grad_floor=1e-4)
+    """Hundreds of steps per ray, many of them through optically thick LN grids (candidate queues, step pairs and
+    zero-opacity runs span many 32-step batches); the criteria of tests/tolerances.py as everywhere."""
+    _parity_fwd_bwd(rt, _random_scene(seed, medium=True), f"random medium scene {seed}", seed=seed)
+
+
+@pytest.mark.parametrize("seed", [81, 97, 143])
+def test_random_medium_scenes_that_once_needed_a_wider_floor(rt, seed):
+    """The three medium scenes on which the uncompensated adjoint left isolated cells 3e-5 of the maximum off."""
+    _parity_fwd_bwd(rt, _random_scene(seed, medium=True), f"random medium scene {seed}", seed=seed)
 
 
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_OFFCENTRE", "8"))))
@@ -554,72 +620,41 @@ def test_batches_of_3d_scenes(rt, kind):
     _parity_fwd_bwd(rt, scs, f"batch of 3 {kind}")
 
 
-def test_optically_thick_central_ray_gradient_bound(rt):
-    """Known limit of the front-to-back adjoint: R_k = I_saved - P_k carries the rounding of the
-    forward's own fp32 sum (~1e-7 I).  On a ray that is optically thick in EVERY channel from its first steps
-    (random scene 228: edge-on ray through the star, 33 channels inside the line core, tau ~ 0.25 per step) all gradient
-    terms sit where T S - R cancels to ~1e-2 of its parts, and the density gradient is good to 7e-4 of its maximum
-    instead of the usual 1e-6: inside BASELINE.json's 1e-3 in the max and L2 norms, outside the element-wise
-    criterion with the 1e-5 floor.  The test pins that behaviour."""
-    sc = _random_scene(228)
-    scenes = [sc]
-    ref = _oracle_cube(scenes)
-    R = _gpu_forward(rt, scenes, need_bwd=True)
-    check_cube("thick central ray cube", R.cube.cpu().numpy(), ref)
+def test_optically_thick_central_ray(rt):
+    """Random scene 228: an edge-on ray through the star, optically thick in EVERY channel from its first steps (33
+    channels inside the line core, tau ~ 0.25 per step).  Every gradient term sits where T S - R cancels to ~1e-2 of its
+    parts, so R_k = I - I_{<=k} must not carry the rounding of the forward's fp32 sum: the low-order words (cube_lo)
+    remove it and the strict criteria hold in both kernel families."""
+    _parity_fwd_bwd(rt, _random_scene(228), "thick central ray", seed=228)
+
+
+@pytest.mark.parametrize("case", ["thick228", "cfg1"])
+def test_adjoint_without_low_order_words(rt, case):
+    """cube_lo = NULL (compensated=False): the cube is the same bit for bit; the adjoint still meets BASELINE.json's 1e-3
+    in the max and L2 norms on the thick ray (element-wise it is the known limit of the plain fp32 difference,
+    DESIGN.md section 6) and the strict criteria on an ordinary scene."""
+    sc = {"thick228": lambda: _random_scene(228), "cfg1": lambda: make_config(1)}[case]()
+    ref = _oracle_cube([sc])
+    Rc = _gpu_forward(rt, [sc], need_bwd=True)
+    R = _gpu_forward(rt, [sc], need_bwd=True, compensated=False)
+    assert R.cube_lo is None and Rc.cube_lo is not None
+    np.testing.assert_array_equal(R.cube.cpu().numpy(), Rc.cube.cpu().numpy())
     tgt, sigma = l2_target(ref[0], 1000 + 228)
     G32 = ((ref[0] - tgt) / (sigma ** 2 * ref[0].size)).astype(np.float32)[None]
     R.dl_dcube.copy_(torch.from_numpy(G32))
     got = [g.cpu().numpy()[0].astype(np.float64) for g in R.render_bwd()]
     want = po.render_bwd(sc, G32[0].astype(np.float64))
-    for nm, a, b in zip(("dens", "temp"), got, want):          # (v_los vanishes on this ray: dL/dv = 1e-25)
-        m = np.abs(b).max()
-        assert np.abs(a - b).max() <= 1e-3 * m and np.linalg.norm(a - b) <= 1e-3 * np.linalg.norm(b), nm
-    check_grad("thick central ray g_temp", got[1], want[1])
-
-
-def _with_compensation(rt):
-    B = rt.binding
-    return B, B.radt_get_option(B.OPT_WIN_PATH) == 1
-
-
-@pytest.mark.parametrize("case", ["thick228", "medium81", "medium97", "medium143", "cfg1"])
-def test_compensated_adjoint(rt, case):
-    """RADT_OPT_COMPENSATED: the forward keeps the low-order word of its fp32 sum in the workspace and the adjoint forms
-    R_k = I - I_{<=k} from both words.  Same cube bit for bit; the scenes that exceed the element-wise gradient floor
-    without it (optically thick rays) now pass the strict criteria.  Window kernels only."""
-    B, win = _with_compensation(rt)
-    if not win:
-        pytest.skip("the channel-table kernels do not carry the low-order words")
-    sc = {"thick228": lambda: _random_scene(228), "medium81": lambda: _random_scene(81, medium=True),
-          "medium97": lambda: _random_scene(97, medium=True), "medium143": lambda: _random_scene(143, medium=True),
-          "cfg1": lambda: make_config(1)}[case]()
-    plain = _gpu_forward(rt, [sc]).cube.cpu().numpy()
-    B.radt_set_option(B.OPT_COMPENSATED, 1)
-    try:
-        R = _parity_fwd_bwd(rt, sc, f"compensated {case}")           # strict floors
-        np.testing.assert_array_equal(R.cube.cpu().numpy(), plain)
-        # a workspace that does not hold this cube's words falls back to the plain difference, voxel by voxel
-        R.ws.zero_()
-        g0 = [g.clone() for g in (R.g_dens, R.g_temp, R.g_vel)]
-        R.render_bwd()
-        B.radt_set_option(B.OPT_COMPENSATED, 0)
-        R2 = rt.Renderer([sc])
-        R2.render()
-        R2.dl_dcube.copy_(R.dl_dcube)
-        R2.render_bwd()
-        for a, b in zip((R.g_dens, R.g_temp, R.g_vel), (R2.g_dens, R2.g_temp, R2.g_vel)):
-            m = float(b.abs().max())
-            assert float((a - b).abs().max()) <= 2e-5 * m + 1e-30        # same arithmetic up to the order of the atomics
-        del g0
-    finally:
-        B.radt_set_option(B.OPT_COMPENSATED, 0)
+    for nm, a, b in zip(("dens", "temp", "vel"), got, want):
+        if case == "cfg1":
+            check_grad(f"plain adjoint g_{nm}", a, b)
+        elif np.abs(b).max() > 1e-20:          # (v_los vanishes on this ray: dL/dv = 1e-25)
+            assert np.abs(a - b).max() <= 1e-3 * np.abs(b).max() and np.linalg.norm(a - b) <= 1e-3 * np.linalg.norm(b), nm
 
 
 @pytest.mark.parametrize("make", [lambda: make_config(2, npix=48), lambda: tiny_axisym_scene(seed=91, nstep=40)])
 def test_skip_zero_opacity_steps_in_the_adjoint(rt, make):
-    """RADT_OPT_ZERO_DENS_GRAD = 0: steps without opacity are not marched in the adjoint.  They only carry dL/dn of
+    """radt_options.zero_dens_grad = 0: steps without opacity are not marched in the adjoint.  They only carry dL/dn of
     cells whose density is exactly zero, so g_temp, g_vel and g_dens at non-zero cells equal the exact gradient."""
-    B = rt.binding
     sc = make()
     d = np.array(sc.grid.dens)
     if not (d == 0).any():                       # the tiny scene has no masked cells of its own
@@ -631,12 +666,10 @@ def test_skip_zero_opacity_steps_in_the_adjoint(rt, make):
     want = po.render_bwd(sc, G32.astype(np.float64))
     R = _gpu_forward(rt, [sc], need_bwd=True)
     R.dl_dcube.copy_(torch.from_numpy(G32[None]))
-    B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 0)
-    try:
-        gd, gt, gv = (g.cpu().numpy()[0].astype(np.float64) for g in R.render_bwd())
-        steps_skip = R.counters()[2]
-    finally:
-        B.radt_set_option(B.OPT_ZERO_DENS_GRAD, 1)
+    R.set_options(zero_dens_grad=0)
+    gd, gt, gv = (g.cpu().numpy()[0].astype(np.float64) for g in R.render_bwd())
+    steps_skip = R.counters()[2]
+    R.set_options(zero_dens_grad=1)
     R.render_bwd()
     steps_all = R.counters()[2]
     assert steps_skip < steps_all
