@@ -1,18 +1,18 @@
-"""Host-side sharding of ONE image across ranks: rays are independent.
+"""Host-side sharding of one render call across ranks: rays are independent
+(PAPER.md:272), so the work splits by BATCH ITEMS first and by IMAGE ROWS second.
 
-A slab of image rows [r0, r1) is itself a valid image description, so sharding needs no kernel support:
+A slab of image rows [r0, r1) of one item is itself a valid image description, so sharding needs no kernel support:
     ny' = r1 - r0,   fov_y' = fov_y * ny' / ny,   y0' = y0 + ((r0 + r1)/2 - ny/2) * fov_y / ny
-The forward needs no collective (each rank owns its cube rows); the adjoint needs one all-reduce(sum) of
-the three gradient buffers, because every rank's rays scatter into the same grid.
+The forward needs no collective (each rank owns its cube rows).  The adjoint leaves each rank with partial gradients of
+the (replicated) grids; they are summed by ONE all-reduce over the packed float4 gradient cells [batch][cells][4] -- the
+buffer the adjoint march accumulates into, before it is unpacked into the three planes -- on the adjoint's stream.
 
-The `engine` does the rendering: on GPUs it is `CudaEngine` (the C-ABI path, NCCL for the reduction);
-tests inject a CPU engine and the gloo backend to cover this plumbing without a GPU.
+The `engine` does the rendering: on GPUs it is `CudaEngine` (the C-ABI path; the all-reduce then runs over NCCL); tests inject
+a CPU engine and the gloo backend to cover this plumbing without a GPU.
 """
 from __future__ import annotations
 
 from dataclasses import replace
-
-import numpy as np
 
 
 def plan_rows(ny: int, world: int):
@@ -26,72 +26,137 @@ def plan_rows(ny: int, world: int):
     return out
 
 
+def plan_units(batch: int, ny: int, world: int):
+    """Work units [(item, r0, r1)] per rank: batch items first, image rows second.
+
+    world <= batch: every rank gets whole items (contiguous, balanced; no item is split).
+    world >  batch: the ranks are dealt to the items (contiguous, balanced) and each item's rows are split among its ranks.
+    Every (item, row) is covered exactly once; a rank may be left without work only if an item has fewer rows than ranks."""
+    if batch < 1 or ny < 1 or world < 1:
+        raise ValueError("need batch, ny, world >= 1")
+    if world <= batch:
+        return [[(b, 0, ny) for b in range(a, e)] for a, e in plan_rows(batch, world)]
+    out = []
+    for b, (k0, k1) in enumerate(plan_rows(world, batch)):      # ranks k0..k1-1 serve item b
+        for r0, r1 in plan_rows(ny, k1 - k0):
+            out.append([(b, r0, r1)] if r1 > r0 else [])
+    return out
+
+
 def row_slab_scene(scene, r0: int, r1: int):
     """The sub-image made of rows r0..r1-1 of `scene` (same pixel centres, same pixel size)."""
     g = scene.geom
     if not (0 <= r0 < r1 <= g.ny):
         raise ValueError("need 0 <= r0 < r1 <= ny")
+    if r0 == 0 and r1 == g.ny:
+        return scene
     pix = g.fov_y / g.ny
     sub = replace(g, ny=r1 - r0, fov_y=pix * (r1 - r0), y0=g.y0 + (0.5 * (r0 + r1) - 0.5 * g.ny) * pix)
     return replace(scene, geom=sub)
 
 
 class CudaEngine:
-    """Product engine: the CUDA render through the C ABI."""
+    """Product engine: the CUDA render of a list of same-shaped scenes (one batched call) through the C ABI."""
 
-    def __init__(self, scene, device):
+    def __init__(self, scenes, device):
         from .render import Renderer
-        self.R = Renderer([scene], device=device)
+        self.R = Renderer(list(scenes), device=device)
 
     def render(self):
-        return self.R.render()[0]
+        return self.R.render()
 
-    def render_bwd(self, dl_dcube):
-        self.R.dl_dcube.copy_(dl_dcube.reshape(self.R.dl_dcube.shape))
-        return [g[0] for g in self.R.render_bwd()]
+    def render_bwd_packed(self, dl_dcube):
+        """Adjoint without unpacking: returns the packed cells [n, cells * 4] as a VIEW into the workspace."""
+        R = self.R
+        R.dl_dcube.copy_(dl_dcube.reshape(R.dl_dcube.shape))
+        R.render_bwd(unpack=False)
+        return R.grad_packed().view(R.desc.batch, -1)
+
+    def unpack(self):
+        """k_unpack_grad on the workspace's own cells (after they were all-reduced in place)."""
+        return self.R.unpack_grad()
 
 
-class ShardedImage:
-    """One image split by rows over the ranks of a torch.distributed process group."""
+class ShardedRender:
+    """One render call (a batch of scenes that share line, grid layout and image size) split over the ranks of a
+    torch.distributed process group.  `engine_factory(scenes)` builds an engine for a list of same-shaped scenes with
+    render() -> [n, ny', nx, nchan] and render_bwd_packed(dl) -> [n, cells * 4]."""
 
-    def __init__(self, scene, engine_factory, rank=None, world=None, group=None):
+    def __init__(self, scenes, engine_factory, rank=None, world=None, group=None):
         import torch.distributed as dist
         self.dist, self.group = dist, group
         self.rank = dist.get_rank(group) if rank is None else rank
         self.world = dist.get_world_size(group) if world is None else world
-        self.scene = scene
-        self.rows = plan_rows(scene.geom.ny, self.world)
-        r0, r1 = self.rows[self.rank]
-        self.r0, self.r1 = r0, r1
-        self.engine = engine_factory(row_slab_scene(scene, r0, r1)) if r1 > r0 else None
+        self.scenes = list(scenes) if isinstance(scenes, (list, tuple)) else [scenes]
+        s0 = self.scenes[0]
+        self.batch, self.ny, self.nx, self.nchan = len(self.scenes), s0.geom.ny, s0.geom.nx, len(s0.line.vchan)
+        self.grid_shape = tuple(s0.grid.n)
+        self.cells = 1
+        for n in self.grid_shape:
+            self.cells *= int(n)
+        self.plan = plan_units(self.batch, self.ny, self.world)
+        self.units = self.plan[self.rank]
+        # one engine per slab height (all units of a rank have the same height unless rows do not divide evenly)
+        self.groups = {}
+        for u in self.units:
+            self.groups.setdefault(u[2] - u[1], []).append(u)
+        self.engines = {h: engine_factory([row_slab_scene(self.scenes[b], r0, r1) for b, r0, r1 in us])
+                        for h, us in self.groups.items()}
 
+    # ---- forward: no communication
     def render(self):
-        """This rank's rows of the cube, [r1 - r0, nx, nchan] (no communication)."""
-        return self.engine.render() if self.engine is not None else None
+        """This rank's cube slabs: {(item, r0, r1): tensor [r1 - r0, nx, nchan]}."""
+        out = {}
+        for h, us in self.groups.items():
+            cube = self.engines[h].render()
+            for k, u in enumerate(us):
+                out[u] = cube[k]
+        return out
 
-    def gather_cube(self, slab):
-        """All ranks' slabs concatenated along rows (all_gather; only when one rank needs the whole cube)."""
+    def gather_cube(self, slabs):
+        """The whole cube [batch, ny, nx, nchan] on every rank (all_gather of padded slabs; only when one rank needs it)."""
         import torch
-        nx, nchan = self.scene.geom.nx, len(self.scene.line.vchan)
-        parts = [torch.empty((b - a, nx, nchan), dtype=slab.dtype if slab is not None else torch.float32,
-                             device=slab.device if slab is not None else "cpu") for a, b in self.rows]
-        mine = slab if slab is not None else parts[self.rank]
-        # all_gather needs equal shapes: pad to the largest slab
-        hmax = max(b - a for a, b in self.rows)
-        pad = torch.zeros((hmax, nx, nchan), dtype=mine.dtype, device=mine.device)
-        pad[: mine.shape[0]] = mine
+        any_slab = next(iter(slabs.values())) if slabs else None
+        dev = any_slab.device if any_slab is not None else "cpu"
+        nmax = max(sum(r1 - r0 for _, r0, r1 in us) for us in self.plan)
+        pad = torch.zeros((max(nmax, 1), self.nx, self.nchan), dtype=torch.float32, device=dev)
+        row = 0
+        for u in self.units:
+            pad[row:row + u[2] - u[1]] = slabs[u]
+            row += u[2] - u[1]
         bufs = [torch.empty_like(pad) for _ in range(self.world)]
         self.dist.all_gather(bufs, pad, group=self.group)
-        return torch.cat([bufs[k][: b - a] for k, (a, b) in enumerate(self.rows)], dim=0)
+        cube = torch.empty((self.batch, self.ny, self.nx, self.nchan), dtype=torch.float32, device=dev)
+        for k, us in enumerate(self.plan):
+            row = 0
+            for b, r0, r1 in us:
+                cube[b, r0:r1] = bufs[k][row:row + r1 - r0]
+                row += r1 - r0
+        return cube
 
-    def render_bwd(self, dl_dcube_slab):
-        """Gradients w.r.t. the (replicated) grid: local adjoint of this rank's rows, then all_reduce(sum)."""
+    # ---- adjoint: ONE all-reduce over the packed gradient cells
+    def render_bwd(self, dl_slabs):
+        """dl_slabs: {(item, r0, r1): dL/dcube of that slab}.  Returns (g_dens, g_temp, g_vel), each [batch, *grid], the
+        same on every rank (the grids are replicated)."""
         import torch
-        if self.engine is not None:
-            grads = [g.clone() for g in self.engine.render_bwd(dl_dcube_slab)]
-        else:
-            shape = tuple(self.scene.grid.n)
-            grads = [torch.zeros(shape, dtype=torch.float32) for _ in range(3)]
-        for g in grads:
-            self.dist.all_reduce(g, op=self.dist.ReduceOp.SUM, group=self.group)
-        return grads
+        acc, inplace = None, None
+        full = [(b, 0, self.ny) for b in range(self.batch)]
+        for h, us in self.groups.items():
+            dl = torch.stack([dl_slabs[u] for u in us])
+            packed = self.engines[h].render_bwd_packed(dl)            # [n, cells * 4]
+            if acc is None and len(self.groups) == 1 and [u[0] for u in us] == list(range(self.batch)):
+                acc, inplace = packed, self.engines[h]               # this rank's cells already span the whole batch
+                continue
+            if acc is None:
+                acc = torch.zeros((self.batch, self.cells * 4), dtype=torch.float32, device=packed.device)
+            for k, (b, _, _) in enumerate(us):
+                acc[b] += packed[k]
+        if acc is None:                                              # a rank without work still joins the collective
+            dev = "cuda" if self.dist.get_backend(self.group) == "nccl" else "cpu"
+            acc = torch.zeros((self.batch, self.cells * 4), dtype=torch.float32, device=dev)
+        del full
+        self.dist.all_reduce(acc, op=self.dist.ReduceOp.SUM, group=self.group)      # the ONE collective of the adjoint
+        if inplace is not None and hasattr(inplace, "unpack"):
+            return inplace.unpack()
+        cells = acc.view(self.batch, self.cells, 4)
+        return tuple(cells[:, :, k].reshape((self.batch,) + self.grid_shape).contiguous() for k in range(3))
