@@ -222,6 +222,43 @@ def time_kernel_group(fn, stream, torch, flush, reps):
     return tot / reps
 
 
+def aggregate_ms(ms_total, ctx):
+    """Time of the K steps as the MAX over ranks (device timing per rank; one all-reduce on the rank's own device)."""
+    if ctx["world"] == 1:
+        return ms_total
+    torch, dist = ctx["torch"], ctx["dist"]
+    t = torch.tensor([ms_total], dtype=torch.float64, device=ctx["reduce_device"])
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(nominal_per_rank, steps, ms_total_max, world):
+    """Aggregate throughput over all ranks: every rank processes `nominal_per_rank` samples per step (weak scaling)."""
+    return world * nominal_per_rank * steps / (ms_total_max * 1e-3)
+
+
+def measure_config_dry(cfg, args, ctx, with_cpu):
+    """--dry-run: no GPU work.  Every rank 'takes' (1 + rank) x 1 ms per step; exercises the rank / barrier / max-over-ranks /
+    aggregation / rank-0-prints logic of the multi-rank bench on CPU (gloo), tests/test_shard_gloo.py."""
+    world, rank = ctx["world"], ctx["rank"]
+    nominal = {1: 3932160, 2: 1073741824, 3: 17179869184, 4: 8589934592, 5: 274877906944, 6: 1073741824}[cfg]
+    if world > 1:
+        ctx["dist"].barrier()
+    ms_total = aggregate_ms(args.steps * 1.0 * (1 + rank), ctx)
+    if world > 1:
+        ctx["dist"].barrier()
+    if rank != 0:
+        return None
+    res = {k: None for k in ("fwd_value", "fwd_ms", "fwd_loss_fused_ms", "l2_ms", "bwd_ms", "bwd_ms_own_setup",
+                             "bwd_ms_zero_dens_grad_off", "step_ms_without_cube_lo", "executed_samples", "roofline",
+                             "roofline_other", "e2e", "e2e_render", "launches_per_step", "clocks", "cpu_baseline", "loss",
+                             "wall_s")}
+    res.update(config={"workload": _workload_name(cfg), "nominal_samples_per_step": nominal, "parallelism": f"independent disks x{world}"},
+               value=whole_job_value(nominal, args.steps, ms_total, world), unit=UNIT, steps=args.steps,
+               warmup=max(args.warmup, 3), ms_per_step=ms_total / args.steps, gpu_launches=0)
+    return res
+
+
 def _load_traffic():
     """DRAM bytes per launch from the committed ncu captures (profiles/traffic_r02.json, one entry per config and kernel);
     configs without a capture report null."""
@@ -291,14 +328,10 @@ def measure_config(cfg, args, ctx, with_cpu):
         dist.barrier()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
-    ms_total = sum(a.elapsed_time(b) for a, b in events)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=R.device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = aggregate_ms(sum(a.elapsed_time(b) for a, b in events), ctx)
     loss = float(R.loss.cpu())
     ms_step = ms_total / args.steps
-    value = world * nominal * args.steps / (ms_total * 1e-3)
+    value = whole_job_value(nominal, args.steps, ms_total, world)
     if rank != 0:
         return None
 
@@ -435,39 +468,51 @@ def prepass_times(ctx, args):
 def run_ours(args, configs):
     import torch
     import torch.distributed as dist
-    from paper_2509_03623_b200 import Renderer, binding as B
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
+    dry = args.dry_run
+    if not dry and not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the render has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    B.lib()
-    ctx = {"torch": torch, "dist": dist, "B": B, "Renderer": Renderer, "world": world, "rank": rank, "local": local,
-           "flush_buf": torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}"),     # > 126 MB L2
-           "traffic": _load_traffic()}
-    # roofline denominators: issue peaks measured now, at the clock the GPU runs at
-    ctx["mufu_peak"], ctx["mufu_clk"] = B.radt_pipe_peak(0)
-    ctx["ffma_peak"], _ = B.radt_pipe_peak(1)
+    ctx = {"torch": torch, "dist": dist, "world": world, "rank": rank, "local": local, "traffic": _load_traffic()}
+    if dry:
+        if world > 1:
+            dist.init_process_group("gloo")
+        ctx["reduce_device"] = "cpu"
+        ctx["mufu_peak"] = ctx["ffma_peak"] = ctx["mufu_clk"] = None
+        measure = measure_config_dry
+    else:
+        from paper_2509_03623_b200 import Renderer, binding as B
+        torch.cuda.set_device(local)
+        if world > 1:
+            # NCCL_DEBUG=INFO (if the launcher sets it) shows the ranks and NVLS; the only collectives of this bench are the
+            # barriers around the timed region and the max-over-ranks of its duration
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        B.lib()
+        ctx.update(B=B, Renderer=Renderer, reduce_device=f"cuda:{local}",
+                   flush_buf=torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}"))     # > 126 MB L2
+        # roofline denominators: issue peaks measured now, at the clock the GPU runs at
+        ctx["mufu_peak"], ctx["mufu_clk"] = B.radt_pipe_peak(0)
+        ctx["ffma_peak"], _ = B.radt_pipe_peak(1)
+        measure = measure_config
 
     head = configs[0] if len(configs) == 1 else (HEADLINE if HEADLINE in configs else configs[-1])
     results = {}
     t_start = time.perf_counter()
     for cfg in configs:
         t0 = time.perf_counter()
-        res = measure_config(cfg, args, ctx, with_cpu=(cfg == head and world == 1 and not args.no_cpu_baseline))
+        res = measure(cfg, args, ctx, with_cpu=(cfg == head and world == 1 and not args.no_cpu_baseline))
         if res is not None:
             res["bench_wall_s"] = time.perf_counter() - t0
             results[cfg] = res
-        torch.cuda.empty_cache()
+        if not dry:
+            torch.cuda.empty_cache()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    prepass = prepass_times(ctx, args) if (world == 1 and not args.no_prepass) else None
+    prepass = prepass_times(ctx, args) if (world == 1 and not args.no_prepass and not dry) else None
 
     H = results[head]
     keep = ("config", "value", "ms_per_step", "steps", "fwd_value", "fwd_ms", "fwd_loss_fused_ms", "l2_ms", "bwd_ms",
@@ -488,6 +533,8 @@ def run_ours(args, configs):
         "per_config": per_config, "prepass": prepass, "bench_total_wall_s": time.perf_counter() - t_start,
         "context": "paper: ~10,000x vs RADMC-3D, ~100 ms per cube, A6000 vs Xeon Gold 6348 (PAPER.md:302-304); another machine and workload",
     }
+    if dry:
+        line["dry_run"] = True
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -504,6 +551,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-prepass", action="store_true")
+    ap.add_argument("--dry-run", action="store_true", help="no GPU work: exercise the multi-rank timing / aggregation logic on CPU (gloo)")
     ap.add_argument("--win-path", type=int, default=1, choices=[0, 1],
                     help="radt_options.win_path: 1 = window kernels on uniform channel lattices (default), 0 = channel-table kernels")
     ap.add_argument("--sph-npix", type=int, default=256, help="config 6: image size (the paper sweeps it at 20 channels)")

@@ -702,3 +702,36 @@ def test_skip_zero_opacity_steps_in_the_adjoint(rt, make):
     m = np.abs(want[0]).max()
     assert np.all(np.abs(gd[nz] - want[0][nz]) <= 1e-3 * np.abs(want[0][nz]) + 1e-5 * m)
     assert np.all(np.isfinite(gd[~nz]))          # zero-density cells keep what the emitting steps around them contribute
+
+
+# ------------------------------------------------------------------ multi-GPU plumbing on one GPU (world size 1, NCCL)
+def test_sharded_render_cuda_engine_nccl_world1():
+    """shard.ShardedRender with the product engine (CudaEngine) and the NCCL backend at world size 1: the packed gradient
+    cells are all-reduced IN the workspace (one collective on the device, batch 1) or in a whole-batch buffer (batch 3) and
+    unpacked afterwards; results equal a plain Renderer.  (Two-rank plans run on CPU: tests/test_shard_gloo.py.)"""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import socket
+    import torch.distributed as dist
+    from paper_2509_03623_b200 import Renderer
+    from paper_2509_03623_b200.shard import CudaEngine, ShardedRender
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        for batch in (1, 3):
+            scs = [tiny_axisym_scene(seed=130 + b, npix=6, npix_y=7, incl_deg=30.0 + 10 * b) for b in range(batch)]
+            sh = ShardedRender(scs, lambda group: CudaEngine(group, "cuda:0"))
+            slabs = sh.render()
+            R = Renderer(scs)
+            R.render()
+            cube = sh.gather_cube(slabs)
+            assert torch.equal(cube, R.cube)
+            G = torch.randn_like(R.cube) * 1e-6
+            R.dl_dcube.copy_(G)
+            want = [g.clone() for g in R.render_bwd()]
+            got = sh.render_bwd({u: G[u[0], u[1]:u[2]] for u in sh.units})
+            for a, b in zip(got, want):
+                check_grad("sharded adjoint", a.cpu().numpy(), b.cpu().numpy().astype(np.float64))
+    finally:
+        dist.destroy_process_group()

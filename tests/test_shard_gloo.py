@@ -1,7 +1,11 @@
-"""World-size-2 gloo test (CPU) of the multi-GPU host logic: row-slab geometry, cube gather, gradient all-reduce.
+"""World-size-2 gloo tests (CPU) of the multi-GPU host logic: batch-first / rows-second work plan,
+row-slab geometry, cube gather, ONE all-reduce over the packed gradient cells, and bench.py's rank / aggregation logic.
 The render engine injected here is the CPU oracle; on GPUs the same plumbing drives the CUDA engine over NCCL."""
+import json
 import os
 import socket
+import subprocess
+import sys
 
 import numpy as np
 import pytest
@@ -10,8 +14,10 @@ import torch.distributed as dist
 import torch.multiprocessing as mp
 
 from oracle import pyoracle as po
-from paper_2509_03623_b200.shard import ShardedImage, plan_rows, row_slab_scene
+from paper_2509_03623_b200.shard import ShardedRender, plan_rows, plan_units, row_slab_scene
 from synth import tiny_axisym_scene
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def test_plan_rows_covers_every_row_once():
@@ -23,49 +29,112 @@ def test_plan_rows_covers_every_row_once():
         assert max(sizes) - min(sizes) <= 1
 
 
+@pytest.mark.parametrize("batch,ny,world", [(16, 512, 1), (16, 512, 2), (16, 512, 8), (16, 512, 16), (16, 512, 32), (3, 7, 2),
+                                            (1, 7, 2), (1, 512, 8), (2, 5, 8), (5, 9, 3), (3, 4, 7)])
+def test_plan_units_batch_items_first_then_rows(batch, ny, world):
+    plan = plan_units(batch, ny, world)
+    assert len(plan) == world
+    seen = np.zeros((batch, ny), int)
+    for us in plan:
+        for b, r0, r1 in us:
+            assert 0 <= r0 < r1 <= ny
+            seen[b, r0:r1] += 1
+    assert np.all(seen == 1)                                   # every (item, row) exactly once
+    if world <= batch:
+        assert all(r0 == 0 and r1 == ny for us in plan for _, r0, r1 in us)      # items are never split
+        n = [len(us) for us in plan]
+        assert max(n) - min(n) <= 1
+    else:
+        assert all(len(us) <= 1 for us in plan)                # one slab of one item per rank
+        per_item = [sum(1 for us in plan for u in us if u[0] == b) for b in range(batch)]
+        assert max(per_item) - min(per_item) <= 1 or ny < max(per_item)
+
+
 def test_row_slab_is_the_same_pixels():
     sc = tiny_axisym_scene(seed=71, npix=6, npix_y=7)
     full = po.render(sc)
-    for r0, r1 in ((0, 3), (3, 7), (2, 5), (6, 7)):
+    for r0, r1 in ((0, 3), (3, 7), (2, 5), (6, 7), (0, 7)):
         np.testing.assert_allclose(po.render(row_slab_scene(sc, r0, r1)), full[r0:r1], rtol=1e-11, atol=1e-300)
     with pytest.raises(ValueError):
         row_slab_scene(sc, 3, 3)
 
 
 class _OracleEngine:
-    def __init__(self, scene):
-        self.scene = scene
+    """CPU stand-in for shard.CudaEngine: a list of same-shaped scenes, packed float4 gradient cells out."""
+
+    def __init__(self, scenes):
+        self.scenes = scenes
 
     def render(self):
-        return torch.from_numpy(po.render(self.scene).astype(np.float32))
+        return torch.from_numpy(np.stack([po.render(s) for s in self.scenes]).astype(np.float32))
 
-    def render_bwd(self, g):
-        return [torch.from_numpy(x.astype(np.float32)) for x in po.render_bwd(self.scene, g.numpy().astype(np.float64))]
+    def render_bwd_packed(self, g):
+        out = []
+        for s, gi in zip(self.scenes, g):
+            gd, gt, gv = po.render_bwd(s, gi.numpy().astype(np.float64))
+            out.append(np.stack([gd, gt, gv, np.zeros_like(gd)], axis=-1).reshape(-1))
+        return torch.from_numpy(np.stack(out).astype(np.float32))
 
 
-def _worker(rank, world, port, out):
+def _scenes(batch):
+    return [tiny_axisym_scene(seed=72 + b, npix=6, npix_y=7, incl_deg=30.0 + 10 * b) for b in range(batch)]
+
+
+def _worker(rank, world, port, out, batch):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), OMP_NUM_THREADS="2")
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        sc = tiny_axisym_scene(seed=72, npix=6, npix_y=7)
-        sh = ShardedImage(sc, _OracleEngine)
-        slab = sh.render()
-        cube = sh.gather_cube(slab)
-        G = torch.from_numpy(np.random.default_rng(5).standard_normal(sc.cube_shape).astype(np.float32))
-        grads = sh.render_bwd(G[sh.r0:sh.r1])
+        scs = _scenes(batch)
+        sh = ShardedRender(scs, _OracleEngine)
+        calls = []
+        orig = dist.all_reduce
+        dist.all_reduce = lambda *a, **k: (calls.append(1), orig(*a, **k))[1]
+        slabs = sh.render()
+        cube = sh.gather_cube(slabs)
+        G = torch.from_numpy(np.random.default_rng(5).standard_normal((batch,) + scs[0].cube_shape).astype(np.float32))
+        grads = sh.render_bwd({u: G[u[0], u[1]:u[2]] for u in sh.units})
+        dist.all_reduce = orig
         if rank == 0:
-            torch.save({"cube": cube, "grads": grads, "G": G}, out)
+            torch.save({"cube": cube, "grads": grads, "G": G, "units": sh.plan, "n_allreduce": len(calls)}, out)
     finally:
         dist.destroy_process_group()
 
 
-def test_two_rank_sharded_image_matches_single_process(tmp_path):
+@pytest.mark.parametrize("batch", [1, 3])
+def test_two_rank_sharded_render_matches_single_process(tmp_path, batch):
+    """batch 1: one image split by rows over the two ranks; batch 3: whole items per rank (2 + 1).  Either way the adjoint
+    issues exactly ONE all-reduce (the packed cells of the whole batch) and every rank ends with the full gradient."""
     s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
     out = str(tmp_path / "res.pt")
-    mp.spawn(_worker, args=(2, port, out), nprocs=2, join=True)
+    mp.spawn(_worker, args=(2, port, out, batch), nprocs=2, join=True)
     res = torch.load(out)
-    sc = tiny_axisym_scene(seed=72, npix=6, npix_y=7)
-    np.testing.assert_allclose(res["cube"].numpy(), po.render(sc), rtol=1e-6, atol=1e-30)
-    ref = po.render_bwd(sc, res["G"].numpy().astype(np.float64))
-    for got, want in zip(res["grads"], ref):
-        np.testing.assert_allclose(got.numpy(), want, rtol=1e-5, atol=1e-6 * np.abs(want).max())
+    assert res["n_allreduce"] == 1
+    if batch == 1:
+        assert res["units"] == [[(0, 0, 4)], [(0, 4, 7)]]
+    else:
+        assert res["units"] == [[(0, 0, 7), (1, 0, 7)], [(2, 0, 7)]]
+    scs = _scenes(batch)
+    for b, sc in enumerate(scs):
+        np.testing.assert_allclose(res["cube"][b].numpy(), po.render(sc), rtol=1e-6, atol=1e-30)
+        ref = po.render_bwd(sc, res["G"][b].numpy().astype(np.float64))
+        for got, want in zip(res["grads"], ref):
+            assert got.shape[0] == batch
+            np.testing.assert_allclose(got[b].numpy(), want, rtol=1e-5, atol=1e-6 * np.abs(want).max())
+
+
+def test_bench_multi_rank_logic_dry_run():
+    """bench.py --gpus 2 --dry-run under torch.distributed.run (gloo, no GPU): one JSON line from rank 0 only, the step time is
+    the MAX over ranks (rank r 'takes' (1 + r) ms per step) and `value` the whole-job aggregate of both ranks."""
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "4", "--warmup", "1", "--dry-run"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT, env={**os.environ, "OMP_NUM_THREADS": "1"})
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                       # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["steps"] == 4 and d["scaling"] == "weak" and d["dry_run"] is True
+    assert d["ms_per_step"] == pytest.approx(2.0)                # max over ranks of (1 + rank) ms
+    assert d["config"]["workload"].startswith("cfg5")
+    assert d["value"] == pytest.approx(2 * 274877906944 * 4 / (8.0e-3))
+    assert [p["config"]["workload"][:4] for p in d["per_config"]] == ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "cfg6"]
