@@ -13,7 +13,7 @@ from typing import Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libradt.so")
+LIB_PATH = os.environ.get("RADT_LIB") or os.path.join(_HERE, "libradt.so")      # (RADT_LIB: another build of the same ABI)
 
 PASS_FWD, PASS_BWD = 0, 1
 

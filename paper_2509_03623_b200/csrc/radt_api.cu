@@ -137,6 +137,9 @@ int validate(const radt_geom *geom, const radt_line *line, const radt_grid *grid
     }
     if (grid->dens_mode < 0 || grid->dens_mode > 1 || grid->vel_mode < 0 || grid->vel_mode > 1)
         return fail(RADT_E_UNSUPPORTED, "unknown dens_mode / vel_mode");
+    if ((grid->kind == RADT_GRID_AXISYM ? (long long)grid->n[0] * grid->n[1] : (long long)grid->n[0] * grid->n[1] * grid->n[2]) >
+        (1ll << 30))
+        return fail(RADT_E_INVALID, "grid too large: at most 2^30 cells per batch item");
     return RADT_OK;
 }
 
@@ -179,6 +182,21 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
         for (int a = 0; a < 3; ++a) {
             d.lo[a] = grid->lo[a]; d.hi[a] = grid->hi[a];
             d.inv_d[a] = (double)(grid->n[a] - 1) / (grid->hi[a] - grid->lo[a]);
+            d.pre_lo[a] = (float)d.lo[a]; d.pre_inv_d[a] = (float)d.inv_d[a];
+        }
+    }
+    d.pre_n0f = (float)d.n0; d.pre_n1f = (float)d.n1; d.pre_n2f = (float)d.n2;
+    if (grid->kind != RADT_GRID_CART3D) {
+        // u = log2(r / r_min) (nr - 1) / log2(r_max / r_min) = lg2(r^2) us_half - lg2(r_min) uscale
+        d.pre_us_half = (float)(0.5 * (double)(grid->n[0] - 1) / d.lg2_ratio);
+        d.pre_uoff = (float)(-std::log2(grid->lo[0]) * (double)(grid->n[0] - 1) / d.lg2_ratio);
+        d.pre_wscale = (float)d.wscale_d;
+        d.pre_woff = (float)(-d.zlo * d.wscale_d);
+        if (grid->kind == RADT_GRID_SPH3D) {
+            // margins: two percent in rho^2, two theta cells in z/rho (|d cos| <= |d theta|)
+            const double dth = 2.0 / (double)d.th_scale;
+            d.pre_r2lo = (float)(d.rmin2 * 0.98); d.pre_r2hi = (float)(d.rmax2 * 1.02);
+            d.pre_czlo = (float)(d.cos_thi - dth); d.pre_czhi = (float)(d.cos_tlo + dth);
         }
     }
 }
@@ -225,6 +243,7 @@ void make_dev_geom(const radt_geom &g, const radt_line *line, DevGeom &d)
     d.x0 = g.x0; d.y0 = g.y0; d.pix_x = g.fov_x / g.nx; d.pix_y = g.fov_y / g.ny;
     d.gm_au_d = std::fmax(g.gm_star, 0.0) / kAU;
     d.sunit = line ? (float)source_unit(g, line) : 1.0f;
+    d.wxf = (float)d.wx; d.wyf = (float)d.wy; d.wzf = (float)d.wz;
 }
 
 void make_dev_line(const radt_line *line, DevLine &d)
@@ -269,8 +288,9 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     size_t cells = (size_t)grid_cells(grid) * (size_t)batch;
     w.cells = off; off = align256(off + cells * sizeof(float4));
     if (grid->kind == RADT_GRID_AXISYM) {
-        w.occ_wpr = (grid->n[1] + 31) / 32;
-        w.occ_words = grid->n[0] * w.occ_wpr;
+        // bit (I, J), I = floor(u) + 1 in 0..nr, J = floor(w) + 1 in 0..nzeta (radt_setup.cu)
+        w.occ_wpr = (grid->n[1] + 1 + 31) / 32;
+        w.occ_words = (grid->n[0] + 1) * w.occ_wpr;
         w.occ_nbj = 1;
     } else if (grid->kind == RADT_GRID_SPH3D) {
         w.occ_wpr = 1; w.occ_words = 1; w.occ_nbj = 1;          // no occupancy bitmap for spherical grids yet

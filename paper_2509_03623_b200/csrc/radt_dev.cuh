@@ -28,6 +28,7 @@ struct DevGeom {
     double gm_au_d;                    // G M / au  [(cm/s)^2 au]  (KEPLER_FRAC)
     double v0;                         // velocity of channel 0 minus v_sys, cm/s (uniform channel lattice)
     float sunit;                       // S0 / intensity unit
+    float wxf, wyf, wzf;               // fp32 copy of the ray direction (prefilter of the window kernels)
 };
 
 struct DevGrid {
@@ -49,6 +50,12 @@ struct DevGrid {
     // spherical (kind 2): n0 = nr (log-spaced, shares rmin2/rmax2/uscale/... with the axisymmetric axis), n1 = ntheta, n2 = nphi
     double cos_tlo, cos_thi;           // cos of the theta range (decreasing in theta)
     float th_c0, th_scale, ph_scale;   // theta index = (th_c0 - asin(z/rho)) th_scale, th_c0 = pi/2 - theta_lo; phi index = phi ph_scale
+    // fp32 constants of the window kernels' prefilter (a superset test with one cell of margin, radt_march_win.cu)
+    float pre_us_half, pre_uoff;       // axisym / spherical: u = lg2(r^2) pre_us_half + pre_uoff
+    float pre_wscale, pre_woff;        // axisym: w = zeta pre_wscale + pre_woff
+    float pre_n0f, pre_n1f, pre_n2f;   // node counts as floats
+    float pre_r2lo, pre_r2hi, pre_czlo, pre_czhi;   // spherical: accepted ranges of rho^2 and z/rho, with margins
+    float pre_lo[3], pre_inv_d[3];     // cartesian
 };
 
 struct DevLine {
@@ -171,6 +178,15 @@ __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// fp64 1/sqrt(x) to ~1e-13: the SFU's fp64 seed (MUFU.RSQ64H: relative error 2^-22, no fp32 round trip) and one Newton step
+__device__ __forceinline__ double rsqrt_d(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y * fma(-0.5 * x, y * y, 1.5);
+}
+// (double)k for 0 <= k < 2^31 without the conversion pipe: 2^52 + k is exact in the low word of the mantissa
+__device__ __forceinline__ double int_to_double(int k) { return __hiloint2double(0x43300000, k) - 4503599627370496.0; }
 
 // Disk-frame position of the s = 0 point of pixel (ix, iy)  (O1-O2).
 __device__ __forceinline__ void pixel_origin(const DevGeom &G, int nx, int ny, int ix, int iy,

@@ -14,12 +14,14 @@
 struct StepState {
     bool inside;
     float vh, A, mvlA, K2, S;           // phase-B scalars: u' = (vcs - vh)*A + mvlA ; d = K2*g ; I += S*(1-e)*T
-    // adjoint extras (dead code in the forward instantiation)
-    float n, T, invT, ex, em1, W, invalpha, proj, vk, dsf, qy;
-    float f0, f1, f2;
-    long long cell;
+    // adjoint extras (dead code in the forward instantiation): the chain rule of phase C as coefficients of the four
+    // channel sums {sum w, sum w u', sum w u'^2, sum G (1-e) T}, formed in phase A so that nothing else of the step's
+    // thermodynamics has to stay in registers across phase B:
+    //   dL/d(stored density) = cd sum_w;  dL/dT = cT0 sum_w + cT2 sum_wuu + cT3 sum_GcT;  dL/d(stored velocity) = cv sum_wu
+    float cd, cT0, cT2, cT3, cv;
+    float f0, f1, f2;                   // in-cell fractions
+    int cell;                           // first corner of the cell (within the batch item)
     int dk;                             // spherical grids: offset of the next phi node (1, or 1 - nphi across the seam)
-    bool tclamp;
     // uniform channel lattice (window path): u'(c) = u0 + (c - cref) dvA; channels wlo..whi can lie inside the line
     float u0, dvA;
     int cref, wlo, whi;
@@ -42,13 +44,11 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     // the r = 0 rule are exact comparisons, and they agree with a plain fp64 evaluation of O4 only if the
     // position carries the same roundings (a ray through the star whose midpoint falls on it gave s = 1e-14 with
     // an FMA and s = 0, a skipped step, without: randomised parity scenes 5, 20, 21).
-    const double s = __dadd_rn(s0, __dmul_rn((double)k + 0.5, ds));
+    const double s = __dadd_rn(s0, __dmul_rn(__hiloint2double(0x43300000, k) - 4503599627370495.5, ds));   // (k + 1/2) ds, exact k + 1/2
     const double x = __dadd_rn(ox, __dmul_rn(s, G.wx)), y = __dadd_rn(oy, __dmul_rn(s, G.wy)), z = __dadd_rn(oz, __dmul_rn(s, G.wz));
     double r2 = x * x + y * y;
     float r2f = (float)r2;
-    // fp64 1/r by one Newton step on the SFU seed
-    double ir_d = (double)rsqrt_approx(r2f);
-    ir_d = ir_d * fma(-0.5 * r2, ir_d * ir_d, 1.5);
+    double ir_d = rsqrt_d(r2);          // fp64 1/r: SFU seed + one Newton step
     float dens, temp;
     double vel_d;
     if (KIND == 0) {
@@ -65,7 +65,7 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
         // change of slope.
         double wd = (az * ir_d - g.zlo) * g.wscale_d;
         int j = min(max(rn_int((float)wd - 0.5f), 0), g.n1 - 2);
-        float fw = (float)(wd - (__hiloint2double(0x43300000, j) - 4503599627370496.0));
+        float fw = (float)(wd - int_to_double(j));
         float uf = lg2_approx(r2f * g.inv_rmin2_f) * g.half_uscale;
         int i = min(max(rn_int(uf - 0.5f), 0), g.n0 - 2);
         double t = r2 * __ldg(P.ws.rnode + i).y;
@@ -89,15 +89,14 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
             double a1 = fma(fwd, (double)c11.z - (double)c10.z, (double)c10.z);
             vel_d = fma(fud, a1 - a0, a0);
         }
-        st.f0 = fu; st.f1 = fw; st.f2 = 0.f; st.cell = cell;
+        if (!FWD) { st.f0 = fu; st.f1 = fw; st.f2 = 0.f; st.cell = cell; }
     } else if (KIND == 2) {
         // spherical (r, theta, phi) grid.  In/out decision in fp64 on rho^2 and cos(theta);
         // radial index as on the axisymmetric grid (cell from an fp32 estimate, in-cell fraction from rho^2/r_i^2);
         // theta through asin(z/rho), which is well conditioned around the equator where disk grids live; phi
         // through atan2 in fp32 (1e-7 rad is 4e-6 of a cell at 256 nodes).
         double rho2 = r2 + z * z;
-        double irho = (double)rsqrt_approx((float)rho2);
-        irho = irho * fma(-0.5 * rho2, irho * irho, 1.5);
+        double irho = rsqrt_d(rho2);
         double cz = z * irho;
         bool in = (k < P.nstep) && (r2 > 0.0) && (rho2 >= g.rmin2) && (rho2 <= g.rmax2) && (cz <= g.cos_tlo) && (cz >= g.cos_thi);
         if (!in) return;
@@ -141,7 +140,7 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
             double b0 = fma(fyd, a01 - a00, a00), b1 = fma(fyd, a11 - a10, a10);
             vel_d = fma(fxd, b1 - b0, b0);
         }
-        st.f0 = fu; st.f1 = fw; st.f2 = fq; st.cell = cell; st.dk = dk;
+        if (!FWD) { st.f0 = fu; st.f1 = fw; st.f2 = fq; st.cell = (int)cell; st.dk = dk; }
     } else {
         bool in = (k < P.nstep) && (r2 > 0.0) && (x >= g.lo[0]) && (x <= g.hi[0]) && (y >= g.lo[1]) && (y <= g.hi[1]) &&
                   (z >= g.lo[2]) && (z <= g.hi[2]);
@@ -171,7 +170,7 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
             double b0 = fma(fyd, a01 - a00, a00), b1 = fma(fyd, a11 - a10, a10);
             vel_d = fma(fxd, b1 - b0, b0);
         }
-        st.f0 = fx; st.f1 = fy; st.f2 = fz; st.cell = cell; st.dk = 1;
+        if (!FWD) { st.f0 = fx; st.f1 = fy; st.f2 = fz; st.cell = (int)cell; st.dk = 1; }
     }
     // ---- O7: channel-independent LTE quantities (Eq. 13-17) ----
     float n = (g.dens_mode == 1) ? ex2_approx(dens * RADT_LOG2E) : dens;
@@ -207,12 +206,9 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     if (g.vel_mode == 1) {
         // Keplerian speed of Eq. 6 without the pressure term: v_K^2 = (GM/au) r^2 / rho^3, lengths in au
         double rho2 = r2 + z * z;
-        double yr = (double)rsqrt_approx((float)rho2);
-        yr = yr * fma(-0.5 * rho2, yr * yr, 1.5);
+        double yr = rsqrt_d(rho2);
         double vk2 = G.gm_au_d * r2 * yr * yr * yr;
-        double yv = (double)rsqrt_approx(fmaxf((float)vk2, 1e-30f));
-        yv = yv * fma(-0.5 * vk2, yv * yv, 1.5);
-        double vk_d = vk2 * yv;
+        double vk_d = vk2 * rsqrt_d(fmax(vk2, 1e-300));
         vk = (float)vk_d;
         vphi_d = vk_d * (1.0 + vel_d);
     }
@@ -247,9 +243,28 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     }
     st.K2 = K2;
     st.S = S;
-    st.n = n; st.T = T; st.invT = invT; st.ex = ex; st.em1 = em1; st.W = W; st.invalpha = invalpha;
-    st.proj = proj; st.vk = vk; st.dsf = dsf; st.tclamp = tcl;
-    st.qy = lerp1(q0.y, q1.y, fq) * iQ;      // dlnQ/dlnT
+    if (!FWD) {
+        // chain rule of O11 (SURVEY.md section 8(a) row i) as coefficients of the channel sums.  The lane sums are moments
+        // of w = a g in log2 units: sum a dtau u^m = K sum w u'^m / log2(e)^(m/2), K = K2 / log2(e).
+        const float iL2 = RADT_LN2;                       // 1 / log2(e)
+        const float ia = invalpha;
+        const float qy = lerp1(q0.y, q1.y, fq) * iQ;      // dlnQ/dlnT
+        const float cdn = (L.Ck2 * iL2) * W * em1 * dsf * ia;          // dK/dn (valid at n = 0)
+        st.cd = (g.dens_mode == 1) ? cdn * n : cdn;
+        const float K = K2 * iL2;
+        const float iT2 = invT * invT;
+        const float iem1 = rcp_approx(em1);
+        const float exs = em1 + 1.0f;                     // e^x, consistent with the series branch
+        const float dlnF_dT = L.Eu * iT2 - L.T0 * iT2 * exs * iem1 - qy * invT;
+        const float dS_dT = S * exs * iem1 * L.T0 * iT2;
+        const float dalpha_dT = 0.5f * L.a1 * ia;
+        // dL/dT = A0 K dlnF/dT + ia (2 A2 - A0 K) dalpha/dT + Bs dS/dT; zero through the 1 K clamp
+        st.cT0 = tcl ? 0.f : K * (dlnF_dT - ia * dalpha_dT);
+        st.cT2 = tcl ? 0.f : 2.0f * ia * dalpha_dT * K2 * (iL2 * iL2);
+        st.cT3 = tcl ? 0.f : dS_dT;
+        // dL/dv_phi = (2/alpha) A1 proj (v_K for KEPLER_FRAC), A1 = K2 sum_wu / (log2(e) sqrt(log2(e)))
+        st.cv = 2.0f * ia * K2 * (iL2 / RADT_SQRT_LOG2E) * proj * vk;
+    }
 }
 
 
@@ -400,33 +415,14 @@ template <int KIND>
 __device__ __forceinline__ void phase_c(const MarchParams &P, const StepState &st, const float4 sm, const bool isE,
                                         float4 *__restrict__ grad)
 {
-    const DevLine &L = P.line;
-    const float iL2 = RADT_LN2;                       // 1 / log2(e)
-    float ia = st.invalpha;
-    float A0 = sm.x;
-    float dL_dn = A0 * (L.Ck2 * iL2) * st.W * st.em1 * st.dsf * ia;
-    float dL_dd = (P.grid.dens_mode == 1) ? dL_dn * st.n : dL_dn;
+    const float dL_dd = sm.x * st.cd;
     float4 *gp = grad + st.cell;
     if (isE) {
-        // the lane sums are moments of w = a g: sum a dtau u^m = K sum w u^m
-        float A1 = st.K2 * sm.y * (iL2 / RADT_SQRT_LOG2E);
-        float A2 = st.K2 * sm.z * (iL2 * iL2);
-        float Bs = sm.w;
-        float K = st.K2 * iL2;
-        float dL_dvlos = 2.0f * ia * A1;
-        float dL_dalpha = ia * (2.0f * A2 - A0 * K);
-        float iT2 = st.invT * st.invT;
-        float iem1 = rcp_approx(st.em1);
-        float exs = (st.em1 + 1.0f);                       // e^x, consistent with the series branch
-        float dlnF_dT = L.Eu * iT2 - L.T0 * iT2 * exs * iem1 - st.qy * st.invT;
-        float dS_dT = st.S * exs * iem1 * L.T0 * iT2;
-        float dalpha_dT = 0.5f * L.a1 * ia;
-        float dL_dT = A0 * K * dlnF_dT + dL_dalpha * dalpha_dT + Bs * dS_dT;
-        if (st.tclamp) dL_dT = 0.f;
-        float dL_dv = dL_dvlos * st.proj * st.vk;
+        const float dL_dT = fmaf(sm.x, st.cT0, fmaf(sm.z, st.cT2, sm.w * st.cT3));
+        const float dL_dv = sm.y * st.cv;
         if (KIND == 0) {
             float fu = st.f0, fw = st.f1;
-            long long n1 = P.grid.n1;
+            int n1 = P.grid.n1;
             red_add_cell(gp, (1.f - fu) * (1.f - fw), dL_dd, dL_dT, dL_dv);
             red_add_cell(gp + 1, (1.f - fu) * fw, dL_dd, dL_dT, dL_dv);
             red_add_cell(gp + n1, fu * (1.f - fw), dL_dd, dL_dT, dL_dv);
@@ -443,7 +439,7 @@ __device__ __forceinline__ void phase_c(const MarchParams &P, const StepState &s
     } else {
         if (KIND == 0) {
             float fu = st.f0, fw = st.f1;
-            long long n1 = P.grid.n1;
+            int n1 = P.grid.n1;
             red_add_dens(gp, (1.f - fu) * (1.f - fw) * dL_dd);
             red_add_dens(gp + 1, (1.f - fu) * fw * dL_dd);
             red_add_dens(gp + n1, fu * (1.f - fw) * dL_dd);

@@ -15,8 +15,12 @@
 // Algorithm: DESIGN.md O4-O11; PAPER.md:262-294 (Eq. 11-17).
 #include "radt_march.cuh"
 
+#ifndef RADT_WIN_MINB_FWD
 #define RADT_WIN_MINB_FWD 4     // CTAs per SM the kernels are compiled for (measured: 4 vs 3 gives fwd -3 %, bwd +2 %)
+#endif
+#ifndef RADT_WIN_MINB_BWD
 #define RADT_WIN_MINB_BWD 3
+#endif
 #define WIN_PAIRS 16         // slot pairs per batch of 32 steps
 #define NO_GROUP 0x7fffffff
 
@@ -24,74 +28,51 @@ struct __align__(16) WinShared {          // per warp
     float4 a[WIN_PAIRS];                  // {u0_a, u0_b, dvA_a, dvA_b}
     float4 b[WIN_PAIRS];                  // {K2_a, K2_b, S_a, S_b}
     float4 c[WIN_PAIRS];                  // {c_ref_a, c_ref_b, bits of u_lo, bits of u_hi}: union window of the pair
-    int cand[64];                         // candidate step indices waiting for phase A
+    int cand[64];                         // candidate step indices waiting for phase A (circular queue)
     int2 win[32];                         // channel windows of the compacted steps
+    double ray[6];                        // ox, oy, oz, s0, ds of the ray (fp64: read once per batch by phase A)
 };
 
-// fp32 copy of the ray and of the grid mapping for the prefilter
-struct PreCtx {
-    float ox, oy, oz, wx, wy, wz, s0, ds;
-    float us_half, lrm;                   // u = lg2(r^2) us_half - lrm
-    float zlo, wscale;
-    float r2lo, r2hi, czlo, czhi;         // spherical: accepted ranges of rho^2 and z/rho, with margins
-    float lo[3], inv_d[3];
+// fp32 copy of the ray for the prefilter (the grid mapping and the ray direction come as fp32 kernel parameters)
+struct PreRay {
+    float ox, oy, oz, s0, ds;
 };
-
-template <int KIND>
-__device__ __forceinline__ void pre_setup(const MarchParams &P, const DevGeom &G, const RayCtx &rc, PreCtx &pc)
-{
-    pc.ox = (float)rc.ox; pc.oy = (float)rc.oy; pc.oz = (float)rc.oz;
-    pc.wx = (float)G.wx; pc.wy = (float)G.wy; pc.wz = (float)G.wz;
-    pc.s0 = (float)rc.s0; pc.ds = (float)rc.ds;
-    if (KIND == 0) {
-        pc.us_half = 0.5f * P.grid.uscale;
-        pc.lrm = -lg2_approx((float)P.grid.inv_rmin) * P.grid.uscale;
-        pc.zlo = (float)P.grid.zlo; pc.wscale = (float)P.grid.wscale_d;
-    } else if (KIND == 2) {
-        // margins: one percent in radius, two theta cells in z/rho (|d cos| <= |d theta|)
-        const float dth = 2.0f / P.grid.th_scale;
-        pc.r2lo = (float)P.grid.rmin2 * 0.98f; pc.r2hi = (float)P.grid.rmax2 * 1.02f;
-        pc.czlo = (float)P.grid.cos_thi - dth; pc.czhi = (float)P.grid.cos_tlo + dth;
-    } else {
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { pc.lo[a] = (float)P.grid.lo[a]; pc.inv_d[a] = (float)P.grid.inv_d[a]; }
-    }
-}
 
 // Can step k lie in a cell that matters?  A superset test in fp32: positions are good to ~1e-4 au, the test
-// accepts one cell of margin around the grid and the bitmap is dilated by one cell (radt_setup.cu).
+// accepts one cell of margin around the grid and the bitmap is dilated accordingly (radt_setup.cu).
 template <int KIND>
-__device__ __forceinline__ bool prefilter(const MarchParams &P, const PreCtx &pc, const unsigned *__restrict__ occ, int k)
+__device__ __forceinline__ bool prefilter(const MarchParams &P, const DevGeom &G, const PreRay &pr, const unsigned *__restrict__ occ,
+                                          int k)
 {
-    float s = fmaf((float)k + 0.5f, pc.ds, pc.s0);
-    float x = fmaf(s, pc.wx, pc.ox), y = fmaf(s, pc.wy, pc.oy), z = fmaf(s, pc.wz, pc.oz);
+    const DevGrid &g = P.grid;
+    const float s = fmaf((float)k + 0.5f, pr.ds, pr.s0);
+    const float x = fmaf(s, G.wxf, pr.ox), y = fmaf(s, G.wyf, pr.oy), z = fmaf(s, G.wzf, pr.oz);
     if (KIND == 0) {
-        float r2 = fmaf(x, x, y * y);
-        float ri = rsqrt_approx(fmaxf(r2, 1e-30f));
-        float zeta = (P.grid.mirror ? fabsf(z) : z) * ri;
-        float uf = fmaf(lg2_approx(fmaxf(r2, 1e-30f)), pc.us_half, -pc.lrm);
-        float wf = (zeta - pc.zlo) * pc.wscale;
-        bool in = uf > -1.0f && uf < (float)P.grid.n0 && wf > -1.0f && wf < (float)P.grid.n1;
+        const float r2 = fmaxf(fmaf(x, x, y * y), 1e-30f);
+        const float zr = z * rsqrt_approx(r2);
+        const float uf = fmaf(lg2_approx(r2), g.pre_us_half, g.pre_uoff);
+        const float wf = fmaf(g.mirror ? fabsf(zr) : zr, g.pre_wscale, g.pre_woff);
+        const bool in = uf > -1.0f && uf < g.pre_n0f && wf > -1.0f && wf < g.pre_n1f;
         if (!in) return false;
         if (!P.use_occ) return true;
-        int i = min(max(rn_int(uf - 0.5f), 0), P.grid.n0 - 2);
-        int j = min(max(rn_int(wf - 0.5f), 0), P.grid.n1 - 2);
-        unsigned w = __ldg(occ + i * P.occ_wpr + (j >> 5));
-        return (w >> (j & 31)) & 1u;
+        // bit (I, J) = (floor(u) + 1, floor(w) + 1): no clamps, the bitmap has the extra row and column
+        const int I = rn_int(uf + 0.5f), J = rn_int(wf + 0.5f);
+        const unsigned w = __ldg(occ + (I * P.occ_wpr + (J >> 5)));
+        return (w >> (J & 31)) & 1u;
     } else if (KIND == 2) {
-        float rho2 = fmaf(x, x, fmaf(y, y, z * z));
-        float cz = z * rsqrt_approx(fmaxf(rho2, 1e-30f));
-        return rho2 > pc.r2lo && rho2 < pc.r2hi && cz > pc.czlo && cz < pc.czhi;
+        const float rho2 = fmaxf(fmaf(x, x, fmaf(y, y, z * z)), 1e-30f);
+        const float cz = z * rsqrt_approx(rho2);
+        return rho2 > g.pre_r2lo && rho2 < g.pre_r2hi && cz > g.pre_czlo && cz < g.pre_czhi;
     } else {
-        float tx = (x - pc.lo[0]) * pc.inv_d[0], ty = (y - pc.lo[1]) * pc.inv_d[1], tz = (z - pc.lo[2]) * pc.inv_d[2];
-        bool in = tx > -1.0f && tx < (float)P.grid.n0 && ty > -1.0f && ty < (float)P.grid.n1 && tz > -1.0f &&
-                  tz < (float)P.grid.n2;
+        const float tx = (x - g.pre_lo[0]) * g.pre_inv_d[0], ty = (y - g.pre_lo[1]) * g.pre_inv_d[1],
+                    tz = (z - g.pre_lo[2]) * g.pre_inv_d[2];
+        const bool in = tx > -1.0f && tx < g.pre_n0f && ty > -1.0f && ty < g.pre_n1f && tz > -1.0f && tz < g.pre_n2f;
         if (!in) return false;
         if (!P.use_occ) return true;
-        int I = min(max(rn_int(tx - 0.5f), 0), P.grid.n0 - 2) >> 2;
-        int J = min(max(rn_int(ty - 0.5f), 0), P.grid.n1 - 2) >> 2;
-        int Lb = min(max(rn_int(tz - 0.5f), 0), P.grid.n2 - 2) >> 2;
-        unsigned w = __ldg(occ + (I * P.occ_nbj + J) * P.occ_wpr + (Lb >> 5));
+        const int I = min(max(rn_int(tx - 0.5f), 0), g.n0 - 2) >> 2;
+        const int J = min(max(rn_int(ty - 0.5f), 0), g.n1 - 2) >> 2;
+        const int Lb = min(max(rn_int(tz - 0.5f), 0), g.n2 - 2) >> 2;
+        const unsigned w = __ldg(occ + ((I * P.occ_nbj + J) * P.occ_wpr + (Lb >> 5)));
         return (w >> (Lb & 31)) & 1u;
     }
 }
@@ -215,33 +196,43 @@ __device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, con
     Ts = __fmul_rn(Ts, e1);
 }
 
-// Candidate steps of the ray, compacted over 32-step blocks: fills S.cand until it holds >= 32 or the ray ends.
+// Candidate steps of the ray, compacted over 32-step blocks into a circular queue of 64 entries (head `ch`, `ncand` waiting):
+// filled until it holds >= 32 or the ray ends.
 template <int KIND>
-__device__ __forceinline__ void gather_candidates(const MarchParams &P, const PreCtx &pc, const unsigned *occ, WinShared &S,
-                                                  const RayCtx &rc, int lane, int &ncand, int &kb)
+__device__ __forceinline__ void gather_candidates(const MarchParams &P, const DevGeom &G, const PreRay &pr, const unsigned *occ,
+                                                  WinShared &S, int k_lo, int k_hi, int lane, int ch, int &ncand, int &kb)
 {
     const unsigned lt = (1u << lane) - 1u;
-    while (ncand < 32 && kb < rc.k_hi) {
+    while (ncand < 32 && kb < k_hi) {
         const int k = kb + lane;
-        const bool cnd = k >= rc.k_lo && k < rc.k_hi && prefilter<KIND>(P, pc, occ, k);
+        const bool cnd = k >= k_lo && k < k_hi && prefilter<KIND>(P, G, pr, occ, k);
         const unsigned m = __ballot_sync(FULL, cnd);
-        if (cnd) S.cand[ncand + __popc(m & lt)] = k;
+        if (cnd) S.cand[(ch + ncand + __popc(m & lt)) & 63] = k;
         ncand += __popc(m);
         kb += 32;
     }
 }
 
-// Take up to 32 candidates (march order) out of S.cand; lanes beyond the count get k = nstep (outside).
-__device__ __forceinline__ int take_candidates(WinShared &S, int lane, int &ncand, int nstep)
+// Take up to 32 candidates (march order) from the head of the queue; lanes beyond the count get k = nstep (outside).
+__device__ __forceinline__ int take_candidates(WinShared &S, int lane, int &ch, int &ncand, int nstep)
 {
     __syncwarp();
     const int n = min(ncand, 32);
-    const int k = lane < n ? S.cand[lane] : nstep;
-    const int kx = lane + 32 < ncand ? S.cand[lane + 32] : 0;
-    __syncwarp();
-    if (lane + 32 < ncand) S.cand[lane] = kx;
+    const int k = lane < n ? S.cand[(ch + lane) & 63] : nstep;
+    __syncwarp();                   // the next fill may wrap around onto the slots just read
+    ch = (ch + n) & 63;
     ncand -= n;
     return k;
+}
+
+// The ray's fp64 origin and interval go to shared memory (phase A reads them once per batch); the prefilter keeps fp32 copies.
+__device__ __forceinline__ PreRay stash_ray(WinShared &S, const RayCtx &rc, int lane)
+{
+    if (lane == 0) { S.ray[0] = rc.ox; S.ray[1] = rc.oy; S.ray[2] = rc.oz; S.ray[3] = rc.s0; S.ray[4] = rc.ds; }
+    PreRay pr;
+    pr.ox = (float)rc.ox; pr.oy = (float)rc.oy; pr.oz = (float)rc.oz; pr.s0 = (float)rc.s0; pr.ds = (float)rc.ds;
+    __syncwarp();
+    return pr;
 }
 
 extern __shared__ __align__(16) unsigned char win_smem[];
@@ -271,16 +262,16 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
     if (rc.ds != 0.0) {
         const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
         const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
-        PreCtx pc;
-        pre_setup<KIND>(P, G, rc, pc);
-        int ncand = 0, kb = rc.k_lo & ~31;
+        const PreRay pr = stash_ray(S, rc, lane);
+        const int k_lo = rc.k_lo, k_hi = rc.k_hi;
+        int ncand = 0, ch = 0, kb = k_lo & ~31;
         while (true) {
-            gather_candidates<KIND>(P, pc, occ, S, rc, lane, ncand, kb);
+            gather_candidates<KIND>(P, G, pr, occ, S, k_lo, k_hi, lane, ch, ncand, kb);
             if (ncand == 0) break;
-            const int k = take_candidates(S, lane, ncand, P.nstep);
+            const int k = take_candidates(S, lane, ch, ncand, P.nstep);
 
             StepState st;
-            phase_a<KIND, true, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, k, st);
+            phase_a<KIND, true, true>(P, G, cells, S.ray[0], S.ray[1], S.ray[2], S.ray[3], S.ray[4], k, st);
             const bool act = st.inside && (st.K2 > K2_EMPTY || !P.opt_skip_empty) && st.whi >= 0 && st.wlo < nchan;
             n_steps += __popc(__ballot_sync(FULL, act));
             bool wide;
@@ -327,9 +318,9 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
 // ---------------------------------------------------------------------------------------------
 // K4 / K5 adjoint march: front-to-back re-march with the saved cube
 //   dL/d dtau_k,c = G_c (T_{k+1,c} S_k - R_k,c),  R_k = I - I_{<=k}        dL/dS_k = sum_c G_c (1-e_k,c) T_k,c
-// Entries with K2 = 0 are zero-opacity steps (LINEAR density grids): they leave the ray state untouched and
-// feed dL/dn only.  Per step every lane writes its partial sums {w, w u', w u'^2, G (1-e) T} (one float4; one float
-// in batches of zero-opacity steps) to shared memory; after BWD_SUB pairs the lanes sum them over the channels.
+// Emitting steps run as pairs with lanes over channels: every lane writes its partial sums {w, w u', w u'^2, G (1-e) T}
+// (one float4 per step) to shared memory and after BWD_SUB pairs the lanes sum them over the channels.  Zero-opacity steps
+// (LINEAR density grids) leave the ray state untouched, feed dL/dn only and run with lanes over steps (refresh_frozen).
 // ---------------------------------------------------------------------------------------------
 #define BWD_SUB 4            // pairs per reduction batch
 
@@ -367,17 +358,26 @@ struct BwdLane {
     __device__ __forceinline__ float neg_r() const { return COMP ? (Ps - Is) + (Qs - Ils) : Ps - Is; }
 };
 
-// Partial sums of a reduction batch, rows padded by one element so that both the per-lane writes and the per-step
-// reads are free of bank conflicts with plain immediate offsets:
-//   emitting batches   float4 [2 BWD_SUB steps][33]   {w, w u', w u'^2, G (1-e) T} per (step, lane)
-//   zero-opacity runs  float  [32 steps][33]          w per (step, lane)
-#define RED_ROW 33
-typedef float4 RedBuf[2 * BWD_SUB][RED_ROW];
+// Partial sums of a reduction batch of BWD_SUB pairs: 4 BWD_SUB rows (pair jj, component q of {w, w u', w u'^2, G (1-e) T}),
+// one float2 {step a, step b} per lane, i.e. exactly the packed f32x2 registers the pair evaluation ends with (one
+// 8-byte store per component, no repacking).  A row is two half-rows of 16 lanes with 16 bytes of padding after each
+// (RED_ROW_BYTES = 288, RED_HALF_BYTES = 144): the 16-byte reads of reduce_steps_e are then free of bank conflicts.
+#define RED_ROW_BYTES 288
+#define RED_HALF_BYTES 144
+#define RED_BYTES (4 * BWD_SUB * RED_ROW_BYTES)
 
-// A pair with at least one emitting step.  Repeats the forward's O9 sequence bit for bit (fwd_pair).
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sts_f2(unsigned addr, f2 v) { asm volatile("st.shared.b64 [%0], %1;" ::"r"(addr), "l"(v) : "memory"); }
+__device__ __forceinline__ void lds_2f2(unsigned addr, f2 &a, f2 &b)
+{
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr) : "memory");
+}
+
+// A pair of emitting steps (or one and a no-op entry).  Repeats the forward's O9 sequence bit for bit (fwd_pair).
+// `red_lane` = shared address of this lane's float2 in row 0 of the pair's four rows.
 template <bool COMP>
 __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, const float4 &qc, BwdLane<COMP> &L,
-                                           float nsmax, float4 (*red)[RED_ROW], int lane)
+                                           float nsmax, unsigned red_lane)
 {
     Pair s;
     pair_eval(pair_u_win(qa, qc, L.cf), pk(qb.x, qb.y), s);
@@ -391,82 +391,129 @@ __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, c
     const float P1 = __fmaf_rn(qb.w, c1, P0);
     const float T2 = __fmul_rn(T1, e1);
     const f2 Tn = pk(T1, T2), G2 = pk1(L.Gs);
-    f2 PmI = sub2(pk(P0, P1), pk1(L.Is));
+    f2 nR = sub2(pk(P0, P1), pk1(L.Is));               // -R = P - I_saved
     if (COMP) {
-        // the same error words the forward collected (fwd_pair), so that P + Q tracks the exact partial sum
+        // the same error words the forward collected (fwd_pair), so that P + Q tracks the exact partial sum; with
+        // them the difference is good to ~1e-14 I and needs no clamp
         const float Q0 = L.Qs + __fmaf_rn(qb.z, c0, __fsub_rn(L.Ps, P0));
         const float Q1 = Q0 + __fmaf_rn(qb.w, c1, __fsub_rn(P0, P1));
-        PmI = add2(PmI, sub2(pk(Q0, Q1), pk1(L.Ils)));
+        nR = add2(nR, sub2(pk(Q0, Q1), pk1(L.Ils)));
         L.Qs = Q1;
+    } else {
+        nR = clamp_nR(nR, Tn, pk1(nsmax));
     }
-    const f2 nR = clamp_nR(PmI, Tn, pk1(nsmax));
     const f2 a = mul2(G2, fma2(Tn, pk(qb.z, qb.w), nR));          // dL/d dtau
-    const f2 w = mul2(a, s.g), wu = mul2(w, s.u), wuu = mul2(wu, s.u), gc = mul2(G2, pk(c0, c1));
-    float w0, w1, x0, x1, y0, y1, z0, z1;
-    upk(w, w0, w1); upk(wu, x0, x1); upk(wuu, y0, y1); upk(gc, z0, z1);
-    red[0][lane] = make_float4(w0, x0, y0, z0);
-    red[1][lane] = make_float4(w1, x1, y1, z1);
+    const f2 w = mul2(a, s.g), wu = mul2(w, s.u);
+    sts_f2(red_lane, w);
+    sts_f2(red_lane + RED_ROW_BYTES, wu);
+    sts_f2(red_lane + 2 * RED_ROW_BYTES, mul2(wu, s.u));
+    sts_f2(red_lane + 3 * RED_ROW_BYTES, mul2(G2, pk(c0, c1)));
     L.Ts = T2; L.Ps = P1;
 }
 
-// Zero-opacity steps leave T and P untouched, so G T and G R are fixed while the lane keeps its channel; only
-// sum w = sum (G T S_k - G R) g is needed.  {GT, GnR} of the served channel:
+// Zero-opacity steps (LINEAR density grids) leave T and P untouched and feed only dL/dn = kappa sum_c (G T S_k - G R) g_c.
+// While no emitting step intervenes, G T and G R of every channel are frozen: they are written once to shared memory
+// ({G T, -G R} per channel) and a whole run of such steps is then evaluated with LANES OVER STEPS, each lane looping
+// over the channels of its own step's line window.  Its sum lands in the lane that runs phase C for that step: no
+// partials, no reduction over lanes (the earlier lanes-over-channels pairs cost 41 + 4 instructions per pair; this
+// loop costs ~8 per channel for 32 steps at once).
 template <bool COMP>
-__device__ __forceinline__ float2 z_frozen(const BwdLane<COMP> &L, float nsmax)
+__device__ __forceinline__ void refresh_frozen(BwdLane<COMP> &L, float2 *sF, float nsmax, int ng, int nchan, int lane)
 {
-    return make_float2(L.Gs * L.Ts, L.Gs * fminf(fmaxf(L.neg_r(), L.Ts * nsmax), 0.f));
+    L.put_back();                                  // (channel c is only ever touched by lane c & 31)
+    for (int g = 0; g < ng; ++g) {
+        const int c = lane + 32 * g;
+        if (c < nchan) {
+            const float T = L.sT[c], Gc = __ldg(L.Gin + c);
+            float nr = L.sP[c] - __ldg(L.Isave + c);
+            if (COMP) nr += L.sQ[c] - __ldg(L.Ilo + c);
+            else nr = fminf(fmaxf(nr, T * nsmax), 0.f);       // same clamp as clamp_nR
+            sF[c] = make_float2(Gc * T, Gc * nr);
+        }
+    }
+    __syncwarp();
 }
-__device__ __forceinline__ f2 z_pair_w(const float4 &qa, float Sa, float Sb, const float4 &qc, float cf, float2 fr)
+// sum_c (G T S + (-G R)) g_c over every `stride`-th channel from c0 + q of the window [c0, c1]; u'(c) as in pair_u_win
+__device__ __forceinline__ float z_slice_sum(float u0, float dvA, float Ss, int cref, int c0, int c1, int q, int stride,
+                                             const float2 *__restrict__ sF)
 {
-    const f2 u = pair_u_win(qa, qc, cf);
-    float t0, t1;
-    upk(mul2(u, u), t0, t1);
-    const f2 g = pk(ex2_approx(-t0), ex2_approx(-t1));
-    return mul2(fma2(pk1(fr.x), pk(Sa, Sb), pk1(fr.y)), g);
+    float cf = (float)(c0 + q - cref), acc = 0.f;
+    const float df = (float)stride;
+    for (int c = c0 + q; c <= c1; c += stride) {
+        const float u = fmaf(cf, dvA, u0);
+        const float g = ex2_approx(-u * u);
+        const float2 f = sF[c];
+        acc = fmaf(fmaf(f.x, Ss, f.y), g, acc);
+        cf += df;
+    }
+    return acc;
+}
+// A run of m zero-opacity steps (lanes `inrun`, r-th step of the run in lane order): 32 >> ceil(log2 m) lanes share one
+// step, each taking a slice of its window; the step's sum returns to the lane that holds the step.
+__device__ __forceinline__ float z_run(WinShared &S, const StepState &st, bool inrun, int r, int m, const float2 *__restrict__ sF,
+                                       int nchan, int lane, unsigned &n_mufu)
+{
+    const int c0 = max(st.wlo, 0), c1 = min(st.whi, nchan - 1);
+    if (m > 16) {                                    // one lane per step
+        const float v = inrun ? z_slice_sum(st.u0, st.dvA, st.S, st.cref, c0, c1, 0, 1, sF) : 0.f;
+        n_mufu += __reduce_max_sync(FULL, inrun ? c1 - c0 + 1 : 0);
+        return v;
+    }
+    const int sh = 5 - (32 - __clz(m - 1));          // log2 of the lanes per step: m = 1 -> 5, 2 -> 4, 3..4 -> 3, ... 9..16 -> 1
+    if (inrun) {
+        S.a[r] = make_float4(st.u0, st.dvA, st.S, (float)st.cref);       // (|c_ref| <= 1e6: exact)
+        S.win[r] = make_int2(c0, c1);
+    }
+    __syncwarp();
+    const int myr = lane >> sh, q = lane & ((1 << sh) - 1);
+    float acc = 0.f;
+    int trips = 0;
+    if (myr < m) {
+        const float4 e = S.a[myr];
+        const int2 w = S.win[myr];
+        acc = z_slice_sum(e.x, e.y, e.z, (int)e.w, w.x, w.y, q, 1 << sh, sF);
+        trips = (w.y - w.x - q + (1 << sh)) >> sh;
+    }
+    n_mufu += __reduce_max_sync(FULL, max(trips, 0));
+    for (int o = (1 << sh) >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(FULL, acc, o);
+    const float v = __shfl_sync(FULL, acc, (r << sh) & 31);
+    __syncwarp();
+    return v;
 }
 
-// Sum the partials of nb <= BWD_SUB pairs (2 nb steps) over the 32 lanes.  Lane (s = lane & 7, h = lane >> 3) adds
-// the source lanes 8h .. 8h+7 of step s, two shuffle rounds combine the four quarters, and lane s < 2 nb stores the
-// four sums of step s.
-__device__ __forceinline__ void reduce_steps_e(const RedBuf &red, int nb, float4 *out, int lane)
+// Sum the partials of nb <= BWD_SUB pairs over the 32 lanes.  Lane l adds the 16 source lanes of half (l & 1) of row
+// l >> 1 (eight 16-byte reads, packed adds), one shuffle round joins the halves, and the even lane of a row stores the two
+// sums {step a, step b} of (pair jj = row >> 2, component q = row & 3) into sum[2 (base_i + jj) + {0, 1}].q.
+__device__ __forceinline__ void reduce_steps_e(unsigned red, int nb, float *sum_base, int lane)
 {
-    // rows as pairs of packed f32x2: one FADD2 per two sums
-    const ulonglong2 *row = reinterpret_cast<const ulonglong2 *>(&red[lane & 7][lane & 24]);
-    ulonglong2 a = row[0];
+    const unsigned src = red + (lane >> 1) * RED_ROW_BYTES + (lane & 1) * RED_HALF_BYTES;
+    f2 a, b;
+    lds_2f2(src, a, b);
 #pragma unroll
     for (int i = 1; i < 8; ++i) {
-        const ulonglong2 v = row[i];
-        a.x = add2(a.x, v.x); a.y = add2(a.y, v.y);
+        f2 c, d;
+        lds_2f2(src + 16 * i, c, d);
+        a = add2(a, c); b = add2(b, d);
     }
-    float4 acc;
-    upk(a.x, acc.x, acc.y); upk(a.y, acc.z, acc.w);
-#pragma unroll
-    for (int m = 8; m <= 16; m <<= 1) {
-        acc.x += __shfl_xor_sync(FULL, acc.x, m);
-        acc.y += __shfl_xor_sync(FULL, acc.y, m);
-        acc.z += __shfl_xor_sync(FULL, acc.z, m);
-        acc.w += __shfl_xor_sync(FULL, acc.w, m);
-    }
-    if (lane < 2 * nb) out[lane] = acc;
-}
-// A run of nz <= 16 zero-opacity pairs: lane s < 2 nz sums the 32 partials of step s.
-__device__ __forceinline__ void reduce_steps_z(const float (*redz)[RED_ROW], int nz, float4 *out, int lane)
-{
-    if (lane < 2 * nz) {
-        const float *row = redz[lane];
-        float a0 = row[0], a1 = row[1], a2 = row[2], a3 = row[3];
-#pragma unroll
-        for (int i = 4; i < 32; i += 4) { a0 += row[i]; a1 += row[i + 1]; a2 += row[i + 2]; a3 += row[i + 3]; }
-        out[lane] = make_float4((a0 + a1) + (a2 + a3), 0.f, 0.f, 0.f);
+    a = add2(a, b);
+    float x, y;
+    upk(a, x, y);
+    x += __shfl_xor_sync(FULL, x, 1);
+    y += __shfl_xor_sync(FULL, y, 1);
+    const int jj = lane >> 3, q = (lane >> 1) & 3;
+    if (!(lane & 1) && jj < nb) {
+        sum_base[8 * jj + q] = x;
+        sum_base[8 * jj + 4 + q] = y;
     }
 }
 
-struct __align__(16) BwdShared {          // per warp, followed by (T, P) of 32 ngroups channels
+struct __align__(16) BwdShared {          // per warp, followed by (T, P[, Q]) and the frozen {G T, -G R} of 32 ngroups channels
     WinShared w;
-    RedBuf red;                           // 8 x 33 float4 = 32 x 33 float
+    unsigned char red[RED_BYTES];         // partial sums of a reduction batch (layout above)
     float4 sum[32];                       // channel sums of the compacted steps
 };
-static size_t bwd_warp_bytes(int ng, bool comp) { return sizeof(BwdShared) + (size_t)ng * (comp ? 384 : 256); }
+#define BWD_CHAN_BYTES(comp) ((comp) ? 640 : 512)      // per 32 channels: T, P (, Q) floats and {G T, -G R} float2
+static size_t bwd_warp_bytes(int ng, bool comp) { return sizeof(BwdShared) + (size_t)ng * BWD_CHAN_BYTES(comp); }
 
 template <int KIND, bool COMP>
 __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_march_bwd_w(const __grid_constant__ MarchParams P)
@@ -476,7 +523,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
     if (!ray_setup(P, rc, warp)) return;
     if (rc.ds == 0.0) return;
     const int ng = P.line.ngroups;
-    unsigned char *base = win_smem + (size_t)warp * (sizeof(BwdShared) + (size_t)ng * (COMP ? 384 : 256));
+    unsigned char *base = win_smem + (size_t)warp * (sizeof(BwdShared) + (size_t)ng * BWD_CHAN_BYTES(COMP));
     BwdShared &B = *reinterpret_cast<BwdShared *>(base);
     WinShared &S = B.w;
     const DevGeom &G = P.geom[rc.b];
@@ -484,6 +531,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
     const int nchan = Ln.nchan;
     BwdLane<COMP> L;
     L.sT = reinterpret_cast<float *>(base + sizeof(BwdShared)); L.sP = L.sT + 32 * ng; L.sQ = L.sP + 32 * ng;
+    float2 *sF = reinterpret_cast<float2 *>(L.sP + (COMP ? 64 : 32) * ng);
     L.Ilo = P.cube_lo + rc.ray * (size_t)nchan;
     L.Isave = P.cube + rc.ray * (size_t)nchan;
     L.Gin = P.dl_dcube + rc.ray * (size_t)nchan;
@@ -503,93 +551,86 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
     const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + 4)), 1.0f);
     const float nsmax = -G.sunit * 1.0001f / (ex2_approx(Ln.T0l2 / tmax) - 1.0f);
     const float kthr = P.opt_skip_empty ? K2_EMPTY : 0.f;    // the forward's own test for an emitting step
-    PreCtx pc;
-    pre_setup<KIND>(P, G, rc, pc);
+    const bool zsteps = P.grid.dens_mode == 0 && P.opt_zero_grad;      // zero-opacity steps carry dL/dn (LINEAR grids)
+    const PreRay pr = stash_ray(S, rc, lane);
+    const int k_lo = rc.k_lo, k_hi = rc.k_hi;
+    const unsigned lt = (1u << lane) - 1u;
+    const unsigned red0 = smem_u32(B.red), red_lane = red0 + (lane >> 4) * RED_HALF_BYTES + (lane & 15) * 8;
     unsigned n_steps = 0, n_mufu = 0;
-    int ncand = 0, kb = rc.k_lo & ~31;
+    bool zdirty = true;                      // the frozen {G T, -G R} in shared memory are stale
+    int ncand = 0, ch = 0, kb = k_lo & ~31;
     while (true) {
-        gather_candidates<KIND>(P, pc, occ, S, rc, lane, ncand, kb);
+        gather_candidates<KIND>(P, G, pr, occ, S, k_lo, k_hi, lane, ch, ncand, kb);
         if (ncand == 0) break;
-        const int k = take_candidates(S, lane, ncand, P.nstep);
+        const int k = take_candidates(S, lane, ch, ncand, P.nstep);
 
         StepState st;
-        phase_a<KIND, false, true>(P, G, cells, rc.ox, rc.oy, rc.oz, rc.s0, rc.ds, k, st);
-        const bool isE = st.inside && st.K2 > kthr;
-        // zero-opacity steps still carry dL/dn when the grid stores n itself (LINEAR)
-        const bool act = st.inside && (isE || (P.grid.dens_mode == 0 && P.opt_zero_grad)) && st.whi >= 0 && st.wlo < nchan;
-        const float K2e = isE ? st.K2 : 0.f;
-        n_steps += __popc(__ballot_sync(FULL, act));
-        bool wide;
-        int pos;
-        int npairs = write_entries(S, lane, act, -1, st, K2e, wide, pos);
-        const int npass = wide ? ng : 1;
+        phase_a<KIND, false, true>(P, G, cells, S.ray[0], S.ray[1], S.ray[2], S.ray[3], S.ray[4], k, st);
+        const bool inwin = st.inside && st.whi >= 0 && st.wlo < nchan;
+        const bool isE = inwin && st.K2 > kthr;
+        const bool isZ = inwin && !isE && zsteps;
+        const unsigned emask = __ballot_sync(FULL, isE), zmask = __ballot_sync(FULL, isZ);
+        n_steps += __popc(emask | zmask);
         float4 sm = make_float4(0.f, 0.f, 0.f, 0.f);
+        // Runs of emitting steps and runs of zero-opacity steps, in march order (lane order): a zero-opacity step sees the
+        // ray state left by every emitting step before it.
+        unsigned rem = emask | zmask;
 #pragma unroll 1
-        for (int p = 0; p < npass; ++p) {
-            bool a = act;
-            if (wide) {
-                bool w2;
-                a = act && st.wlo <= 32 * p + 31 && st.whi >= 32 * p;
-                npairs = write_entries(S, lane, a, 32 * p, st, K2e, w2, pos);
+        while (rem) {
+            const int first = __ffs(rem) - 1;
+            const bool kindE = (emask >> first) & 1u;
+            const unsigned other = (kindE ? zmask : emask) & ~((1u << first) - 1u);
+            const unsigned run = other ? rem & ((1u << (__ffs(other) - 1)) - 1u) : rem;
+            rem &= ~run;
+            const bool inrun = (run >> lane) & 1u;
+            if (!kindE) {
+                if (zdirty) {
+                    refresh_frozen<COMP>(L, sF, nsmax, ng, nchan, lane);
+                    zdirty = false;
+                }
+                const float v = z_run(S, st, inrun, __popc(run & lt), __popc(run), sF, nchan, lane, n_mufu);
+                if (inrun) sm.x = v;
+                continue;
             }
-            if (npairs == 0) continue;
-            // pairs that hold an emitting step
-            const unsigned emask = __ballot_sync(FULL, lane < npairs && (S.b[lane].x > 0.f || S.b[lane].y > 0.f));
-            int base_i = 0;
+            zdirty = true;
+            bool wide;
+            int pos;
+            int npairs = write_entries(S, lane, inrun, -1, st, st.K2, wide, pos);
+            const int npass = wide ? ng : 1;
 #pragma unroll 1
-            while (base_i < npairs) {
-                const unsigned erest = emask >> base_i;
-                if (!(erest & 1u)) {
-                    // a run of zero-opacity pairs (up to the whole batch): the ray state is frozen
-                    const int nz = min(erest ? __ffs(erest) - 1 : 32, npairs - base_i);
-                    float (*redz)[RED_ROW] = reinterpret_cast<float (*)[RED_ROW]>(&B.red[0][0]);
-                    float2 fr = z_frozen(L, nsmax);
+            for (int p = 0; p < npass; ++p) {
+                bool a = inrun;
+                if (wide) {
+                    bool w2;
+                    a = inrun && st.wlo <= 32 * p + 31 && st.whi >= 32 * p;
+                    npairs = write_entries(S, lane, a, 32 * p, st, st.K2, w2, pos);
+                }
+                if (npairs == 0) continue;
 #pragma unroll 1
-                    for (int jj = 0; jj < nz; ++jj) {
+                for (int base_i = 0; base_i < npairs; base_i += BWD_SUB) {
+                    const int nb = min(BWD_SUB, npairs - base_i);
+#pragma unroll 1
+                    for (int jj = 0; jj < nb; ++jj) {
                         const int i = base_i + jj;
-                        const float4 qa = S.a[i], qc = S.c[i];
-                        const float2 Sab = *reinterpret_cast<const float2 *>(&S.b[i].z);
+                        const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
                         const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
-                        if (group_misses(L.cur, ulo, uhi)) {
-                            L.regroup(group_for(ulo, uhi), lane, nchan);
-                            fr = z_frozen(L, nsmax);
-                        }
-                        float w0, w1;
-                        upk(z_pair_w(qa, Sab.x, Sab.y, qc, L.cf, fr), w0, w1);
-                        redz[2 * jj][lane] = w0;
-                        redz[2 * jj + 1][lane] = w1;
+                        if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
+                        bwd_pair_e<COMP>(qa, qb, qc, L, nsmax, red_lane + jj * (4 * RED_ROW_BYTES));
                     }
-                    n_mufu += 2 * nz;
+                    n_mufu += 4 * nb;
                     __syncwarp();
-                    reduce_steps_z(redz, nz, &B.sum[2 * base_i], lane);
+                    reduce_steps_e(red0, nb, reinterpret_cast<float *>(&B.sum[2 * base_i]), lane);
                     __syncwarp();
-                    base_i += nz;
-                    continue;
                 }
-                // up to BWD_SUB consecutive pairs that hold an emitting step
-                const int nb = min(min(BWD_SUB, __ffs(~erest) - 1), npairs - base_i);
-#pragma unroll 1
-                for (int jj = 0; jj < nb; ++jj) {
-                    const int i = base_i + jj;
-                    const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
-                    const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
-                    if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
-                    bwd_pair_e<COMP>(qa, qb, qc, L, nsmax, &B.red[2 * jj], lane);
+                if (a) {
+                    const float4 v = B.sum[pos];
+                    sm.x += v.x; sm.y += v.y; sm.z += v.z; sm.w += v.w;
                 }
-                n_mufu += 4 * nb;
                 __syncwarp();
-                reduce_steps_e(B.red, nb, &B.sum[2 * base_i], lane);
-                __syncwarp();
-                base_i += nb;
             }
-            if (a) {
-                const float4 v = B.sum[pos];
-                sm.x += v.x; sm.y += v.y; sm.z += v.z; sm.w += v.w;
-            }
-            __syncwarp();
         }
         // ---- phase C: chain rule to (n, T, v_phi) at this lane's step, scatter to the grid (O11) ----
-        if (act) phase_c<KIND>(P, st, sm, isE, grad);
+        if (isE || isZ) phase_c<KIND>(P, st, sm, isE, grad);
     }
     if (lane == 0 && n_steps) {
         atomicAdd(P.ws.counters + 2, (unsigned long long)n_steps);

@@ -165,23 +165,25 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
         return;
     }
     if (blk < nb_occ) {
-        // Occupancy bitmap of the (r, zeta) grid for the march prefilter: bit j of word (i, j / 32) is set when
-        // some node of the 4 x 4 block around cell (i, j) -- the corners of the cell and of its eight
-        // neighbours -- stores a density that can emit (or is NaN).  occ_thr = -inf gives all ones.
-        // One warp per word, lanes over the 35 nodes jw*32 - 1 .. jw*32 + 33 of each of the four radial rows.
+        // Occupancy bitmap of the (r, zeta) grid for the march prefilter.  The prefilter locates a step in fp32 as
+        // I = floor(u') + 1, J = floor(w') + 1 (u', w' within a small fraction of a cell of the exact index coordinates,
+        // so the exact cell (i, j) has I in {i, i+1, i+2}, J likewise).  Bit J of word (I, J / 32) is therefore set when
+        // some node of rows I-2 .. I+1 and columns J-2 .. J+1 -- which always include the four corners of the exact
+        // cell -- stores a density that can emit (or is NaN).  occ_thr = -inf gives all ones.
+        // One warp per word, lanes over the 35 node columns jw*32 - 2 .. jw*32 + 32 of each of the four rows.
         long long t = (long long)blk * blockDim.x + threadIdx.x;
         long long wq = t >> 5;
         if (wq >= (long long)P.occ_words * P.nbatch) return;
         const int ln = threadIdx.x & 31;
         int b = (int)(wq / P.occ_words);
         int w = (int)(wq - (long long)b * P.occ_words);
-        int i = w / P.occ_wpr, jw = w - i * P.occ_wpr;
+        int I = w / P.occ_wpr, jw = w - I * P.occ_wpr;
         const float *dn = P.dens + (long long)(P.b0 + b) * P.batch_stride;
-        bool f0 = false, f1 = false;                      // node tt = ln, node tt = ln + 32 (ln < 3)
-        for (int di = -1; di <= 2; ++di) {
-            int ii = i + di;
+        bool f0 = false, f1 = false;                      // column tt = ln, column tt = ln + 32 (ln < 3)
+        for (int di = -2; di <= 1; ++di) {
+            int ii = I + di;
             if (ii < 0 || ii >= P.grid.n0) continue;
-            int j0 = jw * 32 - 1 + ln, j1 = j0 + 32;
+            int j0 = jw * 32 - 2 + ln, j1 = j0 + 32;
             if (j0 >= 0 && j0 < P.grid.n1) f0 |= !(__ldg(dn + (long long)ii * P.grid.n1 + j0) <= P.occ_thr);
             if (ln < 3 && j1 < P.grid.n1) f1 |= !(__ldg(dn + (long long)ii * P.grid.n1 + j1) <= P.occ_thr);
         }
