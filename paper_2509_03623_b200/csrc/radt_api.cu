@@ -193,10 +193,10 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
         d.pre_wscale = (float)d.wscale_d;
         d.pre_woff = (float)(-d.zlo * d.wscale_d);
         if (grid->kind == RADT_GRID_SPH3D) {
-            // margins: two percent in rho^2, two theta cells in z/rho (|d cos| <= |d theta|)
+            // margins: one radial cell (as on the axisymmetric grid), two theta cells in z/rho (|d cos| <= |d theta|)
             const double dth = 2.0 / (double)d.th_scale;
-            d.pre_r2lo = (float)(d.rmin2 * 0.98); d.pre_r2hi = (float)(d.rmax2 * 1.02);
             d.pre_czlo = (float)(d.cos_thi - dth); d.pre_czhi = (float)(d.cos_tlo + dth);
+            d.pre_cscale = (float)((double)grid->n[1] / ((double)d.pre_czhi - (double)d.pre_czlo) * (1.0 - 1e-6));
         }
     }
 }
@@ -271,8 +271,9 @@ void make_dev_line(const radt_line *line, DevLine &d)
 }
 
 struct WsLayout {
-    size_t rays, qtab, vcs, rnode, cells, occ, grad, counters, total;
-    int occ_wpr, occ_words, occ_nbj;
+    size_t rays, qtab, vcs, rnode, cells, occ, grad, counters, nodeflag, total;
+    size_t zero_bytes;                  // counters + spherical node flags: one memset per pass
+    int occ_wpr, occ_words, occ_nbj, flag_wpr;
 };
 
 WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int pass)
@@ -280,7 +281,13 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
     WsLayout w;
     size_t off = 0;
     size_t nrays = (size_t)geom[0].nx * geom[0].ny * (size_t)batch;
-    w.counters = off; off = align256(off + (8 + RADT_LOSS_SLOTS) * sizeof(unsigned long long));
+    w.counters = off; off = off + (8 + RADT_LOSS_SLOTS) * sizeof(unsigned long long);
+    // spherical grids: (i, j) node flags of the occupancy prefilter, zeroed together with the counters
+    w.nodeflag = off;
+    w.flag_wpr = grid->kind == RADT_GRID_SPH3D ? (grid->n[1] + 31) / 32 : 0;
+    off = off + (size_t)w.flag_wpr * (size_t)grid->n[0] * (size_t)batch * sizeof(unsigned);
+    w.zero_bytes = off - w.counters;
+    off = align256(off);
     w.rays = off; off = align256(off + nrays * sizeof(RayRec));
     w.qtab = off; off = align256(off + (RADT_NQ + 2) * sizeof(float2));
     w.vcs = off; off = align256(off + (size_t)batch * RADT_MAXCHAN * sizeof(float2));
@@ -293,7 +300,10 @@ WsLayout ws_layout(const radt_geom *geom, const radt_grid *grid, int batch, int 
         w.occ_words = (grid->n[0] + 1) * w.occ_wpr;
         w.occ_nbj = 1;
     } else if (grid->kind == RADT_GRID_SPH3D) {
-        w.occ_wpr = 1; w.occ_words = 1; w.occ_nbj = 1;          // no occupancy bitmap for spherical grids yet
+        // bit (I, C): I = floor(u) + 1 in 0..nr, C = bin of cos(theta) in 0..ntheta-1, any phi (radt_setup.cu k_occ_sph)
+        w.occ_wpr = (grid->n[1] + 31) / 32;
+        w.occ_words = (grid->n[0] + 1) * w.occ_wpr;
+        w.occ_nbj = 1;
     } else {
         // 3-D: one bit per block of 4 x 4 x 4 cells
         int nbi = (grid->n[0] - 1 + 3) / 4, nbj = (grid->n[1] - 1 + 3) / 4, nbl = (grid->n[2] - 1 + 3) / 4;
@@ -319,6 +329,7 @@ DevWs make_dev_ws(void *ws, const WsLayout &w)
     d.rnode = (double2 *)(base + w.rnode);
     d.cells = (float4 *)(base + w.cells);
     d.occ = (unsigned *)(base + w.occ);
+    d.nodeflag = (unsigned *)(base + w.nodeflag);
     d.grad = (float4 *)(base + w.grad);
     return d;
 }
@@ -418,7 +429,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
     }
 
     // counters: 0-3 work counters, 4 the grid's maximum temperature (setup), 8.. loss slots (forward)
-    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, (reuse ? 4 : 8 + RADT_LOSS_SLOTS) * sizeof(unsigned long long), st));
+    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, reuse ? 4 * sizeof(unsigned long long) : w.zero_bytes, st));
     if (reuse) CUDA_TRY(cudaMemsetAsync(dws.grad, 0, (size_t)grid_cells(grid) * (size_t)batch * sizeof(float4), st));
     for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
         int nb = batch - b0 < RADT_MAXB ? batch - b0 : RADT_MAXB;
@@ -437,14 +448,18 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         // reuse_setup may want them); with LINEAR densities the exact adjoint needs every in-grid step (dL/dn of
         // empty cells) and marches without them.
         const bool win = use_win;
-        const bool occ_fwd = win && opt.skip_empty && grid->kind != RADT_GRID_SPH3D;   // (spherical: range test only)
+        const bool occ_fwd = win && opt.skip_empty;
         const bool occ = occ_fwd && (pass == RADT_PASS_FWD || grid->dens_mode == RADT_DENS_LN || !opt.zero_dens_grad);
-        SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr; SP.occ_nbj = w.occ_nbj;
+        SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr; SP.occ_nbj = w.occ_nbj; SP.flag_wpr = w.flag_wpr;
         SP.occ_thr = grid->dens_mode == RADT_DENS_LN ? -39.1439f : 1e-17f;     // N_EMPTY of the march kernels
         SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;
         if (!reuse) {
             CUDA_TRY(radt_launch_setup(SP, LT, CT, st));
             ++g_launches;
+            if (occ && grid->kind == RADT_GRID_SPH3D) {      // the (r, theta) occupancy words need every node flag: own launch
+                CUDA_TRY(radt_launch_occ_sph(SP, st));
+                ++g_launches;
+            }
         }
 
         memset(&MP, 0, sizeof(MP));

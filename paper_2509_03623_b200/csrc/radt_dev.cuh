@@ -54,7 +54,8 @@ struct DevGrid {
     float pre_us_half, pre_uoff;       // axisym / spherical: u = lg2(r^2) pre_us_half + pre_uoff
     float pre_wscale, pre_woff;        // axisym: w = zeta pre_wscale + pre_woff
     float pre_n0f, pre_n1f, pre_n2f;   // node counts as floats
-    float pre_r2lo, pre_r2hi, pre_czlo, pre_czhi;   // spherical: accepted ranges of rho^2 and z/rho, with margins
+    float pre_czlo, pre_czhi;          // spherical: accepted range of z/rho = cos(theta), two theta cells of margin
+    float pre_cscale;                  // spherical: occupancy bin of cos(theta) = (z/rho - pre_czlo) pre_cscale, n1 bins
     float pre_lo[3], pre_inv_d[3];     // cartesian
 };
 
@@ -91,7 +92,9 @@ struct DevWs {
     float4 *cells;         // [batch][cells] packed {dens, temp, vel, 0}
     float4 *grad;          // [batch][cells] packed gradient accumulators {dens, temp, vel, -} (bwd only)
     unsigned *occ;         // [batch][occ_words] axisym: bit (i, j): some cell within one cell of (i, j) can emit;
-                           // 3-D: one bit per block of 4 x 4 x 4 cells, same dilation (radt_setup.cu)
+                           // 3-D: one bit per block of 4 x 4 x 4 cells, same dilation; spherical: bit (radial cell,
+                           // bin of cos theta), any phi (radt_setup.cu)
+    unsigned *nodeflag;    // spherical: [batch][nr][ceil(ntheta / 32)] bit j of row i: some phi node of (i, j) can emit
     unsigned long long *counters;   // [8 + RADT_LOSS_SLOTS] 0-3 work counters; [4] bits of the grid's maximum
                                     // temperature; [8..] partial sums of the fused loss (double)
 };
@@ -128,6 +131,7 @@ struct SetupParams {
     int nlev, nchan;
     int do_rays, do_tables, do_pack, do_zero_grad, do_occ;
     int occ_words, occ_wpr, occ_nbj;
+    int flag_wpr;          // spherical: words per radial row of nodeflag
     float occ_thr;         // stored density value above which a node can emit
     long long batch_stride;
     const float *dens, *temp, *vel;

@@ -3,6 +3,7 @@
 #include "radt_dev.cuh"
 
 cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const ChanTable &V, cudaStream_t st);
+cudaError_t radt_launch_occ_sph(const SetupParams &P, cudaStream_t st);
 cudaError_t radt_launch_unpack(const float4 *grad, long long cells, int nbatch, long long batch_stride, float *g_dens,
                                float *g_temp, float *g_vel, cudaStream_t st);
 cudaError_t radt_launch_l2(const float *cube, const float *target, double sigma, long long n, float *dl, double *loss,

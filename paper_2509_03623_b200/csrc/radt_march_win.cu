@@ -62,7 +62,14 @@ __device__ __forceinline__ bool prefilter(const MarchParams &P, const DevGeom &G
     } else if (KIND == 2) {
         const float rho2 = fmaxf(fmaf(x, x, fmaf(y, y, z * z)), 1e-30f);
         const float cz = z * rsqrt_approx(rho2);
-        return rho2 > g.pre_r2lo && rho2 < g.pre_r2hi && cz > g.pre_czlo && cz < g.pre_czhi;
+        const float uf = fmaf(lg2_approx(rho2), g.pre_us_half, g.pre_uoff);
+        const bool in = uf > -1.0f && uf < g.pre_n0f && cz > g.pre_czlo && cz < g.pre_czhi;
+        if (!in) return false;
+        if (!P.use_occ) return true;
+        // bit (I, C) = (floor(u) + 1, bin of cos theta), any phi
+        const int I = rn_int(uf + 0.5f), C = rn_int(fmaf(cz - g.pre_czlo, g.pre_cscale, -0.5f));
+        const unsigned w = __ldg(occ + (I * P.occ_wpr + (C >> 5)));
+        return (w >> (C & 31)) & 1u;
     } else {
         const float tx = (x - g.pre_lo[0]) * g.pre_inv_d[0], ty = (y - g.pre_lo[1]) * g.pre_inv_d[1],
                     tz = (z - g.pre_lo[2]) * g.pre_inv_d[2];

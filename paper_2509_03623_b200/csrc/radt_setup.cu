@@ -207,7 +207,23 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
         if (P.do_pack) {
             float tt = __ldg(P.temp + src);
             tmax = fmaxf(tmax, tt);
-            P.ws.cells[dst] = make_float4(__ldg(P.dens + src), tt, __ldg(P.vel + src), 0.0f);
+            const float dd = __ldg(P.dens + src);
+            P.ws.cells[dst] = make_float4(dd, tt, __ldg(P.vel + src), 0.0f);
+            if (P.do_occ && P.grid.kind == 2) {
+                // spherical grids: flag (i, j) when any of its phi nodes can emit (or is NaN); the flags were zeroed with the
+                // counters.  phi runs fastest, so the lanes of a warp normally share (i, j): one atomic per warp.
+                const bool fl = !(dd <= P.occ_thr);
+                const int ij = (int)(c / P.grid.n2), i = ij / P.grid.n1, j = ij - i * P.grid.n1;
+                unsigned *w = P.ws.nodeflag + ((size_t)(P.b0 + b) * P.grid.n0 + i) * P.flag_wpr + (j >> 5);
+                const unsigned am = __activemask();
+                const int leader = __ffs(am) - 1;
+                const long long key = (long long)(P.b0 + b) * P.grid.cells + ij;
+                if (__all_sync(am, key == __shfl_sync(am, key, leader))) {
+                    if (__any_sync(am, fl) && (int)(threadIdx.x & 31) == leader) atomicOr(w, 1u << (j & 31));
+                } else if (fl) {
+                    atomicOr(w, 1u << (j & 31));
+                }
+            }
         }
         if (P.do_zero_grad) {
             P.ws.grad[dst] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -217,6 +233,35 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
 #pragma unroll
     for (int m = 16; m > 0; m >>= 1) tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, m));
     if ((threadIdx.x & 31) == 0 && tmax > 0.f) atomicMax(reinterpret_cast<int *>(P.ws.counters + 4), __float_as_int(tmax));
+}
+
+// Spherical occupancy words from the (i, j) node flags (second launch: needs every flag).  The prefilter locates a step in
+// fp32 as I = floor(u') + 1 (radial, as on the axisymmetric grid) and C = bin of cos(theta) among n1 uniform bins over
+// [pre_czlo, pre_czhi].  Bit C of word (I, C / 32) is set when some node of radial rows I-2 .. I+1 and of the theta nodes that
+// a step in that bin can touch (the bin's theta range widened by one cell on both sides) is flagged.  One thread per bit.
+__global__ void __launch_bounds__(256) k_occ_sph(const __grid_constant__ SetupParams P)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long wq = t >> 5;
+    if (wq >= (long long)P.occ_words * P.nbatch) return;
+    const int ln = threadIdx.x & 31;
+    const int b = (int)(wq / P.occ_words);
+    const int w = (int)(wq - (long long)b * P.occ_words);
+    const int I = w / P.occ_wpr, C = (w - I * P.occ_wpr) * 32 + ln;
+    bool found = false;
+    if (C < P.grid.n1) {
+        // cos(theta) range of the bin -> theta range -> node range, one cell of margin on both sides
+        const double c_lo = (double)P.grid.pre_czlo + (double)C / (double)P.grid.pre_cscale;
+        const double c_hi = (double)P.grid.pre_czlo + (double)(C + 1) / (double)P.grid.pre_cscale;
+        const double th_a = acos(fmin(fmax(c_hi, -1.0), 1.0)), th_b = acos(fmin(fmax(c_lo, -1.0), 1.0));      // th_a <= th_b
+        const double th0 = 1.5707963267948966 - (double)P.grid.th_c0, sc = (double)P.grid.th_scale;
+        const int j0 = max((int)floor((th_a - th0) * sc) - 1, 0), j1 = min((int)floor((th_b - th0) * sc) + 2, P.grid.n1 - 1);
+        const unsigned *fl = P.ws.nodeflag + (size_t)(P.b0 + b) * P.grid.n0 * P.flag_wpr;
+        for (int ii = max(I - 2, 0); ii <= min(I + 1, P.grid.n0 - 1) && !found; ++ii)
+            for (int j = j0; j <= j1; ++j) found |= (fl[(size_t)ii * P.flag_wpr + (j >> 5)] >> (j & 31)) & 1u;
+    }
+    const unsigned word = __ballot_sync(0xffffffffu, found);
+    if (ln == 0) P.ws.occ[(size_t)(P.b0 + b) * P.occ_words + w] = word;
 }
 
 __global__ void __launch_bounds__(256) k_unpack_grad(const float4 *__restrict__ grad, long long cells, int nbatch,
@@ -296,10 +341,17 @@ cudaError_t radt_launch_setup(const SetupParams &P, const LevelTable &L, const C
         nb_pack = (int)(nb < 148 * 16 ? nb : 148 * 16);
     }
     long long occ_threads = (long long)P.occ_words * P.nbatch * 32;
-    int nb_occ = P.do_occ ? (int)((occ_threads + 255) / 256) : 0;
+    int nb_occ = (P.do_occ && P.grid.kind != 2) ? (int)((occ_threads + 255) / 256) : 0;     // (spherical: radt_launch_occ_sph)
     int nb = nb_rays + nb_tab + nb_occ + nb_pack;
     if (nb == 0) return cudaSuccess;
     k_setup<<<nb, 256, 0, st>>>(P, L, V, nb_rays, nb_tab, nb_occ);
+    return cudaGetLastError();
+}
+
+cudaError_t radt_launch_occ_sph(const SetupParams &P, cudaStream_t st)
+{
+    const long long threads = (long long)P.occ_words * P.nbatch * 32;
+    k_occ_sph<<<(int)((threads + 255) / 256), 256, 0, st>>>(P);
     return cudaGetLastError();
 }
 
