@@ -153,34 +153,7 @@ __device__ __forceinline__ void mlp_stage(float *dst, const float *__restrict__ 
     for (int q = (count & ~3) + threadIdx.x; q < count; q += nthreads) dst[q] = __ldg(src + q);
 }
 
-__global__ void __launch_bounds__(MLP_TF / 2 * MLP_P8) k_mlp_fwd(const __grid_constant__ MlpParamsDev Q)
-{
-    // 64 node pairs x 8 parts: thread (pair, part) serves nodes pair and pair + 64 and output units 8 part .. 8 part + 7
-    const int pair = threadIdx.x & (MLP_TF / 2 - 1), part = threadIdx.x / (MLP_TF / 2);     // part is warp uniform
-    const int n0 = pair, n1 = pair + MLP_TF / 2, n = Q.nr * Q.nz;
-    const MlpOff F = mlp_offsets(Q.L);
-    float *A = mlp_smem, *B = mlp_smem + MLP_W * MLP_TF;           // ping-pong [unit][node]
-    float *sP = B + MLP_W * MLP_TF;                                // all parameters (a uniform global load per weight
-    mlp_stage(sP, Q.params, F.b[MLP_H] + 1, MLP_TF / 2 * MLP_P8);  // left the kernel waiting on L1/L2: 17 stall cycles per issue)
-    if (part < 2) {
-        const int node = part == 0 ? n0 : n1, qq = min(blockIdx.x * MLP_TF + node, n - 1);
-        mlp_encode(Q, qq / Q.nz, qq % Q.nz, A, MLP_TF, node);
-    }
-    __syncthreads();
-    // first layer: 4 parts x 16 units for each of the two nodes (parts 0-3: n0, parts 4-7: n1)
-    mlp_layer_first(sP + F.W[0], sP + F.b[0], F.D, A, B, MLP_TF, part < 4 ? n0 : n1, part & 3);
-    __syncthreads();
-    mlp_layer2(sP + F.W[1], sP + F.b[1], B, A, MLP_TF, n0, n1, part);
-    __syncthreads();
-    mlp_layer2(sP + F.W[2], sP + F.b[2], A, B, MLP_TF, n0, n1, part);
-    __syncthreads();
-    mlp_layer2(sP + F.W[3], sP + F.b[3], B, A, MLP_TF, n0, n1, part);
-    __syncthreads();
-    if (part >= 2) return;
-    const int node = part == 0 ? n0 : n1, q = blockIdx.x * MLP_TF + node;
-    const float s = mlp_head(sP + F.W[4], sP[F.b[4]], A, MLP_TF, node);
-    if (q < n) Q.temp_out[q] = fmaf(Q.t_hi - Q.t_lo, s, Q.t_lo);
-}
+// (The forward pass runs on the tensor cores: radt_mlp_tc.cu.  The helpers above serve the adjoint's recompute.)
 
 // dW[o][i] = sum_n delta[o][n] a[i][n] for this block's nodes; thread t owns input unit i = t (its activations over
 // the nodes sit in registers), output units one at a time with broadcast float4 reads of the delta rows.
@@ -402,17 +375,6 @@ __global__ void __launch_bounds__(MLP_TB * MLP_S, 2) k_mlp_bwd(const __grid_cons
 // launchers
 // ---------------------------------------------------------------------------------------------
 static size_t mlp_bwd_smem() { return (size_t)(MLP_WBUF + 4 + 34 * MLP_SA + MLP_H * MLP_W * MLP_SA + 4 + MLP_W * MLP_SD + MLP_TB) * sizeof(float); }
-
-cudaError_t radt_launch_mlp_fwd(const MlpParamsDev &Q, cudaStream_t st)
-{
-    // two activation buffers + the whole parameter vector (padded to the allocation granularity of the caller)
-    const size_t smem = (size_t)(2 * MLP_W * MLP_TF + ((Q.nparams + 3) & ~3)) * sizeof(float);
-    cudaError_t e = cudaFuncSetAttribute(k_mlp_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    const int n = Q.nr * Q.nz;
-    k_mlp_fwd<<<(n + MLP_TF - 1) / MLP_TF, MLP_TF / 2 * MLP_P8, smem, st>>>(Q);
-    return cudaGetLastError();
-}
 
 cudaError_t radt_launch_mlp_bwd(const MlpParamsDev &Q, int nparams, cudaStream_t st)
 {
