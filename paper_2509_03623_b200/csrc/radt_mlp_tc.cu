@@ -2,38 +2,49 @@
 // the 5th-generation tensor cores of sm_100a: tcgen05.mma (kind::tf32) with the accumulators in tensor memory.
 //
 // The four hidden layers are dense 64-wide contractions: per tile of 128 grid nodes, h_l [128 x 64] = relu(h_{l-1} W_l^T + b_l).
-//   - one CTA = 128 threads = one tile of 128 nodes at a time (persistent over tiles); thread t owns node row t, which is
-//     TMEM lane t of the accumulator D [128 lanes x 64 fp32 columns];
-//   - operands live in shared memory in the canonical K-major, no-swizzle UMMA layout: the tile is cut into chunks of 4 K
-//     elements (16 bytes), chunk j of row r at  j * (rows * 16) + r * 16  (8 rows x 16 bytes = one 128-byte core matrix;
-//     leading byte offset = rows * 16 between K-adjacent core matrices, stride byte offset = 128 between groups of 8 rows);
+//   - one CTA = 2 groups of 256 threads, each group with its own tile of 128 nodes in flight (persistent over tiles; the
+//     tensor core works on one group's layer while the other group converts its accumulator); node row r is TMEM lane r of the
+//     accumulator D [128 lanes x 64 fp32 columns] and is served by threads r (columns 0-31) and r + 128 (columns 32-63): two
+//     warps per scheduler, so that one warp's TMEM loads and conversions overlap the other's;
+//   - the A operand (activations, [128 x K]) lives in TENSOR MEMORY as well (lane = node row, one column per K element):
+//     with only 8 K elements per tf32 MMA, an A operand in shared memory made the MMAs wait on 4 KB of operand reads each
+//     (100 cycles per MMA against the 32-cycle floor of a 128 x 64 tile);
+//   - the B operand (weights, [64 x K]) lives in shared memory in the canonical K-major, no-swizzle UMMA layout: chunks of 4
+//     K elements (16 bytes), chunk j of row r at  j * 1024 + r * 16  (8 rows x 16 bytes = one 128-byte core matrix; leading
+//     byte offset = 1024 between K-adjacent core matrices, stride byte offset = 128 between groups of 8 rows);
 //   - fp32 accuracy from TF32 tensor cores by the 3-product split: x = x_hi + x_lo with x_hi = rna_tf32(x), x_lo = x - x_hi
 //     (exact), D = A_hi B_hi + A_lo B_hi + A_hi B_lo, the dropped A_lo B_lo term is 2^-22 of the product;
 //   - one elected thread issues the K/8 x 3 MMAs of a layer and commits them to an mbarrier; all threads then read their
-//     row of D with tcgen05.ld (32x32b.x32), add the bias, apply the ReLU, split and write the next layer's A operand;
-//     the activations never leave the SM between layers;
+//     row of D with tcgen05.ld (32x32b.x32), add the bias, apply the ReLU, split and write the next layer's A operand
+//     back with tcgen05.st; the activations never leave tensor memory / registers between layers;
 //   - weights (hi and lo copies of all four layers, 108 KB) are converted and staged once per CTA.
 // The output unit (64 -> 1) and the sigmoid are a dot product per thread in the last epilogue.  Shares nothing with oracle/.
 #include "radt_dev.cuh"
 #include "radt_kernels.h"
 
-#define TC_M 128                        // nodes per tile = TMEM lanes = threads
+#define TC_M 128                        // nodes per tile = TMEM lanes
+#define TC_GROUP 256                    // threads per tile: two per node row
+#define TC_THREADS 512                  // two groups per CTA, each with its own tile in flight: one group's epilogue runs under
+                                        // the other's MMAs
 #define TC_W 64                         // hidden width = UMMA N
 #define TC_KMAX1 40                     // first-layer fan-in padded to a multiple of 8 (D = 2 + 4 L <= 34)
-#define TC_A_CHUNK (TC_M * 16)          // bytes of one 4-wide K chunk of an A tile   (leading byte offset of A)
 #define TC_B_CHUNK (TC_W * 16)          // bytes of one 4-wide K chunk of a weight tile (leading byte offset of B)
 #define TC_SBO 128                      // 8 rows x 16 bytes
+#define TC_COL_D 0                      // TMEM columns: accumulator, A_hi, A_lo (64 fp32 columns each; 256 allocated)
+#define TC_COL_AHI 64
+#define TC_COL_ALO 128
+#define TC_COLS_GROUP 192               // per group
+#define TC_COLS 512
 
 // shared-memory map (bytes)
-#define TC_OFF_AHI 0
-#define TC_OFF_ALO (TC_OFF_AHI + 16 * TC_A_CHUNK)                  // 32 KB each
-#define TC_OFF_W1HI (TC_OFF_ALO + 16 * TC_A_CHUNK)
+#define TC_OFF_W1HI 0
 #define TC_OFF_W1LO (TC_OFF_W1HI + (TC_KMAX1 / 4) * TC_B_CHUNK)    // 10 KB each
 #define TC_OFF_WHI (TC_OFF_W1LO + (TC_KMAX1 / 4) * TC_B_CHUNK)     // layers 2-4: 3 x 16 KB
 #define TC_OFF_WLO (TC_OFF_WHI + 3 * 16 * TC_B_CHUNK)
 #define TC_OFF_BIAS (TC_OFF_WLO + 3 * 16 * TC_B_CHUNK)             // 4 x 64 biases, 64 output weights, output bias
-#define TC_OFF_BAR (TC_OFF_BIAS + (5 * TC_W + 4) * 4)
-#define TC_SMEM_BYTES (TC_OFF_BAR + 16)
+#define TC_OFF_PART (TC_OFF_BIAS + (5 * TC_W + 4) * 4)              // partial output sums of the upper half-rows
+#define TC_OFF_BAR (TC_OFF_PART + 2 * TC_M * 4)                   // two mbarriers, TMEM base address
+#define TC_SMEM_BYTES (TC_OFF_BAR + 32)
 
 __device__ __forceinline__ unsigned tc_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -46,11 +57,18 @@ __device__ __forceinline__ unsigned long long tc_desc(unsigned saddr, unsigned l
 // instruction descriptor of kind::tf32: D fp32, A and B TF32, both K-major, N = 64, M = 128
 #define TC_IDESC ((1u << 4) | (2u << 7) | (2u << 10) | ((TC_W >> 3) << 17) | ((TC_M >> 4) << 24))
 
-__device__ __forceinline__ void tc_mma(unsigned tmem_d, unsigned long long adesc, unsigned long long bdesc, unsigned accumulate)
+__device__ __forceinline__ bool tc_elect()
+{
+    unsigned pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.b32 %0, 1, 0, P;\n\t}\n" : "=r"(pred));
+    return pred != 0;
+}
+// D[tmem] (+)= A[tmem] B[smem]^T
+__device__ __forceinline__ void tc_mma(unsigned tmem_d, unsigned tmem_a, unsigned long long bdesc, unsigned accumulate)
 {
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(tmem_d),
-                 "l"(adesc), "l"(bdesc), "r"(TC_IDESC), "r"(accumulate)
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}\n" ::"r"(tmem_d),
+                 "r"(tmem_a), "l"(bdesc), "r"(TC_IDESC), "r"(accumulate)
                  : "memory");
 }
 __device__ __forceinline__ void tc_commit(unsigned bar)
@@ -87,6 +105,28 @@ __device__ __forceinline__ float tc_tf32(float x)
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(y) : "f"(x));
     return __uint_as_float(y);
 }
+// four / thirty-two consecutive columns of this thread's TMEM lane
+__device__ __forceinline__ void tc_st4(unsigned taddr, float a, float b, float c, float d)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(__float_as_uint(a)),
+                 "r"(__float_as_uint(b)), "r"(__float_as_uint(c)), "r"(__float_as_uint(d))
+                 : "memory");
+}
+__device__ __forceinline__ void tc_st32(unsigned taddr, const float (&v)[32])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%32], "
+                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, %21, %22, %23, "
+                 "%24, %25, %26, %27, %28, %29, %30, %31};" ::"r"(__float_as_uint(v[0])),
+                 "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])), "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])),
+                 "r"(__float_as_uint(v[5])), "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])), "r"(__float_as_uint(v[8])),
+                 "r"(__float_as_uint(v[9])), "r"(__float_as_uint(v[10])), "r"(__float_as_uint(v[11])), "r"(__float_as_uint(v[12])),
+                 "r"(__float_as_uint(v[13])), "r"(__float_as_uint(v[14])), "r"(__float_as_uint(v[15])), "r"(__float_as_uint(v[16])),
+                 "r"(__float_as_uint(v[17])), "r"(__float_as_uint(v[18])), "r"(__float_as_uint(v[19])), "r"(__float_as_uint(v[20])),
+                 "r"(__float_as_uint(v[21])), "r"(__float_as_uint(v[22])), "r"(__float_as_uint(v[23])), "r"(__float_as_uint(v[24])),
+                 "r"(__float_as_uint(v[25])), "r"(__float_as_uint(v[26])), "r"(__float_as_uint(v[27])), "r"(__float_as_uint(v[28])),
+                 "r"(__float_as_uint(v[29])), "r"(__float_as_uint(v[30])), "r"(__float_as_uint(v[31])), "r"(taddr)
+                 : "memory");
+}
 // four consecutive K elements of row `row` into the hi and lo copies of an operand tile
 __device__ __forceinline__ void tc_store4(unsigned char *hi, unsigned char *lo, int chunk_bytes, int chunk, int row, float a, float b,
                                           float c, float d)
@@ -99,149 +139,156 @@ __device__ __forceinline__ void tc_store4(unsigned char *hi, unsigned char *lo, 
 
 extern __shared__ __align__(128) unsigned char tc_smem[];
 
-__global__ void __launch_bounds__(TC_M, 1) k_mlp_fwd_tc(const __grid_constant__ MlpParamsDev Q, int ntiles)
+__global__ void __launch_bounds__(TC_THREADS, 1) k_mlp_fwd_tc(const __grid_constant__ MlpParamsDev Q, int ntiles)
 {
-    const int t = threadIdx.x, warp = t >> 5;
+    const int t = threadIdx.x, group = t >> 8, tg = t & (TC_GROUP - 1), warp = tg >> 5, row = tg & (TC_M - 1), half = tg >> 7;
     const int D = 2 + 4 * Q.L, K1 = (D + 7) & ~7;
     unsigned char *sm = tc_smem;
-    float *sBias = reinterpret_cast<float *>(sm + TC_OFF_BIAS);
-    const unsigned bar = tc_smem_u32(sm + TC_OFF_BAR);
-    unsigned *tmem_slot = reinterpret_cast<unsigned *>(sm + TC_OFF_BAR + 8);
+    float *sBias = reinterpret_cast<float *>(sm + TC_OFF_BIAS), *sPart = reinterpret_cast<float *>(sm + TC_OFF_PART) + TC_M * group;
+    const unsigned bar = tc_smem_u32(sm + TC_OFF_BAR) + 8 * group;
+    unsigned *tmem_slot = reinterpret_cast<unsigned *>(sm + TC_OFF_BAR + 16);
 
     // ---- one-time set-up: TMEM allocation (warp 0), mbarrier, weights split into hi / lo operand tiles
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc_smem_u32(tmem_slot)), "r"(64));
+    if (t < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tc_smem_u32(tmem_slot)), "r"(TC_COLS));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
-    if (t == 0) {
+    if (tg == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(1));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     {
         // parameter vector: [W1 (64 x D) | b1 | W2 | b2 | W3 | b3 | W4 | b4 | w_out | b_out]
         const float *p = Q.params;
-        for (int q = t; q < TC_W * (K1 / 4); q += TC_M) {          // first layer: rows n, chunks of 4 inputs, zero padded
+        // layers 2-4: 3 x 1024 float4, six per thread, all loads in flight before the first conversion (a load-convert-
+        // store loop left the CTA waiting on L2 for 5 cycles per issued instruction); rows fastest over the threads, so that
+        // the 16-byte stores of a quarter-warp fall into different banks
+        const int off2 = TC_W * D + TC_W, lstride = TC_W * TC_W + TC_W;
+        float4 v[6];
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+            const int g = t + TC_THREADS * i, l = g >> 10, r = g & 1023, n = r & (TC_W - 1), j = r >> 6;
+            v[i] = __ldg(reinterpret_cast<const float4 *>(p + off2 + l * lstride + n * TC_W) + j);     // (offsets are multiples of 4: D is even)
+        }
+        for (int q = t; q < 4 * TC_W; q += TC_THREADS)             // biases of the four layers
+            sBias[q] = __ldg(p + (q < TC_W ? TC_W * D + q : off2 + ((q >> 6) - 1) * lstride + TC_W * TC_W + (q & (TC_W - 1))));
+        const int off5 = off2 + 3 * lstride;
+        for (int q = t; q < TC_W; q += TC_THREADS) sBias[4 * TC_W + q] = __ldg(p + off5 + q);       // output weights
+        if (t == 0) sBias[5 * TC_W] = __ldg(p + off5 + TC_W);                                       // output bias
+        for (int q = t; q < TC_W * (K1 / 4); q += TC_THREADS) {          // first layer: rows n, chunks of 4 inputs, zero padded
             const int n = q % TC_W, j = q / TC_W;
             float v[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) v[e] = (4 * j + e) < D ? __ldg(p + n * D + 4 * j + e) : 0.f;
             tc_store4(sm + TC_OFF_W1HI, sm + TC_OFF_W1LO, TC_B_CHUNK, j, n, v[0], v[1], v[2], v[3]);
         }
-        int off = TC_W * D;
-        for (int q = t; q < TC_W; q += TC_M) sBias[q] = __ldg(p + off + q);
-        off += TC_W;
-        for (int l = 0; l < 3; ++l) {
-            for (int q = t; q < TC_W * 16; q += TC_M) {
-                const int n = q % TC_W, j = q / TC_W;
-                const float4 v = __ldg(reinterpret_cast<const float4 *>(p + off + n * TC_W) + j);     // (offsets are multiples of 4 iff D is even: it is)
-                tc_store4(sm + TC_OFF_WHI + l * 16 * TC_B_CHUNK, sm + TC_OFF_WLO + l * 16 * TC_B_CHUNK, TC_B_CHUNK, j, n, v.x, v.y,
-                          v.z, v.w);
-            }
-            off += TC_W * TC_W;
-            for (int q = t; q < TC_W; q += TC_M) sBias[(l + 1) * TC_W + q] = __ldg(p + off + q);
-            off += TC_W;
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+            const int g = t + TC_THREADS * i, l = g >> 10, r = g & 1023, n = r & (TC_W - 1), j = r >> 6;
+            tc_store4(sm + TC_OFF_WHI + l * 16 * TC_B_CHUNK, sm + TC_OFF_WLO + l * 16 * TC_B_CHUNK, TC_B_CHUNK, j, n, v[i].x, v[i].y,
+                      v[i].z, v[i].w);
         }
-        for (int q = t; q < TC_W; q += TC_M) sBias[4 * TC_W + q] = __ldg(p + off + q);        // output weights
-        if (t == 0) sBias[5 * TC_W] = __ldg(p + off + TC_W);                                  // output bias
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const unsigned tmem = *tmem_slot;
-    const unsigned taddr = tmem + ((unsigned)(warp * 32) << 16);          // this warp's lane quadrant
-    const unsigned sA_hi = tc_smem_u32(sm + TC_OFF_AHI), sA_lo = tc_smem_u32(sm + TC_OFF_ALO);
+    const unsigned tmem = *tmem_slot + TC_COLS_GROUP * group;          // this group's columns
+    const unsigned taddr = tmem + ((unsigned)((warp & 3) * 32) << 16) + TC_COL_D + 32 * half;      // this warp's lane quadrant, this half's columns of D
+    const unsigned tlane = tmem + ((unsigned)((warp & 3) * 32) << 16);                  // this thread's TMEM lane, column 0
     unsigned parity = 0;
     const int n = Q.nr * Q.nz;
 
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    for (int tile = 2 * blockIdx.x + group; tile < ntiles; tile += 2 * gridDim.x) {
         // ---- M1-M2: encoding of this thread's node into the layer-1 A operand (K1 columns, zero padded)
         {
-            const int qq = min(tile * TC_M + t, n - 1);
+            const int qq = min(tile * TC_M + row, n - 1);
             const int i = qq / Q.nz, j = qq - i * Q.nz;
             const float p0 = (float)i / (float)(Q.nr - 1), p1 = (float)j / (float)(Q.nz - 1);
-            float f[TC_KMAX1];
+            // chunk c holds features 4c .. 4c+3 of gamma = (p0, p1, {sin, cos (2^k pi p0), sin, cos (2^k pi p1)}_k); the two
+            // threads of a row write alternate chunks c = 2 cc + half: entries {0, 1} are sin, cos of 2^(c-1) pi p1 (chunk 0:
+            // p0, p1 themselves) and entries {2, 3} are sin, cos of 2^c pi p0 -- one sincospi per pair
 #pragma unroll
-            for (int e = 0; e < TC_KMAX1; ++e) f[e] = 0.f;
-            f[0] = p0; f[1] = p1;
-            float fr = 1.0f;
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                if (k < Q.L) {
-                    f[2 + 4 * k + 0] = sinpif(fr * p0); f[2 + 4 * k + 1] = cospif(fr * p0);
-                    f[2 + 4 * k + 2] = sinpif(fr * p1); f[2 + 4 * k + 3] = cospif(fr * p1);
+            for (int cc = 0; cc < TC_KMAX1 / 8; ++cc) {
+                const int c = 2 * cc + half;
+                if (4 * c < K1) {
+                    float s1, c1, s0, c0;
+                    sincospif(__int_as_float((126 + c) << 23) * p1, &s1, &c1);       // 2^(c-1) p1
+                    sincospif(__int_as_float((127 + c) << 23) * p0, &s0, &c0);       // 2^c p0
+                    if (c == 0) { s1 = p0; c1 = p1; }
+                    if (4 * c + 2 >= D) { s0 = 0.f; c0 = 0.f; }                      // zero padding beyond the D features
+                    if (4 * c >= D) { s1 = 0.f; c1 = 0.f; }
+                    const float h0 = tc_tf32(s1), h1 = tc_tf32(c1), h2 = tc_tf32(s0), h3 = tc_tf32(c0);
+                    tc_st4(tlane + TC_COL_AHI + 4 * c, h0, h1, h2, h3);
+                    tc_st4(tlane + TC_COL_ALO + 4 * c, s1 - h0, c1 - h1, s0 - h2, c0 - h3);
                 }
-                fr *= 2.0f;
             }
-#pragma unroll
-            for (int c = 0; c < TC_KMAX1 / 4; ++c)
-                if (4 * c < K1) tc_store4(sm + TC_OFF_AHI, sm + TC_OFF_ALO, TC_A_CHUNK, c, t, f[4 * c], f[4 * c + 1], f[4 * c + 2], f[4 * c + 3]);
         }
         float temp_out = 0.f;
 #pragma unroll 1
         for (int l = 0; l < 4; ++l) {
-            // the A operand written by the generic proxy must be visible to the tensor core's async proxy; every thread has
-            // also finished reading the previous accumulator
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            // every thread's A columns are in tensor memory and every thread has finished reading the previous accumulator
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncthreads();
-            if (t == 0) {
+            asm volatile("bar.sync %0, %1;" ::"r"(1 + group), "r"(TC_GROUP) : "memory");        // this group's threads only
+            if (warp == 0 && tc_elect()) {                   // one elected lane of warp 0 issues (warp-uniform operands)
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const int ksteps = (l == 0 ? K1 : TC_W) / 8;
                 const unsigned w_hi = tc_smem_u32(sm + (l == 0 ? TC_OFF_W1HI : TC_OFF_WHI + (l - 1) * 16 * TC_B_CHUNK));
                 const unsigned w_lo = tc_smem_u32(sm + (l == 0 ? TC_OFF_W1LO : TC_OFF_WLO + (l - 1) * 16 * TC_B_CHUNK));
+                // a K step of 8 elements: 8 TMEM columns of A, two chunks of B (start-address field of the descriptor)
+                unsigned a_hi = tmem + TC_COL_AHI, a_lo = tmem + TC_COL_ALO;
+                unsigned long long b_hi = tc_desc(w_hi, TC_B_CHUNK, TC_SBO), b_lo = tc_desc(w_lo, TC_B_CHUNK, TC_SBO);
                 unsigned acc = 0;
+#pragma unroll 2
                 for (int s = 0; s < ksteps; ++s) {
-                    const unsigned long long a_hi = tc_desc(sA_hi + 2 * s * TC_A_CHUNK, TC_A_CHUNK, TC_SBO);
-                    const unsigned long long a_lo = tc_desc(sA_lo + 2 * s * TC_A_CHUNK, TC_A_CHUNK, TC_SBO);
-                    const unsigned long long b_hi = tc_desc(w_hi + 2 * s * TC_B_CHUNK, TC_B_CHUNK, TC_SBO);
-                    const unsigned long long b_lo = tc_desc(w_lo + 2 * s * TC_B_CHUNK, TC_B_CHUNK, TC_SBO);
-                    tc_mma(tmem, a_lo, b_hi, acc);          // small terms first
-                    tc_mma(tmem, a_hi, b_lo, 1u);
-                    tc_mma(tmem, a_hi, b_hi, 1u);
+                    tc_mma(tmem + TC_COL_D, a_lo, b_hi, acc);          // small terms first
+                    tc_mma(tmem + TC_COL_D, a_hi, b_lo, 1u);
+                    tc_mma(tmem + TC_COL_D, a_hi, b_hi, 1u);
                     acc = 1u;
+                    a_hi += 8; a_lo += 8;
+                    b_hi += (2 * TC_B_CHUNK) >> 4; b_lo += (2 * TC_B_CHUNK) >> 4;
                 }
                 tc_commit(bar);                              // arrives on the mbarrier when these MMAs have completed
             }
             tc_wait(bar, parity);
             parity ^= 1u;
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const float *bias = sBias + l * TC_W;
+            const float *bias = sBias + l * TC_W + 32 * half;
+            float v[32];
+            tc_ld32(taddr, v);
             if (l < 3) {
+                float hi[32];
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    float v[32];
-                    tc_ld32(taddr + 32 * h, v);
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) {
-                        const int u = 32 * h + 4 * c;
-                        tc_store4(sm + TC_OFF_AHI, sm + TC_OFF_ALO, TC_A_CHUNK, u >> 2, t, fmaxf(v[4 * c] + bias[u], 0.f),
-                                  fmaxf(v[4 * c + 1] + bias[u + 1], 0.f), fmaxf(v[4 * c + 2] + bias[u + 2], 0.f),
-                                  fmaxf(v[4 * c + 3] + bias[u + 3], 0.f));
-                    }
+                for (int c = 0; c < 32; ++c) {
+                    v[c] = fmaxf(v[c] + bias[c], 0.f);
+                    hi[c] = tc_tf32(v[c]);
+                    v[c] -= hi[c];
                 }
+                tc_st32(tlane + TC_COL_AHI + 32 * half, hi);
+                tc_st32(tlane + TC_COL_ALO + 32 * half, v);
             } else {
-                // M3 output unit and M4: sigmoid scaled to [t_lo, t_hi]
-                const float *w5 = sBias + 4 * TC_W;
-                float o = sBias[5 * TC_W];
+                // M3 output unit and M4: each half-row's share of the dot product, then the sigmoid scaled to [t_lo, t_hi]
+                const float *w5 = sBias + 4 * TC_W + 32 * half;
+                float o = 0.f;
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    float v[32];
-                    tc_ld32(taddr + 32 * h, v);
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) o = fmaf(w5[32 * h + c], fmaxf(v[c] + bias[32 * h + c], 0.f), o);
+                for (int c = 0; c < 32; ++c) o = fmaf(w5[c], fmaxf(v[c] + bias[c], 0.f), o);
+                if (half) sPart[row] = o;
+                asm volatile("bar.sync %0, %1;" ::"r"(1 + group), "r"(TC_GROUP) : "memory");
+                if (!half) {
+                    o += sPart[row] + sBias[5 * TC_W];
+                    temp_out = fmaf(Q.t_hi - Q.t_lo, 1.0f / (1.0f + __expf(-o)), Q.t_lo);
                 }
-                temp_out = fmaf(Q.t_hi - Q.t_lo, 1.0f / (1.0f + __expf(-o)), Q.t_lo);
             }
         }
-        const int q = tile * TC_M + t;
-        if (q < n) Q.temp_out[q] = temp_out;
+        const int q = tile * TC_M + row;
+        if (!half && q < n) Q.temp_out[q] = temp_out;
     }
     // ---- teardown: every thread is done with the accumulator before warp 0 frees it
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) {
+    if (t < 32) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(64));
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(TC_COLS));
     }
 }
 
@@ -252,6 +299,7 @@ cudaError_t radt_launch_mlp_fwd(const MlpParamsDev &Q, cudaStream_t st)
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    k_mlp_fwd_tc<<<ntiles < sms ? ntiles : sms, TC_M, TC_SMEM_BYTES, st>>>(Q, ntiles);
+    const int pairs = (ntiles + 1) / 2;
+    k_mlp_fwd_tc<<<pairs < sms ? pairs : sms, TC_THREADS, TC_SMEM_BYTES, st>>>(Q, ntiles);
     return cudaGetLastError();
 }
