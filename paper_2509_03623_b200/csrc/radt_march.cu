@@ -238,7 +238,7 @@ __device__ __forceinline__ void reduce_batch(const float4 (*red)[32], int nb, fl
 }
 
 template <int KIND, int NP, bool CL, bool COMP>
-__global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, (COMP && NP == 4) ? 2 : 3) k_march_bwd(const __grid_constant__ MarchParams P)
+__global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, (COMP && NP == 4) ? 4 : 6) k_march_bwd(const __grid_constant__ MarchParams P)
 {
     __shared__ float4 sh_p[RADT_WARPS_PER_CTA][32];
     __shared__ float sh_s[RADT_WARPS_PER_CTA][32];

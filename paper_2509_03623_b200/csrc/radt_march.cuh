@@ -217,7 +217,8 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     if (UNI) {
         // channel lattice v_c = v0 + c dv: with c_ref the channel nearest to v_los, u'(c) = u0 + (c - c_ref) dvA
         // and |u0| <= |dvA|/2, so u' carries only the relative rounding of dvA
-        double xd = fmin(fmax((vlos_d - G.v0) * L.inv_dv, -1.0e6), 1.0e6);
+        double xd = (vlos_d - G.v0) * L.inv_dv;
+        if (!(fabs(xd) <= 1.0e6)) xd = xd > 0.0 ? 1.0e6 : -1.0e6;      // (far off the cube: any channel out of range will do)
         double xm = xd + 6755399441055744.0;             // 1.5 2^52: the rounded integer sits in the low word
         st.cref = __double2loint(xm);
         float del = (float)((xm - 6755399441055744.0) - xd);   // c_ref - x

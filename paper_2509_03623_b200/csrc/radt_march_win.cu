@@ -16,10 +16,11 @@
 #include "radt_march.cuh"
 
 #ifndef RADT_WIN_MINB_FWD
-#define RADT_WIN_MINB_FWD 4     // CTAs per SM the kernels are compiled for (measured: 4 vs 3 gives fwd -3 %, bwd +2 %)
+#define RADT_WIN_MINB_FWD 8     // CTAs (of 4 warps) per SM the kernels are compiled for: 64 and 80 registers per thread
+                                // (measured: 72 registers and 7 CTAs for the adjoint is slower, the spills cost more)
 #endif
 #ifndef RADT_WIN_MINB_BWD
-#define RADT_WIN_MINB_BWD 3
+#define RADT_WIN_MINB_BWD 6
 #endif
 #define WIN_PAIRS 16         // slot pairs per batch of 32 steps
 #define NO_GROUP 0x7fffffff
@@ -27,7 +28,7 @@
 struct __align__(16) WinShared {          // per warp
     float4 a[WIN_PAIRS];                  // {u0_a, u0_b, dvA_a, dvA_b}
     float4 b[WIN_PAIRS];                  // {K2_a, K2_b, S_a, S_b}
-    float4 c[WIN_PAIRS];                  // {c_ref_a, c_ref_b, bits of u_lo, bits of u_hi}: union window of the pair
+    float4 c[WIN_PAIRS];                  // {c_ref_a, c_ref_b, bits of u_lo, bits of 31 - (u_hi - u_lo)}: union window of the pair
     int cand[64];                         // candidate step indices waiting for phase A (circular queue)
     int2 win[32];                         // channel windows of the compacted steps
     double ray[6];                        // ox, oy, oz, s0, ds of the ray (fp64: read once per batch by phase A)
@@ -118,7 +119,7 @@ __device__ __forceinline__ int write_entries(WinShared &S, int lane, bool act, i
         fc[q] = (float)st.cref;
         if (!(pos & 1)) {
             fc[q + 2] = __int_as_float(ulo);
-            fc[q + 3] = __int_as_float(uhi);
+            fc[q + 3] = __int_as_float(31 - (uhi - ulo));
             if (pos == cnt - 1) { fa[q + 1] = 0.f; fa[q + 3] = 0.f; fb[q + 1] = 0.f; fb[q + 3] = 0.f; fc[q + 1] = 0.f; }
         }
     }
@@ -126,10 +127,11 @@ __device__ __forceinline__ int write_entries(WinShared &S, int lane, bool act, i
     return (cnt + 1) >> 1;
 }
 
-// The pair's union window [ulo, uhi] no longer fits the current group [cur, cur + 32)?
-__device__ __forceinline__ bool group_misses(int cur, int ulo, int uhi) { return ulo < cur || uhi > cur + 31; }
+// The pair's union window [ulo, uhi] (given as ulo and lim = 31 - (uhi - ulo) >= 0) no longer fits the current group
+// [cur, cur + 32)?  It fits iff 0 <= ulo - cur <= lim: one unsigned comparison (cur = NO_GROUP always misses).
+__device__ __forceinline__ bool group_misses(int cur, int ulo, int lim) { return (unsigned)(ulo - cur) > (unsigned)lim; }
 // New group for that union: centred, so that the line can drift either way before the lanes change channel again.
-__device__ __forceinline__ int group_for(int ulo, int uhi) { return ulo - ((31 - (uhi - ulo)) >> 1); }
+__device__ __forceinline__ int group_for(int ulo, int lim) { return ulo - (lim >> 1); }
 
 // Per-lane channel state of the forward window march.  The (I, T) of all channels of the ray live in shared
 // memory (channel c is only ever touched by lane c & 31); the lane keeps the pair of the ONE channel it serves in
@@ -192,13 +194,17 @@ __device__ __forceinline__ void fwd_pair(const float4 &qa, const float4 &qb, con
     upk(s.e, e0, e1);
     const float m0 = __fmul_rn(om0, Ts);
     const float I1 = __fmaf_rn(qb.z, m0, Is);
-    // rounding error of I1 = fl(S m + Is): Is - I1 is exact whenever the contribution is small against the sum, which
-    // is when it matters
-    if (COMP) Ls += __fmaf_rn(qb.z, m0, __fsub_rn(Is, I1));
     Ts = __fmul_rn(Ts, e0);
     const float m1 = __fmul_rn(om1, Ts);
     const float I2 = __fmaf_rn(qb.w, m1, I1);
-    if (COMP) Ls += __fmaf_rn(qb.w, m1, __fsub_rn(I1, I2));
+    if (COMP) {
+        // rounding errors of I1 = fl(S m + Is) and I2: Is - I1 is exact whenever the contribution is small against the
+        // sum, which is when it matters; both steps in one packed subtraction and one packed fma (the same values as the
+        // adjoint's scalar ones)
+        float r0, r1;
+        upk(fma2(pk(qb.z, qb.w), pk(m0, m1), sub2(pk(Is, I1), pk(I1, I2))), r0, r1);
+        Ls = (Ls + r0) + r1;
+    }
     Is = I2;
     Ts = __fmul_rn(Ts, e1);
 }
@@ -295,8 +301,8 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
 #pragma unroll 2
                 for (int i = 0; i < npairs; ++i) {
                     const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
-                    const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
-                    if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
+                    const int ulo = __float_as_int(qc.z), lim = __float_as_int(qc.w);
+                    if (group_misses(L.cur, ulo, lim)) L.regroup(group_for(ulo, lim), lane, nchan);
                     fwd_pair<COMP>(qa, qb, qc, L.cf, L.Is, L.Ts, L.Ls);
                 }
                 n_mufu += 4 * npairs;
@@ -336,10 +342,11 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
 template <bool COMP>
 struct BwdLane {
     float Ts, Ps, Is, Gs, cf;                     // transmittance, partial sum, saved I, dL/dI of the served channel
-    float Qs, Ils;                                // COMP: low-order words of the partial sum and of the saved I
+    float Qs;                                     // COMP: low-order word of the partial sum MINUS that of the saved I (the
+                                                  // word starts at -I_lo instead of 0: only the difference is ever used)
     int cur, myc;
     float *sT, *sP, *sQ;
-    const float *Isave, *Gin, *Ilo;
+    const float *Isave, *Gin;
     __device__ __forceinline__ void put_back()
     {
         if (myc >= 0) {
@@ -354,15 +361,13 @@ struct BwdLane {
         myc = (unsigned)c < (unsigned)nchan ? c : -1;
         cf = (float)c;
         Ts = 1.f; Ps = 0.f; Is = 0.f; Gs = 0.f;    // lanes without a channel contribute nothing (G = 0)
-        Qs = 0.f; Ils = 0.f;
+        Qs = 0.f;
         if (myc >= 0) {
             Ts = sT[c]; Ps = sP[c]; Is = __ldg(Isave + c); Gs = __ldg(Gin + c);
-            if (COMP) { Qs = sQ[c]; Ils = __ldg(Ilo + c); }
+            if (COMP) Qs = sQ[c];
         }
         cur = clo;
     }
-    // -R = (P - I) + (P_lo - I_lo) of the served channel
-    __device__ __forceinline__ float neg_r() const { return COMP ? (Ps - Is) + (Qs - Ils) : Ps - Is; }
 };
 
 // Partial sums of a reduction batch of BWD_SUB pairs: 4 BWD_SUB rows (pair jj, component q of {w, w u', w u'^2, G (1-e) T}),
@@ -404,7 +409,7 @@ __device__ __forceinline__ void bwd_pair_e(const float4 &qa, const float4 &qb, c
         // them the difference is good to ~1e-14 I and needs no clamp
         const float Q0 = L.Qs + __fmaf_rn(qb.z, c0, __fsub_rn(L.Ps, P0));
         const float Q1 = Q0 + __fmaf_rn(qb.w, c1, __fsub_rn(P0, P1));
-        nR = add2(nR, sub2(pk(Q0, Q1), pk1(L.Ils)));
+        nR = add2(nR, pk(Q0, Q1));
         L.Qs = Q1;
     } else {
         nR = clamp_nR(nR, Tn, pk1(nsmax));
@@ -433,7 +438,7 @@ __device__ __forceinline__ void refresh_frozen(BwdLane<COMP> &L, float2 *sF, flo
         if (c < nchan) {
             const float T = L.sT[c], Gc = __ldg(L.Gin + c);
             float nr = L.sP[c] - __ldg(L.Isave + c);
-            if (COMP) nr += L.sQ[c] - __ldg(L.Ilo + c);
+            if (COMP) nr += L.sQ[c];
             else nr = fminf(fmaxf(nr, T * nsmax), 0.f);       // same clamp as clamp_nR
             sF[c] = make_float2(Gc * T, Gc * nr);
         }
@@ -444,14 +449,28 @@ __device__ __forceinline__ void refresh_frozen(BwdLane<COMP> &L, float2 *sF, flo
 __device__ __forceinline__ float z_slice_sum(float u0, float dvA, float Ss, int cref, int c0, int c1, int q, int stride,
                                              const float2 *__restrict__ sF)
 {
-    float cf = (float)(c0 + q - cref), acc = 0.f;
-    const float df = (float)stride;
-    for (int c = c0 + q; c <= c1; c += stride) {
-        const float u = fmaf(cf, dvA, u0);
-        const float g = ex2_approx(-u * u);
+    // two channels (c, c + stride) per trip in packed f32x2 arithmetic; an odd last channel on its own
+    int c = c0 + q;
+    const float cf0 = (float)(c - cref), df = (float)stride;
+    f2 cf2 = pk(cf0, cf0 + df), acc2 = pk1(0.f);
+    const f2 d2 = pk1(2.0f * df), dvA2 = pk1(dvA), u02 = pk1(u0), S2 = pk1(Ss);
+    for (; c + stride <= c1; c += 2 * stride) {
+        const f2 u = fma2(cf2, dvA2, u02);
+        float t0, t1;
+        upk(mul2(u, u), t0, t1);
+        const float2 fa = sF[c], fb = sF[c + stride];
+        acc2 = fma2(fma2(pk(fa.x, fb.x), S2, pk(fa.y, fb.y)), pk(ex2_approx(-t0), ex2_approx(-t1)), acc2);
+        cf2 = add2(cf2, d2);
+    }
+    float a0, a1;
+    upk(acc2, a0, a1);
+    float acc = a0 + a1;
+    if (c <= c1) {
+        float cfl, dummy;
+        upk(cf2, cfl, dummy);
+        const float u = fmaf(cfl, dvA, u0);
         const float2 f = sF[c];
-        acc = fmaf(fmaf(f.x, Ss, f.y), g, acc);
-        cf += df;
+        acc = fmaf(fmaf(f.x, Ss, f.y), ex2_approx(-u * u), acc);
     }
     return acc;
 }
@@ -539,17 +558,16 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
     BwdLane<COMP> L;
     L.sT = reinterpret_cast<float *>(base + sizeof(BwdShared)); L.sP = L.sT + 32 * ng; L.sQ = L.sP + 32 * ng;
     float2 *sF = reinterpret_cast<float2 *>(L.sP + (COMP ? 64 : 32) * ng);
-    L.Ilo = P.cube_lo + rc.ray * (size_t)nchan;
     L.Isave = P.cube + rc.ray * (size_t)nchan;
     L.Gin = P.dl_dcube + rc.ray * (size_t)nchan;
     bool anyg = false;
     for (int g = 0; g < ng; ++g) {
         const int c = lane + 32 * g;
         L.sT[c] = 1.f; L.sP[c] = 0.f;
-        if (COMP) L.sQ[c] = 0.f;
+        if (COMP) L.sQ[c] = c < nchan ? -__ldg(P.cube_lo + rc.ray * (size_t)nchan + c) : 0.f;
         anyg |= c < nchan && __ldg(L.Gin + c) != 0.f;
     }
-    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.cf = 0.f; L.Qs = 0.f; L.Ils = 0.f; L.cur = NO_GROUP; L.myc = -1;
+    L.Ts = 1.f; L.Ps = 0.f; L.Is = 0.f; L.Gs = 0.f; L.cf = 0.f; L.Qs = 0.f; L.cur = NO_GROUP; L.myc = -1;
     if (!__any_sync(FULL, anyg)) return;     // dL/dcube vanishes on this ray: no gradient
     const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
@@ -620,8 +638,8 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
                     for (int jj = 0; jj < nb; ++jj) {
                         const int i = base_i + jj;
                         const float4 qa = S.a[i], qb = S.b[i], qc = S.c[i];
-                        const int ulo = __float_as_int(qc.z), uhi = __float_as_int(qc.w);
-                        if (group_misses(L.cur, ulo, uhi)) L.regroup(group_for(ulo, uhi), lane, nchan);
+                        const int ulo = __float_as_int(qc.z), lim = __float_as_int(qc.w);
+                        if (group_misses(L.cur, ulo, lim)) L.regroup(group_for(ulo, lim), lane, nchan);
                         bwd_pair_e<COMP>(qa, qb, qc, L, nsmax, red_lane + jj * (4 * RED_ROW_BYTES));
                     }
                     n_mufu += 4 * nb;
