@@ -12,8 +12,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libradt.so")
-SOURCES = ["radt_api.cu", "radt_setup.cu", "radt_march.cu", "radt_march_win.cu", "radt_microbench.cu", "radt_disk.cu", "radt_mlp.cu", "radt_mlp_tc.cu"]
-HEADERS = ["radt_dev.cuh", "radt_kernels.h", "radt_march.cuh", os.path.join("..", "..", "include", "radt.h")]
+SOURCES = ["radt_api.cu", "radt_setup.cu", "radt_march.cu", "radt_march_win.cu", "radt_microbench.cu", "radt_disk.cu", "radt_mlp_tc.cu", "radt_mlp_tc_bwd.cu"]
+HEADERS = ["radt_dev.cuh", "radt_kernels.h", "radt_march.cuh", "radt_tc.cuh", os.path.join("..", "..", "include", "radt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

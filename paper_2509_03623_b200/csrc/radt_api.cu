@@ -896,7 +896,7 @@ int radt_disk_fields_bwd(const radt_disk *disk, const radt_grid *grid, int32_t b
 }
 
 // ------------------------------------------------------------------------------------------
-// MLP temperature field (radt_mlp.cu)
+// MLP temperature field (radt_mlp_tc.cu, radt_mlp_tc_bwd.cu)
 // ------------------------------------------------------------------------------------------
 static int mlp_check(const radt_mlp *mlp, const radt_grid *grid, long long *count)
 {

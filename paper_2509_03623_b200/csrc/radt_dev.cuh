@@ -168,7 +168,7 @@ struct DiskParamsDev {
     unsigned char *mask;                 // workspace, [batch][nr][nz]
 };
 
-// ---- MLP temperature field (radt_mlp.cu) ----
+// ---- MLP temperature field (radt_mlp_tc.cu, radt_mlp_tc_bwd.cu) ----
 struct MlpParamsDev {
     int nr, nz, L, nparams;
     float t_lo, t_hi;
