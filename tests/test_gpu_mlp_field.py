@@ -49,6 +49,31 @@ def test_mlp_adjoint_matches_oracle(cfg, L, seed):
     assert np.linalg.norm(got - want) <= 1e-4 * np.linalg.norm(want)
 
 
+@pytest.mark.parametrize("nr,nz,L", [(9, 7, 4), (37, 11, 4), (50, 30, 8), (129, 2, 0)])
+def test_mlp_ragged_node_counts(nr, nz, L):
+    """Node counts that are not a multiple of the 128-node tensor-core tile (63, 407, 1500, 258 nodes): the last tile of the
+    forward and of the adjoint is partly empty; its padding rows must neither show in T nor reach the parameter gradients."""
+    from paper_2509_03623_b200 import binding as B
+    from synth import tiny_axisym_scene
+    B.lib()
+    desc = B.Descriptors([tiny_axisym_scene(seed=5, nr=nr, nz=nz)])
+    assert desc.grid_shape == (nr, nz)
+    mlp = B.make_mlp(L=L)
+    p = 3.0 * mf.init_params(L, 100 + nr)
+    T = torch.full((nr, nz), -1.0, dtype=torch.float32, device="cuda")
+    B.radt_mlp_temperature(mlp, desc, torch.from_numpy(p).cuda(), T)
+    want = mf.forward(p, nr, nz, L)
+    assert np.max(np.abs(T.cpu().numpy() - want)) <= 1e-5 * 395.0
+    gT = np.random.default_rng(nr).standard_normal((nr, nz)).astype(np.float32)
+    gT[mf.near_kink(p, nr, nz, L)] = 0.0
+    gp = torch.full((mf.n_params(L),), 7.0, dtype=torch.float32, device="cuda")
+    B.radt_mlp_temperature_bwd(mlp, desc, torch.from_numpy(p).cuda(), torch.from_numpy(gT).cuda(), gp)
+    wantg = mf.adjoint(p, gT, nr, nz, L)
+    got = gp.cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(got - wantg)) <= 1e-3 * np.abs(wantg).max()
+    assert np.linalg.norm(got - wantg) <= 1e-4 * np.linalg.norm(wantg)
+
+
 def test_neural_field_fit_reduces_the_loss():
     """The paper's chain end to end on the GPU (Fig. 2): parameters -> MLP T grid -> physics pre-pass -> render ->
     chi^2 -> adjoints back to the parameters; a few plain gradient steps towards a target cube rendered from a known
