@@ -14,6 +14,7 @@
 #define RADT_MAXB 16                  // batch items per launch (geometry travels in kernel params)
 #define RADT_NQ 4096                  // partition-function table intervals over log2 T in [0, 14]
 #define RADT_NQ_OCTAVES 14.0f
+#define RADT_TMAX 16384.0f             // upper end of that table: temperatures above it are clamped (zero gradient)
 #define RADT_MAXLEV 64
 #define RADT_MAXCHAN 256
 #define RADT_LOSS_SLOTS 1024           // partial sums of the fused chi^2 loss

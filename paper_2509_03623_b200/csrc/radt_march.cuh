@@ -178,8 +178,9 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
     // when the grid stores n itself (LINEAR) and vanishes with n when it stores ln n
     if ((FWD || g.dens_mode == 1 || !P.opt_zero_grad) && P.opt_skip_empty && !(n > N_EMPTY)) return;
     st.inside = true;
-    bool tcl = !(temp >= 1.0f);
-    float T = tcl ? 1.0f : temp;
+    // T is clamped to [1 K, RADT_TMAX] (the range of the Q(T) table, include/radt.h); no gradient through either clamp
+    bool tcl = !(temp >= 1.0f) || temp > RADT_TMAX;
+    float T = tcl ? (temp > RADT_TMAX ? RADT_TMAX : 1.0f) : temp;
     float invT = rcp_approx(T);
     float xx = L.T0 * invT;
     float ex = ex2_approx(L.T0l2 * invT);

@@ -371,6 +371,23 @@ def test_zero_density_and_clamped_temperature(rt):
     assert not R.g_temp.any()
 
 
+def test_temperature_above_the_table_is_clamped(rt):
+    """include/radt.h: temperatures above 16384 K (the end of the device Q(T) table) are clamped there in EVERY use (S, alpha,
+    Boltzmann factor, Q) with zero gradient; the render of a 20000 K slab equals the oracle's render of a 16384 K slab."""
+    kw = dict(n_co=0.5, vchan_cms=[0.0, 2.0e5, -4.0e5], nstep=4, npix=2)
+    hot, ref_sc = slab_scene(temp=20000.0, **kw), slab_scene(temp=16384.0, **kw)
+    R = _gpu_forward(rt, hot, need_bwd=True)
+    ref = _oracle_cube([ref_sc])
+    assert ref.max() > 0
+    check_cube("clamped hot slab", R.cube.cpu().numpy(), ref)
+    G32 = np.full(ref.shape, 1e-3, np.float32)
+    R.dl_dcube.copy_(torch.from_numpy(G32))
+    gd, gt, gv = (g.cpu().numpy() for g in R.render_bwd())
+    rd, _, rv = po.render_bwd(ref_sc, G32[0].astype(np.float64))
+    check_grad("clamped hot slab g_dens", gd[0], rd)
+    assert not gt.any()
+
+
 def test_max_channels_and_odd_image(rt):
     sc = tiny_axisym_scene(seed=61, nchan=256, npix=5, npix_y=3, nstep=40)
     _parity_fwd_bwd(rt, sc, "256 channels")
