@@ -17,7 +17,9 @@ With N > 1 every rank renders its own disks (independent problems, no data-path 
 in HBM; L2 flushed between steps outside the timed events).  `e2e` = the same step through the HOST-buffer C-ABI entry point
 radt_fit_step_host (pinned host buffers, copies inside the timed region); `e2e_render` = radt_render_host (cube D2H inside).
 `roofline` = the dominant kernel against the issue peak measured in this run: `frac` counts EXECUTED
-samples only; `speedup_from_skipping` = nominal / executed samples (an algorithmic saving, not pipe efficiency).
+samples only; `speedup_from_skipping` = nominal / executed samples (an algorithmic saving, not pipe efficiency);
+`executed_samples.fwd_in_window_over_executed` = the share of executed (channel, step) samples that lie inside their step's line
+window, i.e. of the 32 lanes that can contribute (useful over executed work).
 `cpu_baseline` = the fp64 oracle, as it stands, on this box's host cores, on a bounded ray sample of the headline workload.
 """
 from __future__ import annotations
@@ -339,6 +341,7 @@ def measure_config(cfg, args, ctx, with_cpu):
     reps = max(3, min(args.steps, 20 if nominal < 1e11 else 5))
     t_fwd = time_kernel_group(lambda: R.render(stream), stream, torch, flush, reps)
     cnt = R.counters()
+    lanes = R.lane_counters()          # (samples inside their step's line window, samples executed) of that forward
     t_fl = time_kernel_group(lambda: R.render_loss(stream), stream, torch, flush, reps)
     t_l2 = time_kernel_group(lambda: R.l2_loss_grad(stream), stream, torch, flush, reps)
     R.render_loss(stream)
@@ -424,7 +427,9 @@ def measure_config(cfg, args, ctx, with_cpu):
         "bwd_ms_zero_dens_grad_off": t_bwd_fit, "step_ms_without_cube_lo": t_plain,
         "executed_samples": {"fwd": int(fwd_exec), "bwd": int(bwd_exec), "fwd_active_ray_steps": int(cnt[0]),
                              "bwd_active_ray_steps": int(cnt_b[2]), "nominal": int(nominal),
-                             "fwd_executed_over_nominal": fwd_exec / nominal},
+                             "fwd_executed_over_nominal": fwd_exec / nominal,
+                             "fwd_in_window": int(lanes[0]) if lanes[0] else None,
+                             "fwd_in_window_over_executed": (lanes[0] / max(lanes[1], 1)) if lanes[0] else None},
         "roofline": dominant, "roofline_other": other,
         "e2e": {"value": nominal / e2e_t, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "ms_per_step": 1e3 * e2e_t, "steps": e2e_steps, "api": "radt_fit_step_host (pinned host buffers)"},

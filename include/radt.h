@@ -290,6 +290,10 @@ int radt_pipe_peak(int32_t kind, double *ops_per_s_out, double *sm_clock_mhz_out
  * lane-operations spent on (channel, step) samples), adjoint active ray-steps, adjoint per-sample MUFU.EX2 warp
  * instructions}.  Synchronises cuda_stream. */
 int radt_read_counters(const void *ws, uint64_t *out4, void *cuda_stream);
+/* Lane use of the last FORWARD march on workspace `ws` (window kernels; executed work is reported beside
+ * nominal work): out2 (HOST) = {(channel, step) samples inside the line window of their step, i.e. samples that can contribute;
+ * samples executed = 32 lanes x emitting steps}.  The channel-table kernels leave the first figure 0.  Synchronises cuda_stream. */
+int radt_read_lane_counters(const void *ws, uint64_t *out2, void *cuda_stream);
 
 /* Counters of the last radt_render / radt_render_bwd call on this thread (HOST): number of kernel
  * launches enqueued. */

@@ -22,7 +22,7 @@ EXPORTS = ["radt_version", "radt_last_error", "radt_options_default", "radt_work
            "radt_l2_loss_grad", "radt_render_host",
            "radt_render_loss", "radt_disk_workspace_bytes", "radt_disk_fields", "radt_disk_fields_bwd",
            "radt_mlp_num_params", "radt_mlp_temperature", "radt_mlp_temperature_bwd",
-           "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters",
+           "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters", "radt_read_lane_counters",
            "radt_last_launch_count"]
 
 
@@ -133,6 +133,7 @@ def lib():
         L.radt_render_bwd_host.argtypes = [gp, lp, rp, i32, op, vp, vp, vp, vp, vp, vp]
         L.radt_pipe_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
         L.radt_read_counters.argtypes = [vp, C.POINTER(C.c_uint64), vp]
+        L.radt_read_lane_counters.argtypes = [vp, C.POINTER(C.c_uint64), vp]
         L.radt_last_launch_count.restype = C.c_int
         _lib = L
     return _lib
@@ -328,6 +329,14 @@ def radt_read_counters(ws, stream=None):
     with _on(ws):
         _check(lib().radt_read_counters(_p(ws), out, _stream_ptr(stream, ws)))
     return [int(x) for x in out]
+
+
+def radt_read_lane_counters(ws, stream=None):
+    """(samples inside their line window, samples executed) of the last forward march on `ws`."""
+    out = (C.c_uint64 * 2)()
+    with _on(ws):
+        _check(lib().radt_read_lane_counters(_p(ws), out, _stream_ptr(stream, ws)))
+    return int(out[0]), int(out[1])
 
 
 def radt_last_launch_count() -> int:

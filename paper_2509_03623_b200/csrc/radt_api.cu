@@ -428,7 +428,8 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         }
     }
 
-    // counters: 0-3 work counters, 4 the grid's maximum temperature (setup), 8.. loss slots (forward)
+    // counters: 0-3 work counters, 4 forward in-window samples, 7 the grid's maximum temperature (setup), 8.. loss slots
+    // (forward); an adjoint that reuses the forward's setup keeps 4.. (the forward's figures stay readable)
     CUDA_TRY(cudaMemsetAsync(dws.counters, 0, reuse ? 4 * sizeof(unsigned long long) : w.zero_bytes, st));
     if (reuse) CUDA_TRY(cudaMemsetAsync(dws.grad, 0, (size_t)grid_cells(grid) * (size_t)batch * sizeof(float4), st));
     for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
@@ -628,6 +629,17 @@ int radt_read_counters(const void *ws, uint64_t *out4, void *cuda_stream)
     if (!ws || !out4) return fail(RADT_E_INVALID, "null pointer");
     CUDA_TRY(cudaMemcpyAsync(out4, ws, 4 * sizeof(uint64_t), cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
     CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    return RADT_OK;
+}
+
+int radt_read_lane_counters(const void *ws, uint64_t *out2, void *cuda_stream)
+{
+    if (!ws || !out2) return fail(RADT_E_INVALID, "null pointer");
+    uint64_t c[5];
+    CUDA_TRY(cudaMemcpyAsync(c, ws, 5 * sizeof(uint64_t), cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+    out2[0] = c[RADT_CNT_USEFUL];
+    out2[1] = 32 * c[1] / 2;          // 2 MUFU.EX2 lane-operations per executed sample
     return RADT_OK;
 }
 

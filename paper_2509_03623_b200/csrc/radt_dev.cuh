@@ -18,6 +18,8 @@
 #define RADT_MAXLEV 64
 #define RADT_MAXCHAN 256
 #define RADT_LOSS_SLOTS 1024           // partial sums of the fused chi^2 loss
+#define RADT_CNT_USEFUL 4              // workspace counter: forward (channel, step) samples inside their line window
+#define RADT_CNT_TMAX 7                // workspace counter slot holding the bits of the grid's maximum temperature
 
 #define RADT_LOG2E 1.4426950408889634f
 #define RADT_LN2 0.6931471805599453f
@@ -98,8 +100,8 @@ struct DevWs {
                            // 3-D: one bit per block of 4 x 4 x 4 cells, same dilation; spherical: bit (radial cell,
                            // bin of cos theta), any phi (radt_setup.cu)
     unsigned *nodeflag;    // spherical: [batch][nr][ceil(ntheta / 32)] bit j of row i: some phi node of (i, j) can emit
-    unsigned long long *counters;   // [8 + RADT_LOSS_SLOTS] 0-3 work counters; [4] bits of the grid's maximum
-                                    // temperature; [8..] partial sums of the fused loss (double)
+    unsigned long long *counters;   // [8 + RADT_LOSS_SLOTS] 0-3 work counters; [4] forward samples inside their line window;
+                                    // [7] bits of the grid's maximum temperature; [8..] partial sums of the fused loss (double)
 };
 
 struct MarchParams {

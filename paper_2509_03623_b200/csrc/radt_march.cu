@@ -277,7 +277,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, (COMP && NP == 4) ? 4
     const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     float4 *grad = P.ws.grad + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     // upper bound of the source function anywhere on the grid (S grows with T)
-    const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + 4)), 1.0f);
+    const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + RADT_CNT_TMAX)), 1.0f);
     const float nsmax = -G.sunit * 1.0001f / (ex2_approx(L.T0l2 / tmax) - 1.0f);
     const float kthr = P.opt_skip_empty ? K2_EMPTY : 0.f;    // the forward's own test for an emitting step
     const bool window = P.opt_window;

@@ -271,7 +271,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
     LaneState<COMP> L;
     L.init(sI, sT, lane, ng);
     if (P.target) loss_prefetch(P, rc.ray * (size_t)nchan, nchan, lane);
-    unsigned n_steps = 0, n_mufu = 0;
+    unsigned n_steps = 0, n_mufu = 0, n_useful = 0;
     if (rc.ds != 0.0) {
         const float4 *cells = P.ws.cells + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
         const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
@@ -287,6 +287,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
             phase_a<KIND, true, true>(P, G, cells, S.ray[0], S.ray[1], S.ray[2], S.ray[3], S.ray[4], k, st);
             const bool act = st.inside && (st.K2 > K2_EMPTY || !P.opt_skip_empty) && st.whi >= 0 && st.wlo < nchan;
             n_steps += __popc(__ballot_sync(FULL, act));
+            n_useful += __reduce_add_sync(FULL, act ? min(st.whi, nchan - 1) - max(st.wlo, 0) + 1 : 0);
             bool wide;
             int pos;
             int npairs = write_entries(S, lane, act, -1, st, st.K2, wide, pos);
@@ -325,6 +326,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_FWD) k_
     if (lane == 0 && n_steps) {
         atomicAdd(P.ws.counters + 0, (unsigned long long)n_steps);
         atomicAdd(P.ws.counters + 1, (unsigned long long)n_mufu);
+        atomicAdd(P.ws.counters + RADT_CNT_USEFUL, (unsigned long long)n_useful);
     }
 }
 
@@ -573,7 +575,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, RADT_WIN_MINB_BWD) k_
     const unsigned *occ = P.ws.occ + (size_t)(P.b0 + rc.b) * (size_t)P.occ_words;
     float4 *grad = P.ws.grad + (size_t)(P.b0 + rc.b) * (size_t)P.grid.cells;
     // upper bound of the source function anywhere on the grid (S grows with T)
-    const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + 4)), 1.0f);
+    const float tmax = fmaxf(__int_as_float(*reinterpret_cast<const int *>(P.ws.counters + RADT_CNT_TMAX)), 1.0f);
     const float nsmax = -G.sunit * 1.0001f / (ex2_approx(Ln.T0l2 / tmax) - 1.0f);
     const float kthr = P.opt_skip_empty ? K2_EMPTY : 0.f;    // the forward's own test for an emitting step
     const bool zsteps = P.grid.dens_mode == 0 && P.opt_zero_grad;      // zero-opacity steps carry dL/dn (LINEAR grids)

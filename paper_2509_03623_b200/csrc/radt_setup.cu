@@ -229,10 +229,10 @@ __global__ void __launch_bounds__(256) k_setup(const __grid_constant__ SetupPara
             P.ws.grad[dst] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
     }
-    // grid-wide maximum temperature (bounds the source function in the adjoint); counters[4] holds its bits
+    // grid-wide maximum temperature (bounds the source function in the adjoint); counters[RADT_CNT_TMAX] holds its bits
 #pragma unroll
     for (int m = 16; m > 0; m >>= 1) tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, m));
-    if ((threadIdx.x & 31) == 0 && tmax > 0.f) atomicMax(reinterpret_cast<int *>(P.ws.counters + 4), __float_as_int(tmax));
+    if ((threadIdx.x & 31) == 0 && tmax > 0.f) atomicMax(reinterpret_cast<int *>(P.ws.counters + RADT_CNT_TMAX), __float_as_int(tmax));
 }
 
 // Spherical occupancy words from the (i, j) node flags (second launch: needs every flag).  The prefilter locates a step in

@@ -103,6 +103,9 @@ class Renderer:
     def counters(self):
         return B.radt_read_counters(self.ws)
 
+    def lane_counters(self):
+        return B.radt_read_lane_counters(self.ws)
+
     def ray_table(self):
         d = self.desc
         rays = self.torch.empty((d.batch, d.ny, d.nx, 2), dtype=self.torch.float64, device=self.device)

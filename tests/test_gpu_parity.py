@@ -540,6 +540,19 @@ def test_renderer_on_a_device_that_is_not_current(rt):
     assert torch.cuda.current_device() == 0
 
 
+def test_lane_counters(rt):
+    """radt_read_lane_counters: in-window samples <= executed samples = 32 x emitting steps (window kernels); the channel-table
+    kernels leave the first figure 0."""
+    R = _gpu_forward(rt, make_config(1))
+    steps, mufu = R.counters()[:2]
+    useful, executed = R.lane_counters()
+    assert executed == 32 * mufu // 2 and executed >= 32 * steps
+    if rt.options.get("win_path", 1):
+        assert 0 < useful <= executed
+    else:
+        assert useful == 0
+
+
 def test_pipe_peaks_are_sane(rt):
     ops, clk = rt.binding.radt_pipe_peak(0)
     assert 1000 < clk < 2200
