@@ -7,8 +7,10 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
+#include <vector>
 
 namespace {
 
@@ -340,6 +342,7 @@ struct LossArgs {
     float *dl_out = nullptr;
     double *loss = nullptr;
     double sigma = 0.0;
+    double nvox_total = 0.0;      // > 0: the call renders a chunk of a larger batch; normalise with the whole batch's voxel count
 };
 
 // What shapes the partial sums of a cube (a forward and its adjoint must agree on it) ...
@@ -481,7 +484,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
             }
         MP.cube = cube; MP.cube_lo = cube_lo; MP.dl_dcube = dl_dcube;
         if (pass == RADT_PASS_FWD && loss.target) {
-            const double nvox = (double)batch * geom[0].nx * geom[0].ny * line->nchan;
+            const double nvox = loss.nvox_total > 0 ? loss.nvox_total : (double)batch * geom[0].nx * geom[0].ny * line->nchan;
             const double inv = 1.0 / (loss.sigma * loss.sigma * nvox);
             MP.target = loss.target; MP.dl_out = loss.dl_out;
             MP.inv_s2n = (float)inv;
@@ -494,7 +497,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         ++g_launches;
     }
     if (pass == RADT_PASS_FWD && loss.target) {
-        const double nvox = (double)batch * geom[0].nx * geom[0].ny * line->nchan;
+        const double nvox = loss.nvox_total > 0 ? loss.nvox_total : (double)batch * geom[0].nx * geom[0].ny * line->nchan;
         CUDA_TRY(radt_launch_loss_finish(reinterpret_cast<double *>(dws.counters + 8),
                                          0.5 / (loss.sigma * loss.sigma * nvox), loss.loss, st));
         ++g_launches;
@@ -737,6 +740,111 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
     radt_options ob;
     radt_options_default(&ob);
     if (opt) ob = *opt;
+    // Batched calls (config 5: 16 items, 2.1 GB of target and of cube) run item chunk by item chunk so that PCIe and the SMs
+    // work at the same time: fit step = the upload of chunk c + 1's target under the forward and adjoint of chunk c (and the
+    // chi^2 term FUSED into each chunk's forward, which only waits for its own chunk's upload); render = the download of chunk
+    // c's cube under the march of chunk c + 1.  Results are those of the one-call path (items are independent; the loss is the
+    // sum of the chunks' shares).
+    const size_t item_vox = (size_t)geom[0].nx * geom[0].ny * line->nchan;
+    int chunk = batch;
+    if (batch > 1 && mode != 2) {
+        const size_t per = item_vox * sizeof(float);
+        chunk = (int)(((size_t)32 << 20) / per);
+        if (chunk < 1) chunk = 1;
+        if (chunk > batch) chunk = batch;
+        if ((batch + chunk - 1) / chunk > 256) chunk = (batch + 255) / 256;
+        // test hook: RADT_HOST_CHUNK_ITEMS = n forces chunks of n items (tests/test_gpu_parity.py runs the chunked path on small scenes)
+        if (const char *e = getenv("RADT_HOST_CHUNK_ITEMS")) {
+            const int n = atoi(e);
+            if (n >= 1) chunk = n < batch ? n : batch;
+        }
+    }
+    if (chunk < batch) {
+        static thread_local std::vector<cudaEvent_t> evs;
+        const int nchunks = (batch + chunk - 1) / chunk;
+        if (!s2) {
+            CUDA_TRY(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+            CUDA_TRY(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&ev_copied, cudaEventDisableTiming));
+        }
+        while ((int)evs.size() < nchunks) {
+            cudaEvent_t e;
+            CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            evs.push_back(e);
+        }
+        auto chunk_grid = [&](int b0) {
+            radt_grid g = dgrid;
+            g.dens = d_dens + (size_t)b0 * stride; g.temp = d_temp + (size_t)b0 * stride; g.vel = d_vel + (size_t)b0 * stride;
+            return g;
+        };
+        CUDA_TRY(cudaEventRecord(ev_alloc, B.st));          // (the arena is ours from here on; the fields are on their way)
+        CUDA_TRY(cudaStreamWaitEvent(s2, ev_alloc, 0));
+        if (mode == 0) {
+            for (int c = 0; c < nchunks; ++c) {
+                const int b0 = c * chunk, nb = batch - b0 < chunk ? batch - b0 : chunk;
+                const size_t off = (size_t)b0 * item_vox, nby = (size_t)nb * item_vox * sizeof(float);
+                radt_grid g = chunk_grid(b0);
+                rc = radt_render(geom + b0, line, &g, nb, opt, d_cube + off, d_lo ? d_lo + off : nullptr, ws, wsb, B.st);
+                if (rc) { cudaStreamSynchronize(s2); return rc; }
+                launches += g_launches;
+                CUDA_TRY(cudaEventRecord(evs[c], B.st));
+                CUDA_TRY(cudaStreamWaitEvent(s2, evs[c], 0));
+                CUDA_TRY(cudaMemcpyAsync(cube + off, d_cube + off, nby, cudaMemcpyDeviceToHost, s2));
+                if (cube_lo) CUDA_TRY(cudaMemcpyAsync(cube_lo + off, d_lo + off, nby, cudaMemcpyDeviceToHost, s2));
+            }
+            CUDA_TRY(cudaStreamSynchronize(B.st));
+            CUDA_TRY(cudaStreamSynchronize(s2));
+            g_launches = launches;
+            return RADT_OK;
+        }
+        // mode 1
+        if (!target) return fail(RADT_E_INVALID, "null target");
+        float *d_t = (float *)B.alloc(nvox * sizeof(float));
+        double *d_loss = (double *)B.alloc(sizeof(double) * (size_t)nchunks);
+        float *d_g[3] = { nullptr, nullptr, nullptr };
+        float *h_g[3] = { g_dens, g_temp, g_vel };
+        for (int i = 0; i < 3; ++i)
+            if (h_g[i] && !(d_g[i] = (float *)B.alloc(fbytes))) return fail(RADT_E_CUDA, "device allocation failed");
+        if (!d_t || !d_loss) return fail(RADT_E_CUDA, "device allocation failed");
+        for (int c = 0; c < nchunks; ++c) {
+            const int b0 = c * chunk, nb = batch - b0 < chunk ? batch - b0 : chunk;
+            const size_t off = (size_t)b0 * item_vox;
+            CUDA_TRY(cudaMemcpyAsync(d_t + off, target + off, (size_t)nb * item_vox * sizeof(float), cudaMemcpyHostToDevice, s2));
+            CUDA_TRY(cudaEventRecord(evs[c], s2));
+        }
+        ob.reuse_setup = 1;
+        for (int c = 0; c < nchunks; ++c) {
+            const int b0 = c * chunk, nb = batch - b0 < chunk ? batch - b0 : chunk;
+            const size_t off = (size_t)b0 * item_vox;
+            radt_grid g = chunk_grid(b0);
+            CUDA_TRY(cudaStreamWaitEvent(B.st, evs[c], 0));
+            LossArgs la;
+            la.target = d_t + off; la.dl_out = d_dl + off; la.loss = d_loss + c; la.sigma = sigma; la.nvox_total = (double)nvox;
+            rc = run_pass(geom + b0, line, &g, nb, opt, RADT_PASS_FWD, d_cube + off, d_lo + off, nullptr, nullptr, nullptr, nullptr,
+                          ws, wsb, B.st, la);
+            if (rc) { cudaStreamSynchronize(s2); return rc; }
+            launches += g_launches;
+            rc = radt_render_bwd(geom + b0, line, &g, nb, &ob, d_cube + off, d_lo + off, d_dl + off,
+                                 d_g[0] ? d_g[0] + (size_t)b0 * stride : nullptr, d_g[1] ? d_g[1] + (size_t)b0 * stride : nullptr,
+                                 d_g[2] ? d_g[2] + (size_t)b0 * stride : nullptr, ws, wsb, B.st);
+            if (rc) { cudaStreamSynchronize(s2); return rc; }
+            launches += g_launches;
+        }
+        std::vector<double> parts((size_t)nchunks, 0.0);
+        if (loss_out) CUDA_TRY(cudaMemcpyAsync(parts.data(), d_loss, sizeof(double) * (size_t)nchunks, cudaMemcpyDeviceToHost, B.st));
+        if (cube) CUDA_TRY(cudaMemcpyAsync(cube, d_cube, nvox * sizeof(float), cudaMemcpyDeviceToHost, B.st));
+        for (int i = 0; i < 3; ++i)
+            if (h_g[i]) CUDA_TRY(cudaMemcpyAsync(h_g[i], d_g[i], fbytes, cudaMemcpyDeviceToHost, B.st));
+        CUDA_TRY(cudaStreamSynchronize(B.st));
+        CUDA_TRY(cudaStreamSynchronize(s2));
+        if (loss_out) {
+            double acc = 0.0;
+            for (double v : parts) acc += v;
+            *loss_out = acc;
+        }
+        g_launches = launches;
+        return RADT_OK;
+    }
     if (mode == 0) {
         rc = radt_render(geom, line, &dgrid, batch, opt, d_cube, d_lo, ws, wsb, B.st);
         if (rc) return rc;

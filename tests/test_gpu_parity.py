@@ -425,6 +425,42 @@ def test_host_entry_points(rt):
     check_grad("host3 g_dens", gd2[0], rd); check_grad("host3 g_temp", gt2[0], rtm); check_grad("host3 g_vel", gv2[0], rv)
 
 
+@pytest.mark.parametrize("chunk", [1, 2])
+def test_host_entry_points_in_item_chunks(rt, chunk, monkeypatch):
+    """Batched HOST calls run item chunk by item chunk (PCIe transfers under the marches, chi^2 term fused into each chunk's
+    forward); RADT_HOST_CHUNK_ITEMS forces that path on a small batch.  Same cube bit for bit, same loss and gradients as the
+    one-call path."""
+    B = rt.binding
+    scs = make_config(5, npix=16, batch=3)
+    d = B.Descriptors(scs)
+    h = B.stack_fields(scs)
+    ref = _oracle_cube(scs)
+    tgt32 = np.ascontiguousarray(np.stack([l2_target(ref[b], 40 + b)[0] for b in range(3)]), np.float32)
+    sigma = 0.02 * float(ref.max())
+
+    def run():
+        cube, lo = np.zeros(d.cube_shape, np.float32), np.zeros(d.cube_shape, np.float32)
+        B.radt_render_host(d, *h, cube, rt.opt(), lo)
+        g = [np.zeros_like(h[0]) for _ in range(3)]
+        cube2 = np.zeros_like(cube)
+        loss = B.radt_fit_step_host(d, *h, tgt32, sigma, cube2, *g, rt.opt())
+        return cube, lo, cube2, loss, g
+
+    monkeypatch.delenv("RADT_HOST_CHUNK_ITEMS", raising=False)
+    c0, l0, c20, loss0, g0 = run()
+    monkeypatch.setenv("RADT_HOST_CHUNK_ITEMS", str(chunk))
+    c1, l1, c21, loss1, g1 = run()
+    check_cube("chunked host cube", c1, ref)
+    np.testing.assert_array_equal(c0, c1); np.testing.assert_array_equal(l0, l1); np.testing.assert_array_equal(c20, c21)
+    np.testing.assert_array_equal(c1, c21)
+    assert loss1 == pytest.approx(loss0, rel=1e-12)
+    res = c1.astype(np.float64) - tgt32
+    assert loss1 == pytest.approx(0.5 * np.mean((res / sigma) ** 2), rel=1e-6)
+    for a, b in zip(g0, g1):
+        assert np.abs(a).max() > 0
+        np.testing.assert_allclose(b, a, rtol=1e-4, atol=1e-6 * np.abs(a).max())
+
+
 def test_l2_loss_kernel(rt):
     R = rt.Renderer([make_config(1)])
     R.render()
