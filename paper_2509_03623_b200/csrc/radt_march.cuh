@@ -346,9 +346,9 @@ __device__ __forceinline__ bool ray_setup(const MarchParams &P, RayCtx &rc, int 
     // Tiles are issued from the image centre outwards (rows, and tiles within a row, alternate around the centre):
     // rays through the disk centre carry the most steps, the empty corners fill the tail of the launch
     // (measured on config 2: under 1 % either way; kept because the heavy tiles no longer depend on the PA).
-    int kx = blockIdx.x % P.tiles_x, ky = blockIdx.x / P.tiles_x;
+    const int kx = blockIdx.x, ky = blockIdx.y;        // grid = (tiles_x, tiles_y, batch chunk): no integer division per ray
     int tx = centre_out(kx, P.tiles_x), ty = centre_out(ky, P.tiles_y);
-    rc.b = blockIdx.y;
+    rc.b = blockIdx.z;
     rc.ix = tx * RADT_TILE_X + (warp & (RADT_TILE_X - 1));
     rc.iy = ty * RADT_TILE_Y + (warp / RADT_TILE_X);
     if (rc.ix >= P.nx || rc.iy >= P.ny) return false;
@@ -373,7 +373,7 @@ __device__ __forceinline__ void loss_report(const MarchParams &P, double acc, in
     for (int m = 16; m > 0; m >>= 1) acc += __shfl_xor_sync(FULL, acc, m);
     if (lane == 0 && acc != 0.0) {
         double *part = reinterpret_cast<double *>(P.ws.counters + 8);
-        const unsigned w = (blockIdx.y * gridDim.x + blockIdx.x) * RADT_WARPS_PER_CTA + (threadIdx.x >> 5);
+        const unsigned w = ((blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * RADT_WARPS_PER_CTA + (threadIdx.x >> 5);
         asm volatile("red.global.add.f64 [%0], %1;" ::"l"(part + (w & (RADT_LOSS_SLOTS - 1))), "d"(acc) : "memory");
     }
 }
