@@ -213,8 +213,9 @@ int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_gr
                      const radt_options *opt, float *cube, float *cube_lo);
 /* Forward + chi^2 term against `target` (HOST; uploaded on a second stream under the forward march) + adjoint in one
  * call; the low-order words stay on the device; cube may be NULL.  Batched calls (radt_fit_step_host and radt_render_host)
- * whose items are 32 MB of cube or more run item chunk by item chunk, the transfers of one chunk under the marches of
- * another; the results are those of the one-call path (cube bit for bit). */
+ * whose items are 32 MB of cube or more run item chunk by item chunk, and single images of 32 MB or more in bands of rows
+ * (one setup; per band the forward march and, in a fit step on axisymmetric grids, the adjoint march of the same rows), the
+ * transfers of one chunk / band under the marches of another; the results are those of the one-call path (cube bit for bit). */
 int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                        const radt_options *opt, const float *target, double sigma, float *cube, double *loss_out,
                        float *g_dens, float *g_temp, float *g_vel);

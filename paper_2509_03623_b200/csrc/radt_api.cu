@@ -345,6 +345,14 @@ struct LossArgs {
     double nvox_total = 0.0;      // > 0: the call renders a chunk of a larger batch; normalise with the whole batch's voxel count
 };
 
+// A row band of the image (HOST entry points: transfers of one band under the marches of another).  nty == 0: the whole image
+// in one launch.  Only the FIRST band of a pass runs the setup kernel and the zeroing, only the LAST one the loss reduction /
+// the gradient unpack; the bands of one pass share workspace, ray table and (adjoint) gradient cells.
+struct Band {
+    int ty0 = 0, nty = 0;
+    bool first = true, last = true;
+};
+
 // What shapes the partial sums of a cube (a forward and its adjoint must agree on it) ...
 unsigned long long cube_tag(const Opts &o, bool use_win, bool comp, const radt_geom *geom, const radt_line *line, int batch)
 {
@@ -372,7 +380,7 @@ unsigned long long setup_tag(const Opts &o, bool use_win, const radt_geom *geom,
 // Enqueue setup + march for all batch chunks.  pass 0: forward into `cube`; pass 1: adjoint.
 int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int batch, const radt_options *opt_in,
              int pass, float *cube, float *cube_lo, const float *dl_dcube, float *g_dens, float *g_temp, float *g_vel,
-             void *ws, size_t ws_bytes, cudaStream_t st, const LossArgs &loss = LossArgs())
+             void *ws, size_t ws_bytes, cudaStream_t st, const LossArgs &loss = LossArgs(), const Band &band = Band())
 {
     int rc = validate(geom, line, grid, batch);
     if (rc) return rc;
@@ -433,8 +441,10 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
 
     // counters: 0-3 work counters, 4 forward in-window samples, 7 the grid's maximum temperature (setup), 8.. loss slots
     // (forward); an adjoint that reuses the forward's setup keeps 4.. (the forward's figures stay readable)
-    CUDA_TRY(cudaMemsetAsync(dws.counters, 0, reuse ? 4 * sizeof(unsigned long long) : w.zero_bytes, st));
-    if (reuse) CUDA_TRY(cudaMemsetAsync(dws.grad, 0, (size_t)grid_cells(grid) * (size_t)batch * sizeof(float4), st));
+    if (band.first) {
+        CUDA_TRY(cudaMemsetAsync(dws.counters, 0, reuse ? 4 * sizeof(unsigned long long) : w.zero_bytes, st));
+        if (reuse) CUDA_TRY(cudaMemsetAsync(dws.grad, 0, (size_t)grid_cells(grid) * (size_t)batch * sizeof(float4), st));
+    }
     for (int b0 = 0; b0 < batch; b0 += RADT_MAXB) {
         int nb = batch - b0 < RADT_MAXB ? batch - b0 : RADT_MAXB;
         memset(&SP, 0, sizeof(SP));
@@ -457,7 +467,7 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         SP.do_occ = occ; SP.occ_words = w.occ_words; SP.occ_wpr = w.occ_wpr; SP.occ_nbj = w.occ_nbj; SP.flag_wpr = w.flag_wpr;
         SP.occ_thr = grid->dens_mode == RADT_DENS_LN ? -39.1439f : 1e-17f;     // N_EMPTY of the march kernels
         SP.dens = grid->dens; SP.temp = grid->temp; SP.vel = grid->vel;
-        if (!reuse) {
+        if (!reuse && band.first) {
             CUDA_TRY(radt_launch_setup(SP, LT, CT, st));
             ++g_launches;
             if (occ && grid->kind == RADT_GRID_SPH3D) {      // the (r, theta) occupancy words need every node flag: own launch
@@ -473,6 +483,8 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         MP.nx = SP.nx; MP.ny = SP.ny; MP.nstep = SP.nstep;
         MP.tiles_x = (MP.nx + RADT_TILE_X - 1) / RADT_TILE_X;
         MP.tiles_y = (MP.ny + RADT_TILE_Y - 1) / RADT_TILE_Y;
+        MP.tile_y0 = band.nty ? band.ty0 : 0; MP.launch_ty = band.nty ? band.nty : MP.tiles_y; MP.banded = band.nty ? 1 : 0;
+        if (MP.tile_y0 < 0 || MP.tile_y0 + MP.launch_ty > MP.tiles_y) return fail(RADT_E_INVALID, "row band outside the image");
         MP.b0 = b0;
         MP.opt_window = opt.window; MP.opt_skip_empty = opt.skip_empty;
         MP.opt_zero_grad = opt.zero_dens_grad || !opt.skip_empty;
@@ -496,13 +508,13 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
         else CUDA_TRY(radt_launch_march_bwd(MP, nb, st));
         ++g_launches;
     }
-    if (pass == RADT_PASS_FWD && loss.target) {
+    if (pass == RADT_PASS_FWD && loss.target && band.last) {
         const double nvox = loss.nvox_total > 0 ? loss.nvox_total : (double)batch * geom[0].nx * geom[0].ny * line->nchan;
         CUDA_TRY(radt_launch_loss_finish(reinterpret_cast<double *>(dws.counters + 8),
                                          0.5 / (loss.sigma * loss.sigma * nvox), loss.loss, st));
         ++g_launches;
     }
-    if (pass == RADT_PASS_BWD && (g_dens || g_temp || g_vel)) {
+    if (pass == RADT_PASS_BWD && (g_dens || g_temp || g_vel) && band.last) {
         CUDA_TRY(radt_launch_unpack(dws.grad, dg.cells, batch, stride, g_dens, g_temp, g_vel, st));
         ++g_launches;
     }
@@ -844,6 +856,103 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
         }
         g_launches = launches;
         return RADT_OK;
+    }
+    // A single large image runs in ROW BANDS the same way: ONE setup, then per band of tile rows the forward march (chi^2 term
+    // fused: it only needs its own rows of the target) and, in a fit step, the adjoint march of the same rows, which adds into
+    // the shared gradient cells; the target rows of band r + 1 upload / the cube rows of band r download under those marches.
+    if (batch == 1 && mode != 2) {
+        const int nx = geom[0].nx, ny = geom[0].ny;
+        const size_t row_vox = (size_t)nx * line->nchan;
+        long long rows = (long long)(((size_t)16 << 20) / (row_vox * sizeof(float)));
+        if (const char *e = getenv("RADT_HOST_BAND_ROWS")) {       // test hook, as RADT_HOST_CHUNK_ITEMS
+            const int n = atoi(e);
+            if (n >= 1) rows = n;
+        }
+        rows = (rows + RADT_TILE_Y - 1) / RADT_TILE_Y * RADT_TILE_Y;
+        if (rows < RADT_TILE_Y) rows = RADT_TILE_Y;
+        if ((ny + rows - 1) / rows > 256) rows = ((ny + 255) / 256 + RADT_TILE_Y - 1) / RADT_TILE_Y * RADT_TILE_Y;
+        int nbands = (int)((ny + rows - 1) / rows);
+        // Fit steps on 3-D grids stay in one piece: their forward march is longer than the target upload, which the plain path
+        // already hides under it, and bands only add launch tails (measured on config 4: 13.0 -> 13.4 ms with bands; on the
+        // axisymmetric config 3 the upload is three times the forward: 4.99 -> 3.95 ms).  RADT_HOST_BAND_ROWS overrides.
+        if (mode == 1 && grid->kind != RADT_GRID_AXISYM && !getenv("RADT_HOST_BAND_ROWS")) nbands = 1;
+        if (nbands > 1) {
+            static thread_local std::vector<cudaEvent_t> evs;
+            if (!s2) {
+                CUDA_TRY(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+                CUDA_TRY(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
+                CUDA_TRY(cudaEventCreateWithFlags(&ev_copied, cudaEventDisableTiming));
+            }
+            while ((int)evs.size() < nbands) {
+                cudaEvent_t e;
+                CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                evs.push_back(e);
+            }
+            auto band_of = [&](int k) {
+                Band bd;
+                const long long r0 = (long long)k * rows, r1 = r0 + rows < ny ? r0 + rows : ny;
+                bd.ty0 = (int)(r0 / RADT_TILE_Y); bd.nty = (int)((r1 - r0 + RADT_TILE_Y - 1) / RADT_TILE_Y);
+                bd.first = k == 0; bd.last = k == nbands - 1;
+                return bd;
+            };
+            CUDA_TRY(cudaEventRecord(ev_alloc, B.st));
+            CUDA_TRY(cudaStreamWaitEvent(s2, ev_alloc, 0));
+            if (mode == 0) {
+                for (int k = 0; k < nbands; ++k) {
+                    const long long r0 = (long long)k * rows, r1 = r0 + rows < ny ? r0 + rows : ny;
+                    const size_t off = (size_t)r0 * row_vox, nby = (size_t)(r1 - r0) * row_vox * sizeof(float);
+                    rc = run_pass(geom, line, &dgrid, 1, opt, RADT_PASS_FWD, d_cube, d_lo, nullptr, nullptr, nullptr, nullptr, ws, wsb,
+                                  B.st, LossArgs(), band_of(k));
+                    if (rc) { cudaStreamSynchronize(s2); return rc; }
+                    launches += g_launches;
+                    CUDA_TRY(cudaEventRecord(evs[k], B.st));
+                    CUDA_TRY(cudaStreamWaitEvent(s2, evs[k], 0));
+                    CUDA_TRY(cudaMemcpyAsync(cube + off, d_cube + off, nby, cudaMemcpyDeviceToHost, s2));
+                    if (cube_lo) CUDA_TRY(cudaMemcpyAsync(cube_lo + off, d_lo + off, nby, cudaMemcpyDeviceToHost, s2));
+                }
+                CUDA_TRY(cudaStreamSynchronize(B.st));
+                CUDA_TRY(cudaStreamSynchronize(s2));
+                g_launches = launches;
+                return RADT_OK;
+            }
+            if (!target) return fail(RADT_E_INVALID, "null target");
+            float *d_t = (float *)B.alloc(nvox * sizeof(float));
+            double *d_loss = (double *)B.alloc(sizeof(double));
+            float *d_g[3] = { nullptr, nullptr, nullptr };
+            float *h_g[3] = { g_dens, g_temp, g_vel };
+            for (int i = 0; i < 3; ++i)
+                if (h_g[i] && !(d_g[i] = (float *)B.alloc(fbytes))) return fail(RADT_E_CUDA, "device allocation failed");
+            if (!d_t || !d_loss) return fail(RADT_E_CUDA, "device allocation failed");
+            for (int k = 0; k < nbands; ++k) {
+                const long long r0 = (long long)k * rows, r1 = r0 + rows < ny ? r0 + rows : ny;
+                const size_t off = (size_t)r0 * row_vox;
+                CUDA_TRY(cudaMemcpyAsync(d_t + off, target + off, (size_t)(r1 - r0) * row_vox * sizeof(float), cudaMemcpyHostToDevice, s2));
+                CUDA_TRY(cudaEventRecord(evs[k], s2));
+            }
+            ob.reuse_setup = 1;
+            LossArgs la;
+            la.target = d_t; la.dl_out = d_dl; la.loss = d_loss; la.sigma = sigma;
+            for (int k = 0; k < nbands; ++k) {
+                const Band bd = band_of(k);
+                CUDA_TRY(cudaStreamWaitEvent(B.st, evs[k], 0));
+                rc = run_pass(geom, line, &dgrid, 1, opt, RADT_PASS_FWD, d_cube, d_lo, nullptr, nullptr, nullptr, nullptr, ws, wsb, B.st,
+                              la, bd);
+                if (rc) { cudaStreamSynchronize(s2); return rc; }
+                launches += g_launches;
+                rc = run_pass(geom, line, &dgrid, 1, &ob, RADT_PASS_BWD, d_cube, d_lo, d_dl, d_g[0], d_g[1], d_g[2], ws, wsb, B.st,
+                              LossArgs(), bd);
+                if (rc) { cudaStreamSynchronize(s2); return rc; }
+                launches += g_launches;
+            }
+            if (loss_out) CUDA_TRY(cudaMemcpyAsync(loss_out, d_loss, sizeof(double), cudaMemcpyDeviceToHost, B.st));
+            if (cube) CUDA_TRY(cudaMemcpyAsync(cube, d_cube, nvox * sizeof(float), cudaMemcpyDeviceToHost, B.st));
+            for (int i = 0; i < 3; ++i)
+                if (h_g[i]) CUDA_TRY(cudaMemcpyAsync(h_g[i], d_g[i], fbytes, cudaMemcpyDeviceToHost, B.st));
+            CUDA_TRY(cudaStreamSynchronize(B.st));
+            CUDA_TRY(cudaStreamSynchronize(s2));
+            g_launches = launches;
+            return RADT_OK;
+        }
     }
     if (mode == 0) {
         rc = radt_render(geom, line, &dgrid, batch, opt, d_cube, d_lo, ws, wsb, B.st);

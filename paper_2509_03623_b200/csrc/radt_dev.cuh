@@ -111,6 +111,8 @@ struct MarchParams {
     DevWs ws;
     int nx, ny, nstep;
     int tiles_x, tiles_y;
+    int tile_y0, launch_ty; // this launch covers tile rows [tile_y0, tile_y0 + launch_ty) (row bands of the HOST entry points);
+    int banded;             // 1: tile rows in image order (a band is a contiguous row range); 0: centre-out over the whole image
     int b0;                // first batch item of this launch
     int opt_window, opt_skip_empty;
     int opt_zero_grad;     // adjoint: zero-opacity steps of LINEAR density grids are marched for their dL/dn (default)

@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(RADT_WARPS_PER_CTA * 32, (COMP && NP == 4) ? 4
 template <int KIND, int NP>
 static cudaError_t launch_fwd_t(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    dim3 grid(P.tiles_x, P.tiles_y, nbatch);
+    dim3 grid(P.tiles_x, P.launch_ty, nbatch);
     const bool comp = P.cube_lo != nullptr;
     if (P.chan_lo && comp) k_march_fwd<KIND, NP, true, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
     else if (P.chan_lo) k_march_fwd<KIND, NP, true, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
@@ -360,7 +360,7 @@ static cudaError_t launch_fwd_t(const MarchParams &P, int nbatch, cudaStream_t s
 template <int KIND, int NP>
 static cudaError_t launch_bwd_t(const MarchParams &P, int nbatch, cudaStream_t st)
 {
-    dim3 grid(P.tiles_x, P.tiles_y, nbatch);
+    dim3 grid(P.tiles_x, P.launch_ty, nbatch);
     const bool comp = P.cube_lo != nullptr;
     if (P.chan_lo && comp) k_march_bwd<KIND, NP, true, true><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);
     else if (P.chan_lo) k_march_bwd<KIND, NP, true, false><<<grid, RADT_WARPS_PER_CTA * 32, 0, st>>>(P);

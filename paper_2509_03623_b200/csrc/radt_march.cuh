@@ -346,8 +346,8 @@ __device__ __forceinline__ bool ray_setup(const MarchParams &P, RayCtx &rc, int 
     // Tiles are issued from the image centre outwards (rows, and tiles within a row, alternate around the centre):
     // rays through the disk centre carry the most steps, the empty corners fill the tail of the launch
     // (measured on config 2: under 1 % either way; kept because the heavy tiles no longer depend on the PA).
-    const int kx = blockIdx.x, ky = blockIdx.y;        // grid = (tiles_x, tiles_y, batch chunk): no integer division per ray
-    int tx = centre_out(kx, P.tiles_x), ty = centre_out(ky, P.tiles_y);
+    const int kx = blockIdx.x, ky = blockIdx.y + P.tile_y0;     // grid = (tiles_x, tile rows of this launch, batch chunk)
+    int tx = centre_out(kx, P.tiles_x), ty = P.banded ? ky : centre_out(ky, P.tiles_y);
     rc.b = blockIdx.z;
     rc.ix = tx * RADT_TILE_X + (warp & (RADT_TILE_X - 1));
     rc.iy = ty * RADT_TILE_Y + (warp / RADT_TILE_X);

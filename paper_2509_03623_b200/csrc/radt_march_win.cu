@@ -674,7 +674,7 @@ static cudaError_t launch_w(K kern, const MarchParams &P, int nbatch, size_t war
     const size_t smem = warp_bytes * RADT_WARPS_PER_CTA;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid(P.tiles_x, P.tiles_y, nbatch);
+    dim3 grid(P.tiles_x, P.launch_ty, nbatch);
     kern<<<grid, RADT_WARPS_PER_CTA * 32, smem, st>>>(P);
     return cudaGetLastError();
 }

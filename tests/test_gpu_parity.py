@@ -461,6 +461,41 @@ def test_host_entry_points_in_item_chunks(rt, chunk, monkeypatch):
         np.testing.assert_allclose(b, a, rtol=1e-4, atol=1e-6 * np.abs(a).max())
 
 
+@pytest.mark.parametrize("rows", [2, 6, 16])
+def test_host_entry_points_in_row_bands(rt, rows, monkeypatch):
+    """A single large image runs in row bands in the HOST calls (one setup, per band the fused-loss forward and the adjoint of its
+    rows, transfers under the marches); RADT_HOST_BAND_ROWS forces that path on a small image (32 rows: 16, 6 and 2 bands, the
+    last one partial for 6).  Same cube bit for bit, same loss and gradients as the one-launch path."""
+    B = rt.binding
+    sc = make_config(2, npix=32)
+    d = B.Descriptors(sc)
+    h = B.stack_fields(sc)
+    ref = _oracle_cube(sc)
+    tgt, sigma = l2_target(ref[0], 7)
+    tgt32 = np.ascontiguousarray(tgt[None], np.float32)
+
+    def run():
+        cube, lo = np.zeros(d.cube_shape, np.float32), np.zeros(d.cube_shape, np.float32)
+        B.radt_render_host(d, *h, cube, rt.opt(), lo)
+        g = [np.zeros_like(h[0]) for _ in range(3)]
+        cube2 = np.zeros_like(cube)
+        loss = B.radt_fit_step_host(d, *h, tgt32, sigma, cube2, *g, rt.opt())
+        return cube, lo, cube2, loss, g
+
+    monkeypatch.setenv("RADT_HOST_BAND_ROWS", "100000")          # one band: the plain path
+    c0, l0, c20, loss0, g0 = run()
+    monkeypatch.setenv("RADT_HOST_BAND_ROWS", str(rows))
+    c1, l1, c21, loss1, g1 = run()
+    check_cube("banded host cube", c1, ref)
+    np.testing.assert_array_equal(c0, c1); np.testing.assert_array_equal(l0, l1); np.testing.assert_array_equal(c20, c21)
+    assert loss1 == pytest.approx(loss0, rel=1e-12)
+    G = ((c1.astype(np.float64) - tgt32) / (sigma ** 2 * c1.size)).astype(np.float32)
+    want = po.render_bwd(sc, G[0].astype(np.float64))
+    for nm, a, b, w in zip(("dens", "temp", "vel"), g0, g1, want):
+        np.testing.assert_allclose(b, a, rtol=1e-4, atol=1e-6 * np.abs(a).max())
+        check_grad(f"banded host g_{nm}", b[0], w)
+
+
 def test_l2_loss_kernel(rt):
     R = rt.Renderer([make_config(1)])
     R.render()
