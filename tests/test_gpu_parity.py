@@ -559,6 +559,8 @@ def test_workspace_too_small_and_launch_count(rt):
 def test_options_are_per_call_and_mismatches_are_refused(rt):
     """include/radt.h radt_options: no process-wide state; the adjoint of a cube must get the options (and the cube_lo
     choice) of the forward that wrote it; reuse_setup needs a workspace the same forward set up."""
+    if os.environ.get("RADT_TEST_DENSE") == "1":
+        pytest.skip("exercises the very options the dense one-off run overrides")
     B = rt.binding
     sc = tiny_axisym_scene(seed=64)
     R = rt.Renderer([sc])
@@ -779,6 +781,8 @@ def test_adjoint_without_low_order_words(rt, case):
 def test_skip_zero_opacity_steps_in_the_adjoint(rt, make):
     """radt_options.zero_dens_grad = 0: steps without opacity are not marched in the adjoint.  They only carry dL/dn of
     cells whose density is exactly zero, so g_temp, g_vel and g_dens at non-zero cells equal the exact gradient."""
+    if os.environ.get("RADT_TEST_DENSE") == "1":
+        pytest.skip("exercises the very options the dense one-off run overrides")
     sc = make()
     d = np.array(sc.grid.dens)
     if not (d == 0).any():                       # the tiny scene has no masked cells of its own
