@@ -73,6 +73,10 @@ def test_null_and_unsupported(lib):
     assert lib.radt_workspace_bytes(None, C.byref(d.line), C.byref(d.grid), 1, 0, C.byref(out)) == -1
     assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 0, 0, C.byref(out)) == -1
     assert lib.radt_workspace_bytes(d.geom, C.byref(d.line), C.byref(d.grid), 1, 9, C.byref(out)) == -1
+    # counter read-outs refuse null pointers before touching the device
+    out4, out2 = (C.c_uint64 * 4)(), (C.c_uint64 * 2)()
+    assert lib.radt_read_counters(None, out4, None) == -1 and lib.radt_read_counters(C.c_void_p(16), None, None) == -1
+    assert lib.radt_read_lane_counters(None, out2, None) == -1 and lib.radt_read_lane_counters(C.c_void_p(16), None, None) == -1
 
 
 def test_options_struct_defaults_and_size_check(lib):
