@@ -461,8 +461,8 @@ def test_host_entry_points_in_item_chunks(rt, chunk, monkeypatch):
         np.testing.assert_allclose(b, a, rtol=1e-4, atol=1e-6 * np.abs(a).max())
 
 
-@pytest.mark.parametrize("rows", [2, 6, 16])
-def test_host_entry_points_in_row_bands(rt, rows, monkeypatch):
+@pytest.mark.parametrize("rows,npix", [(2, 32), (6, 32), (16, 32), (6, 31), (4, 9)])
+def test_host_entry_points_in_row_bands(rt, rows, npix, monkeypatch):
     """A single large image runs in row bands in the HOST calls (one setup, per band the fused-loss forward and the adjoint of its
     rows, transfers under the marches); RADT_HOST_BAND_ROWS forces that path on a small image (32 rows: 16, 6 and 2 bands, the
     last one partial for 6).  Same cube bit for bit, same loss and gradients as the one-launch path."""
