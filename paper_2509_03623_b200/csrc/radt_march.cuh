@@ -232,6 +232,15 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
         float ca = L.c_hw * (fmaf(L.a1, T, L.a0) * invalpha);          // channels per unit of u'
         float ul = 14.0f * rcp_approx(ca);
         float U2 = fmaxf(UWIN2_MIN + (float)ek, fminf(UWIN2_MAX + (float)ek, ul * ul));
+        // the 2^-40 window is wider than a 32-channel group: the step runs over the fixed 32-channel blocks whatever its cut,
+        // so it takes the full 2^-60 window (a scene whose whole velocity gradient came from the far wings of very wide lines,
+        // 2 channels of 0.02 km/s under a 0.4 km/s line, showed the relaxed cut at 5e-3 of that - tiny - gradient: random scene
+        // 764).  Windows of 30-32 channels keep the relaxed cut: they still fit one group (frequent among the optically thick steps of configs 3 and 5:
+        // taking the full window there too cost 14 % of the config-5 step).
+        {
+            const float u16 = 15.5f * rcp_approx(ca);
+            if (UWIN2_MIN + (float)ek > u16 * u16) U2 = UWIN2_MAX + (float)ek;
+        }
         float hw = fminf(sqrt_approx(U2) * ca, 1.0e6f);
         if (!P.opt_window) hw = 1.0e6f;
         // channels with |c - x| <= hw, x = c_ref - del: floor(y) = rn(y - 1/2) up to ties, which sit on the cut

@@ -712,6 +712,15 @@ def test_random_scenes(rt, seed):
     _parity_fwd_bwd(rt, _random_scene(seed), f"random scene {seed}", seed=seed)
 
 
+@pytest.mark.parametrize("seed", [764])
+def test_random_scenes_found_by_the_long_runs(rt, seed):
+    """Seeds beyond the committed range that a one-off RADT_RANDOM_SCENES=2000 run found.  764: a spherical grid seen edge-on
+    with 2 channels of 0.02 km/s under a 0.4 km/s wide line; only the central ray is bright and its velocity gradient vanishes
+    exactly, so the whole g_vel (1e-10 of its natural scale) comes from far wings, where the window kernels' relaxed 2^-40
+    cut of lines wider than 29 channels showed at 5e-3 of it; such steps now take the full 2^-60 window."""
+    _parity_fwd_bwd(rt, _random_scene(seed), f"random scene {seed}", seed=seed)
+
+
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_MEDIUM", "6"))))
 def test_random_medium_scenes(rt, seed):
     """Hundreds of steps per ray, many of them through optically thick LN grids (candidate queues, step pairs and
