@@ -160,6 +160,19 @@ void make_dev_grid(const radt_grid *grid, DevGrid &d)
     if (grid->kind == RADT_GRID_AXISYM || grid->kind == RADT_GRID_SPH3D) {
         double rmin = grid->lo[0], rmax = grid->hi[0];
         d.rmin2 = rmin * rmin; d.rmax2 = rmax * rmax; d.inv_rmin = 1.0 / rmin;
+        {
+            // smallest double t with sqrt(t) >= r_min and largest with sqrt(t) <= r_max (IEEE sqrt is correctly rounded and
+            // monotone): a step whose radius equals a boundary up to rounding is then decided as a plain fp64 evaluation
+            // decides it (random scenes 4841, 6865: a ray through the star with |s| = r_min exactly)
+            double t = d.rmin2;
+            while (t > 0.0 && std::sqrt(t) >= rmin) t = std::nextafter(t, 0.0);
+            while (std::sqrt(t) < rmin) t = std::nextafter(t, INFINITY);
+            d.rho2_lo = t;
+            t = d.rmax2;
+            while (std::sqrt(t) <= rmax) t = std::nextafter(t, INFINITY);
+            while (std::sqrt(t) > rmax) t = std::nextafter(t, 0.0);
+            d.rho2_hi = t;
+        }
         d.zlo = grid->lo[1]; d.zhi = grid->hi[1];
         d.lg2_ratio = std::log2(rmax / rmin);
         d.uscale = (float)((double)(grid->n[0] - 1) / d.lg2_ratio);

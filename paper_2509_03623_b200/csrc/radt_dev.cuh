@@ -54,6 +54,9 @@ struct DevGrid {
     double rb2;                        // bounding sphere radius^2 (axisym and spherical clip)
     // spherical (kind 2): n0 = nr (log-spaced, shares rmin2/rmax2/uscale/... with the axisymmetric axis), n1 = ntheta, n2 = nphi
     double cos_tlo, cos_thi;           // cos of the theta range (decreasing in theta)
+    double rho2_lo, rho2_hi;           // in range iff rho2_lo <= rho^2 <= rho2_hi, rho^2 = (x x + y y) + z z with every operation
+                                       // rounded: exactly the doubles t with r_min <= sqrt(t) <= r_max (correctly rounded sqrt),
+                                       // i.e. the decision of a plain fp64 evaluation, ties on the boundary included
     float th_c0, th_scale, ph_scale;   // theta index = (th_c0 - asin(z/rho)) th_scale, th_c0 = pi/2 - theta_lo; phi index = phi ph_scale
     // fp32 constants of the window kernels' prefilter (a superset test with one cell of margin, radt_march_win.cu)
     float pre_us_half, pre_uoff;       // axisym / spherical: u = lg2(r^2) pre_us_half + pre_uoff

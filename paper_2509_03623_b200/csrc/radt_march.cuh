@@ -95,10 +95,12 @@ __device__ __forceinline__ void phase_a(const MarchParams &P, const DevGeom &G, 
         // radial index as on the axisymmetric grid (cell from an fp32 estimate, in-cell fraction from rho^2/r_i^2);
         // theta through asin(z/rho), which is well conditioned around the equator where disk grids live; phi
         // through atan2 in fp32 (1e-7 rad is 4e-6 of a cell at 256 nodes).
-        double rho2 = r2 + z * z;
+        // rho^2 with every product and sum rounded, and thresholds that are exactly the doubles whose square root lies in
+        // [r_min, r_max]: the radial in/out decision of a plain fp64 evaluation, boundary ties included (radt_dev.cuh)
+        double rho2 = __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z));
         double irho = rsqrt_d(rho2);
         double cz = z * irho;
-        bool in = (k < P.nstep) && (r2 > 0.0) && (rho2 >= g.rmin2) && (rho2 <= g.rmax2) && (cz <= g.cos_tlo) && (cz >= g.cos_thi);
+        bool in = (k < P.nstep) && (r2 > 0.0) && (rho2 >= g.rho2_lo) && (rho2 <= g.rho2_hi) && (cz <= g.cos_tlo) && (cz >= g.cos_thi);
         if (!in) return;
         float wf = fminf(fmaxf((g.th_c0 - asinf((float)cz)) * g.th_scale, 0.f), (float)(g.n1 - 1));
         int j = min(max(rn_int(wf - 0.5f), 0), g.n1 - 2);
