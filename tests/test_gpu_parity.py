@@ -738,6 +738,58 @@ def test_random_medium_scenes_that_once_needed_a_wider_floor(rt, seed):
     _parity_fwd_bwd(rt, _random_scene(seed, medium=True), f"random medium scene {seed}", seed=seed)
 
 
+def _rays_with_a_sample_on_a_boundary(sc, tol=1e-12):
+    """Rays (iy, ix) of an AXISYM / SPH3D scene that have a sample within `tol` (relative) of a grid boundary, from a plain numpy
+    evaluation of O4-O5 on the oracle's ray table: the in/out decision of such a sample is a tie between
+    roundings (reading (a))."""
+    g, gr = sc.geom, sc.grid
+    rg = po.ray_geometry(sc)
+    w = rg["dir"]
+    k = np.arange(g.nstep) + 0.5
+    out = set()
+    for ray in np.flatnonzero(rg["valid"]):
+        o = rg["origin"][ray]
+        s = rg["s0"][ray] + k * rg["ds"][ray]
+        x, y, z = o[0] + s * w[0], o[1] + s * w[1], o[2] + s * w[2]
+        with np.errstate(divide="ignore", invalid="ignore"):
+            if gr.kind == 0:
+                r = np.hypot(x, y)
+                q = (np.abs(z) if gr.mirror_z else z) / r
+            else:
+                r = np.sqrt(x * x + y * y + z * z)
+                q = np.arccos(z / r)
+        near = np.zeros_like(s, dtype=bool)
+        for val, bnd in ((r, gr.lo[0]), (r, gr.hi[0]), (q, gr.lo[1]), (q, gr.hi[1])):
+            near |= np.abs(val - bnd) <= tol * max(abs(bnd), 1.0)
+        if near.any():
+            out.add((int(ray) // g.nx, int(ray) % g.nx))
+    return out
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_SPECIAL_ANGLES", "12"))))
+def test_random_scenes_with_special_viewing_angles(rt, seed):
+    """The random scenes again with inclination, PA and azimuth drawn from {0, 30, 45, 60, 90, 180, 270} degrees: round-number
+    geometries put samples EXACTLY on a grid boundary (an edge-on view with a ray at z / r = zeta_lo, a chord that ends on
+    r_max), where the in/out decision is a tie between the roundings of two correct fp64 evaluations (reading (a)).
+    Every voxel must agree except on rays that a plain numpy evaluation shows to have such a sample."""
+    rng = np.random.default_rng(77000 + seed)
+    sc = _random_scene(seed)
+    g = replace(sc.geom, incl=float(np.radians(rng.choice([0.0, 90.0, 45.0, 30.0, 60.0]))),
+                pa=float(np.radians(rng.choice([0.0, 90.0, 180.0, -90.0]))), az=float(np.radians(rng.choice([0.0, 90.0, 180.0, 270.0]))))
+    sc = replace(sc, geom=g)
+    ref = _oracle_cube([sc])
+    R = _gpu_forward(rt, sc)
+    got = R.cube.cpu().numpy()
+    bad = np.abs(got - ref) > 1e-4 * np.abs(ref) + 1e-6 * max(ref.max(), 1e-300)
+    if not bad.any():
+        return
+    assert sc.grid.kind != 1, "Cartesian grids compare the coordinates themselves: no ties"
+    ties = _rays_with_a_sample_on_a_boundary(sc)
+    bad_rays = {(int(iy), int(ix)) for _, iy, ix, _ in np.argwhere(bad)}
+    assert bad_rays <= ties, f"rays {sorted(bad_rays - ties)} differ without a sample on a boundary"
+    assert len(bad_rays) <= max(2, (g.nx * g.ny) // 2)          # (a 6 x 2 image can have its four symmetric rays on ties)
+
+
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_OFFCENTRE", "8"))))
 def test_random_offcentre_scenes(rt, seed):
     """Images that are not centred on the star and not square in extent, in CGS or Jy/pixel units."""
