@@ -109,3 +109,34 @@ def test_disk_fields_feed_the_render_end_to_end():
     eps = 0.25
     fd = (oracle_loss(T0 + eps * d, target, sigma, fw0["mask"]) - oracle_loss(T0 - eps * d, target, sigma, fw0["mask"])) / (2 * eps)
     assert np.sum(gT * d) == pytest.approx(fd, rel=2e-2)
+
+
+@pytest.mark.parametrize("nr,nz", [(9, 7), (37, 45), (20, 200), (33, 33), (130, 3)])
+def test_disk_fields_on_ragged_grid_sizes(nr, nz):
+    """Column lengths that are not a multiple of the 32 lanes a column is split over (7, 45, 200, 33, 3 nodes) and column counts
+    that leave the last block partly empty: forward fields and the adjoint against the oracle."""
+    from synth import tiny_axisym_scene
+    scenes = [tiny_axisym_scene(seed=3, nr=nr, nz=nz), tiny_axisym_scene(seed=4, nr=nr, nz=nz)]
+    B, desc, params, temp, ws = _setup(scenes)
+    dens, vel = torch.empty_like(temp), torch.empty_like(temp)
+    B.radt_disk_fields(B.make_disks(params), desc, temp, dens, vel, ws)
+    gr = scenes[0].grid
+    r, zeta = dp.nodes(gr.n[0], gr.n[1], gr.lo[0], gr.hi[0], gr.hi[1])
+    rng = np.random.default_rng(nr * 1000 + nz)
+    gn = (rng.standard_normal(tuple(temp.shape)) * 1e-8).astype(np.float32)
+    gv = (rng.standard_normal(tuple(temp.shape)) * 1e-6).astype(np.float32)
+    gT = torch.zeros_like(temp)
+    B.radt_disk_fields_bwd(B.make_disks(params), desc, temp, torch.from_numpy(gn).cuda(), torch.from_numpy(gv).cuda(), gT, ws)
+    for b in range(len(scenes)):
+        fw = dp.forward(params[b], temp[b].cpu().numpy(), r, zeta)
+        got_n, got_v = dens[b].cpu().numpy(), vel[b].cpu().numpy()
+        same = (got_n > 0) == fw["mask"]
+        edge = (np.abs(params[b].f_col * fw["N"] / params[b].n_dissoc - 1.0) < 1e-9) | (np.abs(fw["T"] / params[b].t_freeze - 1.0) < 1e-9)
+        assert np.all(same | edge)
+        np.testing.assert_allclose(got_n[same], fw["n_co"][same], rtol=2e-7)
+        np.testing.assert_allclose(got_v, fw["v_phi"], rtol=2e-7, atol=1e-3)
+        want = dp.adjoint(params[b], fw, gn[b], gv[b], r, zeta)
+        got = gT[b].cpu().numpy().astype(np.float64)
+        scale = np.abs(want).max()
+        if scale > 0:
+            assert np.max(np.abs(got - want)) <= 1e-3 * scale
