@@ -259,6 +259,27 @@ int radt_disk_fields_bwd(const radt_disk *disk, const radt_grid *grid, int32_t b
                          const float *g_dens, const float *g_vel, float *g_temp, void *ws, size_t ws_bytes,
                          void *cuda_stream);
 
+/* radt_disk_fields without a workspace, for callers that cannot allocate device memory.  Who that is: a plug-in or
+ * solver running inside a process whose device memory was handed out in full at start-up (to the host application's
+ * pool, or to fixed partitions of a control loop), where a cudaMalloc for the workspace fails or is forbidden, and loops
+ * that cannot accept the device-wide synchronisation and the unbounded latency of cudaMalloc / cudaFree.  The scratch
+ * that radt_disk_fields keeps in `ws` lives here in a fixed array inside the library image instead: about 8 MiB that
+ * EVERY GPU which loads libradt.so holds until the process exits, used or not.  The caller still passes the inputs and
+ * the outputs (DEVICE float32, as radt_disk_fields); results are those of radt_disk_fields (same kernels).
+ *   - Limit: batch * nr * nzeta <= RADT_DISK_STATIC_MAX_CELLS (configs 1-3 whole, config 5 in two halves); more fails
+ *     with RADT_E_INVALID before anything is launched.  Split the batch, or use radt_disk_fields.
+ *   - The call itself makes no cudaMalloc / cudaFree and calls no allocating library routine.  The FIRST call on each
+ *     device looks up the array's device address (cudaGetSymbolAddress, with that device current; the runtime may load
+ *     the library's kernels onto the device at that moment).  Make that first call early, with the device you will use
+ *     current, and before any stream capture is begun.
+ *   - One array per device serves every call, and it keeps what the last call left.  Nothing needs clearing (each call
+ *     overwrites all it reads), but two calls that overlap on the same GPU (different streams, different threads) race
+ *     on it: order them on one stream or with events.  Calls on different devices do not interfere.
+ * Asynchronous on cuda_stream; disk, grid: HOST, as radt_disk_fields. */
+#define RADT_DISK_STATIC_MAX_CELLS 262144
+int radt_disk_fields_static(const radt_disk *disk, const radt_grid *grid, int32_t batch, const float *temp,
+                            float *dens_out, float *vel_out, void *cuda_stream);
+
 /* ---- Symmetric MLP temperature field (Eq. 10) ----------------------------------------
  * T(r, |z|) = MLP_w(gamma(r, |z|)) on the nodes of an AXISYM grid (mirror symmetric, so a function of |z|):
  * p = (i/(nr-1), j/(nzeta-1)); gamma(p) = (p_0, p_1, {sin(2^k pi p_0), cos(2^k pi p_0), sin(2^k pi p_1), cos(2^k pi p_1)},

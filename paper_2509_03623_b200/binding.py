@@ -21,6 +21,7 @@ EXPORTS = ["radt_version", "radt_last_error", "radt_options_default", "radt_work
            "radt_ray_geometry", "radt_render", "radt_render_bwd", "radt_grad_layout", "radt_unpack_grad",
            "radt_l2_loss_grad", "radt_render_host",
            "radt_render_loss", "radt_disk_workspace_bytes", "radt_disk_fields", "radt_disk_fields_bwd",
+           "radt_disk_fields_static",
            "radt_mlp_num_params", "radt_mlp_temperature", "radt_mlp_temperature_bwd",
            "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters", "radt_read_lane_counters",
            "radt_last_launch_count"]
@@ -129,6 +130,7 @@ def lib():
         L.radt_disk_workspace_bytes.argtypes = [rp, i32, C.POINTER(C.c_size_t)]
         L.radt_disk_fields.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, C.c_size_t, vp]
         L.radt_disk_fields_bwd.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp, vp, C.c_size_t, vp]
+        L.radt_disk_fields_static.argtypes = [C.POINTER(radt_disk), rp, i32, vp, vp, vp, vp]
         L.radt_fit_step_host.argtypes = [gp, lp, rp, i32, op, vp, dbl, vp, C.POINTER(dbl), vp, vp, vp]
         L.radt_render_bwd_host.argtypes = [gp, lp, rp, i32, op, vp, vp, vp, vp, vp, vp]
         L.radt_pipe_peak.argtypes = [i32, C.POINTER(dbl), C.POINTER(dbl)]
@@ -296,6 +298,19 @@ def radt_disk_fields(disks, desc: Descriptors, temp, dens_out, vel_out, ws, stre
     with _on(temp):
         _check(lib().radt_disk_fields(disks, C.byref(desc.grid), desc.batch, _p(temp), _p(dens_out), _p(vel_out), _p(ws),
                                       C.c_size_t(ws.numel()), _stream_ptr(stream, temp)))
+
+
+DISK_STATIC_MAX_CELLS = 262144          # RADT_DISK_STATIC_MAX_CELLS of include/radt.h
+
+
+def radt_disk_fields_static(disks, desc: Descriptors, temp, dens_out, vel_out, stream=None):
+    """radt_disk_fields for callers that cannot allocate a workspace (all device memory belongs to someone else, or
+    cudaMalloc's device-wide synchronisation is not acceptable): the scratch is a fixed array inside libradt.so, at most
+    DISK_STATIC_MAX_CELLS cells per call.  One array per GPU: do not overlap two calls on the same GPU; make the first
+    call on a device before any stream capture (include/radt.h)."""
+    with _on(temp):
+        _check(lib().radt_disk_fields_static(disks, C.byref(desc.grid), desc.batch, _p(temp), _p(dens_out), _p(vel_out),
+                                             _stream_ptr(stream, temp)))
 
 
 def radt_disk_fields_bwd(disks, desc: Descriptors, temp, g_dens, g_vel, g_temp, ws, stream=None):

@@ -1123,6 +1123,32 @@ int radt_disk_fields(const radt_disk *disk, const radt_grid *grid, int32_t batch
     return RADT_OK;
 }
 
+// The forward pre-pass for callers that cannot give it a workspace (include/radt.h).  Allocates nothing: the scratch is
+// the fixed array inside radt_disk.cu, whose address radt_launch_disk_fwd_static looks up on the first call per device.
+int radt_disk_fields_static(const radt_disk *disk, const radt_grid *grid, int32_t batch, const float *temp,
+                            float *dens_out, float *vel_out, void *cuda_stream)
+{
+    if (!temp || !dens_out || !vel_out) return fail(RADT_E_INVALID, "null field pointer");
+    static thread_local DiskParamsDev Q;
+    size_t need = 0;
+    int rc = disk_setup(nullptr, grid, batch, nullptr, 0, Q, &need);         // grid and batch checks only
+    if (rc) return rc;
+    const long long cells = (long long)grid->n[0] * grid->n[1] * batch;
+    if (cells > RADT_DISK_STATIC_MAX_CELLS)
+        return fail(RADT_E_INVALID, "radt_disk_fields_static: batch x nr x nzeta = %lld cells exceeds the fixed scratch of "
+                    "%d cells; split the batch or use radt_disk_fields with a workspace", cells, RADT_DISK_STATIC_MAX_CELLS);
+    // descriptor checks and the scalar members of Q; the placeholder workspace is never dereferenced and the launcher
+    // replaces every scratch pointer derived from it
+    rc = disk_setup(disk, grid, batch, (void *)(uintptr_t)256, need, Q, nullptr);
+    if (rc) return rc;
+    Q.rt = Q.rho = Q.P = Q.gP = Q.grho = Q.colscale = Q.colH = nullptr;
+    Q.mask = nullptr;
+    Q.temp = temp; Q.dens_out = dens_out; Q.vel_out = vel_out;
+    CUDA_TRY(radt_launch_disk_fwd_static(Q, (cudaStream_t)cuda_stream));
+    g_launches = 2;
+    return RADT_OK;
+}
+
 int radt_disk_fields_bwd(const radt_disk *disk, const radt_grid *grid, int32_t batch, const float *temp,
                          const float *g_dens, const float *g_vel, float *g_temp, void *ws, size_t ws_bytes,
                          void *cuda_stream)

@@ -5,6 +5,7 @@
 // pass is latency bound, not throughput bound).  Shares nothing with oracle/.
 #include "radt_dev.cuh"
 #include "radt_kernels.h"
+#include <mutex>
 
 #define KB_CGS 1.380649e-16
 #define AU_CM 1.495978707e13
@@ -244,4 +245,68 @@ cudaError_t radt_launch_disk_bwd(const DiskParamsDev &Q, cudaStream_t st)
     k_disk_velocity<false><<<(int)((ncell + 255) / 256), 256, 0, st>>>(Q);
     k_disk_columns_bwd<<<(ncol + 3) / 4, 128, 0, st>>>(Q);
     return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// radt_disk_fields_static: the forward pre-pass on scratch that lives inside the library image
+// ---------------------------------------------------------------------------------------------
+// Some programs that want the pre-pass have no way to hand it a workspace: every byte of device memory was given to
+// another owner when the process started (a host application's memory pool, a fixed partition for a control loop that
+// must not hit cudaMalloc's device-wide synchronisation or its unbounded latency), so a cudaMalloc made on their behalf
+// either fails or is forbidden.  For them the scratch of the forward pre-pass (rt, rho, P per cell; column scale and H
+// per column) is this file-scope array.  It is part of the loaded module: every GPU whose context loads libradt.so
+// carries these 8 MiB (+ 1.25 KiB of alignment slack) until the process exits, whether or not the entry point is used,
+// which is why the limit is kept modest: DISK_STATIC_MAX_CELLS = RADT_DISK_STATIC_MAX_CELLS (include/radt.h) cells per
+// call, batch included.
+//
+// In host code the identifier g_disk_scratch is only the host-side shadow of the symbol, not a device address: a kernel
+// handed `g_disk_scratch` by the host would fault, or on a system where the GPU can reach host memory it would quietly
+// work on the wrong bytes.  The device address comes from cudaGetSymbolAddress, asked once per device with that device
+// current (each device has its own copy of the array) and kept in g_disk_scratch_addr.
+#define DISK_STATIC_MAX_CELLS 262144ll
+#define DISK_STATIC_BYTES (3 * DISK_STATIC_MAX_CELLS * 8 + 2 * (DISK_STATIC_MAX_CELLS / 2) * 8 + 5 * 256)
+#define DISK_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) unsigned char g_disk_scratch[DISK_STATIC_BYTES];
+
+static std::mutex g_disk_scratch_lock;
+static void *g_disk_scratch_addr[DISK_STATIC_MAX_DEVICES];       // per device ordinal; nullptr = not asked yet
+
+// Device address of the current device's copy of g_disk_scratch.  The first call on a device resolves the symbol (which
+// makes the runtime load this module on that device if it has not yet); later calls read the table.
+static cudaError_t disk_static_scratch(unsigned char **ptr_out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= DISK_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> hold(g_disk_scratch_lock);
+    if (!g_disk_scratch_addr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_disk_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p || ((uintptr_t)p & 255) != 0) return cudaErrorInvalidSymbol;
+        g_disk_scratch_addr[dev] = p;
+    }
+    *ptr_out = (unsigned char *)g_disk_scratch_addr[dev];
+    return cudaSuccess;
+}
+
+// Q arrives with everything but the scratch pointers filled in (radt_api.cu checked the descriptors and the size limit).
+// Same two kernels as radt_launch_disk_fwd.  Nothing has to be cleared between calls: k_disk_columns<true> writes every
+// word of rt, rho, P, colscale and colH of the columns of THIS call before it or k_disk_velocity<true> reads them, and
+// neither kernel reads beyond those columns, so whatever an earlier (larger or smaller) call left behind is never seen.
+cudaError_t radt_launch_disk_fwd_static(DiskParamsDev Q, cudaStream_t st)
+{
+    const long long cells = (long long)Q.nr * Q.nz * Q.nbatch, cols = (long long)Q.nr * Q.nbatch;
+    auto up256 = [](long long x) { return (x + 255) & ~255ll; };
+    const long long o_rt = 0, o_rho = up256(o_rt + cells * 8), o_P = up256(o_rho + cells * 8), o_cs = up256(o_P + cells * 8),
+                    o_cH = up256(o_cs + cols * 8), end = up256(o_cH + cols * 8);
+    if (cells < 1 || cells > DISK_STATIC_MAX_CELLS || end > (long long)DISK_STATIC_BYTES) return cudaErrorInvalidValue;
+    unsigned char *base = nullptr;
+    cudaError_t e = disk_static_scratch(&base);
+    if (e != cudaSuccess) return e;
+    Q.rt = (double *)(base + o_rt); Q.rho = (double *)(base + o_rho); Q.P = (double *)(base + o_P);
+    Q.colscale = (double *)(base + o_cs); Q.colH = (double *)(base + o_cH);
+    Q.gP = nullptr; Q.grho = nullptr; Q.mask = nullptr;           // adjoint-only scratch: the forward kernels never touch it
+    return radt_launch_disk_fwd(Q, st);
 }

@@ -16,5 +16,6 @@ cudaError_t radt_launch_march_bwd_win(const MarchParams &P, int nbatch, cudaStre
 cudaError_t radt_run_pipe_peak(int kind, double *ops_per_s, double *clock_mhz);
 cudaError_t radt_launch_disk_fwd(const DiskParamsDev &Q, cudaStream_t st);
 cudaError_t radt_launch_disk_bwd(const DiskParamsDev &Q, cudaStream_t st);
+cudaError_t radt_launch_disk_fwd_static(DiskParamsDev Q, cudaStream_t st);      // scratch inside the library image (radt_disk.cu)
 cudaError_t radt_launch_mlp_fwd(const MlpParamsDev &Q, cudaStream_t st);        // radt_mlp_tc.cu (tcgen05)
 cudaError_t radt_launch_mlp_bwd(const MlpParamsDev &Q, int nparams, cudaStream_t st);        // radt_mlp_tc_bwd.cu (tcgen05)
