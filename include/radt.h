@@ -179,6 +179,13 @@ int radt_render_bwd(const radt_geom *geom, const radt_line *line, const radt_gri
                     const radt_options *opt, const float *cube, const float *cube_lo, const float *dl_dcube,
                     float *g_dens, float *g_temp, float *g_vel, void *ws, size_t ws_bytes, void *cuda_stream);
 
+/* Drops what the library remembers about a device pointer (the options of the last forward that wrote a cube there, the
+ * setup a forward left in a workspace there).  The memory is keyed by raw pointer and knows nothing of cudaFree: call
+ * this when a cube buffer is refilled by something other than radt_render / radt_render_loss (a copy, a collective, an
+ * upload) or when the allocator may hand its address to a new tensor, so that a later radt_render_bwd is not refused on
+ * the strength of a forward that no longer applies.  Unknown pointers are fine.  HOST call, no CUDA work. */
+int radt_forget(const void *device_ptr);
+
 /* Where radt_render_bwd leaves the gradient inside a RADT_PASS_BWD workspace: [batch][cells] packed float4 cells
  * {dL/d dens, dL/d temp, dL/d vel, 0}, *nfloat_out floats starting *offset_out bytes into `ws` (HOST outputs).
  * Multi-GPU image sharding sums exactly this range over the ranks with one all-reduce on the
@@ -213,9 +220,11 @@ int radt_render_host(const radt_geom *geom, const radt_line *line, const radt_gr
                      const radt_options *opt, float *cube, float *cube_lo);
 /* Forward + chi^2 term against `target` (HOST; uploaded on a second stream under the forward march) + adjoint in one
  * call; the low-order words stay on the device; cube may be NULL.  Batched calls (radt_fit_step_host and radt_render_host)
- * whose items are 32 MB of cube or more run item chunk by item chunk, and single images of 32 MB or more in bands of rows
- * (one setup; per band the forward march and, in a fit step on axisymmetric grids, the adjoint march of the same rows), the
- * transfers of one chunk / band under the marches of another; the results are those of the one-call path (cube bit for bit). */
+ * whose cube exceeds 32 MB run in chunks of items of at most 32 MB of cube (at least one item), and single images of more
+ * than 16 MB in bands of rows of about 16 MB (one setup; per band the forward march and, in a fit step on axisymmetric grids,
+ * the adjoint march of the same rows; fit steps on 3-D grids stay in one piece), the transfers of one chunk / band under the
+ * marches of another; the results are those of the one-call path (cube bit for bit).  If a call fails half-way the library
+ * waits for every transfer it started before it returns, so the host buffers are the caller's again on every return. */
 int radt_fit_step_host(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                        const radt_options *opt, const float *target, double sigma, float *cube, double *loss_out,
                        float *g_dens, float *g_temp, float *g_vel);
@@ -322,6 +331,12 @@ int radt_read_lane_counters(const void *ws, uint64_t *out2, void *cuda_stream);
 /* Counters of the last radt_render / radt_render_bwd call on this thread (HOST): number of kernel
  * launches enqueued. */
 int radt_last_launch_count(void);
+
+/* TEST HOOK of the *_host entry points, per calling thread: chunk_items >= 1 forces batched calls into chunks of that many
+ * items, band_rows >= 1 forces single images into bands of that many rows (rounded up to whole tile rows; also for fit steps
+ * on 3-D grids), whatever their size; 0 restores the library's own policy.  Results do not depend on it (tests/ checks that
+ * on small scenes); it exists so that the chunked and banded paths can be exercised without gigabyte inputs. */
+int radt_debug_host_split(int32_t chunk_items, int32_t band_rows);
 
 #ifdef __cplusplus
 }

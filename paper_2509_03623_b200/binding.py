@@ -24,7 +24,7 @@ EXPORTS = ["radt_version", "radt_last_error", "radt_options_default", "radt_work
            "radt_disk_fields_static",
            "radt_mlp_num_params", "radt_mlp_temperature", "radt_mlp_temperature_bwd",
            "radt_fit_step_host", "radt_render_bwd_host", "radt_pipe_peak", "radt_read_counters", "radt_read_lane_counters",
-           "radt_last_launch_count"]
+           "radt_last_launch_count", "radt_forget", "radt_debug_host_split"]
 
 
 class RadtError(RuntimeError):
@@ -137,6 +137,8 @@ def lib():
         L.radt_read_counters.argtypes = [vp, C.POINTER(C.c_uint64), vp]
         L.radt_read_lane_counters.argtypes = [vp, C.POINTER(C.c_uint64), vp]
         L.radt_last_launch_count.restype = C.c_int
+        L.radt_forget.argtypes = [vp]
+        L.radt_debug_host_split.argtypes = [i32, i32]
         _lib = L
     return _lib
 
@@ -285,6 +287,17 @@ def radt_render_loss(desc: Descriptors, dens, temp, vel, target, sigma: float, c
         _check(lib().radt_render_loss(desc.geom, C.byref(desc.line), C.byref(desc.grid), desc.batch, _optp(opt), _p(target),
                                       C.c_double(float(sigma)), _p(cube), _p(cube_lo), _p(dl_dcube), _p(loss_out), _p(ws),
                                       C.c_size_t(ws.numel()), _stream_ptr(stream, cube)))
+
+
+def radt_forget(tensor_or_ptr) -> None:
+    """Drop what the library remembers about a device buffer (a cube's forward options, a workspace's setup)."""
+    ptr = tensor_or_ptr.data_ptr() if hasattr(tensor_or_ptr, "data_ptr") else int(tensor_or_ptr)
+    _check(lib().radt_forget(C.c_void_p(ptr)))
+
+
+def radt_debug_host_split(chunk_items: int = 0, band_rows: int = 0) -> None:
+    """Test hook of the HOST entry points (this thread): forced chunk / band sizes, 0 = the library's policy."""
+    _check(lib().radt_debug_host_split(int(chunk_items), int(band_rows)))
 
 
 def radt_disk_workspace_bytes(desc: Descriptors) -> int:

@@ -76,8 +76,26 @@ struct Registry {
             if (e[i].key == key && e[i].age) { tag = e[i].tag; return true; }
         return false;
     }
+    void forget(const void *key)
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        for (int i = 0; i < N; ++i)
+            if (e[i].key == key) e[i] = Remembered();
+    }
 };
 Registry g_cubes, g_workspaces;
+// Set while a HOST entry point runs its passes on the arena's own buffers: those calls pair every forward with its adjoint
+// themselves, so their cubes and workspaces stay out of the shared tables (a chunked call would otherwise push up to 256
+// entries through the 64 slots and silently evict what the callers of the DEVICE entry points rely on).
+thread_local bool g_internal_pass = false;
+// Test hook of the HOST entry points (radt_debug_host_split): forced chunk / band sizes of the calling thread, 0 = the library's
+// own policy.  (Until round 3 these were environment variables read on every call of the shipped library.)
+thread_local int g_force_chunk_items = 0, g_force_band_rows = 0;
+struct InternalPass {
+    bool prev;
+    InternalPass() : prev(g_internal_pass) { g_internal_pass = true; }
+    ~InternalPass() { g_internal_pass = prev; }
+};
 
 unsigned long long fnv(unsigned long long h, const void *p, size_t n)
 {
@@ -366,11 +384,13 @@ struct Band {
     bool first = true, last = true;
 };
 
-// What shapes the partial sums of a cube (a forward and its adjoint must agree on it) ...
-unsigned long long cube_tag(const Opts &o, bool use_win, bool comp, const radt_geom *geom, const radt_line *line, int batch)
+// What shapes the partial sums of a cube (a forward and its adjoint must agree on it): the skipping and window switches, the
+// kernel family, the low-order words and the channel count.  NOT the batch or the image size: the adjoint of the first items
+// of a batched forward (same pointer, smaller batch) is a valid call ...
+unsigned long long cube_tag(const Opts &o, bool use_win, bool comp, const radt_line *line)
 {
     unsigned long long h = 1469598103934665603ull;
-    const int v[8] = { o.window, o.skip_empty, use_win ? 1 : 0, comp ? 1 : 0, line->nchan, geom[0].nx, geom[0].ny, batch };
+    const int v[5] = { o.window, o.skip_empty, use_win ? 1 : 0, comp ? 1 : 0, line->nchan };
     return fnv(h, v, sizeof(v)) | 1ull;
 }
 // ... and what a forward leaves in its workspace for an adjoint with reuse_setup: every input of the setup kernel.
@@ -431,17 +451,20 @@ int run_pass(const radt_geom *geom, const radt_line *line, const radt_grid *grid
     const bool comp = cube_lo != nullptr;
 
     // a forward and its adjoint must agree on what shapes the partial sums of the cube
-    const unsigned long long ctag = cube_tag(opt, use_win, comp, geom, line, batch);
+    const unsigned long long ctag = cube_tag(opt, use_win, comp, line);
     const unsigned long long stag = setup_tag(opt, use_win, geom, line, grid, batch);
     bool reuse = false;
-    if (pass == RADT_PASS_FWD) {
+    if (g_internal_pass) {
+        reuse = pass == RADT_PASS_BWD && opt.reuse_setup;      // the HOST entry point ran the matching forward in this very call
+    } else if (pass == RADT_PASS_FWD) {
         g_cubes.put(cube, ctag);
         g_workspaces.put(ws, stag);
     } else {
         unsigned long long seen = 0;
         if (g_cubes.get(cube, seen) && seen != 0 && seen != ctag)      // (tag 0: a cube of unknown origin)
             return fail(RADT_E_INVALID, "this cube was rendered with other options (window / skip_empty / win_path / cube_lo) "
-                                        "than radt_render_bwd was given: the adjoint re-marches with the forward's arithmetic");
+                                        "than radt_render_bwd was given: the adjoint re-marches with the forward's arithmetic "
+                                        "(radt_forget(cube) if the buffer now holds a cube of another origin)");
         if (opt.reuse_setup) {
             if (!g_workspaces.get(ws, seen) || seen != stag)
                 return fail(RADT_E_INVALID, "reuse_setup: this workspace was not last set up by a forward with the same "
@@ -541,6 +564,22 @@ extern "C" {
 int radt_version(void) { return RADT_VERSION; }
 const char *radt_last_error(void) { return g_err; }
 int radt_last_launch_count(void) { return g_launches; }
+
+int radt_debug_host_split(int32_t chunk_items, int32_t band_rows)
+{
+    if (chunk_items < 0 || band_rows < 0) return fail(RADT_E_INVALID, "sizes must be >= 0 (0 = library policy)");
+    g_force_chunk_items = chunk_items;
+    g_force_band_rows = band_rows;
+    return RADT_OK;
+}
+
+int radt_forget(const void *device_ptr)
+{
+    if (!device_ptr) return fail(RADT_E_INVALID, "null pointer");
+    g_cubes.forget(device_ptr);
+    g_workspaces.forget(device_ptr);
+    return RADT_OK;
+}
 
 void radt_options_default(radt_options *opt)
 {
@@ -716,10 +755,29 @@ struct DevBufs {
 };
 }  // namespace
 
+static int host_common_impl(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                            const radt_options *opt, int mode, const float *target, double sigma, float *cube, float *cube_lo,
+                            const float *cube_in, const float *lo_in, const float *dl_in, double *loss_out, float *g_dens,
+                            float *g_temp, float *g_vel);
+
 static int host_common(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
                        const radt_options *opt, int mode, const float *target, double sigma, float *cube, float *cube_lo,
                        const float *cube_in, const float *lo_in, const float *dl_in, double *loss_out, float *g_dens,
                        float *g_temp, float *g_vel)
+{
+    InternalPass guard;           // the arena's cubes and workspaces stay out of the shared forward/adjoint tables
+    const int rc = host_common_impl(geom, line, grid, batch, opt, mode, target, sigma, cube, cube_lo, cube_in, lo_in, dl_in,
+                                    loss_out, g_dens, g_temp, g_vel);
+    // An error exit half-way through a chunk or band loop may leave copies into or out of the CALLER's host buffers in flight on
+    // either stream: wait for them before handing the buffers back (error path only; the message of `rc` is kept).
+    if (rc != RADT_OK) cudaDeviceSynchronize();
+    return rc;
+}
+
+static int host_common_impl(const radt_geom *geom, const radt_line *line, const radt_grid *grid, int32_t batch,
+                            const radt_options *opt, int mode, const float *target, double sigma, float *cube, float *cube_lo,
+                            const float *cube_in, const float *lo_in, const float *dl_in, double *loss_out, float *g_dens,
+                            float *g_temp, float *g_vel)
 {
     // mode 0: forward only; 1: forward + chi^2 term + adjoint; 2: adjoint from given cube and dl_dcube
     int rc = validate(geom, line, grid, batch);
@@ -778,11 +836,8 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
         if (chunk < 1) chunk = 1;
         if (chunk > batch) chunk = batch;
         if ((batch + chunk - 1) / chunk > 256) chunk = (batch + 255) / 256;
-        // test hook: RADT_HOST_CHUNK_ITEMS = n forces chunks of n items (tests/test_gpu_parity.py runs the chunked path on small scenes)
-        if (const char *e = getenv("RADT_HOST_CHUNK_ITEMS")) {
-            const int n = atoi(e);
-            if (n >= 1) chunk = n < batch ? n : batch;
-        }
+        // test hook (radt_debug_host_split): chunks of n items (tests/test_gpu_parity.py runs the chunked path on small scenes)
+        if (g_force_chunk_items >= 1) chunk = g_force_chunk_items < batch ? g_force_chunk_items : batch;
     }
     if (chunk < batch) {
         static thread_local std::vector<cudaEvent_t> evs;
@@ -877,18 +932,15 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
         const int nx = geom[0].nx, ny = geom[0].ny;
         const size_t row_vox = (size_t)nx * line->nchan;
         long long rows = (long long)(((size_t)16 << 20) / (row_vox * sizeof(float)));
-        if (const char *e = getenv("RADT_HOST_BAND_ROWS")) {       // test hook, as RADT_HOST_CHUNK_ITEMS
-            const int n = atoi(e);
-            if (n >= 1) rows = n;
-        }
+        if (g_force_band_rows >= 1) rows = g_force_band_rows;      // test hook (radt_debug_host_split)
         rows = (rows + RADT_TILE_Y - 1) / RADT_TILE_Y * RADT_TILE_Y;
         if (rows < RADT_TILE_Y) rows = RADT_TILE_Y;
         if ((ny + rows - 1) / rows > 256) rows = ((ny + 255) / 256 + RADT_TILE_Y - 1) / RADT_TILE_Y * RADT_TILE_Y;
         int nbands = (int)((ny + rows - 1) / rows);
         // Fit steps on 3-D grids stay in one piece: their forward march is longer than the target upload, which the plain path
         // already hides under it, and bands only add launch tails (measured on config 4: 13.0 -> 13.4 ms with bands; on the
-        // axisymmetric config 3 the upload is three times the forward: 4.99 -> 3.95 ms).  RADT_HOST_BAND_ROWS overrides.
-        if (mode == 1 && grid->kind != RADT_GRID_AXISYM && !getenv("RADT_HOST_BAND_ROWS")) nbands = 1;
+        // axisymmetric config 3 the upload is three times the forward: 4.99 -> 3.95 ms).  The test hook overrides.
+        if (mode == 1 && grid->kind != RADT_GRID_AXISYM && g_force_band_rows < 1) nbands = 1;
         if (nbands > 1) {
             static thread_local std::vector<cudaEvent_t> evs;
             if (!s2) {
@@ -1011,7 +1063,6 @@ static int host_common(const radt_geom *geom, const radt_line *line, const radt_
             CUDA_TRY(cudaMemcpyAsync(d_cube, cube_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
             if (lo_in) CUDA_TRY(cudaMemcpyAsync(d_lo, lo_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
             CUDA_TRY(cudaMemcpyAsync(d_dl, dl_in, nvox * sizeof(float), cudaMemcpyHostToDevice, B.st));
-            g_cubes.put(d_cube, 0);          // a cube from the host: nothing is known about the options that made it
         }
         ob.reuse_setup = mode == 1;          // the forward of this very call set the workspace up
         rc = radt_render_bwd(geom, line, &dgrid, batch, &ob, d_cube, d_lo, d_dl, d_g[0], d_g[1], d_g[2], ws, wsb, B.st);

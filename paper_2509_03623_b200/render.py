@@ -40,21 +40,33 @@ class Renderer:
             self.loss = torch.zeros(1, dtype=torch.float64, device=self.device)
         self.target = None
         self.sigma = None
+        # True while the workspace holds the setup (packed cells, occupancy words, T_max) of this object's last forward of the
+        # CURRENT field values and options.  The library can only compare descriptors and pointers; set_fields copies in place,
+        # so the pointers stay the same when the values change: that part of the reuse_setup contract is checked here.
+        self._setup_valid = False
 
     def set_options(self, **kw):
         """Change this object's radt_options for the calls that follow (a forward and its adjoint must share them)."""
         self.options.update(kw)
         self.opt = B.make_options(**self.options)
         self.opt_reuse = B.make_options(**self.options, reuse_setup=1)
+        self._setup_valid = False
 
     # ---- hot path: every call below is one C-ABI entry point ----
     def render(self, stream=None):
         B.radt_render(self.desc, self.dens, self.temp, self.vel, self.cube, self.ws, stream, self.opt, self.cube_lo)
+        self._setup_valid = True
         return self.cube
 
     def render_bwd(self, dl_dcube=None, stream=None, reuse_setup=False, unpack=True):
         """reuse_setup: the workspace still holds what this object's last render()/render_loss() of the same fields left
-        there.  unpack=False leaves the gradient as packed cells in the workspace (grad_packed())."""
+        there; refused (RadtError) when the fields or options changed since, or an adjoint rebuilt the workspace for itself.
+        unpack=False leaves the gradient as packed cells in the workspace (grad_packed())."""
+        if reuse_setup and not self._setup_valid:
+            raise B.RadtError("-1 (RADT_E_INVALID): reuse_setup, but the workspace does not hold the setup of a forward of the "
+                              "current fields and options (set_fields / set_options / an adjoint with its own setup came after it)")
+        if not reuse_setup:
+            self._setup_valid = False          # the adjoint's own setup replaces the forward's
         g = self.dl_dcube if dl_dcube is None else dl_dcube
         outs = (self.g_dens, self.g_temp, self.g_vel) if unpack else (None, None, None)
         B.radt_render_bwd(self.desc, self.dens, self.temp, self.vel, self.cube, g, *outs, self.ws, stream,
@@ -83,6 +95,7 @@ class Renderer:
         """forward with the chi^2 data term fused into its epilogue: cube, dl_dcube and loss in one pass."""
         B.radt_render_loss(self.desc, self.dens, self.temp, self.vel, self.target, self.sigma, self.cube, self.dl_dcube,
                            self.loss, self.ws, stream, self.opt, self.cube_lo)
+        self._setup_valid = True
         return self.loss
 
     def fit_step(self, stream=None, fused=True):
@@ -95,6 +108,7 @@ class Renderer:
         self.render_bwd(stream=stream, reuse_setup=True)
 
     def set_fields(self, dens=None, temp=None, vel=None):
+        self._setup_valid = False
         for name, val in (("dens", dens), ("temp", temp), ("vel", vel)):
             if val is not None:
                 getattr(self, name).copy_(self.torch.as_tensor(np.ascontiguousarray(val, np.float32)).reshape(

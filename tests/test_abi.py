@@ -122,6 +122,45 @@ def test_forward_adjoint_option_mismatch_is_refused_on_the_host(lib):
     assert lib.radt_render_bwd(*args, C.byref(r), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -1       # other geometry
 
 
+def test_cube_memory_ignores_batch_and_can_be_forgotten(lib):
+    """What the library remembers about a cube pointer is what shapes its partial sums (window, skip_empty, kernel family,
+    cube_lo, channel count), not the batch or the image size: the adjoint of the first item of a batched forward (same
+    pointer, smaller batch) is accepted.  radt_forget drops the memory of a pointer whose buffer was refilled or recycled.
+    No GPU: fake pointers, calls that pass the host checks end in RADT_E_CUDA (-4)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present: fake device pointers would be dereferenced")
+    scs = make_config(5, npix=8, batch=3)
+    d3, d1 = B.Descriptors(scs), B.Descriptors(scs[:1])
+    for d in (d3, d1):
+        d.with_fields(0x10000, 0x20000, 0x30000)
+    cube, lo, dl, ws = (C.c_void_p(a) for a in (0x1100000, 0x1200000, 0x1300000, 0x1400000))
+    o = B.make_options()
+    a3 = (d3.geom, C.byref(d3.line), C.byref(d3.grid), 3)
+    a1 = (d1.geom, C.byref(d1.line), C.byref(d1.grid), 1)
+    assert lib.radt_render(*a3, C.byref(o), cube, lo, ws, 1 << 30, None) == -4
+    assert lib.radt_render_bwd(*a1, C.byref(o), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -4        # sub-batch: fine
+    bad = B.make_options(window=0)
+    assert lib.radt_render_bwd(*a1, C.byref(bad), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -1      # other options
+    assert b"radt_forget" in lib.radt_last_error()
+    assert lib.radt_forget(cube) == 0                                                                          # buffer recycled
+    assert lib.radt_render_bwd(*a1, C.byref(bad), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -4      # unknown origin: accepted
+    assert lib.radt_forget(C.c_void_p(0x7777000)) == 0 and lib.radt_forget(None) == -1
+    # a forgotten workspace no longer vouches for reuse_setup
+    r = B.make_options(reuse_setup=1)
+    assert lib.radt_render(*a3, C.byref(o), cube, lo, ws, 1 << 30, None) == -4
+    assert lib.radt_render_bwd(*a3, C.byref(r), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -4
+    assert lib.radt_forget(ws) == 0
+    assert lib.radt_render_bwd(*a3, C.byref(r), cube, lo, dl, None, None, None, ws, 1 << 30, None) == -1
+
+
+def test_host_split_hook_takes_sizes_not_environment_variables(lib):
+    assert lib.radt_debug_host_split(2, 16) == 0 and lib.radt_debug_host_split(0, 0) == 0
+    assert lib.radt_debug_host_split(-1, 0) == -1
+    src = open(os.path.join(ROOT, "paper_2509_03623_b200", "csrc", "radt_api.cu")).read()
+    assert "getenv" not in src                                    # the shipped library reads no environment variables
+
+
 def test_grad_layout(lib):
     d = B.Descriptors(make_config(1))
     off, n = B.radt_grad_layout(d)

@@ -426,9 +426,9 @@ def test_host_entry_points(rt):
 
 
 @pytest.mark.parametrize("chunk", [1, 2])
-def test_host_entry_points_in_item_chunks(rt, chunk, monkeypatch):
+def test_host_entry_points_in_item_chunks(rt, chunk):
     """Batched HOST calls run item chunk by item chunk (PCIe transfers under the marches, chi^2 term fused into each chunk's
-    forward); RADT_HOST_CHUNK_ITEMS forces that path on a small batch.  Same cube bit for bit, same loss and gradients as the
+    forward); radt_debug_host_split forces that path on a small batch.  Same cube bit for bit, same loss and gradients as the
     one-call path."""
     B = rt.binding
     scs = make_config(5, npix=16, batch=3)
@@ -446,10 +446,13 @@ def test_host_entry_points_in_item_chunks(rt, chunk, monkeypatch):
         loss = B.radt_fit_step_host(d, *h, tgt32, sigma, cube2, *g, rt.opt())
         return cube, lo, cube2, loss, g
 
-    monkeypatch.delenv("RADT_HOST_CHUNK_ITEMS", raising=False)
+    B.radt_debug_host_split(0, 0)
     c0, l0, c20, loss0, g0 = run()
-    monkeypatch.setenv("RADT_HOST_CHUNK_ITEMS", str(chunk))
-    c1, l1, c21, loss1, g1 = run()
+    try:
+        B.radt_debug_host_split(chunk_items=chunk)
+        c1, l1, c21, loss1, g1 = run()
+    finally:
+        B.radt_debug_host_split(0, 0)
     check_cube("chunked host cube", c1, ref)
     np.testing.assert_array_equal(c0, c1); np.testing.assert_array_equal(l0, l1); np.testing.assert_array_equal(c20, c21)
     np.testing.assert_array_equal(c1, c21)
@@ -462,9 +465,9 @@ def test_host_entry_points_in_item_chunks(rt, chunk, monkeypatch):
 
 
 @pytest.mark.parametrize("rows,npix", [(2, 32), (6, 32), (16, 32), (6, 31), (4, 9)])
-def test_host_entry_points_in_row_bands(rt, rows, npix, monkeypatch):
+def test_host_entry_points_in_row_bands(rt, rows, npix):
     """A single large image runs in row bands in the HOST calls (one setup, per band the fused-loss forward and the adjoint of its
-    rows, transfers under the marches); RADT_HOST_BAND_ROWS forces that path on a small image (32 rows: 16, 6 and 2 bands, the
+    rows, transfers under the marches); radt_debug_host_split forces that path on a small image (32 rows: 16, 6 and 2 bands, the
     last one partial for 6).  Same cube bit for bit, same loss and gradients as the one-launch path."""
     B = rt.binding
     sc = make_config(2, npix=32)
@@ -482,10 +485,13 @@ def test_host_entry_points_in_row_bands(rt, rows, npix, monkeypatch):
         loss = B.radt_fit_step_host(d, *h, tgt32, sigma, cube2, *g, rt.opt())
         return cube, lo, cube2, loss, g
 
-    monkeypatch.setenv("RADT_HOST_BAND_ROWS", "100000")          # one band: the plain path
-    c0, l0, c20, loss0, g0 = run()
-    monkeypatch.setenv("RADT_HOST_BAND_ROWS", str(rows))
-    c1, l1, c21, loss1, g1 = run()
+    try:
+        B.radt_debug_host_split(band_rows=100000)                # one band: the plain path
+        c0, l0, c20, loss0, g0 = run()
+        B.radt_debug_host_split(band_rows=rows)
+        c1, l1, c21, loss1, g1 = run()
+    finally:
+        B.radt_debug_host_split(0, 0)
     check_cube("banded host cube", c1, ref)
     np.testing.assert_array_equal(c0, c1); np.testing.assert_array_equal(l0, l1); np.testing.assert_array_equal(c20, c21)
     assert loss1 == pytest.approx(loss0, rel=1e-12)
@@ -494,6 +500,30 @@ def test_host_entry_points_in_row_bands(rt, rows, npix, monkeypatch):
     for nm, a, b, w in zip(("dens", "temp", "vel"), g0, g1, want):
         np.testing.assert_allclose(b, a, rtol=1e-4, atol=1e-6 * np.abs(a).max())
         check_grad(f"banded host g_{nm}", b[0], w)
+
+
+def test_reuse_setup_is_refused_after_the_fields_changed_in_place(rt):
+    """Renderer.set_fields copies into the same tensors: pointers and descriptors are unchanged, so the library's own check of
+    reuse_setup cannot see it.  The Renderer does: render(); set_fields(); render_bwd(reuse_setup=True) is refused instead of
+    marching with the forward's stale packed cells; after a new forward it is accepted and equals the adjoint with its own setup."""
+    B = rt.binding
+    sc = tiny_axisym_scene(seed=65)
+    R = rt.Renderer([sc])
+    R.dl_dcube.fill_(1e-6)
+    R.render()
+    R.render_bwd(reuse_setup=True)
+    R.set_fields(temp=R.temp.cpu().numpy() * 1.25)
+    with pytest.raises(B.RadtError, match="-1"):
+        R.render_bwd(reuse_setup=True)
+    R.render()
+    got = [g.clone() for g in R.render_bwd(reuse_setup=True)]
+    want = [g.clone() for g in R.render_bwd()]
+    for nm, a, b in zip(("dens", "temp", "vel"), got, want):
+        check_grad(f"reuse after set_fields g_{nm}", a.cpu().numpy(), b.cpu().numpy().astype(np.float64))
+    R.render()
+    R.set_options(zero_dens_grad=1)
+    with pytest.raises(B.RadtError, match="-1"):
+        R.render_bwd(reuse_setup=True)
 
 
 def test_l2_loss_kernel(rt):
