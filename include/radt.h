@@ -308,7 +308,15 @@ int radt_mlp_num_params(const radt_mlp *mlp, int64_t *count_out);
 int radt_mlp_temperature(const radt_mlp *mlp, const radt_grid *grid, const float *params, float *temp_out,
                          void *cuda_stream);
 /* g_params (DEVICE float32 [num_params], OVERWRITTEN) = (dT/dparams)^T g_temp; g_temp: DEVICE float32 [nr][nzeta].
- * Recomputes the activations (nothing is kept from the forward); float atomics make the last bits order dependent. */
+ * Recomputes the activations (nothing is kept from the forward); float atomics make the last bits order dependent.
+ * Accuracy: every contraction of the adjoint, the recomputation of the activations included, runs as split-bf16 products with
+ * fp32 accumulation, about 2^-16 relative per product, where the forward's three-product split is good to about fp32.  Away
+ * from the ReLU kinks the parameter gradient of a whole grid agrees with an fp64 evaluation to ~2.5e-5 of its largest entry.
+ * relu' is decided on the adjoint's own recomputed pre-activation: a unit within ~1e-4 (relative to the layer's scale) of
+ * its kink may take the other branch than the forward and an fp64 evaluation do.  Both branches are valid subgradients, but
+ * the result is then NOT within the 1e-3 gradient tolerance of an fp64 reference: measured 6e-3 of the largest entry (4e-3
+ * in L2) on a 256 x 128 grid with a random network of three times the initialisation scale, no node masked
+ * (tests/test_gpu_mlp_field.py).  A recomputation with a third bf16 term would remove this; it is not built. */
 int radt_mlp_temperature_bwd(const radt_mlp *mlp, const radt_grid *grid, const float *params, const float *g_temp,
                              float *g_params, void *cuda_stream);
 

@@ -6,6 +6,7 @@ import pytest
 
 from oracle import disk_physics as dp
 from synth import make_config
+from tests.tolerances import check_grad
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -69,6 +70,13 @@ def test_disk_fields_adjoint_matches_oracle(make):
         scale = np.abs(want).max()
         assert np.max(np.abs(got - want)) <= 1e-3 * scale               # BASELINE.json gradient tolerance
         assert np.linalg.norm(got - want) <= 1e-5 * np.linalg.norm(want) + 1e-7 * np.abs(g0[b]).max() * want.size ** 0.5
+    # element by element (tests/tolerances.py, as the render's gradients), on a call that adds to zeros so that the fp32
+    # rounding of `g0 + .` is not part of the comparison
+    gZ = torch.zeros_like(gT)
+    B.radt_disk_fields_bwd(B.make_disks(params), desc, temp, torch.from_numpy(gn).cuda(), torch.from_numpy(gv).cuda(), gZ, ws)
+    for b in range(len(scenes)):
+        fw = dp.forward(params[b], temp[b].cpu().numpy(), r, zeta)
+        check_grad(f"pre-pass dL/dT item {b}", gZ[b].cpu().numpy(), dp.adjoint(params[b], fw, gn[b], gv[b], r, zeta))
 
 
 def test_disk_fields_feed_the_render_end_to_end():

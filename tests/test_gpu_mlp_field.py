@@ -4,6 +4,7 @@ import pytest
 
 from oracle import mlp_field as mf
 from synth import make_config
+from tests.tolerances import check_grad
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -47,6 +48,7 @@ def test_mlp_adjoint_matches_oracle(cfg, L, seed):
     # BASELINE.json gradient tolerance (1e-3 of the maximum); measured far below
     assert np.max(np.abs(got - want)) <= 1e-3 * np.abs(want).max()
     assert np.linalg.norm(got - want) <= 1e-4 * np.linalg.norm(want)
+    check_grad("mlp g_params", got, want)      # and element by element, as the render's gradients (tests/tolerances.py)
 
 
 @pytest.mark.parametrize("nr,nz,L", [(9, 7, 4), (37, 11, 4), (50, 30, 8), (129, 2, 0)])
@@ -72,6 +74,33 @@ def test_mlp_ragged_node_counts(nr, nz, L):
     got = gp.cpu().numpy().astype(np.float64)
     assert np.max(np.abs(got - wantg)) <= 1e-3 * np.abs(wantg).max()
     assert np.linalg.norm(got - wantg) <= 1e-4 * np.linalg.norm(wantg)
+    check_grad(f"mlp g_params {nr}x{nz}", got, wantg)
+
+
+def test_mlp_adjoint_without_masking_the_relu_kinks():
+    """include/radt.h radt_mlp_temperature_bwd: the adjoint recomputes the activations with two-term bf16 products (about
+    2^-16 per product) while the forward uses the three-product split (about fp32), so relu' of a unit whose pre-activation
+    lies within ~1e-4 of zero may be taken on the other branch than the oracle's.  Either branch is a valid subgradient, but
+    the parameter gradient then leaves the 1e-3 tolerance: a KNOWN LIMIT, stated in the header with the figures measured
+    here (max 6.0e-3, L2 4.0e-3 on this harsh case: three times the initialisation scale, NO node masked; the other tests
+    zero g_T at near-kink nodes and meet 1e-3 / 1e-4 and the element-wise criterion).  The bound below keeps it from growing."""
+    from paper_2509_03623_b200 import binding as B
+    B.lib()
+    desc = B.Descriptors([make_config(2)])
+    nr, nz = desc.grid_shape
+    L = 4
+    mlp = B.make_mlp(L=L)
+    p = 3.0 * mf.init_params(L, 77)
+    assert mf.near_kink(p, nr, nz, L).any()
+    gT = np.random.default_rng(78).standard_normal((nr, nz)).astype(np.float32)
+    gp = torch.full((mf.n_params(L),), 7.0, dtype=torch.float32, device="cuda")
+    B.radt_mlp_temperature_bwd(mlp, desc, torch.from_numpy(p).cuda(), torch.from_numpy(gT).cuda(), gp)
+    want = mf.adjoint(p, gT, nr, nz, L)
+    got = gp.cpu().numpy().astype(np.float64)
+    err_max = np.max(np.abs(got - want)) / np.abs(want).max()
+    err_l2 = np.linalg.norm(got - want) / np.linalg.norm(want)
+    print(f"unmasked MLP adjoint: max {err_max:.3e}, L2 {err_l2:.3e}")
+    assert err_max <= 1e-2 and err_l2 <= 1e-2
 
 
 def test_neural_field_fit_reduces_the_loss():
