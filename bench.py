@@ -13,7 +13,10 @@ a 512 x 96 x 256 spherical grid) and rank 0 prints ONE JSON line of less than 3 
 512 steps, 2.75e11 nominal samples), the largest single-GPU configuration; `per_config_ms` has one short row per config and
 gpurun_out/bench_detail.json (named in `detail_file`) carries every measurement of every config, the pre-pass times and the
 work counters.
-With N > 1 every rank renders its own disks (independent problems, no data-path collective): weak scaling.
+With N > 1 every rank renders its own disks (independent problems, no data-path collective): weak scaling.  `--shard` instead
+splits ONE job (config 5's 16 disks) over the ranks through shard.ShardedRender: whole items per rank
+and one all-gather of the packed gradient cells per step (rows and an all-reduce when there are more ranks than items); strong
+scaling, `value` = the job's samples / max-over-ranks time.
 
 `value` = nominal samples (rays x channels x steps, summed over ranks and steps) / device time of the K steps (inputs resident
 in HBM; L2 flushed between steps outside the timed events).  `e2e` = the same step through the HOST-buffer C-ABI entry point
@@ -259,6 +262,97 @@ def measure_config_dry(cfg, args, ctx, with_cpu):
     res.update(config={"workload": _workload_name(cfg), "nominal_samples_per_step": nominal, "parallelism": f"independent disks x{world}"},
                value=whole_job_value(nominal, args.steps, ms_total, world), unit=UNIT, steps=args.steps,
                warmup=max(args.warmup, 3), ms_per_step=ms_total / args.steps, gpu_launches=0)
+    return res
+
+
+class _DryEngine:
+    """--dry-run --shard: stands in for shard.CudaEngine with zero tensors of the right shapes (no render, no oracle)."""
+
+    def __init__(self, scenes):
+        import torch
+        self.torch, self.n = torch, len(scenes)
+        self.cells = int(np.prod(scenes[0].grid.n))
+
+    def set_target(self, target, sigma):
+        pass
+
+    def fit_step_packed(self):
+        return self.torch.zeros((self.n, self.cells * 4)), self.torch.zeros(1, dtype=self.torch.float64)
+
+
+def measure_config_shard(cfg, args, ctx, with_cpu):
+    """--shard: ONE job (the config's whole batch) split over the ranks by shard.plan_units (batch items first, rows second;
+    SURVEY.md section 8(e)): per step every rank runs forward + fused chi^2 + adjoint of its units and the ranks exchange the
+    packed gradient cells with ONE collective (all-gather for whole items, all-reduce for split rows).  Strong scaling:
+    `value` = the job's nominal samples / max-over-ranks device time."""
+    from paper_2509_03623_b200.shard import ShardedRender
+    torch, dist = ctx["torch"], ctx["dist"]
+    world, rank, local = ctx["world"], ctx["rank"], ctx["local"]
+    dry = args.dry_run
+    if world > 1 or not dry:
+        assert dist.is_initialized(), "--shard needs a process group (torch.distributed.run sets it up)"
+    if dry:
+        from synth import make_config
+        scenes = make_config(cfg, npix=8) if cfg != 6 else _scenes(cfg)
+        scenes = scenes if isinstance(scenes, list) else [scenes]
+        nominal = {1: 3932160, 2: 1073741824, 3: 17179869184, 4: 8589934592, 5: 274877906944, 6: 1073741824}[cfg]
+        sh = ShardedRender(scenes, _DryEngine)
+    else:
+        from paper_2509_03623_b200.shard import CudaEngine
+        scenes = _scenes(cfg)
+        nominal = sum(s.nominal_samples for s in scenes)
+        sh = ShardedRender(scenes, lambda group: CudaEngine(group, f"cuda:{local}"))
+        slabs = sh.render()
+        gen = torch.Generator(device=f"cuda:{local}").manual_seed(36230 + cfg + 97 * rank)
+        peak = max([float(v.amax()) for v in slabs.values()] or [1.0])
+        sig = 0.015 * peak
+        sh.set_targets({u: v * (1.0 + 0.05 * torch.randn(v.shape, generator=gen, device=v.device))
+                        + sig * torch.randn(v.shape, generator=gen, device=v.device) for u, v in slabs.items()}, sig)
+        del slabs
+    warm = max(args.warmup, 3)
+    for _ in range(warm if not dry else 1):
+        sh.fit_step()
+    n0 = sh.n_collectives
+    if dry:
+        if world > 1:
+            dist.barrier()
+        for _ in range(args.steps):
+            sh.fit_step()
+        ms_local, clocks = args.steps * 1.0 * (1 + rank), None
+    else:
+        stream = torch.cuda.current_stream()
+        torch.cuda.synchronize()
+        dist.barrier()
+        sampler = ClockSampler(local)
+        sampler.start()
+        torch.cuda.synchronize()
+        events = []
+        for _ in range(args.steps):
+            ctx["flush_buf"].fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            sh.fit_step()
+            e1.record(stream)
+            events.append((e0, e1))
+        torch.cuda.synchronize()
+        dist.barrier()
+        clocks = sampler.stop()
+        ms_local = sum(a.elapsed_time(b) for a, b in events)
+    per_step = (sh.n_collectives - n0) / args.steps
+    ms_total = aggregate_ms(ms_local, ctx)
+    if world > 1:
+        dist.barrier()
+    if rank != 0:
+        return None
+    res = {k: None for k in ("fwd_value", "fwd_ms", "fwd_loss_fused_ms", "l2_ms", "bwd_ms", "bwd_ms_own_setup",
+                             "bwd_ms_zero_dens_grad_off", "step_ms_without_cube_lo", "executed_samples", "roofline",
+                             "roofline_other", "e2e", "e2e_render", "launches_per_step", "cpu_baseline", "loss", "wall_s")}
+    res.update(config={"workload": _workload_name(cfg), "nominal_samples_per_step": int(nominal),
+                       "parallelism": f"one job sharded over {world} rank(s): {len(sh.units)} unit(s) on rank 0, {sh.collective} of the packed gradient cells"},
+               value=nominal * args.steps / (ms_total * 1e-3), unit=UNIT, steps=args.steps, warmup=warm,
+               ms_per_step=ms_total / args.steps, clocks=clocks, scaling="strong",
+               gpu_launches=0 if dry else int(5 * len(sh.groups) * args.steps),
+               shard={"collective": sh.collective, "collectives_per_step": per_step, "units_per_rank": [len(us) for us in sh.plan]})
     return res
 
 
@@ -514,7 +608,7 @@ def headline_line(H, results, configs, world, args, dry=False):
     clocks = H.get("clocks")
     line = {
         "metric": METRIC, "value": H["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": H["warmup"],
-        "ms_per_step": H["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": H["ms_per_step"], "higher_is_better": True, "scaling": H.get("scaling", "weak"), "vs_baseline": None,
         "dtype": "f32", "data": "synthetic", "config": H["config"],
         "roofline": roof(H.get("roofline")), "roofline_other": roof(H.get("roofline_other")),
         "cpu_baseline": cpu, "e2e": e2e(H.get("e2e")), "e2e_render": e2e(H.get("e2e_render")),
@@ -523,6 +617,8 @@ def headline_line(H, results, configs, world, args, dry=False):
         "per_config_ms": {"columns": "step,fwd,bwd,frac_fwd,frac_bwd,e2e_step",
                           **{f"cfg{c}": summary(results[c]) for c in configs}},
     }
+    if H.get("shard"):
+        line["shard"] = H["shard"]
     if dry:
         line["dry_run"] = True
     line = _clean(line)
@@ -564,13 +660,20 @@ def run_ours(args, configs):
         ctx["reduce_device"] = "cpu"
         ctx["mufu_peak"] = ctx["ffma_peak"] = ctx["mufu_clk"] = None
         measure = measure_config_dry
+        if args.shard and world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29517")
+            dist.init_process_group("gloo", rank=0, world_size=1)
     else:
         from paper_2509_03623_b200 import Renderer, binding as B
         torch.cuda.set_device(local)
-        if world > 1:
-            # NCCL_DEBUG=INFO (if the launcher sets it) shows the ranks and NVLS; the only collectives of this bench are the
-            # barriers around the timed region and the max-over-ranks of its duration
-            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if world > 1 or args.shard:
+            # NCCL_DEBUG=INFO (if the launcher sets it) shows the ranks and NVLS; without --shard the only collectives of this
+            # bench are the barriers around the timed region and the max-over-ranks of its duration
+            if world == 1:
+                os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+                os.environ.setdefault("MASTER_PORT", "29517")
+            dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
         B.lib()
         ctx.update(B=B, Renderer=Renderer, reduce_device=f"cuda:{local}",
                    flush_buf=torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local}"))     # > 126 MB L2
@@ -578,6 +681,8 @@ def run_ours(args, configs):
         ctx["mufu_peak"], ctx["mufu_clk"] = B.radt_pipe_peak(0)
         ctx["ffma_peak"], _ = B.radt_pipe_peak(1)
         measure = measure_config
+    if args.shard:
+        measure = measure_config_shard
 
     head = configs[0] if len(configs) == 1 else (HEADLINE if HEADLINE in configs else configs[-1])
     results = {}
@@ -591,17 +696,17 @@ def run_ours(args, configs):
         if not dry:
             torch.cuda.empty_cache()
     if rank != 0:
-        if world > 1:
+        if dist.is_initialized():
             dist.destroy_process_group()
         return
-    prepass = prepass_times(ctx, args) if (world == 1 and not args.no_prepass and not dry) else None
+    prepass = prepass_times(ctx, args) if (world == 1 and not args.no_prepass and not dry and not args.shard) else None
 
     H = results[head]
     keep = ("config", "value", "ms_per_step", "steps", "fwd_value", "fwd_ms", "fwd_loss_fused_ms", "l2_ms", "bwd_ms",
             "bwd_ms_own_setup", "bwd_ms_zero_dens_grad_off", "step_ms_without_cube_lo", "executed_samples", "roofline",
             "roofline_other", "e2e", "e2e_render", "launches_per_step", "clocks", "bench_wall_s")
     detail = {
-        "per_config": [{k: results[c][k] for k in keep} for c in configs], "prepass": prepass,
+        "per_config": [{k: results[c].get(k) for k in keep} for c in configs], "prepass": prepass,
         "pipe_peaks": {"mufu_lane_ops_per_s": ctx["mufu_peak"], "ffma_lane_ops_per_s": ctx["ffma_peak"], "sm_mhz": ctx["mufu_clk"]},
         "executed_samples": H["executed_samples"], "loss": H["loss"], "wall_s": H["wall_s"],
         "kernels": "window (uniform channel lattice)" if args.win_path else "channel table",
@@ -614,7 +719,7 @@ def run_ours(args, configs):
     if not dry:
         line["detail_file"] = write_detail(detail, args)
     print(json.dumps(line, allow_nan=False, separators=(",", ":")), flush=True)
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 
@@ -629,6 +734,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-prepass", action="store_true")
+    ap.add_argument("--shard", action="store_true", help="ONE job (the headline config's 16 disks) split over the ranks through "
+                    "shard.ShardedRender: items first, rows second, one collective per step over the packed gradient cells; strong scaling "
+                    "(default without it: every rank renders its own disks, weak scaling)")
     ap.add_argument("--dry-run", action="store_true", help="no GPU work: exercise the multi-rank timing / aggregation logic on CPU (gloo)")
     ap.add_argument("--win-path", type=int, default=1, choices=[0, 1],
                     help="radt_options.win_path: 1 = window kernels on uniform channel lattices (default), 0 = channel-table kernels")
@@ -641,7 +749,7 @@ def main():
     elif args.configs:
         configs = [int(c) for c in args.configs.split(",")]
     else:
-        configs = list(ALL_CONFIGS)
+        configs = [HEADLINE] if args.shard else list(ALL_CONFIGS)
     if args.impl == "reference":
         run_reference(args, configs)
     else:

@@ -3,9 +3,13 @@
 
 A slab of image rows [r0, r1) of one item is itself a valid image description, so sharding needs no kernel support:
     ny' = r1 - r0,   fov_y' = fov_y * ny' / ny,   y0' = y0 + ((r0 + r1)/2 - ny/2) * fov_y / ny
-The forward needs no collective (each rank owns its cube rows).  The adjoint leaves each rank with partial gradients of
-the (replicated) grids; they are summed by ONE all-reduce over the packed float4 gradient cells [batch][cells][4] -- the
-buffer the adjoint march accumulates into, before it is unpacked into the three planes -- on the adjoint's stream.
+The forward needs no collective (each rank owns its cube rows).  The adjoint ends with ONE collective over the packed float4
+gradient cells [item][cells][4] -- the buffer the adjoint march accumulates into, before it is unpacked into the three planes:
+  - whole items per rank (world <= batch): every item's gradient is complete on the rank that owns it, so the ranks only
+    exchange what they own: an ALL-GATHER of the owned items' cells (an all-reduce would move and add a [batch, cells * 4]
+    buffer that is zero for every item a rank does not own: 268 MB per rank on config 4's shape);
+  - rows of an item split over ranks (world > batch): the ranks hold partial sums of the same cells: an ALL-REDUCE.
+`ShardedRender.collective` names which one a plan uses; `n_collectives` counts the calls.
 
 The `engine` does the rendering: on GPUs it is `CudaEngine` (the C-ABI path; the all-reduce then runs over NCCL); tests inject
 a CPU engine and the gloo backend to cover this plumbing without a GPU.
@@ -76,6 +80,16 @@ class CudaEngine:
         """k_unpack_grad on the workspace's own cells (after they were all-reduced in place)."""
         return self.R.unpack_grad()
 
+    def set_target(self, target, sigma):
+        self.R.set_target(target, sigma)
+
+    def fit_step_packed(self):
+        """Forward with the fused chi^2 term + adjoint (setup reused), gradient left packed: (cells [n, cells * 4], loss [1])."""
+        R = self.R
+        R.render_loss()
+        R.render_bwd(unpack=False, reuse_setup=True)
+        return R.grad_packed().view(R.desc.batch, -1), R.loss
+
 
 class ShardedRender:
     """One render call (a batch of scenes that share line, grid layout and image size) split over the ranks of a
@@ -96,6 +110,9 @@ class ShardedRender:
             self.cells *= int(n)
         self.plan = plan_units(self.batch, self.ny, self.world)
         self.units = self.plan[self.rank]
+        # which collective ends the adjoint (module docstring): whole items per rank -> all-gather, split rows -> all-reduce
+        self.collective = "all_gather" if (self.world <= self.batch and self.world > 1) else "all_reduce"
+        self.n_collectives = 0
         # one engine per slab height (all units of a rank have the same height unless rows do not divide evenly)
         self.groups = {}
         for u in self.units:
@@ -134,29 +151,74 @@ class ShardedRender:
                 row += r1 - r0
         return cube
 
-    # ---- adjoint: ONE all-reduce over the packed gradient cells
+    # ---- adjoint: ONE collective over the packed gradient cells
     def render_bwd(self, dl_slabs):
         """dl_slabs: {(item, r0, r1): dL/dcube of that slab}.  Returns (g_dens, g_temp, g_vel), each [batch, *grid], the
         same on every rank (the grids are replicated)."""
         import torch
-        acc, inplace = None, None
-        full = [(b, 0, self.ny) for b in range(self.batch)]
+        packed = {}
         for h, us in self.groups.items():
             dl = torch.stack([dl_slabs[u] for u in us])
-            packed = self.engines[h].render_bwd_packed(dl)            # [n, cells * 4]
-            if acc is None and len(self.groups) == 1 and [u[0] for u in us] == list(range(self.batch)):
-                acc, inplace = packed, self.engines[h]               # this rank's cells already span the whole batch
-                continue
-            if acc is None:
-                acc = torch.zeros((self.batch, self.cells * 4), dtype=torch.float32, device=packed.device)
-            for k, (b, _, _) in enumerate(us):
-                acc[b] += packed[k]
-        if acc is None:                                              # a rank without work still joins the collective
-            dev = "cuda" if self.dist.get_backend(self.group) == "nccl" else "cpu"
-            acc = torch.zeros((self.batch, self.cells * 4), dtype=torch.float32, device=dev)
-        del full
-        self.dist.all_reduce(acc, op=self.dist.ReduceOp.SUM, group=self.group)      # the ONE collective of the adjoint
-        if inplace is not None and hasattr(inplace, "unpack"):
-            return inplace.unpack()
+            packed[h] = self.engines[h].render_bwd_packed(dl)        # [n, cells * 4]
+        return self._combine(packed)
+
+    # ---- fit step: forward + chi^2 + adjoint per rank, then the same ONE collective
+    def set_targets(self, target_slabs, sigma):
+        """target_slabs: {(item, r0, r1): data cube rows of that slab}.  The chi^2 term is normalised by the voxel count of the
+        WHOLE job, L = sum (I - D)^2 / (2 sigma^2 n_job): an engine normalises by the voxels of its own call, so it is given
+        sigma sqrt(n_job / n_call), which yields exactly dL/dcube = (I - D) / (sigma^2 n_job) and this rank's share of L."""
+        import torch
+        n_job = self.batch * self.ny * self.nx * self.nchan
+        for h, us in self.groups.items():
+            n_call = len(us) * h * self.nx * self.nchan
+            self.engines[h].set_target(torch.stack([target_slabs[u] for u in us]), float(sigma) * (n_job / n_call) ** 0.5)
+
+    def fit_step(self):
+        """One pass of the hot path over this rank's units and the collective.  Returns ((g_dens, g_temp, g_vel), loss_share):
+        the gradients of the whole batch on every rank; loss_share is THIS rank's part of L (a tensor; summing it over ranks is
+        left to the caller so that the step keeps its single collective)."""
+        packed, loss = {}, None
+        for h in self.groups:
+            packed[h], l = self.engines[h].fit_step_packed()
+            loss = l.clone() if loss is None else loss + l
+        return self._combine(packed), loss
+
+    def _combine(self, packed):
+        """packed: {slab height: [n, cells * 4] of that engine's units} -> gradients of the whole batch on every rank."""
+        import torch
+        width = self.cells * 4
+        if self.collective == "all_gather":
+            # whole items per rank, contiguous and balanced (plan_units): rank k owns items plan[k][0][0] .. + len(plan[k])
+            counts = [len(us) for us in self.plan]
+            nmax = max(counts)
+            (h, mine), = packed.items()                              # world <= batch: one group (full-height items) per rank
+            if counts[self.rank] < nmax:
+                pad = torch.zeros((nmax, width), dtype=torch.float32, device=mine.device)
+                pad[:counts[self.rank]] = mine
+                mine = pad
+            out = torch.empty((self.world, nmax, width), dtype=torch.float32, device=mine.device)
+            self.dist.all_gather([out[k] for k in range(self.world)], mine.contiguous(), group=self.group)      # the ONE collective
+            self.n_collectives += 1
+            if min(counts) == nmax:
+                acc = out.view(self.batch, width)
+            else:
+                acc = torch.cat([out[k, :counts[k]] for k in range(self.world)])
+        else:
+            acc, inplace = None, None
+            for h, us in self.groups.items():
+                if acc is None and len(self.groups) == 1 and [u[0] for u in us] == list(range(self.batch)):
+                    acc, inplace = packed[h], self.engines[h]        # this rank's cells already span the whole batch
+                    continue
+                if acc is None:
+                    acc = torch.zeros((self.batch, width), dtype=torch.float32, device=packed[h].device)
+                for k, (b, _, _) in enumerate(us):
+                    acc[b] += packed[h][k]
+            if acc is None:                                          # a rank without work still joins the collective
+                dev = "cuda" if self.dist.get_backend(self.group) == "nccl" else "cpu"
+                acc = torch.zeros((self.batch, width), dtype=torch.float32, device=dev)
+            self.dist.all_reduce(acc, op=self.dist.ReduceOp.SUM, group=self.group)          # the ONE collective
+            self.n_collectives += 1
+            if inplace is not None and hasattr(inplace, "unpack"):
+                return inplace.unpack()
         cells = acc.view(self.batch, self.cells, 4)
         return tuple(cells[:, :, k].reshape((self.batch,) + self.grid_shape).contiguous() for k in range(3))

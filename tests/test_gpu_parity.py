@@ -933,5 +933,17 @@ def test_sharded_render_cuda_engine_nccl_world1():
             got = sh.render_bwd({u: G[u[0], u[1]:u[2]] for u in sh.units})
             for a, b in zip(got, want):
                 check_grad("sharded adjoint", a.cpu().numpy(), b.cpu().numpy().astype(np.float64))
+            # the sharded fit step (fused chi^2 + adjoint with the forward's setup, then the one collective) = Renderer.fit_step
+            D = R.cube * (1.0 + 0.1 * torch.randn_like(R.cube))
+            R.set_target(D, 0.02 * float(R.cube.max()))
+            R.fit_step()
+            want = [g.clone() for g in (R.g_dens, R.g_temp, R.g_vel)]
+            sh.set_targets({u: D[u[0], u[1]:u[2]] for u in sh.units}, 0.02 * float(R.cube.max()))
+            n0 = sh.n_collectives
+            got, share = sh.fit_step()
+            assert sh.n_collectives == n0 + 1
+            assert float(share) == pytest.approx(float(R.loss), rel=1e-6)
+            for a, b in zip(got, want):
+                check_grad("sharded fit step", a.cpu().numpy(), b.cpu().numpy().astype(np.float64))
     finally:
         dist.destroy_process_group()
