@@ -801,23 +801,39 @@ def test_random_scenes_with_special_viewing_angles(rt, seed):
     """The random scenes again with inclination, PA and azimuth drawn from {0, 30, 45, 60, 90, 180, 270} degrees: round-number
     geometries put samples EXACTLY on a grid boundary (an edge-on view with a ray at z / r = zeta_lo, a chord that ends on
     r_max), where the in/out decision is a tie between the roundings of two correct fp64 evaluations (reading (a)).
-    Every voxel must agree except on rays that a plain numpy evaluation shows to have such a sample."""
+    Every voxel must agree except on rays that a plain numpy evaluation shows to have such a sample, and the gradients of a
+    loss that does not look at those rays must agree everywhere."""
     rng = np.random.default_rng(77000 + seed)
     sc = _random_scene(seed)
     g = replace(sc.geom, incl=float(np.radians(rng.choice([0.0, 90.0, 45.0, 30.0, 60.0]))),
                 pa=float(np.radians(rng.choice([0.0, 90.0, 180.0, -90.0]))), az=float(np.radians(rng.choice([0.0, 90.0, 180.0, 270.0]))))
     sc = replace(sc, geom=g)
     ref = _oracle_cube([sc])
-    R = _gpu_forward(rt, sc)
+    R = _gpu_forward(rt, sc, need_bwd=True)
     got = R.cube.cpu().numpy()
     bad = np.abs(got - ref) > 1e-4 * np.abs(ref) + 1e-6 * max(ref.max(), 1e-300)
-    if not bad.any():
-        return
-    assert sc.grid.kind != 1, "Cartesian grids compare the coordinates themselves: no ties"
-    ties = _rays_with_a_sample_on_a_boundary(sc)
-    bad_rays = {(int(iy), int(ix)) for _, iy, ix, _ in np.argwhere(bad)}
-    assert bad_rays <= ties, f"rays {sorted(bad_rays - ties)} differ without a sample on a boundary"
-    assert len(bad_rays) <= max(2, (g.nx * g.ny) // 2)          # (a 6 x 2 image can have its four symmetric rays on ties)
+    ties = set()
+    if bad.any():
+        assert sc.grid.kind != 1, "Cartesian grids compare the coordinates themselves: no ties"
+        ties = _rays_with_a_sample_on_a_boundary(sc)
+        bad_rays = {(int(iy), int(ix)) for _, iy, ix, _ in np.argwhere(bad)}
+        assert bad_rays <= ties, f"rays {sorted(bad_rays - ties)} differ without a sample on a boundary"
+        assert len(bad_rays) <= max(2, (g.nx * g.ny) // 2)          # (a 6 x 2 image can have its four symmetric rays on ties)
+    # The adjoint on the same scene: the gradients may differ from the oracle's only THROUGH the tie rays, so with dL/dcube
+    # zeroed on those rays (on both sides) every gradient must meet the usual criteria.
+    if ref[0].max() > 0:
+        tgt, sigma = l2_target(ref[0], 3000 + seed)
+        G = (ref[0] - tgt) / (sigma ** 2 * ref[0].size)
+    else:
+        G = 1e-6 * rng.standard_normal(ref[0].shape)
+    for iy, ix in ties:
+        G[iy, ix, :] = 0.0
+    G32 = G.astype(np.float32)
+    R.dl_dcube.copy_(torch.from_numpy(G32[None]))
+    gd, gt, gv = (x.cpu().numpy() for x in R.render_bwd())
+    rd, rtm, rv = po.render_bwd(sc, G32.astype(np.float64))
+    for nm, a, w in (("dens", gd[0], rd), ("temp", gt[0], rtm), ("vel", gv[0], rv)):
+        check_grad(f"special angles {seed} g_{nm}", a, w)
 
 
 @pytest.mark.parametrize("seed", range(int(os.environ.get("RADT_RANDOM_OFFCENTRE", "8"))))
