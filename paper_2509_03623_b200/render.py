@@ -45,6 +45,16 @@ class Renderer:
         # so the pointers stay the same when the values change: that part of the reuse_setup contract is checked here.
         self._setup_valid = False
 
+    def __del__(self):
+        # The library remembers cubes and workspaces by raw device pointer and knows nothing of torch's allocator, which may hand
+        # these addresses to the next tensor: drop that memory with the buffers (include/radt.h radt_forget).
+        try:
+            for t in (getattr(self, "cube", None), getattr(self, "ws", None)):
+                if t is not None:
+                    B.radt_forget(t)
+        except Exception:      # noqa: BLE001  (interpreter shutdown: the binding may already be gone)
+            pass
+
     def set_options(self, **kw):
         """Change this object's radt_options for the calls that follow (a forward and its adjoint must share them)."""
         self.options.update(kw)

@@ -526,6 +526,29 @@ def test_reuse_setup_is_refused_after_the_fields_changed_in_place(rt):
         R.render_bwd(reuse_setup=True)
 
 
+def test_a_deleted_renderer_leaves_no_memory_of_its_buffers(rt):
+    """The library keys what it remembers by raw device pointer; torch's caching allocator reuses addresses.  A Renderer forgets
+    its cube and workspace when it is deleted, so a new cube that lands on the old address (here: the very same storage, kept
+    alive by a second reference) is a cube of unknown origin: an adjoint with other options is accepted, not refused on the
+    strength of the dead Renderer's forward."""
+    B = rt.binding
+    sc = tiny_axisym_scene(seed=66)
+    R = rt.Renderer([sc], compensated=False)
+    R.render()
+    cube, ws, dl = R.cube, R.ws, torch.full_like(R.cube, 1e-6)
+    desc, fields = R.desc, (R.dens, R.temp, R.vel)
+    outs = [torch.empty_like(f) for f in fields]
+    other = rt.opt(window=0)
+    with pytest.raises(B.RadtError, match="-1"):                 # while R lives, the mismatch is refused
+        B.radt_render_bwd(desc, *fields, cube, dl, *outs, ws, opt=other)
+    del R
+    import gc
+    gc.collect()
+    B.radt_render_bwd(desc, *fields, cube, dl, *outs, ws, opt=other)      # same address, no memory of the forward: accepted
+    torch.cuda.synchronize()
+    assert all(torch.isfinite(o).all() for o in outs)
+
+
 def test_l2_loss_kernel(rt):
     R = rt.Renderer([make_config(1)])
     R.render()
